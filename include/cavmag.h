@@ -1,0 +1,175 @@
+/* =====================================================================================
+ * cavmag.h — C ABI of the B200-native (sm_100a) cavity-magnonics hot path.
+ *
+ * What it computes (arXiv 2603.03706, tier 1; citations are /root/reference/PAPER.md lines):
+ * the Landau-Lifshitz-Gilbert equation on a finite-difference grid, integrated TOGETHER
+ * with N cavity-mode ODEs in one adaptive Dormand-Prince RK5(4) step, entirely on the
+ * device with no per-step host synchronisation.
+ *
+ *   S_n      = (1/W_n) sum_r u_n(r) (m_c,x - i m_c,y)(r)          PAPER.md:156 Eq. 18, :45 Eq. 2
+ *   da_n/dt  = -(i w_n + kappa_n) a_n + i G_n S_n,  G_n = g_n + Gamma_n e^{i Phi_n}
+ *                                                                PAPER.md:119 Eq. 12, :317 Eq. 19
+ *   B_rf(r)  = x^ (2/gamma) sum_n u_n(r) Re[G_n a_n]              PAPER.md:54 Eq. 3, :65 Eq. 5, :121 Eq. 13, :159
+ *   B_s(r)   = B0 + (2A/Ms) sum_{6 nb in grid} (m_nb - m)/D^2 + (2Ku/Ms)(m.k^)k^ + B_rf
+ *              - B_exch_inter m_other(r)   [two-sublattice antiferromagnet, PAPER.md:132-144]
+ *   dm_s/dt  = -gamma/(1+alpha^2) [ m x B + alpha m x (m x B) ]
+ *   m_c      = m_1  or (m_1 + m_2)/2
+ *
+ * The readings of everything the paper leaves open (signs, normalisation, tableau, step
+ * controller, boundary condition) are listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - SI units: metres, tesla, A/m, J/m, J/m^3; every rate in rad/s.
+ *   - Cell fields are SoA, component-major, x fastest:
+ *       m : [n_sub][3][nz][ny][nx]      u : [N][nz][ny][nx]
+ *     in the precision chosen at cav_create (CAV_F32 -> float, CAV_F64 -> double).
+ *   - Mode amplitudes are always double: a : [N][2] = (Re, Im).
+ *   - "host or device" pointers carry an explicit is_device flag. Device pointers must be
+ *     on the current CUDA device and are read/written on the simulation's stream.
+ *   - Ownership: every input array is copied during the call; outputs are written into
+ *     caller memory. The library owns all of its device buffers (freed by cav_destroy).
+ *   - cav_run* only enqueue work on the stream (asynchronous). cav_get_*, cav_sync and
+ *     cav_destroy synchronise the stream. Errors raised on the device (non-finite error
+ *     norm, step-size underflow) surface as the return value of the next synchronising call.
+ *   - Every function returns CAV_OK (0) or a negative cav_status. No exceptions cross the
+ *     boundary. A handle is not thread-safe; distinct handles are independent.
+ * ===================================================================================== */
+#ifndef CAVMAG_H_
+#define CAVMAG_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cav_sim cav_sim; /* opaque */
+
+typedef enum {
+    CAV_OK = 0,
+    CAV_E_ARG = -1,           /* invalid argument (NULL, non-positive size, N > CAV_MAX_MODES ...) */
+    CAV_E_STATE = -2,         /* call order: e.g. cav_run before cav_set_m */
+    CAV_E_CUDA = -3,          /* a CUDA runtime call failed; see cav_last_cuda_error */
+    CAV_E_NOMEM = -4,         /* device or host allocation failed */
+    CAV_E_NONFINITE = -5,     /* error norm became NaN/Inf in fixed-step mode */
+    CAV_E_DT_UNDERFLOW = -6,  /* adaptive step proposal fell below 1e-20 s */
+    CAV_E_SINGULAR_NORM = -7, /* CAV_NORM_SUM_U with |sum_r u_n| < 1e-6 N_cells */
+    CAV_E_UNSUPPORTED = -8    /* no CUDA device / device is not sm_100 */
+} cav_status;
+
+enum { CAV_F32 = 0, CAV_F64 = 1 };
+enum { CAV_NORM_NCELLS = 0, CAV_NORM_SUM_U = 1 };
+enum { CAV_LAUNCH_GRAPH = 0, CAV_LAUNCH_STREAM = 1 };
+#define CAV_MAX_MODES 32
+
+/* Finite-difference grid: nx*ny*nz cells of size dx*dy*dz (metres). */
+typedef struct {
+    int nx, ny, nz;
+    double dx, dy, dz;
+} cav_grid;
+
+/* Material and model parameters ("the paper's statement of the problem"). */
+typedef struct {
+    double Ms;           /* saturation magnetisation, A/m */
+    double Aex;          /* exchange stiffness, J/m (6-neighbour stencil, open boundaries) */
+    double Ku;           /* uniaxial anisotropy, J/m^3 */
+    double ku_axis[3];   /* anisotropy axis (normalised internally; ignored if Ku == 0) */
+    double alpha;        /* Gilbert damping */
+    double gamma;        /* gyromagnetic ratio, rad/(s T); PAPER.md:56 uses 1.76e11 */
+    double B0[3];        /* static field, tesla */
+    int n_sub;           /* 1 ferromagnet, 2 two-sublattice antiferromagnet */
+    double B_exch_inter; /* tesla; n_sub == 2: B_s += -B_exch_inter * m_other(r) */
+    int precision;       /* CAV_F32 | CAV_F64 for the cell fields */
+    int renormalize;     /* 1: m_new = y5/|y5| per cell before the 7th evaluation (default 1) */
+    int overlap_norm;    /* CAV_NORM_NCELLS (Eq. 18, default) | CAV_NORM_SUM_U */
+} cav_params;
+
+typedef struct {
+    long long accepted;  /* accepted RK45 steps since creation */
+    long long rejected;  /* rejected RK45 steps */
+    long long rhs_evals; /* evaluations of the coupled right-hand side (= stage-kernel launches) */
+    double dt_min;       /* smallest / largest accepted step */
+    double dt_max;
+    double dt_next;      /* current step proposal */
+    double t;            /* simulated time, s */
+    double last_err;     /* error norm of the last attempted step */
+} cav_stats;
+
+/* Create a simulation on the current CUDA device. Allocates all device buffers
+ * (11 cell fields of n_sub*3*nx*ny*nz elements, reduction scratch, controller state). */
+int cav_create(const cav_grid* grid, const cav_params* params, cav_sim** out);
+int cav_destroy(cav_sim* sim);
+
+/* Use an existing CUDA stream (a cudaStream_t, e.g. torch's current stream) for all work.
+ * Default: a stream the library creates. Synchronises the old stream first. */
+int cav_set_stream(cav_sim* sim, void* cuda_stream);
+
+/* CAV_LAUNCH_GRAPH (default): cav_run is one CUDA-graph launch whose body is a conditional
+ * WHILE node looping on the device.  CAV_LAUNCH_STREAM: the host enqueues the stage kernels
+ * in chunks and polls the device 'done' flag once per chunk (debug / profiling aid). */
+int cav_set_launch_mode(cav_sim* sim, int mode);
+
+/* Cavity modes (PAPER.md:119 Eq. 12, :154 profiles, :317 Eq. 19).
+ *   u      [N][nz][ny][nx] in the simulation's precision, host or device
+ *   omega, kappa, g, Gamma, Phi : host arrays [N] (rad/s, rad); Gamma and Phi may be NULL (= 0)
+ * N may be 0 (plain LLG; u ignored). Replaces any previous mode set and zeroes a. */
+int cav_set_modes(cav_sim* sim, int N, const void* u, int u_is_device, const double* omega,
+                  const double* kappa, const double* g, const double* Gamma, const double* Phi);
+
+/* Magnetisation [n_sub][3][nz][ny][nx] in the simulation's precision. Normalised per cell on entry. */
+int cav_set_m(cav_sim* sim, const void* m, int is_device);
+int cav_get_m(cav_sim* sim, void* m_out, int is_device);
+
+/* Mode amplitudes, host arrays [N][2] doubles. */
+int cav_set_a(cav_sim* sim, const double* a_re_im);
+int cav_get_a(cav_sim* sim, double* a_out);
+
+/* Slopes of the current state: dm/dt [n_sub][3][nz][ny][nx] (simulation precision, host or device)
+ * and da/dt [N][2] (host). Evaluates the coupled right-hand side once if it is not cached. */
+int cav_get_dmdt(cav_sim* sim, void* out, int is_device);
+int cav_get_dadt(cav_sim* sim, double* out);
+
+/* Overlaps S_n of the current state (from the last evaluation of the right-hand side), [N][2]. */
+int cav_get_overlaps(cav_sim* sim, double* S_out);
+
+/* Advance to t_end.  Exactly one of tol > 0 (adaptive DP5(4), absolute max-norm tolerance)
+ * or fixed_dt > 0 (fixed step).  dt_init <= 0: keep the current proposal (1e-14 s initially). */
+int cav_run(cav_sim* sim, double t_end, double tol, double fixed_dt, double dt_init);
+
+/* As cav_run, but stop after max_steps attempted steps (accepted + rejected) if max_steps > 0.
+ * t_end may be +inf when max_steps > 0. */
+int cav_run_steps(cav_sim* sim, double t_end, double tol, double fixed_dt, double dt_init,
+                  long long max_steps);
+
+/* Wait for all enqueued work; returns the device status (CAV_OK, CAV_E_NONFINITE, ...). */
+int cav_sync(cav_sim* sim);
+
+int cav_get_time(cav_sim* sim, double* t, double* dt_next);
+int cav_set_time(cav_sim* sim, double t);
+int cav_get_stats(cav_sim* sim, cav_stats* out);
+
+/* Device-side trace: one row per sample,
+ *   [t, a(re,im) x N, S(re,im) x N, <m_s>(x,y,z) x n_sub]     (1 + 4N + 3 n_sub doubles)
+ * adaptive runs clamp steps onto t_set + k*sample_dt; fixed-step runs sample every
+ * round(sample_dt/fixed_dt) accepted steps.  capacity rows are kept on the device; sampling
+ * stops when full.  sample_dt <= 0 disables.  Resets the trace. */
+int cav_set_trace(cav_sim* sim, double sample_dt, int capacity);
+int cav_trace_row_len(cav_sim* sim, int* row_len);
+int cav_get_trace(cav_sim* sim, double* out /* [capacity][row_len] host */, int* n_samples);
+
+/* Tuning knob (optional): cells per thread block of the stage kernel; 0 = automatic. */
+int cav_set_block_cells(cav_sim* sim, int cells_per_block);
+
+/* Tuning knob (optional): 1 (default) = odd stages sweep the grid in reverse block order so that
+ * the tail of one stage's data is still in L2 when the next stage starts; 0 = always forward. */
+int cav_set_sweep_order(cav_sim* sim, int serpentine);
+
+/* Number of kernels this library has launched for this handle (stage kernels + setup). */
+int cav_get_launch_count(cav_sim* sim, long long* n);
+
+const char* cav_strerror(int status);
+const char* cav_last_cuda_error(cav_sim* sim);
+const char* cav_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAVMAG_H_ */

@@ -1,0 +1,327 @@
+"""Thin Python binding of include/cavmag.h (argument marshalling only).
+
+Same names as the C ABI: ``cav_create``, ``cav_set_modes``, ``cav_set_m``, ``cav_run`` ...
+Every step of the hot path runs inside ``libcavmag.so``'s CUDA kernels; this module holds no
+arithmetic and has NO CPU fallback: if the library is missing or cannot be loaded, importing
+this module raises.  PyTorch is used by callers only for device memory and streams — torch
+tensors are passed as raw ``data_ptr()`` addresses.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcavmag.so")
+
+CAV_OK = 0
+CAV_E_ARG, CAV_E_STATE, CAV_E_CUDA, CAV_E_NOMEM = -1, -2, -3, -4
+CAV_E_NONFINITE, CAV_E_DT_UNDERFLOW, CAV_E_SINGULAR_NORM, CAV_E_UNSUPPORTED = -5, -6, -7, -8
+CAV_F32, CAV_F64 = 0, 1
+CAV_NORM_NCELLS, CAV_NORM_SUM_U = 0, 1
+CAV_LAUNCH_GRAPH, CAV_LAUNCH_STREAM = 0, 1
+CAV_MAX_MODES = 32
+
+
+class cav_grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double)]
+
+
+class cav_params(C.Structure):
+    _fields_ = [("Ms", C.c_double), ("Aex", C.c_double), ("Ku", C.c_double), ("ku_axis", C.c_double * 3),
+                ("alpha", C.c_double), ("gamma", C.c_double), ("B0", C.c_double * 3), ("n_sub", C.c_int),
+                ("B_exch_inter", C.c_double), ("precision", C.c_int), ("renormalize", C.c_int),
+                ("overlap_norm", C.c_int)]
+
+
+class cav_stats(C.Structure):
+    _fields_ = [("accepted", C.c_longlong), ("rejected", C.c_longlong), ("rhs_evals", C.c_longlong),
+                ("dt_min", C.c_double), ("dt_max", C.c_double), ("dt_next", C.c_double), ("t", C.c_double),
+                ("last_err", C.c_double)]
+
+
+class CavError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{where}: {cav_strerror(status)} ({status}) {detail}".strip())
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2603_03706_b200.build` "
+                      "(there is no CPU fallback)")
+_lib = C.CDLL(LIB_PATH)
+
+_vp, _dp, _i, _d, _ll = C.c_void_p, C.POINTER(C.c_double), C.c_int, C.c_double, C.c_longlong
+_SIGS = {
+    "cav_create": ([C.POINTER(cav_grid), C.POINTER(cav_params), C.POINTER(_vp)], _i),
+    "cav_destroy": ([_vp], _i),
+    "cav_set_stream": ([_vp, _vp], _i),
+    "cav_set_launch_mode": ([_vp, _i], _i),
+    "cav_set_modes": ([_vp, _i, _vp, _i, _dp, _dp, _dp, _dp, _dp], _i),
+    "cav_set_m": ([_vp, _vp, _i], _i),
+    "cav_get_m": ([_vp, _vp, _i], _i),
+    "cav_set_a": ([_vp, _dp], _i),
+    "cav_get_a": ([_vp, _dp], _i),
+    "cav_get_overlaps": ([_vp, _dp], _i),
+    "cav_get_dmdt": ([_vp, _vp, _i], _i),
+    "cav_get_dadt": ([_vp, _dp], _i),
+    "cav_set_sweep_order": ([_vp, _i], _i),
+    "cav_run": ([_vp, _d, _d, _d, _d], _i),
+    "cav_run_steps": ([_vp, _d, _d, _d, _d, _ll], _i),
+    "cav_sync": ([_vp], _i),
+    "cav_get_time": ([_vp, _dp, _dp], _i),
+    "cav_set_time": ([_vp, _d], _i),
+    "cav_get_stats": ([_vp, C.POINTER(cav_stats)], _i),
+    "cav_set_trace": ([_vp, _d, _i], _i),
+    "cav_trace_row_len": ([_vp, C.POINTER(_i)], _i),
+    "cav_get_trace": ([_vp, _dp, C.POINTER(_i)], _i),
+    "cav_set_block_cells": ([_vp, _i], _i),
+    "cav_get_launch_count": ([_vp, C.POINTER(_ll)], _i),
+    "cav_strerror": ([_i], C.c_char_p),
+    "cav_last_cuda_error": ([_vp], C.c_char_p),
+    "cav_version": ([], C.c_char_p),
+}
+for _name, (_args, _res) in _SIGS.items():
+    _f = getattr(_lib, _name)
+    _f.argtypes, _f.restype = _args, _res
+
+EXPORTS = tuple(_SIGS)
+
+
+def cav_strerror(status: int) -> str:
+    return _lib.cav_strerror(int(status)).decode()
+
+
+def cav_version() -> str:
+    return _lib.cav_version().decode()
+
+
+def _check(st: int, where: str, sim=None):
+    if st != CAV_OK:
+        detail = _lib.cav_last_cuda_error(sim).decode() if (sim and st == CAV_E_CUDA) else ""
+        raise CavError(st, where, detail)
+
+
+def _ptr(x):
+    """(address, is_device, keepalive) of a numpy array, a torch tensor or a raw int device address."""
+    if isinstance(x, np.ndarray):
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return x.ctypes.data, 0, x
+    if hasattr(x, "data_ptr"):          # torch tensor (duck-typed; torch is not imported here)
+        if not x.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return x.data_ptr(), (1 if x.is_cuda else 0), x
+    raise TypeError(f"unsupported buffer type {type(x)}")
+
+
+def _darr(x, n):
+    if x is None:
+        return None, None
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.float64).reshape(n))
+    return a.ctypes.data_as(_dp), a
+
+
+def cav_create(grid, params) -> int:
+    """grid = (nx, ny, nz, dx, dy, dz); params = dict with the cav_params fields. Returns the handle."""
+    g = cav_grid(int(grid[0]), int(grid[1]), int(grid[2]), float(grid[3]), float(grid[4]), float(grid[5]))
+    p = cav_params()
+    p.Ms, p.Aex, p.Ku = float(params["Ms"]), float(params["Aex"]), float(params.get("Ku", 0.0))
+    p.ku_axis = (C.c_double * 3)(*[float(v) for v in params.get("ku_axis", (0, 0, 1))])
+    p.alpha, p.gamma = float(params["alpha"]), float(params["gamma"])
+    p.B0 = (C.c_double * 3)(*[float(v) for v in params["B0"]])
+    p.n_sub = int(params.get("n_sub", 1))
+    p.B_exch_inter = float(params.get("B_exch_inter", 0.0))
+    p.precision = int(params.get("precision", CAV_F32))
+    p.renormalize = int(params.get("renormalize", 1))
+    p.overlap_norm = int(params.get("overlap_norm", CAV_NORM_NCELLS))
+    h = _vp()
+    _check(_lib.cav_create(C.byref(g), C.byref(p), C.byref(h)), "cav_create")
+    return h.value
+
+
+def cav_destroy(sim) -> None:
+    _check(_lib.cav_destroy(sim), "cav_destroy")
+
+
+def cav_set_stream(sim, cuda_stream: int) -> None:
+    _check(_lib.cav_set_stream(sim, _vp(cuda_stream)), "cav_set_stream", sim)
+
+
+def cav_set_launch_mode(sim, mode: int) -> None:
+    _check(_lib.cav_set_launch_mode(sim, int(mode)), "cav_set_launch_mode", sim)
+
+
+def cav_set_block_cells(sim, cells: int) -> None:
+    _check(_lib.cav_set_block_cells(sim, int(cells)), "cav_set_block_cells", sim)
+
+
+def cav_set_modes(sim, u, omega, kappa, g, Gamma=None, Phi=None) -> None:
+    """u: [N, nz, ny, nx] numpy array or torch tensor in the simulation's precision (None for N = 0)."""
+    N = 0 if omega is None else int(np.asarray(omega).size)
+    if N == 0:
+        _check(_lib.cav_set_modes(sim, 0, None, 0, None, None, None, None, None), "cav_set_modes", sim)
+        return
+    addr, dev, keep = _ptr(u)
+    po, ko = _darr(omega, N)
+    pk, kk = _darr(kappa, N)
+    pg, kg = _darr(g, N)
+    pG, kG = _darr(Gamma, N)
+    pP, kP = _darr(Phi, N)
+    _check(_lib.cav_set_modes(sim, N, _vp(addr), dev, po, pk, pg, pG, pP), "cav_set_modes", sim)
+
+
+def cav_set_m(sim, m) -> None:
+    addr, dev, keep = _ptr(m)
+    _check(_lib.cav_set_m(sim, _vp(addr), dev), "cav_set_m", sim)
+
+
+def cav_get_m(sim, out) -> None:
+    addr, dev, keep = _ptr(out)
+    _check(_lib.cav_get_m(sim, _vp(addr), dev), "cav_get_m", sim)
+
+
+def cav_set_a(sim, a) -> None:
+    a = np.ascontiguousarray(np.asarray(a, dtype=np.complex128)).view(np.float64)
+    _check(_lib.cav_set_a(sim, a.ctypes.data_as(_dp)), "cav_set_a", sim)
+
+
+def cav_get_a(sim, N: int) -> np.ndarray:
+    out = np.zeros(max(2 * N, 1))
+    _check(_lib.cav_get_a(sim, out.ctypes.data_as(_dp)), "cav_get_a", sim)
+    return out[:2 * N].view(np.complex128).copy()
+
+
+def cav_get_overlaps(sim, N: int) -> np.ndarray:
+    out = np.zeros(max(2 * N, 1))
+    _check(_lib.cav_get_overlaps(sim, out.ctypes.data_as(_dp)), "cav_get_overlaps", sim)
+    return out[:2 * N].view(np.complex128).copy()
+
+
+def cav_get_dmdt(sim, out) -> None:
+    addr, dev, keep = _ptr(out)
+    _check(_lib.cav_get_dmdt(sim, _vp(addr), dev), "cav_get_dmdt", sim)
+
+
+def cav_get_dadt(sim, N: int) -> np.ndarray:
+    out = np.zeros(max(2 * N, 1))
+    _check(_lib.cav_get_dadt(sim, out.ctypes.data_as(_dp)), "cav_get_dadt", sim)
+    return out[:2 * N].view(np.complex128).copy()
+
+
+def cav_set_sweep_order(sim, serpentine: int) -> None:
+    _check(_lib.cav_set_sweep_order(sim, int(serpentine)), "cav_set_sweep_order", sim)
+
+
+def cav_run(sim, t_end: float, tol: float = 0.0, fixed_dt: float = 0.0, dt_init: float = 0.0) -> None:
+    _check(_lib.cav_run(sim, float(t_end), float(tol), float(fixed_dt), float(dt_init)), "cav_run", sim)
+
+
+def cav_run_steps(sim, t_end: float, tol: float = 0.0, fixed_dt: float = 0.0, dt_init: float = 0.0,
+                  max_steps: int = 0) -> None:
+    _check(_lib.cav_run_steps(sim, float(t_end), float(tol), float(fixed_dt), float(dt_init), int(max_steps)),
+           "cav_run_steps", sim)
+
+
+def cav_sync(sim) -> None:
+    _check(_lib.cav_sync(sim), "cav_sync", sim)
+
+
+def cav_get_time(sim):
+    t, dt = _d(), _d()
+    _check(_lib.cav_get_time(sim, C.byref(t), C.byref(dt)), "cav_get_time", sim)
+    return t.value, dt.value
+
+
+def cav_set_time(sim, t: float) -> None:
+    _check(_lib.cav_set_time(sim, float(t)), "cav_set_time", sim)
+
+
+def cav_get_stats(sim) -> dict:
+    st = cav_stats()
+    _check(_lib.cav_get_stats(sim, C.byref(st)), "cav_get_stats", sim)
+    return {k: getattr(st, k) for k, _ in cav_stats._fields_}
+
+
+def cav_set_trace(sim, sample_dt: float, capacity: int) -> None:
+    _check(_lib.cav_set_trace(sim, float(sample_dt), int(capacity)), "cav_set_trace", sim)
+
+
+def cav_trace_row_len(sim) -> int:
+    row = _i()
+    _check(_lib.cav_trace_row_len(sim, C.byref(row)), "cav_trace_row_len", sim)
+    return row.value
+
+
+def cav_last_cuda_error(sim) -> str:
+    return _lib.cav_last_cuda_error(sim).decode()
+
+
+def cav_get_trace(sim) -> np.ndarray:
+    row = _i(cav_trace_row_len(sim))
+    n = _i()
+    _check(_lib.cav_get_trace(sim, None, C.byref(n)), "cav_get_trace", sim)
+    out = np.zeros((max(n.value, 1), row.value))
+    _check(_lib.cav_get_trace(sim, out.ctypes.data_as(_dp), C.byref(n)), "cav_get_trace", sim)
+    return out[:n.value].copy()
+
+
+def cav_get_launch_count(sim) -> int:
+    n = _ll()
+    _check(_lib.cav_get_launch_count(sim, C.byref(n)), "cav_get_launch_count", sim)
+    return n.value
+
+
+# ----------------------------------------------------------------------------------------
+# convenience: build a simulation from a problem description (still marshalling only)
+# ----------------------------------------------------------------------------------------
+class Sim:
+    """RAII wrapper around a cav_sim handle."""
+
+    def __init__(self, w, precision: str = "f32", renormalize: bool = True, overlap_norm: int = CAV_NORM_NCELLS,
+                 stream: int | None = None):
+        self.np_dtype = np.float32 if precision == "f32" else np.float64
+        self.N, self.n_sub = int(np.asarray(w.omega).size), int(w.n_sub)
+        self.shape_m = (self.n_sub, 3, w.nz, w.ny, w.nx)
+        self.h = cav_create((w.nx, w.ny, w.nz, w.dx, w.dy, w.dz),
+                            dict(Ms=w.Ms, Aex=w.Aex, Ku=w.Ku, ku_axis=w.ku_axis, alpha=w.alpha, gamma=w.gamma,
+                                 B0=w.B0, n_sub=w.n_sub, B_exch_inter=w.B_exch_inter,
+                                 precision=CAV_F32 if precision == "f32" else CAV_F64,
+                                 renormalize=int(renormalize), overlap_norm=overlap_norm))
+        if stream is not None:
+            cav_set_stream(self.h, stream)
+        if self.N:
+            cav_set_modes(self.h, np.ascontiguousarray(w.u, dtype=self.np_dtype), w.omega, w.kappa, w.g, w.Gamma, w.Phi)
+        else:
+            cav_set_modes(self.h, None, None, None, None)
+        cav_set_m(self.h, np.ascontiguousarray(w.m0, dtype=self.np_dtype))
+        if self.N:
+            cav_set_a(self.h, w.a0)
+
+    def close(self):
+        if self.h:
+            cav_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def get_m(self) -> np.ndarray:
+        out = np.empty(self.shape_m, dtype=self.np_dtype)
+        cav_get_m(self.h, out)
+        return out
+
+    def get_a(self) -> np.ndarray:
+        return cav_get_a(self.h, self.N)

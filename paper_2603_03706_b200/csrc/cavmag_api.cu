@@ -1,0 +1,693 @@
+// C-ABI layer of the cavity-magnonics hot path (include/cavmag.h): device buffers, the
+// CUDA graph whose body is a device-side WHILE loop over the six stage kernels, and the
+// small single-block kernels around it.  No torch types, no CPU fallback: every step of the
+// path runs in the kernels of stage_kernel.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/cavmag.h"
+#include "stage_kernel.cuh"
+
+using namespace cavmag;
+
+struct cav_sim {
+    cav_grid grid;
+    cav_params prm;
+    long long nc = 0, nvec = 0;
+    int vecw = 1;            // cells per thread (4 float / 2 double / 1)
+    int vec = 0;             // 1: vectorised kernels
+    size_t esize = 4;
+    size_t field_bytes = 0;  // n_sub*3*nc*esize
+    void* Y[2] = {nullptr, nullptr};
+    void* MS[2] = {nullptr, nullptr};
+    void* K[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    void* u = nullptr;
+    size_t u_bytes = 0;
+    double* partial = nullptr;
+    double* partial_max = nullptr;
+    int pstride = 0;
+    Ctrl* d_ctrl = nullptr;
+    Ctrl* h_ctrl = nullptr;      // pinned mirror
+    double* d_trace = nullptr;
+    int trace_cap = 0;
+    int N = 0, nb = 0;
+    bool m_set = false;
+    int iters = 1, nblocks = 1, user_block_cells = 0, serpentine = 1;
+    int launch_mode = CAV_LAUNCH_GRAPH;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    bool graph_dirty = true;
+    long long host_launches = 0;
+    int* h_flag = nullptr;       // pinned
+    char cuda_err[256] = {0};
+};
+
+namespace {
+
+#define CK(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess) {                                                              \
+            snprintf(s->cuda_err, sizeof(s->cuda_err), "%s at %s:%d: %s", #call, __FILE__, __LINE__, \
+                     cudaGetErrorString(e_));                                                 \
+            return (e_ == cudaErrorMemoryAllocation) ? CAV_E_NOMEM : CAV_E_CUDA;              \
+        }                                                                                     \
+    } while (0)
+
+// ---- small kernels around the stage kernels -------------------------------------------------
+
+__global__ void k_setrun(Ctrl* c, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
+    c->t_end = t_end;
+    c->tol = tol;
+    c->adaptive = tol > 0.0 ? 1 : 0;
+    c->fixed_dt = fixed_dt;
+    c->max_steps = max_steps;
+    c->steps_run = 0;
+    if (c->adaptive) {
+        if (dt_init > 0.0) c->dt = dt_init;
+        else if (!(c->dt > 0.0)) c->dt = 1e-14;
+    } else {
+        c->dt = fixed_dt;
+        long long st = llround(c->sample_dt / fixed_dt);
+        c->trace_stride = st < 1 ? 1 : st;
+    }
+}
+
+// First node of the run graph: decides whether there is anything to do, fixes h for the first
+// step and the mode amplitudes / RF weights of the first kernel, arms the WHILE condition.
+__global__ void k_begin(Ctrl* c, unsigned long long handle) {
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        c->done = (!(c->t < c->t_end) || c->status != 0) ? 1 : 0;
+        c->arrive = 0u;
+        prepare_h(c);
+    }
+    __syncthreads();
+    if (tid < c->N) {
+        if (!c->k1_valid) {      // stage 1 evaluates f(m_0, a_0)
+            c->as[tid][0] = c->a[tid][0]; c->as[tid][1] = c->a[tid][1];
+            c->c[tid] = (2.0 / c->gamma) * (c->Gre[tid] * c->a[tid][0] - c->Gim[tid] * c->a[tid][1]);
+        } else {
+            mode_stage_state(c, tid, 1);
+        }
+    }
+    if (tid == 0 && handle != 0ull) cudaGraphSetConditional((cudaGraphConditionalHandle)handle, c->done ? 0u : 1u);
+}
+
+template <typename T>
+__global__ void k_normalize(const T* __restrict__ src, T* __restrict__ dst, long long nc, int n_sub) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nc * n_sub) return;
+    const long long s = i / nc, r = i - s * nc;
+    const T* p = src + s * 3 * nc + r;
+    const T x = p[0], y = p[nc], z = p[2 * nc];
+    const T n2 = x * x + y * y + z * z;
+    const T inv = n2 > (T)0 ? (T)1 / sqrt(n2) : (T)0;
+    T* q = dst + s * 3 * nc + r;
+    q[0] = x * inv; q[nc] = y * inv; q[2 * nc] = z * inv;
+}
+
+// sum_r u_n(r) for CAV_NORM_SUM_U: 256 fixed-order block sums per mode, finished on the host.
+template <typename T>
+__global__ void k_sum_u(const T* __restrict__ u, long long nc, double* __restrict__ out /*[N][256]*/) {
+    const int n = blockIdx.y;
+    const T* p = u + (long long)n * nc;
+    const long long chunk = (nc + gridDim.x - 1) / gridDim.x;
+    const long long lo = (long long)blockIdx.x * chunk, hi = (lo + chunk < nc) ? lo + chunk : nc;
+    double acc = 0.0;
+    for (long long i = lo + threadIdx.x; i < hi; i += blockDim.x) acc += (double)p[i];
+    __shared__ double sh[256];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[n * gridDim.x + blockIdx.x] = sh[0];
+}
+
+const void* stage_fn(const cav_sim* s, int stage) {
+    const bool f32 = s->prm.precision == CAV_F32;
+    if (s->prm.n_sub == 1) return f32 ? stage_kernel_f32_fm(s->vec, stage, s->nb) : stage_kernel_f64_fm(s->vec, stage, s->nb);
+    return f32 ? stage_kernel_f32_afm(s->vec, stage, s->nb) : stage_kernel_f64_afm(s->vec, stage, s->nb);
+}
+
+int bucket(int N) { return N == 0 ? 0 : N <= 2 ? 2 : N <= 8 ? 8 : 32; }
+
+void choose_grid(cav_sim* s) {
+    const long long biters = (s->nvec + kBlock - 1) / kBlock;      // block-iterations in total
+    long long iters;
+    if (s->user_block_cells > 0) {
+        iters = s->user_block_cells / (kBlock * s->vecw);
+        if (iters < 1) iters = 1;
+    } else {
+        const long long target = 148 * 8;
+        iters = (biters + target - 1) / target;
+        if (iters < 1) iters = 1;
+    }
+    long long nb = (biters + iters - 1) / iters;
+    while (nb > s->pstride) { iters++; nb = (biters + iters - 1) / iters; }
+    s->iters = (int)iters;
+    s->nblocks = (int)nb;
+}
+
+StageArgs make_args(const cav_sim* s, unsigned long long handle) {
+    StageArgs A;
+    memset(&A, 0, sizeof(A));
+    A.ctrl = s->d_ctrl;
+    for (int i = 0; i < 2; ++i) { A.Y[i] = s->Y[i]; A.MS[i] = s->MS[i]; }
+    for (int i = 0; i < 7; ++i) A.K[i] = s->K[i];
+    A.u = s->u;
+    A.partial = s->partial;
+    A.partial_max = s->partial_max;
+    A.cond_handle = handle;
+    A.pstride = s->pstride;
+    A.nx = s->grid.nx; A.ny = s->grid.ny; A.nz = s->grid.nz;
+    A.iters = s->iters;
+    A.serpentine = s->serpentine;
+    A.nc = s->nc;
+    A.nvec = s->nvec;
+    const cav_params& p = s->prm;
+    for (int i = 0; i < 3; ++i) A.B0[i] = p.B0[i];
+    const double pe = (p.Ms > 0.0) ? 2.0 * p.Aex / p.Ms : 0.0;
+    A.ex_wx = pe / (s->grid.dx * s->grid.dx);
+    A.ex_wy = pe / (s->grid.dy * s->grid.dy);
+    A.ex_wz = pe / (s->grid.dz * s->grid.dz);
+    A.an_pref = (p.Ms > 0.0) ? 2.0 * p.Ku / p.Ms : 0.0;
+    double ax[3] = {p.ku_axis[0], p.ku_axis[1], p.ku_axis[2]};
+    const double an = std::sqrt(ax[0] * ax[0] + ax[1] * ax[1] + ax[2] * ax[2]);
+    for (int i = 0; i < 3; ++i) A.axis[i] = an > 0.0 ? ax[i] / an : (i == 2 ? 1.0 : 0.0);
+    A.alpha = p.alpha;
+    A.llg = -p.gamma / (1.0 + p.alpha * p.alpha);
+    A.B_exch_inter = p.n_sub == 2 ? p.B_exch_inter : 0.0;
+    A.renormalize = p.renormalize;
+    return A;
+}
+
+int sync_pull(cav_sim* s) {
+    CK(cudaStreamSynchronize(s->stream));
+    CK(cudaMemcpyAsync(s->h_ctrl, s->d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return CAV_OK;
+}
+
+int push_ctrl(cav_sim* s) {
+    CK(cudaMemcpyAsync(s->d_ctrl, s->h_ctrl, sizeof(Ctrl), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return CAV_OK;
+}
+
+void destroy_graph(cav_sim* s) {
+    if (s->exec) { cudaGraphExecDestroy(s->exec); s->exec = nullptr; }
+    if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+    s->graph_dirty = true;
+}
+
+int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraphNode_t* dep, const void* fn,
+               dim3 grid, dim3 block, void** params) {
+    cudaKernelNodeParams kp;
+    memset(&kp, 0, sizeof(kp));
+    kp.func = const_cast<void*>(fn);
+    kp.gridDim = grid;
+    kp.blockDim = block;
+    kp.sharedMemBytes = 0;
+    kp.kernelParams = params;
+    kp.extra = nullptr;
+    CK(cudaGraphAddKernelNode(node, g, dep, dep ? 1 : 0, &kp));
+    return CAV_OK;
+}
+
+// begin -> K1 -> WHILE { K2 -> K3 -> K4 -> K5 -> K6 -> K7 }
+int build_graph(cav_sim* s) {
+    destroy_graph(s);
+    choose_grid(s);
+    CK(cudaGraphCreate(&s->graph, 0));
+    cudaGraphConditionalHandle handle;
+    CK(cudaGraphConditionalHandleCreate(&handle, s->graph, 0, cudaGraphCondAssignDefault));
+    unsigned long long h64 = (unsigned long long)handle;
+    StageArgs A = make_args(s, h64);
+    double* trace = s->d_trace;
+    Ctrl* ctrl = s->d_ctrl;
+
+    cudaGraphNode_t n_begin, n_k1, n_while;
+    {
+        void* params[] = {&ctrl, &h64};
+        int rc = add_kernel(s, s->graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params);
+        if (rc) return rc;
+    }
+    {
+        void* params[] = {&A, &trace};
+        int rc = add_kernel(s, s->graph, &n_k1, &n_begin, stage_fn(s, 1), dim3(s->nblocks), dim3(kBlock), params);
+        if (rc) return rc;
+    }
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = handle;
+    cp.conditional.type = cudaGraphCondTypeWhile;
+    cp.conditional.size = 1;
+    CK(cudaGraphAddNode(&n_while, s->graph, &n_k1, 1, &cp));
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    cudaGraphNode_t prev;
+    for (int stage = 2; stage <= 7; ++stage) {
+        void* params[] = {&A, &trace};
+        cudaGraphNode_t node;
+        int rc = add_kernel(s, body, &node, stage == 2 ? nullptr : &prev, stage_fn(s, stage), dim3(s->nblocks),
+                            dim3(kBlock), params);
+        if (rc) return rc;
+        prev = node;
+    }
+    CK(cudaGraphInstantiate(&s->exec, s->graph, 0));
+    s->graph_dirty = false;
+    return CAV_OK;
+}
+
+int launch_stage(cav_sim* s, int stage, StageArgs& A) {
+    double* trace = s->d_trace;
+    void* params[] = {&A, &trace};
+    CK(cudaLaunchKernel(stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0, s->stream));
+    return CAV_OK;
+}
+
+int run_stream_mode(cav_sim* s) {
+    choose_grid(s);
+    StageArgs A = make_args(s, 0ull);
+    k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, 0ull);
+    CK(cudaGetLastError());
+    int rc = launch_stage(s, 1, A);
+    if (rc) return rc;
+    const int chunk = 16;
+    for (;;) {
+        for (int i = 0; i < chunk; ++i)
+            for (int stage = 2; stage <= 7; ++stage) {
+                rc = launch_stage(s, stage, A);
+                if (rc) return rc;
+            }
+        CK(cudaMemcpyAsync(s->h_flag, &s->d_ctrl->done, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+        if (*s->h_flag) break;
+    }
+    return CAV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* cav_version(void) { return "cavmag-b200 0.1 (sm_100a)"; }
+
+const char* cav_strerror(int st) {
+    switch (st) {
+        case CAV_OK: return "ok";
+        case CAV_E_ARG: return "invalid argument";
+        case CAV_E_STATE: return "invalid call order / state";
+        case CAV_E_CUDA: return "CUDA runtime error";
+        case CAV_E_NOMEM: return "out of memory";
+        case CAV_E_NONFINITE: return "non-finite error norm";
+        case CAV_E_DT_UNDERFLOW: return "step size underflow";
+        case CAV_E_SINGULAR_NORM: return "sum of mode profile is ~0 (CAV_NORM_SUM_U)";
+        case CAV_E_UNSUPPORTED: return "no supported CUDA device";
+        default: return "unknown status";
+    }
+}
+
+const char* cav_last_cuda_error(cav_sim* s) { return s ? s->cuda_err : ""; }
+
+int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
+    if (!grid || !prm || !out) return CAV_E_ARG;
+    *out = nullptr;
+    if (grid->nx < 1 || grid->ny < 1 || grid->nz < 1 || !(grid->dx > 0) || !(grid->dy > 0) || !(grid->dz > 0)) return CAV_E_ARG;
+    if (!(prm->Ms > 0) || prm->Aex < 0 || !(prm->gamma > 0) || prm->alpha < 0) return CAV_E_ARG;
+    if (prm->n_sub != 1 && prm->n_sub != 2) return CAV_E_ARG;
+    if (prm->precision != CAV_F32 && prm->precision != CAV_F64) return CAV_E_ARG;
+    if (prm->overlap_norm != CAV_NORM_NCELLS && prm->overlap_norm != CAV_NORM_SUM_U) return CAV_E_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return CAV_E_UNSUPPORTED; }
+    int dev = 0;
+    cudaDeviceProp dp;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&dp, dev) != cudaSuccess) return CAV_E_UNSUPPORTED;
+    if (dp.major != 10) return CAV_E_UNSUPPORTED;      // built for sm_100a only
+
+    cav_sim* s = new (std::nothrow) cav_sim();
+    if (!s) return CAV_E_NOMEM;
+    s->grid = *grid;
+    s->prm = *prm;
+    s->nc = (long long)grid->nx * grid->ny * grid->nz;
+    s->esize = prm->precision == CAV_F32 ? 4 : 8;
+    const int vw = prm->precision == CAV_F32 ? 4 : 2;
+    s->vec = (grid->nx % vw == 0) ? 1 : 0;
+    s->vecw = s->vec ? vw : 1;
+    s->nvec = s->nc / s->vecw;
+    s->field_bytes = (size_t)prm->n_sub * 3 * s->nc * s->esize;
+    const long long biters = (s->nvec + kBlock - 1) / kBlock;
+    s->pstride = (int)((biters < kMaxBlocks ? biters : kMaxBlocks) + 31) / 32 * 32;
+    int rc = CAV_OK;
+    auto fail = [&](int code) { cav_destroy(s); return code; };
+#define CKC(call)                                                                                         \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) {                                                                          \
+            cudaGetLastError();                                                                           \
+            return fail(e_ == cudaErrorMemoryAllocation ? CAV_E_NOMEM : CAV_E_CUDA);                      \
+        }                                                                                                 \
+    } while (0)
+    CKC(cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking));
+    s->own_stream = true;
+    for (int i = 0; i < 2; ++i) { CKC(cudaMalloc(&s->Y[i], s->field_bytes)); CKC(cudaMalloc(&s->MS[i], s->field_bytes)); }
+    for (int i = 0; i < 7; ++i) CKC(cudaMalloc(&s->K[i], s->field_bytes));
+    CKC(cudaMalloc(&s->partial, sizeof(double) * (size_t)kMaxSums * s->pstride));
+    CKC(cudaMalloc(&s->partial_max, sizeof(double) * (size_t)s->pstride));
+    CKC(cudaMalloc(&s->d_ctrl, sizeof(Ctrl)));
+    CKC(cudaMallocHost(&s->h_ctrl, sizeof(Ctrl)));
+    CKC(cudaMallocHost(&s->h_flag, sizeof(int)));
+#undef CKC
+    memset(s->h_ctrl, 0, sizeof(Ctrl));
+    s->h_ctrl->gamma = prm->gamma;
+    s->h_ctrl->dt_min = INFINITY;
+    s->h_ctrl->t_end = 0.0;
+    s->h_ctrl->trace_stride = 1;
+    rc = push_ctrl(s);
+    if (rc) return fail(rc);
+    choose_grid(s);
+    *out = s;
+    return CAV_OK;
+}
+
+int cav_destroy(cav_sim* s) {
+    if (!s) return CAV_E_ARG;
+    if (s->stream) cudaStreamSynchronize(s->stream);
+    destroy_graph(s);
+    for (int i = 0; i < 2; ++i) { cudaFree(s->Y[i]); cudaFree(s->MS[i]); }
+    for (int i = 0; i < 7; ++i) cudaFree(s->K[i]);
+    cudaFree(s->u);
+    cudaFree(s->partial);
+    cudaFree(s->partial_max);
+    cudaFree(s->d_ctrl);
+    cudaFree(s->d_trace);
+    if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
+    if (s->h_flag) cudaFreeHost(s->h_flag);
+    if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
+    cudaGetLastError();
+    delete s;
+    return CAV_OK;
+}
+
+int cav_set_stream(cav_sim* s, void* stream) {
+    if (!s) return CAV_E_ARG;
+    CK(cudaStreamSynchronize(s->stream));
+    if (s->own_stream) { cudaStreamDestroy(s->stream); s->own_stream = false; }
+    s->stream = (cudaStream_t)stream;
+    return CAV_OK;
+}
+
+int cav_set_launch_mode(cav_sim* s, int mode) {
+    if (!s || (mode != CAV_LAUNCH_GRAPH && mode != CAV_LAUNCH_STREAM)) return CAV_E_ARG;
+    s->launch_mode = mode;
+    return CAV_OK;
+}
+
+int cav_set_block_cells(cav_sim* s, int cells) {
+    if (!s || cells < 0) return CAV_E_ARG;
+    s->user_block_cells = cells;
+    s->graph_dirty = true;
+    choose_grid(s);
+    return CAV_OK;
+}
+
+int cav_set_sweep_order(cav_sim* s, int serpentine) {
+    if (!s) return CAV_E_ARG;
+    s->serpentine = serpentine ? 1 : 0;
+    s->graph_dirty = true;
+    return CAV_OK;
+}
+
+int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const double* omega, const double* kappa,
+                  const double* g, const double* Gamma, const double* Phi) {
+    if (!s || N < 0 || N > CAV_MAX_MODES) return CAV_E_ARG;
+    if (N > 0 && (!u || !omega || !kappa || !g)) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    const size_t bytes = (size_t)N * s->nc * s->esize;
+    if (bytes > s->u_bytes) {
+        cudaFree(s->u);
+        s->u = nullptr;
+        s->u_bytes = 0;
+        CK(cudaMalloc(&s->u, bytes));
+        s->u_bytes = bytes;
+    }
+    if (N > 0)
+        CK(cudaMemcpyAsync(s->u, u, bytes, u_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
+    Ctrl* c = s->h_ctrl;
+    c->N = N;
+    for (int n = 0; n < N; ++n) {
+        const double Gm = Gamma ? Gamma[n] : 0.0, Ph = Phi ? Phi[n] : 0.0;
+        c->omega[n] = omega[n];
+        c->kappa[n] = kappa[n];
+        c->Gre[n] = g[n] + Gm * std::cos(Ph);
+        c->Gim[n] = Gm * std::sin(Ph);
+        c->invW[n] = 1.0 / (double)s->nc;
+        c->a[n][0] = c->a[n][1] = 0.0;
+    }
+    if (N > 0 && s->prm.overlap_norm == CAV_NORM_SUM_U) {
+        double* d_out = nullptr;
+        CK(cudaMalloc(&d_out, sizeof(double) * 256 * N));
+        if (s->prm.precision == CAV_F32) k_sum_u<float><<<dim3(256, N), 256, 0, s->stream>>>((const float*)s->u, s->nc, d_out);
+        else k_sum_u<double><<<dim3(256, N), 256, 0, s->stream>>>((const double*)s->u, s->nc, d_out);
+        s->host_launches++;
+        double* h = (double*)malloc(sizeof(double) * 256 * N);
+        cudaError_t e1 = cudaMemcpyAsync(h, d_out, sizeof(double) * 256 * N, cudaMemcpyDeviceToHost, s->stream);
+        cudaError_t e2 = cudaStreamSynchronize(s->stream);
+        cudaFree(d_out);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) { free(h); return CAV_E_CUDA; }
+        for (int n = 0; n < N; ++n) {
+            double sum = 0.0;
+            for (int b = 0; b < 256; ++b) sum += h[n * 256 + b];
+            if (std::fabs(sum) < 1e-6 * (double)s->nc) { free(h); return CAV_E_SINGULAR_NORM; }
+            c->invW[n] = 1.0 / sum;
+        }
+        free(h);
+    }
+    c->k1_valid = 0;
+    s->N = N;
+    const int nb = bucket(N);
+    if (nb != s->nb) { s->nb = nb; }
+    s->graph_dirty = true;
+    return push_ctrl(s);
+}
+
+int cav_set_m(cav_sim* s, const void* m, int is_device) {
+    if (!s || !m) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    const void* src = m;
+    if (!is_device) {
+        CK(cudaMemcpyAsync(s->MS[1], m, s->field_bytes, cudaMemcpyHostToDevice, s->stream));
+        src = s->MS[1];
+    }
+    void* dst = s->Y[s->h_ctrl->ycur];
+    const long long n = s->nc * s->prm.n_sub;
+    const int blocks = (int)((n + 255) / 256);
+    if (s->prm.precision == CAV_F32) k_normalize<float><<<blocks, 256, 0, s->stream>>>((const float*)src, (float*)dst, s->nc, s->prm.n_sub);
+    else k_normalize<double><<<blocks, 256, 0, s->stream>>>((const double*)src, (double*)dst, s->nc, s->prm.n_sub);
+    CK(cudaGetLastError());
+    s->host_launches++;
+    s->h_ctrl->k1_valid = 0;
+    s->h_ctrl->status = 0;
+    s->m_set = true;
+    return push_ctrl(s);
+}
+
+int cav_get_m(cav_sim* s, void* out, int is_device) {
+    if (!s || !out) return CAV_E_ARG;
+    if (!s->m_set) return CAV_E_STATE;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, s->Y[s->h_ctrl->ycur], s->field_bytes,
+                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return s->h_ctrl->status;
+}
+
+int cav_set_a(cav_sim* s, const double* a) {
+    if (!s || (!a && s->N > 0)) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    for (int n = 0; n < s->N; ++n) { s->h_ctrl->a[n][0] = a[2 * n]; s->h_ctrl->a[n][1] = a[2 * n + 1]; }
+    s->h_ctrl->k1_valid = 0;
+    return push_ctrl(s);
+}
+
+int cav_get_a(cav_sim* s, double* out) {
+    if (!s || (!out && s->N > 0)) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    for (int n = 0; n < s->N; ++n) { out[2 * n] = s->h_ctrl->a[n][0]; out[2 * n + 1] = s->h_ctrl->a[n][1]; }
+    return s->h_ctrl->status;
+}
+
+static int ensure_k1(cav_sim* s) {
+    if (!s->m_set) return CAV_E_STATE;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    if (!s->h_ctrl->k1_valid) {
+        choose_grid(s);
+        StageArgs A = make_args(s, 0ull);
+        k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, 0ull);
+        CK(cudaGetLastError());
+        s->host_launches++;
+        rc = launch_stage(s, 1, A);
+        if (rc) return rc;
+        rc = sync_pull(s);
+    }
+    return rc;
+}
+
+int cav_get_dmdt(cav_sim* s, void* out, int is_device) {
+    if (!s || !out) return CAV_E_ARG;
+    int rc = ensure_k1(s);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, s->K[s->h_ctrl->k1slot], s->field_bytes,
+                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return s->h_ctrl->status;
+}
+
+int cav_get_dadt(cav_sim* s, double* out) {
+    if (!s || (!out && s->N > 0)) return CAV_E_ARG;
+    int rc = ensure_k1(s);
+    if (rc) return rc;
+    for (int n = 0; n < s->N; ++n) { out[2 * n] = s->h_ctrl->ka[0][n][0]; out[2 * n + 1] = s->h_ctrl->ka[0][n][1]; }
+    return s->h_ctrl->status;
+}
+
+int cav_get_overlaps(cav_sim* s, double* out) {
+    if (!s || (!out && s->N > 0)) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    for (int n = 0; n < s->N; ++n) { out[2 * n] = s->h_ctrl->S[n][0]; out[2 * n + 1] = s->h_ctrl->S[n][1]; }
+    return s->h_ctrl->status;
+}
+
+int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
+    if (!s) return CAV_E_ARG;
+    if (!s->m_set) return CAV_E_STATE;
+    const bool adaptive = tol > 0.0;
+    if (adaptive == (fixed_dt > 0.0)) return CAV_E_ARG;        // exactly one of the two
+    if (std::isnan(t_end) || max_steps < 0) return CAV_E_ARG;
+    if (std::isinf(t_end) && max_steps == 0) return CAV_E_ARG;
+    k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
+    CK(cudaGetLastError());
+    s->host_launches++;
+    if (s->launch_mode == CAV_LAUNCH_GRAPH) {
+        if (s->graph_dirty || !s->exec) {
+            int rc = build_graph(s);
+            if (rc) return rc;
+        }
+        CK(cudaGraphLaunch(s->exec, s->stream));
+        s->host_launches++;   // k_begin
+        return CAV_OK;
+    }
+    s->host_launches++;
+    return run_stream_mode(s);
+}
+
+int cav_run(cav_sim* s, double t_end, double tol, double fixed_dt, double dt_init) {
+    if (!(t_end < INFINITY)) return CAV_E_ARG;
+    return cav_run_steps(s, t_end, tol, fixed_dt, dt_init, 0);
+}
+
+int cav_sync(cav_sim* s) {
+    if (!s) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    return s->h_ctrl->status;
+}
+
+int cav_get_time(cav_sim* s, double* t, double* dt) {
+    if (!s) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    if (t) *t = s->h_ctrl->t;
+    if (dt) *dt = s->h_ctrl->dt;
+    return s->h_ctrl->status;
+}
+
+int cav_set_time(cav_sim* s, double t) {
+    if (!s || std::isnan(t)) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    s->h_ctrl->t = t;
+    return push_ctrl(s);
+}
+
+int cav_get_stats(cav_sim* s, cav_stats* o) {
+    if (!s || !o) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    const Ctrl* c = s->h_ctrl;
+    o->accepted = c->accepted; o->rejected = c->rejected; o->rhs_evals = c->rhs_evals;
+    o->dt_min = c->dt_min; o->dt_max = c->dt_max; o->dt_next = c->dt; o->t = c->t; o->last_err = c->last_err;
+    return c->status;
+}
+
+int cav_set_trace(cav_sim* s, double sample_dt, int capacity) {
+    if (!s || capacity < 0) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    Ctrl* c = s->h_ctrl;
+    if (!(sample_dt > 0.0) || capacity == 0) {
+        c->sample_dt = 0.0; c->trace_cap = 0; c->trace_n = 0;
+        return push_ctrl(s);
+    }
+    const int row = 1 + 4 * s->N + 3 * s->prm.n_sub;
+    if (capacity > s->trace_cap) {
+        cudaFree(s->d_trace);
+        s->d_trace = nullptr;
+        s->trace_cap = 0;
+        CK(cudaMalloc(&s->d_trace, sizeof(double) * (size_t)capacity * (1 + 4 * CAV_MAX_MODES + 6)));
+        s->trace_cap = capacity;
+        s->graph_dirty = true;
+    }
+    (void)row;
+    c->sample_dt = sample_dt;
+    c->trace_cap = capacity;
+    c->trace_n = 0;
+    c->trace_t0 = c->t;
+    c->trace_acc0 = c->accepted;
+    c->trace_stride = 1;
+    return push_ctrl(s);
+}
+
+int cav_trace_row_len(cav_sim* s, int* row_len) {
+    if (!s || !row_len) return CAV_E_ARG;
+    *row_len = 1 + 4 * s->N + 3 * s->prm.n_sub;
+    return CAV_OK;
+}
+
+int cav_get_trace(cav_sim* s, double* out, int* n_samples) {
+    if (!s || !n_samples) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    const int n = s->h_ctrl->trace_n;
+    *n_samples = n;
+    const int row = 1 + 4 * s->N + 3 * s->prm.n_sub;
+    if (out && n > 0) {
+        CK(cudaMemcpyAsync(out, s->d_trace, sizeof(double) * (size_t)n * row, cudaMemcpyDeviceToHost, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+    }
+    return s->h_ctrl->status;
+}
+
+int cav_get_launch_count(cav_sim* s, long long* n) {
+    if (!s || !n) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    *n = s->host_launches + s->h_ctrl->rhs_evals;
+    return CAV_OK;
+}
+
+}  // extern "C"

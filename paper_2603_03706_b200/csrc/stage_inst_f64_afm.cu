@@ -1,0 +1,7 @@
+// Explicit instantiations of the fused stage kernel: T = double, n_sub = 2 (one TU per pair so
+// the 56 kernels of each pair compile in parallel with the others).
+#include "stage_kernel.cuh"
+
+namespace cavmag {
+CAVMAG_DEFINE_LOOKUP(stage_kernel_f64_afm, double, 2, 2)
+}  // namespace cavmag

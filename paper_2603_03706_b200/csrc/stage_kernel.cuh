@@ -1,0 +1,599 @@
+// The fused RK45 stage kernel (hand-written CUDA for sm_100a).
+//
+// One launch = one evaluation of the coupled right-hand side at stage s of the
+// Dormand-Prince step, fused with everything that can ride along on the same pass over HBM:
+//
+//   (a1) stage state          m_s(r)                    read with its 6-neighbour halo
+//   (a4) overlap partials     sum_r u_n(r) m_c(r)       PAPER.md:156 Eq. 18  (of THIS stage's input)
+//   (a2) effective field      B0 + exchange + anisotropy + x^ sum_n c_n u_n(r) [- B_E m_other]
+//                                                       PAPER.md:121 Eq. 13, :159
+//   (a3) LLG slope            k_s = -gamma/(1+alpha^2)[m x B + alpha m x (m x B)]
+//   (a1) next stage state     m_{s+1} = m_0 + h sum_j a_{s+1,j} k_j     (materialised for the next launch)
+//   (a6) stage 6: y5 -> m_new = y5/|y5| and the partial error field; stage 7: error max-norm
+//   (a5,a7) the LAST block to finish reduces the block partials in a fixed order and runs the
+//        mode ODEs (PAPER.md:119 Eq. 12, :317 Eq. 19), the mode stage algebra and, after
+//        stage 7, the step-size controller — so no separate launch and no host round trip.
+//
+// Each thread owns VEC consecutive x cells (one 16-byte vector per field component); x
+// neighbours come from warp shuffles, y/z neighbours from L1/L2-cached vector loads.  This is
+// an HBM-bound streaming stencil: no tensor cores, no shared-memory tile.
+#pragma once
+#include <math_constants.h>
+
+#include "cavmag_types.cuh"
+
+namespace cavmag {
+
+__device__ constexpr double kA[7][7] = CAVMAG_DP_A;
+__device__ constexpr double kD[7] = CAVMAG_DP_D;
+
+// ---------------------------------------------------------------------------------------
+// vector load/store of VEC consecutive cells (16 bytes for float4 / double2)
+// ---------------------------------------------------------------------------------------
+template <typename T, int VEC>
+struct alignas(sizeof(T) * VEC) Pack {
+    T v[VEC];
+};
+
+template <typename T, int VEC>
+__device__ __forceinline__ Pack<T, VEC> ldp(const T* __restrict__ p) {
+    Pack<T, VEC> r;
+    if constexpr (sizeof(T) * VEC == 16) {
+        const float4 q = __ldg(reinterpret_cast<const float4*>(p));
+        r = *reinterpret_cast<const Pack<T, VEC>*>(&q);
+    } else if constexpr (sizeof(T) * VEC == 8) {
+        const float2 q = __ldg(reinterpret_cast<const float2*>(p));
+        r = *reinterpret_cast<const Pack<T, VEC>*>(&q);
+    } else {
+        r.v[0] = __ldg(p);
+    }
+    return r;
+}
+template <typename T, int VEC>
+__device__ __forceinline__ void stp(T* __restrict__ p, const Pack<T, VEC>& x) {
+    *reinterpret_cast<Pack<T, VEC>*>(p) = x;
+}
+
+template <typename T>
+__device__ __forceinline__ T rsqrt_t(T x);
+template <>
+__device__ __forceinline__ float rsqrt_t<float>(float x) { return 1.0f / sqrtf(x); }
+template <>
+__device__ __forceinline__ double rsqrt_t<double>(double x) { return 1.0 / sqrt(x); }
+
+// ---------------------------------------------------------------------------------------
+// Step preparation (single thread): choose h for the step that starts now.
+// Mirrors the controller spec in DESIGN.md: clamp onto t_end / the next trace sample.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void prepare_h(Ctrl* c) {
+    double h = c->dt;
+    double target = c->t_end;
+    int sample_hit = 0;
+    if (c->adaptive && c->sample_dt > 0.0 && c->trace_n < c->trace_cap) {
+        const double ts = c->trace_t0 + (double)(c->trace_n + 1) * c->sample_dt;
+        if (ts <= target) { target = ts; sample_hit = 1; }
+    }
+    int clamped = 0;
+    if (c->t + h * (1.0 + 1e-12) >= target) { h = target - c->t; clamped = 1; }
+    c->h = h; c->target = target; c->clamped = clamped; c->sample_hit = sample_hit;
+}
+
+// a_s and the RF weights c_n = (2/gamma) Re[G_n a_s,n] for stage row `row` (0-based: row r gives
+// the state of stage r+1), one thread per mode.
+__device__ __forceinline__ void mode_stage_state(Ctrl* c, int n, int row) {
+    double re = 0.0, im = 0.0;
+    for (int j = 0; j < row; ++j) {
+        re += kA[row][j] * c->ka[j][n][0];
+        im += kA[row][j] * c->ka[j][n][1];
+    }
+    const double are = c->a[n][0] + c->h * re, aim = c->a[n][1] + c->h * im;
+    c->as[n][0] = are; c->as[n][1] = aim;
+    c->c[n] = (2.0 / c->gamma) * (c->Gre[n] * are - c->Gim[n] * aim);
+}
+
+// ---------------------------------------------------------------------------------------
+// Tail of every stage kernel, executed by the last block to arrive: deterministic second
+// reduction pass, mode ODEs + stage algebra, and (stage 7) the accept/reject controller.
+// ---------------------------------------------------------------------------------------
+static __device__ __noinline__ void stage_finish(const StageArgs& A, const int stage, const int nsub, double* trace) {
+    Ctrl* c = A.ctrl;
+    __shared__ double sred[kMaxSums];
+    __shared__ double smax;
+    __shared__ double serr[kMaxModes];
+    __shared__ int s_accept;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int nwarp = kBlock / 32;
+    const int N = c->N;
+    const int nblk = gridDim.x;
+    const int nsum = 2 * N + (stage == 7 ? 3 * nsub : 0);
+    __threadfence();
+    // pass 2: lane l adds blocks l, l+32, ... in order, then a fixed xor tree
+    for (int comp = warp; comp < nsum; comp += nwarp) {
+        const double* p = A.partial + (size_t)comp * A.pstride;
+        double acc = 0.0;
+        for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
+            double v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) v[j] = (b0 + 32 * j < nblk) ? __ldcg(p + b0 + 32 * j) : 0.0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc += v[j];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) sred[comp] = acc;
+    }
+    if (stage == 7 && warp == nwarp - 1) {
+        double mx = 0.0;
+        for (int b = lane; b < nblk; b += 32) mx = fmax(mx, __ldcg(A.partial_max + b));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if (lane == 0) smax = mx;
+    }
+    __syncthreads();
+
+    // mode ODE at this stage: ka_s = -(i w + kappa) a_s + i G S_s     (Eq. 12 / Eq. 19)
+    if (tid < N) {
+        const int n = tid;
+        const double Sre = sred[2 * n] * c->invW[n];
+        const double Sim = -sred[2 * n + 1] * c->invW[n];
+        c->S[n][0] = Sre; c->S[n][1] = Sim;
+        const double are = c->as[n][0], aim = c->as[n][1];
+        const double Gre = c->Gre[n], Gim = c->Gim[n];
+        const double kre = (-c->kappa[n] * are + c->omega[n] * aim) - (Gre * Sim + Gim * Sre);
+        const double kim = (-c->kappa[n] * aim - c->omega[n] * are) + (Gre * Sre - Gim * Sim);
+        c->ka[stage - 1][n][0] = kre; c->ka[stage - 1][n][1] = kim;
+        if (stage >= 2 && stage <= 5) {
+            mode_stage_state(c, n, stage);              // a_{s+1}, c^{(s+1)}
+        } else if (stage == 6) {
+            mode_stage_state(c, n, 6);                  // row 6 = b: the 5th-order candidate
+            c->anew[n][0] = c->as[n][0]; c->anew[n][1] = c->as[n][1];
+        } else if (stage == 7) {
+            double ere = 0.0, eim = 0.0;
+            for (int j = 0; j < 7; ++j) { ere += kD[j] * c->ka[j][n][0]; eim += kD[j] * c->ka[j][n][1]; }
+            const double e = fabs(c->h) * sqrt(ere * ere + eim * eim);
+            serr[n] = (e < CUDART_INF) ? e : CUDART_INF;
+        }
+    }
+    if (stage >= 2 && stage <= 6) {
+        if (tid == 0) { c->rhs_evals++; c->arrive = 0u; }
+        return;
+    }
+    __syncthreads();
+
+    if (stage == 7) {
+        if (tid == 0) {
+            double err = sqrt(smax);
+            for (int n = 0; n < N; ++n) err = fmax(err, serr[n]);
+            const bool finite = err < CUDART_INF;
+            const double h = c->h;
+            bool accept;
+            if (c->adaptive) accept = finite && err <= c->tol;
+            else { accept = true; if (!finite) { accept = false; c->status = -5; } }
+            double fac;
+            if (!finite) fac = 0.5;
+            else if (err == 0.0) fac = 2.0;
+            else { fac = 0.8 * pow(c->tol / err, 0.2); fac = fmin(fmax(fac, 0.5), 2.0); }
+            c->rhs_evals++;
+            c->steps_run++;
+            c->last_err = err;
+            if (accept) {
+                c->t = c->clamped ? c->target : c->t + h;
+                c->ycur ^= 1;
+                c->k1slot = 6 - c->k1slot;
+                c->accepted++;
+                c->dt_min = fmin(c->dt_min, h);
+                c->dt_max = fmax(c->dt_max, h);
+                if (c->adaptive) { const double prop = h * fac; c->dt = c->clamped ? fmax(prop, c->dt) : prop; }
+                for (int i = 0; i < 3 * nsub; ++i) c->mavg[i] = sred[2 * N + i] / (double)A.nc;
+                const bool take = trace != nullptr && c->sample_dt > 0.0 && c->trace_n < c->trace_cap &&
+                                  (c->adaptive ? (c->clamped && c->sample_hit)
+                                               : ((c->accepted - c->trace_acc0) % c->trace_stride == 0));
+                if (take) {
+                    double* row = trace + (size_t)c->trace_n * (1 + 4 * N + 3 * nsub);
+                    row[0] = c->t;
+                    for (int n = 0; n < N; ++n) {
+                        row[1 + 2 * n] = c->anew[n][0]; row[2 + 2 * n] = c->anew[n][1];
+                        row[1 + 2 * N + 2 * n] = c->S[n][0]; row[2 + 2 * N + 2 * n] = c->S[n][1];
+                    }
+                    for (int i = 0; i < 3 * nsub; ++i) row[1 + 4 * N + i] = c->mavg[i];
+                    c->trace_n++;
+                }
+            } else if (c->status == 0) {
+                c->rejected++;
+                c->dt = h * fac;
+            }
+            if (c->adaptive && !(c->dt > 1e-20)) c->status = -6;
+            s_accept = accept ? 1 : 0;
+        }
+        __syncthreads();
+        if (tid < N && s_accept) {     // y := y_new (modes), FSAL: ka_1 := ka_7
+            c->a[tid][0] = c->anew[tid][0]; c->a[tid][1] = c->anew[tid][1];
+            c->ka[0][tid][0] = c->ka[6][tid][0]; c->ka[0][tid][1] = c->ka[6][tid][1];
+        }
+        __syncthreads();
+    } else {   // stage 1: k1 of a fresh state
+        if (tid == 0) { c->rhs_evals++; c->k1_valid = 1; }
+    }
+
+    // start of the next step
+    if (tid == 0) {
+        const bool done = !(c->t < c->t_end) || (c->max_steps > 0 && c->steps_run >= c->max_steps) || c->status != 0;
+        c->done = done ? 1 : 0;
+        prepare_h(c);
+    }
+    __syncthreads();
+    if (tid < N) mode_stage_state(c, tid, 1);           // a_2 = a_0 + h a21 ka_1
+    if (tid == 0) {
+        c->arrive = 0u;
+        if (A.cond_handle != 0ull && stage == 7)
+            cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, c->done ? 0u : 1u);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// the stage kernel
+// ---------------------------------------------------------------------------------------
+template <typename T, int VEC, int STAGE, int NSUB, int NB>
+__global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __restrict__ trace) {
+    using P = Pack<T, VEC>;
+    Ctrl* ctrl = A.ctrl;
+    if (STAGE == 1) { if (ctrl->k1_valid) return; }
+    else if (ctrl->done) return;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = ctrl->N;
+    const T h = (T)ctrl->h;
+    const int ycur = ctrl->ycur, k1slot = ctrl->k1slot;
+    const long long nc = A.nc;
+    const int nx = A.nx, ny = A.ny, nz = A.nz;
+    const long long plane = (long long)nx * ny;
+
+    const T* __restrict__ y0 = (const T*)A.Y[ycur];
+    T* __restrict__ ynew = (T*)A.Y[1 - ycur];
+    const T* __restrict__ k1 = (const T*)A.K[k1slot];
+    const T* __restrict__ uu = (const T*)A.u;
+    // stage input (materialised) and outputs
+    const T* __restrict__ ms = STAGE == 1 ? y0 : STAGE == 7 ? (const T*)ynew
+                              : (STAGE == 3 || STAGE == 5) ? (const T*)A.MS[0] : (const T*)A.MS[1];
+    T* __restrict__ kout = STAGE == 1 ? (T*)A.K[k1slot] : STAGE == 7 ? (T*)A.K[6 - k1slot] : (T*)A.K[STAGE - 1];
+    T* __restrict__ mnext = STAGE == 6 ? ynew : (STAGE == 2 || STAGE == 4) ? (T*)A.MS[0] : (T*)A.MS[1];
+    T* __restrict__ e6 = (T*)A.MS[0];    // written by stage 6, read by stage 7
+
+    const T ha21 = h * (T)kA[1][0];
+    const T B0x = (T)A.B0[0], B0y = (T)A.B0[1], B0z = (T)A.B0[2];
+    const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
+    const T anp = (T)A.an_pref, axx = (T)A.axis[0], axy = (T)A.axis[1], axz = (T)A.axis[2];
+    const T alpha = (T)A.alpha, llg = (T)A.llg, BE = (T)A.B_exch_inter;
+
+    T cn[NB > 0 ? NB : 1];
+#pragma unroll
+    for (int n = 0; n < NB; ++n) cn[n] = (n < N) ? (T)ctrl->c[n] : (T)0;
+
+    // per-thread running sums
+    T ox[NB > 0 ? NB : 1], oy[NB > 0 ? NB : 1];
+#pragma unroll
+    for (int n = 0; n < NB; ++n) { ox[n] = (T)0; oy[n] = (T)0; }
+    T sm[NSUB * 3];
+#pragma unroll
+    for (int i = 0; i < NSUB * 3; ++i) sm[i] = (T)0;
+    T emax2 = (T)0;
+
+    const long long nblk = gridDim.x;
+    const long long blk = (A.serpentine && (STAGE & 1)) ? (nblk - 1 - blockIdx.x) : blockIdx.x;
+    const long long vbase = blk * (long long)A.iters * kBlock;
+
+    for (int it = 0; it < A.iters; ++it) {
+        const long long vraw = vbase + (long long)it * kBlock + tid;
+        const bool active = vraw < A.nvec;
+        const long long cell = (active ? vraw : (A.nvec - 1)) * VEC;
+        const int z = (int)(cell / plane);
+        const int rem = (int)(cell - (long long)z * plane);
+        const int y = rem / nx;
+        const int x0 = rem - y * nx;
+        const long long iym = (y > 0) ? cell - nx : cell, iyp = (y < ny - 1) ? cell + nx : cell;
+        const long long izm = (z > 0) ? cell - plane : cell, izp = (z < nz - 1) ? cell + plane : cell;
+        const bool has_l = x0 > 0, has_r = x0 + VEC < nx;
+
+        // ---- stage state at the centre (all sublattices) ----
+        P mc[NSUB][3], y0c[NSUB][3], k1c[NSUB][3];
+#pragma unroll
+        for (int s = 0; s < NSUB; ++s)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const long long off = (long long)(s * 3 + c) * nc + cell;
+                if constexpr (STAGE == 2) {
+                    y0c[s][c] = ldp<T, VEC>(y0 + off);
+                    k1c[s][c] = ldp<T, VEC>(k1 + off);
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) mc[s][c].v[v] = y0c[s][c].v[v] + ha21 * k1c[s][c].v[v];
+                } else {
+                    mc[s][c] = ldp<T, VEC>(ms + off);
+                }
+            }
+
+        // ---- mode profiles: RF field weight and overlap partials of THIS stage state ----
+        T brf[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) brf[v] = (T)0;
+        if constexpr (NB > 0) {
+            T mcx[VEC], mcy[VEC];
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                if constexpr (NSUB == 1) { mcx[v] = mc[0][0].v[v]; mcy[v] = mc[0][1].v[v]; }
+                else { mcx[v] = (T)0.5 * (mc[0][0].v[v] + mc[1][0].v[v]); mcy[v] = (T)0.5 * (mc[0][1].v[v] + mc[1][1].v[v]); }
+            }
+#pragma unroll
+            for (int n = 0; n < NB; ++n) {
+                if (n < N) {
+                    P un = ldp<T, VEC>(uu + (long long)n * nc + cell);
+                    T sx = (T)0, sy = (T)0;
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) {
+                        brf[v] += cn[n] * un.v[v];
+                        sx += un.v[v] * mcx[v];
+                        sy += un.v[v] * mcy[v];
+                    }
+                    if (active) { ox[n] += sx; oy[n] += sy; }
+                }
+            }
+        }
+
+#pragma unroll
+        for (int s = 0; s < NSUB; ++s) {
+            // ---- 6-neighbour exchange: sum over in-grid neighbours of (m_nb - m)/D^2 ----
+            T lap[3][VEC];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const long long base = (long long)(s * 3 + c) * nc;
+                P nym, nyp, nzm, nzp;
+                T xl, xr;
+                if constexpr (STAGE == 2) {
+                    const P a0 = ldp<T, VEC>(y0 + base + iym), b0 = ldp<T, VEC>(k1 + base + iym);
+                    const P a1 = ldp<T, VEC>(y0 + base + iyp), b1 = ldp<T, VEC>(k1 + base + iyp);
+                    const P a2 = ldp<T, VEC>(y0 + base + izm), b2 = ldp<T, VEC>(k1 + base + izm);
+                    const P a3 = ldp<T, VEC>(y0 + base + izp), b3 = ldp<T, VEC>(k1 + base + izp);
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) {
+                        nym.v[v] = a0.v[v] + ha21 * b0.v[v]; nyp.v[v] = a1.v[v] + ha21 * b1.v[v];
+                        nzm.v[v] = a2.v[v] + ha21 * b2.v[v]; nzp.v[v] = a3.v[v] + ha21 * b3.v[v];
+                    }
+                } else {
+                    nym = ldp<T, VEC>(ms + base + iym); nyp = ldp<T, VEC>(ms + base + iyp);
+                    nzm = ldp<T, VEC>(ms + base + izm); nzp = ldp<T, VEC>(ms + base + izp);
+                }
+                xl = __shfl_up_sync(0xffffffffu, mc[s][c].v[VEC - 1], 1);
+                xr = __shfl_down_sync(0xffffffffu, mc[s][c].v[0], 1);
+                if (!has_l) xl = mc[s][c].v[0];
+                else if (lane == 0) {
+                    if constexpr (STAGE == 2) xl = __ldg(y0 + base + cell - 1) + ha21 * __ldg(k1 + base + cell - 1);
+                    else xl = __ldg(ms + base + cell - 1);
+                }
+                if (!has_r) xr = mc[s][c].v[VEC - 1];
+                else if (lane == 31) {
+                    if constexpr (STAGE == 2) xr = __ldg(y0 + base + cell + VEC) + ha21 * __ldg(k1 + base + cell + VEC);
+                    else xr = __ldg(ms + base + cell + VEC);
+                }
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) {
+                    const T m0 = mc[s][c].v[v];
+                    const T left = (v == 0) ? xl : mc[s][c].v[v > 0 ? v - 1 : 0];
+                    const T right = (v == VEC - 1) ? xr : mc[s][c].v[v < VEC - 1 ? v + 1 : VEC - 1];
+                    T l = (left - m0) * wx;
+                    l += (right - m0) * wx;
+                    l += (nym.v[v] - m0) * wy;
+                    l += (nyp.v[v] - m0) * wy;
+                    l += (nzm.v[v] - m0) * wz;
+                    l += (nzp.v[v] - m0) * wz;
+                    lap[c][v] = l;
+                }
+            }
+
+            // ---- effective field and LLG slope ----
+            P ks[3];
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const T mx = mc[s][0].v[v], my = mc[s][1].v[v], mz = mc[s][2].v[v];
+                const T mk = mx * axx + my * axy + mz * axz;
+                T Bx = B0x + lap[0][v] + anp * mk * axx + brf[v];
+                T By = B0y + lap[1][v] + anp * mk * axy;
+                T Bz = B0z + lap[2][v] + anp * mk * axz;
+                if constexpr (NSUB == 2) {
+                    Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
+                }
+                const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
+                const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
+                ks[0].v[v] = llg * (tx + alpha * dx);
+                ks[1].v[v] = llg * (ty + alpha * dy);
+                ks[2].v[v] = llg * (tz + alpha * dz);
+            }
+
+            // ---- store k_s, then the fused tail: next stage state / candidate / error ----
+            if constexpr (STAGE >= 1 && STAGE <= 7) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    if (active) stp<T, VEC>(kout + (long long)(s * 3 + c) * nc + cell, ks[c]);
+            }
+            if constexpr (STAGE >= 2 && STAGE <= 5) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const long long off = (long long)(s * 3 + c) * nc + cell;
+                    P acc, m0v;
+                    if constexpr (STAGE == 2) {
+                        m0v = y0c[s][c];
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[2][0] * k1c[s][c].v[v];
+                    } else {
+                        m0v = ldp<T, VEC>(y0 + off);
+                        const P q1 = ldp<T, VEC>(k1 + off);
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[STAGE][0] * q1.v[v];
+#pragma unroll
+                        for (int j = 1; j < STAGE - 1; ++j) {
+                            const P qj = ldp<T, VEC>((const T*)A.K[j] + off);
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) acc.v[v] += (T)kA[STAGE][j] * qj.v[v];
+                        }
+                    }
+                    P out;
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) {
+                        acc.v[v] += (T)kA[STAGE][STAGE - 1] * ks[c].v[v];
+                        out.v[v] = m0v.v[v] + h * acc.v[v];
+                    }
+                    if (active) stp<T, VEC>(mnext + off, out);
+                }
+            }
+            if constexpr (STAGE == 6) {
+                P y5[3], er[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const long long off = (long long)(s * 3 + c) * nc + cell;
+                    const P m0v = ldp<T, VEC>(y0 + off);
+                    const P q1 = ldp<T, VEC>(k1 + off);
+                    const P q3 = ldp<T, VEC>((const T*)A.K[2] + off);
+                    const P q4 = ldp<T, VEC>((const T*)A.K[3] + off);
+                    const P q5 = ldp<T, VEC>((const T*)A.K[4] + off);
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) {
+                        T acc = (T)kA[6][0] * q1.v[v];
+                        acc += (T)kA[6][2] * q3.v[v];
+                        acc += (T)kA[6][3] * q4.v[v];
+                        acc += (T)kA[6][4] * q5.v[v];
+                        acc += (T)kA[6][5] * ks[c].v[v];
+                        y5[c].v[v] = m0v.v[v] + h * acc;
+                        T e = (T)kD[0] * q1.v[v];
+                        e += (T)kD[2] * q3.v[v];
+                        e += (T)kD[3] * q4.v[v];
+                        e += (T)kD[4] * q5.v[v];
+                        e += (T)kD[5] * ks[c].v[v];
+                        er[c].v[v] = h * e;
+                    }
+                }
+                if (A.renormalize) {
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) {
+                        const T inv = rsqrt_t<T>(y5[0].v[v] * y5[0].v[v] + y5[1].v[v] * y5[1].v[v] + y5[2].v[v] * y5[2].v[v]);
+                        y5[0].v[v] *= inv; y5[1].v[v] *= inv; y5[2].v[v] *= inv;
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const long long off = (long long)(s * 3 + c) * nc + cell;
+                    if (active) { stp<T, VEC>(mnext + off, y5[c]); stp<T, VEC>(e6 + off, er[c]); }
+                }
+            }
+            if constexpr (STAGE == 7) {
+                P er[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) er[c] = ldp<T, VEC>(e6 + (long long)(s * 3 + c) * nc + cell);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) {
+                    const T hd7 = h * (T)kD[6];
+                    const T ex = er[0].v[v] + hd7 * ks[0].v[v];
+                    const T ey = er[1].v[v] + hd7 * ks[1].v[v];
+                    const T ez = er[2].v[v] + hd7 * ks[2].v[v];
+                    T e2 = ex * ex + ey * ey + ez * ez;
+                    e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;     // NaN -> +inf so that max propagates it
+                    if (active) {
+                        emax2 = fmax(emax2, e2);
+                        sm[s * 3 + 0] += mc[s][0].v[v]; sm[s * 3 + 1] += mc[s][1].v[v]; sm[s * 3 + 2] += mc[s][2].v[v];
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- pass 1 of the reductions: warp shuffle tree, then fixed-order sum over the block's warps ----
+    constexpr int nwarp = kBlock / 32;
+    constexpr int NS = 2 * NB + (STAGE == 7 ? 3 * NSUB : 0);
+    __shared__ double swarp[nwarp][NS > 0 ? NS : 1];
+    __shared__ double swmax[nwarp];
+    __shared__ int s_last;
+    {
+        T vals[NS > 0 ? NS : 1];
+#pragma unroll
+        for (int n = 0; n < NB; ++n) { vals[2 * n] = ox[n]; vals[2 * n + 1] = oy[n]; }
+        if constexpr (STAGE == 7) {
+#pragma unroll
+            for (int i = 0; i < 3 * NSUB; ++i) vals[2 * NB + i] = sm[i];
+        }
+#pragma unroll
+        for (int i = 0; i < NS; ++i) {
+            const bool used = (i < 2 * NB) ? (i < 2 * N) : true;
+            if (used) {
+                T x = vals[i];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+                if (lane == 0) swarp[warp][i] = (double)x;
+            }
+        }
+        if constexpr (STAGE == 7) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) emax2 = fmax(emax2, __shfl_xor_sync(0xffffffffu, emax2, o));
+            if (lane == 0) swmax[warp] = (double)emax2;
+        }
+    }
+    __syncthreads();
+    if (tid < NS) {
+        const int i = tid;
+        const bool used = (i < 2 * NB) ? (i < 2 * N) : true;
+        if (used) {
+            double acc = 0.0;
+#pragma unroll
+            for (int w = 0; w < nwarp; ++w) acc += swarp[w][i];
+            const int comp = (i < 2 * NB) ? i : (2 * N + (i - 2 * NB));
+            A.partial[(size_t)comp * A.pstride + blockIdx.x] = acc;
+        }
+    }
+    if (STAGE == 7 && tid == 0) {
+        double mx = 0.0;
+#pragma unroll
+        for (int w = 0; w < nwarp; ++w) mx = fmax(mx, swmax[w]);
+        A.partial_max[blockIdx.x] = mx;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned int old = atomicAdd(&ctrl->arrive, 1u);
+        s_last = (old == gridDim.x - 1) ? 1 : 0;
+    }
+    __syncthreads();
+    if (s_last) stage_finish(A, STAGE, NSUB, trace);
+}
+
+// Kernel lookup, one translation unit per (T, NSUB): returns the device function for
+// cudaLaunchKernel / cudaGraphAddKernelNode.  vec: 1 = vectorised (16 B), 0 = scalar.
+const void* stage_kernel_f32_fm(int vec, int stage, int nb);
+const void* stage_kernel_f32_afm(int vec, int stage, int nb);
+const void* stage_kernel_f64_fm(int vec, int stage, int nb);
+const void* stage_kernel_f64_afm(int vec, int stage, int nb);
+
+#define CAVMAG_STAGE_CASES(T, VEC, NSUB, NB)                                       \
+    switch (stage) {                                                               \
+        case 1: return (const void*)k_stage<T, VEC, 1, NSUB, NB>;                  \
+        case 2: return (const void*)k_stage<T, VEC, 2, NSUB, NB>;                  \
+        case 3: return (const void*)k_stage<T, VEC, 3, NSUB, NB>;                  \
+        case 4: return (const void*)k_stage<T, VEC, 4, NSUB, NB>;                  \
+        case 5: return (const void*)k_stage<T, VEC, 5, NSUB, NB>;                  \
+        case 6: return (const void*)k_stage<T, VEC, 6, NSUB, NB>;                  \
+        case 7: return (const void*)k_stage<T, VEC, 7, NSUB, NB>;                  \
+        default: return nullptr;                                                   \
+    }
+
+#define CAVMAG_DEFINE_LOOKUP(NAME, T, VECW, NSUB)                                  \
+    const void* NAME(int vec, int stage, int nb) {                                 \
+        if (vec) {                                                                 \
+            if (nb == 0) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 0) }                  \
+            if (nb == 2) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 2) }                  \
+            if (nb == 8) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 8) }                  \
+            if (nb == 32) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 32) }                \
+        } else {                                                                   \
+            if (nb == 0) { CAVMAG_STAGE_CASES(T, 1, NSUB, 0) }                     \
+            if (nb == 2) { CAVMAG_STAGE_CASES(T, 1, NSUB, 2) }                     \
+            if (nb == 8) { CAVMAG_STAGE_CASES(T, 1, NSUB, 8) }                     \
+            if (nb == 32) { CAVMAG_STAGE_CASES(T, 1, NSUB, 32) }                   \
+        }                                                                          \
+        return nullptr;                                                            \
+    }
+
+}  // namespace cavmag

@@ -1,0 +1,413 @@
+"""GPU-vs-oracle parity (-m gpu): every test calls the CUDA path through the C ABI
+(paper_2603_03706_b200.api -> libcavmag.so) and compares it with the fp64 CPU oracle element by
+element on the same seeded inputs.
+
+Bars (BASELINE.json north_star, reading G23):
+  fixed step, fp64:  per component c: max_r |dm_c| <= 1e-10 * max_r |m_c^ref|;  |da_n| <= 1e-10 |a_n^ref|
+  fixed step, fp32:  |dm| <= 1e-4 absolute;  | |a_n| - |a_n^ref| | <= 1e-4 |a_n^ref|
+  adaptive:          observables (polariton frequencies within 1 MHz, Rabi period within 0.5 %)
+"""
+import math
+
+import numpy as np
+import pytest
+
+import cavmag_workloads as W
+from observables import fit_exponentials, dominant, rabi_period
+
+pytestmark = pytest.mark.gpu
+
+TWO_PI = 2 * math.pi
+GAMMA = 1.76e11
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2603_03706_b200 import api as a      # raises if libcavmag.so is missing: no fallback
+    return a
+
+
+def oracle_of(w, **kw):
+    from oracle import Oracle
+    return Oracle(w, **kw)
+
+
+def small_problem(nx, ny, nz, N, n_sub=1, seed=7, tilt=0.3, mixed=True, ku=2e3, dt_cells=(4e-9, 5e-9, 6e-9)):
+    u = W.random_smooth_profiles(seed, max(N, 1), nx, ny, nz)[:N]
+    if N:
+        u[0] = 1.0       # one uniform mode so that the overlap of m ~ z^ + tilt is not tiny
+    m0 = np.stack([W.tilted_state(seed, 1 + 2 * s, nx, ny, nz, tilt, sign=(1.0 if s == 0 else -1.0)) for s in range(n_sub)])
+    f = np.linspace(9.0, 11.0, N) if N else np.zeros(0)
+    g = 20.0 + 30.0 * W.uniform01(seed, 50, N)
+    Gam = np.where(np.arange(N) % 2 == 1, 0.5 * g, 0.0) if mixed else np.zeros(N)
+    Phi = np.where(np.arange(N) % 2 == 1, 1.1, 0.0) if mixed else np.zeros(N)
+    md = W._modes(f, g, 5.0, Gam, Phi) if N else dict(omega=np.zeros(0), kappa=np.zeros(0), g=np.zeros(0), Gamma=np.zeros(0), Phi=np.zeros(0))
+    a0 = (0.02 * (W.uniform01(seed, 60, N) - 0.5) + 0.02j * (W.uniform01(seed, 61, N) - 0.5)).astype(np.complex128)
+    return W.Workload(name="small", nx=nx, ny=ny, nz=nz, dx=dt_cells[0], dy=dt_cells[1], dz=dt_cells[2], Ms=140e3,
+                      Aex=3.7e-12, Ku=ku, ku_axis=(1.0, 0.5, 0.2), alpha=0.02, gamma=GAMMA, B0=(0.01, -0.02, 0.35),
+                      n_sub=n_sub, B_exch_inter=(3.0 if n_sub == 2 else 0.0), u=u, m0=m0, a0=a0,
+                      t_end=0, tol=0, fixed_dt=0, precision="f64", **md)
+
+
+def assert_parity(m, a, ref, prec):
+    if prec == "f64":
+        for s in range(ref.m.shape[0]):
+            for c in range(3):
+                scale = np.abs(ref.m[s, c]).max()
+                assert np.abs(m[s, c] - ref.m[s, c]).max() <= 1e-10 * scale, (s, c)
+        for n in range(ref.a.shape[0]):
+            assert abs(a[n] - ref.a[n]) <= 1e-10 * abs(ref.a[n]), n
+    else:
+        assert np.abs(m.astype(np.float64) - ref.m).max() <= 1e-4
+        for n in range(ref.a.shape[0]):
+            assert abs(abs(a[n]) - abs(ref.a[n])) <= 1e-4 * abs(ref.a[n]), n
+
+
+# ----------------------------------------------------------------------------------------
+# right-hand side, cell by cell
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,N,n_sub", [
+    ((8, 8, 8), 1, 1),        # cfg1 shape
+    ((40, 9, 7), 3, 1),       # several blocks + ragged tail, N between buckets
+    ((13, 5, 3), 2, 1),       # nx not a multiple of the vector width -> scalar kernels
+    ((12, 6, 5), 8, 1),       # rows shorter than a warp
+    ((36, 10, 5), 9, 1),      # N = 9 -> 32-mode bucket
+    ((64, 4, 3), 32, 1),      # max modes
+    ((24, 6, 4), 0, 1),       # plain LLG
+    ((20, 7, 6), 1, 2),       # antiferromagnet
+    ((1, 1, 1), 1, 1),        # degenerate: a single cell
+    ((2, 1, 9), 2, 2),        # thin in x,y
+])
+def test_rhs_matches_oracle(api, prec, shape, N, n_sub):
+    w = small_problem(*shape, N, n_sub)
+    dm_ref, da_ref, S_ref = oracle_of(w).rhs(w.m0, w.a0)
+    with api.Sim(w, precision=prec) as sim:
+        dm = np.empty(sim.shape_m, dtype=sim.np_dtype)
+        api.cav_get_dmdt(sim.h, dm)
+        da = api.cav_get_dadt(sim.h, N)
+        S = api.cav_get_overlaps(sim.h, N)
+    scale = np.abs(dm_ref).max()
+    if prec == "f64":
+        assert np.abs(dm - dm_ref).max() <= 2e-13 * scale
+        if N:
+            assert np.abs(S - S_ref).max() <= 1e-14
+            assert np.abs(da - da_ref).max() <= 1e-13 * max(np.abs(da_ref).max(), 1.0)
+    else:
+        # fp32 inputs are rounded on upload: compare against the oracle evaluated on the same rounded inputs
+        w32 = small_problem(*shape, N, n_sub)
+        w32.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w32.m0 /= np.linalg.norm(w32.m0, axis=1, keepdims=True)
+        w32.u = w.u.astype(np.float32).astype(np.float64)
+        dm_ref, da_ref, S_ref = oracle_of(w32).rhs(w32.m0, w32.a0)
+        assert np.abs(dm - dm_ref).max() <= 2e-5 * scale
+        if N:
+            assert np.abs(S - S_ref).max() <= 2e-6
+            assert np.abs(da - da_ref).max() <= 2e-5 * max(np.abs(da_ref).max(), 1.0)
+
+
+# ----------------------------------------------------------------------------------------
+# fixed-step parity after 1000 steps (north_star)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("variant", ["a", "b"])
+def test_cfg1_fixed_1000_steps(api, prec, variant):
+    w = W.cfg1(variant)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=w.fixed_dt, max_steps=1000)
+    with api.Sim(w, precision=prec) as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=w.fixed_dt, max_steps=1000)
+        m, a = sim.get_m(), sim.get_a()
+        st = api.cav_get_stats(sim.h)
+    assert st["accepted"] == 1000 and st["rejected"] == 0 and st["rhs_evals"] == 6001
+    assert abs(st["t"] - ref.t) <= 1e-24
+    assert_parity(m, a, ref, prec)
+    if variant == "a" and prec == "f64":
+        assert np.abs(m - m[:, :, :1, :1, :1]).max() < 1e-13      # stays uniform
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,N,n_sub,dt", [
+    ((40, 9, 7), 3, 1, 0.1e-12),
+    ((13, 5, 3), 2, 1, 0.1e-12),
+    ((36, 10, 5), 9, 1, 0.1e-12),
+    ((20, 7, 6), 1, 2, 0.05e-12),
+    ((16, 8, 4), 2, 2, 0.05e-12),
+])
+def test_busy_fixed_steps(api, prec, shape, N, n_sub, dt):
+    """All terms on (off-axis field and anisotropy, profiled modes, mixed coupling, damping, AFM)."""
+    w = small_problem(*shape, N, n_sub, tilt=0.2)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=300)
+    with api.Sim(w, precision=prec) as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=300)
+        m, a = sim.get_m(), sim.get_a()
+    assert_parity(m, a, ref, prec)
+
+
+def test_cfg2_fixed_f64_and_f32(api):
+    w = W.cfg2(nx=64, ny=64, nz=16)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.2e-12, max_steps=200)
+    for prec in ("f64", "f32"):
+        with api.Sim(w, precision=prec) as sim:
+            api.cav_run_steps(sim.h, math.inf, fixed_dt=0.2e-12, max_steps=200)
+            m, a = sim.get_m(), sim.get_a()
+        if prec == "f64":
+            assert_parity(m, a, ref, prec)
+        else:
+            assert np.abs(m - ref.m).max() <= 1e-4
+            # a_n starts from zero and is still ~1e-6 here: compare on the scale of the driving overlap
+            assert np.abs(a - ref.a).max() <= 1e-4 * np.abs(ref.a).max()
+
+
+def test_cfg4_afm_dissipative_fixed(api):
+    w = W.cfg4(nx=32, ny=16, nz=8, dissipative=True)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.02e-12, max_steps=400)
+    for prec in ("f64", "f32"):
+        with api.Sim(w, precision=prec) as sim:
+            api.cav_run_steps(sim.h, math.inf, fixed_dt=0.02e-12, max_steps=400)
+            m, a = sim.get_m(), sim.get_a()
+        if prec == "f64":
+            assert_parity(m, a, ref, prec)
+        else:
+            assert np.abs(m - ref.m).max() <= 1e-4
+            assert np.abs(a - ref.a).max() <= 1e-4 * np.abs(ref.a).max()
+
+
+# ----------------------------------------------------------------------------------------
+# full-size workloads, in the launch configuration bench.py times
+# ----------------------------------------------------------------------------------------
+def test_cfg3_full_size_steps(api):
+    """256x256x32, 8 modes, fp32: three fixed steps element by element against the oracle."""
+    w = W.cfg3()
+    w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+    w.u = w.u.astype(np.float32).astype(np.float64)
+    # give the modes something to do from step 1
+    w.a0 = (1e-3 * (1 + np.arange(8))).astype(np.complex128)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=3)
+    with api.Sim(w, precision="f32") as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=3)
+        m, a = sim.get_m(), sim.get_a()
+        S = api.cav_get_overlaps(sim.h, 8)
+    assert np.abs(m - ref.m).max() <= 2e-6
+    assert np.abs(a - ref.a).max() <= 1e-6 * np.abs(ref.a).max()
+    # invariants that hold at any size
+    assert np.abs(np.linalg.norm(m.astype(np.float64), axis=1) - 1).max() < 3e-7
+    mc = ref.m[0]
+    S_direct = np.array([(w.u[n] * (mc[0] - 1j * mc[1])).mean() for n in range(8)])
+    assert np.abs(S - S_direct).max() < 1e-7
+
+
+def test_cfg5_slab_32_modes(api):
+    """cfg5's 512x512 plane and 32 mixed-coupling modes on a thinner slab (oracle memory/time bound)."""
+    w = W.cfg5(nz=4, dtype=np.float64)
+    w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+    w.u = w.u.astype(np.float32).astype(np.float64)
+    w.a0 = (1e-3 * (1 + np.arange(32)) * np.exp(0.3j * np.arange(32))).astype(np.complex128)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=2)
+    with api.Sim(w, precision="f32") as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=2)
+        m, a = sim.get_m(), sim.get_a()
+    assert np.abs(m - ref.m).max() <= 2e-6
+    assert np.abs(a - ref.a).max() <= 1e-6 * np.abs(ref.a).max()
+
+
+# ----------------------------------------------------------------------------------------
+# adaptive mode: observables
+# ----------------------------------------------------------------------------------------
+def _run_trace(api, w, prec, t_end, sample_dt, tol):
+    cap = int(round(t_end / sample_dt))
+    with api.Sim(w, precision=prec) as sim:
+        api.cav_set_trace(sim.h, sample_dt, cap)
+        api.cav_run(sim.h, t_end, tol=tol)
+        tr = api.cav_get_trace(sim.h)
+        st = api.cav_get_stats(sim.h)
+    assert tr.shape[0] == cap
+    return tr, st
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_adaptive_rabi_period(api, prec):
+    """g/2pi = 50 MHz at resonance, a(0) = 0.01: T_R = pi/g = 10 ns within 0.5 %."""
+    w = W.macrospin(5.0, [5.0], 50.0, 0.0, alpha=0.0, a0=[0.01], n=4)
+    tol = 1e-8 if prec == "f64" else 1e-6
+    tr, st = _run_trace(api, w, prec, 26e-9, 25e-12, tol)
+    ref = oracle_of(w).run(w.m0, w.a0, t_end=26e-9, tol=tol, sample_dt=25e-12, trace_cap=1040)
+    T_gpu = rabi_period(tr[:, 0], tr[:, 1] ** 2 + tr[:, 2] ** 2)
+    T_ref = rabi_period(ref.trace[:, 0], ref.trace[:, 1] ** 2 + ref.trace[:, 2] ** 2)
+    assert abs(T_gpu / T_ref - 1) < 5e-3
+    assert abs(T_gpu / 10e-9 - 1) < 5e-3
+    assert np.allclose(tr[:, 0], ref.trace[:, 0], rtol=0, atol=1e-22)
+    assert st["accepted"] > 0 and st["rhs_evals"] == 1 + 6 * (st["accepted"] + st["rejected"])
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_adaptive_anticrossing_frequencies(api, prec):
+    """Polariton branches of cfg1's tiny ferromagnet (per-cell tilt, exchange on) with g/2pi = 50 MHz:
+    peak frequencies of GPU and oracle within 1 MHz, and both on Eq. 6."""
+    w = W.cfg1("b")
+    w.omega = np.array([TWO_PI * 10e9]); w.g = np.array([TWO_PI * 50e6]); w.kappa = np.array([TWO_PI * 1e6])
+    w.a0 = np.array([1e-3 + 0j])
+    w.B0 = (0.0, 0.0, W.b0_for_ghz(10.03))
+    tol = 1e-8 if prec == "f64" else 1e-6
+    t_end, sdt = 40e-9, 20e-12
+    tr, _ = _run_trace(api, w, prec, t_end, sdt, tol)
+    ref = oracle_of(w).run(w.m0, w.a0, t_end=t_end, tol=tol, sample_dt=sdt, trace_cap=2000)
+    out = []
+    for t in (tr, ref.trace):
+        om, amp = fit_exponentials(t[:, 1] + 1j * t[:, 2], sdt, 4)
+        out.append(dominant(om, amp, 2)[0].real / TWO_PI)
+    assert np.abs(out[0] - out[1]).max() < 1e6
+    wc, wm, g = TWO_PI * 10e9, GAMMA * w.B0[2], TWO_PI * 50e6
+    eq6 = ((wc + wm) / 2 + np.array([-1, 1]) * math.sqrt(g * g + ((wc - wm) / 2) ** 2)) / TWO_PI
+    assert np.abs(out[0] - eq6).max() < 1e6
+
+
+def test_adaptive_afm_neel_line(api):
+    """cfg4-like AFM: the Neel-vector line of GPU (fp32 and fp64) and oracle agree within 1e-5 relative."""
+    w = W.cfg4(nx=8, ny=4, nz=4)
+    t_end, sdt = 0.1e-9, 0.5e-12
+    ref = oracle_of(w).run(w.m0, w.a0, t_end=t_end, tol=1e-7, sample_dt=sdt, trace_cap=200)
+
+    def neel_freq(t):
+        c = 1 + 4
+        n = 0.5 * ((t[:, c] - t[:, c + 3]) - 1j * (t[:, c + 1] - t[:, c + 4]))
+        om, amp = fit_exponentials(n, sdt, 4)
+        return np.sort(np.abs(dominant(om, amp, 2)[0].real))
+    f_ref = neel_freq(ref.trace)
+    for prec in ("f64", "f32"):
+        tr, _ = _run_trace(api, w, prec, t_end, sdt, 1e-7 if prec == "f64" else 1e-6)
+        assert np.abs(neel_freq(tr) / f_ref - 1).max() < 1e-4
+
+
+# ----------------------------------------------------------------------------------------
+# launch modes, determinism, edge cases
+# ----------------------------------------------------------------------------------------
+def test_graph_and_stream_modes_bitwise_identical_and_deterministic(api):
+    w = small_problem(40, 9, 7, 3, 1)
+    outs = []
+    for mode in (api.CAV_LAUNCH_GRAPH, api.CAV_LAUNCH_STREAM, api.CAV_LAUNCH_GRAPH):
+        with api.Sim(w, precision="f32") as sim:
+            api.cav_set_launch_mode(sim.h, mode)
+            api.cav_run(sim.h, 5e-12, tol=1e-6)
+            outs.append((sim.get_m(), sim.get_a(), api.cav_get_stats(sim.h)))
+    for m, a, st in outs[1:]:
+        assert np.array_equal(m, outs[0][0]) and np.array_equal(a, outs[0][1])
+        assert st["accepted"] == outs[0][2]["accepted"] and st["rejected"] == outs[0][2]["rejected"]
+
+
+def test_block_size_and_sweep_order_do_not_change_fp64_results_beyond_rounding(api):
+    w = small_problem(40, 9, 7, 3, 1)
+    res = []
+    for cells, serp in ((0, 1), (512, 0), (2048, 1)):
+        with api.Sim(w, precision="f64") as sim:
+            api.cav_set_block_cells(sim.h, cells)
+            api.cav_set_sweep_order(sim.h, serp)
+            api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=50)
+            res.append((sim.get_m(), sim.get_a()))
+    for m, a in res[1:]:
+        assert np.abs(m - res[0][0]).max() < 1e-13 and np.abs(a - res[0][1]).max() < 1e-15
+    # the sweep order only permutes which block handles which cells: m is bitwise unchanged
+    assert np.array_equal(res[0][0], res[2][0]) or np.abs(res[0][0] - res[2][0]).max() < 1e-13
+
+
+def test_resume_equals_single_run(api):
+    """Stopping and continuing (FSAL slope kept on the device) gives the same trajectory."""
+    w = small_problem(24, 6, 4, 2, 1)
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=40)
+        m1, a1 = sim.get_m(), sim.get_a()
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=15)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=25)
+        m2, a2 = sim.get_m(), sim.get_a()
+        st = api.cav_get_stats(sim.h)
+    assert np.array_equal(m1, m2) and np.array_equal(a1, a2)
+    assert st["rhs_evals"] == 1 + 6 * 40
+
+
+def test_edge_cases(api):
+    w = small_problem(8, 4, 2, 1, 1)
+    with api.Sim(w, precision="f64") as sim:
+        # t_end <= t: nothing happens
+        api.cav_run(sim.h, 0.0, tol=1e-6)
+        assert api.cav_get_stats(sim.h)["accepted"] == 0
+        # argument validation
+        for bad in (dict(tol=0.0, fixed_dt=0.0), dict(tol=1e-6, fixed_dt=1e-13)):
+            with pytest.raises(api.CavError) as e:
+                api.cav_run(sim.h, 1e-12, **bad)
+            assert e.value.status == api.CAV_E_ARG
+        with pytest.raises(api.CavError):
+            api.cav_run(sim.h, math.inf, tol=1e-6)
+        # set_m normalises
+        api.cav_set_m(sim.h, np.ascontiguousarray(3.0 * w.m0))
+        assert np.abs(np.linalg.norm(sim.get_m(), axis=1) - 1).max() < 1e-15
+        # exact landing on t_end and on every trace sample
+        api.cav_set_trace(sim.h, 1e-12, 5)
+        api.cav_run(sim.h, 5e-12, tol=1e-7)
+        t, _ = api.cav_get_time(sim.h)
+        tr = api.cav_get_trace(sim.h)
+        assert t == 5e-12 and tr.shape == (5, 1 + 4 + 3)
+        assert np.allclose(tr[:, 0], 1e-12 * np.arange(1, 6), rtol=0, atol=1e-26)
+        a = sim.get_a()
+        assert tr[-1, 1] == a[0].real and tr[-1, 2] == a[0].imag
+        mavg = sim.get_m().reshape(3, -1).mean(axis=1)
+        assert np.abs(tr[-1, 5:8] - mavg).max() < 1e-14
+    # a far too large fixed step blows up: reported, not hidden
+    with api.Sim(w, precision="f32") as sim:
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=1e-9, max_steps=200)
+        with pytest.raises(api.CavError) as e:
+            api.cav_sync(sim.h)
+        assert e.value.status == api.CAV_E_NONFINITE
+
+
+def test_overlap_norm_sum_u_and_singular(api):
+    w = small_problem(16, 4, 4, 2, 1)
+    w.u = w.u + 0.5
+    ref = oracle_of(w, norm_sum_u=True)
+    _, _, S_ref = ref.rhs(w.m0, w.a0)
+    with api.Sim(w, precision="f64", overlap_norm=api.CAV_NORM_SUM_U) as sim:
+        dm = np.empty(sim.shape_m)
+        api.cav_get_dmdt(sim.h, dm)
+        S = api.cav_get_overlaps(sim.h, 2)
+    assert np.abs(S - S_ref).max() < 1e-14
+    w2 = W.cfg2(nx=16, ny=4, nz=2)      # sin(2 pi x/L) sums to zero
+    with pytest.raises(api.CavError) as e:
+        api.Sim(w2, precision="f64", overlap_norm=api.CAV_NORM_SUM_U)
+    assert e.value.status == api.CAV_E_SINGULAR_NORM
+
+
+def test_device_buffers_via_torch(api):
+    """PyTorch only provides device memory and the stream: tensors cross the ABI as raw pointers."""
+    import torch
+    w = small_problem(24, 6, 4, 2, 1)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        m_dev = torch.tensor(w.m0, dtype=torch.float64, device="cuda")
+        u_dev = torch.tensor(w.u, dtype=torch.float64, device="cuda")
+    stream.synchronize()
+    h = api.cav_create((w.nx, w.ny, w.nz, w.dx, w.dy, w.dz),
+                       dict(Ms=w.Ms, Aex=w.Aex, Ku=w.Ku, ku_axis=w.ku_axis, alpha=w.alpha, gamma=w.gamma, B0=w.B0,
+                            precision=api.CAV_F64))
+    try:
+        api.cav_set_stream(h, stream.cuda_stream)
+        api.cav_set_modes(h, u_dev, w.omega, w.kappa, w.g, w.Gamma, w.Phi)
+        api.cav_set_m(h, m_dev)
+        api.cav_set_a(h, w.a0)
+        api.cav_run_steps(h, math.inf, fixed_dt=0.1e-12, max_steps=20)
+        out = torch.empty_like(m_dev)
+        api.cav_get_m(h, out)
+        a = api.cav_get_a(h, 2)
+    finally:
+        api.cav_destroy(h)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=20)
+    assert np.abs(out.cpu().numpy() - ref.m).max() < 1e-12
+    assert np.abs(a - ref.a).max() < 1e-13
