@@ -1,0 +1,388 @@
+"""bench.py — throughput of the fused LLG + cavity-mode RK45 step (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg5|cfg4|cfg4_f64|cfg2]
+    python bench.py --impl reference ...          # the fp64 CPU oracle on the host cores
+
+A "step" is one Dormand-Prince RK45 step of the whole coupled system: six fused stage kernels
+(field + LLG slope + overlap partials + stage combination + mode ODEs + controller), accepted or
+rejected.  The metric is cell-stage updates/s = N_cells x right-hand-side evaluations / second
+(SURVEY.md section 8(d)); simulated ns per wall-second is reported beside it.
+
+Default workload: cfg3 = BASELINE.json configs[2] (256x256x32 cells, 8 cavity modes, fp32, adaptive
+tol 1e-6) — the configuration the north_star's roofline target is quoted on ("2M+-cell grid with
+8 cavity modes").  Inputs are synthetic and seeded (cavmag_workloads); the per-step working set
+(11 cell fields + 8 profiles = 344 MB) is larger than the 126 MB L2.
+
+Timing: CUDA events recorded on the stream the library launches on (a torch stream handed over
+with cav_set_stream), barrier + synchronize on both sides, max over ranks.  The K timed steps are
+ONE cav_run_steps call = one CUDA-graph launch whose WHILE node loops on the device.
+N > 1: independent replicas (different seeds) per GPU, no data-path collective ("replicas only",
+DESIGN.md) -> weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "cell-stage updates/s"
+UNIT = "cell-stage/s"
+
+# dram__bytes_read.sum + dram__bytes_write.sum per stage-kernel launch (mean over the six stages of
+# one step) from the `ncu --set full` capture summarised in profiles/ (file named beside each value).
+NCU_TRAFFIC_BYTES = {
+}
+
+
+def make_workload(name: str, rank: int = 0):
+    import cavmag_workloads as W
+    seed_shift = 17 * rank
+    if name == "cfg3":
+        return W.cfg3(seed=3000 + seed_shift, dtype=np.float32), "f32"
+    if name == "cfg5":
+        return W.cfg5(seed=5000 + seed_shift, dtype=np.float32), "f32"
+    if name == "cfg4":
+        return W.cfg4(seed=4000 + seed_shift), "f32"
+    if name == "cfg4_f64":
+        return W.cfg4(seed=4000 + seed_shift), "f64"
+    if name == "cfg4d":
+        return W.cfg4(seed=4000 + seed_shift, dissipative=True), "f32"
+    if name == "cfg2":
+        return W.cfg2(seed=2000 + seed_shift), "f32"
+    if name == "cfg2_f64":
+        return W.cfg2(seed=2000 + seed_shift), "f64"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def algorithmic_bytes_per_cell_step(n_modes: int, n_sub: int, esize: int) -> int:
+    """(111 + 6N) elements per cell per RK45 step, (222 + 6N) for two sublattices (SURVEY.md 8(d),
+    DESIGN.md 'Algorithmic bytes'): 75 n_sub + 6N reads, 36 n_sub writes."""
+    return (111 * n_sub + 6 * n_modes) * esize
+
+
+def config_of(w, prec, name):
+    return {"workload": name, "grid": [w.nx, w.ny, w.nz], "cells": w.n_cells, "n_sub": w.n_sub,
+            "modes": w.n_modes, "cell_nm": w.dx * 1e9, "mode": "adaptive RK45 (Dormand-Prince 5(4))",
+            "tol": w.tol, "precision": prec,
+            "l2": "working set per step (11 cell fields + mode profiles) exceeds the 126 MB L2"
+                  if (11 * 3 * w.n_sub + w.n_modes) * w.n_cells * (4 if prec == "f32" else 8) > 126e6
+                  else "working set fits in L2 (latency-bound small case; no roofline claim)"}
+
+
+# ----------------------------------------------------------------------------------------
+# clocks during the timed region
+# ----------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML every 10 ms in a thread
+    (nvidia-smi subprocess as a fallback)."""
+    _REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+                0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nvml = None
+
+    def _once(self):
+        if self._nvml is not None:
+            p = self._nvml
+            self.samples.append(p.nvmlDeviceGetClockInfo(self._h, p.NVML_CLOCK_SM))
+            mask = p.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+            for bit, nm in self._REASONS.items():
+                if mask & bit and nm != "gpu_idle":
+                    self.reasons.add(nm)
+        else:
+            out = subprocess.run(["nvidia-smi", f"--id={self.index}", "--query-gpu=clocks.sm,clocks.max.sm,"
+                                  "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                                  "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap",
+                                  "--format=csv,noheader,nounits"], capture_output=True, text=True).stdout.strip()
+            f = [x.strip() for x in out.split(",")]
+            if len(f) >= 6:
+                self.samples.append(int(f[0])); self.max_mhz = int(f[1])
+                for nm, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(nm)
+
+    def _loop(self):
+        while not self._stop.is_set():
+            try:
+                self._once()
+            except Exception:
+                pass
+            self._stop.wait(0.01)
+
+    def start(self):
+        self._thr = threading.Thread(target=self._loop, daemon=True)
+        self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        if not self.samples:
+            try:
+                self._once()
+            except Exception:
+                pass
+        return {"sm_mhz": (statistics.median(self.samples) if self.samples else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------
+# the fp64 CPU oracle, timed as it stands (cpu_baseline leg and --impl reference)
+# ----------------------------------------------------------------------------------------
+def slab_workload(name: str, nz: int):
+    """The workload's recipe on a thinner z-slab of the same x-y plane (bounded CPU sample)."""
+    import cavmag_workloads as W
+    base = name.split("_")[0]
+    kw = dict(nz=nz)
+    if base in ("cfg3", "cfg5"):
+        kw["dtype"] = np.float64
+    return W.by_name(base, **kw)
+
+
+def time_oracle(w, steps: int, warmup: int, tol: float):
+    """Runs warmup + steps adaptive RK45 steps of the oracle; returns (seconds, rhs_evals, sim_time) of the
+    timed part."""
+    from oracle import Oracle
+    orc = Oracle(w)
+    m, a, t, dt = w.m0, w.a0, 0.0, 0.0
+    if warmup > 0:
+        r = orc.run(m, a, t0=t, tol=tol, dt_init=dt, max_steps=warmup)
+        m, a, t, dt = r.m, r.a, r.t, r.dt
+    t0 = time.perf_counter()
+    r = orc.run(m, a, t0=t, tol=tol, dt_init=dt, max_steps=steps)
+    sec = time.perf_counter() - t0
+    return sec, r.rhs_evals, r.t - t
+
+
+def cpu_baseline(name: str, w_full, budget_s: float = 15.0):
+    """Bounded sample: the oracle on a z-slab of the same workload, sized from a one-step calibration so
+    that the timed part takes about budget_s seconds."""
+    import oracle
+    cores = oracle.get_threads()
+    nz_cal = min(2, w_full.nz)
+    wc = slab_workload(name, nz_cal)
+    sec, evals, _ = time_oracle(wc, 1, 0, w_full.tol)
+    per_cs = sec / (evals * wc.n_cells)                       # seconds per cell-stage
+    steps = 3
+    plane = w_full.nx * w_full.ny
+    nz = int(max(1, min(w_full.nz, budget_s / (per_cs * plane * (6 * steps + 1)))))
+    ws = slab_workload(name, nz)
+    sec, evals, simt = time_oracle(ws, steps, 0, w_full.tol)
+    return {"value": ws.n_cells * evals / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{name} recipe on a {ws.nx}x{ws.ny}x{ws.nz} slab ({ws.n_cells} cells, {ws.n_modes} modes), "
+                      f"{steps} adaptive RK45 steps ({evals} RHS evaluations), fp64, {sec:.1f} s",
+            "ms_per_step": 1e3 * sec / steps}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    name = args.workload
+    w_full, prec = make_workload(name)
+    cores = oracle.get_threads()
+    # calibrate on a 2-plane slab, then size the slab so that warmup+steps take about 2 minutes
+    wc = slab_workload(name, min(2, w_full.nz))
+    sec, evals, _ = time_oracle(wc, 1, 0, w_full.tol)
+    per_cs = sec / (evals * wc.n_cells)
+    total_steps = args.steps + args.warmup
+    plane = w_full.nx * w_full.ny
+    nz = int(max(1, min(w_full.nz, 120.0 / (per_cs * plane * (6 * total_steps + 2)))))
+    ws = slab_workload(name, nz)
+    sec, evals, simt = time_oracle(ws, args.steps, args.warmup, w_full.tol)
+    value = ws.n_cells * evals / sec
+    sample = (f"{name} recipe on a {ws.nx}x{ws.ny}x{ws.nz} slab ({ws.n_cells} cells, {ws.n_modes} modes) per step; "
+              f"{args.steps} timed adaptive RK45 steps after {args.warmup} warm-up steps, fp64")
+    cfg = config_of(w_full, prec, name)
+    cfg["reference_sample"] = sample
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": cfg, "sim_ns_per_s": simt * 1e9 / sec,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------
+# the CUDA path
+# ----------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2603_03706_b200 import api          # raises if libcavmag.so is missing: no CPU fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    name = args.workload
+    w, prec = make_workload(name, rank)
+    esize = 4 if prec == "f32" else 8
+    np_dtype = np.float32 if prec == "f32" else np.float64
+    tol = w.tol
+    stream = torch.cuda.Stream()
+    sim = api.Sim(w, precision=prec, stream=stream.cuda_stream)
+    h = sim.h
+    N, nc = w.n_modes, w.n_cells
+
+    # spin-up (setup, untimed): the controller grows dt from 1e-14 s to the stability-limited step
+    if args.launch_mode == "stream":                  # profiling aid: host-enqueued stage kernels, same kernels
+        api.cav_set_launch_mode(h, api.CAV_LAUNCH_STREAM)
+    api.cav_run_steps(h, math.inf, tol=tol, max_steps=args.spinup)
+    # warm-up: W steps through the very same graph launch that is timed below
+    api.cav_run_steps(h, math.inf, tol=tol, max_steps=max(args.warmup, 1))
+    api.cav_sync(h)
+    st0 = api.cav_get_stats(h)
+    n0 = api.cav_get_launch_count(h)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(torch.cuda.current_device() if os.environ.get("CUDA_VISIBLE_DEVICES") is None else local)
+    barrier()
+    sampler.start()
+    ev0.record(stream)
+    api.cav_run_steps(h, math.inf, tol=tol, max_steps=args.steps)
+    ev1.record(stream)
+    stream.synchronize()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    api.cav_sync(h)                                   # raises on a device-side error status
+    st1 = api.cav_get_stats(h)
+    n1 = api.cav_get_launch_count(h)
+    evals = st1["rhs_evals"] - st0["rhs_evals"]
+    steps_done = (st1["accepted"] + st1["rejected"]) - (st0["accepted"] + st0["rejected"])
+    assert steps_done == args.steps and evals == 6 * args.steps, (steps_done, evals)
+    sim_t = st1["t"] - st0["t"]
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region, every step ----
+    k_e2e = min(args.steps, args.e2e_steps)
+    m_host = torch.empty(sim.shape_m, dtype=torch.float32 if prec == "f32" else torch.float64).pin_memory()
+    api.cav_get_m(h, m_host)
+    a_host = api.cav_get_a(h, N)
+    for _ in range(3):                                # warm-up of the host-buffer path
+        api.cav_set_m(h, m_host); api.cav_set_a(h, a_host)
+        api.cav_run_steps(h, math.inf, tol=tol, max_steps=1)
+        api.cav_get_m(h, m_host); a_host = api.cav_get_a(h, N)
+    se0 = api.cav_get_stats(h)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(k_e2e):
+        api.cav_set_m(h, m_host)                      # H2D from pinned host memory
+        api.cav_set_a(h, a_host)
+        api.cav_run_steps(h, math.inf, tol=tol, max_steps=1)
+        api.cav_get_m(h, m_host)                      # D2H of the step's result (synchronises)
+        a_host = api.cav_get_a(h, N)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    barrier()
+    se1 = api.cav_get_stats(h)
+    e2e_evals = se1["rhs_evals"] - se0["rhs_evals"]
+    io_bytes = int(np.prod(sim.shape_m)) * esize + 16 * N
+
+    # ---- max over ranks, sum of units ----
+    vals = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+    units = torch.tensor([float(nc * evals), float(nc * e2e_evals), sim_t], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+        dist.all_reduce(units, op=dist.ReduceOp.SUM)
+    ms_max, e2e_max = float(vals[0]), float(vals[1])
+    value = float(units[0]) / (ms_max * 1e-3)
+    e2e_value = float(units[1]) / e2e_max
+
+    if rank == 0:
+        launches = 6 * args.steps
+        launch_us = ms * 1e3 / launches                       # this rank's mean stage-kernel duration
+        bytes_per_launch = algorithmic_bytes_per_cell_step(N, w.n_sub, esize) * nc / 6.0
+        achieved = bytes_per_launch / (launch_us * 1e-6) / 1e9
+        peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(peaks_path):
+            peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        else:
+            peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+        traffic = NCU_TRAFFIC_BYTES.get(name)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
+            "config": dict(config_of(w, prec, name), parallelism=f"replicas x{world} (no collective)",
+                           launch_mode=args.launch_mode),
+            "sim_ns_per_s": float(units[2]) * 1e9 / (ms_max * 1e-3) / world,
+            "mean_dt_ps": sim_t * 1e12 / max(st1["accepted"] - st0["accepted"], 1),
+            "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
+                    "steps": k_e2e, "ms_per_step": 1e3 * e2e_max / k_e2e,
+                    "note": "every step: cav_set_m/cav_set_a from pinned host memory, cav_run_steps(1), cav_get_m/cav_get_a "
+                            "to host; FSAL is lost at each upload (7 RHS evaluations per step)"},
+            "gpu_launches": int(n1 - n0),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic, "peak_source": peak_src, "kernel": "cavmag::k_stage (fused RK45 stage)",
+                         "launch_us": launch_us, "algorithmic_bytes_per_launch": bytes_per_launch,
+                         "frac_of_nominal_8TBs": achieved / 8000.0},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(name, w)
+        print(json.dumps(line), flush=True)
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--e2e-steps", type=int, default=300)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--spinup", type=int, default=40, help="untimed setup steps that let dt settle")
+    ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()
