@@ -58,6 +58,7 @@ typedef enum {
 enum { CAV_F32 = 0, CAV_F64 = 1 };
 enum { CAV_NORM_NCELLS = 0, CAV_NORM_SUM_U = 1 };
 enum { CAV_LAUNCH_GRAPH = 0, CAV_LAUNCH_STREAM = 1 };
+enum { CAV_PATH_AUTO = 0, CAV_PATH_GENERIC = 1, CAV_PATH_TMA = 2 };
 #define CAV_MAX_MODES 32
 
 /* Finite-difference grid: nx*ny*nz cells of size dx*dy*dz (metres). */
@@ -161,6 +162,15 @@ int cav_set_block_cells(cav_sim* sim, int cells_per_block);
 /* Tuning knob (optional): 1 (default) = odd stages sweep the grid in reverse block order so that
  * the tail of one stage's data is still in L2 when the next stage starts; 0 = always forward. */
 int cav_set_sweep_order(cav_sim* sim, int serpentine);
+
+/* Which implementation of the fused stage kernel runs (same arithmetic, PAPER.md:150-159 / DESIGN.md "Kernels"):
+ *   CAV_PATH_TMA      persistent TMA/mbarrier-pipelined kernel; needs nx*sizeof(T) % 16 == 0 and a mode count whose
+ *                     streams fit the shared-memory rings, else cav_set_kernel_path returns CAV_E_UNSUPPORTED;
+ *   CAV_PATH_GENERIC  register/LDG kernel for any shape;
+ *   CAV_PATH_AUTO     (default) TMA when eligible and the grid has at least one plane-tile per SM.
+ * cav_get_kernel_path reports the kernel the next run will use (CAV_PATH_GENERIC or CAV_PATH_TMA). */
+int cav_set_kernel_path(cav_sim* sim, int path);
+int cav_get_kernel_path(cav_sim* sim, int* path);
 
 /* Number of kernels this library has launched for this handle (stage kernels + setup). */
 int cav_get_launch_count(cav_sim* sim, long long* n);

@@ -22,6 +22,7 @@ CAV_E_NONFINITE, CAV_E_DT_UNDERFLOW, CAV_E_SINGULAR_NORM, CAV_E_UNSUPPORTED = -5
 CAV_F32, CAV_F64 = 0, 1
 CAV_NORM_NCELLS, CAV_NORM_SUM_U = 0, 1
 CAV_LAUNCH_GRAPH, CAV_LAUNCH_STREAM = 0, 1
+CAV_PATH_AUTO, CAV_PATH_GENERIC, CAV_PATH_TMA = 0, 1, 2
 CAV_MAX_MODES = 32
 
 
@@ -69,6 +70,8 @@ _SIGS = {
     "cav_get_dmdt": ([_vp, _vp, _i], _i),
     "cav_get_dadt": ([_vp, _dp], _i),
     "cav_set_sweep_order": ([_vp, _i], _i),
+    "cav_set_kernel_path": ([_vp, _i], _i),
+    "cav_get_kernel_path": ([_vp, C.POINTER(_i)], _i),
     "cav_run": ([_vp, _d, _d, _d, _d], _i),
     "cav_run_steps": ([_vp, _d, _d, _d, _d, _ll], _i),
     "cav_sync": ([_vp], _i),
@@ -212,6 +215,16 @@ def cav_get_dadt(sim, N: int) -> np.ndarray:
     return out[:2 * N].view(np.complex128).copy()
 
 
+def cav_set_kernel_path(sim, path: int) -> None:
+    _check(_lib.cav_set_kernel_path(sim, int(path)), "cav_set_kernel_path", sim)
+
+
+def cav_get_kernel_path(sim) -> int:
+    p = _i()
+    _check(_lib.cav_get_kernel_path(sim, C.byref(p)), "cav_get_kernel_path", sim)
+    return p.value
+
+
 def cav_set_sweep_order(sim, serpentine: int) -> None:
     _check(_lib.cav_set_sweep_order(sim, int(serpentine)), "cav_set_sweep_order", sim)
 
@@ -282,7 +295,7 @@ class Sim:
     """RAII wrapper around a cav_sim handle."""
 
     def __init__(self, w, precision: str = "f32", renormalize: bool = True, overlap_norm: int = CAV_NORM_NCELLS,
-                 stream: int | None = None):
+                 stream: int | None = None, path: int | None = None):
         self.np_dtype = np.float32 if precision == "f32" else np.float64
         self.N, self.n_sub = int(np.asarray(w.omega).size), int(w.n_sub)
         self.shape_m = (self.n_sub, 3, w.nz, w.ny, w.nx)
@@ -300,6 +313,8 @@ class Sim:
         cav_set_m(self.h, np.ascontiguousarray(w.m0, dtype=self.np_dtype))
         if self.N:
             cav_set_a(self.h, w.a0)
+        if path is not None:
+            cav_set_kernel_path(self.h, path)
 
     def close(self):
         if self.h:

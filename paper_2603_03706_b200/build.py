@@ -14,8 +14,9 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcavmag.so")
 SOURCES = ["cavmag_api.cu", "stage_inst_f32_fm.cu", "stage_inst_f32_afm.cu", "stage_inst_f64_fm.cu",
-           "stage_inst_f64_afm.cu"]
-HEADERS = ["cavmag_types.cuh", "stage_kernel.cuh", os.path.join("..", "..", "include", "cavmag.h")]
+           "stage_inst_f64_afm.cu", "stage_tma_inst_f32_fm.cu", "stage_tma_inst_f32_afm.cu",
+           "stage_tma_inst_f64_fm.cu", "stage_tma_inst_f64_afm.cu"]
+HEADERS = ["cavmag_types.cuh", "stage_kernel.cuh", "stage_tma.cuh", os.path.join("..", "..", "include", "cavmag.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

@@ -8,8 +8,10 @@
 #include <cstring>
 #include <new>
 
+#include <cuda.h>      // CUtensorMap types only; the encoder is fetched with cudaGetDriverEntryPoint
+
 #include "../../include/cavmag.h"
-#include "stage_kernel.cuh"
+#include "stage_tma.cuh"
 
 using namespace cavmag;
 
@@ -45,6 +47,17 @@ struct cav_sim {
     long long host_launches = 0;
     int* h_flag = nullptr;       // pinned
     char cuda_err[256] = {0};
+    // ---- TMA-pipelined path ----
+    int kernel_path = CAV_PATH_AUTO;
+    int n_sm = 148;
+    size_t smem_optin = 0;
+    unsigned char* d_maps = nullptr;   // [MAP_COUNT][128] CUtensorMap table
+    bool maps_ok = false;              // cell-field maps encoded
+    bool tma_eligible = false;         // alignment + shared-memory budget allow the TMA kernels
+    bool use_tma = false;              // decision for the current graph / launches
+    TmaArgs targs[8];
+    size_t tsmem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int tgrid = 1;
 };
 
 namespace {
@@ -131,6 +144,12 @@ __global__ void k_sum_u(const T* __restrict__ u, long long nc, double* __restric
     if (threadIdx.x == 0) out[n * gridDim.x + blockIdx.x] = sh[0];
 }
 
+const void* stage_tma_fn(const cav_sim* s, int stage) {
+    const bool f32 = s->prm.precision == CAV_F32;
+    if (s->prm.n_sub == 1) return f32 ? stage_tma_kernel_f32_fm(stage, s->nb) : stage_tma_kernel_f64_fm(stage, s->nb);
+    return f32 ? stage_tma_kernel_f32_afm(stage, s->nb) : stage_tma_kernel_f64_afm(stage, s->nb);
+}
+
 const void* stage_fn(const cav_sim* s, int stage) {
     const bool f32 = s->prm.precision == CAV_F32;
     if (s->prm.n_sub == 1) return f32 ? stage_kernel_f32_fm(s->vec, stage, s->nb) : stage_kernel_f64_fm(s->vec, stage, s->nb);
@@ -138,6 +157,121 @@ const void* stage_fn(const cav_sim* s, int stage) {
 }
 
 int bucket(int N) { return N == 0 ? 0 : N <= 2 ? 2 : N <= 8 ? 8 : 32; }
+
+// ---- TMA path: tensor maps, ring depths, shared-memory budget -----------------------------------
+
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+encode_tiled_fn get_encoder() {
+    static encode_tiled_fn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (encode_tiled_fn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// 4-D map over [C][nz][ny][nx] (x fastest) with box [C][1][by][bx].
+bool encode_map(const cav_sim* s, CUtensorMap* out, void* base, int C, int bx, int by, int boxC = 0) {
+    encode_tiled_fn enc = get_encoder();
+    if (!enc || !base || C < 1) return false;
+    const cuuint64_t es = s->esize;
+    cuuint64_t dims[4] = {(cuuint64_t)s->grid.nx, (cuuint64_t)s->grid.ny, (cuuint64_t)s->grid.nz, (cuuint64_t)C};
+    cuuint64_t strides[3] = {dims[0] * es, dims[0] * dims[1] * es, (cuuint64_t)s->nc * es};
+    cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, (cuuint32_t)(boxC > 0 ? boxC : C)};
+    cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUtensorMapDataType dt = s->prm.precision == CAV_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+    return enc(out, dt, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int tma_stage_naux(int stage) { return stage <= 2 ? 0 : stage == 7 ? 1 : stage == 6 ? 5 : stage; }
+
+// Encodes the maps of the fixed cell-field buffers (once) and of u (whenever the mode set changes), then sizes
+// the rings of every stage for the current N.  Leaves tma_eligible = false if anything does not fit.
+int plan_tma(cav_sim* s) {
+    s->tma_eligible = false;
+    const int es = (int)s->esize;
+    if (((long long)s->grid.nx * es) % 16 != 0) return CAV_OK;         // TMA global strides must be multiples of 16 B
+    if (!get_encoder() || !s->d_maps) return CAV_OK;
+    const int TX = kTmaRowBytes / es, HX = kTmaHaloBytes / es, C = 3 * s->prm.n_sub;
+    CUtensorMap h[MAP_COUNT];
+    memset(h, 0, sizeof(h));
+    bool ok = true;
+    ok = ok && encode_map(s, &h[MAP_H_Y0], s->Y[0], C, TX + 2 * HX, kTmaTY + 2);
+    ok = ok && encode_map(s, &h[MAP_H_Y1], s->Y[1], C, TX + 2 * HX, kTmaTY + 2);
+    ok = ok && encode_map(s, &h[MAP_H_MS0], s->MS[0], C, TX + 2 * HX, kTmaTY + 2);
+    ok = ok && encode_map(s, &h[MAP_H_MS1], s->MS[1], C, TX + 2 * HX, kTmaTY + 2);
+    ok = ok && encode_map(s, &h[MAP_H_K0], s->K[0], C, TX + 2 * HX, kTmaTY + 2);
+    ok = ok && encode_map(s, &h[MAP_H_K6], s->K[6], C, TX + 2 * HX, kTmaTY + 2);
+    ok = ok && encode_map(s, &h[MAP_P_Y0], s->Y[0], C, TX, kTmaTY);
+    ok = ok && encode_map(s, &h[MAP_P_Y1], s->Y[1], C, TX, kTmaTY);
+    ok = ok && encode_map(s, &h[MAP_P_MS0], s->MS[0], C, TX, kTmaTY);
+    for (int j = 0; j < 7; ++j) ok = ok && encode_map(s, &h[MAP_P_K0 + j], s->K[j], C, TX, kTmaTY);
+    if (s->N > 0) ok = ok && encode_map(s, &h[MAP_P_U], s->u, s->N, TX, kTmaTY, s->N < kTmaUChunk ? s->N : kTmaUChunk);
+    if (!ok) return CAV_OK;
+    CK(cudaMemcpyAsync(s->d_maps, h, sizeof(h), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+
+    const unsigned hbox_tx = (unsigned)(kTmaHaloRowBytes * (kTmaTY + 2) * C);
+    const unsigned hbox = (hbox_tx + 127u) & ~127u;
+    const int ntx = (s->grid.nx + TX - 1) / TX, nty = (s->grid.ny + kTmaTY - 1) / kTmaTY;
+    const long long Q = (long long)ntx * nty * s->grid.nz;
+    s->tgrid = (int)(Q < s->n_sm ? Q : s->n_sm);
+    for (int stage = 1; stage <= 7; ++stage) {
+        const void* fn = stage_tma_fn(s, stage);
+        if (!fn) return CAV_OK;
+        cudaFuncAttributes fa;
+        CK(cudaFuncGetAttributes(&fa, fn));
+        // dynamic budget = opt-in limit - the kernel's static shared memory - a little slack
+        const size_t budget = s->smem_optin > fa.sharedSizeBytes + 256 ? s->smem_optin - fa.sharedSizeBytes - 256 : 0;
+        TmaArgs& t = s->targs[stage];
+        memset(&t, 0, sizeof(t));
+        t.maps = s->d_maps;
+        t.ntx = ntx; t.nty = nty; t.Q = Q;
+        t.hbox_bytes = hbox; t.hbox_tx = hbox_tx;
+        t.ms_slot_bytes = (stage == 2 ? 2u : 1u) * hbox;
+        t.aux_slot_bytes = (unsigned)(tma_stage_naux(stage) * C) * (unsigned)(kTmaRowBytes * kTmaTY);
+        t.n_uchunks = (s->N + kTmaUChunk - 1) / kTmaUChunk;
+        t.u_slot_bytes = (unsigned)(s->N < kTmaUChunk ? s->N : kTmaUChunk) * (unsigned)(kTmaRowBytes * kTmaTY);
+        // ring depths: maximise the smallest look-ahead (in planes) of the rings the stage uses
+        const bool has_a = t.aux_slot_bytes > 0, has_u = t.u_slot_bytes > 0;
+        double best = -1e9;
+        int bDa = 0, bDu = 0, bDm = 0;
+        for (int Da = has_a ? 2 : 0; Da <= (has_a ? 4 : 0); ++Da)
+            for (int Du = has_u ? 2 : 0; Du <= (has_u ? kTmaMaxDepth : 0); ++Du)
+                for (int Dm = 4; Dm <= 8; ++Dm) {
+                    const size_t bytes = (size_t)Da * t.aux_slot_bytes + (size_t)Du * t.u_slot_bytes + (size_t)Dm * t.ms_slot_bytes + 128;
+                    if (bytes > budget) continue;
+                    const double la_m = Dm - 3, la_a = has_a ? Da - 1 : 1e3, la_u = has_u ? (double)Du / t.n_uchunks - 1.0 : 1e3;
+                    const double mn = la_m < la_a ? (la_m < la_u ? la_m : la_u) : (la_a < la_u ? la_a : la_u);
+                    const double score = 100.0 * mn + (has_a ? la_a : 0) + (has_u ? la_u : 0) + 0.5 * la_m;
+                    if (score > best) { best = score; bDa = Da; bDu = Du; bDm = Dm; }
+                }
+        if (bDm == 0) return CAV_OK;             // does not fit: stay on the generic kernels
+        t.Da = bDa > 0 ? bDa : 1; t.Du = bDu > 0 ? bDu : 1; t.Dm = bDm;
+        s->tsmem[stage] = (size_t)bDa * t.aux_slot_bytes + (size_t)bDu * t.u_slot_bytes + (size_t)bDm * t.ms_slot_bytes + 128;
+        // the attribute is per function, not per simulation: always raise it to the device limit
+        CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(s->smem_optin - fa.sharedSizeBytes)));
+    }
+    s->tma_eligible = true;
+    return CAV_OK;
+}
+
+void decide_path(cav_sim* s) {
+    if (s->kernel_path == CAV_PATH_GENERIC) s->use_tma = false;
+    else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
+    else s->use_tma = s->tma_eligible && s->targs[1].Q >= (long long)s->n_sm;
+}
 
 void choose_grid(cav_sim* s) {
     const long long biters = (s->nvec + kBlock - 1) / kBlock;      // block-iterations in total
@@ -209,13 +343,13 @@ void destroy_graph(cav_sim* s) {
 }
 
 int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraphNode_t* dep, const void* fn,
-               dim3 grid, dim3 block, void** params) {
+               dim3 grid, dim3 block, void** params, size_t smem) {
     cudaKernelNodeParams kp;
     memset(&kp, 0, sizeof(kp));
     kp.func = const_cast<void*>(fn);
     kp.gridDim = grid;
     kp.blockDim = block;
-    kp.sharedMemBytes = 0;
+    kp.sharedMemBytes = (unsigned)smem;
     kp.kernelParams = params;
     kp.extra = nullptr;
     CK(cudaGraphAddKernelNode(node, g, dep, dep ? 1 : 0, &kp));
@@ -226,6 +360,7 @@ int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraph
 int build_graph(cav_sim* s) {
     destroy_graph(s);
     choose_grid(s);
+    decide_path(s);
     CK(cudaGraphCreate(&s->graph, 0));
     cudaGraphConditionalHandle handle;
     CK(cudaGraphConditionalHandleCreate(&handle, s->graph, 0, cudaGraphCondAssignDefault));
@@ -237,12 +372,14 @@ int build_graph(cav_sim* s) {
     cudaGraphNode_t n_begin, n_k1, n_while;
     {
         void* params[] = {&ctrl, &h64};
-        int rc = add_kernel(s, s->graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params);
+        int rc = add_kernel(s, s->graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params, 0);
         if (rc) return rc;
     }
     {
         void* params[] = {&A, &trace};
-        int rc = add_kernel(s, s->graph, &n_k1, &n_begin, stage_fn(s, 1), dim3(s->nblocks), dim3(kBlock), params);
+        void* tparams[] = {&A, &s->targs[1], &trace};
+        int rc = s->use_tma ? add_kernel(s, s->graph, &n_k1, &n_begin, stage_tma_fn(s, 1), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[1])
+                            : add_kernel(s, s->graph, &n_k1, &n_begin, stage_fn(s, 1), dim3(s->nblocks), dim3(kBlock), params, 0);
         if (rc) return rc;
     }
     cudaGraphNodeParams cp = {};
@@ -255,9 +392,11 @@ int build_graph(cav_sim* s) {
     cudaGraphNode_t prev;
     for (int stage = 2; stage <= 7; ++stage) {
         void* params[] = {&A, &trace};
+        void* tparams[] = {&A, &s->targs[stage], &trace};
         cudaGraphNode_t node;
-        int rc = add_kernel(s, body, &node, stage == 2 ? nullptr : &prev, stage_fn(s, stage), dim3(s->nblocks),
-                            dim3(kBlock), params);
+        const cudaGraphNode_t* dep = stage == 2 ? nullptr : &prev;
+        int rc = s->use_tma ? add_kernel(s, body, &node, dep, stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage])
+                            : add_kernel(s, body, &node, dep, stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0);
         if (rc) return rc;
         prev = node;
     }
@@ -268,13 +407,19 @@ int build_graph(cav_sim* s) {
 
 int launch_stage(cav_sim* s, int stage, StageArgs& A) {
     double* trace = s->d_trace;
-    void* params[] = {&A, &trace};
-    CK(cudaLaunchKernel(stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0, s->stream));
+    if (s->use_tma) {
+        void* tparams[] = {&A, &s->targs[stage], &trace};
+        CK(cudaLaunchKernel(stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], s->stream));
+    } else {
+        void* params[] = {&A, &trace};
+        CK(cudaLaunchKernel(stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0, s->stream));
+    }
     return CAV_OK;
 }
 
 int run_stream_mode(cav_sim* s) {
     choose_grid(s);
+    decide_path(s);
     StageArgs A = make_args(s, 0ull);
     k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, 0ull);
     CK(cudaGetLastError());
@@ -344,7 +489,9 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     s->nvec = s->nc / s->vecw;
     s->field_bytes = (size_t)prm->n_sub * 3 * s->nc * s->esize;
     const long long biters = (s->nvec + kBlock - 1) / kBlock;
-    s->pstride = (int)((biters < kMaxBlocks ? biters : kMaxBlocks) + 31) / 32 * 32;
+    long long pmax = biters < kMaxBlocks ? biters : kMaxBlocks;       // generic kernel: one partial per block
+    if (pmax < dp.multiProcessorCount) pmax = dp.multiProcessorCount;  // TMA kernel: one partial per SM
+    s->pstride = (int)((pmax + 31) / 32 * 32);
     int rc = CAV_OK;
     auto fail = [&](int code) { cav_destroy(s); return code; };
 #define CKC(call)                                                                                         \
@@ -364,7 +511,10 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     CKC(cudaMalloc(&s->d_ctrl, sizeof(Ctrl)));
     CKC(cudaMallocHost(&s->h_ctrl, sizeof(Ctrl)));
     CKC(cudaMallocHost(&s->h_flag, sizeof(int)));
+    CKC(cudaMalloc(&s->d_maps, 128 * MAP_COUNT));
 #undef CKC
+    s->n_sm = dp.multiProcessorCount;
+    s->smem_optin = dp.sharedMemPerBlockOptin;
     memset(s->h_ctrl, 0, sizeof(Ctrl));
     s->h_ctrl->gamma = prm->gamma;
     s->h_ctrl->dt_min = INFINITY;
@@ -373,6 +523,8 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     rc = push_ctrl(s);
     if (rc) return fail(rc);
     choose_grid(s);
+    rc = plan_tma(s);
+    if (rc) return fail(rc);
     *out = s;
     return CAV_OK;
 }
@@ -388,6 +540,7 @@ int cav_destroy(cav_sim* s) {
     cudaFree(s->partial_max);
     cudaFree(s->d_ctrl);
     cudaFree(s->d_trace);
+    cudaFree(s->d_maps);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     if (s->h_flag) cudaFreeHost(s->h_flag);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -415,6 +568,21 @@ int cav_set_block_cells(cav_sim* s, int cells) {
     s->user_block_cells = cells;
     s->graph_dirty = true;
     choose_grid(s);
+    return CAV_OK;
+}
+
+int cav_set_kernel_path(cav_sim* s, int path) {
+    if (!s || (path != CAV_PATH_AUTO && path != CAV_PATH_GENERIC && path != CAV_PATH_TMA)) return CAV_E_ARG;
+    if (path == CAV_PATH_TMA && !s->tma_eligible) return CAV_E_UNSUPPORTED;
+    s->kernel_path = path;
+    s->graph_dirty = true;
+    return CAV_OK;
+}
+
+int cav_get_kernel_path(cav_sim* s, int* path) {
+    if (!s || !path) return CAV_E_ARG;
+    decide_path(s);
+    *path = s->use_tma ? CAV_PATH_TMA : CAV_PATH_GENERIC;
     return CAV_OK;
 }
 
@@ -476,6 +644,8 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
     const int nb = bucket(N);
     if (nb != s->nb) { s->nb = nb; }
     s->graph_dirty = true;
+    rc = plan_tma(s);
+    if (rc) return rc;
     return push_ctrl(s);
 }
 
@@ -535,6 +705,7 @@ static int ensure_k1(cav_sim* s) {
     if (rc) return rc;
     if (!s->h_ctrl->k1_valid) {
         choose_grid(s);
+        decide_path(s);
         StageArgs A = make_args(s, 0ull);
         k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, 0ull);
         CK(cudaGetLastError());

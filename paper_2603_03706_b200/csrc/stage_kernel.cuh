@@ -102,7 +102,7 @@ static __device__ __noinline__ void stage_finish(const StageArgs& A, const int s
     __shared__ double serr[kMaxModes];
     __shared__ int s_accept;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int nwarp = kBlock / 32;
+    const int nwarp = blockDim.x >> 5;      // 4 (generic kernel) or 9 (TMA kernel)
     const int N = c->N;
     const int nblk = gridDim.x;
     const int nsum = 2 * N + (stage == 7 ? 3 * nsub : 0);
@@ -248,14 +248,14 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
     const int nx = A.nx, ny = A.ny, nz = A.nz;
     const long long plane = (long long)nx * ny;
 
-    const T* __restrict__ y0 = (const T*)A.Y[ycur];
-    T* __restrict__ ynew = (T*)A.Y[1 - ycur];
-    const T* __restrict__ k1 = (const T*)A.K[k1slot];
+    const T* __restrict__ y0 = (const T*)(ycur ? A.Y[1] : A.Y[0]);
+    T* __restrict__ ynew = (T*)(ycur ? A.Y[0] : A.Y[1]);
+    const T* __restrict__ k1 = (const T*)(k1slot ? A.K[6] : A.K[0]);
     const T* __restrict__ uu = (const T*)A.u;
     // stage input (materialised) and outputs
     const T* __restrict__ ms = STAGE == 1 ? y0 : STAGE == 7 ? (const T*)ynew
                               : (STAGE == 3 || STAGE == 5) ? (const T*)A.MS[0] : (const T*)A.MS[1];
-    T* __restrict__ kout = STAGE == 1 ? (T*)A.K[k1slot] : STAGE == 7 ? (T*)A.K[6 - k1slot] : (T*)A.K[STAGE - 1];
+    T* __restrict__ kout = STAGE == 1 ? (T*)(k1slot ? A.K[6] : A.K[0]) : STAGE == 7 ? (T*)(k1slot ? A.K[0] : A.K[6]) : (T*)A.K[STAGE - 1];
     T* __restrict__ mnext = STAGE == 6 ? ynew : (STAGE == 2 || STAGE == 4) ? (T*)A.MS[0] : (T*)A.MS[1];
     T* __restrict__ e6 = (T*)A.MS[0];    // written by stage 6, read by stage 7
 

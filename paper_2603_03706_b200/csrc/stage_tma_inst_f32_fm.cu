@@ -1,0 +1,6 @@
+// Explicit instantiations of the TMA-pipelined stage kernel: T = float, n_sub = 1.
+#include "stage_tma.cuh"
+
+namespace cavmag {
+CAVMAG_DEFINE_TMA_LOOKUP(stage_tma_kernel_f32_fm, float, 1)
+}  // namespace cavmag

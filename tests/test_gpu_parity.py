@@ -34,6 +34,25 @@ def oracle_of(w, **kw):
     return Oracle(w, **kw)
 
 
+PATHS = ["generic", "tma"]
+
+
+def open_sim(api, w, prec, path, **kw):
+    """A Sim forced onto one implementation of the stage kernel; skips when the TMA kernel is not
+    eligible for this shape (nx*sizeof(T) not a multiple of 16 bytes)."""
+    sim = api.Sim(w, precision=prec, **kw)
+    try:
+        api.cav_set_kernel_path(sim.h, api.CAV_PATH_TMA if path == "tma" else api.CAV_PATH_GENERIC)
+    except api.CavError as e:
+        sim.close()
+        assert e.status == api.CAV_E_UNSUPPORTED and path == "tma"
+        es = 4 if prec == "f32" else 8
+        assert (w.nx * es) % 16 != 0, "TMA path refused although the row pitch is 16-byte aligned"
+        pytest.skip("TMA kernel not eligible for this shape")
+    assert api.cav_get_kernel_path(sim.h) == (api.CAV_PATH_TMA if path == "tma" else api.CAV_PATH_GENERIC)
+    return sim
+
+
 def small_problem(nx, ny, nz, N, n_sub=1, seed=7, tilt=0.3, mixed=True, ku=2e3, dt_cells=(4e-9, 5e-9, 6e-9)):
     u = W.random_smooth_profiles(seed, max(N, 1), nx, ny, nz)[:N]
     if N:
@@ -80,11 +99,16 @@ def assert_parity(m, a, ref, prec):
     ((20, 7, 6), 1, 2),       # antiferromagnet
     ((1, 1, 1), 1, 1),        # degenerate: a single cell
     ((2, 1, 9), 2, 2),        # thin in x,y
+    ((72, 19, 5), 3, 1),      # TMA: two x tiles (ragged), three y tiles (ragged)
+    ((132, 9, 11), 8, 1),     # TMA: three x tiles, the last 4 cells wide
+    ((68, 17, 6), 1, 2),      # TMA: antiferromagnet, ragged in x and y
+    ((4, 2, 40), 2, 1),       # TMA: one tile, long z march
 ])
-def test_rhs_matches_oracle(api, prec, shape, N, n_sub):
+@pytest.mark.parametrize("path", PATHS)
+def test_rhs_matches_oracle(api, prec, shape, N, n_sub, path):
     w = small_problem(*shape, N, n_sub)
     dm_ref, da_ref, S_ref = oracle_of(w).rhs(w.m0, w.a0)
-    with api.Sim(w, precision=prec) as sim:
+    with open_sim(api, w, prec, path) as sim:
         dm = np.empty(sim.shape_m, dtype=sim.np_dtype)
         api.cav_get_dmdt(sim.h, dm)
         da = api.cav_get_dadt(sim.h, N)
@@ -113,12 +137,13 @@ def test_rhs_matches_oracle(api, prec, shape, N, n_sub):
 # ----------------------------------------------------------------------------------------
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("variant", ["a", "b"])
-def test_cfg1_fixed_1000_steps(api, prec, variant):
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg1_fixed_1000_steps(api, prec, variant, path):
     w = W.cfg1(variant)
     if prec == "f32":
         w.m0 = w.m0.astype(np.float32).astype(np.float64)
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=w.fixed_dt, max_steps=1000)
-    with api.Sim(w, precision=prec) as sim:
+    with open_sim(api, w, prec, path) as sim:
         api.cav_run_steps(sim.h, math.inf, fixed_dt=w.fixed_dt, max_steps=1000)
         m, a = sim.get_m(), sim.get_a()
         st = api.cav_get_stats(sim.h)
@@ -136,8 +161,13 @@ def test_cfg1_fixed_1000_steps(api, prec, variant):
     ((36, 10, 5), 9, 1, 0.1e-12),
     ((20, 7, 6), 1, 2, 0.05e-12),
     ((16, 8, 4), 2, 2, 0.05e-12),
+    ((72, 19, 5), 3, 1, 0.1e-12),
+    ((132, 9, 11), 8, 1, 0.1e-12),
+    ((68, 17, 6), 1, 2, 0.05e-12),
+    ((64, 8, 3), 32, 1, 0.1e-12),
 ])
-def test_busy_fixed_steps(api, prec, shape, N, n_sub, dt):
+@pytest.mark.parametrize("path", PATHS)
+def test_busy_fixed_steps(api, prec, shape, N, n_sub, dt, path):
     """All terms on (off-axis field and anisotropy, profiled modes, mixed coupling, damping, AFM)."""
     w = small_problem(*shape, N, n_sub, tilt=0.2)
     if prec == "f32":
@@ -145,17 +175,18 @@ def test_busy_fixed_steps(api, prec, shape, N, n_sub, dt):
         w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
         w.u = w.u.astype(np.float32).astype(np.float64)
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=300)
-    with api.Sim(w, precision=prec) as sim:
+    with open_sim(api, w, prec, path) as sim:
         api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=300)
         m, a = sim.get_m(), sim.get_a()
     assert_parity(m, a, ref, prec)
 
 
-def test_cfg2_fixed_f64_and_f32(api):
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg2_fixed_f64_and_f32(api, path):
     w = W.cfg2(nx=64, ny=64, nz=16)
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.2e-12, max_steps=200)
     for prec in ("f64", "f32"):
-        with api.Sim(w, precision=prec) as sim:
+        with open_sim(api, w, prec, path) as sim:
             api.cav_run_steps(sim.h, math.inf, fixed_dt=0.2e-12, max_steps=200)
             m, a = sim.get_m(), sim.get_a()
         if prec == "f64":
@@ -166,11 +197,12 @@ def test_cfg2_fixed_f64_and_f32(api):
             assert np.abs(a - ref.a).max() <= 1e-4 * np.abs(ref.a).max()
 
 
-def test_cfg4_afm_dissipative_fixed(api):
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg4_afm_dissipative_fixed(api, path):
     w = W.cfg4(nx=32, ny=16, nz=8, dissipative=True)
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.02e-12, max_steps=400)
     for prec in ("f64", "f32"):
-        with api.Sim(w, precision=prec) as sim:
+        with open_sim(api, w, prec, path) as sim:
             api.cav_run_steps(sim.h, math.inf, fixed_dt=0.02e-12, max_steps=400)
             m, a = sim.get_m(), sim.get_a()
         if prec == "f64":
@@ -193,6 +225,7 @@ def test_cfg3_full_size_steps(api):
     w.a0 = (1e-3 * (1 + np.arange(8))).astype(np.complex128)
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=3)
     with api.Sim(w, precision="f32") as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA      # the configuration bench.py times
         api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=3)
         m, a = sim.get_m(), sim.get_a()
         S = api.cav_get_overlaps(sim.h, 8)
@@ -214,6 +247,7 @@ def test_cfg5_slab_32_modes(api):
     w.a0 = (1e-3 * (1 + np.arange(32)) * np.exp(0.3j * np.arange(32))).astype(np.complex128)
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=2)
     with api.Sim(w, precision="f32") as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
         api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=2)
         m, a = sim.get_m(), sim.get_a()
     assert np.abs(m - ref.m).max() <= 2e-6
@@ -223,9 +257,9 @@ def test_cfg5_slab_32_modes(api):
 # ----------------------------------------------------------------------------------------
 # adaptive mode: observables
 # ----------------------------------------------------------------------------------------
-def _run_trace(api, w, prec, t_end, sample_dt, tol):
+def _run_trace(api, w, prec, t_end, sample_dt, tol, path="generic"):
     cap = int(round(t_end / sample_dt))
-    with api.Sim(w, precision=prec) as sim:
+    with open_sim(api, w, prec, path) as sim:
         api.cav_set_trace(sim.h, sample_dt, cap)
         api.cav_run(sim.h, t_end, tol=tol)
         tr = api.cav_get_trace(sim.h)
@@ -234,12 +268,13 @@ def _run_trace(api, w, prec, t_end, sample_dt, tol):
     return tr, st
 
 
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_adaptive_rabi_period(api, prec):
+def test_adaptive_rabi_period(api, prec, path):
     """g/2pi = 50 MHz at resonance, a(0) = 0.01: T_R = pi/g = 10 ns within 0.5 %."""
     w = W.macrospin(5.0, [5.0], 50.0, 0.0, alpha=0.0, a0=[0.01], n=4)
     tol = 1e-8 if prec == "f64" else 1e-6
-    tr, st = _run_trace(api, w, prec, 26e-9, 25e-12, tol)
+    tr, st = _run_trace(api, w, prec, 26e-9, 25e-12, tol, path)
     ref = oracle_of(w).run(w.m0, w.a0, t_end=26e-9, tol=tol, sample_dt=25e-12, trace_cap=1040)
     T_gpu = rabi_period(tr[:, 0], tr[:, 1] ** 2 + tr[:, 2] ** 2)
     T_ref = rabi_period(ref.trace[:, 0], ref.trace[:, 1] ** 2 + ref.trace[:, 2] ** 2)
@@ -249,8 +284,9 @@ def test_adaptive_rabi_period(api, prec):
     assert st["accepted"] > 0 and st["rhs_evals"] == 1 + 6 * (st["accepted"] + st["rejected"])
 
 
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_adaptive_anticrossing_frequencies(api, prec):
+def test_adaptive_anticrossing_frequencies(api, prec, path):
     """Polariton branches of cfg1's tiny ferromagnet (per-cell tilt, exchange on) with g/2pi = 50 MHz:
     peak frequencies of GPU and oracle within 1 MHz, and both on Eq. 6."""
     w = W.cfg1("b")
@@ -259,7 +295,7 @@ def test_adaptive_anticrossing_frequencies(api, prec):
     w.B0 = (0.0, 0.0, W.b0_for_ghz(10.03))
     tol = 1e-8 if prec == "f64" else 1e-6
     t_end, sdt = 40e-9, 20e-12
-    tr, _ = _run_trace(api, w, prec, t_end, sdt, tol)
+    tr, _ = _run_trace(api, w, prec, t_end, sdt, tol, path)
     ref = oracle_of(w).run(w.m0, w.a0, t_end=t_end, tol=tol, sample_dt=sdt, trace_cap=2000)
     out = []
     for t in (tr, ref.trace):
@@ -284,18 +320,20 @@ def test_adaptive_afm_neel_line(api):
         return np.sort(np.abs(dominant(om, amp, 2)[0].real))
     f_ref = neel_freq(ref.trace)
     for prec in ("f64", "f32"):
-        tr, _ = _run_trace(api, w, prec, t_end, sdt, 1e-7 if prec == "f64" else 1e-6)
-        assert np.abs(neel_freq(tr) / f_ref - 1).max() < 1e-4
+        for path in PATHS:
+            tr, _ = _run_trace(api, w, prec, t_end, sdt, 1e-7 if prec == "f64" else 1e-6, path)
+            assert np.abs(neel_freq(tr) / f_ref - 1).max() < 1e-4
 
 
 # ----------------------------------------------------------------------------------------
 # launch modes, determinism, edge cases
 # ----------------------------------------------------------------------------------------
-def test_graph_and_stream_modes_bitwise_identical_and_deterministic(api):
+@pytest.mark.parametrize("path", PATHS)
+def test_graph_and_stream_modes_bitwise_identical_and_deterministic(api, path):
     w = small_problem(40, 9, 7, 3, 1)
     outs = []
     for mode in (api.CAV_LAUNCH_GRAPH, api.CAV_LAUNCH_STREAM, api.CAV_LAUNCH_GRAPH):
-        with api.Sim(w, precision="f32") as sim:
+        with open_sim(api, w, "f32", path) as sim:
             api.cav_set_launch_mode(sim.h, mode)
             api.cav_run(sim.h, 5e-12, tol=1e-6)
             outs.append((sim.get_m(), sim.get_a(), api.cav_get_stats(sim.h)))
@@ -319,13 +357,14 @@ def test_block_size_and_sweep_order_do_not_change_fp64_results_beyond_rounding(a
     assert np.array_equal(res[0][0], res[2][0]) or np.abs(res[0][0] - res[2][0]).max() < 1e-13
 
 
-def test_resume_equals_single_run(api):
+@pytest.mark.parametrize("path", PATHS)
+def test_resume_equals_single_run(api, path):
     """Stopping and continuing (FSAL slope kept on the device) gives the same trajectory."""
     w = small_problem(24, 6, 4, 2, 1)
-    with api.Sim(w, precision="f64") as sim:
+    with open_sim(api, w, "f64", path) as sim:
         api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=40)
         m1, a1 = sim.get_m(), sim.get_a()
-    with api.Sim(w, precision="f64") as sim:
+    with open_sim(api, w, "f64", path) as sim:
         api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=15)
         api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=25)
         m2, a2 = sim.get_m(), sim.get_a()
