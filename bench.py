@@ -258,8 +258,10 @@ def run_cuda(args):
     np_dtype = np.float32 if prec == "f32" else np.float64
     tol = w.tol
     stream = torch.cuda.Stream()
-    sim = api.Sim(w, precision=prec, stream=stream.cuda_stream)
+    path = {"auto": None, "generic": api.CAV_PATH_GENERIC, "tma": api.CAV_PATH_TMA}[args.kernel_path]
+    sim = api.Sim(w, precision=prec, stream=stream.cuda_stream, path=path)
     h = sim.h
+    path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma"}[api.cav_get_kernel_path(h)]
     N, nc = w.n_modes, w.n_cells
 
     # spin-up (setup, untimed): the controller grows dt from 1e-14 s to the stability-limited step
@@ -341,7 +343,7 @@ def run_cuda(args):
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": dict(config_of(w, prec, name), parallelism=f"replicas x{world} (no collective)",
-                           launch_mode=args.launch_mode),
+                           launch_mode=args.launch_mode, kernel_path=path_used),
             "sim_ns_per_s": float(units[2]) * 1e9 / (ms_max * 1e-3) / world,
             "mean_dt_ps": sim_t * 1e12 / max(st1["accepted"] - st0["accepted"], 1),
             "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
@@ -375,6 +377,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--spinup", type=int, default=40, help="untimed setup steps that let dt settle")
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
+    ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma"])
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
