@@ -156,7 +156,7 @@ const void* stage_fn(const cav_sim* s, int stage) {
     return f32 ? stage_kernel_f32_afm(s->vec, stage, s->nb) : stage_kernel_f64_afm(s->vec, stage, s->nb);
 }
 
-int bucket(int N) { return N == 0 ? 0 : N <= 2 ? 2 : N <= 8 ? 8 : 32; }
+int bucket(int N) { return N == 0 ? 0 : N == 1 ? 1 : N <= 2 ? 2 : N <= 8 ? 8 : 32; }
 
 // ---- TMA path: tensor maps, ring depths, shared-memory budget -----------------------------------
 
@@ -217,7 +217,7 @@ int plan_tma(cav_sim* s) {
     ok = ok && encode_map(s, &h[MAP_P_Y1], s->Y[1], C, TX, kTmaTY);
     ok = ok && encode_map(s, &h[MAP_P_MS0], s->MS[0], C, TX, kTmaTY);
     for (int j = 0; j < 7; ++j) ok = ok && encode_map(s, &h[MAP_P_K0 + j], s->K[j], C, TX, kTmaTY);
-    if (s->N > 0) ok = ok && encode_map(s, &h[MAP_P_U], s->u, s->N, TX, kTmaTY, s->N < kTmaUChunk ? s->N : kTmaUChunk);
+    if (s->N > 0) ok = ok && encode_map(s, &h[MAP_P_U], s->u, s->N, TX, kTmaTY, s->nb < kTmaUChunk ? s->nb : kTmaUChunk);
     if (!ok) return CAV_OK;
     CK(cudaMemcpyAsync(s->d_maps, h, sizeof(h), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream));
@@ -241,8 +241,8 @@ int plan_tma(cav_sim* s) {
         t.hbox_bytes = hbox; t.hbox_tx = hbox_tx;
         t.ms_slot_bytes = (stage == 2 ? 2u : 1u) * hbox;
         t.aux_slot_bytes = (unsigned)(tma_stage_naux(stage) * C) * (unsigned)(kTmaRowBytes * kTmaTY);
-        t.n_uchunks = (s->N + kTmaUChunk - 1) / kTmaUChunk;
-        t.u_slot_bytes = (unsigned)(s->N < kTmaUChunk ? s->N : kTmaUChunk) * (unsigned)(kTmaRowBytes * kTmaTY);
+        t.n_uchunks = (s->nb + kTmaUChunk - 1) / kTmaUChunk;      // the kernel streams the whole mode bucket; modes >= N are TMA zero fill
+        t.u_slot_bytes = (unsigned)(s->nb < kTmaUChunk ? s->nb : kTmaUChunk) * (unsigned)(kTmaRowBytes * kTmaTY);
         // ring depths: maximise the smallest look-ahead (in planes) of the rings the stage uses
         const bool has_a = t.aux_slot_bytes > 0, has_u = t.u_slot_bytes > 0;
         double best = -1e9;

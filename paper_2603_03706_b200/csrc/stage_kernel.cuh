@@ -584,11 +584,13 @@ const void* stage_kernel_f64_afm(int vec, int stage, int nb);
     const void* NAME(int vec, int stage, int nb) {                                 \
         if (vec) {                                                                 \
             if (nb == 0) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 0) }                  \
+            if (nb == 1) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 1) }                  \
             if (nb == 2) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 2) }                  \
             if (nb == 8) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 8) }                  \
             if (nb == 32) { CAVMAG_STAGE_CASES(T, VECW, NSUB, 32) }                \
         } else {                                                                   \
             if (nb == 0) { CAVMAG_STAGE_CASES(T, 1, NSUB, 0) }                     \
+            if (nb == 1) { CAVMAG_STAGE_CASES(T, 1, NSUB, 1) }                     \
             if (nb == 2) { CAVMAG_STAGE_CASES(T, 1, NSUB, 2) }                     \
             if (nb == 8) { CAVMAG_STAGE_CASES(T, 1, NSUB, 8) }                     \
             if (nb == 32) { CAVMAG_STAGE_CASES(T, 1, NSUB, 32) }                   \

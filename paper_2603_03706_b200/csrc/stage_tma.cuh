@@ -57,6 +57,8 @@ struct TmaArgs {
 };
 
 // ---- PTX wrappers ----------------------------------------------------------------------
+// All shared-memory traffic of the pipeline goes through 32-bit shared-space addresses and explicit
+// ld.shared / mbarrier PTX, so that ptxas emits LDS (not generic LD) with immediate offsets.
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -67,21 +69,44 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+__device__ __forceinline__ unsigned mbar_try(unsigned bar, unsigned parity) {
+    unsigned ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok;
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    while (!mbar_try(bar, parity)) {}
 }
 __device__ __forceinline__ void tma_load_4d(unsigned dst, const void* map, int c0, int c1, int c2, int c3, unsigned bar) {
     asm volatile(
         "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
         ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+// 8-byte pack (2 floats / 1 double) and scalar loads from a shared-space address
+__device__ __forceinline__ Pack<float, 2> lds_pack(unsigned a, const float*) {
+    Pack<float, 2> r;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.v[0]), "=f"(r.v[1]) : "r"(a));
+    return r;
+}
+__device__ __forceinline__ Pack<double, 1> lds_pack(unsigned a, const double*) {
+    Pack<double, 1> r;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(r.v[0]) : "r"(a));
+    return r;
+}
+__device__ __forceinline__ float lds_one(unsigned a, const float*) {
+    float r;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a));
+    return r;
+}
+__device__ __forceinline__ double lds_one(unsigned a, const double*) {
+    double r;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(r) : "r"(a));
+    return r;
 }
 
 // number of halo'd fields / plain cell fields the stage streams
@@ -98,7 +123,12 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     constexpr int C = 3 * NSUB;
     constexpr int NH = StageStreams<STAGE>::n_halo;
     constexpr int NAUX = StageStreams<STAGE>::n_aux;
+    constexpr int NCH = (NB + kTmaUChunk - 1) / kTmaUChunk;          // u chunks per plane
+    constexpr int UCB = NB < kTmaUChunk ? NB : kTmaUChunk;           // modes per chunk (box depth)
+    constexpr int HPLANE = kTmaHaloRowBytes * (kTmaTY + 2);          // one comp of a halo box
+    constexpr int APLANE = kTmaRowBytes * kTmaTY;                    // one comp of a plain box
     using P = Pack<T, VEC>;
+    const T* const tag = nullptr;
 
     Ctrl* ctrl = A.ctrl;
     if (STAGE == 1) { if (ctrl->k1_valid) return; }
@@ -114,10 +144,9 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     const long long nc = A.nc;
     const int Dm = TA.Dm, Da = TA.Da, Du = TA.Du;
 
-    unsigned char* smem = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
-    unsigned char* ms_ring = smem;
-    unsigned char* aux_ring = smem + (size_t)Dm * TA.ms_slot_bytes;
-    unsigned char* u_ring = aux_ring + (size_t)Da * TA.aux_slot_bytes;
+    const unsigned ms_ring = (smem_u32(smem_raw) + 127u) & ~127u;
+    const unsigned aux_ring = ms_ring + (unsigned)Dm * TA.ms_slot_bytes;
+    const unsigned u_ring = aux_ring + (unsigned)Da * TA.aux_slot_bytes;
     const unsigned full_ms = smem_u32(&bars[0]), empty_ms = smem_u32(&bars[kTmaMaxDepth]);
     const unsigned full_aux = smem_u32(&bars[2 * kTmaMaxDepth]), empty_aux = smem_u32(&bars[3 * kTmaMaxDepth]);
     const unsigned full_u = smem_u32(&bars[4 * kTmaMaxDepth]), empty_u = smem_u32(&bars[5 * kTmaMaxDepth]);
@@ -131,17 +160,20 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)ctrl->c[tid] : (T)0;
     __syncthreads();
 
-    // this CTA's run of plane-tiles
+    // this CTA's run of plane-tiles; tile coordinates are advanced incrementally (no divisions in the loops)
     const long long q0 = (TA.Q * (long long)blockIdx.x) / gridDim.x;
     const long long q1 = (TA.Q * (long long)(blockIdx.x + 1)) / gridDim.x;
+    const int nplanes = (int)(q1 - q0);
     const int ycur = ctrl->ycur, k1slot = ctrl->k1slot;
+    const long long t0 = q0 / nz;
+    const int z0 = (int)(q0 - t0 * nz);
+    const int tx0 = (int)(t0 % TA.ntx), ty0 = (int)(t0 / TA.ntx);
 
     if (warp == kTmaTY) {
         // =============================== TMA producer ===============================
-        if (lane == 0 && q0 < q1) {
+        if (lane == 0 && nplanes > 0) {
             const unsigned char* maps = TA.maps;
             auto mp = [&](int i) { return (const void*)(maps + 128 * i); };
-            // halo'd stage-state field(s)
             const void* hmap0 = STAGE == 1 ? mp(MAP_H_Y0 + ycur) : STAGE == 2 ? mp(MAP_H_Y0 + ycur)
                                : STAGE == 7 ? mp(MAP_H_Y0 + (1 - ycur))
                                : (STAGE == 3 || STAGE == 5) ? mp(MAP_H_MS0) : mp(MAP_H_MS1);
@@ -159,48 +191,48 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 amap[0] = mp(MAP_P_MS0);      // e6
             }
             const void* umap = mp(MAP_P_U);
-            const unsigned aux_tx = (unsigned)(NAUX * C) * (unsigned)(kTmaRowBytes * kTmaTY);
-            const int nch = (NB > 0) ? TA.n_uchunks : 0;
+            constexpr unsigned aux_tx = (unsigned)(NAUX * C) * (unsigned)APLANE;
+            constexpr unsigned u_tx = (unsigned)UCB * (unsigned)APLANE;   // the full box is always counted (OOB modes zero-filled)
 
-            long long t = q0 / nz;
-            int z = (int)(q0 - t * nz);
-            unsigned jm = 0, ja = 0, ju = 0;
+            int z = z0, tx = tx0, ty = ty0;
+            int hm = 0, ha = 0, hu = 0;                 // ring heads
+            unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
             auto issue_ms = [&](int x0, int y0, int zz) {
-                const unsigned slot = jm % (unsigned)Dm, par = (jm / (unsigned)Dm) & 1u;
-                mbar_wait(empty_ms + 8 * slot, par ^ 1u);
-                const unsigned bar = full_ms + 8 * slot;
+                mbar_wait(empty_ms + 8 * hm, pm);
+                const unsigned bar = full_ms + 8 * hm;
                 mbar_expect_tx(bar, NH * TA.hbox_tx);
-                const unsigned dst = smem_u32(ms_ring + (size_t)slot * TA.ms_slot_bytes);
+                const unsigned dst = ms_ring + (unsigned)hm * TA.ms_slot_bytes;
                 tma_load_4d(dst, hmap0, x0 - HX, y0 - 1, zz, 0, bar);
                 if constexpr (NH == 2) tma_load_4d(dst + TA.hbox_bytes, hmap1, x0 - HX, y0 - 1, zz, 0, bar);
-                ++jm;
+                if (++hm == Dm) { hm = 0; pm ^= 1u; }
             };
-            for (long long q = q0; q < q1; ++q) {
-                const int x0 = (int)(t % TA.ntx) * TX, y0 = (int)(t / TA.ntx) * kTmaTY;
-                if (q == q0 || z == 0) { issue_ms(x0, y0, z - 1); issue_ms(x0, y0, z); }
+            for (int p = 0; p < nplanes; ++p) {
+                const int x0 = tx * TX, y0 = ty * kTmaTY;
+                if (p == 0 || z == 0) { issue_ms(x0, y0, z - 1); issue_ms(x0, y0, z); }
                 issue_ms(x0, y0, z + 1);
-                for (int ch = 0; ch < nch; ++ch) {       // mode profiles, 8 per slot (out-of-range modes zero-filled)
-                    const unsigned slot = ju % (unsigned)Du, par = (ju / (unsigned)Du) & 1u;
-                    mbar_wait(empty_u + 8 * slot, par ^ 1u);
-                    const unsigned bar = full_u + 8 * slot;
-                    mbar_expect_tx(bar, TA.u_slot_bytes);
-                    tma_load_4d(smem_u32(u_ring + (size_t)slot * TA.u_slot_bytes), umap, x0, y0, z, ch * kTmaUChunk, bar);
-                    ++ju;
+                if constexpr (NB > 0) {
+#pragma unroll 1
+                    for (int ch = 0; ch < NCH; ++ch) {       // mode profiles, UCB per slot (out-of-range modes zero-filled)
+                        mbar_wait(empty_u + 8 * hu, pu);
+                        const unsigned bar = full_u + 8 * hu;
+                        mbar_expect_tx(bar, u_tx);
+                        tma_load_4d(u_ring + (unsigned)hu * u_tx, umap, x0, y0, z, ch * kTmaUChunk, bar);
+                        if (++hu == Du) { hu = 0; pu ^= 1u; }
+                    }
                 }
                 if constexpr (NAUX > 0) {
-                    const unsigned slot = ja % (unsigned)Da, par = (ja / (unsigned)Da) & 1u;
-                    mbar_wait(empty_aux + 8 * slot, par ^ 1u);
-                    const unsigned bar = full_aux + 8 * slot;
+                    mbar_wait(empty_aux + 8 * ha, pa);
+                    const unsigned bar = full_aux + 8 * ha;
                     mbar_expect_tx(bar, aux_tx);
-                    unsigned dst = smem_u32(aux_ring + (size_t)slot * TA.aux_slot_bytes);
+                    unsigned dst = aux_ring + (unsigned)ha * aux_tx;
 #pragma unroll
                     for (int f = 0; f < NAUX; ++f) {
                         tma_load_4d(dst, amap[f], x0, y0, z, 0, bar);
-                        dst += C * (kTmaRowBytes * kTmaTY);
+                        dst += C * APLANE;
                     }
-                    ++ja;
+                    if (++ha == Da) { ha = 0; pa ^= 1u; }
                 }
-                if (++z == nz) { z = 0; ++t; }
+                if (++z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } }
             }
         }
     } else {
@@ -211,13 +243,12 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
         const T anp = (T)A.an_pref, axx = (T)A.axis[0], axy = (T)A.axis[1], axz = (T)A.axis[2];
         const T alpha = (T)A.alpha, llg = (T)A.llg, BE = (T)A.B_exch_inter;
+        const bool renorm = A.renormalize != 0;
 
-        const T* __restrict__ y0g = (const T*)(ycur ? A.Y[1] : A.Y[0]);
         T* __restrict__ ynew = (T*)(ycur ? A.Y[0] : A.Y[1]);
         T* __restrict__ kout = STAGE == 1 ? (T*)(k1slot ? A.K[6] : A.K[0]) : STAGE == 7 ? (T*)(k1slot ? A.K[0] : A.K[6]) : (T*)A.K[STAGE - 1];
         T* __restrict__ mnext = STAGE == 6 ? ynew : (STAGE == 2 || STAGE == 4) ? (T*)A.MS[0] : (T*)A.MS[1];
         T* __restrict__ e6g = (T*)A.MS[0];
-        (void)y0g;
 
         T ox[NB > 0 ? NB : 1], oy[NB > 0 ? NB : 1];
 #pragma unroll
@@ -227,51 +258,67 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         for (int i = 0; i < NSUB * 3; ++i) sm[i] = (T)0;
         T emax2 = (T)0;
 
-        long long t = q0 / nz;
-        int z = (int)(q0 - t * nz);
-        unsigned jm = 0, ja = 0, ju = 0, jzm = 0, jzc = 0, jzp = 0;
-        const int nch = (NB > 0) ? TA.n_uchunks : 0;
-        const int crow = (warp + 1) * kTmaHaloRowBytes + kTmaHaloBytes + lane * 8;   // centre, within a comp plane
-        constexpr int HPLANE = kTmaHaloRowBytes * (kTmaTY + 2);                            // one comp of a halo box
-        constexpr int APLANE = kTmaRowBytes * kTmaTY;                                       // one comp of a plain box
-        const int arow = warp * kTmaRowBytes + lane * 8;
+        const long long plane = (long long)nx * ny;
+        const unsigned crow = (unsigned)((warp + 1) * kTmaHaloRowBytes + kTmaHaloBytes + lane * 8);   // centre, within a comp plane
+        const unsigned arow = (unsigned)(warp * kTmaRowBytes + lane * 8);
 
-        for (long long q = q0; q < q1; ++q) {
-            const int x0 = (int)(t % TA.ntx) * TX, y0 = (int)(t / TA.ntx) * kTmaTY;
-            const int gx = x0 + lane * VEC, gy = y0 + warp;
-            const bool active = gx < nx && gy < ny;
-            const bool seg_start = (q == q0 || z == 0);
-            const bool seg_end = (q + 1 == q1 || z == nz - 1);
-            if (seg_start) {
-                jzm = jm++; jzc = jm++;
-                mbar_wait(full_ms + 8 * (jzm % (unsigned)Dm), (jzm / (unsigned)Dm) & 1u);
-                mbar_wait(full_ms + 8 * (jzc % (unsigned)Dm), (jzc / (unsigned)Dm) & 1u);
-            }
-            jzp = jm++;
-            mbar_wait(full_ms + 8 * (jzp % (unsigned)Dm), (jzp / (unsigned)Dm) & 1u);
-            const unsigned char* sm_zm = ms_ring + (size_t)(jzm % (unsigned)Dm) * TA.ms_slot_bytes;
-            const unsigned char* sm_zc = ms_ring + (size_t)(jzc % (unsigned)Dm) * TA.ms_slot_bytes;
-            const unsigned char* sm_zp = ms_ring + (size_t)(jzp % (unsigned)Dm) * TA.ms_slot_bytes;
-            const bool has_l = gx > 0, has_r = gx + VEC < nx;
-            const bool has_ym = gy > 0, has_yp = gy < ny - 1, has_zm = z > 0, has_zp = z < nz - 1;
+        int z = z0, tx = tx0, ty = ty0;
+        int hm = 0, ha = 0, hu = 0, tm = 0;          // ring heads (next slot to acquire) and the ms tail (next to release)
+        unsigned pm = 0, pa = 0, pu = 0;             // parity to wait on for "full"
+        unsigned sm_zm = 0, sm_zc = 0, sm_zp = 0;    // shared addresses of the live stage-state planes
+        auto acquire_ms = [&]() -> unsigned {
+            mbar_wait(full_ms + 8 * hm, pm);
+            const unsigned a = ms_ring + (unsigned)hm * TA.ms_slot_bytes;
+            if (++hm == Dm) { hm = 0; pm ^= 1u; }
+            return a;
+        };
+        auto release_ms = [&]() {
+            mbar_arrive(empty_ms + 8 * tm);
+            if (++tm == Dm) tm = 0;
+        };
 
-            // stage state from a halo box (STAGE 2: formed on the fly from y0 and k1)
-            auto ldm = [&](const unsigned char* slot, int comp, int off) -> P {
-                const unsigned char* p = slot + comp * HPLANE + off;
-                P a = *reinterpret_cast<const P*>(p);
-                if constexpr (STAGE == 2) {
-                    const P b = *reinterpret_cast<const P*>(p + TA.hbox_bytes);
+        // per-tile quantities (refreshed when the tile changes)
+        bool active = false;
+        long long cell = 0;                          // global cell index of this lane's first cell in plane z
+        T wxl = (T)0, wxr = (T)0, wym = (T)0, wyp = (T)0;
+        bool new_tile = true;
+
+        // stage state from a halo box (STAGE 2: formed on the fly from y0 and k1)
+        auto ldm = [&](unsigned slot, int comp, unsigned off) -> P {
+            const unsigned p = slot + (unsigned)(comp * HPLANE) + off;
+            P a = lds_pack(p, tag);
+            if constexpr (STAGE == 2) {
+                const P b = lds_pack(p + TA.hbox_bytes, tag);
 #pragma unroll
-                    for (int v = 0; v < VEC; ++v) a.v[v] = a.v[v] + ha21 * b.v[v];
-                }
-                return a;
-            };
-            auto ldm1 = [&](const unsigned char* slot, int comp, int off) -> T {
-                const unsigned char* p = slot + comp * HPLANE + off;
-                T a = *reinterpret_cast<const T*>(p);
-                if constexpr (STAGE == 2) a = a + ha21 * *reinterpret_cast<const T*>(p + TA.hbox_bytes);
-                return a;
-            };
+                for (int v = 0; v < VEC; ++v) a.v[v] = a.v[v] + ha21 * b.v[v];
+            }
+            return a;
+        };
+        auto ldm1 = [&](unsigned slot, int comp, unsigned off) -> T {
+            const unsigned p = slot + (unsigned)(comp * HPLANE) + off;
+            T a = lds_one(p, tag);
+            if constexpr (STAGE == 2) a = a + ha21 * lds_one(p + TA.hbox_bytes, tag);
+            return a;
+        };
+
+#pragma unroll 1
+        for (int pl = 0; pl < nplanes; ++pl) {
+            if (new_tile) {
+                const int gx = tx * TX + lane * VEC, gy = ty * kTmaTY + warp;
+                active = gx < nx && gy < ny;
+                // open boundary (G9): an out-of-grid neighbour gets weight 0; its TMA-zero-filled value is finite
+                wxl = gx > 0 ? wx : (T)0;
+                wxr = gx + VEC < nx ? wx : (T)0;
+                wym = gy > 0 ? wy : (T)0;
+                wyp = gy < ny - 1 ? wy : (T)0;
+                cell = (long long)z * plane + (long long)gy * nx + gx;
+                new_tile = false;
+            }
+            const bool seg_start = (pl == 0 || z == 0);
+            const bool seg_end = (pl + 1 == nplanes || z == nz - 1);
+            if (seg_start) { sm_zm = acquire_ms(); sm_zc = acquire_ms(); }
+            sm_zp = acquire_ms();
+            const T wzm = z > 0 ? wz : (T)0, wzp = z < nz - 1 ? wz : (T)0;
 
             P mc[NSUB][3];
 #pragma unroll
@@ -290,48 +337,42 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     if constexpr (NSUB == 1) { mcx[v] = mc[0][0].v[v]; mcy[v] = mc[0][1].v[v]; }
                     else { mcx[v] = (T)0.5 * (mc[0][0].v[v] + mc[1][0].v[v]); mcy[v] = (T)0.5 * (mc[0][1].v[v] + mc[1][1].v[v]); }
                 }
-                constexpr int NCH = (NB + kTmaUChunk - 1) / kTmaUChunk;
-                constexpr int UCB = NB < kTmaUChunk ? NB : kTmaUChunk;
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
-                    if (ch < nch) {
-                        const unsigned uslot = ju % (unsigned)Du;
-                        mbar_wait(full_u + 8 * uslot, (ju / (unsigned)Du) & 1u);
-                        const unsigned char* us = u_ring + (size_t)uslot * TA.u_slot_bytes;
-                        ++ju;
+                    mbar_wait(full_u + 8 * hu, pu);
+                    const unsigned us = u_ring + (unsigned)hu * (unsigned)(UCB * APLANE) + arow;
+                    P un[UCB];
 #pragma unroll
-                        for (int i = 0; i < UCB; ++i) {
-                            const int n = ch * kTmaUChunk + i;
-                            if (n < N) {
-                                const P un = *reinterpret_cast<const P*>(us + i * APLANE + arow);
-                                const T cn = s_cn[n];
-                                T sx = (T)0, sy = (T)0;
+                    for (int i = 0; i < UCB; ++i) un[i] = lds_pack(us + (unsigned)(i * APLANE), tag);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty_u + 8 * hu);
+                    if (++hu == Du) { hu = 0; pu ^= 1u; }
 #pragma unroll
-                                for (int v = 0; v < VEC; ++v) {
-                                    brf[v] += cn * un.v[v];
-                                    sx += un.v[v] * mcx[v];
-                                    sy += un.v[v] * mcy[v];
-                                }
-                                if (active) { ox[n] += sx; oy[n] += sy; }
-                            }
+                    for (int i = 0; i < UCB; ++i) {
+                        const int n = ch * kTmaUChunk + i;          // modes >= N: u zero-filled, c_n = 0
+                        const T cn = s_cn[n];
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) {
+                            brf[v] += cn * un[i].v[v];
+                            ox[n] += un[i].v[v] * mcx[v];
+                            oy[n] += un[i].v[v] * mcy[v];
                         }
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(empty_u + 8 * uslot);
                     }
                 }
             }
-            // ---- halo-free cell streams (ring aux): only the tail below reads them ----
-            const unsigned char* axf = nullptr;
-            unsigned aslot = 0;
+            // ---- halo-free cell streams (ring aux): only the fused tail below reads them ----
+            unsigned axf = 0;
+            int aslot = 0;
             if constexpr (NAUX > 0) {
-                aslot = ja % (unsigned)Da;
-                mbar_wait(full_aux + 8 * aslot, (ja / (unsigned)Da) & 1u);
-                axf = aux_ring + (size_t)aslot * TA.aux_slot_bytes;
-                ++ja;
+                aslot = ha;
+                mbar_wait(full_aux + 8 * ha, pa);
+                axf = aux_ring + (unsigned)ha * (unsigned)(NAUX * C * APLANE) + arow;
+                if (++ha == Da) { ha = 0; pa ^= 1u; }
             }
 
 #pragma unroll
             for (int s = 0; s < NSUB; ++s) {
+                // ---- 6-neighbour exchange: sum over in-grid neighbours of (m_nb - m) (2A/Ms)/D^2 ----
                 T lap[3][VEC];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -342,27 +383,24 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     const P nzp = ldm(sm_zp, comp, crow);
                     T xl = __shfl_up_sync(0xffffffffu, mc[s][c].v[VEC - 1], 1);
                     T xr = __shfl_down_sync(0xffffffffu, mc[s][c].v[0], 1);
-                    if (lane == 0) xl = ldm1(sm_zc, comp, crow - (int)sizeof(T));
-                    if (lane == 31) xr = ldm1(sm_zc, comp, crow + 8);
+                    if (lane == 0) xl = ldm1(sm_zc, comp, crow - (unsigned)sizeof(T));
+                    if (lane == 31) xr = ldm1(sm_zc, comp, crow + 8u);
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
                         const T m0 = mc[s][c].v[v];
-                        T left = (v == 0) ? xl : mc[s][c].v[v > 0 ? v - 1 : 0];
-                        T right = (v == VEC - 1) ? xr : mc[s][c].v[v < VEC - 1 ? v + 1 : VEC - 1];
-                        if (v == 0 && !has_l) left = m0;
-                        if (v == VEC - 1 && !has_r) right = m0;
-                        const T ym = has_ym ? nym.v[v] : m0, yp = has_yp ? nyp.v[v] : m0;
-                        const T zm = has_zm ? nzm.v[v] : m0, zp = has_zp ? nzp.v[v] : m0;
-                        T l = (left - m0) * wx;
-                        l += (right - m0) * wx;
-                        l += (ym - m0) * wy;
-                        l += (yp - m0) * wy;
-                        l += (zm - m0) * wz;
-                        l += (zp - m0) * wz;
+                        const T left = (v == 0) ? xl : mc[s][c].v[v > 0 ? v - 1 : 0];
+                        const T right = (v == VEC - 1) ? xr : mc[s][c].v[v < VEC - 1 ? v + 1 : VEC - 1];
+                        T l = (left - m0) * ((v == 0) ? wxl : wx);
+                        l += (right - m0) * ((v == VEC - 1) ? wxr : wx);
+                        l += (nym.v[v] - m0) * wym;
+                        l += (nyp.v[v] - m0) * wyp;
+                        l += (nzm.v[v] - m0) * wzm;
+                        l += (nzp.v[v] - m0) * wzp;
                         lap[c][v] = l;
                     }
                 }
 
+                // ---- effective field and LLG slope ----
                 P ks[3];
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
@@ -374,14 +412,13 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     if constexpr (NSUB == 2) {
                         Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
                     }
-                    const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
-                    const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
-                    ks[0].v[v] = llg * (tx + alpha * dx);
-                    ks[1].v[v] = llg * (ty + alpha * dy);
-                    ks[2].v[v] = llg * (tz + alpha * dz);
+                    const T tx_ = my * Bz - mz * By, ty_ = mz * Bx - mx * Bz, tz_ = mx * By - my * Bx;
+                    const T dx = my * tz_ - mz * ty_, dy = mz * tx_ - mx * tz_, dz = mx * ty_ - my * tx_;
+                    ks[0].v[v] = llg * (tx_ + alpha * dx);
+                    ks[1].v[v] = llg * (ty_ + alpha * dy);
+                    ks[2].v[v] = llg * (tz_ + alpha * dz);
                 }
 
-                const long long cell = ((long long)z * ny + gy) * nx + gx;
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
                     if (active) stp<T, VEC>(kout + (long long)(s * 3 + c) * nc + cell, ks[c]);
@@ -392,18 +429,18 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                         const int comp = s * 3 + c;
                         P acc, m0v;
                         if constexpr (STAGE == 2) {
-                            m0v = *reinterpret_cast<const P*>(sm_zc + comp * HPLANE + crow);
-                            const P q1 = *reinterpret_cast<const P*>(sm_zc + TA.hbox_bytes + comp * HPLANE + crow);
+                            m0v = lds_pack(sm_zc + (unsigned)(comp * HPLANE) + crow, tag);
+                            const P q1 = lds_pack(sm_zc + TA.hbox_bytes + (unsigned)(comp * HPLANE) + crow, tag);
 #pragma unroll
                             for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[2][0] * q1.v[v];
                         } else {
-                            m0v = *reinterpret_cast<const P*>(axf + comp * APLANE + arow);
-                            const P q1 = *reinterpret_cast<const P*>(axf + (C + comp) * APLANE + arow);
+                            m0v = lds_pack(axf + (unsigned)(comp * APLANE), tag);
+                            const P q1 = lds_pack(axf + (unsigned)((C + comp) * APLANE), tag);
 #pragma unroll
                             for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[STAGE][0] * q1.v[v];
 #pragma unroll
                             for (int j = 1; j < STAGE - 1; ++j) {
-                                const P qj = *reinterpret_cast<const P*>(axf + ((1 + j) * C + comp) * APLANE + arow);
+                                const P qj = lds_pack(axf + (unsigned)(((1 + j) * C + comp) * APLANE), tag);
 #pragma unroll
                                 for (int v = 0; v < VEC; ++v) acc.v[v] += (T)kA[STAGE][j] * qj.v[v];
                             }
@@ -422,11 +459,11 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
                         const int comp = s * 3 + c;
-                        const P m0v = *reinterpret_cast<const P*>(axf + comp * APLANE + arow);
-                        const P q1 = *reinterpret_cast<const P*>(axf + (C + comp) * APLANE + arow);
-                        const P q3 = *reinterpret_cast<const P*>(axf + (2 * C + comp) * APLANE + arow);
-                        const P q4 = *reinterpret_cast<const P*>(axf + (3 * C + comp) * APLANE + arow);
-                        const P q5 = *reinterpret_cast<const P*>(axf + (4 * C + comp) * APLANE + arow);
+                        const P m0v = lds_pack(axf + (unsigned)(comp * APLANE), tag);
+                        const P q1 = lds_pack(axf + (unsigned)((C + comp) * APLANE), tag);
+                        const P q3 = lds_pack(axf + (unsigned)((2 * C + comp) * APLANE), tag);
+                        const P q4 = lds_pack(axf + (unsigned)((3 * C + comp) * APLANE), tag);
+                        const P q5 = lds_pack(axf + (unsigned)((4 * C + comp) * APLANE), tag);
 #pragma unroll
                         for (int v = 0; v < VEC; ++v) {
                             T acc = (T)kA[6][0] * q1.v[v];
@@ -443,7 +480,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                             er[c].v[v] = h * e;
                         }
                     }
-                    if (A.renormalize) {
+                    if (renorm) {
 #pragma unroll
                         for (int v = 0; v < VEC; ++v) {
                             const T inv = rsqrt_t<T>(y5[0].v[v] * y5[0].v[v] + y5[1].v[v] * y5[1].v[v] + y5[2].v[v] * y5[2].v[v]);
@@ -459,7 +496,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 if constexpr (STAGE == 7) {
                     P er[3];
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) er[c] = *reinterpret_cast<const P*>(axf + (s * 3 + c) * APLANE + arow);
+                    for (int c = 0; c < 3; ++c) er[c] = lds_pack(axf + (unsigned)((s * 3 + c) * APLANE), tag);
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
                         const T hd7 = h * (T)kD[6];
@@ -467,11 +504,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                         const T ey = er[1].v[v] + hd7 * ks[1].v[v];
                         const T ez = er[2].v[v] + hd7 * ks[2].v[v];
                         T e2 = ex * ex + ey * ey + ez * ez;
-                        e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;
-                        if (active) {
-                            emax2 = fmax(emax2, e2);
-                            sm[s * 3 + 0] += mc[s][0].v[v]; sm[s * 3 + 1] += mc[s][1].v[v]; sm[s * 3 + 2] += mc[s][2].v[v];
-                        }
+                        e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;     // NaN -> +inf so that max propagates it
+                        // out-of-grid lanes hold TMA zero fill: e2 = 0 and m = 0, so they need no mask
+                        emax2 = fmax(emax2, e2);
+                        sm[s * 3 + 0] += mc[s][0].v[v]; sm[s * 3 + 1] += mc[s][1].v[v]; sm[s * 3 + 2] += mc[s][2].v[v];
                     }
                 }
             }
@@ -480,14 +516,12 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             __syncwarp();
             if (lane == 0) {
                 if constexpr (NAUX > 0) mbar_arrive(empty_aux + 8 * aslot);
-                mbar_arrive(empty_ms + 8 * (jzm % (unsigned)Dm));
-                if (seg_end) {
-                    mbar_arrive(empty_ms + 8 * (jzc % (unsigned)Dm));
-                    mbar_arrive(empty_ms + 8 * (jzp % (unsigned)Dm));
-                }
+                release_ms();                                   // plane z-1
+                if (seg_end) { release_ms(); release_ms(); }    // planes z, z+1 (the next segment reloads its own)
             }
-            jzm = jzc; jzc = jzp;
-            if (++z == nz) { z = 0; ++t; }
+            sm_zm = sm_zc; sm_zc = sm_zp;
+            cell += plane;
+            if (++z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } new_tile = true; }
         }
 
         // ---- pass 1 of the reductions: warp shuffle tree; lane 0 of each consumer warp deposits ----
@@ -504,13 +538,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             }
 #pragma unroll
             for (int i = 0; i < NS; ++i) {
-                const bool used = (i < 2 * NB) ? (i < 2 * N) : true;
-                if (used) {
-                    T x = vals[i];
+                T x = vals[i];
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-                    if (lane == 0) swarp[warp][i] = (double)x;
-                }
+                for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+                if (lane == 0) swarp[warp][i] = (double)x;
             }
             if constexpr (STAGE == 7) {
 #pragma unroll
@@ -571,6 +602,7 @@ const void* stage_tma_kernel_f64_afm(int stage, int nb);
 #define CAVMAG_DEFINE_TMA_LOOKUP(NAME, T, NSUB)                                    \
     const void* NAME(int stage, int nb) {                                          \
         if (nb == 0) { CAVMAG_TMA_STAGE_CASES(T, NSUB, 0) }                        \
+        if (nb == 1) { CAVMAG_TMA_STAGE_CASES(T, NSUB, 1) }                        \
         if (nb == 2) { CAVMAG_TMA_STAGE_CASES(T, NSUB, 2) }                        \
         if (nb == 8) { CAVMAG_TMA_STAGE_CASES(T, NSUB, 8) }                        \
         if (nb == 32) { CAVMAG_TMA_STAGE_CASES(T, NSUB, 32) }                      \
