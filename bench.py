@@ -262,6 +262,8 @@ def run_cuda(args):
     sim = api.Sim(w, precision=prec, stream=stream.cuda_stream, path=path)
     h = sim.h
     path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma"}[api.cav_get_kernel_path(h)]
+    if args.no_stage_overlap:
+        api.cav_set_stage_overlap(h, 0)
     N, nc = w.n_modes, w.n_cells
 
     # spin-up (setup, untimed): the controller grows dt from 1e-14 s to the stability-limited step
@@ -284,6 +286,7 @@ def run_cuda(args):
     barrier()
     clocks = sampler.stop()
     ms = ev0.elapsed_time(ev1)
+    overlap_active = api.cav_get_stage_overlap(h)
     api.cav_sync(h)                                   # raises on a device-side error status
     st1 = api.cav_get_stats(h)
     n1 = api.cav_get_launch_count(h)
@@ -343,7 +346,8 @@ def run_cuda(args):
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": dict(config_of(w, prec, name), parallelism=f"replicas x{world} (no collective)",
-                           launch_mode=args.launch_mode, kernel_path=path_used),
+                           launch_mode=args.launch_mode, kernel_path=path_used,
+                           stage_overlap=bool(overlap_active)),
             "sim_ns_per_s": float(units[2]) * 1e9 / (ms_max * 1e-3) / world,
             "mean_dt_ps": sim_t * 1e12 / max(st1["accepted"] - st0["accepted"], 1),
             "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
@@ -378,6 +382,7 @@ def main():
     ap.add_argument("--spinup", type=int, default=40, help="untimed setup steps that let dt settle")
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
     ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma"])
+    ap.add_argument("--no-stage-overlap", action="store_true", help="full dependencies between stage kernels (A/B aid)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3

@@ -172,6 +172,14 @@ int cav_set_sweep_order(cav_sim* sim, int serpentine);
 int cav_set_kernel_path(cav_sim* sim, int path);
 int cav_get_kernel_path(cav_sim* sim, int* path);
 
+/* Tuning knob (optional): 1 (default) = inside the device-side step loop, consecutive stage kernels of the TMA path
+ * are joined by programmatic dependencies (the next kernel's blocks become resident and run their data-independent
+ * prologue while the previous kernel drains; results are unchanged); 0 = full kernel-to-kernel dependencies.
+ * cav_get_stage_overlap reports whether the graph of the last run was built with them (0 before any run, on the
+ * generic path, in CAV_LAUNCH_STREAM mode, or when the driver refused the edges and the library fell back). */
+int cav_set_stage_overlap(cav_sim* sim, int on);
+int cav_get_stage_overlap(cav_sim* sim, int* active);
+
 /* Number of kernels this library has launched for this handle (stage kernels + setup). */
 int cav_get_launch_count(cav_sim* sim, long long* n);
 

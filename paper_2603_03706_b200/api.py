@@ -72,6 +72,8 @@ _SIGS = {
     "cav_set_sweep_order": ([_vp, _i], _i),
     "cav_set_kernel_path": ([_vp, _i], _i),
     "cav_get_kernel_path": ([_vp, C.POINTER(_i)], _i),
+    "cav_set_stage_overlap": ([_vp, _i], _i),
+    "cav_get_stage_overlap": ([_vp, C.POINTER(_i)], _i),
     "cav_run": ([_vp, _d, _d, _d, _d], _i),
     "cav_run_steps": ([_vp, _d, _d, _d, _d, _ll], _i),
     "cav_sync": ([_vp], _i),
@@ -222,6 +224,16 @@ def cav_set_kernel_path(sim, path: int) -> None:
 def cav_get_kernel_path(sim) -> int:
     p = _i()
     _check(_lib.cav_get_kernel_path(sim, C.byref(p)), "cav_get_kernel_path", sim)
+    return p.value
+
+
+def cav_set_stage_overlap(sim, on: int) -> None:
+    _check(_lib.cav_set_stage_overlap(sim, int(on)), "cav_set_stage_overlap", sim)
+
+
+def cav_get_stage_overlap(sim) -> int:
+    p = _i()
+    _check(_lib.cav_get_stage_overlap(sim, C.byref(p)), "cav_get_stage_overlap", sim)
     return p.value
 
 

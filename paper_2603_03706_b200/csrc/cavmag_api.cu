@@ -52,12 +52,17 @@ struct cav_sim {
     int n_sm = 148;
     size_t smem_optin = 0;
     unsigned char* d_maps = nullptr;   // [MAP_COUNT][128] CUtensorMap table
+#ifdef CAVMAG_PROBE
+    unsigned long long* d_probe = nullptr;
+#endif
     bool maps_ok = false;              // cell-field maps encoded
     bool tma_eligible = false;         // alignment + shared-memory budget allow the TMA kernels
     bool use_tma = false;              // decision for the current graph / launches
     TmaArgs targs[8];
     size_t tsmem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int tgrid = 1;
+    bool want_pdl = true;              // cav_set_stage_overlap
+    bool graph_pdl = false;            // loop-body edges of the current graph are programmatic dependencies
 };
 
 namespace {
@@ -104,9 +109,9 @@ __global__ void k_begin(Ctrl* c, unsigned long long handle) {
     if (tid < c->N) {
         if (!c->k1_valid) {      // stage 1 evaluates f(m_0, a_0)
             c->as[tid][0] = c->a[tid][0]; c->as[tid][1] = c->a[tid][1];
-            c->c[tid] = (2.0 / c->gamma) * (c->Gre[tid] * c->a[tid][0] - c->Gim[tid] * c->a[tid][1]);
+            c->c[tid] = c->two_over_gamma * (c->Gre[tid] * c->a[tid][0] - c->Gim[tid] * c->a[tid][1]);
         } else {
-            mode_stage_state(c, tid, 1);
+            mode_stage_state<1>(c, tid);
         }
     }
     if (tid == 0 && handle != 0ull) cudaGraphSetConditional((cudaGraphConditionalHandle)handle, c->done ? 0u : 1u);
@@ -305,6 +310,7 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     A.iters = s->iters;
     A.serpentine = s->serpentine;
     A.nc = s->nc;
+    A.inv_nc = 1.0 / (double)s->nc;
     A.nvec = s->nvec;
     const cav_params& p = s->prm;
     for (int i = 0; i < 3; ++i) A.B0[i] = p.B0[i];
@@ -320,6 +326,9 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     A.llg = -p.gamma / (1.0 + p.alpha * p.alpha);
     A.B_exch_inter = p.n_sub == 2 ? p.B_exch_inter : 0.0;
     A.renormalize = p.renormalize;
+#ifdef CAVMAG_PROBE
+    A.probe = s->d_probe;
+#endif
     return A;
 }
 
@@ -342,8 +351,10 @@ void destroy_graph(cav_sim* s) {
     s->graph_dirty = true;
 }
 
+// programmatic = true: the edge dep -> node is a programmatic dependency (the node may be scheduled once every
+// block of dep has executed griddepcontrol.launch_dependents; it synchronises with griddepcontrol.wait).
 int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraphNode_t* dep, const void* fn,
-               dim3 grid, dim3 block, void** params, size_t smem) {
+               dim3 grid, dim3 block, void** params, size_t smem, bool programmatic = false) {
     cudaKernelNodeParams kp;
     memset(&kp, 0, sizeof(kp));
     kp.func = const_cast<void*>(fn);
@@ -352,12 +363,24 @@ int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraph
     kp.sharedMemBytes = (unsigned)smem;
     kp.kernelParams = params;
     kp.extra = nullptr;
-    CK(cudaGraphAddKernelNode(node, g, dep, dep ? 1 : 0, &kp));
+    if (dep && programmatic) {
+        CK(cudaGraphAddKernelNode(node, g, nullptr, 0, &kp));
+        cudaGraphEdgeData ed;
+        memset(&ed, 0, sizeof(ed));
+        ed.type = cudaGraphDependencyTypeProgrammatic;
+        ed.from_port = cudaGraphKernelNodePortProgrammatic;
+        CK(cudaGraphAddDependencies_v2(g, dep, node, &ed, 1));
+    } else {
+        CK(cudaGraphAddKernelNode(node, g, dep, dep ? 1 : 0, &kp));
+    }
     return CAV_OK;
 }
 
 // begin -> K1 -> WHILE { K2 -> K3 -> K4 -> K5 -> K6 -> K7 }
-int build_graph(cav_sim* s) {
+// On the TMA path the edges K2 -> ... -> K7 inside the loop body are programmatic dependencies: the next
+// stage kernel's blocks become resident (barrier init, tensor-map prefetch) as the SMs drain and only then
+// wait for the previous kernel to complete.
+int build_graph_impl(cav_sim* s, bool pdl) {
     destroy_graph(s);
     choose_grid(s);
     decide_path(s);
@@ -395,7 +418,7 @@ int build_graph(cav_sim* s) {
         void* tparams[] = {&A, &s->targs[stage], &trace};
         cudaGraphNode_t node;
         const cudaGraphNode_t* dep = stage == 2 ? nullptr : &prev;
-        int rc = s->use_tma ? add_kernel(s, body, &node, dep, stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage])
+        int rc = s->use_tma ? add_kernel(s, body, &node, dep, stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], pdl)
                             : add_kernel(s, body, &node, dep, stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0);
         if (rc) return rc;
         prev = node;
@@ -403,6 +426,16 @@ int build_graph(cav_sim* s) {
     CK(cudaGraphInstantiate(&s->exec, s->graph, 0));
     s->graph_dirty = false;
     return CAV_OK;
+}
+
+int build_graph(cav_sim* s) {
+    decide_path(s);
+    if (s->use_tma && s->want_pdl) {
+        if (build_graph_impl(s, true) == CAV_OK) { s->graph_pdl = true; return CAV_OK; }
+        cudaGetLastError();          // programmatic edges refused here: fall back to full dependencies
+    }
+    s->graph_pdl = false;
+    return build_graph_impl(s, false);
 }
 
 int launch_stage(cav_sim* s, int stage, StageArgs& A) {
@@ -512,11 +545,16 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     CKC(cudaMallocHost(&s->h_ctrl, sizeof(Ctrl)));
     CKC(cudaMallocHost(&s->h_flag, sizeof(int)));
     CKC(cudaMalloc(&s->d_maps, 128 * MAP_COUNT));
+#ifdef CAVMAG_PROBE
+    CKC(cudaMalloc(&s->d_probe, 8 * 256 * 32 * sizeof(unsigned long long)));
+    CKC(cudaMemset(s->d_probe, 0, 8 * 256 * 32 * sizeof(unsigned long long)));
+#endif
 #undef CKC
     s->n_sm = dp.multiProcessorCount;
     s->smem_optin = dp.sharedMemPerBlockOptin;
     memset(s->h_ctrl, 0, sizeof(Ctrl));
     s->h_ctrl->gamma = prm->gamma;
+    s->h_ctrl->two_over_gamma = 2.0 / prm->gamma;
     s->h_ctrl->dt_min = INFINITY;
     s->h_ctrl->t_end = 0.0;
     s->h_ctrl->trace_stride = 1;
@@ -583,6 +621,19 @@ int cav_get_kernel_path(cav_sim* s, int* path) {
     if (!s || !path) return CAV_E_ARG;
     decide_path(s);
     *path = s->use_tma ? CAV_PATH_TMA : CAV_PATH_GENERIC;
+    return CAV_OK;
+}
+
+int cav_set_stage_overlap(cav_sim* s, int on) {
+    if (!s) return CAV_E_ARG;
+    s->want_pdl = on != 0;
+    s->graph_dirty = true;
+    return CAV_OK;
+}
+
+int cav_get_stage_overlap(cav_sim* s, int* active) {
+    if (!s || !active) return CAV_E_ARG;
+    *active = (s->exec && !s->graph_dirty && s->graph_pdl) ? 1 : 0;
     return CAV_OK;
 }
 
@@ -862,3 +913,13 @@ int cav_get_launch_count(cav_sim* s, long long* n) {
 }
 
 }  // extern "C"
+
+#ifdef CAVMAG_PROBE
+// profiling builds only: copies the [8][tgrid][32] timestamp table to the host
+extern "C" int cav_debug_probe(cav_sim* s, unsigned long long* out, int* tgrid) {
+    cudaStreamSynchronize(s->stream);
+    cudaMemcpy(out, s->d_probe, 8 * 256 * 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    *tgrid = s->tgrid;
+    return 0;
+}
+#endif

@@ -44,7 +44,7 @@ struct Ctrl {
     double dt_min, dt_max, last_err;
     // ---- cavity modes (always fp64) ----
     int N;
-    double gamma;
+    double gamma, two_over_gamma;   // two_over_gamma = 2/gamma (host-computed: no fp64 division on the critical path)
     double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes];
     double a[kMaxModes][2];        // a_0: amplitudes of the current accepted state
     double as[kMaxModes][2];       // a_s: amplitudes of the stage the next kernel evaluates
@@ -77,6 +77,7 @@ struct StageArgs {
     int iters;           // block-iterations per block (kBlock*VEC cells each)
     int serpentine;      // 1: odd stages sweep the grid backwards (L2 reuse across kernels)
     long long nc;        // cells
+    double inv_nc;       // 1/nc
     long long nvec;      // nc / VEC
     double B0[3];
     double ex_wx, ex_wy, ex_wz;   // (2A/Ms)/D_d^2, tesla
@@ -85,6 +86,9 @@ struct StageArgs {
     double alpha, llg;            // llg = -gamma/(1+alpha^2)
     double B_exch_inter;
     int renormalize;
+#ifdef CAVMAG_PROBE
+    unsigned long long* probe;   // [8 stages][gridDim.x][32] timestamps (profiling builds only)
+#endif
 };
 
 }  // namespace cavmag

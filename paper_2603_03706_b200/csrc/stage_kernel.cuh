@@ -24,6 +24,22 @@
 
 namespace cavmag {
 
+#ifdef CAVMAG_PROBE
+// profiling builds only: globaltimer (slot) and clock64 (16 + slot) of this block at a marked point
+template <typename Args>
+__device__ __forceinline__ void probe_mark(const Args& A, int stage, int slot) {
+    unsigned long long g, c = clock64();
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g));
+    unsigned long long* p = A.probe + ((size_t)stage * gridDim.x + blockIdx.x) * 32;
+    p[slot] = g; p[16 + slot] = c;
+}
+#define CAVMAG_MARK(slot) probe_mark(A, STAGE, slot)
+#define CAVMAG_MARKF(slot) do { if (threadIdx.x == 0) probe_mark(A, stage, slot); } while (0)
+#else
+#define CAVMAG_MARK(slot) ((void)0)
+#define CAVMAG_MARKF(slot) ((void)0)
+#endif
+
 __device__ constexpr double kA[7][7] = CAVMAG_DP_A;
 __device__ constexpr double kD[7] = CAVMAG_DP_D;
 
@@ -80,56 +96,130 @@ __device__ __forceinline__ void prepare_h(Ctrl* c) {
 
 // a_s and the RF weights c_n = (2/gamma) Re[G_n a_s,n] for stage row `row` (0-based: row r gives
 // the state of stage r+1), one thread per mode.
-__device__ __forceinline__ void mode_stage_state(Ctrl* c, int n, int row) {
+template <int ROW>
+__device__ __forceinline__ void mode_stage_state(Ctrl* c, int n) {
     double re = 0.0, im = 0.0;
-    for (int j = 0; j < row; ++j) {
-        re += kA[row][j] * c->ka[j][n][0];
-        im += kA[row][j] * c->ka[j][n][1];
+#pragma unroll
+    for (int j = 0; j < ROW; ++j) {          // compile-time coefficients: no table loads on the critical path
+        re += kA[ROW][j] * c->ka[j][n][0];
+        im += kA[ROW][j] * c->ka[j][n][1];
     }
     const double are = c->a[n][0] + c->h * re, aim = c->a[n][1] + c->h * im;
     c->as[n][0] = are; c->as[n][1] = aim;
-    c->c[n] = (2.0 / c->gamma) * (c->Gre[n] * are - c->Gim[n] * aim);
+    c->c[n] = c->two_over_gamma * (c->Gre[n] * are - c->Gim[n] * aim);
 }
 
 // ---------------------------------------------------------------------------------------
 // Tail of every stage kernel, executed by the last block to arrive: deterministic second
 // reduction pass, mode ODEs + stage algebra, and (stage 7) the accept/reject controller.
+//
+// Everything here sits on the critical path between two stage kernels, so global-memory round
+// trips are what it costs: the whole Ctrl struct and all block partials are fetched with one
+// batch of independent loads, the arithmetic runs on a shared-memory copy of Ctrl, and the copy
+// is written back with one batch of coalesced stores.
 // ---------------------------------------------------------------------------------------
-static __device__ __noinline__ void stage_finish(const StageArgs& A, const int stage, const int nsub, double* trace) {
-    Ctrl* c = A.ctrl;
+constexpr int kCtrlWords = (int)(sizeof(Ctrl) / 8);
+static_assert(sizeof(Ctrl) % 8 == 0, "Ctrl is copied as 8-byte words");
+static_assert(kCtrlWords <= 8 * kBlock, "Ctrl copy: at most 8 words per thread");
+
+// r^(1/5) for r in [1e-2, 1e3]: float seed + one Newton step in fp64 (relative error < 1e-13).  A libm pow()
+// in fp64 costs several microseconds of single-thread latency on this part, all of it between two stage kernels.
+__device__ __forceinline__ double fifth_root(double r) {
+    const double y = (double)powf((float)r, 0.2f);
+    const double y2 = y * y;
+    return y * (4.0 + r / (y2 * y2 * y)) * 0.2;
+}
+
+// The arguments stage_finish needs, by value (a reference to the kernel's StageArgs would sit in local memory
+// and cost one more dependent memory round trip before the first load can issue).
+struct FinishArgs {
+    Ctrl* ctrl;
+    const double* partial;
+    const double* partial_max;
+    unsigned long long cond_handle;
+    double inv_nc;
+    int pstride;
+#ifdef CAVMAG_PROBE
+    unsigned long long* probe;
+#endif
+};
+__device__ __forceinline__ FinishArgs finish_args(const StageArgs& S) {
+    FinishArgs F;
+    F.ctrl = S.ctrl; F.partial = S.partial; F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
+    F.inv_nc = S.inv_nc; F.pstride = S.pstride;
+#ifdef CAVMAG_PROBE
+    F.probe = S.probe;
+#endif
+    return F;
+}
+
+template <int stage>
+static __device__ __noinline__ void stage_finish(const FinishArgs A, const int nsub, const int N, double* trace) {
+    __shared__ __align__(16) unsigned long long sc_words[kCtrlWords];
     __shared__ double sred[kMaxSums];
     __shared__ double smax;
     __shared__ double serr[kMaxModes];
     __shared__ int s_accept;
+    Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);          // shared-memory working copy
+    unsigned long long* const gcw = reinterpret_cast<unsigned long long*>(A.ctrl);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nwarp = blockDim.x >> 5;      // 4 (generic kernel) or 9 (TMA kernel)
-    const int N = c->N;
+    const int nthr = blockDim.x;
+    const int nwarp = nthr >> 5;            // 4 (generic kernel) or 9 (TMA kernel)
     const int nblk = gridDim.x;
     const int nsum = 2 * N + (stage == 7 ? 3 * nsub : 0);
-    __threadfence();
-    // pass 2: lane l adds blocks l, l+32, ... in order, then a fixed xor tree
-    for (int comp = warp; comp < nsum; comp += nwarp) {
-        const double* p = A.partial + (size_t)comp * A.pstride;
-        double acc = 0.0;
+    CAVMAG_MARKF(8);
+    // Ctrl -> registers (consumed after the partial sums so that all loads are in flight together)
+    unsigned long long cw[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int idx = tid + k * nthr;
+        cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
+    }
+    // pass 2: lane l adds blocks l, l+32, ... in order, then a fixed xor tree; two sums per warp at a time
+    for (int comp = warp; comp < nsum; comp += 2 * nwarp) {
+        const int comp2 = comp + nwarp;
+        const bool two = comp2 < nsum;
+        const double* p1 = A.partial + (size_t)comp * A.pstride;
+        const double* p2 = A.partial + (size_t)(two ? comp2 : comp) * A.pstride;
+        double acc1 = 0.0, acc2 = 0.0;
         for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
-            double v[8];
+            double v1[8], v2[8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) v[j] = (b0 + 32 * j < nblk) ? __ldcg(p + b0 + 32 * j) : 0.0;
+            for (int j = 0; j < 8; ++j) {
+                const bool in = b0 + 32 * j < nblk;
+                v1[j] = in ? __ldcg(p1 + b0 + 32 * j) : 0.0;
+                v2[j] = (in && two) ? __ldcg(p2 + b0 + 32 * j) : 0.0;
+            }
 #pragma unroll
-            for (int j = 0; j < 8; ++j) acc += v[j];
+            for (int j = 0; j < 8; ++j) { acc1 += v1[j]; acc2 += v2[j]; }
         }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if (lane == 0) sred[comp] = acc;
+        for (int o = 16; o > 0; o >>= 1) {
+            acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
+            acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
+        }
+        if (lane == 0) { sred[comp] = acc1; if (two) sred[comp2] = acc2; }
     }
     if (stage == 7 && warp == nwarp - 1) {
         double mx = 0.0;
-        for (int b = lane; b < nblk; b += 32) mx = fmax(mx, __ldcg(A.partial_max + b));
+        for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
+            double v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) v[j] = (b0 + 32 * j < nblk) ? __ldcg(A.partial_max + b0 + 32 * j) : 0.0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) mx = fmax(mx, v[j]);
+        }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
         if (lane == 0) smax = mx;
     }
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int idx = tid + k * nthr;
+        if (idx < kCtrlWords) sc_words[idx] = cw[k];
+    }
     __syncthreads();
+    CAVMAG_MARKF(9);
 
     // mode ODE at this stage: ka_s = -(i w + kappa) a_s + i G S_s     (Eq. 12 / Eq. 19)
     if (tid < N) {
@@ -142,92 +232,96 @@ static __device__ __noinline__ void stage_finish(const StageArgs& A, const int s
         const double kre = (-c->kappa[n] * are + c->omega[n] * aim) - (Gre * Sim + Gim * Sre);
         const double kim = (-c->kappa[n] * aim - c->omega[n] * are) + (Gre * Sre - Gim * Sim);
         c->ka[stage - 1][n][0] = kre; c->ka[stage - 1][n][1] = kim;
-        if (stage >= 2 && stage <= 5) {
-            mode_stage_state(c, n, stage);              // a_{s+1}, c^{(s+1)}
-        } else if (stage == 6) {
-            mode_stage_state(c, n, 6);                  // row 6 = b: the 5th-order candidate
+        if constexpr (stage >= 2 && stage <= 5) {
+            mode_stage_state<stage>(c, n);              // a_{s+1}, c^{(s+1)}
+        } else if constexpr (stage == 6) {
+            mode_stage_state<6>(c, n);                  // row 6 = b: the 5th-order candidate
             c->anew[n][0] = c->as[n][0]; c->anew[n][1] = c->as[n][1];
-        } else if (stage == 7) {
+        } else if constexpr (stage == 7) {
             double ere = 0.0, eim = 0.0;
+#pragma unroll
             for (int j = 0; j < 7; ++j) { ere += kD[j] * c->ka[j][n][0]; eim += kD[j] * c->ka[j][n][1]; }
             const double e = fabs(c->h) * sqrt(ere * ere + eim * eim);
             serr[n] = (e < CUDART_INF) ? e : CUDART_INF;
         }
     }
+    bool set_cond = false;
     if (stage >= 2 && stage <= 6) {
         if (tid == 0) { c->rhs_evals++; c->arrive = 0u; }
-        return;
-    }
-    __syncthreads();
-
-    if (stage == 7) {
-        if (tid == 0) {
-            double err = sqrt(smax);
-            for (int n = 0; n < N; ++n) err = fmax(err, serr[n]);
-            const bool finite = err < CUDART_INF;
-            const double h = c->h;
-            bool accept;
-            if (c->adaptive) accept = finite && err <= c->tol;
-            else { accept = true; if (!finite) { accept = false; c->status = -5; } }
-            double fac;
-            if (!finite) fac = 0.5;
-            else if (err == 0.0) fac = 2.0;
-            else { fac = 0.8 * pow(c->tol / err, 0.2); fac = fmin(fmax(fac, 0.5), 2.0); }
-            c->rhs_evals++;
-            c->steps_run++;
-            c->last_err = err;
-            if (accept) {
-                c->t = c->clamped ? c->target : c->t + h;
-                c->ycur ^= 1;
-                c->k1slot = 6 - c->k1slot;
-                c->accepted++;
-                c->dt_min = fmin(c->dt_min, h);
-                c->dt_max = fmax(c->dt_max, h);
-                if (c->adaptive) { const double prop = h * fac; c->dt = c->clamped ? fmax(prop, c->dt) : prop; }
-                for (int i = 0; i < 3 * nsub; ++i) c->mavg[i] = sred[2 * N + i] / (double)A.nc;
-                const bool take = trace != nullptr && c->sample_dt > 0.0 && c->trace_n < c->trace_cap &&
-                                  (c->adaptive ? (c->clamped && c->sample_hit)
-                                               : ((c->accepted - c->trace_acc0) % c->trace_stride == 0));
-                if (take) {
-                    double* row = trace + (size_t)c->trace_n * (1 + 4 * N + 3 * nsub);
-                    row[0] = c->t;
-                    for (int n = 0; n < N; ++n) {
-                        row[1 + 2 * n] = c->anew[n][0]; row[2 + 2 * n] = c->anew[n][1];
-                        row[1 + 2 * N + 2 * n] = c->S[n][0]; row[2 + 2 * N + 2 * n] = c->S[n][1];
+    } else {
+        __syncthreads();
+        if (stage == 7) {
+            if (tid == 0) {
+                double err = sqrt(smax);
+                for (int n = 0; n < N; ++n) err = fmax(err, serr[n]);
+                const bool finite = err < CUDART_INF;
+                const double h = c->h;
+                bool accept;
+                if (c->adaptive) accept = finite && err <= c->tol;
+                else { accept = true; if (!finite) { accept = false; c->status = -5; } }
+                double fac;
+                if (!finite) fac = 0.5;
+                else if (err == 0.0) fac = 2.0;
+                else { fac = 0.8 * fifth_root(fmin(fmax(c->tol / err, 1e-2), 1e3)); fac = fmin(fmax(fac, 0.5), 2.0); }
+                c->rhs_evals++;
+                c->steps_run++;
+                c->last_err = err;
+                if (accept) {
+                    c->t = c->clamped ? c->target : c->t + h;
+                    c->ycur ^= 1;
+                    c->k1slot = 6 - c->k1slot;
+                    c->accepted++;
+                    c->dt_min = fmin(c->dt_min, h);
+                    c->dt_max = fmax(c->dt_max, h);
+                    if (c->adaptive) { const double prop = h * fac; c->dt = c->clamped ? fmax(prop, c->dt) : prop; }
+                    for (int i = 0; i < 3 * nsub; ++i) c->mavg[i] = sred[2 * N + i] * A.inv_nc;
+                    const bool take = trace != nullptr && c->sample_dt > 0.0 && c->trace_n < c->trace_cap &&
+                                      (c->adaptive ? (c->clamped && c->sample_hit)
+                                                   : ((c->accepted - c->trace_acc0) % c->trace_stride == 0));
+                    if (take) {
+                        double* row = trace + (size_t)c->trace_n * (1 + 4 * N + 3 * nsub);
+                        row[0] = c->t;
+                        for (int n = 0; n < N; ++n) {
+                            row[1 + 2 * n] = c->anew[n][0]; row[2 + 2 * n] = c->anew[n][1];
+                            row[1 + 2 * N + 2 * n] = c->S[n][0]; row[2 + 2 * N + 2 * n] = c->S[n][1];
+                        }
+                        for (int i = 0; i < 3 * nsub; ++i) row[1 + 4 * N + i] = c->mavg[i];
+                        c->trace_n++;
                     }
-                    for (int i = 0; i < 3 * nsub; ++i) row[1 + 4 * N + i] = c->mavg[i];
-                    c->trace_n++;
+                } else if (c->status == 0) {
+                    c->rejected++;
+                    c->dt = h * fac;
                 }
-            } else if (c->status == 0) {
-                c->rejected++;
-                c->dt = h * fac;
+                if (c->adaptive && !(c->dt > 1e-20)) c->status = -6;
+                s_accept = accept ? 1 : 0;
             }
-            if (c->adaptive && !(c->dt > 1e-20)) c->status = -6;
-            s_accept = accept ? 1 : 0;
+            __syncthreads();
+            if (tid < N && s_accept) {     // y := y_new (modes), FSAL: ka_1 := ka_7
+                c->a[tid][0] = c->anew[tid][0]; c->a[tid][1] = c->anew[tid][1];
+                c->ka[0][tid][0] = c->ka[6][tid][0]; c->ka[0][tid][1] = c->ka[6][tid][1];
+            }
+            __syncthreads();
+        } else {   // stage 1: k1 of a fresh state
+            if (tid == 0) { c->rhs_evals++; c->k1_valid = 1; }
         }
-        __syncthreads();
-        if (tid < N && s_accept) {     // y := y_new (modes), FSAL: ka_1 := ka_7
-            c->a[tid][0] = c->anew[tid][0]; c->a[tid][1] = c->anew[tid][1];
-            c->ka[0][tid][0] = c->ka[6][tid][0]; c->ka[0][tid][1] = c->ka[6][tid][1];
-        }
-        __syncthreads();
-    } else {   // stage 1: k1 of a fresh state
-        if (tid == 0) { c->rhs_evals++; c->k1_valid = 1; }
-    }
 
-    // start of the next step
-    if (tid == 0) {
-        const bool done = !(c->t < c->t_end) || (c->max_steps > 0 && c->steps_run >= c->max_steps) || c->status != 0;
-        c->done = done ? 1 : 0;
-        prepare_h(c);
+        // start of the next step
+        if (tid == 0) {
+            const bool done = !(c->t < c->t_end) || (c->max_steps > 0 && c->steps_run >= c->max_steps) || c->status != 0;
+            c->done = done ? 1 : 0;
+            prepare_h(c);
+        }
+        __syncthreads();
+        if (tid < N) mode_stage_state<1>(c, tid);           // a_2 = a_0 + h a21 ka_1
+        if (tid == 0) { c->arrive = 0u; set_cond = (A.cond_handle != 0ull && stage == 7); }
     }
+    // write the working copy back
     __syncthreads();
-    if (tid < N) mode_stage_state(c, tid, 1);           // a_2 = a_0 + h a21 ka_1
-    if (tid == 0) {
-        c->arrive = 0u;
-        if (A.cond_handle != 0ull && stage == 7)
-            cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, c->done ? 0u : 1u);
-    }
+    CAVMAG_MARKF(10);
+    for (int idx = tid; idx < kCtrlWords; idx += nthr) gcw[idx] = sc_words[idx];
+    CAVMAG_MARKF(11);
+    if (set_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, c->done ? 0u : 1u);
+    CAVMAG_MARKF(12);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -551,14 +645,18 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
         for (int w = 0; w < nwarp; ++w) mx = fmax(mx, swmax[w]);
         A.partial_max[blockIdx.x] = mx;
     }
-    __threadfence();
+    // One fence per block: the barrier orders every thread's stores before thread 0's gpu-scope fence (release),
+    // the last block's thread 0 fences again after the ticket (acquire) before the barrier that lets its
+    // threads read the other blocks' partials.
     __syncthreads();
     if (tid == 0) {
+        __threadfence();
         const unsigned int old = atomicAdd(&ctrl->arrive, 1u);
         s_last = (old == gridDim.x - 1) ? 1 : 0;
+        if (s_last) __threadfence();
     }
     __syncthreads();
-    if (s_last) stage_finish(A, STAGE, NSUB, trace);
+    if (s_last) stage_finish<STAGE>(finish_args(A), NSUB, N, trace);
 }
 
 // Kernel lookup, one translation unit per (T, NSUB): returns the device function for

@@ -131,15 +131,12 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     const T* const tag = nullptr;
 
     Ctrl* ctrl = A.ctrl;
-    if (STAGE == 1) { if (ctrl->k1_valid) return; }
-    else if (ctrl->done) return;
-
+    if (threadIdx.x == 0) CAVMAG_MARK(0);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[6 * kTmaMaxDepth];
     __shared__ T s_cn[NB > 0 ? NB : 1];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int N = ctrl->N;
     const int nx = A.nx, ny = A.ny, nz = A.nz;
     const long long nc = A.nc;
     const int Dm = TA.Dm, Da = TA.Da, Du = TA.Du;
@@ -151,14 +148,27 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     const unsigned full_aux = smem_u32(&bars[2 * kTmaMaxDepth]), empty_aux = smem_u32(&bars[3 * kTmaMaxDepth]);
     const unsigned full_u = smem_u32(&bars[4 * kTmaMaxDepth]), empty_u = smem_u32(&bars[5 * kTmaMaxDepth]);
 
+    // ---- prologue that does not depend on the previous stage kernel (overlaps its tail under a
+    //      programmatic graph edge): barrier init, tensor-map prefetch ----
     if (tid == 0) {
         for (int i = 0; i < Dm; ++i) { mbar_init(full_ms + 8 * i, 1); mbar_init(empty_ms + 8 * i, kTmaTY); }
         for (int i = 0; i < Da; ++i) { mbar_init(full_aux + 8 * i, 1); mbar_init(empty_aux + 8 * i, kTmaTY); }
         for (int i = 0; i < Du; ++i) { mbar_init(full_u + 8 * i, 1); mbar_init(empty_u + 8 * i, kTmaTY); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (warp == kTmaTY && lane < MAP_COUNT)
+        asm volatile("prefetch.tensormap [%0];" ::"l"(TA.maps + 128 * lane) : "memory");
+    // let the next stage kernel be scheduled as SMs drain, then wait for the previous one to have
+    // completed and flushed (both are no-ops without a programmatic dependency)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+
+    if (STAGE == 1) { if (ctrl->k1_valid) return; }
+    else if (ctrl->done) return;
+    const int N = ctrl->N;
     if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)ctrl->c[tid] : (T)0;
     __syncthreads();
+    if (tid == 0) CAVMAG_MARK(1);
 
     // this CTA's run of plane-tiles; tile coordinates are advanced incrementally (no divisions in the loops)
     const long long q0 = (TA.Q * (long long)blockIdx.x) / gridDim.x;
@@ -234,6 +244,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 }
                 if (++z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } }
             }
+            CAVMAG_MARK(6);
         }
     } else {
         // ================================ consumers =================================
@@ -318,6 +329,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             const bool seg_end = (pl + 1 == nplanes || z == nz - 1);
             if (seg_start) { sm_zm = acquire_ms(); sm_zc = acquire_ms(); }
             sm_zp = acquire_ms();
+            if (pl == 0 && tid == 0) CAVMAG_MARK(2);
             const T wzm = z > 0 ? wz : (T)0, wzp = z < nz - 1 ? wz : (T)0;
 
             P mc[NSUB][3];
@@ -524,6 +536,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             if (++z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } new_tile = true; }
         }
 
+        if (tid == 0) CAVMAG_MARK(3);
         // ---- pass 1 of the reductions: warp shuffle tree; lane 0 of each consumer warp deposits ----
         constexpr int NS = 2 * NB + (STAGE == 7 ? 3 * NSUB : 0);
         __shared__ double swarp[kTmaTY][NS > 0 ? NS : 1];
@@ -571,15 +584,24 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     }
 
     // ---- last-block-done: second reduction pass, mode ODEs, controller ----
+    // One fence per block: the barrier orders every thread's stores before thread 0's gpu-scope fence (release),
+    // the last block's thread 0 fences again after the ticket (acquire) before the barrier that lets its
+    // threads read the other blocks' partials.
     __shared__ int s_last;
-    __threadfence();
     __syncthreads();
     if (tid == 0) {
+        __threadfence();
+        CAVMAG_MARK(4);
         const unsigned int old = atomicAdd(&ctrl->arrive, 1u);
         s_last = (old == gridDim.x - 1) ? 1 : 0;
+        if (s_last) __threadfence();
     }
     __syncthreads();
-    if (s_last) stage_finish(A, STAGE, NSUB, trace);
+    if (s_last) stage_finish<STAGE>(finish_args(A), NSUB, N, trace);
+#ifdef CAVMAG_PROBE
+    __syncthreads();
+    if (tid == 0) { CAVMAG_MARK(5); A.probe[((size_t)STAGE * gridDim.x + blockIdx.x) * 32 + 7] = (unsigned long long)s_last; }
+#endif
 }
 
 const void* stage_tma_kernel_f32_fm(int stage, int nb);

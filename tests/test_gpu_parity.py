@@ -342,6 +342,23 @@ def test_graph_and_stream_modes_bitwise_identical_and_deterministic(api, path):
         assert st["accepted"] == outs[0][2]["accepted"] and st["rejected"] == outs[0][2]["rejected"]
 
 
+def test_stage_overlap_is_bitwise_neutral(api):
+    """Programmatic dependencies between the stage kernels of the loop body only move the data-independent
+    prologue of a kernel under the tail of the previous one: results are bitwise identical with and without."""
+    w = small_problem(96, 24, 12, 3, 1)
+    outs, active = [], []
+    for on in (1, 0, 1):
+        with open_sim(api, w, "f32", "tma") as sim:
+            api.cav_set_stage_overlap(sim.h, on)
+            api.cav_run(sim.h, 5e-12, tol=1e-6)
+            active.append(api.cav_get_stage_overlap(sim.h))
+            outs.append((sim.get_m(), sim.get_a(), api.cav_get_stats(sim.h)))
+    assert active[1] == 0
+    for m, a, st in outs[1:]:
+        assert np.array_equal(m, outs[0][0]) and np.array_equal(a, outs[0][1])
+        assert st["accepted"] == outs[0][2]["accepted"] and st["rejected"] == outs[0][2]["rejected"]
+
+
 def test_block_size_and_sweep_order_do_not_change_fp64_results_beyond_rounding(api):
     w = small_problem(40, 9, 7, 3, 1)
     res = []
