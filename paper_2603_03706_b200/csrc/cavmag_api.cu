@@ -108,7 +108,7 @@ __global__ void k_begin(Ctrl* c, unsigned long long handle) {
     __syncthreads();
     if (tid < c->N) {
         if (!c->k1_valid) {      // stage 1 evaluates f(m_0, a_0)
-            c->as[tid][0] = c->a[tid][0]; c->as[tid][1] = c->a[tid][1];
+            c->as[1][tid][0] = c->a[tid][0]; c->as[1][tid][1] = c->a[tid][1];
             c->c[tid] = c->two_over_gamma * (c->Gre[tid] * c->a[tid][0] - c->Gim[tid] * c->a[tid][1]);
         } else {
             mode_stage_state<1>(c, tid);

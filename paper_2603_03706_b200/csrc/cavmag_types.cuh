@@ -47,7 +47,8 @@ struct Ctrl {
     double gamma, two_over_gamma;   // two_over_gamma = 2/gamma (host-computed: no fp64 division on the critical path)
     double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes];
     double a[kMaxModes][2];        // a_0: amplitudes of the current accepted state
-    double as[kMaxModes][2];       // a_s: amplitudes of the stage the next kernel evaluates
+    double as[2][kMaxModes][2];    // a_s: amplitudes of the state stage s is evaluated at, in as[s & 1] (double-buffered:
+                                   // on the TMA path block 0 of kernel s+1 writes a_{s+1} while the other blocks still read a_s)
     double anew[kMaxModes][2];     // 5th-order candidate
     double ka[7][kMaxModes][2];    // mode slopes ka_1..ka_7
     double S[kMaxModes][2];        // overlaps of the last evaluated stage state

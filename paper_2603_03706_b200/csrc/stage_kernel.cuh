@@ -105,8 +105,67 @@ __device__ __forceinline__ void mode_stage_state(Ctrl* c, int n) {
         im += kA[ROW][j] * c->ka[j][n][1];
     }
     const double are = c->a[n][0] + c->h * re, aim = c->a[n][1] + c->h * im;
-    c->as[n][0] = are; c->as[n][1] = aim;
+    c->as[(ROW + 1) & 1][n][0] = are; c->as[(ROW + 1) & 1][n][1] = aim;      // the state of stage ROW+1
     c->c[n] = c->two_over_gamma * (c->Gre[n] * are - c->Gim[n] * aim);
+}
+
+// Mode ODE at stage `stage` for mode n (Eq. 12 / Eq. 19): ka_s = -(i w + kappa) a_s + i G S_s with S_s from the
+// reduced overlap sums sred[2n], sred[2n+1]; then the amplitudes / RF weights of the next stage state (stages
+// 2..5), the 5th-order candidate (stage 6) or the mode error (stage 7).  c may point to shared memory.
+template <int stage>
+__device__ __forceinline__ void mode_ode_stage(Ctrl* c, const int n, const double* sred, double* serr) {
+    const double Sre = sred[2 * n] * c->invW[n];
+    const double Sim = -sred[2 * n + 1] * c->invW[n];
+    c->S[n][0] = Sre; c->S[n][1] = Sim;
+    const double are = c->as[stage & 1][n][0], aim = c->as[stage & 1][n][1];
+    const double Gre = c->Gre[n], Gim = c->Gim[n];
+    const double kre = (-c->kappa[n] * are + c->omega[n] * aim) - (Gre * Sim + Gim * Sre);
+    const double kim = (-c->kappa[n] * aim - c->omega[n] * are) + (Gre * Sre - Gim * Sim);
+    c->ka[stage - 1][n][0] = kre; c->ka[stage - 1][n][1] = kim;
+    if constexpr (stage >= 2 && stage <= 5) {
+        mode_stage_state<stage>(c, n);              // a_{s+1}, c^{(s+1)}
+    } else if constexpr (stage == 6) {
+        mode_stage_state<6>(c, n);                  // row 6 = b: the 5th-order candidate
+        c->anew[n][0] = c->as[1][n][0]; c->anew[n][1] = c->as[1][n][1];
+    } else if constexpr (stage == 7) {
+        double ere = 0.0, eim = 0.0;
+#pragma unroll
+        for (int j = 0; j < 7; ++j) { ere += kD[j] * c->ka[j][n][0]; eim += kD[j] * c->ka[j][n][1]; }
+        const double e = fabs(c->h) * sqrt(ere * ere + eim * eim);
+        serr[n] = (e < CUDART_INF) ? e : CUDART_INF;
+    }
+}
+
+// Fixed-order second reduction pass shared by stage_finish and the TMA kernels' deferred finish: warp w of nwarp
+// sums components w, w + nwarp, ...; lane l adds blocks l, l+32, ... in order, then a fixed xor tree.  Two
+// components per warp are in flight at a time.
+__device__ __forceinline__ void reduce_block_partials(const double* partial, const int pstride, const int nsum,
+                                                      const int nblk, const int warp, const int nwarp, const int lane,
+                                                      double* sred) {
+    for (int comp = warp; comp < nsum; comp += 2 * nwarp) {
+        const int comp2 = comp + nwarp;
+        const bool two = comp2 < nsum;
+        const double* p1 = partial + (size_t)comp * pstride;
+        const double* p2 = partial + (size_t)(two ? comp2 : comp) * pstride;
+        double acc1 = 0.0, acc2 = 0.0;
+        for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
+            double v1[8], v2[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const bool in = b0 + 32 * j < nblk;
+                v1[j] = in ? __ldcg(p1 + b0 + 32 * j) : 0.0;
+                v2[j] = (in && two) ? __ldcg(p2 + b0 + 32 * j) : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { acc1 += v1[j]; acc2 += v2[j]; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
+            acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
+        }
+        if (lane == 0) { sred[comp] = acc1; if (two) sred[comp2] = acc2; }
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -175,31 +234,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
         const int idx = tid + k * nthr;
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
-    // pass 2: lane l adds blocks l, l+32, ... in order, then a fixed xor tree; two sums per warp at a time
-    for (int comp = warp; comp < nsum; comp += 2 * nwarp) {
-        const int comp2 = comp + nwarp;
-        const bool two = comp2 < nsum;
-        const double* p1 = A.partial + (size_t)comp * A.pstride;
-        const double* p2 = A.partial + (size_t)(two ? comp2 : comp) * A.pstride;
-        double acc1 = 0.0, acc2 = 0.0;
-        for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
-            double v1[8], v2[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const bool in = b0 + 32 * j < nblk;
-                v1[j] = in ? __ldcg(p1 + b0 + 32 * j) : 0.0;
-                v2[j] = (in && two) ? __ldcg(p2 + b0 + 32 * j) : 0.0;
-            }
-#pragma unroll
-            for (int j = 0; j < 8; ++j) { acc1 += v1[j]; acc2 += v2[j]; }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
-            acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
-        }
-        if (lane == 0) { sred[comp] = acc1; if (two) sred[comp2] = acc2; }
-    }
+    reduce_block_partials(A.partial, A.pstride, nsum, nblk, warp, nwarp, lane, sred);
     if (stage == 7 && warp == nwarp - 1) {
         double mx = 0.0;
         for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
@@ -221,30 +256,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
     __syncthreads();
     CAVMAG_MARKF(9);
 
-    // mode ODE at this stage: ka_s = -(i w + kappa) a_s + i G S_s     (Eq. 12 / Eq. 19)
-    if (tid < N) {
-        const int n = tid;
-        const double Sre = sred[2 * n] * c->invW[n];
-        const double Sim = -sred[2 * n + 1] * c->invW[n];
-        c->S[n][0] = Sre; c->S[n][1] = Sim;
-        const double are = c->as[n][0], aim = c->as[n][1];
-        const double Gre = c->Gre[n], Gim = c->Gim[n];
-        const double kre = (-c->kappa[n] * are + c->omega[n] * aim) - (Gre * Sim + Gim * Sre);
-        const double kim = (-c->kappa[n] * aim - c->omega[n] * are) + (Gre * Sre - Gim * Sim);
-        c->ka[stage - 1][n][0] = kre; c->ka[stage - 1][n][1] = kim;
-        if constexpr (stage >= 2 && stage <= 5) {
-            mode_stage_state<stage>(c, n);              // a_{s+1}, c^{(s+1)}
-        } else if constexpr (stage == 6) {
-            mode_stage_state<6>(c, n);                  // row 6 = b: the 5th-order candidate
-            c->anew[n][0] = c->as[n][0]; c->anew[n][1] = c->as[n][1];
-        } else if constexpr (stage == 7) {
-            double ere = 0.0, eim = 0.0;
-#pragma unroll
-            for (int j = 0; j < 7; ++j) { ere += kD[j] * c->ka[j][n][0]; eim += kD[j] * c->ka[j][n][1]; }
-            const double e = fabs(c->h) * sqrt(ere * ere + eim * eim);
-            serr[n] = (e < CUDART_INF) ? e : CUDART_INF;
-        }
-    }
+    if (tid < N) mode_ode_stage<stage>(c, tid, sred, serr);
     bool set_cond = false;
     if (stage >= 2 && stage <= 6) {
         if (tid == 0) { c->rhs_evals++; c->arrive = 0u; }

@@ -115,6 +115,47 @@ template <int STAGE> struct StageStreams {
     static constexpr int n_aux = (STAGE <= 2) ? 0 : (STAGE == 7) ? 1 : (STAGE == 6) ? 5 : STAGE;   // y0,k1,.. / e6
 };
 
+// Deferred finish of stage PREV = STAGE-1, run by the consumer warps of EVERY block of the stage-STAGE kernel while
+// the producer warp is already filling the rings: the fixed-order sum of the previous kernel's block partials, the
+// mode ODE ka_PREV (Eq. 12 / Eq. 19) and the amplitudes / RF weights c_n of this stage.  All blocks compute the
+// same bits from the same inputs; block 0 alone writes the results back to Ctrl.  This replaces the "last block
+// to arrive" tail of stages 2..6 (an atomic ticket, two fences and ~4 dependent L2 round trips with 147 SMs
+// idle) by work that overlaps the pipeline fill.  Fields written by block 0 (S, ka[PREV-1], as[(PREV+1)&1], c,
+// anew, rhs_evals) are never inputs of another block in the same kernel.
+static_assert(kCtrlWords <= 4 * kTmaConsumers, "deferred finish copies Ctrl with 4 words per consumer thread");
+
+template <int PREV>
+__device__ __forceinline__ void deferred_finish(const StageArgs& A, Ctrl* __restrict__ gctrl, const int N, const int tidc,
+                                                unsigned long long* sc_words, double* sred) {
+    const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(gctrl);
+    unsigned long long cw[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int idx = tidc + k * kTmaConsumers;
+        cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
+    }
+    reduce_block_partials(A.partial, A.pstride, 2 * N, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int idx = tidc + k * kTmaConsumers;
+        if (idx < kCtrlWords) sc_words[idx] = cw[k];
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+    Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
+    if (tidc < N) {
+        const int n = tidc;
+        mode_ode_stage<PREV>(c, n, sred, nullptr);
+        if (blockIdx.x == 0) {
+            constexpr int nxt = (PREV + 1) & 1;
+            gctrl->S[n][0] = c->S[n][0]; gctrl->S[n][1] = c->S[n][1];
+            gctrl->ka[PREV - 1][n][0] = c->ka[PREV - 1][n][0]; gctrl->ka[PREV - 1][n][1] = c->ka[PREV - 1][n][1];
+            gctrl->as[nxt][n][0] = c->as[nxt][n][0]; gctrl->as[nxt][n][1] = c->as[nxt][n][1];
+            gctrl->c[n] = c->c[n];
+            if constexpr (PREV == 6) { gctrl->anew[n][0] = c->anew[n][0]; gctrl->anew[n][1] = c->anew[n][1]; }
+        }
+    }
+}
+
 template <typename T, int STAGE, int NSUB, int NB>
 __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A, const TmaArgs TA, double* __restrict__ trace) {
     constexpr int VEC = 8 / (int)sizeof(T);              // cells per lane: 2 floats / 1 double
@@ -166,8 +207,13 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     if (STAGE == 1) { if (ctrl->k1_valid) return; }
     else if (ctrl->done) return;
     const int N = ctrl->N;
-    if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)ctrl->c[tid] : (T)0;
-    __syncthreads();
+    constexpr bool kDeferred = STAGE >= 3;      // this kernel first finishes stage STAGE-1 (see deferred_finish)
+    __shared__ __align__(16) unsigned long long s_ctrl[kDeferred && NB > 0 ? kCtrlWords : 1];
+    __shared__ double s_red[kDeferred && NB > 0 ? 2 * NB : 1];
+    if constexpr (!kDeferred) {
+        if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)ctrl->c[tid] : (T)0;
+        __syncthreads();
+    }
     if (tid == 0) CAVMAG_MARK(1);
 
     // this CTA's run of plane-tiles; tile coordinates are advanced incrementally (no divisions in the loops)
@@ -248,6 +294,14 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         }
     } else {
         // ================================ consumers =================================
+        if constexpr (kDeferred) {
+            if constexpr (NB > 0) {
+                deferred_finish<STAGE - 1>(A, ctrl, N, tid, s_ctrl, s_red);
+                if (tid < NB) s_cn[tid] = (tid < N) ? (T)reinterpret_cast<const Ctrl*>(s_ctrl)->c[tid] : (T)0;
+                asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+            }
+            if (blockIdx.x == 0 && tid == 0) ctrl->rhs_evals = ctrl->rhs_evals + 1;
+        }
         const T h = (T)ctrl->h;
         const T ha21 = h * (T)kA[1][0];
         const T B0x = (T)A.B0[0], B0y = (T)A.B0[1], B0z = (T)A.B0[2];
@@ -583,25 +637,33 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         }
     }
 
-    // ---- last-block-done: second reduction pass, mode ODEs, controller ----
-    // One fence per block: the barrier orders every thread's stores before thread 0's gpu-scope fence (release),
-    // the last block's thread 0 fences again after the ticket (acquire) before the barrier that lets its
-    // threads read the other blocks' partials.
-    __shared__ int s_last;
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        CAVMAG_MARK(4);
-        const unsigned int old = atomicAdd(&ctrl->arrive, 1u);
-        s_last = (old == gridDim.x - 1) ? 1 : 0;
-        if (s_last) __threadfence();
-    }
-    __syncthreads();
-    if (s_last) stage_finish<STAGE>(finish_args(A), NSUB, N, trace);
+    // ---- stages 1 and 7: last-block-done -> second reduction pass, mode ODE, controller.  Stages 2..6 end
+    //      here: their finish runs in the prologue of the next stage kernel (deferred_finish). ----
+    if constexpr (STAGE == 1 || STAGE == 7) {
+        // One fence per block: the barrier orders every thread's stores before thread 0's gpu-scope fence
+        // (release); the last block's thread 0 fences again after the ticket (acquire) before the barrier that
+        // lets its threads read the other blocks' partials.
+        __shared__ int s_last;
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            CAVMAG_MARK(4);
+            const unsigned int old = atomicAdd(&ctrl->arrive, 1u);
+            s_last = (old == gridDim.x - 1) ? 1 : 0;
+            if (s_last) __threadfence();
+        }
+        __syncthreads();
+        if (s_last) stage_finish<STAGE>(finish_args(A), NSUB, N, trace);
 #ifdef CAVMAG_PROBE
-    __syncthreads();
-    if (tid == 0) { CAVMAG_MARK(5); A.probe[((size_t)STAGE * gridDim.x + blockIdx.x) * 32 + 7] = (unsigned long long)s_last; }
+        __syncthreads();
+        if (tid == 0) { CAVMAG_MARK(5); A.probe[((size_t)STAGE * gridDim.x + blockIdx.x) * 32 + 7] = (unsigned long long)s_last; }
 #endif
+    } else {
+#ifdef CAVMAG_PROBE
+        __syncthreads();
+        if (tid == 0) { CAVMAG_MARK(4); CAVMAG_MARK(5); }
+#endif
+    }
 }
 
 const void* stage_tma_kernel_f32_fm(int stage, int nb);
