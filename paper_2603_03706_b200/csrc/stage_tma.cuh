@@ -124,9 +124,11 @@ template <int STAGE> struct StageStreams {
 // anew, rhs_evals) are never inputs of another block in the same kernel.
 static_assert(kCtrlWords <= 4 * kTmaConsumers, "deferred finish copies Ctrl with 4 words per consumer thread");
 
-template <int PREV>
-__device__ __forceinline__ void deferred_finish(const StageArgs& A, Ctrl* __restrict__ gctrl, const int N, const int tidc,
+template <int PREV, int NB>
+__device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __restrict__ gctrl, const int tidc,
                                                 unsigned long long* sc_words, double* sred) {
+    // one batch of independent loads: the whole Ctrl (4 words per thread) and all 2*NB x gridDim block partials
+    // (rows of modes >= N hold stale values that nothing reads)
     const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(gctrl);
     unsigned long long cw[4];
 #pragma unroll
@@ -134,7 +136,7 @@ __device__ __forceinline__ void deferred_finish(const StageArgs& A, Ctrl* __rest
         const int idx = tidc + k * kTmaConsumers;
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
-    reduce_block_partials(A.partial, A.pstride, 2 * N, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
+    reduce_block_partials(A.partial, A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const int idx = tidc + k * kTmaConsumers;
@@ -142,7 +144,8 @@ __device__ __forceinline__ void deferred_finish(const StageArgs& A, Ctrl* __rest
     }
     asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
     Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
-    if (tidc < N) {
+    if (c->done) return false;                      // launched after the run ended (host-enqueued mode): nothing to do
+    if (tidc < c->N) {
         const int n = tidc;
         mode_ode_stage<PREV>(c, n, sred, nullptr);
         if (blockIdx.x == 0) {
@@ -154,6 +157,7 @@ __device__ __forceinline__ void deferred_finish(const StageArgs& A, Ctrl* __rest
             if constexpr (PREV == 6) { gctrl->anew[n][0] = c->anew[n][0]; gctrl->anew[n][1] = c->anew[n][1]; }
         }
     }
+    return true;
 }
 
 template <typename T, int STAGE, int NSUB, int NB>
@@ -204,29 +208,29 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
 
-    if (STAGE == 1) { if (ctrl->k1_valid) return; }
-    else if (ctrl->done) return;
-    const int N = ctrl->N;
     constexpr bool kDeferred = STAGE >= 3;      // this kernel first finishes stage STAGE-1 (see deferred_finish)
     __shared__ __align__(16) unsigned long long s_ctrl[kDeferred && NB > 0 ? kCtrlWords : 1];
     __shared__ double s_red[kDeferred && NB > 0 ? 2 * NB : 1];
-    if constexpr (!kDeferred) {
-        if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)ctrl->c[tid] : (T)0;
-        __syncthreads();
-    }
-    if (tid == 0) CAVMAG_MARK(1);
 
     // this CTA's run of plane-tiles; tile coordinates are advanced incrementally (no divisions in the loops)
     const long long q0 = (TA.Q * (long long)blockIdx.x) / gridDim.x;
     const long long q1 = (TA.Q * (long long)(blockIdx.x + 1)) / gridDim.x;
     const int nplanes = (int)(q1 - q0);
-    const int ycur = ctrl->ycur, k1slot = ctrl->k1slot;
     const long long t0 = q0 / nz;
     const int z0 = (int)(q0 - t0 * nz);
     const int tx0 = (int)(t0 % TA.ntx), ty0 = (int)(t0 / TA.ntx);
 
+    // Each role fetches what it needs from Ctrl with ONE batch of independent loads (one L2 round trip after the
+    // dependency wait): the producer four words, the consumers the whole struct or, in stages 1-2, a few fields.
+    int N, ycur, k1slot;
+
     if (warp == kTmaTY) {
         // =============================== TMA producer ===============================
+        {
+            const int done = STAGE == 1 ? ctrl->k1_valid : ctrl->done;
+            N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
+            if (done) return;
+        }
         if (lane == 0 && nplanes > 0) {
             const unsigned char* maps = TA.maps;
             auto mp = [&](int i) { return (const void*)(maps + 128 * i); };
@@ -294,15 +298,27 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         }
     } else {
         // ================================ consumers =================================
-        if constexpr (kDeferred) {
-            if constexpr (NB > 0) {
-                deferred_finish<STAGE - 1>(A, ctrl, N, tid, s_ctrl, s_red);
-                if (tid < NB) s_cn[tid] = (tid < N) ? (T)reinterpret_cast<const Ctrl*>(s_ctrl)->c[tid] : (T)0;
-                asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
-            }
-            if (blockIdx.x == 0 && tid == 0) ctrl->rhs_evals = ctrl->rhs_evals + 1;
+        double hd;
+        if constexpr (kDeferred && NB > 0) {
+            if (!deferred_finish<STAGE - 1, NB>(A, ctrl, tid, s_ctrl, s_red)) return;
+            const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
+            N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot; hd = sc->h;
+            if (tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
+            if (blockIdx.x == 0 && tid == 0) ctrl->rhs_evals = sc->rhs_evals + 1;
+        } else {
+            const int done = STAGE == 1 ? ctrl->k1_valid : ctrl->done;
+            N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot; hd = ctrl->h;
+            double cv = 0.0;
+            long long evals = 0;
+            if (NB > 0 && tid < NB) cv = ctrl->c[tid];
+            if (kDeferred && blockIdx.x == 0 && tid == 0) evals = ctrl->rhs_evals;
+            if (done) return;
+            if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)cv : (T)0;
+            if (kDeferred && blockIdx.x == 0 && tid == 0) ctrl->rhs_evals = evals + 1;     // no modes: nothing else to finish
         }
-        const T h = (T)ctrl->h;
+        asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+        if (tid == 0) CAVMAG_MARK(1);
+        const T h = (T)hd;
         const T ha21 = h * (T)kA[1][0];
         const T B0x = (T)A.B0[0], B0y = (T)A.B0[1], B0z = (T)A.B0[2];
         const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
