@@ -14,7 +14,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcavmag.so")
+# CAVMAG_LIB selects another build of the same library (the profiling build libcavmag_probe.so); there is no fallback.
+LIB_PATH = os.environ.get("CAVMAG_LIB") or os.path.join(_HERE, "libcavmag.so")
 
 CAV_OK = 0
 CAV_E_ARG, CAV_E_STATE, CAV_E_CUDA, CAV_E_NOMEM = -1, -2, -3, -4

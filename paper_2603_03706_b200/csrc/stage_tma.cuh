@@ -203,10 +203,16 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     }
     if (warp == kTmaTY && lane < MAP_COUNT)
         asm volatile("prefetch.tensormap [%0];" ::"l"(TA.maps + 128 * lane) : "memory");
-    // let the next stage kernel be scheduled as SMs drain, then wait for the previous one to have
-    // completed and flushed (both are no-ops without a programmatic dependency)
+    __syncthreads();                            // the barriers are initialised before the producer arms them
+    // Let the next stage kernel be scheduled as SMs drain.  Every thread executes griddepcontrol.wait (the previous
+    // kernel has completed and flushed) before it touches anything that kernel wrote - the consumers at once, the
+    // producer lane after it has prefetched what the previous kernel does NOT write (kPre below).  Both
+    // instructions are no-ops without a programmatic dependency.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // In stages 3..7 the producer reads its control words (written by the previous STEP's stage 7 / k_begin, not by
+    // kernel STAGE-1) and issues the first tiles of the mode profiles and of the aux streams y0, k1..k_{s-2} before the
+    // wait: DRAM is under-used while the previous kernel's slowest blocks finish, and this fill is ~10 % of a stage.
+    constexpr bool kPre = STAGE >= 3;
 
     constexpr bool kDeferred = STAGE >= 3;      // this kernel first finishes stage STAGE-1 (see deferred_finish)
     __shared__ __align__(16) unsigned long long s_ctrl[kDeferred && NB > 0 ? kCtrlWords : 1];
@@ -226,11 +232,13 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 
     if (warp == kTmaTY) {
         // =============================== TMA producer ===============================
+        if constexpr (!kPre) asm volatile("griddepcontrol.wait;" ::: "memory");
         {
             const int done = STAGE == 1 ? ctrl->k1_valid : ctrl->done;
             N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
             if (done) return;
         }
+        if (kPre && !(lane == 0 && nplanes > 0)) asm volatile("griddepcontrol.wait;" ::: "memory");
         if (lane == 0 && nplanes > 0) {
             const unsigned char* maps = TA.maps;
             auto mp = [&](int i) { return (const void*)(maps + 128 * i); };
@@ -257,6 +265,42 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             int z = z0, tx = tx0, ty = ty0;
             int hm = 0, ha = 0, hu = 0;                 // ring heads
             unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
+            int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
+            if constexpr (kPre) {
+                int zz = z0, txx = tx0, tyy = ty0;
+                for (int p = 0; p < nplanes; ++p) {
+                    const bool do_u = NB > 0 && pre_u + NCH <= Du;
+                    const bool do_a = NAUX > 1 && pre_a < Da;
+                    if (!do_u && !do_a) break;
+                    const int x0 = txx * TX, y0 = tyy * kTmaTY;
+                    if constexpr (NB > 0) {
+                        if (do_u) {
+#pragma unroll 1
+                            for (int ch = 0; ch < NCH; ++ch) {
+                                const unsigned bar = full_u + 8 * pre_u;
+                                mbar_expect_tx(bar, u_tx);
+                                tma_load_4d(u_ring + (unsigned)pre_u * u_tx, umap, x0, y0, zz, ch * kTmaUChunk, bar);
+                                ++pre_u;
+                            }
+                        }
+                    }
+                    if constexpr (NAUX > 1) {
+                        if (do_a) {
+                            const unsigned bar = full_aux + 8 * pre_a;
+                            mbar_expect_tx(bar, aux_tx);            // the whole slot; its last field follows after the wait
+                            unsigned dst = aux_ring + (unsigned)pre_a * aux_tx;
+#pragma unroll
+                            for (int f = 0; f < NAUX - 1; ++f) {
+                                tma_load_4d(dst, amap[f], x0, y0, zz, 0, bar);
+                                dst += C * APLANE;
+                            }
+                            ++pre_a;
+                        }
+                    }
+                    if (++zz == nz) { zz = 0; if (++txx == TA.ntx) { txx = 0; ++tyy; } }
+                }
+                asm volatile("griddepcontrol.wait;" ::: "memory");
+            }
             auto issue_ms = [&](int x0, int y0, int zz) {
                 mbar_wait(empty_ms + 8 * hm, pm);
                 const unsigned bar = full_ms + 8 * hm;
@@ -273,22 +317,30 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 if constexpr (NB > 0) {
 #pragma unroll 1
                     for (int ch = 0; ch < NCH; ++ch) {       // mode profiles, UCB per slot (out-of-range modes zero-filled)
-                        mbar_wait(empty_u + 8 * hu, pu);
-                        const unsigned bar = full_u + 8 * hu;
-                        mbar_expect_tx(bar, u_tx);
-                        tma_load_4d(u_ring + (unsigned)hu * u_tx, umap, x0, y0, z, ch * kTmaUChunk, bar);
+                        if (pre_u > 0) { --pre_u; }          // filled before the dependency wait
+                        else {
+                            mbar_wait(empty_u + 8 * hu, pu);
+                            const unsigned bar = full_u + 8 * hu;
+                            mbar_expect_tx(bar, u_tx);
+                            tma_load_4d(u_ring + (unsigned)hu * u_tx, umap, x0, y0, z, ch * kTmaUChunk, bar);
+                        }
                         if (++hu == Du) { hu = 0; pu ^= 1u; }
                     }
                 }
                 if constexpr (NAUX > 0) {
-                    mbar_wait(empty_aux + 8 * ha, pa);
                     const unsigned bar = full_aux + 8 * ha;
-                    mbar_expect_tx(bar, aux_tx);
                     unsigned dst = aux_ring + (unsigned)ha * aux_tx;
+                    if (pre_a > 0) {                          // armed before the dependency wait: only k_{s-1} is missing
+                        --pre_a;
+                        tma_load_4d(dst + (unsigned)((NAUX - 1) * C * APLANE), amap[NAUX - 1], x0, y0, z, 0, bar);
+                    } else {
+                        mbar_wait(empty_aux + 8 * ha, pa);
+                        mbar_expect_tx(bar, aux_tx);
 #pragma unroll
-                    for (int f = 0; f < NAUX; ++f) {
-                        tma_load_4d(dst, amap[f], x0, y0, z, 0, bar);
-                        dst += C * APLANE;
+                        for (int f = 0; f < NAUX; ++f) {
+                            tma_load_4d(dst, amap[f], x0, y0, z, 0, bar);
+                            dst += C * APLANE;
+                        }
                     }
                     if (++ha == Da) { ha = 0; pa ^= 1u; }
                 }
@@ -298,6 +350,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         }
     } else {
         // ================================ consumers =================================
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         double hd;
         if constexpr (kDeferred && NB > 0) {
             if (!deferred_finish<STAGE - 1, NB>(A, ctrl, tid, s_ctrl, s_red)) return;
