@@ -300,6 +300,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     if (++zz == nz) { zz = 0; if (++txx == TA.ntx) { txx = 0; ++tyy; } }
                 }
                 asm volatile("griddepcontrol.wait;" ::: "memory");
+                CAVMAG_MARK(13);
             }
             auto issue_ms = [&](int x0, int y0, int zz) {
                 mbar_wait(empty_ms + 8 * hm, pm);
@@ -351,6 +352,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     } else {
         // ================================ consumers =================================
         asm volatile("griddepcontrol.wait;" ::: "memory");
+        if (tid == 0) CAVMAG_MARK(15);
         double hd;
         if constexpr (kDeferred && NB > 0) {
             if (!deferred_finish<STAGE - 1, NB>(A, ctrl, tid, s_ctrl, s_red)) return;
