@@ -183,6 +183,51 @@ int cav_get_stage_overlap(cav_sim* sim, int* active);
 /* Number of kernels this library has launched for this handle (stage kernels + setup). */
 int cav_get_launch_count(cav_sim* sim, long long* n);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * Batched sweeps of small grids.  The paper's own workloads are parameter sweeps of a tiny grid
+ * (8 x 8 x 1 cells x 41 / 21 field values): independent simulations that differ in B0
+ * and/or the mode parameters.  A batch integrates n_rep such replicas in ONE kernel launch: one thread block per
+ * replica, one thread per cell, the whole adaptive RK45 loop of the same coupled system (same tableau, controller,
+ * error norm and renormalisation as cav_run) inside the kernel with the stage
+ * state in shared memory and the slopes in registers - no kernel launch, no global-memory round trip and no
+ * grid-wide reduction per stage.  Limits: nx*ny*nz <= 1024 cells, N <= CAV_MAX_MODES.
+ * All arrays are HOST arrays copied at the call; replicas are laid out [n_rep][...] with the single-simulation
+ * layouts above.  Not thread-safe per handle.
+ * --------------------------------------------------------------------------------------------------------- */
+typedef struct cav_batch cav_batch; /* opaque */
+
+/* params->B0 is the default static field of every replica.  CAV_E_ARG if the grid has more than 1024 cells. */
+int cav_batch_create(const cav_grid* grid, const cav_params* params, int n_rep, cav_batch** out);
+int cav_batch_destroy(cav_batch* b);
+int cav_batch_set_stream(cav_batch* b, void* cuda_stream);
+
+/* Static field per replica, [n_rep][3] tesla. */
+int cav_batch_set_field(cav_batch* b, const double* B0);
+
+/* Modes: profiles u [N][nz][ny][nx] (batch precision) are common to all replicas; omega, kappa, g, Gamma, Phi are
+ * [N] (per_replica == 0) or [n_rep][N] (per_replica != 0); Gamma, Phi may be NULL.  Zeroes the amplitudes. */
+int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega, const double* kappa,
+                        const double* g, const double* Gamma, const double* Phi, int per_replica);
+
+/* Initial magnetisation [n_sub][3][nz][ny][nx] for all replicas (per_replica == 0) or [n_rep][n_sub][3][nz][ny][nx];
+ * normalised per cell on entry.  Amplitudes [N][2] or [n_rep][N][2]. */
+int cav_batch_set_m(cav_batch* b, const void* m, int per_replica);
+int cav_batch_set_a(cav_batch* b, const double* a_re_im, int per_replica);
+
+/* Trace rows as cav_set_trace, per replica; resets the traces. */
+int cav_batch_set_trace(cav_batch* b, double sample_dt, int capacity);
+int cav_batch_trace_row_len(cav_batch* b, int* row_len);
+
+/* Advance every replica to t_end (or by max_steps attempted steps if max_steps > 0); arguments as cav_run_steps.
+ * Asynchronous on the stream; the cav_batch_get_* calls synchronise. */
+int cav_batch_run(cav_batch* b, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps);
+
+/* Results.  cav_batch_get_stats also returns the first non-zero device status of any replica. */
+int cav_batch_get_m(cav_batch* b, void* m_out /* [n_rep][n_sub][3][nz][ny][nx] */);
+int cav_batch_get_a(cav_batch* b, double* a_out /* [n_rep][N][2] */);
+int cav_batch_get_stats(cav_batch* b, cav_stats* out /* [n_rep] */);
+int cav_batch_get_trace(cav_batch* b, double* out /* [n_rep][capacity][row_len] */, int* n_samples /* [n_rep] */);
+
 const char* cav_strerror(int status);
 const char* cav_last_cuda_error(cav_sim* sim);
 const char* cav_version(void);

@@ -89,6 +89,20 @@ _SIGS = {
     "cav_strerror": ([_i], C.c_char_p),
     "cav_last_cuda_error": ([_vp], C.c_char_p),
     "cav_version": ([], C.c_char_p),
+    "cav_batch_create": ([C.POINTER(cav_grid), C.POINTER(cav_params), _i, C.POINTER(_vp)], _i),
+    "cav_batch_destroy": ([_vp], _i),
+    "cav_batch_set_stream": ([_vp, _vp], _i),
+    "cav_batch_set_field": ([_vp, _dp], _i),
+    "cav_batch_set_modes": ([_vp, _i, _vp, _dp, _dp, _dp, _dp, _dp, _i], _i),
+    "cav_batch_set_m": ([_vp, _vp, _i], _i),
+    "cav_batch_set_a": ([_vp, _dp, _i], _i),
+    "cav_batch_set_trace": ([_vp, _d, _i], _i),
+    "cav_batch_trace_row_len": ([_vp, C.POINTER(_i)], _i),
+    "cav_batch_run": ([_vp, _d, _d, _d, _d, _ll], _i),
+    "cav_batch_get_m": ([_vp, _vp], _i),
+    "cav_batch_get_a": ([_vp, _dp], _i),
+    "cav_batch_get_stats": ([_vp, C.POINTER(cav_stats)], _i),
+    "cav_batch_get_trace": ([_vp, _dp, C.POINTER(_i)], _i),
 }
 for _name, (_args, _res) in _SIGS.items():
     _f = getattr(_lib, _name)
@@ -131,8 +145,7 @@ def _darr(x, n):
     return a.ctypes.data_as(_dp), a
 
 
-def cav_create(grid, params) -> int:
-    """grid = (nx, ny, nz, dx, dy, dz); params = dict with the cav_params fields. Returns the handle."""
+def _grid_params(grid, params):
     g = cav_grid(int(grid[0]), int(grid[1]), int(grid[2]), float(grid[3]), float(grid[4]), float(grid[5]))
     p = cav_params()
     p.Ms, p.Aex, p.Ku = float(params["Ms"]), float(params["Aex"]), float(params.get("Ku", 0.0))
@@ -144,6 +157,12 @@ def cav_create(grid, params) -> int:
     p.precision = int(params.get("precision", CAV_F32))
     p.renormalize = int(params.get("renormalize", 1))
     p.overlap_norm = int(params.get("overlap_norm", CAV_NORM_NCELLS))
+    return g, p
+
+
+def cav_create(grid, params) -> int:
+    """grid = (nx, ny, nz, dx, dy, dz); params = dict with the cav_params fields. Returns the handle."""
+    g, p = _grid_params(grid, params)
     h = _vp()
     _check(_lib.cav_create(C.byref(g), C.byref(p), C.byref(h)), "cav_create")
     return h.value
@@ -353,3 +372,149 @@ class Sim:
 
     def get_a(self) -> np.ndarray:
         return cav_get_a(self.h, self.N)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Batched sweeps of small grids (include/cavmag.h): same names, marshalling only
+# ---------------------------------------------------------------------------------------------------------
+def cav_batch_create(grid, params, n_rep: int) -> int:
+    g, p = _grid_params(grid, params)
+    h = _vp()
+    _check(_lib.cav_batch_create(C.byref(g), C.byref(p), int(n_rep), C.byref(h)), "cav_batch_create")
+    return h.value
+
+
+def cav_batch_destroy(b) -> None:
+    _check(_lib.cav_batch_destroy(b), "cav_batch_destroy")
+
+
+def cav_batch_set_stream(b, cuda_stream: int) -> None:
+    _check(_lib.cav_batch_set_stream(b, _vp(cuda_stream)), "cav_batch_set_stream")
+
+
+def cav_batch_set_field(b, B0) -> None:
+    a = np.ascontiguousarray(np.asarray(B0, dtype=np.float64))
+    _check(_lib.cav_batch_set_field(b, a.ctypes.data_as(_dp)), "cav_batch_set_field")
+
+
+def cav_batch_set_modes(b, u, omega, kappa, g, Gamma=None, Phi=None, per_replica: bool = False) -> None:
+    """u: host array [N][nz][ny][nx] in the batch precision; parameters [N] or [n_rep][N]."""
+    om = np.asarray(omega, dtype=np.float64) if omega is not None else np.zeros(0)
+    N = 0 if om.size == 0 else int(om.shape[-1])
+    if N == 0:
+        _check(_lib.cav_batch_set_modes(b, 0, None, None, None, None, None, None, 0), "cav_batch_set_modes")
+        return
+    n = om.size
+    addr, _, keep = _ptr(u)
+    po, ko = _darr(omega, n)
+    pk, kk = _darr(kappa, n)
+    pg, kg = _darr(g, n)
+    pG, kG = _darr(Gamma, n)
+    pP, kP = _darr(Phi, n)
+    _check(_lib.cav_batch_set_modes(b, N, _vp(addr), po, pk, pg, pG, pP, int(bool(per_replica))), "cav_batch_set_modes")
+
+
+def cav_batch_set_m(b, m: np.ndarray, per_replica: bool = False) -> None:
+    addr, _, keep = _ptr(m)
+    _check(_lib.cav_batch_set_m(b, _vp(addr), int(bool(per_replica))), "cav_batch_set_m")
+
+
+def cav_batch_set_a(b, a, per_replica: bool = False) -> None:
+    arr = np.ascontiguousarray(np.asarray(a, dtype=np.complex128)).view(np.float64)
+    _check(_lib.cav_batch_set_a(b, arr.ctypes.data_as(_dp), int(bool(per_replica))), "cav_batch_set_a")
+
+
+def cav_batch_set_trace(b, sample_dt: float, capacity: int) -> None:
+    _check(_lib.cav_batch_set_trace(b, float(sample_dt), int(capacity)), "cav_batch_set_trace")
+
+
+def cav_batch_trace_row_len(b) -> int:
+    n = _i()
+    _check(_lib.cav_batch_trace_row_len(b, C.byref(n)), "cav_batch_trace_row_len")
+    return n.value
+
+
+def cav_batch_run(b, t_end: float, tol: float = 0.0, fixed_dt: float = 0.0, dt_init: float = 0.0, max_steps: int = 0) -> None:
+    _check(_lib.cav_batch_run(b, float(t_end), float(tol), float(fixed_dt), float(dt_init), int(max_steps)), "cav_batch_run")
+
+
+def cav_batch_get_m(b, out: np.ndarray) -> None:
+    addr, _, keep = _ptr(out)
+    _check(_lib.cav_batch_get_m(b, _vp(addr)), "cav_batch_get_m")
+
+
+def cav_batch_get_a(b, n_rep: int, N: int) -> np.ndarray:
+    out = np.zeros((n_rep, max(N, 0), 2), dtype=np.float64)
+    _check(_lib.cav_batch_get_a(b, out.ctypes.data_as(_dp) if N else None), "cav_batch_get_a")
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def cav_batch_get_stats(b, n_rep: int) -> list:
+    arr = (cav_stats * n_rep)()
+    _check(_lib.cav_batch_get_stats(b, arr), "cav_batch_get_stats")
+    return [{k: getattr(st, k) for k, _ in cav_stats._fields_} for st in arr]
+
+
+def cav_batch_get_trace(b, n_rep: int, capacity: int) -> list:
+    """Per replica: array [n_samples][row_len]."""
+    rl = cav_batch_trace_row_len(b)
+    out = np.zeros((n_rep, max(capacity, 1), rl), dtype=np.float64)
+    ns = (_i * n_rep)()
+    _check(_lib.cav_batch_get_trace(b, out.ctypes.data_as(_dp) if capacity > 0 else None, ns), "cav_batch_get_trace")
+    return [out[r, :ns[r]].copy() for r in range(n_rep)]
+
+
+class Batch:
+    """RAII wrapper around a cav_batch handle: n_rep replicas of workload w that differ in B0 (and optionally in the
+    mode parameters)."""
+
+    def __init__(self, w, n_rep: int, precision: str = "f64", B0=None, renormalize: bool = True,
+                 overlap_norm: int = CAV_NORM_NCELLS, stream: int | None = None):
+        self.np_dtype = np.float32 if precision == "f32" else np.float64
+        self.n_rep, self.N, self.n_sub = int(n_rep), int(np.asarray(w.omega).size), int(w.n_sub)
+        self.shape_m = (self.n_rep, self.n_sub, 3, w.nz, w.ny, w.nx)
+        self.h = cav_batch_create((w.nx, w.ny, w.nz, w.dx, w.dy, w.dz),
+                                  dict(Ms=w.Ms, Aex=w.Aex, Ku=w.Ku, ku_axis=w.ku_axis, alpha=w.alpha, gamma=w.gamma,
+                                       B0=w.B0, n_sub=w.n_sub, B_exch_inter=w.B_exch_inter,
+                                       precision=CAV_F32 if precision == "f32" else CAV_F64,
+                                       renormalize=int(renormalize), overlap_norm=overlap_norm), n_rep)
+        if stream is not None:
+            cav_batch_set_stream(self.h, stream)
+        if B0 is not None:
+            cav_batch_set_field(self.h, B0)
+        if self.N:
+            cav_batch_set_modes(self.h, np.ascontiguousarray(w.u, dtype=self.np_dtype), w.omega, w.kappa, w.g, w.Gamma, w.Phi)
+        cav_batch_set_m(self.h, np.ascontiguousarray(w.m0, dtype=self.np_dtype))
+        if self.N:
+            cav_batch_set_a(self.h, w.a0)
+
+    def close(self):
+        if self.h:
+            cav_batch_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def run(self, t_end, tol=0.0, fixed_dt=0.0, dt_init=0.0, max_steps=0):
+        cav_batch_run(self.h, t_end, tol, fixed_dt, dt_init, max_steps)
+
+    def get_m(self) -> np.ndarray:
+        out = np.empty(self.shape_m, dtype=self.np_dtype)
+        cav_batch_get_m(self.h, out)
+        return out
+
+    def get_a(self) -> np.ndarray:
+        return cav_batch_get_a(self.h, self.n_rep, self.N)
+
+    def stats(self) -> list:
+        return cav_batch_get_stats(self.h, self.n_rep)

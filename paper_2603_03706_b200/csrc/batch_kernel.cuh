@@ -1,0 +1,382 @@
+// Batched small-grid integrator (SURVEY.md 8(f1); PAPER.md:217, :229, :335 - the paper's sweeps of a tiny grid).
+//
+// One thread block per replica, one thread per cell.  The whole adaptive Dormand-Prince loop of the coupled
+// LLG + cavity-mode system runs inside the kernel:
+//   * the stage state m_s lives in shared memory (neighbours of the 6-point exchange stencil are shared-memory
+//     reads), y, k1..k7 and the candidate of a thread's own cell live in registers;
+//   * per evaluation: publish m_s, barrier, [field + LLG slope of the own cell] and [warp-shuffle partial sums of
+//     u_n m_c^-], barrier, thread n finishes S_n, the mode ODE ka_s (Eq. 12 / Eq. 19) and the amplitudes / RF
+//     weights of the next stage state -> 2 block barriers per evaluation, no global memory, no kernel launch;
+//   * error norm, accept/reject, dt control, FSAL and trace sampling as in stage_finish<7> (same formulas, same
+//     constants: DESIGN.md readings G11-G13).
+// Same arithmetic per cell as k_stage (subtract-first exchange stencil, explicit Landau-Lifshitz form), so a
+// replica agrees with cav_run on the same inputs to rounding; the overlap sums are added in a different (fixed)
+// order.  Mode amplitudes, overlap sums and the controller are fp64 in both precisions.
+#pragma once
+#include <type_traits>
+
+#include "stage_kernel.cuh"
+
+namespace cavmag {
+
+constexpr int kBatchMaxCells = 1024;
+
+struct BatchCtl {                 // per replica, persistent across cav_batch_run calls
+    double t, dt;
+    double dt_min, dt_max, last_err;
+    long long accepted, rejected, rhs_evals, trace_acc0;
+    int status, trace_n;
+};
+
+struct BatchArgs {
+    int nx, ny, nz, nc, N, n_rep;
+    double ex_wx, ex_wy, ex_wz, an_pref, axis[3], alpha, llg, B_exch_inter, two_over_gamma, inv_nc;
+    int renormalize;
+    const double* B0;             // [n_rep][3]
+    const void* u;                // [N][nc] T
+    const double* modep;          // [n_rep or 1][5][N]: omega, kappa, Gre, Gim, invW
+    int modep_per_rep;
+    void* m;                      // [n_rep][NSUB][3][nc] T, in/out
+    double* a;                    // [n_rep][N][2], in/out
+    BatchCtl* ctl;                // [n_rep]
+    double t_end, tol, fixed_dt, dt_init;
+    long long max_steps;
+    double sample_dt, trace_t0;
+    int trace_cap, row_len;
+    double* trace;                // [n_rep][trace_cap][row_len]
+    int u_in_smem;                // profiles staged in dynamic shared memory
+};
+
+// Shared mode / controller state of one replica.
+struct BatchShared {
+    double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes];
+    double a[kMaxModes][2], as[kMaxModes][2], anew[kMaxModes][2], ka[7][kMaxModes][2], S[kMaxModes][2];
+    double c[kMaxModes], serr[kMaxModes];
+    double part[32][2 * kMaxModes + 6];     // per-warp partial sums: overlaps (2N) then <m_s> (3 n_sub)
+    double wmax[32];
+    double red[2 * kMaxModes + 6];
+    double t, dt, h, target, err;
+    long long steps;
+    int clamped, sample_hit, accept, done, status, trace_n;
+    long long accepted, rejected, rhs_evals, trace_stride, trace_acc0;
+    double dt_min, dt_max;
+};
+
+template <int ROW>
+__device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, const double two_over_gamma) {
+    double re = 0.0, im = 0.0;
+#pragma unroll
+    for (int j = 0; j < ROW; ++j) { re += kA[ROW][j] * sh.ka[j][n][0]; im += kA[ROW][j] * sh.ka[j][n][1]; }
+    const double are = sh.a[n][0] + sh.h * re, aim = sh.a[n][1] + sh.h * im;
+    sh.as[n][0] = are; sh.as[n][1] = aim;
+    sh.c[n] = two_over_gamma * (sh.Gre[n] * are - sh.Gim[n] * aim);
+}
+
+
+// MAXT: block-size bucket (128 / 256 / 512 / 1024 threads) - the register budget per thread follows from it.
+template <typename T, int NSUB, int MAXT>
+__global__ void __launch_bounds__(MAXT) k_batch(const BatchArgs A) {
+    extern __shared__ __align__(16) unsigned char batch_dsm[];
+    __shared__ BatchShared sh;
+    const int nc = A.nc, N = A.N;
+    T* const sm_m = reinterpret_cast<T*>(batch_dsm);                 // [NSUB*3][nc] stage state
+    T* const sm_u = sm_m + (size_t)NSUB * 3 * nc;                     // [N][nc] profiles (if u_in_smem)
+    const int rep = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+    const bool active = tid < nc;
+    const int cell = active ? tid : nc - 1;
+    const int x = cell % A.nx, yy = (cell / A.nx) % A.ny, z = cell / (A.nx * A.ny);
+
+    // open boundary (G9): an out-of-grid neighbour gets weight 0 and the centre's index
+    const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
+    const int ixm = x > 0 ? cell - 1 : cell, ixp = x < A.nx - 1 ? cell + 1 : cell;
+    const int iym = yy > 0 ? cell - A.nx : cell, iyp = yy < A.ny - 1 ? cell + A.nx : cell;
+    const int izm = z > 0 ? cell - A.nx * A.ny : cell, izp = z < A.nz - 1 ? cell + A.nx * A.ny : cell;
+    const T wxm = x > 0 ? wx : (T)0, wxp = x < A.nx - 1 ? wx : (T)0;
+    const T wym = yy > 0 ? wy : (T)0, wyp = yy < A.ny - 1 ? wy : (T)0;
+    const T wzm = z > 0 ? wz : (T)0, wzp = z < A.nz - 1 ? wz : (T)0;
+
+    const T B0x = (T)A.B0[rep * 3 + 0], B0y = (T)A.B0[rep * 3 + 1], B0z = (T)A.B0[rep * 3 + 2];
+    const T anp = (T)A.an_pref, axx = (T)A.axis[0], axy = (T)A.axis[1], axz = (T)A.axis[2];
+    const T alpha = (T)A.alpha, llg = (T)A.llg, BE = (T)A.B_exch_inter;
+    const T* __restrict__ ug = reinterpret_cast<const T*>(A.u);
+    T* __restrict__ mg = reinterpret_cast<T*>(A.m) + (size_t)rep * NSUB * 3 * nc;
+
+    // ---- load the replica ----
+    T y[NSUB][3];
+#pragma unroll
+    for (int s = 0; s < NSUB; ++s)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) y[s][c] = mg[(size_t)(s * 3 + c) * nc + cell];
+    if (A.u_in_smem)
+        for (int i = tid; i < N * nc; i += blockDim.x) sm_u[i] = ug[i];
+    if (tid < N) {
+        const double* mp = A.modep + (A.modep_per_rep ? (size_t)rep * 5 * N : 0);
+        sh.omega[tid] = mp[tid]; sh.kappa[tid] = mp[N + tid]; sh.Gre[tid] = mp[2 * N + tid];
+        sh.Gim[tid] = mp[3 * N + tid]; sh.invW[tid] = mp[4 * N + tid];
+        const double are = A.a[((size_t)rep * N + tid) * 2], aim = A.a[((size_t)rep * N + tid) * 2 + 1];
+        sh.a[tid][0] = are; sh.a[tid][1] = aim;
+        sh.as[tid][0] = are; sh.as[tid][1] = aim;                       // stage 1 evaluates f(m_0, a_0)
+        sh.c[tid] = A.two_over_gamma * (sh.Gre[tid] * are - sh.Gim[tid] * aim);
+    }
+    if (tid == 0) {
+        const BatchCtl& cl = A.ctl[rep];
+        sh.t = cl.t; sh.dt_min = cl.dt_min; sh.dt_max = cl.dt_max; sh.err = cl.last_err;
+        sh.accepted = cl.accepted; sh.rejected = cl.rejected; sh.rhs_evals = cl.rhs_evals; sh.trace_acc0 = cl.trace_acc0;
+        sh.status = cl.status; sh.trace_n = cl.trace_n; sh.steps = 0;
+        const bool adaptive = A.tol > 0.0;
+        if (adaptive) sh.dt = A.dt_init > 0.0 ? A.dt_init : (cl.dt > 0.0 ? cl.dt : 1e-14);
+        else {
+            sh.dt = A.fixed_dt;
+            const long long st = llround(A.sample_dt / A.fixed_dt);
+            sh.trace_stride = st < 1 ? 1 : st;
+        }
+    }
+    __syncthreads();
+    const T* __restrict__ up = A.u_in_smem ? sm_u : ug;
+
+    // ---- one evaluation of the coupled right-hand side at stage s (1..7): slope k of the own cell, and in
+    //      thread n the mode slope ka_s and the amplitudes / RF weights of the next stage state ----
+    auto eval = [&](auto stage_tag, const T (&ms)[NSUB][3], T (&k)[NSUB][3]) {
+        constexpr int s = decltype(stage_tag)::value;
+        if (active) {
+#pragma unroll
+            for (int q = 0; q < NSUB; ++q)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) sm_m[(size_t)(q * 3 + c) * nc + cell] = ms[q][c];
+        }
+        __syncthreads();                                             // [A] stage state and c_n published
+        T mcx, mcy;
+        if constexpr (NSUB == 1) { mcx = ms[0][0]; mcy = ms[0][1]; }
+        else { mcx = (T)0.5 * (ms[0][0] + ms[1][0]); mcy = (T)0.5 * (ms[0][1] + ms[1][1]); }
+        T brf = (T)0;
+        for (int n = 0; n < N; ++n) {
+            const T un = up[(size_t)n * nc + cell];
+            brf += (T)sh.c[n] * un;
+            double px = active ? (double)(un * mcx) : 0.0, py = active ? (double)(un * mcy) : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                px += __shfl_xor_sync(0xffffffffu, px, o);
+                py += __shfl_xor_sync(0xffffffffu, py, o);
+            }
+            if (lane == 0) { sh.part[warp][2 * n] = px; sh.part[warp][2 * n + 1] = py; }
+        }
+        if constexpr (s == 7) {                                      // <m_s> of the candidate, for the trace
+#pragma unroll
+            for (int i = 0; i < 3 * NSUB; ++i) {
+                double v = active ? (double)ms[i / 3][i % 3] : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0) sh.part[warp][2 * N + i] = v;
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q) {
+            T lap[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const T* f = sm_m + (size_t)(q * 3 + c) * nc;
+                const T m0 = ms[q][c];
+                T l = (f[ixm] - m0) * wxm;
+                l += (f[ixp] - m0) * wxp;
+                l += (f[iym] - m0) * wym;
+                l += (f[iyp] - m0) * wyp;
+                l += (f[izm] - m0) * wzm;
+                l += (f[izp] - m0) * wzp;
+                lap[c] = l;
+            }
+            const T mx = ms[q][0], my = ms[q][1], mz = ms[q][2];
+            const T mk = mx * axx + my * axy + mz * axz;
+            T Bx = B0x + lap[0] + anp * mk * axx + brf;
+            T By = B0y + lap[1] + anp * mk * axy;
+            T Bz = B0z + lap[2] + anp * mk * axz;
+            if constexpr (NSUB == 2) { Bx -= BE * ms[1 - q][0]; By -= BE * ms[1 - q][1]; Bz -= BE * ms[1 - q][2]; }
+            const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
+            const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
+            k[q][0] = llg * (tx + alpha * dx);
+            k[q][1] = llg * (ty + alpha * dy);
+            k[q][2] = llg * (tz + alpha * dz);
+        }
+        __syncthreads();                                             // [B] warp partials published, sm_m free again
+        if (tid < N) {
+            const int n = tid;
+            double sx = 0.0, sy = 0.0;
+            for (int w = 0; w < nwarp; ++w) { sx += sh.part[w][2 * n]; sy += sh.part[w][2 * n + 1]; }
+            const double Sre = sx * sh.invW[n], Sim = -sy * sh.invW[n];
+            sh.S[n][0] = Sre; sh.S[n][1] = Sim;
+            const double are = sh.as[n][0], aim = sh.as[n][1];
+            const double Gre = sh.Gre[n], Gim = sh.Gim[n];
+            sh.ka[s - 1][n][0] = (-sh.kappa[n] * are + sh.omega[n] * aim) - (Gre * Sim + Gim * Sre);
+            sh.ka[s - 1][n][1] = (-sh.kappa[n] * aim - sh.omega[n] * are) + (Gre * Sre - Gim * Sim);
+            if constexpr (s >= 2 && s <= 5) batch_stage_state<s>(sh, n, A.two_over_gamma);
+            else if constexpr (s == 6) {
+                batch_stage_state<6>(sh, n, A.two_over_gamma);       // row 6 = b: the 5th-order candidate
+                sh.anew[n][0] = sh.as[n][0]; sh.anew[n][1] = sh.as[n][1];
+            } else if constexpr (s == 7) {
+                double ere = 0.0, eim = 0.0;
+#pragma unroll
+                for (int j = 0; j < 7; ++j) { ere += kD[j] * sh.ka[j][n][0]; eim += kD[j] * sh.ka[j][n][1]; }
+                const double e = fabs(sh.h) * sqrt(ere * ere + eim * eim);
+                sh.serr[n] = (e < CUDART_INF) ? e : CUDART_INF;
+            }
+        } else if (s == 7 && tid >= 32 && tid < 32 + 3 * NSUB) {     // a second warp sums <m_s>
+            const int i = tid - 32;
+            double v = 0.0;
+            for (int w = 0; w < nwarp; ++w) v += sh.part[w][2 * N + i];
+            sh.red[i] = v * A.inv_nc;
+        }
+        if (tid == 0) sh.rhs_evals++;
+    };
+
+
+    // ---- k1 of the loaded state ----
+    T k1[NSUB][3], k2[NSUB][3], k3[NSUB][3], k4[NSUB][3], k5[NSUB][3], k6[NSUB][3], k7[NSUB][3], ms[NSUB][3], yn[NSUB][3];
+    eval(std::integral_constant<int, 1>{}, y, k1);
+    const bool adaptive = A.tol > 0.0;
+
+    for (;;) {
+        // ---- start of a step (thread 0): anything left to do?  h for this step (prepare_h in stage_kernel.cuh) ----
+        if (tid == 0) {
+            const bool done = !(sh.t < A.t_end) || (A.max_steps > 0 && sh.steps >= A.max_steps) || sh.status != 0;
+            sh.done = done ? 1 : 0;
+            double h = sh.dt, target = A.t_end;
+            int sample_hit = 0;
+            if (adaptive && A.sample_dt > 0.0 && sh.trace_n < A.trace_cap) {
+                const double ts = A.trace_t0 + (double)(sh.trace_n + 1) * A.sample_dt;
+                if (ts <= target) { target = ts; sample_hit = 1; }
+            }
+            int clamped = 0;
+            if (sh.t + h * (1.0 + 1e-12) >= target) { h = target - sh.t; clamped = 1; }
+            sh.h = h; sh.target = target; sh.clamped = clamped; sh.sample_hit = sample_hit;
+        }
+        __syncthreads();
+        if (sh.done) break;
+        if (tid < N) batch_stage_state<1>(sh, tid, A.two_over_gamma);      // a_2 = a_0 + h a21 ka_1
+        const T h = (T)sh.h;
+
+#define CAVMAG_BATCH_STAGE(S, EXPR)                                                        \
+        _Pragma("unroll") for (int q = 0; q < NSUB; ++q)                                   \
+        _Pragma("unroll") for (int c = 0; c < 3; ++c) ms[q][c] = y[q][c] + h * (EXPR);
+        CAVMAG_BATCH_STAGE(2, (T)kA[1][0] * k1[q][c])
+        eval(std::integral_constant<int, 2>{}, ms, k2);
+        CAVMAG_BATCH_STAGE(3, ((T)kA[2][0] * k1[q][c] + (T)kA[2][1] * k2[q][c]))
+        eval(std::integral_constant<int, 3>{}, ms, k3);
+        CAVMAG_BATCH_STAGE(4, (((T)kA[3][0] * k1[q][c] + (T)kA[3][1] * k2[q][c]) + (T)kA[3][2] * k3[q][c]))
+        eval(std::integral_constant<int, 4>{}, ms, k4);
+        CAVMAG_BATCH_STAGE(5, ((((T)kA[4][0] * k1[q][c] + (T)kA[4][1] * k2[q][c]) + (T)kA[4][2] * k3[q][c]) + (T)kA[4][3] * k4[q][c]))
+        eval(std::integral_constant<int, 5>{}, ms, k5);
+        CAVMAG_BATCH_STAGE(6, (((((T)kA[5][0] * k1[q][c] + (T)kA[5][1] * k2[q][c]) + (T)kA[5][2] * k3[q][c]) + (T)kA[5][3] * k4[q][c]) + (T)kA[5][4] * k5[q][c]))
+        eval(std::integral_constant<int, 6>{}, ms, k6);
+#undef CAVMAG_BATCH_STAGE
+
+        // ---- 5th-order candidate, renormalised per cell (G13), 7th evaluation, error (G12) ----
+        T e2max = (T)0;
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q) {
+            T er[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                T acc = (T)kA[6][0] * k1[q][c];
+                acc += (T)kA[6][2] * k3[q][c];
+                acc += (T)kA[6][3] * k4[q][c];
+                acc += (T)kA[6][4] * k5[q][c];
+                acc += (T)kA[6][5] * k6[q][c];
+                yn[q][c] = y[q][c] + h * acc;
+                T e = (T)kD[0] * k1[q][c];
+                e += (T)kD[2] * k3[q][c];
+                e += (T)kD[3] * k4[q][c];
+                e += (T)kD[4] * k5[q][c];
+                e += (T)kD[5] * k6[q][c];
+                er[c] = h * e;
+            }
+            if (A.renormalize) {
+                const T inv = rsqrt_t<T>(yn[q][0] * yn[q][0] + yn[q][1] * yn[q][1] + yn[q][2] * yn[q][2]);
+                yn[q][0] *= inv; yn[q][1] *= inv; yn[q][2] *= inv;
+            }
+            k6[q][0] = er[0]; k6[q][1] = er[1]; k6[q][2] = er[2];      // k6 is dead: keep the partial error there
+        }
+        eval(std::integral_constant<int, 7>{}, yn, k7);
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q) {
+            const T hd7 = h * (T)kD[6];
+            const T ex = k6[q][0] + hd7 * k7[q][0], ey = k6[q][1] + hd7 * k7[q][1], ez = k6[q][2] + hd7 * k7[q][2];
+            T e2 = ex * ex + ey * ey + ez * ez;
+            e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;               // NaN -> +inf so that max propagates it
+            if (active) e2max = fmax(e2max, e2);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e2max = fmax(e2max, __shfl_xor_sync(0xffffffffu, e2max, o));
+        if (lane == 0) sh.wmax[warp] = (double)e2max;
+        __syncthreads();                                                 // [C]
+
+        // ---- controller (stage_finish<7> in stage_kernel.cuh, same constants) ----
+        if (tid == 0) {
+            double mx = 0.0;
+            for (int w = 0; w < nwarp; ++w) mx = fmax(mx, sh.wmax[w]);
+            double err = sqrt(mx);
+            for (int n = 0; n < N; ++n) err = fmax(err, sh.serr[n]);
+            const bool finite = err < CUDART_INF;
+            const double hh = sh.h;
+            bool accept;
+            if (adaptive) accept = finite && err <= A.tol;
+            else { accept = true; if (!finite) { accept = false; sh.status = -5; } }
+            double fac;
+            if (!finite) fac = 0.5;
+            else if (err == 0.0) fac = 2.0;
+            else { fac = 0.8 * fifth_root(fmin(fmax(A.tol / err, 1e-2), 1e3)); fac = fmin(fmax(fac, 0.5), 2.0); }
+            sh.steps++;
+            sh.err = err;
+            if (accept) {
+                sh.t = sh.clamped ? sh.target : sh.t + hh;
+                sh.accepted++;
+                sh.dt_min = fmin(sh.dt_min, hh);
+                sh.dt_max = fmax(sh.dt_max, hh);
+                if (adaptive) { const double prop = hh * fac; sh.dt = sh.clamped ? fmax(prop, sh.dt) : prop; }
+                const bool take = A.trace != nullptr && A.sample_dt > 0.0 && sh.trace_n < A.trace_cap &&
+                                  (adaptive ? (sh.clamped && sh.sample_hit)
+                                            : ((sh.accepted - sh.trace_acc0) % sh.trace_stride == 0));
+                if (take) {
+                    double* row = A.trace + ((size_t)rep * A.trace_cap + sh.trace_n) * A.row_len;
+                    row[0] = sh.t;
+                    for (int n = 0; n < N; ++n) {
+                        row[1 + 2 * n] = sh.anew[n][0]; row[2 + 2 * n] = sh.anew[n][1];
+                        row[1 + 2 * N + 2 * n] = sh.S[n][0]; row[2 + 2 * N + 2 * n] = sh.S[n][1];
+                    }
+                    for (int i = 0; i < 3 * NSUB; ++i) row[1 + 4 * N + i] = sh.red[i];
+                    sh.trace_n++;
+                }
+            } else if (sh.status == 0) {
+                sh.rejected++;
+                sh.dt = hh * fac;
+            }
+            if (adaptive && !(sh.dt > 1e-20)) sh.status = -6;
+            sh.accept = accept ? 1 : 0;
+        }
+        __syncthreads();                                                 // [D]
+        if (sh.accept) {                                                 // y := y_new, FSAL: k1 := k7
+#pragma unroll
+            for (int q = 0; q < NSUB; ++q)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { y[q][c] = yn[q][c]; k1[q][c] = k7[q][c]; }
+            if (tid < N) {
+                sh.a[tid][0] = sh.anew[tid][0]; sh.a[tid][1] = sh.anew[tid][1];
+                sh.ka[0][tid][0] = sh.ka[6][tid][0]; sh.ka[0][tid][1] = sh.ka[6][tid][1];
+            }
+        }
+    }
+
+    // ---- store the replica ----
+    if (active) {
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) mg[(size_t)(q * 3 + c) * nc + cell] = y[q][c];
+    }
+    if (tid < N) { A.a[((size_t)rep * N + tid) * 2] = sh.a[tid][0]; A.a[((size_t)rep * N + tid) * 2 + 1] = sh.a[tid][1]; }
+    if (tid == 0) {
+        BatchCtl& cl = A.ctl[rep];
+        cl.t = sh.t; cl.dt = sh.dt; cl.dt_min = sh.dt_min; cl.dt_max = sh.dt_max; cl.last_err = sh.err;
+        cl.accepted = sh.accepted; cl.rejected = sh.rejected; cl.rhs_evals = sh.rhs_evals;
+        cl.status = sh.status; cl.trace_n = sh.trace_n;
+    }
+}
+}  // namespace cavmag
