@@ -25,7 +25,8 @@ class _Problem(C.Structure):
                 ("axis", C.c_double * 3), ("alpha", C.c_double), ("gamma", C.c_double),
                 ("B0", C.c_double * 3), ("n_sub", C.c_int), ("B_exch_inter", C.c_double),
                 ("renormalize", C.c_int), ("norm_sum_u", C.c_int), ("N", C.c_int),
-                ("u", _dp), ("omega", _dp), ("kappa", _dp), ("g", _dp), ("Gamma", _dp), ("Phi", _dp)]
+                ("u", _dp), ("omega", _dp), ("kappa", _dp), ("g", _dp), ("Gamma", _dp), ("Phi", _dp),
+                ("eta_amp", _dp), ("eta_t0", _dp), ("eta_sigma", _dp), ("eta_wd", _dp)]
 
 
 class _Stats(C.Structure):
@@ -41,7 +42,7 @@ def lib():
     global _lib
     if _lib is None:
         _lib = C.CDLL(_build.build())
-        _lib.orc_rhs.argtypes = [C.POINTER(_Problem), _dp, _dp, _dp, _dp, _dp]
+        _lib.orc_rhs.argtypes = [C.POINTER(_Problem), C.c_double, _dp, _dp, _dp, _dp, _dp]
         _lib.orc_rhs.restype = None
         _lib.orc_run.argtypes = [C.POINTER(_Problem), _dp, _dp, _dp, C.c_double, C.c_double, C.c_double, _dp,
                                  C.c_longlong, C.c_double, _dp, C.c_int, C.POINTER(C.c_int), C.POINTER(_Stats)]
@@ -79,7 +80,9 @@ class Oracle:
     """One problem instance (grid + material + modes), built from a cavmag_workloads.Workload
     or from keyword arguments with the same names."""
 
-    def __init__(self, w=None, renormalize: bool = True, norm_sum_u: bool = False, **kw):
+    def __init__(self, w=None, renormalize: bool = True, norm_sum_u: bool = False, drive: Optional[dict] = None, **kw):
+        """drive = dict(amp [N] complex, t0 [N], sigma [N], omega_d [N] or None): the Gaussian-pulse drive
+        eta_n(t) = amp_n exp(-(t-t0_n)^2/(2 sigma_n^2)) exp(-i omega_d,n (t-t0_n)) of Eq. 1 / Eq. 12."""
         get = (lambda k: kw[k] if k in kw else getattr(w, k))
         self.nx, self.ny, self.nz = int(get("nx")), int(get("ny")), int(get("nz"))
         self.n_sub = int(get("n_sub"))
@@ -100,19 +103,26 @@ class Oracle:
         P.renormalize, P.norm_sum_u, P.N = int(renormalize), int(norm_sum_u), self.N
         P.u, P.omega, P.kappa, P.g = _p(self.u), _p(self.omega), _p(self.kappa), _p(self.g)
         P.Gamma, P.Phi = _p(self.Gamma), _p(self.Phi)
+        if drive is not None and self.N:
+            self.eta_amp = _c64(np.asarray(drive["amp"], dtype=np.complex128).reshape(self.N).view(np.float64))
+            self.eta_t0 = _c64(np.broadcast_to(np.asarray(drive["t0"], dtype=np.float64), (self.N,)))
+            self.eta_sigma = _c64(np.broadcast_to(np.asarray(drive["sigma"], dtype=np.float64), (self.N,)))
+            wd = drive.get("omega_d")
+            self.eta_wd = None if wd is None else _c64(np.broadcast_to(np.asarray(wd, dtype=np.float64), (self.N,)))
+            P.eta_amp, P.eta_t0, P.eta_sigma, P.eta_wd = _p(self.eta_amp), _p(self.eta_t0), _p(self.eta_sigma), _p(self.eta_wd)
         self.P = P
         self.nc = self.nx * self.ny * self.nz
         self.gamma = P.gamma
 
     # -- f(m, a) --------------------------------------------------------------------
-    def rhs(self, m: np.ndarray, a: np.ndarray):
-        """Returns (dm [n_sub,3,nz,ny,nx], da [N] complex, S [N] complex)."""
+    def rhs(self, m: np.ndarray, a: np.ndarray, t: float = 0.0):
+        """Returns (dm [n_sub,3,nz,ny,nx], da [N] complex, S [N] complex) at time t."""
         m = _c64(m).reshape(self.n_sub, 3, self.nz, self.ny, self.nx)
         a2 = _c64(np.asarray(a, dtype=np.complex128).view(np.float64))
         dm = np.empty_like(m)
         da = np.zeros(max(2 * self.N, 1))
         S = np.zeros(max(2 * self.N, 1))
-        lib().orc_rhs(C.byref(self.P), _p(m), _p(a2), _p(dm), _p(da), _p(S))
+        lib().orc_rhs(C.byref(self.P), float(t), _p(m), _p(a2), _p(dm), _p(da), _p(S))
         return dm, da[:2 * self.N].view(np.complex128).copy(), S[:2 * self.N].view(np.complex128).copy()
 
     # -- time integration -----------------------------------------------------------

@@ -15,7 +15,9 @@
 //    (1) m_c  = m_1  or (m_1+m_2)/2
 //    (2) S_n  = (1/W_n) sum_r u_n(r) (m_c,x - i m_c,y)       PAPER.md:156 Eq.18, :45 Eq.2
 //    (3) G_n  = g_n + Gamma_n e^{i Phi_n};
-//        da_n/dt = -(i w_n + kappa_n) a_n + i G_n S_n       PAPER.md:119 Eq.12, :317 Eq.19
+//        da_n/dt = -(i w_n + kappa_n) a_n + i G_n S_n + eta_n(t)   PAPER.md:119 Eq.12, :317 Eq.19
+//        eta_n(t) = A_n exp(-(t-t0_n)^2/(2 sigma_n^2)) exp(-i w_d,n (t-t0_n))   Gaussian pulse
+//        (evaluated at the stage times t + c_s h; absent unless drive arrays are given - reading G27)
 //    (4) c_n  = (2/gamma) Re[G_n a_n];  B_rf(r) = x^ sum_n c_n u_n(r)
 //                                                           PAPER.md:65 Eq.5, :121 Eq.13, :159
 //    (5) B_s  = B0 + (2A/Ms) sum_{d,+-} [m_s(r +- e_d) - m_s(r)]/D_d^2   (open boundary)
@@ -60,6 +62,11 @@ struct orc_problem {
     const double* g;         // [N] rad/s
     const double* Gamma;     // [N] rad/s
     const double* Phi;       // [N] rad
+    // external drive eta_n(t) (PAPER.md:43 Eq. 1, :119 Eq. 12; Gaussian pulse of PAPER.md:229); eta_amp == NULL: none
+    const double* eta_amp;   // [N][2] complex amplitude A_n (units of a per second)
+    const double* eta_t0;    // [N] pulse centre, s
+    const double* eta_sigma; // [N] pulse width, s
+    const double* eta_wd;    // [N] carrier, rad/s (NULL: baseband pulse)
 };
 
 struct orc_stats {
@@ -122,8 +129,8 @@ void overlaps(const orc_problem* P, const double* m, double* S /*[N][2]*/) {
     }
 }
 
-// ---- the coupled right-hand side f(m, a) ----------------------------------------------
-void rhs(const orc_problem* P, const double* m, const double* a, double* dm, double* da, double* S_out) {
+// ---- the coupled right-hand side f(t, m, a) ---------------------------------------------
+void rhs(const orc_problem* P, double t, const double* m, const double* a, double* dm, double* da, double* S_out) {
     const int nx = P->nx, ny = P->ny, nz = P->nz, N = P->N;
     const long long nc = ncell(P);
     std::vector<double> S(2 * (size_t)(N > 0 ? N : 1));
@@ -142,6 +149,14 @@ void rhs(const orc_problem* P, const double* m, const double* a, double* dm, dou
         da[2 * n + 0] = (-P->kappa[n] * are + P->omega[n] * aim) - (Gre * Sim + Gim * Sre);
         da[2 * n + 1] = (-P->kappa[n] * aim - P->omega[n] * are) + (Gre * Sre - Gim * Sim);
         c[n] = (2.0 / P->gamma) * (Gre * are - Gim * aim);   // (2/gamma) Re[G a]
+        if (P->eta_amp) {   // + eta_n(t): Gaussian envelope times carrier e^{-i w_d (t - t0)}
+            const double x = t - P->eta_t0[n];
+            const double env = std::exp(-(x * x) / (2.0 * P->eta_sigma[n] * P->eta_sigma[n]));
+            const double ph = P->eta_wd ? P->eta_wd[n] * x : 0.0;
+            const double Are = P->eta_amp[2 * n], Aim = P->eta_amp[2 * n + 1];
+            da[2 * n + 0] += env * (Are * std::cos(ph) + Aim * std::sin(ph));
+            da[2 * n + 1] += env * (Aim * std::cos(ph) - Are * std::sin(ph));
+        }
     }
 
     const double pref_ex = 2.0 * P->Aex / P->Ms;
@@ -222,13 +237,13 @@ void combine(Work& W, const double* y, const double* a, double h, const double* 
 
 // One DP5(4) trial step of size h from (m,a) with k1 already in W.k[0], W.ka[0].
 // Leaves the candidate in W.ynew/W.anew, k7 in W.k[6]/W.ka[6], returns the error norm.
-double trial_step(const orc_problem* P, Work& W, const double* m, const double* a, double h, double* S7) {
+double trial_step(const orc_problem* P, Work& W, double t, const double* m, const double* a, double h, double* S7) {
     const long long nc = ncell(P);
-    { const double c[] = {A21};                     combine(W, m, a, h, c, 1, W.ys.data(), W.as.data()); rhs(P, W.ys.data(), W.as.data(), W.k[1].data(), W.ka[1].data(), nullptr); }
-    { const double c[] = {A31, A32};                combine(W, m, a, h, c, 2, W.ys.data(), W.as.data()); rhs(P, W.ys.data(), W.as.data(), W.k[2].data(), W.ka[2].data(), nullptr); }
-    { const double c[] = {A41, A42, A43};           combine(W, m, a, h, c, 3, W.ys.data(), W.as.data()); rhs(P, W.ys.data(), W.as.data(), W.k[3].data(), W.ka[3].data(), nullptr); }
-    { const double c[] = {A51, A52, A53, A54};      combine(W, m, a, h, c, 4, W.ys.data(), W.as.data()); rhs(P, W.ys.data(), W.as.data(), W.k[4].data(), W.ka[4].data(), nullptr); }
-    { const double c[] = {A61, A62, A63, A64, A65}; combine(W, m, a, h, c, 5, W.ys.data(), W.as.data()); rhs(P, W.ys.data(), W.as.data(), W.k[5].data(), W.ka[5].data(), nullptr); }
+    { const double c[] = {A21};                     combine(W, m, a, h, c, 1, W.ys.data(), W.as.data()); rhs(P, t + (1.0 / 5.0) * h, W.ys.data(), W.as.data(), W.k[1].data(), W.ka[1].data(), nullptr); }
+    { const double c[] = {A31, A32};                combine(W, m, a, h, c, 2, W.ys.data(), W.as.data()); rhs(P, t + (3.0 / 10.0) * h, W.ys.data(), W.as.data(), W.k[2].data(), W.ka[2].data(), nullptr); }
+    { const double c[] = {A41, A42, A43};           combine(W, m, a, h, c, 3, W.ys.data(), W.as.data()); rhs(P, t + (4.0 / 5.0) * h, W.ys.data(), W.as.data(), W.k[3].data(), W.ka[3].data(), nullptr); }
+    { const double c[] = {A51, A52, A53, A54};      combine(W, m, a, h, c, 4, W.ys.data(), W.as.data()); rhs(P, t + (8.0 / 9.0) * h, W.ys.data(), W.as.data(), W.k[4].data(), W.ka[4].data(), nullptr); }
+    { const double c[] = {A61, A62, A63, A64, A65}; combine(W, m, a, h, c, 5, W.ys.data(), W.as.data()); rhs(P, t + (1.0) * h, W.ys.data(), W.as.data(), W.k[5].data(), W.ka[5].data(), nullptr); }
     { const double c[] = {B1, 0.0, B3, B4, B5, B6}; combine(W, m, a, h, c, 6, W.ynew.data(), W.anew.data()); }
     if (P->renormalize) {   // G13: normalise the 5th-order solution per cell before the 7th evaluation
         for (int s = 0; s < P->n_sub; ++s) {
@@ -241,7 +256,7 @@ double trial_step(const orc_problem* P, Work& W, const double* m, const double* 
             }
         }
     }
-    rhs(P, W.ynew.data(), W.anew.data(), W.k[6].data(), W.ka[6].data(), S7);
+    rhs(P, t + h, W.ynew.data(), W.anew.data(), W.k[6].data(), W.ka[6].data(), S7);   // c_7 = 1
     // e = h sum_j d_j k_j,  d = b - bhat
     const double d[7] = {B1 - BH1, 0.0, B3 - BH3, B4 - BH4, B5 - BH5, B6 - BH6, -BH7};
     double err = 0.0;
@@ -279,9 +294,9 @@ double trial_step(const orc_problem* P, Work& W, const double* m, const double* 
 
 extern "C" {
 
-// f(m, a): dm [n_sub][3][nc], da [N][2], S [N][2] (may be NULL).
-void orc_rhs(const orc_problem* P, const double* m, const double* a, double* dm, double* da, double* S) {
-    rhs(P, m, a, dm, da, S);
+// f(t, m, a): dm [n_sub][3][nc], da [N][2], S [N][2] (may be NULL).
+void orc_rhs(const orc_problem* P, double t, const double* m, const double* a, double* dm, double* da, double* S) {
+    rhs(P, t, m, a, dm, da, S);
 }
 
 // Integrate from *t to t_end (or for max_steps attempted steps if max_steps > 0).
@@ -302,7 +317,7 @@ int orc_run(const orc_problem* P, double* m, double* a, double* t_io, double t_e
     orc_stats s = {0, 0, 0, INFINITY, 0.0, dt, t, 0};
     std::vector<double> S7((size_t)(na > 0 ? na : 1));
 
-    rhs(P, m, a, W.k[0].data(), W.ka[0].data(), nullptr);   // k1 = f(y), once; afterwards FSAL
+    rhs(P, t, m, a, W.k[0].data(), W.ka[0].data(), nullptr);   // k1 = f(t, y), once; afterwards FSAL
     s.rhs_evals++;
 
     const int rowlen = 1 + 4 * P->N + 3 * P->n_sub;
@@ -323,7 +338,7 @@ int orc_run(const orc_problem* P, double* m, double* a, double* t_io, double t_e
         }
         bool clamped = false;
         if (t + h * (1.0 + 1e-12) >= target) { h = target - t; clamped = true; }
-        const double err = trial_step(P, W, m, a, h, S7.data());
+        const double err = trial_step(P, W, t, m, a, h, S7.data());
         s.rhs_evals += 6;
         steps++;
         bool accept;
