@@ -569,3 +569,66 @@ def test_adaptive_controller_bookkeeping():
     # fixed-step trace: every 5th step
     r = o.run(w.m0, w.a0, fixed_dt=0.2e-12, max_steps=50, sample_dt=1e-12, trace_cap=100)
     assert r.trace.shape[0] == 10 and r.accepted == 50 and r.rejected == 0
+
+
+# ----------------------------------------------------------------------------------------
+# external drive eta_n(t) (PAPER.md:43 Eq. 1, :119 Eq. 12; Gaussian pulse of PAPER.md:229)
+# ----------------------------------------------------------------------------------------
+def _pulse(N, sigma=20e-12, t0=0.2e-9):
+    amp = np.array([1e9 * (1 + 0.5j), 2e9 * (-0.3 + 1j), 0.5e9 * (0.2 - 1j)])[:N]
+    return dict(amp=amp, t0=np.full(N, t0), sigma=np.full(N, sigma))
+
+
+@pytest.mark.parametrize("mode", ["fixed", "adaptive"])
+def test_gaussian_pulse_closed_form_uncoupled_cavity(mode):
+    """g = 0: da/dt = -lambda a + A exp(-(t-t0)^2/(2 s^2)) exp(-i w_d (t-t0)), lambda = kappa + i w, has, once the pulse
+    is over (t0 = 10 sigma, T - t0 = 15 sigma: truncation < 1e-20),
+        a(T) = A s sqrt(2 pi) exp((lambda - i w_d)^2 s^2 / 2) exp(-lambda (T - t0)).
+    Pins the drive's amplitude, envelope, carrier sign and the stage times t + c_s h (with all stages evaluated at t
+    the result would be off by O(h / sigma))."""
+    w = W.macrospin(10.0, [9.0, 10.5, 10.0], 0.0, [1.0, 50.0, 10.0], alpha=1e-3, a0=[0, 0, 0], n=2)
+    dr = _pulse(3)
+    dr["omega_d"] = np.array([0.0, TWO_PI * 10.5e9, TWO_PI * 9.7e9])     # baseband, resonant and detuned carrier
+    o = Oracle(w, drive=dr)
+    T = 0.5e-9
+    r = o.run(w.m0, w.a0, t_end=T, fixed_dt=0.25e-12) if mode == "fixed" else o.run(w.m0, w.a0, t_end=T, tol=1e-12)
+    lam = w.kappa + 1j * w.omega
+    s = dr["sigma"]
+    exact = dr["amp"] * s * math.sqrt(TWO_PI) * np.exp((lam - 1j * dr["omega_d"]) ** 2 * s ** 2 / 2) * np.exp(-lam * (T - dr["t0"]))
+    assert np.all(np.abs(r.a - exact) <= (1e-10 if mode == "fixed" else 3e-9) * np.abs(exact))
+    # the resonant carrier delivers the most: |a| = |A| s sqrt(2 pi) exp(kappa^2 s^2/2) exp(-kappa (T-t0))
+    assert abs(abs(exact[1]) / (abs(dr["amp"][1]) * s[1] * math.sqrt(TWO_PI) * math.exp(-w.kappa[1] * (T - 0.2e-9))) - 1) < 1e-4
+
+
+def test_drive_enters_at_the_stage_times_order_five():
+    """With a time-dependent drive the scheme stays 5th order only if stage s is evaluated at t + c_s h."""
+    w = _busy_problem()
+    N = w.omega.size
+    o = Oracle(w, renormalize=False, drive=dict(amp=np.full(N, 4e10 * (1 - 1j)), t0=np.full(N, 4e-12),
+                                                  sigma=np.full(N, 2e-12), omega_d=w.omega))
+    T = 8e-12
+    ref = o.run(w.m0, w.a0, fixed_dt=T / 1024, max_steps=1024)
+    errs = []
+    for n in (32, 64, 128):
+        r = o.run(w.m0, w.a0, fixed_dt=T / n, max_steps=n)
+        errs.append(max(np.abs(r.m - ref.m).max(), np.abs(r.a - ref.a).max()))
+    assert 22 < errs[0] / errs[1] < 44 and 22 < errs[1] / errs[2] < 44
+    undriven = Oracle(w, renormalize=False).run(w.m0, w.a0, fixed_dt=T / 128, max_steps=128)
+    assert np.abs(ref.a - undriven.a).max() > 1e3 * errs[2]          # the drive matters at this accuracy
+
+
+def test_pulse_spectroscopy_shows_both_polariton_branches():
+    """The paper's protocol: a short Gaussian pulse (sigma = 20 ps, t0 = 0.1 ns) on the cavity at
+    resonance, then free evolution; the ring-down of a(t) holds both branches w_c +- g of Eq. 6 with equal weight."""
+    g_mhz = 50.0
+    w = W.macrospin(10.0, [10.0], g_mhz, 1.0, alpha=1e-4, a0=[0.0], n=2)
+    o = Oracle(w, drive=dict(amp=np.array([1e8 + 0j]), t0=np.array([0.1e-9]), sigma=np.array([20e-12])))
+    sdt = 20e-12
+    r = o.run(w.m0, w.a0, t_end=40e-9, tol=1e-9, sample_dt=sdt, trace_cap=2000)
+    tr = r.trace[r.trace[:, 0] > 0.3e-9]                              # after the pulse
+    z = tr[:, 1] + 1j * tr[:, 2]
+    om, amp = fit_exponentials(z, sdt, 4)
+    om2, amp2 = dominant(om, amp, 2)
+    f = om2.real / TWO_PI
+    assert abs(f[0] - (10e9 - g_mhz * 1e6)) < 1e6 and abs(f[1] - (10e9 + g_mhz * 1e6)) < 1e6
+    assert 0.8 < abs(amp2[0]) / abs(amp2[1]) < 1.25
