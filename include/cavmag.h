@@ -115,6 +115,15 @@ int cav_set_launch_mode(cav_sim* sim, int mode);
 int cav_set_modes(cav_sim* sim, int N, const void* u, int u_is_device, const double* omega,
                   const double* kappa, const double* g, const double* Gamma, const double* Phi);
 
+/* External microwave drive eta_n(t) of Eq. 1 / Eq. 12, as the Gaussian pulse of the paper's
+ * spectroscopy protocol (sigma = 20 ps, t0 = 0.1 ns) with an optional carrier (reading G27):
+ *     eta_n(t) = A_n exp(-(t - t0_n)^2 / (2 sigma_n^2)) exp(-i omega_d,n (t - t0_n)),
+ * added to da_n/dt at the stage times t + c_s h of the RK45 step.
+ *   amp_re_im [N][2] complex amplitude A_n (units of a per second); NULL switches the drive off
+ *   t0, sigma [N] seconds (sigma > 0, else CAV_E_ARG); omega_d [N] rad/s or NULL (= 0: baseband pulse)
+ * Host arrays, copied.  Call after cav_set_modes (a new mode set clears the drive). */
+int cav_set_drive(cav_sim* sim, const double* amp_re_im, const double* t0, const double* sigma, const double* omega_d);
+
 /* Magnetisation [n_sub][3][nz][ny][nx] in the simulation's precision. Normalised per cell on entry. */
 int cav_set_m(cav_sim* sim, const void* m, int is_device);
 int cav_get_m(cav_sim* sim, void* m_out, int is_device);
@@ -213,6 +222,9 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
  * normalised per cell on entry.  Amplitudes [N][2] or [n_rep][N][2]. */
 int cav_batch_set_m(cav_batch* b, const void* m, int per_replica);
 int cav_batch_set_a(cav_batch* b, const double* a_re_im, int per_replica);
+
+/* Drive as cav_set_drive, common to all replicas ([N] arrays).  Call after cav_batch_set_modes. */
+int cav_batch_set_drive(cav_batch* b, const double* amp_re_im, const double* t0, const double* sigma, const double* omega_d);
 
 /* Trace rows as cav_set_trace, per replica; resets the traces. */
 int cav_batch_set_trace(cav_batch* b, double sample_dt, int capacity);

@@ -63,6 +63,7 @@ _SIGS = {
     "cav_set_stream": ([_vp, _vp], _i),
     "cav_set_launch_mode": ([_vp, _i], _i),
     "cav_set_modes": ([_vp, _i, _vp, _i, _dp, _dp, _dp, _dp, _dp], _i),
+    "cav_set_drive": ([_vp, _dp, _dp, _dp, _dp], _i),
     "cav_set_m": ([_vp, _vp, _i], _i),
     "cav_get_m": ([_vp, _vp, _i], _i),
     "cav_set_a": ([_vp, _dp], _i),
@@ -94,6 +95,7 @@ _SIGS = {
     "cav_batch_set_stream": ([_vp, _vp], _i),
     "cav_batch_set_field": ([_vp, _dp], _i),
     "cav_batch_set_modes": ([_vp, _i, _vp, _dp, _dp, _dp, _dp, _dp, _i], _i),
+    "cav_batch_set_drive": ([_vp, _dp, _dp, _dp, _dp], _i),
     "cav_batch_set_m": ([_vp, _vp, _i], _i),
     "cav_batch_set_a": ([_vp, _dp, _i], _i),
     "cav_batch_set_trace": ([_vp, _d, _i], _i),
@@ -412,6 +414,28 @@ def cav_batch_set_modes(b, u, omega, kappa, g, Gamma=None, Phi=None, per_replica
     pG, kG = _darr(Gamma, n)
     pP, kP = _darr(Phi, n)
     _check(_lib.cav_batch_set_modes(b, N, _vp(addr), po, pk, pg, pG, pP, int(bool(per_replica))), "cav_batch_set_modes")
+
+
+def _drive_args(amp, t0, sigma, omega_d):
+    if amp is None:
+        return (None, None, None, None), ()
+    a = np.ascontiguousarray(np.asarray(amp, dtype=np.complex128).reshape(-1)).view(np.float64)
+    n = a.size // 2
+    pt, kt = _darr(np.broadcast_to(np.asarray(t0, dtype=np.float64), (n,)), n)
+    ps, ks = _darr(np.broadcast_to(np.asarray(sigma, dtype=np.float64), (n,)), n)
+    pw, kw = _darr(None if omega_d is None else np.broadcast_to(np.asarray(omega_d, dtype=np.float64), (n,)), n)
+    return (a.ctypes.data_as(_dp), pt, ps, pw), (a, kt, ks, kw)
+
+
+def cav_set_drive(sim, amp, t0=None, sigma=None, omega_d=None) -> None:
+    """amp [N] complex or None (off); t0, sigma [N] or scalars; omega_d [N], scalar or None."""
+    args, keep = _drive_args(amp, t0, sigma, omega_d)
+    _check(_lib.cav_set_drive(sim, *args), "cav_set_drive", sim)
+
+
+def cav_batch_set_drive(b, amp, t0=None, sigma=None, omega_d=None) -> None:
+    args, keep = _drive_args(amp, t0, sigma, omega_d)
+    _check(_lib.cav_batch_set_drive(b, *args), "cav_batch_set_drive")
 
 
 def cav_batch_set_m(b, m: np.ndarray, per_replica: bool = False) -> None:

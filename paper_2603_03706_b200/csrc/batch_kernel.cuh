@@ -45,6 +45,7 @@ struct BatchArgs {
     int trace_cap, row_len;
     double* trace;                // [n_rep][trace_cap][row_len]
     int u_in_smem;                // profiles staged in dynamic shared memory
+    const double* drive;          // [5][N]: eta_re, eta_im, t0, 1/(2 sigma^2), omega_d (common to all replicas) or NULL
 };
 
 // Shared mode / controller state of one replica.
@@ -52,6 +53,7 @@ struct BatchShared {
     double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes];
     double a[kMaxModes][2], as[kMaxModes][2], anew[kMaxModes][2], ka[7][kMaxModes][2], S[kMaxModes][2];
     double c[kMaxModes], serr[kMaxModes];
+    double eta_re[kMaxModes], eta_im[kMaxModes], eta_t0[kMaxModes], eta_i2s2[kMaxModes], eta_wd[kMaxModes];
     double part[32][2 * kMaxModes + 6];     // per-warp partial sums: overlaps (2N) then <m_s> (3 n_sub)
     double wmax[32];
     double red[2 * kMaxModes + 6];
@@ -117,6 +119,10 @@ __global__ void __launch_bounds__(MAXT) k_batch(const BatchArgs A) {
         sh.a[tid][0] = are; sh.a[tid][1] = aim;
         sh.as[tid][0] = are; sh.as[tid][1] = aim;                       // stage 1 evaluates f(m_0, a_0)
         sh.c[tid] = A.two_over_gamma * (sh.Gre[tid] * are - sh.Gim[tid] * aim);
+        if (A.drive) {
+            sh.eta_re[tid] = A.drive[tid]; sh.eta_im[tid] = A.drive[N + tid]; sh.eta_t0[tid] = A.drive[2 * N + tid];
+            sh.eta_i2s2[tid] = A.drive[3 * N + tid]; sh.eta_wd[tid] = A.drive[4 * N + tid];
+        }
     }
     if (tid == 0) {
         const BatchCtl& cl = A.ctl[rep];
@@ -205,8 +211,17 @@ __global__ void __launch_bounds__(MAXT) k_batch(const BatchArgs A) {
             sh.S[n][0] = Sre; sh.S[n][1] = Sim;
             const double are = sh.as[n][0], aim = sh.as[n][1];
             const double Gre = sh.Gre[n], Gim = sh.Gim[n];
-            sh.ka[s - 1][n][0] = (-sh.kappa[n] * are + sh.omega[n] * aim) - (Gre * Sim + Gim * Sre);
-            sh.ka[s - 1][n][1] = (-sh.kappa[n] * aim - sh.omega[n] * are) + (Gre * Sre - Gim * Sim);
+            double kre = (-sh.kappa[n] * are + sh.omega[n] * aim) - (Gre * Sim + Gim * Sre);
+            double kim = (-sh.kappa[n] * aim - sh.omega[n] * are) + (Gre * Sre - Gim * Sim);
+            if (A.drive) {          // + eta_n(t + c_s h)  (Eq. 1 / Eq. 12; stage 1 runs before h is set: c_1 = 0)
+                const double x = (s == 1 ? sh.t : sh.t + kC[s - 1] * sh.h) - sh.eta_t0[n];
+                const double env = exp(-(x * x) * sh.eta_i2s2[n]);
+                double sn, cs;
+                sincos(sh.eta_wd[n] * x, &sn, &cs);
+                kre += env * (sh.eta_re[n] * cs + sh.eta_im[n] * sn);
+                kim += env * (sh.eta_im[n] * cs - sh.eta_re[n] * sn);
+            }
+            sh.ka[s - 1][n][0] = kre; sh.ka[s - 1][n][1] = kim;
             if constexpr (s >= 2 && s <= 5) batch_stage_state<s>(sh, n, A.two_over_gamma);
             else if constexpr (s == 6) {
                 batch_stage_state<6>(sh, n, A.two_over_gamma);       // row 6 = b: the 5th-order candidate

@@ -671,6 +671,7 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         c->invW[n] = 1.0 / (double)s->nc;
         c->a[n][0] = c->a[n][1] = 0.0;
     }
+    c->drive_on = 0;                     // a new mode set clears the drive
     if (N > 0 && s->prm.overlap_norm == CAV_NORM_SUM_U) {
         double* d_out = nullptr;
         CK(cudaMalloc(&d_out, sizeof(double) * 256 * N));
@@ -697,6 +698,29 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
     s->graph_dirty = true;
     rc = plan_tma(s);
     if (rc) return rc;
+    return push_ctrl(s);
+}
+
+int cav_set_drive(cav_sim* s, const double* amp, const double* t0, const double* sigma, const double* omega_d) {
+    if (!s) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    Ctrl* c = s->h_ctrl;
+    if (!amp || c->N == 0) {
+        c->drive_on = 0;
+    } else {
+        if (!t0 || !sigma) return CAV_E_ARG;
+        for (int n = 0; n < c->N; ++n)
+            if (!(sigma[n] > 0.0)) return CAV_E_ARG;
+        for (int n = 0; n < c->N; ++n) {
+            c->eta_re[n] = amp[2 * n]; c->eta_im[n] = amp[2 * n + 1];
+            c->eta_t0[n] = t0[n];
+            c->eta_i2s2[n] = 1.0 / (2.0 * sigma[n] * sigma[n]);
+            c->eta_wd[n] = omega_d ? omega_d[n] : 0.0;
+        }
+        c->drive_on = 1;
+    }
+    c->k1_valid = 0;                     // da/dt of the current state changes
     return push_ctrl(s);
 }
 

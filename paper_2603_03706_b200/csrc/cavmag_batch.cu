@@ -20,6 +20,7 @@ struct cav_batch {
     double* d_B0 = nullptr;
     void* d_u = nullptr;
     double* d_modep = nullptr;
+    double* d_drive = nullptr;     // [5][N] or NULL: no drive
     int modep_per_rep = 0;
     void* d_m = nullptr;
     double* d_a = nullptr;
@@ -123,7 +124,7 @@ int cav_batch_create(const cav_grid* grid, const cav_params* prm, int n_rep, cav
 int cav_batch_destroy(cav_batch* b) {
     if (!b) return CAV_E_ARG;
     if (b->stream) cudaStreamSynchronize(b->stream);
-    cudaFree(b->d_B0); cudaFree(b->d_u); cudaFree(b->d_modep); cudaFree(b->d_m); cudaFree(b->d_a);
+    cudaFree(b->d_B0); cudaFree(b->d_u); cudaFree(b->d_modep); cudaFree(b->d_drive); cudaFree(b->d_m); cudaFree(b->d_a);
     cudaFree(b->d_ctl); cudaFree(b->d_trace);
     if (b->own_stream && b->stream) cudaStreamDestroy(b->stream);
     cudaGetLastError();
@@ -154,6 +155,8 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
     CKB(cudaStreamSynchronize(b->stream));
     cudaFree(b->d_u);
     b->d_u = nullptr;
+    cudaFree(b->d_drive);
+    b->d_drive = nullptr;                  // a new mode set clears the drive
     b->N = N;
     b->modep_per_rep = per_replica ? 1 : 0;
     if (N > 0) {
@@ -187,6 +190,26 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
     CKB(cudaMemsetAsync(b->d_a, 0, sizeof(double) * 2 * CAV_MAX_MODES * b->n_rep, b->stream));
     cudaFree(b->d_trace);
     b->d_trace = nullptr; b->trace_cap = 0; b->sample_dt = 0.0;      // the row length changed
+    CKB(cudaStreamSynchronize(b->stream));
+    return CAV_OK;
+}
+
+int cav_batch_set_drive(cav_batch* b, const double* amp, const double* t0, const double* sigma, const double* omega_d) {
+    if (!b) return CAV_E_ARG;
+    CKB(cudaStreamSynchronize(b->stream));
+    cudaFree(b->d_drive);
+    b->d_drive = nullptr;
+    if (!amp || b->N == 0) return CAV_OK;
+    if (!t0 || !sigma) return CAV_E_ARG;
+    const int N = b->N;
+    std::vector<double> d(5 * (size_t)N);
+    for (int n = 0; n < N; ++n) {
+        if (!(sigma[n] > 0.0)) return CAV_E_ARG;
+        d[n] = amp[2 * n]; d[N + n] = amp[2 * n + 1]; d[2 * N + n] = t0[n];
+        d[3 * N + n] = 1.0 / (2.0 * sigma[n] * sigma[n]); d[4 * N + n] = omega_d ? omega_d[n] : 0.0;
+    }
+    CKB(cudaMalloc(&b->d_drive, sizeof(double) * d.size()));
+    CKB(cudaMemcpyAsync(b->d_drive, d.data(), sizeof(double) * d.size(), cudaMemcpyHostToDevice, b->stream));
     CKB(cudaStreamSynchronize(b->stream));
     return CAV_OK;
 }
@@ -276,6 +299,7 @@ int cav_batch_run(cav_batch* b, double t_end, double tol, double fixed_dt, doubl
     A.max_steps = max_steps;
     A.sample_dt = b->sample_dt; A.trace_t0 = b->trace_t0; A.trace_cap = b->trace_cap; A.row_len = row_len_of(b);
     A.trace = b->d_trace;
+    A.drive = b->d_drive;
 
     int threads = (b->nc + 31) / 32 * 32;
     if (threads < 64) threads = 64;

@@ -54,6 +54,9 @@ struct Ctrl {
     double S[kMaxModes][2];        // overlaps of the last evaluated stage state
     double c[kMaxModes];           // (2/gamma) Re[G_n a_s,n]: RF-field weights for the next kernel
     double mavg[6];                // <m_s> of the last accepted state
+    // ---- external drive eta_n(t) = A_n exp(-(t-t0)^2 i2s2) exp(-i wd (t-t0)) ----
+    int drive_on, drive_pad;
+    double eta_re[kMaxModes], eta_im[kMaxModes], eta_t0[kMaxModes], eta_i2s2[kMaxModes], eta_wd[kMaxModes];
     // ---- trace ----
     double sample_dt, trace_t0;
     int trace_cap, trace_n;

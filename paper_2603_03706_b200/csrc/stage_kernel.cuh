@@ -42,6 +42,7 @@ __device__ __forceinline__ void probe_mark(const Args& A, int stage, int slot) {
 
 __device__ constexpr double kA[7][7] = CAVMAG_DP_A;
 __device__ constexpr double kD[7] = CAVMAG_DP_D;
+__device__ constexpr double kC[7] = {0.0, 1.0 / 5.0, 3.0 / 10.0, 4.0 / 5.0, 8.0 / 9.0, 1.0, 1.0};   // stage times t + c_s h
 
 // ---------------------------------------------------------------------------------------
 // vector load/store of VEC consecutive cells (16 bytes for float4 / double2)
@@ -119,8 +120,16 @@ __device__ __forceinline__ void mode_ode_stage(Ctrl* c, const int n, const doubl
     c->S[n][0] = Sre; c->S[n][1] = Sim;
     const double are = c->as[stage & 1][n][0], aim = c->as[stage & 1][n][1];
     const double Gre = c->Gre[n], Gim = c->Gim[n];
-    const double kre = (-c->kappa[n] * are + c->omega[n] * aim) - (Gre * Sim + Gim * Sre);
-    const double kim = (-c->kappa[n] * aim - c->omega[n] * are) + (Gre * Sre - Gim * Sim);
+    double kre = (-c->kappa[n] * are + c->omega[n] * aim) - (Gre * Sim + Gim * Sre);
+    double kim = (-c->kappa[n] * aim - c->omega[n] * are) + (Gre * Sre - Gim * Sim);
+    if (c->drive_on) {          // + eta_n(t + c_s h): Gaussian pulse with carrier (Eq. 1 / Eq. 12)
+        const double x = (c->t + kC[stage - 1] * c->h) - c->eta_t0[n];
+        const double env = exp(-(x * x) * c->eta_i2s2[n]);
+        double sn, cs;
+        sincos(c->eta_wd[n] * x, &sn, &cs);
+        kre += env * (c->eta_re[n] * cs + c->eta_im[n] * sn);
+        kim += env * (c->eta_im[n] * cs - c->eta_re[n] * sn);
+    }
     c->ka[stage - 1][n][0] = kre; c->ka[stage - 1][n][1] = kim;
     if constexpr (stage >= 2 && stage <= 5) {
         mode_stage_state<stage>(c, n);              // a_{s+1}, c^{(s+1)}
@@ -179,7 +188,7 @@ __device__ __forceinline__ void reduce_block_partials(const double* partial, con
 // ---------------------------------------------------------------------------------------
 constexpr int kCtrlWords = (int)(sizeof(Ctrl) / 8);
 static_assert(sizeof(Ctrl) % 8 == 0, "Ctrl is copied as 8-byte words");
-static_assert(kCtrlWords <= 8 * kBlock, "Ctrl copy: at most 8 words per thread");
+constexpr int kCtrlWordsPerThread = (kCtrlWords + kBlock - 1) / kBlock;     // stage_finish, 128-thread blocks
 
 // r^(1/5) for r in [1e-2, 1e3]: float seed + one Newton step in fp64 (relative error < 1e-13).  A libm pow()
 // in fp64 costs several microseconds of single-thread latency on this part, all of it between two stage kernels.
@@ -228,9 +237,9 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
     const int nsum = 2 * N + (stage == 7 ? 3 * nsub : 0);
     CAVMAG_MARKF(8);
     // Ctrl -> registers (consumed after the partial sums so that all loads are in flight together)
-    unsigned long long cw[8];
+    unsigned long long cw[kCtrlWordsPerThread];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < kCtrlWordsPerThread; ++k) {
         const int idx = tid + k * nthr;
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
@@ -249,7 +258,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
         if (lane == 0) smax = mx;
     }
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < kCtrlWordsPerThread; ++k) {
         const int idx = tid + k * nthr;
         if (idx < kCtrlWords) sc_words[idx] = cw[k];
     }

@@ -122,23 +122,23 @@ template <int STAGE> struct StageStreams {
 // to arrive" tail of stages 2..6 (an atomic ticket, two fences and ~4 dependent L2 round trips with 147 SMs
 // idle) by work that overlaps the pipeline fill.  Fields written by block 0 (S, ka[PREV-1], as[(PREV+1)&1], c,
 // anew, rhs_evals) are never inputs of another block in the same kernel.
-static_assert(kCtrlWords <= 4 * kTmaConsumers, "deferred finish copies Ctrl with 4 words per consumer thread");
+constexpr int kCtrlWordsPerConsumer = (kCtrlWords + kTmaConsumers - 1) / kTmaConsumers;
 
 template <int PREV, int NB>
 __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __restrict__ gctrl, const int tidc,
                                                 unsigned long long* sc_words, double* sred) {
-    // one batch of independent loads: the whole Ctrl (4 words per thread) and all 2*NB x gridDim block partials
+    // one batch of independent loads: the whole Ctrl (a few words per thread) and all 2*NB x gridDim block partials
     // (rows of modes >= N hold stale values that nothing reads)
     const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(gctrl);
-    unsigned long long cw[4];
+    unsigned long long cw[kCtrlWordsPerConsumer];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
         const int idx = tidc + k * kTmaConsumers;
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
     reduce_block_partials(A.partial, A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
         const int idx = tidc + k * kTmaConsumers;
         if (idx < kCtrlWords) sc_words[idx] = cw[k];
     }

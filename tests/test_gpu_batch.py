@@ -166,3 +166,29 @@ def test_resume_and_edge_cases(api):
     with pytest.raises(api.CavError) as e:
         api.Batch(big, 1)
     assert e.value.status == api.CAV_E_ARG
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_driven_sweep_fixed_steps(api, prec):
+    """The paper's spectroscopy protocol in one launch: every replica (its own B0) gets the same Gaussian pulse on the
+    cavity (cav_batch_set_drive), compared with the driven oracle replica by replica."""
+    w = small_problem(8, 8, 2, 2, 1)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    dt = 0.1e-12
+    N = w.omega.size
+    dr = dict(amp=np.array([3e10 + 1e10j, -2e10j]), t0=np.full(N, 30 * dt), sigma=np.full(N, 12 * dt), omega_d=w.omega * 1.02)
+    ghz = np.array([9.0, 9.8, 10.6])
+    B0 = np.array([[0.01, -0.02, W.b0_for_ghz(f)] for f in ghz])
+    with api.Batch(w, 3, precision=prec, B0=B0) as b:
+        api.cav_batch_set_drive(b.h, dr["amp"], dr["t0"], dr["sigma"], dr["omega_d"])
+        b.run(math.inf, fixed_dt=dt, max_steps=80)
+        m, a = b.get_m(), b.get_a()
+    for r in range(3):
+        wr = copy.deepcopy(w)
+        wr.B0 = tuple(B0[r])
+        ref = oracle_of(wr, drive=dr).run(wr.m0, wr.a0, fixed_dt=dt, max_steps=80)
+        assert_parity(m[r], a[r], ref, prec)
+    wr = copy.deepcopy(w); wr.B0 = tuple(B0[0])
+    undriven = oracle_of(wr).run(wr.m0, wr.a0, fixed_dt=dt, max_steps=80)
+    assert np.abs(a[0] - undriven.a).max() > 0.05 * np.abs(undriven.a).max()

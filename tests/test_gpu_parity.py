@@ -467,3 +467,52 @@ def test_device_buffers_via_torch(api):
     ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=20)
     assert np.abs(out.cpu().numpy() - ref.m).max() < 1e-12
     assert np.abs(a - ref.a).max() < 1e-13
+
+
+# ----------------------------------------------------------------------------------------
+# external drive eta_n(t) (cav_set_drive; G27)
+# ----------------------------------------------------------------------------------------
+def _drive_for(w, t0=3e-12, sigma=1.5e-12):
+    N = w.omega.size
+    amp = (2e10 * (1 + np.arange(N)) * np.exp(0.7j * np.arange(N))).astype(np.complex128)
+    return dict(amp=amp, t0=np.full(N, t0), sigma=np.full(N, sigma), omega_d=np.asarray(w.omega) * 0.97)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,N,n_sub,dt", [((40, 9, 7), 3, 1, 0.1e-12), ((24, 6, 4), 1, 2, 0.02e-12)])
+def test_driven_fixed_steps(api, prec, shape, N, n_sub, dt, path):
+    """The pulse passes through the run (t0 = 30 / 150 steps in): every stage time t + c_s h matters."""
+    w = small_problem(*shape, N, n_sub)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    dr = _drive_for(w, t0=30 * dt, sigma=12 * dt)
+    ref = oracle_of(w, drive=dr).run(w.m0, w.a0, fixed_dt=dt, max_steps=80)
+    with open_sim(api, w, prec, path) as sim:
+        api.cav_set_drive(sim.h, dr["amp"], dr["t0"], dr["sigma"], dr["omega_d"])
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=80)
+        m, a = sim.get_m(), sim.get_a()
+        # switching the drive off again restores the undriven slopes
+        api.cav_set_drive(sim.h, None)
+        dadt_off = api.cav_get_dadt(sim.h, N)
+    assert_parity(m, a, ref, prec)
+    undriven = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=80)
+    assert np.abs(ref.a - undriven.a).max() > 0.05 * np.abs(undriven.a).max()       # the drive is not a detail here
+    _, da_ref, _ = oracle_of(w).rhs(ref.m, ref.a)
+    assert np.abs(dadt_off - da_ref).max() <= (1e-9 if prec == "f64" else 1e-3) * np.abs(da_ref).max()
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_driven_adaptive_closed_form(api, path):
+    """g = 0, fp64, adaptive: a(T) of the pulsed uncoupled cavity against the closed form the oracle is pinned with."""
+    w = W.macrospin(10.0, [9.0, 10.5], 0.0, [1.0, 50.0], alpha=1e-3, a0=[0, 0], n=4)
+    sig, t0, T = 20e-12, 0.2e-9, 0.5e-9
+    amp = np.array([1e9 * (1 + 0.5j), 2e9 * (-0.3 + 1j)])
+    wd = np.array([0.0, TWO_PI * 10.5e9])
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_drive(sim.h, amp, t0, sig, wd)
+        api.cav_run(sim.h, T, tol=1e-12)
+        a = sim.get_a()
+    lam = w.kappa + 1j * w.omega
+    exact = amp * sig * math.sqrt(TWO_PI) * np.exp((lam - 1j * wd) ** 2 * sig ** 2 / 2) * np.exp(-lam * (T - t0))
+    assert np.all(np.abs(a - exact) <= 3e-9 * np.abs(exact))
