@@ -293,6 +293,8 @@ def run_cuda(args):
     path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma"}[api.cav_get_kernel_path(h)]
     if args.no_stage_overlap:
         api.cav_set_stage_overlap(h, 0)
+    if args.no_serpentine:
+        api.cav_set_sweep_order(h, 0)
     N, nc = w.n_modes, w.n_cells
 
     # spin-up (setup, untimed): the controller grows dt from 1e-14 s to the stability-limited step
@@ -372,7 +374,7 @@ def run_cuda(args):
             "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": dict(config_of(w, prec, name), parallelism=f"replicas x{world} (no collective)",
                            launch_mode=args.launch_mode, kernel_path=path_used,
-                           stage_overlap=bool(overlap_active)),
+                           stage_overlap=bool(overlap_active), serpentine=not args.no_serpentine),
             "sim_ns_per_s": float(units[2]) * 1e9 / (ms_max * 1e-3) / world,
             "mean_dt_ps": sim_t * 1e12 / max(st1["accepted"] - st0["accepted"], 1),
             "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
@@ -494,6 +496,7 @@ def main():
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
     ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma"])
     ap.add_argument("--replicas", type=int, default=1184, help="cfg1_sweep: replicas in the batch")
+    ap.add_argument("--no-serpentine", action="store_true", help="every stage sweeps forward (A/B aid)")
     ap.add_argument("--no-stage-overlap", action="store_true", help="full dependencies between stage kernels (A/B aid)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":

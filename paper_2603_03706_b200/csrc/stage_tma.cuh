@@ -7,7 +7,8 @@
 //   * persistent grid, one CTA per SM; the flattened list of plane-tiles (x-y tile, z) is split
 //     into contiguous, equally long runs, one per CTA, so every SM gets the same number of
 //     planes and marches in z (each plane of m_s is fetched once per run, plus one halo plane
-//     per run end);
+//     per run end); odd stages walk their run backwards so that a stage starts on data the previous
+//     stage left in L2;
 //   * a producer warp (one elected lane) issues cp.async.bulk.tensor (TMA) loads of 4-D boxes
 //     [comp][1][TY(+2)][TX(+2 HX)] into three shared-memory rings — the stage state with its
 //     x/y halo (ring "ms": planes z-1, z, z+1 live), the mode profiles u_n in chunks of 8
@@ -222,9 +223,21 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     const long long q0 = (TA.Q * (long long)blockIdx.x) / gridDim.x;
     const long long q1 = (TA.Q * (long long)(blockIdx.x + 1)) / gridDim.x;
     const int nplanes = (int)(q1 - q0);
-    const long long t0 = q0 / nz;
-    const int z0 = (int)(q0 - t0 * nz);
+    // Sweep direction: odd stages walk their run backwards (cav_set_sweep_order), so a block starts stage s+1 on the
+    // plane-tiles it finished stage s with - their stage state, slopes, y0 and profiles are still in the 126 MB L2.
+    const int dir = (A.serpentine && (STAGE & 1)) ? -1 : 1;
+    const int zfirst = dir > 0 ? 0 : nz - 1, zlast = dir > 0 ? nz - 1 : 0;
+    const long long qs = dir > 0 ? q0 : q1 - 1;
+    const long long t0 = qs / nz;
+    const int z0 = (int)(qs - t0 * nz);
     const int tx0 = (int)(t0 % TA.ntx), ty0 = (int)(t0 / TA.ntx);
+    // next plane-tile of the run in sweep order; returns true when the tile column changes
+    auto advance = [&](int& z, int& tx, int& ty) -> bool {
+        z += dir;
+        if (z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } return true; }
+        if (z < 0) { z = nz - 1; if (--tx < 0) { tx = TA.ntx - 1; --ty; } return true; }
+        return false;
+    };
 
     // Each role fetches what it needs from Ctrl with ONE batch of independent loads (one L2 round trip after the
     // dependency wait): the producer four words, the consumers the whole struct or, in stages 1-2, a few fields.
@@ -297,7 +310,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                             ++pre_a;
                         }
                     }
-                    if (++zz == nz) { zz = 0; if (++txx == TA.ntx) { txx = 0; ++tyy; } }
+                    advance(zz, txx, tyy);
                 }
                 asm volatile("griddepcontrol.wait;" ::: "memory");
                 CAVMAG_MARK(13);
@@ -313,8 +326,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             };
             for (int p = 0; p < nplanes; ++p) {
                 const int x0 = tx * TX, y0 = ty * kTmaTY;
-                if (p == 0 || z == 0) { issue_ms(x0, y0, z - 1); issue_ms(x0, y0, z); }
-                issue_ms(x0, y0, z + 1);
+                if (p == 0 || z == zfirst) { issue_ms(x0, y0, z - dir); issue_ms(x0, y0, z); }
+                issue_ms(x0, y0, z + dir);
                 if constexpr (NB > 0) {
 #pragma unroll 1
                     for (int ch = 0; ch < NCH; ++ch) {       // mode profiles, UCB per slot (out-of-range modes zero-filled)
@@ -345,7 +358,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     }
                     if (++ha == Da) { ha = 0; pa ^= 1u; }
                 }
-                if (++z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } }
+                advance(z, tx, ty);
             }
             CAVMAG_MARK(6);
         }
@@ -450,8 +463,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 cell = (long long)z * plane + (long long)gy * nx + gx;
                 new_tile = false;
             }
-            const bool seg_start = (pl == 0 || z == 0);
-            const bool seg_end = (pl + 1 == nplanes || z == nz - 1);
+            const bool seg_start = (pl == 0 || z == zfirst);
+            const bool seg_end = (pl + 1 == nplanes || z == zlast);
             if (seg_start) { sm_zm = acquire_ms(); sm_zc = acquire_ms(); }
             sm_zp = acquire_ms();
             if (pl == 0 && tid == 0) CAVMAG_MARK(2);
@@ -516,8 +529,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     const int comp = s * 3 + c;
                     const P nym = ldm(sm_zc, comp, crow - kTmaHaloRowBytes);
                     const P nyp = ldm(sm_zc, comp, crow + kTmaHaloRowBytes);
-                    const P nzm = ldm(sm_zm, comp, crow);
-                    const P nzp = ldm(sm_zp, comp, crow);
+                    const P nzm = ldm(dir > 0 ? sm_zm : sm_zp, comp, crow);      // sm_zm / sm_zp: previous / next plane of the sweep
+                    const P nzp = ldm(dir > 0 ? sm_zp : sm_zm, comp, crow);
                     T xl = __shfl_up_sync(0xffffffffu, mc[s][c].v[VEC - 1], 1);
                     T xr = __shfl_down_sync(0xffffffffu, mc[s][c].v[0], 1);
                     if (lane == 0) xl = ldm1(sm_zc, comp, crow - (unsigned)sizeof(T));
@@ -657,8 +670,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 if (seg_end) { release_ms(); release_ms(); }    // planes z, z+1 (the next segment reloads its own)
             }
             sm_zm = sm_zc; sm_zc = sm_zp;
-            cell += plane;
-            if (++z == nz) { z = 0; if (++tx == TA.ntx) { tx = 0; ++ty; } new_tile = true; }
+            cell += dir > 0 ? plane : -plane;
+            if (advance(z, tx, ty)) new_tile = true;
         }
 
         if (tid == 0) CAVMAG_MARK(3);
