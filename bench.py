@@ -483,6 +483,100 @@ def run_batch(args):
     print(json.dumps(line), flush=True)
 
 
+# ----------------------------------------------------------------------------------------
+# the 41-point field sweep of configs[1] as concurrent simulations: --workload cfg2_sweep
+# ----------------------------------------------------------------------------------------
+def run_concurrent_sweep(args):
+    """BASELINE.json configs[1] (64x64x16 cells, two sine modes, fp32, adaptive tol 1e-6) at its 41 field values:
+    41 independent cav_run graphs on 41 streams, launched back to back (cav_run_steps is asynchronous), timed by
+    CUDA events on a master stream that every simulation stream waits on / is waited for."""
+    import torch
+    import cavmag_workloads as W
+    from paper_2603_03706_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    ghz = W.cfg2_sweep_ghz()
+    ws = [W.cfg2(f_kittel_ghz=float(f), seed=2000 + i) for i, f in enumerate(ghz)]
+    streams = [torch.cuda.Stream() for _ in ws]
+    sims = [api.Sim(w, precision="f32", stream=st.cuda_stream) for w, st in zip(ws, streams)]
+    tol, nc, N = ws[0].tol, ws[0].n_cells, ws[0].n_modes
+    master = torch.cuda.Stream()
+
+    def run_all(k):
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record(master)
+        ends = []
+        for sim, st in zip(sims, streams):
+            st.wait_event(ev0)
+            api.cav_run_steps(sim.h, math.inf, tol=tol, max_steps=k)
+            e = torch.cuda.Event(); e.record(st); ends.append(e)
+        for e in ends:
+            master.wait_event(e)
+        ev1.record(master)
+        master.synchronize()
+        return ev0.elapsed_time(ev1)
+
+    run_all(args.spinup)
+    run_all(max(args.warmup, 3))
+    st0 = [api.cav_get_stats(s.h) for s in sims]
+    sampler = ClockSampler(torch.cuda.current_device())
+    torch.cuda.synchronize()
+    sampler.start()
+    ms = run_all(args.steps)
+    clocks = sampler.stop()
+    st1 = [api.cav_get_stats(s.h) for s in sims]
+    evals = sum(b["rhs_evals"] - a["rhs_evals"] for a, b in zip(st0, st1))
+    sim_t = sum(b["t"] - a["t"] for a, b in zip(st0, st1))
+    # one simulation alone, same graph: the latency-bound single-run number
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(streams[0]); api.cav_run_steps(sims[0].h, math.inf, tol=tol, max_steps=args.steps); e1.record(streams[0])
+    streams[0].synchronize()
+    single = nc * 6 * args.steps / (e0.elapsed_time(e1) * 1e-3)
+    # e2e: host buffers, every step, all simulations
+    k_e2e = min(args.e2e_steps, 20)
+    hosts = [torch.empty(s.shape_m, dtype=torch.float32).pin_memory() for s in sims]
+    for s, hbuf in zip(sims, hosts):
+        api.cav_get_m(s.h, hbuf)
+    a_hosts = [api.cav_get_a(s.h, N) for s in sims]
+    se0 = [api.cav_get_stats(s.h) for s in sims]
+    t0 = time.perf_counter()
+    for _ in range(k_e2e):
+        for i, s in enumerate(sims):
+            api.cav_set_m(s.h, hosts[i]); api.cav_set_a(s.h, a_hosts[i])
+            api.cav_run_steps(s.h, math.inf, tol=tol, max_steps=1)
+        for i, s in enumerate(sims):
+            api.cav_get_m(s.h, hosts[i]); a_hosts[i] = api.cav_get_a(s.h, N)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    se1 = [api.cav_get_stats(s.h) for s in sims]
+    e2e_evals = sum(b["rhs_evals"] - a["rhs_evals"] for a, b in zip(se0, se1))
+    launches = sum(api.cav_get_launch_count(s.h) for s in sims)
+    for s in sims:
+        s.close()
+    value = nc * evals / (ms * 1e-3)
+    bytes_per_cs = algorithmic_bytes_per_cell_step(N, 1, 4) / 6.0
+    achieved = value * bytes_per_cs / 1e9
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    peak = float(json.load(open(peaks_path))["hbm_gbs"]) if os.path.exists(peaks_path) else 6650.0
+    io = int(np.prod(sims[0].shape_m)) * 4 * len(sims) + 16 * N * len(sims)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "cfg2_sweep", "grid": [ws[0].nx, ws[0].ny, ws[0].nz], "cells": nc, "simulations": len(sims),
+                       "modes": N, "mode": "adaptive RK45; 41 cav_run graphs on 41 streams", "tol": tol,
+                       "l2": "41 x 8.7 MB of cell fields = 355 MB in total exceeds the 126 MB L2"},
+            "sim_ns_per_s": sim_t * 1e9 / (ms * 1e-3), "clocks": clocks,
+            "e2e": {"value": nc * e2e_evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": io, "d2h_bytes_per_step": io,
+                    "steps": k_e2e, "ms_per_step": 1e3 * e2e_s / k_e2e},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "cavmag::k_stage (generic path, 128 blocks per launch, 41 concurrent graphs)"},
+            "single_simulation_cell_stage_per_s": single,
+            "speedup_vs_one_simulation_at_a_time": value / single}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -505,6 +599,8 @@ def main():
         run_reference(args)
     elif args.workload == "cfg1_sweep":
         run_batch(args)
+    elif args.workload == "cfg2_sweep":
+        run_concurrent_sweep(args)
     else:
         run_cuda(args)
 
