@@ -52,7 +52,7 @@ typedef enum {
     CAV_E_NONFINITE = -5,     /* error norm became NaN/Inf in fixed-step mode */
     CAV_E_DT_UNDERFLOW = -6,  /* adaptive step proposal fell below 1e-20 s */
     CAV_E_SINGULAR_NORM = -7, /* CAV_NORM_SUM_U with |sum_r u_n| < 1e-6 N_cells */
-    CAV_E_UNSUPPORTED = -8    /* no CUDA device / device is not sm_100 */
+    CAV_E_UNSUPPORTED = -8    /* no CUDA device / device is not sm_100 / requested kernel path not eligible for this problem */
 } cav_status;
 
 enum { CAV_F32 = 0, CAV_F64 = 1 };

@@ -488,7 +488,7 @@ const char* cav_strerror(int st) {
         case CAV_E_NONFINITE: return "non-finite error norm";
         case CAV_E_DT_UNDERFLOW: return "step size underflow";
         case CAV_E_SINGULAR_NORM: return "sum of mode profile is ~0 (CAV_NORM_SUM_U)";
-        case CAV_E_UNSUPPORTED: return "no supported CUDA device";
+        case CAV_E_UNSUPPORTED: return "unsupported: no sm_100 CUDA device, or the requested kernel path does not fit this problem";
         default: return "unknown status";
     }
 }
