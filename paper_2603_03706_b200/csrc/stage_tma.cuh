@@ -143,7 +143,13 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
         const int idx = tidc + k * kTmaConsumers;
         if (idx < kCtrlWords) sc_words[idx] = cw[k];
     }
+#ifdef CAVMAG_PROBE
+    if (tidc == 0) probe_mark(A, PREV + 1, 9);          // Ctrl + partials have landed (this thread's share)
+#endif
     asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+#ifdef CAVMAG_PROBE
+    if (tidc == 0) probe_mark(A, PREV + 1, 10);         // all consumers' shares are in shared memory
+#endif
     Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
     if (c->done) return false;                      // launched after the run ended (host-enqueued mode): nothing to do
     if (tidc < c->N) {

@@ -25,7 +25,8 @@ if ROOT not in sys.path:
 SLOTS = 32          # per block: [0..15] %globaltimer ns, [16..31] clock64, by mark index
 MARKS = {0: "entry", 1: "control data ready (consumers)", 2: "first tile acquired", 3: "main loop done",
          4: "ticket (stages 1, 7)", 5: "exit", 6: "producer: all loads issued", 13: "producer: dependency wait returned",
-         15: "consumers: dependency wait returned"}
+         15: "consumers: dependency wait returned", 9: "deferred finish: own loads landed",
+         10: "deferred finish: all loads in smem"}
 
 
 def main():
@@ -63,7 +64,7 @@ def main():
             v = (g[:, col] - t0) / 1e3
             return [round(float(x), 2) for x in np.percentile(v, [0, 50, 100])]
 
-        d = {MARKS[k]: mmm(k) for k in ((0, 15, 13, 1, 2, 6, 3, 5) if st >= 3 else (0, 15, 1, 2, 6, 3, 5))}
+        d = {MARKS[k]: mmm(k) for k in ((0, 15, 13, 9, 10, 1, 2, 6, 3, 5) if st >= 3 else (0, 15, 1, 2, 6, 3, 5))}
         d["main loop, median us"] = round(float(np.median(g[:, 3] - g[:, 2]) / 1e3), 2)
         d["main loop, slowest / median"] = round(float((g[:, 3] - g[:, 2]).max() / np.median(g[:, 3] - g[:, 2])), 3)
         if st == 7:
