@@ -75,11 +75,12 @@ __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, 
 }
 
 
-// MAXT: block-size bucket (128 / 256 / 512 / 1024 threads) - the register budget per thread follows from it.  The 512-thread
-// ferromagnet bucket asks for two blocks per SM (64 registers, < 100 B of spills): barrier stalls of one replica hide
-// behind the other.
-template <typename T, int NSUB, int MAXT>
-__global__ void __launch_bounds__(MAXT, (MAXT == 512 && NSUB == 1) ? 2 : 1) k_batch(const BatchArgs A) {
+// MAXT: block-size bucket (128 / 256 / 512 / 1024 threads) - the register budget per thread follows from it.  MINB = 2 (the
+// 512-thread ferromagnet bucket, chosen by the host when there are more replicas than SMs) asks for two blocks per SM: 64
+// registers and < 100 B of spills make one replica ~10 % slower, but the barrier stalls of one replica hide behind the
+// other (+31 % with 1184 replicas of CFG1).
+template <typename T, int NSUB, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
     extern __shared__ __align__(16) unsigned char batch_dsm[];
     __shared__ BatchShared sh;
     const int nc = A.nc, N = A.N;

@@ -30,6 +30,7 @@ struct cav_batch {
     int trace_cap = 0;
     bool m_set = false;
     size_t smem_optin = 0;
+    int n_sm = 148;
     char cuda_err[256] = {0};
 };
 
@@ -60,11 +61,14 @@ __global__ void k_batch_normalize(T* m, int nc, int n_sub, int n_rep) {
 int row_len_of(const cav_batch* b) { return 1 + 4 * b->N + 3 * b->prm.n_sub; }
 
 template <typename T, int NSUB>
-const void* batch_fn(int threads) {
-    if (threads <= 128) return (const void*)k_batch<T, NSUB, 128>;
-    if (threads <= 256) return (const void*)k_batch<T, NSUB, 256>;
-    if (threads <= 512) return (const void*)k_batch<T, NSUB, 512>;
-    return (const void*)k_batch<T, NSUB, 1024>;
+const void* batch_fn(int threads, bool two_per_sm) {
+    if (threads <= 128) return (const void*)k_batch<T, NSUB, 128, 1>;
+    if (threads <= 256) return (const void*)k_batch<T, NSUB, 256, 1>;
+    if (threads <= 512) {
+        if constexpr (NSUB == 1) { if (two_per_sm) return (const void*)k_batch<T, NSUB, 512, 2>; }
+        return (const void*)k_batch<T, NSUB, 512, 1>;
+    }
+    return (const void*)k_batch<T, NSUB, 1024, 1>;
 }
 
 int pull_ctl(cav_batch* b, std::vector<BatchCtl>& h) {
@@ -98,6 +102,7 @@ int cav_batch_create(const cav_grid* grid, const cav_params* prm, int n_rep, cav
     b->grid = *grid; b->prm = *prm; b->n_rep = n_rep; b->nc = (int)nc;
     b->esize = prm->precision == CAV_F32 ? 4 : 8;
     b->smem_optin = dp.sharedMemPerBlockOptin;
+    b->n_sm = dp.multiProcessorCount;
     auto fail = [&](int code) { cav_batch_destroy(b); return code; };
     if (cudaStreamCreateWithFlags(&b->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(CAV_E_CUDA);
     b->own_stream = true;
@@ -304,8 +309,9 @@ int cav_batch_run(cav_batch* b, double t_end, double tol, double fixed_dt, doubl
     int threads = (b->nc + 31) / 32 * 32;
     if (threads < 64) threads = 64;
     const size_t ms_bytes = (size_t)p.n_sub * 3 * b->nc * b->esize, u_bytes = (size_t)b->N * b->nc * b->esize;
-    const void* fn = p.precision == CAV_F32 ? (p.n_sub == 1 ? batch_fn<float, 1>(threads) : batch_fn<float, 2>(threads))
-                                            : (p.n_sub == 1 ? batch_fn<double, 1>(threads) : batch_fn<double, 2>(threads));
+    const bool two = b->n_rep > b->n_sm;         // more replicas than SMs: throughput over single-replica latency
+    const void* fn = p.precision == CAV_F32 ? (p.n_sub == 1 ? batch_fn<float, 1>(threads, two) : batch_fn<float, 2>(threads, two))
+                                            : (p.n_sub == 1 ? batch_fn<double, 1>(threads, two) : batch_fn<double, 2>(threads, two));
     cudaFuncAttributes fa;
     CKB(cudaFuncGetAttributes(&fa, fn));
     const size_t room = b->smem_optin > fa.sharedSizeBytes ? b->smem_optin - fa.sharedSizeBytes : 0;
