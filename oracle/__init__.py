@@ -26,7 +26,8 @@ class _Problem(C.Structure):
                 ("B0", C.c_double * 3), ("n_sub", C.c_int), ("B_exch_inter", C.c_double),
                 ("renormalize", C.c_int), ("norm_sum_u", C.c_int), ("N", C.c_int),
                 ("u", _dp), ("omega", _dp), ("kappa", _dp), ("g", _dp), ("Gamma", _dp), ("Phi", _dp),
-                ("eta_amp", _dp), ("eta_t0", _dp), ("eta_sigma", _dp), ("eta_wd", _dp)]
+                ("eta_amp", _dp), ("eta_t0", _dp), ("eta_sigma", _dp), ("eta_wd", _dp),
+                ("g_b", _dp), ("Gamma_b", _dp), ("Phi_b", _dp)]
 
 
 class _Stats(C.Structure):
@@ -80,7 +81,8 @@ class Oracle:
     """One problem instance (grid + material + modes), built from a cavmag_workloads.Workload
     or from keyword arguments with the same names."""
 
-    def __init__(self, w=None, renormalize: bool = True, norm_sum_u: bool = False, drive: Optional[dict] = None, **kw):
+    def __init__(self, w=None, renormalize: bool = True, norm_sum_u: bool = False, drive: Optional[dict] = None,
+                 backward: Optional[dict] = None, **kw):
         """drive = dict(amp [N] complex, t0 [N], sigma [N], omega_d [N] or None): the Gaussian-pulse drive
         eta_n(t) = amp_n exp(-(t-t0_n)^2/(2 sigma_n^2)) exp(-i omega_d,n (t-t0_n)) of Eq. 1 / Eq. 12."""
         get = (lambda k: kw[k] if k in kw else getattr(w, k))
@@ -110,6 +112,13 @@ class Oracle:
             wd = drive.get("omega_d")
             self.eta_wd = None if wd is None else _c64(np.broadcast_to(np.asarray(wd, dtype=np.float64), (self.N,)))
             P.eta_amp, P.eta_t0, P.eta_sigma, P.eta_wd = _p(self.eta_amp), _p(self.eta_t0), _p(self.eta_sigma), _p(self.eta_wd)
+        if backward is not None and self.N:
+            # non-reciprocal coupling: backward = dict(g [N], Gamma [N] or None, Phi [N] or None)
+            self.g_b = _c64(np.broadcast_to(np.asarray(backward["g"], dtype=np.float64), (self.N,)))
+            Gb, Pb = backward.get("Gamma"), backward.get("Phi")
+            self.Gamma_b = None if Gb is None else _c64(np.broadcast_to(np.asarray(Gb, dtype=np.float64), (self.N,)))
+            self.Phi_b = None if Pb is None else _c64(np.broadcast_to(np.asarray(Pb, dtype=np.float64), (self.N,)))
+            P.g_b, P.Gamma_b, P.Phi_b = _p(self.g_b), _p(self.Gamma_b), _p(self.Phi_b)
         self.P = P
         self.nc = self.nx * self.ny * self.nz
         self.gamma = P.gamma

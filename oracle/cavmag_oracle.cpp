@@ -18,7 +18,8 @@
 //        da_n/dt = -(i w_n + kappa_n) a_n + i G_n S_n + eta_n(t)   PAPER.md:119 Eq.12, :317 Eq.19
 //        eta_n(t) = A_n exp(-(t-t0_n)^2/(2 sigma_n^2)) exp(-i w_d,n (t-t0_n))   Gaussian pulse
 //        (evaluated at the stage times t + c_s h; absent unless drive arrays are given - reading G27)
-//    (4) c_n  = (2/gamma) Re[G_n a_n];  B_rf(r) = x^ sum_n c_n u_n(r)
+//    (4) c_n  = (2/gamma) Re[G_b,n a_n];  B_rf(r) = x^ sum_n c_n u_n(r)      (G_b = G unless a separate backward
+//        coupling is given: non-reciprocal g_f != g_b with h0 = 2 g_b/gamma)
 //                                                           PAPER.md:65 Eq.5, :121 Eq.13, :159
 //    (5) B_s  = B0 + (2A/Ms) sum_{d,+-} [m_s(r +- e_d) - m_s(r)]/D_d^2   (open boundary)
 //             + (2Ku/Ms)(m_s . k^) k^ + B_rf - B_E m_other
@@ -67,6 +68,11 @@ struct orc_problem {
     const double* eta_t0;    // [N] pulse centre, s
     const double* eta_sigma; // [N] pulse width, s
     const double* eta_wd;    // [N] carrier, rad/s (NULL: baseband pulse)
+    // non-reciprocal coupling: backward (cavity-to-magnon) coupling G_b = g_b + Gamma_b e^{i Phi_b} used in
+    // the feedback field h0 = 2 g_b / gamma; g_b == NULL: reciprocal (G_b = G)
+    const double* g_b;       // [N] rad/s
+    const double* Gamma_b;   // [N] rad/s (NULL: 0)
+    const double* Phi_b;     // [N] rad   (NULL: 0)
 };
 
 struct orc_stats {
@@ -148,7 +154,13 @@ void rhs(const orc_problem* P, double t, const double* m, const double* a, doubl
         // i G S             =  (-(Gre Sim + Gim Sre)) + i (Gre Sre - Gim Sim)
         da[2 * n + 0] = (-P->kappa[n] * are + P->omega[n] * aim) - (Gre * Sim + Gim * Sre);
         da[2 * n + 1] = (-P->kappa[n] * aim - P->omega[n] * are) + (Gre * Sre - Gim * Sim);
-        c[n] = (2.0 / P->gamma) * (Gre * are - Gim * aim);   // (2/gamma) Re[G a]
+        double Gbre = Gre, Gbim = Gim;                        // backward coupling: reciprocal unless given
+        if (P->g_b) {
+            const double Gm = P->Gamma_b ? P->Gamma_b[n] : 0.0, Ph = P->Phi_b ? P->Phi_b[n] : 0.0;
+            Gbre = P->g_b[n] + Gm * std::cos(Ph);
+            Gbim = Gm * std::sin(Ph);
+        }
+        c[n] = (2.0 / P->gamma) * (Gbre * are - Gbim * aim);   // (2/gamma) Re[G_b a]
         if (P->eta_amp) {   // + eta_n(t): Gaussian envelope times carrier e^{-i w_d (t - t0)}
             const double x = t - P->eta_t0[n];
             const double env = std::exp(-(x * x) / (2.0 * P->eta_sigma[n] * P->eta_sigma[n]));

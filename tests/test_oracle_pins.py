@@ -632,3 +632,31 @@ def test_pulse_spectroscopy_shows_both_polariton_branches():
     f = om2.real / TWO_PI
     assert abs(f[0] - (10e9 - g_mhz * 1e6)) < 1e6 and abs(f[1] - (10e9 + g_mhz * 1e6)) < 1e6
     assert 0.8 < abs(amp2[0]) / abs(amp2[1]) < 1.25
+
+
+# ----------------------------------------------------------------------------------------
+# non-reciprocal coupling g_f != g_b (h0 = 2 g_b / gamma for the backward channel)
+# ----------------------------------------------------------------------------------------
+def test_nonreciprocal_coupling_geometric_mean():
+    """Forward coefficient i g_f (Eq. 1), backward field h0 = 2 g_b/gamma: the linearised pair has
+    (w - w_c)(w - w_m) = g_f g_b, i.e. the splitting and the Rabi period of a reciprocal system with g = sqrt(g_f g_b):
+    g_f/2pi = 100 MHz, g_b/2pi = 25 MHz  ->  T_R = pi / (2pi 50 MHz) = 10 ns, like PAPER.md:237-239's g/2pi = 50 MHz."""
+    w = W.macrospin(5.0, [5.0], 100.0, 0.0, alpha=0.0, a0=[0.01], n=2)
+    o = Oracle(w, backward=dict(g=np.array([TWO_PI * 25e6])))
+    r = o.run(w.m0, w.a0, t_end=26e-9, tol=1e-9, sample_dt=25e-12, trace_cap=1040)
+    T = rabi_period(r.trace[:, 0], r.trace[:, 1] ** 2 + r.trace[:, 2] ** 2)
+    assert abs(T / 10e-9 - 1) < 2e-3
+    # the reciprocal system with g_f alone would oscillate twice as fast
+    r2 = Oracle(w).run(w.m0, w.a0, t_end=26e-9, tol=1e-9, sample_dt=25e-12, trace_cap=1040)
+    T2 = rabi_period(r2.trace[:, 0], r2.trace[:, 1] ** 2 + r2.trace[:, 2] ** 2)
+    assert abs(T2 / 5e-9 - 1) < 2e-3
+    # energy bookkeeping is asymmetric: the magnon amplitude reached is scaled by sqrt(g_b/g_f) relative to the
+    # reciprocal case with the geometric-mean coupling (same a(0))
+    w3 = W.macrospin(5.0, [5.0], 50.0, 0.0, alpha=0.0, a0=[0.01], n=2)
+    r3 = Oracle(w3).run(w3.m0, w3.a0, t_end=26e-9, tol=1e-9, sample_dt=25e-12, trace_cap=1040)
+    S_max, S3_max = np.abs(r.trace[:, 3] + 1j * r.trace[:, 4]).max(), np.abs(r3.trace[:, 3] + 1j * r3.trace[:, 4]).max()
+    assert abs(S_max / S3_max - math.sqrt(25.0 / 100.0)) < 0.01
+    # giving the backward coupling equal to the forward one changes nothing
+    r4 = Oracle(w, backward=dict(g=w.g, Gamma=w.Gamma, Phi=w.Phi)).run(w.m0, w.a0, fixed_dt=0.5e-12, max_steps=200)
+    r5 = Oracle(w).run(w.m0, w.a0, fixed_dt=0.5e-12, max_steps=200)
+    assert np.array_equal(r4.m, r5.m) and np.array_equal(r4.a, r5.a)
