@@ -115,6 +115,12 @@ int cav_set_launch_mode(cav_sim* sim, int mode);
 int cav_set_modes(cav_sim* sim, int N, const void* u, int u_is_device, const double* omega,
                   const double* kappa, const double* g, const double* Gamma, const double* Phi);
 
+/* Non-reciprocal coupling: a backward (cavity-to-magnon) coupling G_b,n = g_b,n + Gamma_b,n e^{i Phi_b,n}
+ * for the feedback field, B_rf,x = (2/gamma) sum_n u_n Re[G_b,n a_n] (h0 = 2 g_b/gamma), while the mode ODE keeps the forward
+ * coefficient i G_n of cav_set_modes.  Host arrays [N] (rad/s, rad); Gamma_b, Phi_b may be NULL (= 0); g_b == NULL restores
+ * reciprocal coupling (G_b = G).  Call after cav_set_modes (a new mode set is reciprocal again). */
+int cav_set_backaction(cav_sim* sim, const double* g_b, const double* Gamma_b, const double* Phi_b);
+
 /* External microwave drive eta_n(t) of Eq. 1 / Eq. 12, as the Gaussian pulse of the paper's
  * spectroscopy protocol (sigma = 20 ps, t0 = 0.1 ns) with an optional carrier (reading G27):
  *     eta_n(t) = A_n exp(-(t - t0_n)^2 / (2 sigma_n^2)) exp(-i omega_d,n (t - t0_n)),
@@ -222,6 +228,9 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
  * normalised per cell on entry.  Amplitudes [N][2] or [n_rep][N][2]. */
 int cav_batch_set_m(cav_batch* b, const void* m, int per_replica);
 int cav_batch_set_a(cav_batch* b, const double* a_re_im, int per_replica);
+
+/* Backward coupling as cav_set_backaction, common to all replicas ([N] arrays).  Call after cav_batch_set_modes. */
+int cav_batch_set_backaction(cav_batch* b, const double* g_b, const double* Gamma_b, const double* Phi_b);
 
 /* Drive as cav_set_drive, common to all replicas ([N] arrays).  Call after cav_batch_set_modes. */
 int cav_batch_set_drive(cav_batch* b, const double* amp_re_im, const double* t0, const double* sigma, const double* omega_d);

@@ -64,6 +64,8 @@ _SIGS = {
     "cav_set_launch_mode": ([_vp, _i], _i),
     "cav_set_modes": ([_vp, _i, _vp, _i, _dp, _dp, _dp, _dp, _dp], _i),
     "cav_set_drive": ([_vp, _dp, _dp, _dp, _dp], _i),
+    "cav_set_backaction": ([_vp, _dp, _dp, _dp], _i),
+    "cav_batch_set_backaction": ([_vp, _dp, _dp, _dp], _i),
     "cav_set_m": ([_vp, _vp, _i], _i),
     "cav_get_m": ([_vp, _vp, _i], _i),
     "cav_set_a": ([_vp, _dp], _i),
@@ -425,6 +427,27 @@ def _drive_args(amp, t0, sigma, omega_d):
     ps, ks = _darr(np.broadcast_to(np.asarray(sigma, dtype=np.float64), (n,)), n)
     pw, kw = _darr(None if omega_d is None else np.broadcast_to(np.asarray(omega_d, dtype=np.float64), (n,)), n)
     return (a.ctypes.data_as(_dp), pt, ps, pw), (a, kt, ks, kw)
+
+
+def _back_args(g_b, Gamma_b, Phi_b):
+    if g_b is None:
+        return (None, None, None), ()
+    n = int(np.asarray(g_b).size)
+    pg, kg = _darr(g_b, n)
+    pG, kG = _darr(Gamma_b, n)
+    pP, kP = _darr(Phi_b, n)
+    return (pg, pG, pP), (kg, kG, kP)
+
+
+def cav_set_backaction(sim, g_b, Gamma_b=None, Phi_b=None) -> None:
+    """Backward coupling of the feedback field ([N] arrays; g_b None = reciprocal again)."""
+    args, keep = _back_args(g_b, Gamma_b, Phi_b)
+    _check(_lib.cav_set_backaction(sim, *args), "cav_set_backaction", sim)
+
+
+def cav_batch_set_backaction(b, g_b, Gamma_b=None, Phi_b=None) -> None:
+    args, keep = _back_args(g_b, Gamma_b, Phi_b)
+    _check(_lib.cav_batch_set_backaction(b, *args), "cav_batch_set_backaction")
 
 
 def cav_set_drive(sim, amp, t0=None, sigma=None, omega_d=None) -> None:

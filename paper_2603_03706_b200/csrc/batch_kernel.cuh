@@ -34,7 +34,7 @@ struct BatchArgs {
     int renormalize;
     const double* B0;             // [n_rep][3]
     const void* u;                // [N][nc] T
-    const double* modep;          // [n_rep or 1][5][N]: omega, kappa, Gre, Gim, invW
+    const double* modep;          // [n_rep or 1][7][N]: omega, kappa, Gre, Gim, invW, Gbre, Gbim
     int modep_per_rep;
     void* m;                      // [n_rep][NSUB][3][nc] T, in/out
     double* a;                    // [n_rep][N][2], in/out
@@ -50,7 +50,7 @@ struct BatchArgs {
 
 // Shared mode / controller state of one replica.
 struct BatchShared {
-    double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes];
+    double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes], Gbre[kMaxModes], Gbim[kMaxModes];
     double a[kMaxModes][2], as[kMaxModes][2], anew[kMaxModes][2], ka[7][kMaxModes][2], S[kMaxModes][2];
     double c[kMaxModes], serr[kMaxModes];
     double eta_re[kMaxModes], eta_im[kMaxModes], eta_t0[kMaxModes], eta_i2s2[kMaxModes], eta_wd[kMaxModes];
@@ -71,7 +71,7 @@ __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, 
     for (int j = 0; j < ROW; ++j) { re += kA[ROW][j] * sh.ka[j][n][0]; im += kA[ROW][j] * sh.ka[j][n][1]; }
     const double are = sh.a[n][0] + sh.h * re, aim = sh.a[n][1] + sh.h * im;
     sh.as[n][0] = are; sh.as[n][1] = aim;
-    sh.c[n] = two_over_gamma * (sh.Gre[n] * are - sh.Gim[n] * aim);
+    sh.c[n] = two_over_gamma * (sh.Gbre[n] * are - sh.Gbim[n] * aim);
 }
 
 
@@ -115,13 +115,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
     if (A.u_in_smem)
         for (int i = tid; i < N * nc; i += blockDim.x) sm_u[i] = ug[i];
     if (tid < N) {
-        const double* mp = A.modep + (A.modep_per_rep ? (size_t)rep * 5 * N : 0);
+        const double* mp = A.modep + (A.modep_per_rep ? (size_t)rep * 7 * N : 0);
         sh.omega[tid] = mp[tid]; sh.kappa[tid] = mp[N + tid]; sh.Gre[tid] = mp[2 * N + tid];
         sh.Gim[tid] = mp[3 * N + tid]; sh.invW[tid] = mp[4 * N + tid];
+        sh.Gbre[tid] = mp[5 * N + tid]; sh.Gbim[tid] = mp[6 * N + tid];
         const double are = A.a[((size_t)rep * N + tid) * 2], aim = A.a[((size_t)rep * N + tid) * 2 + 1];
         sh.a[tid][0] = are; sh.a[tid][1] = aim;
         sh.as[tid][0] = are; sh.as[tid][1] = aim;                       // stage 1 evaluates f(m_0, a_0)
-        sh.c[tid] = A.two_over_gamma * (sh.Gre[tid] * are - sh.Gim[tid] * aim);
+        sh.c[tid] = A.two_over_gamma * (sh.Gbre[tid] * are - sh.Gbim[tid] * aim);
         if (A.drive) {
             sh.eta_re[tid] = A.drive[tid]; sh.eta_im[tid] = A.drive[N + tid]; sh.eta_t0[tid] = A.drive[2 * N + tid];
             sh.eta_i2s2[tid] = A.drive[3 * N + tid]; sh.eta_wd[tid] = A.drive[4 * N + tid];

@@ -109,7 +109,7 @@ __global__ void k_begin(Ctrl* c, unsigned long long handle) {
     if (tid < c->N) {
         if (!c->k1_valid) {      // stage 1 evaluates f(m_0, a_0)
             c->as[1][tid][0] = c->a[tid][0]; c->as[1][tid][1] = c->a[tid][1];
-            c->c[tid] = c->two_over_gamma * (c->Gre[tid] * c->a[tid][0] - c->Gim[tid] * c->a[tid][1]);
+            c->c[tid] = c->two_over_gamma * (c->Gbre[tid] * c->a[tid][0] - c->Gbim[tid] * c->a[tid][1]);
         } else {
             mode_stage_state<1>(c, tid);
         }
@@ -668,6 +668,7 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         c->kappa[n] = kappa[n];
         c->Gre[n] = g[n] + Gm * std::cos(Ph);
         c->Gim[n] = Gm * std::sin(Ph);
+        c->Gbre[n] = c->Gre[n]; c->Gbim[n] = c->Gim[n];      // reciprocal until cav_set_backaction
         c->invW[n] = 1.0 / (double)s->nc;
         c->a[n][0] = c->a[n][1] = 0.0;
     }
@@ -698,6 +699,24 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
     s->graph_dirty = true;
     rc = plan_tma(s);
     if (rc) return rc;
+    return push_ctrl(s);
+}
+
+int cav_set_backaction(cav_sim* s, const double* g_b, const double* Gamma_b, const double* Phi_b) {
+    if (!s) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    Ctrl* c = s->h_ctrl;
+    for (int n = 0; n < c->N; ++n) {
+        if (g_b) {
+            const double Gm = Gamma_b ? Gamma_b[n] : 0.0, Ph = Phi_b ? Phi_b[n] : 0.0;
+            c->Gbre[n] = g_b[n] + Gm * std::cos(Ph);
+            c->Gbim[n] = Gm * std::sin(Ph);
+        } else {
+            c->Gbre[n] = c->Gre[n]; c->Gbim[n] = c->Gim[n];
+        }
+    }
+    c->k1_valid = 0;                     // dm/dt of the current state changes
     return push_ctrl(s);
 }
 

@@ -20,6 +20,7 @@ struct cav_batch {
     double* d_B0 = nullptr;
     void* d_u = nullptr;
     double* d_modep = nullptr;
+    std::vector<double> h_modep;   // host mirror of d_modep
     double* d_drive = nullptr;     // [5][N] or NULL: no drive
     int modep_per_rep = 0;
     void* d_m = nullptr;
@@ -110,7 +111,7 @@ int cav_batch_create(const cav_grid* grid, const cav_params* prm, int n_rep, cav
     if (cudaMalloc(&b->d_B0, sizeof(double) * 3 * n_rep) != cudaSuccess || cudaMalloc(&b->d_m, mbytes) != cudaSuccess ||
         cudaMalloc(&b->d_ctl, sizeof(BatchCtl) * n_rep) != cudaSuccess ||
         cudaMalloc(&b->d_a, sizeof(double) * 2 * CAV_MAX_MODES * n_rep) != cudaSuccess ||
-        cudaMalloc(&b->d_modep, sizeof(double) * 5 * CAV_MAX_MODES * n_rep) != cudaSuccess) {
+        cudaMalloc(&b->d_modep, sizeof(double) * 7 * CAV_MAX_MODES * n_rep) != cudaSuccess) {
         cudaGetLastError();
         return fail(CAV_E_NOMEM);
     }
@@ -180,21 +181,44 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
             }
         }
         const int reps = per_replica ? b->n_rep : 1;
-        std::vector<double> mp((size_t)reps * 5 * N);
+        std::vector<double> mp((size_t)reps * 7 * N);
         for (int r = 0; r < reps; ++r)
             for (int n = 0; n < N; ++n) {
                 const size_t i = (size_t)r * N + n;
                 const double Gm = Gamma ? Gamma[i] : 0.0, Ph = Phi ? Phi[i] : 0.0;
-                double* q = mp.data() + (size_t)r * 5 * N;
+                double* q = mp.data() + (size_t)r * 7 * N;
                 q[n] = omega[i]; q[N + n] = kappa[i];
                 q[2 * N + n] = g[i] + Gm * std::cos(Ph); q[3 * N + n] = Gm * std::sin(Ph); q[4 * N + n] = invW[n];
+                q[5 * N + n] = q[2 * N + n]; q[6 * N + n] = q[3 * N + n];          // reciprocal until cav_batch_set_backaction
             }
+        b->h_modep = mp;
         CKB(cudaMemcpyAsync(b->d_modep, mp.data(), sizeof(double) * mp.size(), cudaMemcpyHostToDevice, b->stream));
         CKB(cudaStreamSynchronize(b->stream));
     }
     CKB(cudaMemsetAsync(b->d_a, 0, sizeof(double) * 2 * CAV_MAX_MODES * b->n_rep, b->stream));
     cudaFree(b->d_trace);
     b->d_trace = nullptr; b->trace_cap = 0; b->sample_dt = 0.0;      // the row length changed
+    CKB(cudaStreamSynchronize(b->stream));
+    return CAV_OK;
+}
+
+int cav_batch_set_backaction(cav_batch* b, const double* g_b, const double* Gamma_b, const double* Phi_b) {
+    if (!b) return CAV_E_ARG;
+    const int N = b->N;
+    if (N == 0) return CAV_OK;
+    const int reps = b->modep_per_rep ? b->n_rep : 1;
+    for (int r = 0; r < reps; ++r) {
+        double* q = b->h_modep.data() + (size_t)r * 7 * N;
+        for (int n = 0; n < N; ++n) {
+            if (g_b) {
+                const double Gm = Gamma_b ? Gamma_b[n] : 0.0, Ph = Phi_b ? Phi_b[n] : 0.0;
+                q[5 * N + n] = g_b[n] + Gm * std::cos(Ph); q[6 * N + n] = Gm * std::sin(Ph);
+            } else {
+                q[5 * N + n] = q[2 * N + n]; q[6 * N + n] = q[3 * N + n];
+            }
+        }
+    }
+    CKB(cudaMemcpyAsync(b->d_modep, b->h_modep.data(), sizeof(double) * b->h_modep.size(), cudaMemcpyHostToDevice, b->stream));
     CKB(cudaStreamSynchronize(b->stream));
     return CAV_OK;
 }

@@ -46,6 +46,7 @@ struct Ctrl {
     int N;
     double gamma, two_over_gamma;   // two_over_gamma = 2/gamma (host-computed: no fp64 division on the critical path)
     double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes];
+    double Gbre[kMaxModes], Gbim[kMaxModes];   // backward coupling G_b of the feedback field (= G unless cav_set_backaction)
     double a[kMaxModes][2];        // a_0: amplitudes of the current accepted state
     double as[2][kMaxModes][2];    // a_s: amplitudes of the state stage s is evaluated at, in as[s & 1] (double-buffered:
                                    // on the TMA path block 0 of kernel s+1 writes a_{s+1} while the other blocks still read a_s)

@@ -107,7 +107,7 @@ __device__ __forceinline__ void mode_stage_state(Ctrl* c, int n) {
     }
     const double are = c->a[n][0] + c->h * re, aim = c->a[n][1] + c->h * im;
     c->as[(ROW + 1) & 1][n][0] = are; c->as[(ROW + 1) & 1][n][1] = aim;      // the state of stage ROW+1
-    c->c[n] = c->two_over_gamma * (c->Gre[n] * are - c->Gim[n] * aim);
+    c->c[n] = c->two_over_gamma * (c->Gbre[n] * are - c->Gbim[n] * aim);
 }
 
 // Mode ODE at stage `stage` for mode n (Eq. 12 / Eq. 19): ka_s = -(i w + kappa) a_s + i G S_s with S_s from the

@@ -192,3 +192,18 @@ def test_driven_sweep_fixed_steps(api, prec):
     wr = copy.deepcopy(w); wr.B0 = tuple(B0[0])
     undriven = oracle_of(wr).run(wr.m0, wr.a0, fixed_dt=dt, max_steps=80)
     assert np.abs(a[0] - undriven.a).max() > 0.05 * np.abs(undriven.a).max()
+
+
+def test_nonreciprocal_sweep(api):
+    """cav_batch_set_backaction: every replica of a field sweep with g_b != g_f against the oracle."""
+    w = small_problem(8, 8, 2, 2, 1)
+    back = dict(g=0.25 * w.g, Gamma=2.0 * w.Gamma, Phi=w.Phi + 0.4)
+    B0 = np.array([[0.01, -0.02, W.b0_for_ghz(f)] for f in (9.5, 10.5)])
+    with api.Batch(w, 2, precision="f64", B0=B0) as b:
+        api.cav_batch_set_backaction(b.h, back["g"], back["Gamma"], back["Phi"])
+        b.run(math.inf, fixed_dt=0.1e-12, max_steps=80)
+        m, a = b.get_m(), b.get_a()
+    for r in range(2):
+        wr = copy.deepcopy(w); wr.B0 = tuple(B0[r])
+        ref = oracle_of(wr, backward=back).run(wr.m0, wr.a0, fixed_dt=0.1e-12, max_steps=80)
+        assert_parity(m[r], a[r], ref, "f64")

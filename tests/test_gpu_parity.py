@@ -516,3 +516,40 @@ def test_driven_adaptive_closed_form(api, path):
     lam = w.kappa + 1j * w.omega
     exact = amp * sig * math.sqrt(TWO_PI) * np.exp((lam - 1j * wd) ** 2 * sig ** 2 / 2) * np.exp(-lam * (T - t0))
     assert np.all(np.abs(a - exact) <= 3e-9 * np.abs(exact))
+
+
+# ----------------------------------------------------------------------------------------
+# non-reciprocal coupling (cav_set_backaction; G31)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_nonreciprocal_fixed_steps(api, prec, path):
+    w = small_problem(40, 9, 7, 3, 1)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    back = dict(g=0.25 * w.g, Gamma=2.0 * w.Gamma, Phi=w.Phi + 0.4)
+    ref = oracle_of(w, backward=back).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=80)
+    with open_sim(api, w, prec, path) as sim:
+        api.cav_set_backaction(sim.h, back["g"], back["Gamma"], back["Phi"])
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=80)
+        m, a = sim.get_m(), sim.get_a()
+    assert_parity(m, a, ref, prec)
+    recip = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=80)
+    assert np.abs(ref.m - recip.m).max() > 1e-5            # the backward coupling is not a detail here
+    # g_b = None restores reciprocal coupling
+    with open_sim(api, w, prec, path) as sim:
+        api.cav_set_backaction(sim.h, back["g"], back["Gamma"], back["Phi"])
+        api.cav_set_backaction(sim.h, None)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=80)
+        assert_parity(sim.get_m(), sim.get_a(), recip, prec)
+
+
+def test_nonreciprocal_rabi_period_geometric_mean(api):
+    """g_f/2pi = 100 MHz, g_b/2pi = 25 MHz: T_R = pi / sqrt(g_f g_b) = 10 ns within 0.5 % (the oracle's pin, on the GPU)."""
+    w = W.macrospin(5.0, [5.0], 100.0, 0.0, alpha=0.0, a0=[0.01], n=4)
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_set_backaction(sim.h, np.array([TWO_PI * 25e6]))
+        api.cav_set_trace(sim.h, 25e-12, 1040)
+        api.cav_run(sim.h, 26e-9, tol=1e-8)
+        tr = api.cav_get_trace(sim.h)
+    assert abs(rabi_period(tr[:, 0], tr[:, 1] ** 2 + tr[:, 2] ** 2) / 10e-9 - 1) < 5e-3
