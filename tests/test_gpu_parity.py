@@ -553,3 +553,25 @@ def test_nonreciprocal_rabi_period_geometric_mean(api):
         api.cav_run(sim.h, 26e-9, tol=1e-8)
         tr = api.cav_get_trace(sim.h)
     assert abs(rabi_period(tr[:, 0], tr[:, 1] ** 2 + tr[:, 2] ** 2) / 10e-9 - 1) < 5e-3
+
+
+# ----------------------------------------------------------------------------------------
+# TMA path with several plane-tiles per block (marching in z, tile-column changes inside a run, serpentine sweep)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n_sub,N", [(1, 3), (2, 1)])
+@pytest.mark.parametrize("serpentine", [1, 0])
+def test_tma_multi_plane_runs(api, prec, n_sub, N, serpentine):
+    """128 x 64 x 20 cells: 320 (fp32) / 640 (fp64) plane-tiles over 148 persistent blocks, so every block marches over
+    2-5 planes, most runs cross a tile-column boundary (nz = 20 does not divide the run length) and odd stages walk
+    backwards.  Element by element against the oracle, with both sweep orders."""
+    w = small_problem(128, 64, 20, N, n_sub)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=6)
+    with open_sim(api, w, prec, "tma") as sim:
+        api.cav_set_sweep_order(sim.h, serpentine)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=6)
+        m, a = sim.get_m(), sim.get_a()
+    assert_parity(m, a, ref, prec)
