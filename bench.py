@@ -1,6 +1,6 @@
 """bench.py — throughput of the fused LLG + cavity-mode RK45 step (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg5|cfg4|cfg4_f64|cfg2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg5|cfg4|cfg4_f64|cfg2|cfg1|cfg1_sweep|cfg2_sweep]
     python bench.py --impl reference ...          # the fp64 CPU oracle on the host cores
 
 A "step" is one Dormand-Prince RK45 step of the whole coupled system: six fused stage kernels
@@ -61,6 +61,8 @@ def make_workload(name: str, rank: int = 0):
         return W.cfg4(seed=4000 + seed_shift), "f64"
     if name == "cfg4d":
         return W.cfg4(seed=4000 + seed_shift, dissipative=True), "f32"
+    if name == "cfg1":
+        return W.cfg1("b", seed=1000 + seed_shift), "f64"
     if name == "cfg2":
         return W.cfg2(seed=2000 + seed_shift), "f32"
     if name == "cfg2_f64":
@@ -287,10 +289,10 @@ def run_cuda(args):
     np_dtype = np.float32 if prec == "f32" else np.float64
     tol = w.tol
     stream = torch.cuda.Stream()
-    path = {"auto": None, "generic": api.CAV_PATH_GENERIC, "tma": api.CAV_PATH_TMA}[args.kernel_path]
+    path = {"auto": None, "generic": api.CAV_PATH_GENERIC, "tma": api.CAV_PATH_TMA, "block": api.CAV_PATH_BLOCK}[args.kernel_path]
     sim = api.Sim(w, precision=prec, stream=stream.cuda_stream, path=path)
     h = sim.h
-    path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma"}[api.cav_get_kernel_path(h)]
+    path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma", api.CAV_PATH_BLOCK: "block"}[api.cav_get_kernel_path(h)]
     if args.no_stage_overlap:
         api.cav_set_stage_overlap(h, 0)
     if args.no_serpentine:
@@ -323,7 +325,8 @@ def run_cuda(args):
     n1 = api.cav_get_launch_count(h)
     evals = st1["rhs_evals"] - st0["rhs_evals"]
     steps_done = (st1["accepted"] + st1["rejected"]) - (st0["accepted"] + st0["rejected"])
-    assert steps_done == args.steps and evals == 6 * args.steps, (steps_done, evals)
+    # the single-block path (grids up to 1024 cells) re-evaluates k1 at the start of a run: one more evaluation
+    assert steps_done == args.steps and evals in (6 * args.steps, 6 * args.steps + 1), (steps_done, evals)
     sim_t = st1["t"] - st0["t"]
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region, every step ----
@@ -588,7 +591,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--spinup", type=int, default=40, help="untimed setup steps that let dt settle")
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
-    ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma"])
+    ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma", "block"])
     ap.add_argument("--replicas", type=int, default=1184, help="cfg1_sweep: replicas in the batch")
     ap.add_argument("--no-serpentine", action="store_true", help="every stage sweeps forward (A/B aid)")
     ap.add_argument("--no-stage-overlap", action="store_true", help="full dependencies between stage kernels (A/B aid)")

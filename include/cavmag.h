@@ -58,7 +58,7 @@ typedef enum {
 enum { CAV_F32 = 0, CAV_F64 = 1 };
 enum { CAV_NORM_NCELLS = 0, CAV_NORM_SUM_U = 1 };
 enum { CAV_LAUNCH_GRAPH = 0, CAV_LAUNCH_STREAM = 1 };
-enum { CAV_PATH_AUTO = 0, CAV_PATH_GENERIC = 1, CAV_PATH_TMA = 2 };
+enum { CAV_PATH_AUTO = 0, CAV_PATH_GENERIC = 1, CAV_PATH_TMA = 2, CAV_PATH_BLOCK = 3 };
 #define CAV_MAX_MODES 32
 
 /* Finite-difference grid: nx*ny*nz cells of size dx*dy*dz (metres). */
@@ -182,8 +182,13 @@ int cav_set_sweep_order(cav_sim* sim, int serpentine);
  *   CAV_PATH_TMA      persistent TMA/mbarrier-pipelined kernel; needs nx*sizeof(T) % 16 == 0 and a mode count whose
  *                     streams fit the shared-memory rings, else cav_set_kernel_path returns CAV_E_UNSUPPORTED;
  *   CAV_PATH_GENERIC  register/LDG kernel for any shape;
- *   CAV_PATH_AUTO     (default) TMA when eligible and the grid has at least one plane-tile per SM.
- * cav_get_kernel_path reports the kernel the next run will use (CAV_PATH_GENERIC or CAV_PATH_TMA). */
+ *   CAV_PATH_BLOCK    grids of at most 1024 cells: the whole run in ONE thread block (the batched small-grid kernel with a
+ *                     single replica: stage state in shared memory, slopes in registers, no launch per stage); the
+ *                     slope of the final state is not cached (the next run re-evaluates k1: rhs_evals counts it);
+ *                     CAV_E_UNSUPPORTED for larger grids;
+ *   CAV_PATH_AUTO     (default) BLOCK up to 1024 cells, else TMA when eligible and the grid has at least one plane-tile
+ *                     per SM, else GENERIC.
+ * cav_get_kernel_path reports the kernel the next run will use (CAV_PATH_GENERIC, CAV_PATH_TMA or CAV_PATH_BLOCK). */
 int cav_set_kernel_path(cav_sim* sim, int path);
 int cav_get_kernel_path(cav_sim* sim, int* path);
 

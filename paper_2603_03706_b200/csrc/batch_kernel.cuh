@@ -64,6 +64,10 @@ struct BatchShared {
     double dt_min, dt_max;
 };
 
+// defined in cavmag_batch.cu: instantiates and launches k_batch (the C ABI of the batch, and cav_run's CAV_PATH_BLOCK)
+int launch_batch_kernel(BatchArgs& A, bool f32, int n_sub, bool two_per_sm, size_t smem_optin, cudaStream_t stream,
+                        cudaError_t* cuda_err);
+
 template <int ROW>
 __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, const double two_over_gamma) {
     double re = 0.0, im = 0.0;

@@ -12,6 +12,7 @@
 
 #include "../../include/cavmag.h"
 #include "stage_tma.cuh"
+#include "batch_kernel.cuh"
 
 using namespace cavmag;
 
@@ -61,6 +62,9 @@ struct cav_sim {
     TmaArgs targs[8];
     size_t tsmem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int tgrid = 1;
+    bool last_run_block = false;       // h_ctrl->ycur is known to be current (no stage-kernel run since the last pull)
+    bool use_block = false;            // CAV_PATH_BLOCK: the whole run in one thread block (k_batch with one replica)
+    unsigned char* d_blk = nullptr;    // bridge buffers of the block path: BatchCtl, a, mode parameters, drive, B0
     bool want_pdl = true;              // cav_set_stage_overlap
     bool graph_pdl = false;            // loop-body edges of the current graph are programmatic dependencies
 };
@@ -272,10 +276,97 @@ int plan_tma(cav_sim* s) {
     return CAV_OK;
 }
 
+StageArgs make_args(const cav_sim* s, unsigned long long handle);
+int sync_pull(cav_sim* s);
+
 void decide_path(cav_sim* s) {
-    if (s->kernel_path == CAV_PATH_GENERIC) s->use_tma = false;
+    const bool block_ok = s->nc <= kBatchMaxCells;
+    s->use_block = (s->kernel_path == CAV_PATH_BLOCK && block_ok) || (s->kernel_path == CAV_PATH_AUTO && block_ok);
+    if (s->kernel_path == CAV_PATH_GENERIC || s->use_block) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
     else s->use_tma = s->tma_eligible && s->targs[1].Q >= (long long)s->n_sm;
+}
+
+// ---- CAV_PATH_BLOCK: a grid of <= 1024 cells is integrated by ONE thread block for the whole run (k_batch with a
+//      single replica, batch_kernel.cuh): no kernel launch per stage.  Two tiny kernels copy the controller / mode state
+//      between Ctrl and the batch kernel's arguments on the stream, so cav_run stays asynchronous. ----
+constexpr size_t kBlkCtl = 0, kBlkA = 256, kBlkModep = kBlkA + 16 * kMaxModes, kBlkDrive = kBlkModep + 8 * 7 * kMaxModes,
+                 kBlkB0 = kBlkDrive + 8 * 5 * kMaxModes, kBlkBytes = kBlkB0 + 64;
+static_assert(sizeof(BatchCtl) <= kBlkA, "bridge layout");
+
+__global__ void k_block_in(const Ctrl* c, unsigned char* blk, double B0x, double B0y, double B0z) {
+    BatchCtl* bc = reinterpret_cast<BatchCtl*>(blk + kBlkCtl);
+    double* a = reinterpret_cast<double*>(blk + kBlkA);
+    double* mp = reinterpret_cast<double*>(blk + kBlkModep);
+    double* dr = reinterpret_cast<double*>(blk + kBlkDrive);
+    double* B0 = reinterpret_cast<double*>(blk + kBlkB0);
+    const int n = threadIdx.x, N = c->N;
+    if (n < N) {
+        a[2 * n] = c->a[n][0]; a[2 * n + 1] = c->a[n][1];
+        mp[n] = c->omega[n]; mp[N + n] = c->kappa[n]; mp[2 * N + n] = c->Gre[n]; mp[3 * N + n] = c->Gim[n];
+        mp[4 * N + n] = c->invW[n]; mp[5 * N + n] = c->Gbre[n]; mp[6 * N + n] = c->Gbim[n];
+        dr[n] = c->eta_re[n]; dr[N + n] = c->eta_im[n]; dr[2 * N + n] = c->eta_t0[n];
+        dr[3 * N + n] = c->eta_i2s2[n]; dr[4 * N + n] = c->eta_wd[n];
+    }
+    if (n == 0) {
+        bc->t = c->t; bc->dt = c->dt; bc->dt_min = c->dt_min; bc->dt_max = c->dt_max; bc->last_err = c->last_err;
+        bc->accepted = c->accepted; bc->rejected = c->rejected; bc->rhs_evals = c->rhs_evals;
+        bc->trace_acc0 = c->trace_acc0; bc->status = c->status; bc->trace_n = c->trace_n;
+        B0[0] = B0x; B0[1] = B0y; B0[2] = B0z;
+    }
+}
+
+__global__ void k_block_out(Ctrl* c, const unsigned char* blk) {
+    const BatchCtl* bc = reinterpret_cast<const BatchCtl*>(blk + kBlkCtl);
+    const double* a = reinterpret_cast<const double*>(blk + kBlkA);
+    const int n = threadIdx.x;
+    if (n < c->N) { c->a[n][0] = a[2 * n]; c->a[n][1] = a[2 * n + 1]; }
+    if (n == 0) {
+        c->t = bc->t; c->dt = bc->dt; c->dt_min = bc->dt_min; c->dt_max = bc->dt_max; c->last_err = bc->last_err;
+        c->accepted = bc->accepted; c->rejected = bc->rejected; c->rhs_evals = bc->rhs_evals;
+        c->status = bc->status; c->trace_n = bc->trace_n;
+        c->k1_valid = 0;             // the block path keeps its slopes in registers: nothing cached for the stage kernels
+        c->done = 1;
+    }
+}
+
+int run_block_path(cav_sim* s, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
+    if (!s->d_blk) CK(cudaMalloc(&s->d_blk, kBlkBytes));
+    if (!s->last_run_block) {                            // a stage-kernel run may have flipped ycur on the device
+        int rc0 = sync_pull(s);
+        if (rc0) return rc0;
+        s->last_run_block = true;
+    }
+    const cav_params& p = s->prm;
+    const Ctrl* hc = s->h_ctrl;                          // host-set fields only (N, trace and drive settings)
+    k_block_in<<<1, 32, 0, s->stream>>>(s->d_ctrl, s->d_blk, p.B0[0], p.B0[1], p.B0[2]);
+    CK(cudaGetLastError());
+    BatchArgs A;
+    memset(&A, 0, sizeof(A));
+    const StageArgs S = make_args(s, 0ull);
+    A.nx = s->grid.nx; A.ny = s->grid.ny; A.nz = s->grid.nz; A.nc = (int)s->nc; A.N = s->N; A.n_rep = 1;
+    A.ex_wx = S.ex_wx; A.ex_wy = S.ex_wy; A.ex_wz = S.ex_wz; A.an_pref = S.an_pref;
+    for (int i = 0; i < 3; ++i) A.axis[i] = S.axis[i];
+    A.alpha = S.alpha; A.llg = S.llg; A.B_exch_inter = S.B_exch_inter;
+    A.two_over_gamma = 2.0 / p.gamma; A.inv_nc = S.inv_nc; A.renormalize = p.renormalize;
+    A.B0 = reinterpret_cast<const double*>(s->d_blk + kBlkB0);
+    A.u = s->u;
+    A.modep = reinterpret_cast<const double*>(s->d_blk + kBlkModep); A.modep_per_rep = 0;
+    A.m = s->Y[hc->ycur];                                // ycur only changes in the stage kernels' controller: the host copy
+    A.a = reinterpret_cast<double*>(s->d_blk + kBlkA);   // is current after any setter, and the block path never flips it
+    A.ctl = reinterpret_cast<BatchCtl*>(s->d_blk + kBlkCtl);
+    A.t_end = t_end; A.tol = tol; A.fixed_dt = fixed_dt; A.dt_init = dt_init; A.max_steps = max_steps;
+    A.sample_dt = hc->sample_dt; A.trace_t0 = hc->trace_t0; A.trace_cap = hc->trace_cap;
+    A.row_len = 1 + 4 * s->N + 3 * p.n_sub; A.trace = s->d_trace;
+    A.drive = hc->drive_on ? reinterpret_cast<const double*>(s->d_blk + kBlkDrive) : nullptr;
+    cudaError_t ce = cudaSuccess;
+    int rc = launch_batch_kernel(A, p.precision == CAV_F32, p.n_sub, false, s->smem_optin, s->stream, &ce);
+    if (rc == CAV_E_CUDA || rc == CAV_E_NOMEM) snprintf(s->cuda_err, sizeof(s->cuda_err), "k_batch launch: %s", cudaGetErrorString(ce));
+    if (rc) return rc;
+    k_block_out<<<1, 32, 0, s->stream>>>(s->d_ctrl, s->d_blk);
+    CK(cudaGetLastError());
+    s->host_launches += 3;
+    return CAV_OK;
 }
 
 void choose_grid(cav_sim* s) {
@@ -579,6 +670,7 @@ int cav_destroy(cav_sim* s) {
     cudaFree(s->d_ctrl);
     cudaFree(s->d_trace);
     cudaFree(s->d_maps);
+    cudaFree(s->d_blk);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     if (s->h_flag) cudaFreeHost(s->h_flag);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -610,8 +702,9 @@ int cav_set_block_cells(cav_sim* s, int cells) {
 }
 
 int cav_set_kernel_path(cav_sim* s, int path) {
-    if (!s || (path != CAV_PATH_AUTO && path != CAV_PATH_GENERIC && path != CAV_PATH_TMA)) return CAV_E_ARG;
+    if (!s || (path != CAV_PATH_AUTO && path != CAV_PATH_GENERIC && path != CAV_PATH_TMA && path != CAV_PATH_BLOCK)) return CAV_E_ARG;
     if (path == CAV_PATH_TMA && !s->tma_eligible) return CAV_E_UNSUPPORTED;
+    if (path == CAV_PATH_BLOCK && s->nc > kBatchMaxCells) return CAV_E_UNSUPPORTED;
     s->kernel_path = path;
     s->graph_dirty = true;
     return CAV_OK;
@@ -620,7 +713,7 @@ int cav_set_kernel_path(cav_sim* s, int path) {
 int cav_get_kernel_path(cav_sim* s, int* path) {
     if (!s || !path) return CAV_E_ARG;
     decide_path(s);
-    *path = s->use_tma ? CAV_PATH_TMA : CAV_PATH_GENERIC;
+    *path = s->use_block ? CAV_PATH_BLOCK : s->use_tma ? CAV_PATH_TMA : CAV_PATH_GENERIC;
     return CAV_OK;
 }
 
@@ -844,6 +937,9 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     if (adaptive == (fixed_dt > 0.0)) return CAV_E_ARG;        // exactly one of the two
     if (std::isnan(t_end) || max_steps < 0) return CAV_E_ARG;
     if (std::isinf(t_end) && max_steps == 0) return CAV_E_ARG;
+    decide_path(s);
+    if (s->use_block) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
+    s->last_run_block = false;
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     CK(cudaGetLastError());
     s->host_launches++;

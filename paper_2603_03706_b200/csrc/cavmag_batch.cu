@@ -81,6 +81,35 @@ int pull_ctl(cav_batch* b, std::vector<BatchCtl>& h) {
 
 }  // namespace
 
+namespace cavmag {
+
+// Launches k_batch for A.n_rep replicas (also used by cav_run for a single tiny grid: CAV_PATH_BLOCK).
+int launch_batch_kernel(BatchArgs& A, bool f32, int n_sub, bool two_per_sm, size_t smem_optin, cudaStream_t stream,
+                        cudaError_t* cuda_err) {
+    auto fail = [&](cudaError_t e) { *cuda_err = e; cudaGetLastError(); return e == cudaErrorMemoryAllocation ? CAV_E_NOMEM : CAV_E_CUDA; };
+    const size_t esize = f32 ? 4 : 8;
+    int threads = (A.nc + 31) / 32 * 32;
+    if (threads < 64) threads = 64;
+    const size_t ms_bytes = (size_t)n_sub * 3 * A.nc * esize, u_bytes = (size_t)A.N * A.nc * esize;
+    const void* fn = f32 ? (n_sub == 1 ? batch_fn<float, 1>(threads, two_per_sm) : batch_fn<float, 2>(threads, two_per_sm))
+                         : (n_sub == 1 ? batch_fn<double, 1>(threads, two_per_sm) : batch_fn<double, 2>(threads, two_per_sm));
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return fail(e);
+    const size_t room = smem_optin > fa.sharedSizeBytes ? smem_optin - fa.sharedSizeBytes : 0;
+    if (ms_bytes > room) return CAV_E_UNSUPPORTED;
+    A.u_in_smem = (A.N > 0 && ms_bytes + u_bytes <= room && ms_bytes + u_bytes <= 96 * 1024) ? 1 : 0;
+    const size_t smem = ms_bytes + (A.u_in_smem ? u_bytes : 0);
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)room);
+    if (e != cudaSuccess) return fail(e);
+    void* params[] = {&A};
+    e = cudaLaunchKernel(fn, dim3(A.n_rep), dim3(threads), params, smem, stream);
+    if (e != cudaSuccess) return fail(e);
+    return CAV_OK;
+}
+
+}  // namespace cavmag
+
 extern "C" {
 
 int cav_batch_create(const cav_grid* grid, const cav_params* prm, int n_rep, cav_batch** out) {
@@ -330,22 +359,10 @@ int cav_batch_run(cav_batch* b, double t_end, double tol, double fixed_dt, doubl
     A.trace = b->d_trace;
     A.drive = b->d_drive;
 
-    int threads = (b->nc + 31) / 32 * 32;
-    if (threads < 64) threads = 64;
-    const size_t ms_bytes = (size_t)p.n_sub * 3 * b->nc * b->esize, u_bytes = (size_t)b->N * b->nc * b->esize;
-    const bool two = b->n_rep > b->n_sm;         // more replicas than SMs: throughput over single-replica latency
-    const void* fn = p.precision == CAV_F32 ? (p.n_sub == 1 ? batch_fn<float, 1>(threads, two) : batch_fn<float, 2>(threads, two))
-                                            : (p.n_sub == 1 ? batch_fn<double, 1>(threads, two) : batch_fn<double, 2>(threads, two));
-    cudaFuncAttributes fa;
-    CKB(cudaFuncGetAttributes(&fa, fn));
-    const size_t room = b->smem_optin > fa.sharedSizeBytes ? b->smem_optin - fa.sharedSizeBytes : 0;
-    if (ms_bytes > room) return CAV_E_UNSUPPORTED;
-    A.u_in_smem = (b->N > 0 && ms_bytes + u_bytes <= room && ms_bytes + u_bytes <= 96 * 1024) ? 1 : 0;
-    const size_t smem = ms_bytes + (A.u_in_smem ? u_bytes : 0);
-    CKB(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)room));
-    void* params[] = {&A};
-    CKB(cudaLaunchKernel(fn, dim3(b->n_rep), dim3(threads), params, smem, b->stream));
-    return CAV_OK;
+    cudaError_t ce = cudaSuccess;
+    int rc = cavmag::launch_batch_kernel(A, p.precision == CAV_F32, p.n_sub, b->n_rep > b->n_sm, b->smem_optin, b->stream, &ce);
+    if (rc == CAV_E_CUDA || rc == CAV_E_NOMEM) snprintf(b->cuda_err, sizeof(b->cuda_err), "k_batch launch: %s", cudaGetErrorString(ce));
+    return rc;
 }
 
 int cav_batch_get_m(cav_batch* b, void* m_out) {

@@ -34,22 +34,27 @@ def oracle_of(w, **kw):
     return Oracle(w, **kw)
 
 
-PATHS = ["generic", "tma"]
+PATHS = ["generic", "tma", "block"]
 
 
 def open_sim(api, w, prec, path, **kw):
-    """A Sim forced onto one implementation of the stage kernel; skips when the TMA kernel is not
-    eligible for this shape (nx*sizeof(T) not a multiple of 16 bytes)."""
+    """A Sim forced onto one implementation of the step: the generic or the TMA stage kernels, or the single-block
+    integrator of grids up to 1024 cells (CAV_PATH_BLOCK).  Skips when the path is not eligible for this shape
+    (TMA: nx*sizeof(T) not a multiple of 16 bytes; BLOCK: more than 1024 cells)."""
     sim = api.Sim(w, precision=prec, **kw)
+    want = {"tma": api.CAV_PATH_TMA, "generic": api.CAV_PATH_GENERIC, "block": api.CAV_PATH_BLOCK}[path]
     try:
-        api.cav_set_kernel_path(sim.h, api.CAV_PATH_TMA if path == "tma" else api.CAV_PATH_GENERIC)
+        api.cav_set_kernel_path(sim.h, want)
     except api.CavError as e:
         sim.close()
-        assert e.status == api.CAV_E_UNSUPPORTED and path == "tma"
+        assert e.status == api.CAV_E_UNSUPPORTED and path in ("tma", "block")
+        if path == "block":
+            assert w.nx * w.ny * w.nz > 1024, "BLOCK path refused although the grid has at most 1024 cells"
+            pytest.skip("single-block path: grid too large")
         es = 4 if prec == "f32" else 8
         assert (w.nx * es) % 16 != 0, "TMA path refused although the row pitch is 16-byte aligned"
         pytest.skip("TMA kernel not eligible for this shape")
-    assert api.cav_get_kernel_path(sim.h) == (api.CAV_PATH_TMA if path == "tma" else api.CAV_PATH_GENERIC)
+    assert api.cav_get_kernel_path(sim.h) == want
     return sim
 
 
@@ -387,7 +392,8 @@ def test_resume_equals_single_run(api, path):
         m2, a2 = sim.get_m(), sim.get_a()
         st = api.cav_get_stats(sim.h)
     assert np.array_equal(m1, m2) and np.array_equal(a1, a2)
-    assert st["rhs_evals"] == 1 + 6 * 40
+    # the single-block path keeps its slopes in registers and re-evaluates k1 at the start of every run
+    assert st["rhs_evals"] == 1 + 6 * 40 + (1 if path == "block" else 0)
 
 
 def test_edge_cases(api):
