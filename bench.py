@@ -289,10 +289,10 @@ def run_cuda(args):
     np_dtype = np.float32 if prec == "f32" else np.float64
     tol = w.tol
     stream = torch.cuda.Stream()
-    path = {"auto": None, "generic": api.CAV_PATH_GENERIC, "tma": api.CAV_PATH_TMA, "block": api.CAV_PATH_BLOCK}[args.kernel_path]
+    path = {"auto": None, "generic": api.CAV_PATH_GENERIC, "tma": api.CAV_PATH_TMA, "block": api.CAV_PATH_BLOCK, "coop": api.CAV_PATH_COOP}[args.kernel_path]
     sim = api.Sim(w, precision=prec, stream=stream.cuda_stream, path=path)
     h = sim.h
-    path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma", api.CAV_PATH_BLOCK: "block"}[api.cav_get_kernel_path(h)]
+    path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma", api.CAV_PATH_BLOCK: "block", api.CAV_PATH_COOP: "coop"}[api.cav_get_kernel_path(h)]
     if args.no_stage_overlap:
         api.cav_set_stage_overlap(h, 0)
     if args.no_serpentine:
@@ -502,7 +502,8 @@ def run_concurrent_sweep(args):
     ghz = W.cfg2_sweep_ghz()
     ws = [W.cfg2(f_kittel_ghz=float(f), seed=2000 + i) for i, f in enumerate(ghz)]
     streams = [torch.cuda.Stream() for _ in ws]
-    sims = [api.Sim(w, precision="f32", stream=st.cuda_stream) for w, st in zip(ws, streams)]
+    # the generic stage kernels: graphs of different simulations overlap (cooperative grids would serialise)
+    sims = [api.Sim(w, precision="f32", stream=st.cuda_stream, path=api.CAV_PATH_GENERIC) for w, st in zip(ws, streams)]
     tol, nc, N = ws[0].tol, ws[0].n_cells, ws[0].n_modes
     master = torch.cuda.Stream()
 
@@ -591,7 +592,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--spinup", type=int, default=40, help="untimed setup steps that let dt settle")
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
-    ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma", "block"])
+    ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma", "block", "coop"])
     ap.add_argument("--replicas", type=int, default=1184, help="cfg1_sweep: replicas in the batch")
     ap.add_argument("--no-serpentine", action="store_true", help="every stage sweeps forward (A/B aid)")
     ap.add_argument("--no-stage-overlap", action="store_true", help="full dependencies between stage kernels (A/B aid)")

@@ -58,7 +58,7 @@ typedef enum {
 enum { CAV_F32 = 0, CAV_F64 = 1 };
 enum { CAV_NORM_NCELLS = 0, CAV_NORM_SUM_U = 1 };
 enum { CAV_LAUNCH_GRAPH = 0, CAV_LAUNCH_STREAM = 1 };
-enum { CAV_PATH_AUTO = 0, CAV_PATH_GENERIC = 1, CAV_PATH_TMA = 2, CAV_PATH_BLOCK = 3 };
+enum { CAV_PATH_AUTO = 0, CAV_PATH_GENERIC = 1, CAV_PATH_TMA = 2, CAV_PATH_BLOCK = 3, CAV_PATH_COOP = 4 };
 #define CAV_MAX_MODES 32
 
 /* Finite-difference grid: nx*ny*nz cells of size dx*dy*dz (metres). */
@@ -186,9 +186,14 @@ int cav_set_sweep_order(cav_sim* sim, int serpentine);
  *                     single replica: stage state in shared memory, slopes in registers, no launch per stage); the
  *                     slope of the final state is not cached (the next run re-evaluates k1: rhs_evals counts it);
  *                     CAV_E_UNSUPPORTED for larger grids;
- *   CAV_PATH_AUTO     (default) BLOCK up to 1024 cells, else TMA when eligible and the grid has at least one plane-tile
- *                     per SM, else GENERIC.
- * cav_get_kernel_path reports the kernel the next run will use (CAV_PATH_GENERIC, CAV_PATH_TMA or CAV_PATH_BLOCK). */
+ *   CAV_PATH_COOP     grids of 1025 .. 512 x (number of SMs) cells: the whole run in ONE cooperative launch of
+ *                     ceil(cells/512) co-resident blocks, a grid barrier per evaluation instead of a kernel boundary (the
+ *                     same kernel as BLOCK, stage state and block partials through global memory); like BLOCK it does not
+ *                     cache the final slope.  Cooperative grids do not overlap with each other: for many concurrent
+ *                     simulations on several streams (a sweep) choose GENERIC.  CAV_E_UNSUPPORTED outside that range;
+ *   CAV_PATH_AUTO     (default) BLOCK up to 1024 cells; TMA when eligible and the grid has at least one plane-tile per
+ *                     SM; COOP for the sizes in between; else GENERIC.
+ * cav_get_kernel_path reports what the next run will use (CAV_PATH_GENERIC, _TMA, _BLOCK or _COOP). */
 int cav_set_kernel_path(cav_sim* sim, int path);
 int cav_get_kernel_path(cav_sim* sim, int* path);
 

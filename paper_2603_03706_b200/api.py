@@ -23,7 +23,7 @@ CAV_E_NONFINITE, CAV_E_DT_UNDERFLOW, CAV_E_SINGULAR_NORM, CAV_E_UNSUPPORTED = -5
 CAV_F32, CAV_F64 = 0, 1
 CAV_NORM_NCELLS, CAV_NORM_SUM_U = 0, 1
 CAV_LAUNCH_GRAPH, CAV_LAUNCH_STREAM = 0, 1
-CAV_PATH_AUTO, CAV_PATH_GENERIC, CAV_PATH_TMA, CAV_PATH_BLOCK = 0, 1, 2, 3
+CAV_PATH_AUTO, CAV_PATH_GENERIC, CAV_PATH_TMA, CAV_PATH_BLOCK, CAV_PATH_COOP = 0, 1, 2, 3, 4
 CAV_MAX_MODES = 32
 
 

@@ -46,6 +46,12 @@ struct BatchArgs {
     double* trace;                // [n_rep][trace_cap][row_len]
     int u_in_smem;                // profiles staged in dynamic shared memory
     const double* drive;          // [5][N]: eta_re, eta_im, t0, 1/(2 sigma^2), omega_d (common to all replicas) or NULL
+    // cooperative variant (COOP: one simulation spread over nblk co-resident blocks, grid barriers between the phases)
+    void* gms[2];                 // [NSUB][3][nc] T: stage state in global memory, double-buffered by evaluation parity
+    double* cpart[2];             // [2N + 3 NSUB][nblk] block partial sums, double-buffered
+    double* cmax[2];              // [nblk] block maxima of |e|^2, double-buffered by step parity
+    unsigned long long* bar;      // grid-barrier counter (zeroed before the launch)
+    int nblk;
 };
 
 // Shared mode / controller state of one replica.
@@ -57,6 +63,7 @@ struct BatchShared {
     double part[32][2 * kMaxModes + 6];     // per-warp partial sums: overlaps (2N) then <m_s> (3 n_sub)
     double wmax[32];
     double red[2 * kMaxModes + 6];
+    double red2[2 * kMaxModes + 6];         // COOP: sums over all blocks
     double t, dt, h, target, err;
     long long steps;
     int clamped, sample_hit, accept, done, status, trace_n;
@@ -67,6 +74,7 @@ struct BatchShared {
 // defined in cavmag_batch.cu: instantiates and launches k_batch (the C ABI of the batch, and cav_run's CAV_PATH_BLOCK)
 int launch_batch_kernel(BatchArgs& A, bool f32, int n_sub, bool two_per_sm, size_t smem_optin, cudaStream_t stream,
                         cudaError_t* cuda_err);
+int launch_coop_kernel(BatchArgs& A, bool f32, int n_sub, cudaStream_t stream, cudaError_t* cuda_err);
 
 template <int ROW>
 __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, const double two_over_gamma) {
@@ -83,17 +91,37 @@ __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, 
 // 512-thread ferromagnet bucket, chosen by the host when there are more replicas than SMs) asks for two blocks per SM: 64
 // registers and < 100 B of spills make one replica ~10 % slower, but the barrier stalls of one replica hide behind the
 // other (+31 % with 1184 replicas of CFG1).
-template <typename T, int NSUB, int MAXT, int MINB>
+// COOP = true: ONE simulation of up to gridDim.x * blockDim.x cells spread over co-resident blocks (cooperative launch): the
+// stage state goes through a double-buffered global array (neighbours are L2 reads), block partial sums and block error
+// maxima through global memory, and one grid barrier per evaluation (+ one per step for the error norm) replaces the kernel
+// boundary; every block replays the mode algebra and the controller (identical bits), block 0 writes trace and state.
+template <typename T, int NSUB, int MAXT, int MINB, bool COOP = false>
 __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
     extern __shared__ __align__(16) unsigned char batch_dsm[];
     __shared__ BatchShared sh;
     const int nc = A.nc, N = A.N;
     T* const sm_m = reinterpret_cast<T*>(batch_dsm);                 // [NSUB*3][nc] stage state
     T* const sm_u = sm_m + (size_t)NSUB * 3 * nc;                     // [N][nc] profiles (if u_in_smem)
-    const int rep = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
-    const bool active = tid < nc;
-    const int cell = active ? tid : nc - 1;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+    const int rep = COOP ? 0 : (int)blockIdx.x;
+    const int gcell = COOP ? (int)(blockIdx.x * blockDim.x) + tid : tid;
+    const bool active = gcell < nc;
+    const int cell = active ? gcell : nc - 1;
+    const bool writer = !COOP || blockIdx.x == 0;                    // trace rows, amplitudes and controller state
     const int x = cell % A.nx, yy = (cell / A.nx) % A.ny, z = cell / (A.nx * A.ny);
+    unsigned long long epoch = 0;                                    // grid barriers passed (COOP)
+    int ev = 0;                                                      // evaluations done (COOP: buffer parity)
+    auto grid_barrier = [&]() {
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            atomicAdd(A.bar, 1ull);
+            const unsigned long long target = (++epoch) * (unsigned long long)A.nblk;
+            unsigned long long seen;
+            do { asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(A.bar) : "memory"); } while (seen < target);
+        }
+        __syncthreads();
+    };
 
     // open boundary (G9): an out-of-grid neighbour gets weight 0 and the centre's index
     const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
@@ -116,7 +144,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
     for (int s = 0; s < NSUB; ++s)
 #pragma unroll
         for (int c = 0; c < 3; ++c) y[s][c] = mg[(size_t)(s * 3 + c) * nc + cell];
-    if (A.u_in_smem)
+    if (!COOP && A.u_in_smem)
         for (int i = tid; i < N * nc; i += blockDim.x) sm_u[i] = ug[i];
     if (tid < N) {
         const double* mp = A.modep + (A.modep_per_rep ? (size_t)rep * 7 * N : 0);
@@ -146,19 +174,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         }
     }
     __syncthreads();
-    const T* __restrict__ up = A.u_in_smem ? sm_u : ug;
+    const T* __restrict__ up = (!COOP && A.u_in_smem) ? sm_u : ug;
 
     // ---- one evaluation of the coupled right-hand side at stage s (1..7): slope k of the own cell, and in
     //      thread n the mode slope ka_s and the amplitudes / RF weights of the next stage state ----
     auto eval = [&](auto stage_tag, const T (&ms)[NSUB][3], T (&k)[NSUB][3]) {
         constexpr int s = decltype(stage_tag)::value;
+        constexpr int nsum_extra = (s == 7) ? 3 * NSUB : 0;
+        T* const fld = COOP ? reinterpret_cast<T*>(A.gms[ev & 1]) : sm_m;      // where neighbours read the stage state
         if (active) {
 #pragma unroll
             for (int q = 0; q < NSUB; ++q)
 #pragma unroll
-                for (int c = 0; c < 3; ++c) sm_m[(size_t)(q * 3 + c) * nc + cell] = ms[q][c];
+                for (int c = 0; c < 3; ++c) fld[(size_t)(q * 3 + c) * nc + cell] = ms[q][c];
         }
-        __syncthreads();                                             // [A] stage state and c_n published
+        __syncthreads();                                             // [A] c_n of this stage (and, !COOP, the stage state) published
         T mcx, mcy;
         if constexpr (NSUB == 1) { mcx = ms[0][0]; mcy = ms[0][1]; }
         else { mcx = (T)0.5 * (ms[0][0] + ms[1][0]); mcy = (T)0.5 * (ms[0][1] + ms[1][1]); }
@@ -183,19 +213,32 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                 if (lane == 0) sh.part[warp][2 * N + i] = v;
             }
         }
+        if constexpr (COOP) {
+            __syncthreads();
+            if (tid < 2 * N + nsum_extra) {                          // fixed-order block sum -> this block's slot
+                double v = 0.0;
+                for (int w = 0; w < nwarp; ++w) v += sh.part[w][tid];
+                A.cpart[ev & 1][(size_t)tid * A.nblk + blockIdx.x] = v;
+            }
+            grid_barrier();                                          // stage state, partials and c_n of all blocks published
+        }
+        auto rd = [&](const T* f, int i) -> T {
+            if constexpr (COOP) return __ldcg(f + i);                // written by other SMs: read at L2
+            else return f[i];
+        };
 #pragma unroll
         for (int q = 0; q < NSUB; ++q) {
             T lap[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const T* f = sm_m + (size_t)(q * 3 + c) * nc;
+                const T* f = fld + (size_t)(q * 3 + c) * nc;
                 const T m0 = ms[q][c];
-                T l = (f[ixm] - m0) * wxm;
-                l += (f[ixp] - m0) * wxp;
-                l += (f[iym] - m0) * wym;
-                l += (f[iyp] - m0) * wyp;
-                l += (f[izm] - m0) * wzm;
-                l += (f[izp] - m0) * wzp;
+                T l = (rd(f, ixm) - m0) * wxm;
+                l += (rd(f, ixp) - m0) * wxp;
+                l += (rd(f, iym) - m0) * wym;
+                l += (rd(f, iyp) - m0) * wyp;
+                l += (rd(f, izm) - m0) * wzm;
+                l += (rd(f, izp) - m0) * wzp;
                 lap[c] = l;
             }
             const T mx = ms[q][0], my = ms[q][1], mz = ms[q][2];
@@ -210,11 +253,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
             k[q][1] = llg * (ty + alpha * dy);
             k[q][2] = llg * (tz + alpha * dz);
         }
-        __syncthreads();                                             // [B] warp partials published, sm_m free again
+        if constexpr (COOP)                                          // fixed-order sum over the blocks' slots (every block: same bits)
+            reduce_block_partials(A.cpart[ev & 1], A.nblk, 2 * N + nsum_extra, A.nblk, warp, nwarp, lane, sh.red2);
+        __syncthreads();                                             // [B] partial sums published, stage-state buffer free again
         if (tid < N) {
             const int n = tid;
             double sx = 0.0, sy = 0.0;
-            for (int w = 0; w < nwarp; ++w) { sx += sh.part[w][2 * n]; sy += sh.part[w][2 * n + 1]; }
+            if constexpr (COOP) {
+                sx = sh.red2[2 * n]; sy = sh.red2[2 * n + 1];
+            } else {
+                for (int w = 0; w < nwarp; ++w) { sx += sh.part[w][2 * n]; sy += sh.part[w][2 * n + 1]; }
+            }
             const double Sre = sx * sh.invW[n], Sim = -sy * sh.invW[n];
             sh.S[n][0] = Sre; sh.S[n][1] = Sim;
             const double are = sh.as[n][0], aim = sh.as[n][1];
@@ -244,10 +293,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         } else if (s == 7 && tid >= 32 && tid < 32 + 3 * NSUB) {     // a second warp sums <m_s>
             const int i = tid - 32;
             double v = 0.0;
-            for (int w = 0; w < nwarp; ++w) v += sh.part[w][2 * N + i];
+            if constexpr (COOP) {
+                v = sh.red2[2 * N + i];
+            } else {
+                for (int w = 0; w < nwarp; ++w) v += sh.part[w][2 * N + i];
+            }
             sh.red[i] = v * A.inv_nc;
         }
         if (tid == 0) sh.rhs_evals++;
+        ++ev;
     };
 
 
@@ -330,11 +384,28 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         for (int o = 16; o > 0; o >>= 1) e2max = fmax(e2max, __shfl_xor_sync(0xffffffffu, e2max, o));
         if (lane == 0) sh.wmax[warp] = (double)e2max;
         __syncthreads();                                                 // [C]
+        if constexpr (COOP) {                                            // max over all blocks (order-independent)
+            double* const gmax = A.cmax[(int)(sh.steps & 1)];
+            if (tid == 0) {
+                double mxb = 0.0;
+                for (int w = 0; w < nwarp; ++w) mxb = fmax(mxb, sh.wmax[w]);
+                gmax[blockIdx.x] = mxb;
+            }
+            grid_barrier();
+            if (warp == 0) {
+                double v = 0.0;
+                for (int b = lane; b < A.nblk; b += 32) v = fmax(v, __ldcg(gmax + b));
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+                if (lane == 0) sh.wmax[0] = v;
+            }
+            __syncthreads();
+        }
 
         // ---- controller (stage_finish<7> in stage_kernel.cuh, same constants) ----
         if (tid == 0) {
             double mx = 0.0;
-            for (int w = 0; w < nwarp; ++w) mx = fmax(mx, sh.wmax[w]);
+            for (int w = 0; w < (COOP ? 1 : nwarp); ++w) mx = fmax(mx, sh.wmax[w]);
             double err = sqrt(mx);
             for (int n = 0; n < N; ++n) err = fmax(err, sh.serr[n]);
             const bool finite = err < CUDART_INF;
@@ -354,10 +425,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                 sh.dt_min = fmin(sh.dt_min, hh);
                 sh.dt_max = fmax(sh.dt_max, hh);
                 if (adaptive) { const double prop = hh * fac; sh.dt = sh.clamped ? fmax(prop, sh.dt) : prop; }
-                const bool take = A.trace != nullptr && A.sample_dt > 0.0 && sh.trace_n < A.trace_cap &&
+                const bool take = A.trace != nullptr && A.sample_dt > 0.0 && sh.trace_n < A.trace_cap &&      // every block counts,
                                   (adaptive ? (sh.clamped && sh.sample_hit)
                                             : ((sh.accepted - sh.trace_acc0) % sh.trace_stride == 0));
-                if (take) {
+                if (take && writer) {                                                                       // block 0 writes
                     double* row = A.trace + ((size_t)rep * A.trace_cap + sh.trace_n) * A.row_len;
                     row[0] = sh.t;
                     for (int n = 0; n < N; ++n) {
@@ -365,8 +436,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                         row[1 + 2 * N + 2 * n] = sh.S[n][0]; row[2 + 2 * N + 2 * n] = sh.S[n][1];
                     }
                     for (int i = 0; i < 3 * NSUB; ++i) row[1 + 4 * N + i] = sh.red[i];
-                    sh.trace_n++;
                 }
+                if (take) sh.trace_n++;
             } else if (sh.status == 0) {
                 sh.rejected++;
                 sh.dt = hh * fac;
@@ -394,8 +465,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) mg[(size_t)(q * 3 + c) * nc + cell] = y[q][c];
     }
-    if (tid < N) { A.a[((size_t)rep * N + tid) * 2] = sh.a[tid][0]; A.a[((size_t)rep * N + tid) * 2 + 1] = sh.a[tid][1]; }
-    if (tid == 0) {
+    if (writer && tid < N) { A.a[((size_t)rep * N + tid) * 2] = sh.a[tid][0]; A.a[((size_t)rep * N + tid) * 2 + 1] = sh.a[tid][1]; }
+    if (writer && tid == 0) {
         BatchCtl& cl = A.ctl[rep];
         cl.t = sh.t; cl.dt = sh.dt; cl.dt_min = sh.dt_min; cl.dt_max = sh.dt_max; cl.last_err = sh.err;
         cl.accepted = sh.accepted; cl.rejected = sh.rejected; cl.rhs_evals = sh.rhs_evals;

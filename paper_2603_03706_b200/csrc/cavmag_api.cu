@@ -63,6 +63,8 @@ struct cav_sim {
     size_t tsmem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int tgrid = 1;
     bool last_run_block = false;       // h_ctrl->ycur is known to be current (no stage-kernel run since the last pull)
+    bool use_coop = false;             // CAV_PATH_COOP: one cooperative launch per run, grid barriers instead of kernel boundaries
+    unsigned char* d_coop = nullptr;   // COOP scratch: block partials x2, block maxima x2, barrier counter
     bool use_block = false;            // CAV_PATH_BLOCK: the whole run in one thread block (k_batch with one replica)
     unsigned char* d_blk = nullptr;    // bridge buffers of the block path: BatchCtl, a, mode parameters, drive, B0
     bool want_pdl = true;              // cav_set_stage_overlap
@@ -279,12 +281,17 @@ int plan_tma(cav_sim* s) {
 StageArgs make_args(const cav_sim* s, unsigned long long handle);
 int sync_pull(cav_sim* s);
 
+constexpr int kCoopThreads = 512;
+
 void decide_path(cav_sim* s) {
     const bool block_ok = s->nc <= kBatchMaxCells;
+    const bool coop_ok = !block_ok && s->nc <= (long long)s->n_sm * kCoopThreads;
     s->use_block = (s->kernel_path == CAV_PATH_BLOCK && block_ok) || (s->kernel_path == CAV_PATH_AUTO && block_ok);
     if (s->kernel_path == CAV_PATH_GENERIC || s->use_block) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
+    else if (s->kernel_path == CAV_PATH_COOP) s->use_tma = false;
     else s->use_tma = s->tma_eligible && s->targs[1].Q >= (long long)s->n_sm;
+    s->use_coop = coop_ok && !s->use_tma && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO);
 }
 
 // ---- CAV_PATH_BLOCK: a grid of <= 1024 cells is integrated by ONE thread block for the whole run (k_batch with a
@@ -332,6 +339,8 @@ __global__ void k_block_out(Ctrl* c, const unsigned char* blk) {
 
 int run_block_path(cav_sim* s, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
     if (!s->d_blk) CK(cudaMalloc(&s->d_blk, kBlkBytes));
+    const size_t coop_part = sizeof(double) * (size_t)kMaxSums * s->n_sm, coop_max = sizeof(double) * (size_t)s->n_sm;
+    if (s->use_coop && !s->d_coop) CK(cudaMalloc(&s->d_coop, 2 * coop_part + 2 * coop_max + 64));
     if (!s->last_run_block) {                            // a stage-kernel run may have flipped ycur on the device
         int rc0 = sync_pull(s);
         if (rc0) return rc0;
@@ -360,7 +369,16 @@ int run_block_path(cav_sim* s, double t_end, double tol, double fixed_dt, double
     A.row_len = 1 + 4 * s->N + 3 * p.n_sub; A.trace = s->d_trace;
     A.drive = hc->drive_on ? reinterpret_cast<const double*>(s->d_blk + kBlkDrive) : nullptr;
     cudaError_t ce = cudaSuccess;
-    int rc = launch_batch_kernel(A, p.precision == CAV_F32, p.n_sub, false, s->smem_optin, s->stream, &ce);
+    int rc;
+    if (s->use_coop) {
+        A.gms[0] = s->MS[0]; A.gms[1] = s->MS[1];
+        A.cpart[0] = reinterpret_cast<double*>(s->d_coop); A.cpart[1] = reinterpret_cast<double*>(s->d_coop + coop_part);
+        A.cmax[0] = reinterpret_cast<double*>(s->d_coop + 2 * coop_part); A.cmax[1] = reinterpret_cast<double*>(s->d_coop + 2 * coop_part + coop_max);
+        A.bar = reinterpret_cast<unsigned long long*>(s->d_coop + 2 * coop_part + 2 * coop_max);
+        rc = launch_coop_kernel(A, p.precision == CAV_F32, p.n_sub, s->stream, &ce);
+    } else {
+        rc = launch_batch_kernel(A, p.precision == CAV_F32, p.n_sub, false, s->smem_optin, s->stream, &ce);
+    }
     if (rc == CAV_E_CUDA || rc == CAV_E_NOMEM) snprintf(s->cuda_err, sizeof(s->cuda_err), "k_batch launch: %s", cudaGetErrorString(ce));
     if (rc) return rc;
     k_block_out<<<1, 32, 0, s->stream>>>(s->d_ctrl, s->d_blk);
@@ -671,6 +689,7 @@ int cav_destroy(cav_sim* s) {
     cudaFree(s->d_trace);
     cudaFree(s->d_maps);
     cudaFree(s->d_blk);
+    cudaFree(s->d_coop);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     if (s->h_flag) cudaFreeHost(s->h_flag);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -702,9 +721,10 @@ int cav_set_block_cells(cav_sim* s, int cells) {
 }
 
 int cav_set_kernel_path(cav_sim* s, int path) {
-    if (!s || (path != CAV_PATH_AUTO && path != CAV_PATH_GENERIC && path != CAV_PATH_TMA && path != CAV_PATH_BLOCK)) return CAV_E_ARG;
+    if (!s || (path != CAV_PATH_AUTO && path != CAV_PATH_GENERIC && path != CAV_PATH_TMA && path != CAV_PATH_BLOCK && path != CAV_PATH_COOP)) return CAV_E_ARG;
     if (path == CAV_PATH_TMA && !s->tma_eligible) return CAV_E_UNSUPPORTED;
     if (path == CAV_PATH_BLOCK && s->nc > kBatchMaxCells) return CAV_E_UNSUPPORTED;
+    if (path == CAV_PATH_COOP && (s->nc <= kBatchMaxCells || s->nc > (long long)s->n_sm * kCoopThreads)) return CAV_E_UNSUPPORTED;
     s->kernel_path = path;
     s->graph_dirty = true;
     return CAV_OK;
@@ -713,7 +733,7 @@ int cav_set_kernel_path(cav_sim* s, int path) {
 int cav_get_kernel_path(cav_sim* s, int* path) {
     if (!s || !path) return CAV_E_ARG;
     decide_path(s);
-    *path = s->use_block ? CAV_PATH_BLOCK : s->use_tma ? CAV_PATH_TMA : CAV_PATH_GENERIC;
+    *path = s->use_block ? CAV_PATH_BLOCK : s->use_coop ? CAV_PATH_COOP : s->use_tma ? CAV_PATH_TMA : CAV_PATH_GENERIC;
     return CAV_OK;
 }
 
@@ -938,7 +958,7 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     if (std::isnan(t_end) || max_steps < 0) return CAV_E_ARG;
     if (std::isinf(t_end) && max_steps == 0) return CAV_E_ARG;
     decide_path(s);
-    if (s->use_block) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
+    if (s->use_block || s->use_coop) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     s->last_run_block = false;
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     CK(cudaGetLastError());

@@ -108,6 +108,28 @@ int launch_batch_kernel(BatchArgs& A, bool f32, int n_sub, bool two_per_sm, size
     return CAV_OK;
 }
 
+// Launches the cooperative variant (COOP) for ONE simulation of A.nc cells on ceil(nc / 512) co-resident blocks.
+int launch_coop_kernel(BatchArgs& A, bool f32, int n_sub, cudaStream_t stream, cudaError_t* cuda_err) {
+    auto fail = [&](cudaError_t e) { *cuda_err = e; cudaGetLastError(); return e == cudaErrorMemoryAllocation ? CAV_E_NOMEM : CAV_E_CUDA; };
+    const int threads = 512;
+    A.nblk = (A.nc + threads - 1) / threads;
+    A.n_rep = 1; A.u_in_smem = 0;
+    const void* fn = f32 ? (n_sub == 1 ? (const void*)k_batch<float, 1, 512, 1, true> : (const void*)k_batch<float, 2, 512, 1, true>)
+                         : (n_sub == 1 ? (const void*)k_batch<double, 1, 512, 1, true> : (const void*)k_batch<double, 2, 512, 1, true>);
+    int per_sm = 0, dev = 0, n_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0);
+    if (e != cudaSuccess) return fail(e);
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (A.nblk > per_sm * n_sm) return CAV_E_UNSUPPORTED;          // the grid barrier needs every block resident
+    e = cudaMemsetAsync(A.bar, 0, sizeof(unsigned long long), stream);
+    if (e != cudaSuccess) return fail(e);
+    void* params[] = {&A};
+    e = cudaLaunchCooperativeKernel(fn, dim3(A.nblk), dim3(threads), params, 0, stream);
+    if (e != cudaSuccess) return fail(e);
+    return CAV_OK;
+}
+
 }  // namespace cavmag
 
 extern "C" {

@@ -34,20 +34,25 @@ def oracle_of(w, **kw):
     return Oracle(w, **kw)
 
 
-PATHS = ["generic", "tma", "block"]
+PATHS = ["generic", "tma", "block", "coop"]
 
 
 def open_sim(api, w, prec, path, **kw):
     """A Sim forced onto one implementation of the step: the generic or the TMA stage kernels, or the single-block
-    integrator of grids up to 1024 cells (CAV_PATH_BLOCK).  Skips when the path is not eligible for this shape
-    (TMA: nx*sizeof(T) not a multiple of 16 bytes; BLOCK: more than 1024 cells)."""
+    integrator of grids up to 1024 cells (CAV_PATH_BLOCK), or the cooperative multi-block variant of it (CAV_PATH_COOP).
+    Skips when the path is not eligible for this shape (TMA: nx*sizeof(T) not a multiple of 16 bytes; BLOCK: more than 1024
+    cells; COOP: 1024 cells or fewer)."""
     sim = api.Sim(w, precision=prec, **kw)
-    want = {"tma": api.CAV_PATH_TMA, "generic": api.CAV_PATH_GENERIC, "block": api.CAV_PATH_BLOCK}[path]
+    want = {"tma": api.CAV_PATH_TMA, "generic": api.CAV_PATH_GENERIC, "block": api.CAV_PATH_BLOCK, "coop": api.CAV_PATH_COOP}[path]
     try:
         api.cav_set_kernel_path(sim.h, want)
     except api.CavError as e:
         sim.close()
-        assert e.status == api.CAV_E_UNSUPPORTED and path in ("tma", "block")
+        assert e.status == api.CAV_E_UNSUPPORTED and path in ("tma", "block", "coop")
+        if path == "coop":
+            nc = w.nx * w.ny * w.nz
+            assert nc <= 1024 or nc > 512 * 132, "COOP path refused although the grid is in its range"
+            pytest.skip("cooperative path: grid outside 1025 .. 512 x SMs cells")
         if path == "block":
             assert w.nx * w.ny * w.nz > 1024, "BLOCK path refused although the grid has at most 1024 cells"
             pytest.skip("single-block path: grid too large")
@@ -393,7 +398,7 @@ def test_resume_equals_single_run(api, path):
         st = api.cav_get_stats(sim.h)
     assert np.array_equal(m1, m2) and np.array_equal(a1, a2)
     # the single-block path keeps its slopes in registers and re-evaluates k1 at the start of every run
-    assert st["rhs_evals"] == 1 + 6 * 40 + (1 if path == "block" else 0)
+    assert st["rhs_evals"] == 1 + 6 * 40 + (1 if path in ("block", "coop") else 0)
 
 
 def test_edge_cases(api):
