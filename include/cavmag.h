@@ -191,8 +191,8 @@ int cav_set_sweep_order(cav_sim* sim, int serpentine);
  *                     same kernel as BLOCK, stage state and block partials through global memory); like BLOCK it does not
  *                     cache the final slope.  Cooperative grids do not overlap with each other: for many concurrent
  *                     simulations on several streams (a sweep) choose GENERIC.  CAV_E_UNSUPPORTED outside that range;
- *   CAV_PATH_AUTO     (default) BLOCK up to 1024 cells; TMA when eligible and the grid has at least one plane-tile per
- *                     SM; COOP for the sizes in between; else GENERIC.
+ *   CAV_PATH_AUTO     (default) BLOCK up to 1024 cells; COOP up to 512 x (number of SMs) cells; above that TMA when
+ *                     eligible, else GENERIC.
  * cav_get_kernel_path reports what the next run will use (CAV_PATH_GENERIC, _TMA, _BLOCK or _COOP). */
 int cav_set_kernel_path(cav_sim* sim, int path);
 int cav_get_kernel_path(cav_sim* sim, int* path);

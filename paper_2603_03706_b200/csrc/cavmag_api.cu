@@ -287,11 +287,10 @@ void decide_path(cav_sim* s) {
     const bool block_ok = s->nc <= kBatchMaxCells;
     const bool coop_ok = !block_ok && s->nc <= (long long)s->n_sm * kCoopThreads;
     s->use_block = (s->kernel_path == CAV_PATH_BLOCK && block_ok) || (s->kernel_path == CAV_PATH_AUTO && block_ok);
-    if (s->kernel_path == CAV_PATH_GENERIC || s->use_block) s->use_tma = false;
+    s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO);
+    if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
-    else if (s->kernel_path == CAV_PATH_COOP) s->use_tma = false;
     else s->use_tma = s->tma_eligible && s->targs[1].Q >= (long long)s->n_sm;
-    s->use_coop = coop_ok && !s->use_tma && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO);
 }
 
 // ---- CAV_PATH_BLOCK: a grid of <= 1024 cells is integrated by ONE thread block for the whole run (k_batch with a
