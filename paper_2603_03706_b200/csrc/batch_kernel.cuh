@@ -12,6 +12,10 @@
 // Same arithmetic per cell as k_stage (subtract-first exchange stencil, explicit Landau-Lifshitz form), so a
 // replica agrees with cav_run on the same inputs to rounding; the overlap sums are added in a different (fixed)
 // order.  Mode amplitudes, overlap sums and the controller are fp64 in both precisions.
+//
+// The same kernel also serves cav_run: with one replica for grids of up to 1024 cells (CAV_PATH_BLOCK), and as a
+// cooperative launch over several co-resident blocks for grids of up to 512 cells per SM (CAV_PATH_COOP, template flag
+// COOP: stage state and block partial sums through global memory, a grid barrier per evaluation).
 #pragma once
 #include <type_traits>
 

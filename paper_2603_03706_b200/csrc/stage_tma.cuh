@@ -1,8 +1,9 @@
 // The fused RK45 stage kernel, TMA-pipelined variant (hand-written CUDA for sm_100a).
 //
 // Same arithmetic as stage_kernel.cuh (one launch = one evaluation of the coupled right-hand
-// side at stage s, fused with the overlap partials, the next stage state, the error norm and,
-// in the last block, the mode ODEs + controller), but the data movement is Blackwell-native:
+// side at stage s, fused with the overlap partials, the next stage state and the error norm; the mode
+// ODEs of stages 2..6 are replayed by every block in the next kernel's prologue (deferred_finish), those of
+// stages 1 and 7 and the controller run in the last block), but the data movement is Blackwell-native:
 //
 //   * persistent grid, one CTA per SM; the flattened list of plane-tiles (x-y tile, z) is split
 //     into contiguous, equally long runs, one per CTA, so every SM gets the same number of
@@ -18,7 +19,10 @@
 //     x neighbours by warp shuffle, y/z neighbours from the halo box / the neighbouring ring
 //     slots, so no global load sits on the dependent path and the bytes in flight are set by
 //     the ring depth (~100-180 KB per SM) instead of by registers and occupancy;
-//   * results go straight from registers to global memory with coalesced 8-byte stores.
+//   * results go straight from registers to global memory with coalesced 8-byte stores;
+//   * inside the run graph consecutive stage kernels are joined by programmatic dependencies: a block's
+//     prologue (barrier init, tensor-map prefetch, control words, TMA loads of the streams the previous
+//     kernel does not write) runs before griddepcontrol.wait.
 //
 // Out-of-grid parts of a box are zero-filled by the TMA unit; the open (Neumann) boundary of
 // the exchange stencil (reading G9) is applied by substituting the centre value.
