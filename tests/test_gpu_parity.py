@@ -175,6 +175,8 @@ def test_cfg1_fixed_1000_steps(api, prec, variant, path):
     ((132, 9, 11), 8, 1, 0.1e-12),
     ((68, 17, 6), 1, 2, 0.05e-12),
     ((64, 8, 3), 32, 1, 0.1e-12),
+    ((24, 6, 4), 0, 1, 0.1e-12),       # plain LLG: no modes to finish between the stages
+    ((96, 20, 14), 0, 1, 0.1e-12),     # the same beyond the single-block range
 ])
 @pytest.mark.parametrize("path", PATHS)
 def test_busy_fixed_steps(api, prec, shape, N, n_sub, dt, path):
