@@ -250,6 +250,25 @@ def test_cfg3_full_size_steps(api):
     assert np.abs(S - S_direct).max() < 1e-7
 
 
+def test_cfg4_full_size_steps(api):
+    """128x128x64 two-sublattice antiferromagnet with dissipative coupling (BASELINE.json configs[3]), fp32 and fp64 on
+    the TMA path as bench.py times it: three fixed steps element by element against the oracle."""
+    w = W.cfg4(dissipative=True)
+    w.m0 = w.m0.astype(np.float32).astype(np.float64)
+    w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+    w.a0 = np.array([2e-3 + 1e-3j])
+    dt = 0.01e-12
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=3)
+    for prec, tol_m, tol_a in (("f64", 1e-12, 1e-12), ("f32", 2e-6, 1e-5)):
+        with api.Sim(w, precision=prec) as sim:
+            assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+            api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=3)
+            m, a = sim.get_m(), sim.get_a()
+        assert np.abs(m - ref.m).max() <= tol_m, prec
+        assert np.abs(a - ref.a).max() <= tol_a * np.abs(ref.a).max(), prec
+        assert np.abs(np.linalg.norm(m.astype(np.float64), axis=1) - 1).max() < (3e-7 if prec == "f32" else 1e-14)
+
+
 def test_cfg5_slab_32_modes(api):
     """cfg5's 512x512 plane and 32 mixed-coupling modes on a thinner slab (oracle memory/time bound)."""
     w = W.cfg5(nz=4, dtype=np.float64)
