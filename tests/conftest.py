@@ -13,6 +13,14 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on the B200 box)")
 
 
+def pytest_collection_modifyitems(config, items):
+    # a hung kernel (e.g. a grid barrier that never completes) must fail the test, not stall the run
+    if config.pluginmanager.hasplugin("timeout"):
+        for item in items:
+            if item.get_closest_marker("timeout") is None:
+                item.add_marker(pytest.mark.timeout(900))
+
+
 @pytest.fixture(scope="session", autouse=True)
 def _build_oracle():
     # building the checker is not using it; g++ only, a few seconds
