@@ -581,6 +581,45 @@ def run_concurrent_sweep(args):
     print(json.dumps(line), flush=True)
 
 
+# ----------------------------------------------------------------------------------------
+# --full-run: the configuration exactly as BASELINE.json states it, from t = 0 to its t_end
+# ----------------------------------------------------------------------------------------
+def run_full(args):
+    """Time to solution of one BASELINE.json config (adaptive tol, its own duration): ONE cav_run call = one launch of the
+    device-side step loop; wall time by CUDA events; |m| = 1, finiteness and the step statistics are checked."""
+    import torch
+    from paper_2603_03706_b200 import api
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    name = args.workload
+    w, prec = make_workload(name)
+    stream = torch.cuda.Stream()
+    with api.Sim(w, precision=prec, stream=stream.cuda_stream) as sim:
+        api.cav_set_trace(sim.h, w.t_end / 1000.0, 1000)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        api.cav_run(sim.h, w.t_end, tol=w.tol)
+        ev1.record(stream)
+        stream.synchronize()
+        sec = ev0.elapsed_time(ev1) * 1e-3
+        st = api.cav_get_stats(sim.h)
+        m = sim.get_m()
+        a = sim.get_a()
+        tr = api.cav_get_trace(sim.h)
+        path_used = api.cav_get_kernel_path(sim.h)
+    norm_err = float(np.abs(np.linalg.norm(m.astype(np.float64), axis=1) - 1.0).max())
+    assert st["t"] == w.t_end and np.isfinite(m).all() and np.isfinite(a).all() and tr.shape[0] == 1000
+    line = {"metric": "time to solution", "value": sec, "unit": "s", "higher_is_better": False, "n_gpus": 1,
+            "dtype": prec, "data": "synthetic",
+            "config": dict(config_of(w, prec, name), t_end_ns=w.t_end * 1e9,
+                           kernel_path={1: "generic", 2: "tma", 3: "block", 4: "coop"}[path_used]),
+            "accepted": st["accepted"], "rejected": st["rejected"], "rhs_evals": st["rhs_evals"],
+            "mean_dt_ps": w.t_end * 1e12 / max(st["accepted"], 1), "dt_min_ps": st["dt_min"] * 1e12, "dt_max_ps": st["dt_max"] * 1e12,
+            "sim_ns_per_s": w.t_end * 1e9 / sec, "cell_stage_per_s": w.n_cells * st["rhs_evals"] / sec,
+            "max_norm_error": norm_err, "max_abs_a": float(np.abs(a).max()) if a.size else 0.0, "trace_rows": int(tr.shape[0])}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -594,12 +633,16 @@ def main():
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
     ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma", "block", "coop"])
     ap.add_argument("--replicas", type=int, default=1184, help="cfg1_sweep: replicas in the batch")
+    ap.add_argument("--full-run", action="store_true",
+                    help="run the workload as BASELINE.json states it (t = 0 .. t_end, adaptive) and report the time to solution")
     ap.add_argument("--no-serpentine", action="store_true", help="every stage sweeps forward (A/B aid)")
     ap.add_argument("--no-stage-overlap", action="store_true", help="full dependencies between stage kernels (A/B aid)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
-    if args.impl == "reference":
+    if args.full_run:
+        run_full(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.workload == "cfg1_sweep":
         run_batch(args)
