@@ -398,6 +398,11 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         if (tid == 0) CAVMAG_MARK(1);
         const T h = (T)hd;
         const T ha21 = h * (T)kA[1][0];
+        T cn_reg[(NB > 0 && NB <= 8) ? NB : 1];
+        if constexpr (NB > 0 && NB <= 8) {
+#pragma unroll
+            for (int n = 0; n < NB; ++n) cn_reg[n] = s_cn[n];
+        }
         const T B0x = (T)A.B0[0], B0y = (T)A.B0[1], B0z = (T)A.B0[2];
         const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
         const T anp = (T)A.an_pref, axx = (T)A.axis[0], axy = (T)A.axis[1], axz = (T)A.axis[2];
@@ -510,7 +515,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 #pragma unroll
                     for (int i = 0; i < UCB; ++i) {
                         const int n = ch * kTmaUChunk + i;          // modes >= N: u zero-filled, c_n = 0
-                        const T cn = s_cn[n];
+                        const T cn = (NB <= 8) ? cn_reg[NB <= 8 ? n : 0] : s_cn[n];     // few modes: RF weights live in registers
 #pragma unroll
                         for (int v = 0; v < VEC; ++v) {
                             brf[v] += cn * un[i].v[v];
