@@ -114,6 +114,19 @@ __device__ __forceinline__ double lds_one(unsigned a, const double*) {
     return r;
 }
 
+// predicated scalar load from a shared-space address (0 when the predicate is off): the two edge lanes of a row take
+// their x neighbour from the halo without a divergent branch
+__device__ __forceinline__ float lds_one_if(unsigned a, unsigned pred, const float*) {
+    float r = 0.0f;
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.shared.f32 %0, [%1];\n}\n" : "+f"(r) : "r"(a), "r"(pred));
+    return r;
+}
+__device__ __forceinline__ double lds_one_if(unsigned a, unsigned pred, const double*) {
+    double r = 0.0;
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.shared.f64 %0, [%1];\n}\n" : "+d"(r) : "r"(a), "r"(pred));
+    return r;
+}
+
 // number of halo'd fields / plain cell fields the stage streams
 template <int STAGE> struct StageStreams {
     static constexpr int n_halo = (STAGE == 2) ? 2 : 1;
@@ -458,12 +471,13 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             }
             return a;
         };
-        auto ldm1 = [&](unsigned slot, int comp, unsigned off) -> T {
+        auto ldm1_if = [&](unsigned slot, int comp, unsigned off, unsigned pred) -> T {
             const unsigned p = slot + (unsigned)(comp * HPLANE) + off;
-            T a = lds_one(p, tag);
-            if constexpr (STAGE == 2) a = a + ha21 * lds_one(p + TA.hbox_bytes, tag);
+            T a = lds_one_if(p, pred, tag);
+            if constexpr (STAGE == 2) a = a + ha21 * lds_one_if(p + TA.hbox_bytes, pred, tag);
             return a;
         };
+        const unsigned is_lane0 = lane == 0 ? 1u : 0u, is_lane31 = lane == 31 ? 1u : 0u;
 
 #pragma unroll 1
         for (int pl = 0; pl < nplanes; ++pl) {
@@ -548,8 +562,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     const P nzp = ldm(dir > 0 ? sm_zp : sm_zm, comp, crow);
                     T xl = __shfl_up_sync(0xffffffffu, mc[s][c].v[VEC - 1], 1);
                     T xr = __shfl_down_sync(0xffffffffu, mc[s][c].v[0], 1);
-                    if (lane == 0) xl = ldm1(sm_zc, comp, crow - (unsigned)sizeof(T));
-                    if (lane == 31) xr = ldm1(sm_zc, comp, crow + 8u);
+                    const T xl_h = ldm1_if(sm_zc, comp, crow - (unsigned)sizeof(T), is_lane0);
+                    const T xr_h = ldm1_if(sm_zc, comp, crow + 8u, is_lane31);
+                    xl = is_lane0 ? xl_h : xl;
+                    xr = is_lane31 ? xr_h : xr;
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
                         const T m0 = mc[s][c].v[v];
