@@ -43,7 +43,7 @@ UNIT = "cell-stage/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per stage-kernel launch (mean over the six stages of
 # one step) from the `ncu --set full` capture summarised in profiles/ (file named beside each value).
 NCU_TRAFFIC_BYTES = {
-    "cfg3": 210.8e6,      # profiles/r1_v5_cfg3_stage_kernels.md (cold cache): read 181.3 MB + write 29.5 MB (algorithmic: 222.3 MB;
+    "cfg3": 211.2e6,      # profiles/r1_v6_cfg3_stage_kernels.md (cold cache): read 181.4 MB + write 29.8 MB (algorithmic: 222.3 MB;
                            # part of the stores is still in L2 when the next stage reads them)
 }
 
