@@ -478,16 +478,19 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
                 }
                 xl = __shfl_up_sync(0xffffffffu, mc[s][c].v[VEC - 1], 1);
                 xr = __shfl_down_sync(0xffffffffu, mc[s][c].v[0], 1);
-                if (!has_l) xl = mc[s][c].v[0];
-                else if (lane == 0) {
-                    if constexpr (STAGE == 2) xl = __ldg(y0 + base + cell - 1) + ha21 * __ldg(k1 + base + cell - 1);
-                    else xl = __ldg(ms + base + cell - 1);
+                // the two edge lanes of the warp fetch their x neighbour from memory: predicated loads, no divergent branch
+                const bool need_l = has_l && lane == 0, need_r = has_r && lane == 31;
+                T gl, gr;
+                if constexpr (STAGE == 2) {
+                    const T a0 = need_l ? __ldg(y0 + base + cell - 1) : (T)0, b0 = need_l ? __ldg(k1 + base + cell - 1) : (T)0;
+                    const T a1 = need_r ? __ldg(y0 + base + cell + VEC) : (T)0, b1 = need_r ? __ldg(k1 + base + cell + VEC) : (T)0;
+                    gl = a0 + ha21 * b0; gr = a1 + ha21 * b1;
+                } else {
+                    gl = need_l ? __ldg(ms + base + cell - 1) : (T)0;
+                    gr = need_r ? __ldg(ms + base + cell + VEC) : (T)0;
                 }
-                if (!has_r) xr = mc[s][c].v[VEC - 1];
-                else if (lane == 31) {
-                    if constexpr (STAGE == 2) xr = __ldg(y0 + base + cell + VEC) + ha21 * __ldg(k1 + base + cell + VEC);
-                    else xr = __ldg(ms + base + cell + VEC);
-                }
+                xl = !has_l ? mc[s][c].v[0] : (need_l ? gl : xl);
+                xr = !has_r ? mc[s][c].v[VEC - 1] : (need_r ? gr : xr);
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
                     const T m0 = mc[s][c].v[v];
