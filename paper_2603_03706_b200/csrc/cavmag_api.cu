@@ -202,7 +202,7 @@ bool encode_map(const cav_sim* s, CUtensorMap* out, void* base, int C, int bx, i
     cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     const CUtensorMapDataType dt = s->prm.precision == CAV_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
     return enc(out, dt, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 int tma_stage_naux(int stage) { return stage <= 2 ? 0 : stage == 7 ? 1 : stage == 6 ? 5 : stage; }
