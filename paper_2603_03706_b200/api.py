@@ -14,7 +14,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# CAVMAG_LIB selects another build of the same library (the profiling build libcavmag_probe.so); there is no fallback.
+# CAVMAG_LIB selects another build of the same library (same ABI); there is no fallback.
 LIB_PATH = os.environ.get("CAVMAG_LIB") or os.path.join(_HERE, "libcavmag.so")
 
 CAV_OK = 0

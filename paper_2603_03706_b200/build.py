@@ -32,16 +32,6 @@ def _newest(paths):
     return max(os.path.getmtime(p) for p in paths)
 
 
-PROBE_LIB = os.path.join(HERE, "libcavmag_probe.so")
-
-
-def build_probe(force: bool = False) -> str:
-    """The profiling build (-DCAVMAG_PROBE: per-block %globaltimer/clock64 marks inside the TMA stage kernels and
-    stage_finish, read back with cav_debug_probe) -> paper_2603_03706_b200/libcavmag_probe.so.  Used only by
-    `python -m paper_2603_03706_b200.probe`; the product library carries none of it."""
-    return build(force=force, defines=("-DCAVMAG_PROBE",), lib=PROBE_LIB, objdir=os.path.join(HERE, "build", "probe"))
-
-
 def build(force: bool = False, verbose: bool = False, defines=(), lib: str = LIB, objdir: str = OBJ) -> str:
     LIB, OBJ = lib, objdir
     srcs = [os.path.join(CSRC, s) for s in SOURCES]

@@ -1071,13 +1071,3 @@ int cav_get_launch_count(cav_sim* s, long long* n) {
 }
 
 }  // extern "C"
-
-#ifdef CAVMAG_PROBE
-// profiling builds only: copies the [8][tgrid][32] timestamp table to the host
-extern "C" int cav_debug_probe(cav_sim* s, unsigned long long* out, int* tgrid) {
-    cudaStreamSynchronize(s->stream);
-    cudaMemcpy(out, s->d_probe, 8 * 256 * 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
-    *tgrid = s->tgrid;
-    return 0;
-}
-#endif
