@@ -76,8 +76,11 @@ def algorithmic_bytes_per_cell_step(n_modes: int, n_sub: int, esize: int) -> int
     return (111 * n_sub + 6 * n_modes) * esize
 
 
-def config_of(w, prec, name):
+def config_of(w, prec, name, gpus=1):
+    """The workload, in the same words for the CUDA arm and the --impl reference arm (what differs between the arms -
+    kernel path, launch mode, the oracle's bounded sample - is reported outside `config`)."""
     return {"workload": name, "grid": [w.nx, w.ny, w.nz], "cells": w.n_cells, "n_sub": w.n_sub,
+            "parallelism": f"replicas x{gpus} (no collective)",
             "modes": w.n_modes, "cell_nm": w.dx * 1e9, "mode": "adaptive RK45 (Dormand-Prince 5(4))",
             "tol": w.tol, "precision": prec,
             "l2": "working set per step (11 cell fields + mode profiles) exceeds the 126 MB L2"
@@ -205,10 +208,24 @@ def cpu_baseline(name: str, w_full, budget_s: float = 15.0):
         ws = slab_workload(name, nz)
         steps = int(max(3, min(2000, budget_s / (per_cs * ws.n_cells * 6))))
         sec, evals, simt = time_oracle(ws, steps, 0, w_full.tol)
-    return {"value": ws.n_cells * evals / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{name} recipe on a {ws.nx}x{ws.ny}x{ws.nz} slab ({ws.n_cells} cells, {ws.n_modes} modes), "
-                      f"{steps} adaptive RK45 steps ({evals} RHS evaluations), fp64, {sec:.1f} s",
-            "ms_per_step": 1e3 * sec / steps}
+    out = {"value": ws.n_cells * evals / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"{name} recipe on a {ws.nx}x{ws.ny}x{ws.nz} slab ({ws.n_cells} cells, {ws.n_modes} modes), "
+                     f"{steps} adaptive RK45 steps ({evals} RHS evaluations), fp64, {sec:.1f} s",
+           "ms_per_step": 1e3 * sec / steps}
+    # the same oracle on ONE thread: a thinner slab, about a third of the budget
+    try:
+        oracle.set_threads(1)
+        per_cs1 = per_cs * cores                                  # first guess: perfect scaling
+        nz1 = int(max(1, min(w_full.nz, (budget_s / 3.0) / (per_cs1 * plane * 6 * 3))))
+        w1 = slab_workload(name, nz1)
+        steps1 = int(max(2, min(200, (budget_s / 3.0) / (per_cs1 * w1.n_cells * 6))))
+        sec1, evals1, _ = time_oracle(w1, steps1, 0, w_full.tol)
+        out["one_thread"] = {"value": w1.n_cells * evals1 / sec1, "unit": UNIT, "cores": 1,
+                             "sample": f"{name} recipe on a {w1.nx}x{w1.ny}x{w1.nz} slab, {steps1} adaptive RK45 steps "
+                                       f"({evals1} RHS evaluations), fp64, {sec1:.1f} s"}
+    finally:
+        oracle.set_threads(cores)
+    return out
 
 
 def run_reference(args):
@@ -231,14 +248,14 @@ def run_reference(args):
     value = ws.n_cells * evals / sec
     sample = (f"{name} recipe on a {ws.nx}x{ws.ny}x{ws.nz} slab ({ws.n_cells} cells, {ws.n_modes} modes) per step; "
               f"{args.steps} timed adaptive RK45 steps after {args.warmup} warm-up steps, fp64")
-    cfg = config_of(w_full, prec, name)
-    cfg["reference_sample"] = sample
+    cfg = config_of(w_full, prec, name, args.gpus)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": cfg, "sim_ns_per_s": simt * 1e9 / sec,
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "impl_config": {"reference_sample": sample, "arithmetic": "f64"},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
@@ -264,6 +281,72 @@ def aggregate_over_ranks(ms: float, e2e_s: float, units: float, e2e_units: float
 # ----------------------------------------------------------------------------------------
 # the CUDA path
 # ----------------------------------------------------------------------------------------
+def hbm_peak():
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        return float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def roofline_of(name, w, prec, ms, steps):
+    """Algorithmic bytes of one stage-kernel launch (mean of the six stages of a step) over its mean duration."""
+    esize = 4 if prec == "f32" else 8
+    launch_us = ms * 1e3 / (6 * steps)
+    bytes_per_launch = algorithmic_bytes_per_cell_step(w.n_modes, w.n_sub, esize) * w.n_cells / 6.0
+    achieved = bytes_per_launch / (launch_us * 1e-6) / 1e9
+    peak, peak_src = hbm_peak()
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": NCU_TRAFFIC_BYTES.get(name), "peak_source": peak_src, "kernel": "cavmag::k_stage_tma / k_stage (fused RK45 stage)",
+            "launch_us": launch_us, "algorithmic_bytes_per_launch": bytes_per_launch,
+            "frac_of_nominal_8TBs": achieved / 8000.0}
+
+
+def timed_steps(api, torch, h, stream, tol, steps, sampler=None, barrier=None):
+    """K steps = ONE cav_run_steps call (one CUDA-graph launch), CUDA events on the launching stream."""
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if barrier:
+        barrier()
+    if sampler:
+        sampler.start()
+    ev0.record(stream)
+    api.cav_run_steps(h, math.inf, tol=tol, max_steps=steps)
+    ev1.record(stream)
+    stream.synchronize()
+    if barrier:
+        barrier()
+    clocks = sampler.stop() if sampler else None
+    return ev0.elapsed_time(ev1), clocks
+
+
+def measure_extra(api, torch, name, args, local):
+    """One more large workload in the same process (device-resident timing only): value, ms per step, roofline
+    fraction and the clocks seen during its timed region."""
+    w, prec = make_workload(name, 0)
+    stream = torch.cuda.Stream()
+    with api.Sim(w, precision=prec, stream=stream.cuda_stream) as sim:
+        h = sim.h
+        path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma", api.CAV_PATH_BLOCK: "block",
+                     api.CAV_PATH_COOP: "coop"}[api.cav_get_kernel_path(h)]
+        api.cav_run_steps(h, math.inf, tol=w.tol, max_steps=args.spinup)
+        api.cav_run_steps(h, math.inf, tol=w.tol, max_steps=max(args.warmup, 3))
+        api.cav_sync(h)
+        st0 = api.cav_get_stats(h)
+        steps = args.extra_steps
+        sampler = ClockSampler(torch.cuda.current_device() if os.environ.get("CUDA_VISIBLE_DEVICES") is None else local)
+        ms, clocks = timed_steps(api, torch, h, stream, w.tol, steps, sampler)
+        api.cav_sync(h)
+        st1 = api.cav_get_stats(h)
+        evals = st1["rhs_evals"] - st0["rhs_evals"]
+        assert evals == 6 * steps, (name, evals)
+        m = sim.get_m()
+    assert np.isfinite(m).all() and abs(float(np.abs(np.linalg.norm(m.astype(np.float64), axis=1) - 1).max())) < 1e-5
+    return {"value": w.n_cells * evals / (ms * 1e-3), "unit": UNIT, "steps": steps, "ms_per_step": ms / steps,
+            "dtype": prec, "config": config_of(w, prec, name), "kernel_path": path_used,
+            "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
+            "sim_ns_per_s": (st1["t"] - st0["t"]) * 1e9 / (ms * 1e-3),
+            "roofline": roofline_of(name, w, prec, ms, steps), "clocks": clocks}
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -286,7 +369,6 @@ def run_cuda(args):
     name = args.workload
     w, prec = make_workload(name, rank)
     esize = 4 if prec == "f32" else 8
-    np_dtype = np.float32 if prec == "f32" else np.float64
     tol = w.tol
     stream = torch.cuda.Stream()
     path = {"auto": None, "generic": api.CAV_PATH_GENERIC, "tma": api.CAV_PATH_TMA, "block": api.CAV_PATH_BLOCK, "coop": api.CAV_PATH_COOP}[args.kernel_path]
@@ -308,17 +390,8 @@ def run_cuda(args):
     api.cav_sync(h)
     st0 = api.cav_get_stats(h)
     n0 = api.cav_get_launch_count(h)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler = ClockSampler(torch.cuda.current_device() if os.environ.get("CUDA_VISIBLE_DEVICES") is None else local)
-    barrier()
-    sampler.start()
-    ev0.record(stream)
-    api.cav_run_steps(h, math.inf, tol=tol, max_steps=args.steps)
-    ev1.record(stream)
-    stream.synchronize()
-    barrier()
-    clocks = sampler.stop()
-    ms = ev0.elapsed_time(ev1)
+    ms, clocks = timed_steps(api, torch, h, stream, tol, args.steps, sampler, barrier)
     overlap_active = api.cav_get_stage_overlap(h)
     api.cav_sync(h)                                   # raises on a device-side error status
     st1 = api.cav_get_stats(h)
@@ -328,6 +401,9 @@ def run_cuda(args):
     # the single-block path (grids up to 1024 cells) re-evaluates k1 at the start of a run: one more evaluation
     assert steps_done == args.steps and evals in (6 * args.steps, 6 * args.steps + 1), (steps_done, evals)
     sim_t = st1["t"] - st0["t"]
+    # SURVEY.md 8(d) "median of 5": the same K-step launch five more times (reported beside the contract's one timed region)
+    rep_ms = [timed_steps(api, torch, h, stream, tol, args.steps)[0] for _ in range(args.repeats)]
+    api.cav_sync(h)
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region, every step ----
     k_e2e = min(args.steps, args.e2e_steps)
@@ -353,6 +429,7 @@ def run_cuda(args):
     se1 = api.cav_get_stats(h)
     e2e_evals = se1["rhs_evals"] - se0["rhs_evals"]
     io_bytes = int(np.prod(sim.shape_m)) * esize + 16 * N
+    sim.close()
 
     # ---- max over ranks, sum of units ----
     agg = aggregate_over_ranks(ms, e2e_s, float(nc * evals), float(nc * e2e_evals), sim_t, world, "cuda")
@@ -361,23 +438,13 @@ def run_cuda(args):
     units = [agg["units"], agg["e2e_units"], agg["sim_t_sum"]]
 
     if rank == 0:
-        launches = 6 * args.steps
-        launch_us = ms * 1e3 / launches                       # this rank's mean stage-kernel duration
-        bytes_per_launch = algorithmic_bytes_per_cell_step(N, w.n_sub, esize) * nc / 6.0
-        achieved = bytes_per_launch / (launch_us * 1e-6) / 1e9
-        peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-        if os.path.exists(peaks_path):
-            peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-        else:
-            peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-        traffic = NCU_TRAFFIC_BYTES.get(name)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
-            "config": dict(config_of(w, prec, name), parallelism=f"replicas x{world} (no collective)",
-                           launch_mode=args.launch_mode, kernel_path=path_used,
-                           stage_overlap=bool(overlap_active), serpentine=not args.no_serpentine),
+            "config": config_of(w, prec, name, world),
+            "impl_config": {"launch_mode": args.launch_mode, "kernel_path": path_used,
+                            "stage_overlap": bool(overlap_active), "serpentine": not args.no_serpentine},
             "sim_ns_per_s": float(units[2]) * 1e9 / (ms_max * 1e-3) / world,
             "mean_dt_ps": sim_t * 1e12 / max(st1["accepted"] - st0["accepted"], 1),
             "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
@@ -387,15 +454,25 @@ def run_cuda(args):
                     "note": "every step: cav_set_m/cav_set_a from pinned host memory, cav_run_steps(1), cav_get_m/cav_get_a "
                             "to host; FSAL is lost at each upload (7 RHS evaluations per step)"},
             "gpu_launches": int(n1 - n0),
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "peak_source": peak_src, "kernel": "cavmag::k_stage (fused RK45 stage)",
-                         "launch_us": launch_us, "algorithmic_bytes_per_launch": bytes_per_launch,
-                         "frac_of_nominal_8TBs": achieved / 8000.0},
+            "roofline": roofline_of(name, w, prec, ms, args.steps),
         }
+        if rep_ms:
+            med = statistics.median(rep_ms)
+            line["repeats"] = {"n": len(rep_ms), "ms_per_step": [x / args.steps for x in rep_ms],
+                               "ms_per_step_median": med / args.steps, "value_median": nc * 6 * args.steps / (med * 1e-3),
+                               "roofline_frac_median": roofline_of(name, w, prec, med, args.steps)["frac"],
+                               "note": "the same K-step graph launch repeated (this rank), after the contract's timed region"}
+        if world == 1 and not args.no_extras and name == "cfg3":
+            # the other large configs of BASELINE.json, measured in the same process (device-resident timing)
+            line["workloads"] = {}
+            for extra in ("cfg4", "cfg4_f64", "cfg5"):
+                try:
+                    line["workloads"][extra] = measure_extra(api, torch, extra, args, local)
+                except Exception as e:              # an extra must never cost the headline line
+                    line["workloads"][extra] = {"error": f"{type(e).__name__}: {e}"}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(name, w)
         print(json.dumps(line), flush=True)
-    sim.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -611,8 +688,8 @@ def run_full(args):
     assert st["t"] == w.t_end and np.isfinite(m).all() and np.isfinite(a).all() and tr.shape[0] == 1000
     line = {"metric": "time to solution", "value": sec, "unit": "s", "higher_is_better": False, "n_gpus": 1,
             "dtype": prec, "data": "synthetic",
-            "config": dict(config_of(w, prec, name), t_end_ns=w.t_end * 1e9,
-                           kernel_path={1: "generic", 2: "tma", 3: "block", 4: "coop"}[path_used]),
+            "config": dict(config_of(w, prec, name), t_end_ns=w.t_end * 1e9),
+            "impl_config": {"kernel_path": {1: "generic", 2: "tma", 3: "block", 4: "coop"}[path_used]},
             "accepted": st["accepted"], "rejected": st["rejected"], "rhs_evals": st["rhs_evals"],
             "mean_dt_ps": w.t_end * 1e12 / max(st["accepted"], 1), "dt_min_ps": st["dt_min"] * 1e12, "dt_max_ps": st["dt_max"] * 1e12,
             "sim_ns_per_s": w.t_end * 1e9 / sec, "cell_stage_per_s": w.n_cells * st["rhs_evals"] / sec,
@@ -629,6 +706,9 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--e2e-steps", type=int, default=300)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the cfg4 / cfg4_f64 / cfg5 sub-records of the default cfg3 run")
+    ap.add_argument("--extra-steps", type=int, default=300, help="timed steps of each extra workload")
+    ap.add_argument("--repeats", type=int, default=5, help="extra repetitions of the K-step launch (median reported)")
     ap.add_argument("--spinup", type=int, default=40, help="untimed setup steps that let dt settle")
     ap.add_argument("--launch-mode", default="graph", choices=["graph", "stream"])
     ap.add_argument("--kernel-path", default="auto", choices=["auto", "generic", "tma", "block", "coop"])

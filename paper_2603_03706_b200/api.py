@@ -129,17 +129,40 @@ def _check(st: int, where: str, sim=None):
         raise CavError(st, where, detail)
 
 
-def _ptr(x):
-    """(address, is_device, keepalive) of a numpy array, a torch tensor or a raw int device address."""
+# handle -> (numpy dtype of the cell fields, n_sub, cells, replicas): what a cell-field buffer handed to the
+# library must look like.  The C ABI takes untyped pointers, so the binding is the place to refuse a float64
+# array for an f32 simulation, or a wrongly sized one, before the library reads or writes out of bounds.
+_HANDLES: dict = {}
+
+
+def _ptr(x, dtype=None, count=None, what="buffer"):
+    """(address, is_device, keepalive) of a numpy array or a torch tensor; with dtype / count given, the
+    element type and the number of elements must match exactly (ValueError otherwise)."""
     if isinstance(x, np.ndarray):
         if not x.flags["C_CONTIGUOUS"]:
             raise ValueError("array must be C-contiguous")
+        if dtype is not None and x.dtype != np.dtype(dtype):
+            raise ValueError(f"{what}: dtype {x.dtype} does not match the simulation's precision ({np.dtype(dtype)})")
+        if count is not None and x.size != count:
+            raise ValueError(f"{what}: {x.size} elements, expected {count}")
         return x.ctypes.data, 0, x
     if hasattr(x, "data_ptr"):          # torch tensor (duck-typed; torch is not imported here)
         if not x.is_contiguous():
             raise ValueError("tensor must be contiguous")
+        if dtype is not None and str(x.dtype) != "torch." + np.dtype(dtype).name:
+            raise ValueError(f"{what}: dtype {x.dtype} does not match the simulation's precision ({np.dtype(dtype)})")
+        if count is not None and x.numel() != count:
+            raise ValueError(f"{what}: {x.numel()} elements, expected {count}")
         return x.data_ptr(), (1 if x.is_cuda else 0), x
     raise TypeError(f"unsupported buffer type {type(x)}")
+
+
+def _field_spec(h, n_fields=None, per_replica=True):
+    """(dtype, element count) of a cell-field buffer of handle h: n_fields components per cell (default: the
+    magnetisation, 3 n_sub), times the replicas of a batch when per_replica."""
+    dt, n_sub, nc, n_rep = _HANDLES[h]
+    nf = 3 * n_sub if n_fields is None else n_fields
+    return dt, nf * nc * (n_rep if per_replica else 1)
 
 
 def _darr(x, n):
@@ -169,10 +192,12 @@ def cav_create(grid, params) -> int:
     g, p = _grid_params(grid, params)
     h = _vp()
     _check(_lib.cav_create(C.byref(g), C.byref(p), C.byref(h)), "cav_create")
+    _HANDLES[h.value] = (np.float32 if p.precision == CAV_F32 else np.float64, p.n_sub, g.nx * g.ny * g.nz, 1)
     return h.value
 
 
 def cav_destroy(sim) -> None:
+    _HANDLES.pop(sim, None)
     _check(_lib.cav_destroy(sim), "cav_destroy")
 
 
@@ -194,7 +219,7 @@ def cav_set_modes(sim, u, omega, kappa, g, Gamma=None, Phi=None) -> None:
     if N == 0:
         _check(_lib.cav_set_modes(sim, 0, None, 0, None, None, None, None, None), "cav_set_modes", sim)
         return
-    addr, dev, keep = _ptr(u)
+    addr, dev, keep = _ptr(u, *_field_spec(sim, N), what="u")
     po, ko = _darr(omega, N)
     pk, kk = _darr(kappa, N)
     pg, kg = _darr(g, N)
@@ -204,17 +229,19 @@ def cav_set_modes(sim, u, omega, kappa, g, Gamma=None, Phi=None) -> None:
 
 
 def cav_set_m(sim, m) -> None:
-    addr, dev, keep = _ptr(m)
+    addr, dev, keep = _ptr(m, *_field_spec(sim), what="m")
     _check(_lib.cav_set_m(sim, _vp(addr), dev), "cav_set_m", sim)
 
 
 def cav_get_m(sim, out) -> None:
-    addr, dev, keep = _ptr(out)
+    addr, dev, keep = _ptr(out, *_field_spec(sim), what="m_out")
     _check(_lib.cav_get_m(sim, _vp(addr), dev), "cav_get_m", sim)
 
 
 def cav_set_a(sim, a) -> None:
     a = np.ascontiguousarray(np.asarray(a, dtype=np.complex128)).view(np.float64)
+    if a.size > 2 * CAV_MAX_MODES:
+        raise ValueError("a: more than CAV_MAX_MODES amplitudes")
     _check(_lib.cav_set_a(sim, a.ctypes.data_as(_dp)), "cav_set_a", sim)
 
 
@@ -231,7 +258,7 @@ def cav_get_overlaps(sim, N: int) -> np.ndarray:
 
 
 def cav_get_dmdt(sim, out) -> None:
-    addr, dev, keep = _ptr(out)
+    addr, dev, keep = _ptr(out, *_field_spec(sim), what="dmdt_out")
     _check(_lib.cav_get_dmdt(sim, _vp(addr), dev), "cav_get_dmdt", sim)
 
 
@@ -385,10 +412,12 @@ def cav_batch_create(grid, params, n_rep: int) -> int:
     g, p = _grid_params(grid, params)
     h = _vp()
     _check(_lib.cav_batch_create(C.byref(g), C.byref(p), int(n_rep), C.byref(h)), "cav_batch_create")
+    _HANDLES[h.value] = (np.float32 if p.precision == CAV_F32 else np.float64, p.n_sub, g.nx * g.ny * g.nz, int(n_rep))
     return h.value
 
 
 def cav_batch_destroy(b) -> None:
+    _HANDLES.pop(b, None)
     _check(_lib.cav_batch_destroy(b), "cav_batch_destroy")
 
 
@@ -409,7 +438,7 @@ def cav_batch_set_modes(b, u, omega, kappa, g, Gamma=None, Phi=None, per_replica
         _check(_lib.cav_batch_set_modes(b, 0, None, None, None, None, None, None, 0), "cav_batch_set_modes")
         return
     n = om.size
-    addr, _, keep = _ptr(u)
+    addr, _, keep = _ptr(u, *_field_spec(b, N, per_replica=False), what="u")
     po, ko = _darr(omega, n)
     pk, kk = _darr(kappa, n)
     pg, kg = _darr(g, n)
@@ -462,7 +491,7 @@ def cav_batch_set_drive(b, amp, t0=None, sigma=None, omega_d=None) -> None:
 
 
 def cav_batch_set_m(b, m: np.ndarray, per_replica: bool = False) -> None:
-    addr, _, keep = _ptr(m)
+    addr, _, keep = _ptr(m, *_field_spec(b, per_replica=bool(per_replica)), what="m")
     _check(_lib.cav_batch_set_m(b, _vp(addr), int(bool(per_replica))), "cav_batch_set_m")
 
 
@@ -486,7 +515,7 @@ def cav_batch_run(b, t_end: float, tol: float = 0.0, fixed_dt: float = 0.0, dt_i
 
 
 def cav_batch_get_m(b, out: np.ndarray) -> None:
-    addr, _, keep = _ptr(out)
+    addr, _, keep = _ptr(out, *_field_spec(b), what="m_out")
     _check(_lib.cav_batch_get_m(b, _vp(addr)), "cav_batch_get_m")
 
 

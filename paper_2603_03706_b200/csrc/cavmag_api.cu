@@ -238,6 +238,13 @@ int plan_tma(cav_sim* s) {
     const int ntx = (s->grid.nx + TX - 1) / TX, nty = (s->grid.ny + kTmaTY - 1) / kTmaTY;
     const long long Q = (long long)ntx * nty * s->grid.nz;
     s->tgrid = (int)(Q < s->n_sm ? Q : s->n_sm);
+    // Prefetching k_2..k_{s-2} before griddepcontrol.wait is only ordered after kernel s-2 when a block of kernel s
+    // cannot be resident beside a block of kernel s-1 that has not passed its own wait (stage_tma.cuh): one CTA per SM
+    // for every stage kernel (each asks for more than half an SM's shared memory) and a grid that fills every SM.
+    int smem_sm = 0, dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev) != cudaSuccess) { cudaGetLastError(); smem_sm = 0; }
+    bool all_big = true;
     for (int stage = 1; stage <= 7; ++stage) {
         const void* fn = stage_tma_fn(s, stage);
         if (!fn) return CAV_OK;
@@ -271,9 +278,14 @@ int plan_tma(cav_sim* s) {
         if (bDm == 0) return CAV_OK;             // does not fit: stay on the generic kernels
         t.Da = bDa > 0 ? bDa : 1; t.Du = bDu > 0 ? bDu : 1; t.Dm = bDm;
         s->tsmem[stage] = (size_t)bDa * t.aux_slot_bytes + (size_t)bDu * t.u_slot_bytes + (size_t)bDm * t.ms_slot_bytes + 128;
+        const size_t half = (size_t)smem_sm / 2 + 1024;
+        if (s->tsmem[stage] < half && half <= budget) s->tsmem[stage] = half;      // shallow rings: still one CTA per SM
+        if (2 * s->tsmem[stage] <= (size_t)smem_sm) all_big = false;
         // the attribute is per function, not per simulation: always raise it to the device limit
         CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(s->smem_optin - fa.sharedSizeBytes)));
     }
+    const bool one_cta = smem_sm > 0 && s->tgrid == s->n_sm;
+    for (int stage = 1; stage <= 7; ++stage) s->targs[stage].pre_k = (one_cta && all_big) ? 1 : 0;
     s->tma_eligible = true;
     return CAV_OK;
 }
@@ -647,7 +659,7 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     s->own_stream = true;
     for (int i = 0; i < 2; ++i) { CKC(cudaMalloc(&s->Y[i], s->field_bytes)); CKC(cudaMalloc(&s->MS[i], s->field_bytes)); }
     for (int i = 0; i < 7; ++i) CKC(cudaMalloc(&s->K[i], s->field_bytes));
-    CKC(cudaMalloc(&s->partial, sizeof(double) * (size_t)kMaxSums * s->pstride));
+    CKC(cudaMalloc(&s->partial, sizeof(double) * 2 * (size_t)kMaxSums * s->pstride));      // two buffers: stage parity
     CKC(cudaMalloc(&s->partial_max, sizeof(double) * (size_t)s->pstride));
     CKC(cudaMalloc(&s->d_ctrl, sizeof(Ctrl)));
     CKC(cudaMallocHost(&s->h_ctrl, sizeof(Ctrl)));
@@ -762,16 +774,58 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
     if (N > 0 && (!u || !omega || !kappa || !g)) return CAV_E_ARG;
     int rc = sync_pull(s);
     if (rc) return rc;
+    // Any failure below leaves the handle in a consistent state with NO modes: the old graph and the u tensor map
+    // may point at a buffer that has been freed or overwritten, so they are dropped, not kept.
+    auto fail = [&](int code, cudaError_t e = cudaSuccess) {
+        if (e != cudaSuccess) {
+            snprintf(s->cuda_err, sizeof(s->cuda_err), "cav_set_modes: %s", cudaGetErrorString(e));
+            cudaGetLastError();
+        }
+        s->N = 0; s->nb = 0;
+        Ctrl* c = s->h_ctrl;
+        c->N = 0; c->k1_valid = 0; c->drive_on = 0;
+        destroy_graph(s);
+        plan_tma(s);
+        push_ctrl(s);
+        return code;
+    };
+    auto cuda_fail = [&](cudaError_t e) { return fail(e == cudaErrorMemoryAllocation ? CAV_E_NOMEM : CAV_E_CUDA, e); };
     const size_t bytes = (size_t)N * s->nc * s->esize;
+    cudaError_t e;
     if (bytes > s->u_bytes) {
         cudaFree(s->u);
         s->u = nullptr;
         s->u_bytes = 0;
-        CK(cudaMalloc(&s->u, bytes));
+        if ((e = cudaMalloc(&s->u, bytes)) != cudaSuccess) return cuda_fail(e);
         s->u_bytes = bytes;
     }
-    if (N > 0)
-        CK(cudaMemcpyAsync(s->u, u, bytes, u_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
+    if (N > 0 && (e = cudaMemcpyAsync(s->u, u, bytes, u_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream)) != cudaSuccess)
+        return cuda_fail(e);
+    // overlap normalisation W_n into a temporary first: CAV_E_SINGULAR_NORM must not leave half-set mode tables behind
+    double invW[kMaxModes];
+    for (int n = 0; n < N; ++n) invW[n] = 1.0 / (double)s->nc;
+    if (N > 0 && s->prm.overlap_norm == CAV_NORM_SUM_U) {
+        double* d_out = nullptr;
+        if ((e = cudaMalloc(&d_out, sizeof(double) * 256 * N)) != cudaSuccess) return cuda_fail(e);
+        if (s->prm.precision == CAV_F32) k_sum_u<float><<<dim3(256, N), 256, 0, s->stream>>>((const float*)s->u, s->nc, d_out);
+        else k_sum_u<double><<<dim3(256, N), 256, 0, s->stream>>>((const double*)s->u, s->nc, d_out);
+        s->host_launches++;
+        double* h = new (std::nothrow) double[256 * (size_t)N];
+        if (!h) { cudaFree(d_out); return fail(CAV_E_NOMEM); }
+        e = cudaMemcpyAsync(h, d_out, sizeof(double) * 256 * N, cudaMemcpyDeviceToHost, s->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+        cudaFree(d_out);
+        if (e != cudaSuccess) { delete[] h; return cuda_fail(e); }
+        bool singular = false;
+        for (int n = 0; n < N; ++n) {
+            double sum = 0.0;
+            for (int b = 0; b < 256; ++b) sum += h[n * 256 + b];
+            if (std::fabs(sum) < 1e-6 * (double)s->nc) singular = true;
+            else invW[n] = 1.0 / sum;
+        }
+        delete[] h;
+        if (singular) return fail(CAV_E_SINGULAR_NORM);
+    }
     Ctrl* c = s->h_ctrl;
     c->N = N;
     for (int n = 0; n < N; ++n) {
@@ -781,36 +835,16 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         c->Gre[n] = g[n] + Gm * std::cos(Ph);
         c->Gim[n] = Gm * std::sin(Ph);
         c->Gbre[n] = c->Gre[n]; c->Gbim[n] = c->Gim[n];      // reciprocal until cav_set_backaction
-        c->invW[n] = 1.0 / (double)s->nc;
+        c->invW[n] = invW[n];
         c->a[n][0] = c->a[n][1] = 0.0;
     }
     c->drive_on = 0;                     // a new mode set clears the drive
-    if (N > 0 && s->prm.overlap_norm == CAV_NORM_SUM_U) {
-        double* d_out = nullptr;
-        CK(cudaMalloc(&d_out, sizeof(double) * 256 * N));
-        if (s->prm.precision == CAV_F32) k_sum_u<float><<<dim3(256, N), 256, 0, s->stream>>>((const float*)s->u, s->nc, d_out);
-        else k_sum_u<double><<<dim3(256, N), 256, 0, s->stream>>>((const double*)s->u, s->nc, d_out);
-        s->host_launches++;
-        double* h = (double*)malloc(sizeof(double) * 256 * N);
-        cudaError_t e1 = cudaMemcpyAsync(h, d_out, sizeof(double) * 256 * N, cudaMemcpyDeviceToHost, s->stream);
-        cudaError_t e2 = cudaStreamSynchronize(s->stream);
-        cudaFree(d_out);
-        if (e1 != cudaSuccess || e2 != cudaSuccess) { free(h); return CAV_E_CUDA; }
-        for (int n = 0; n < N; ++n) {
-            double sum = 0.0;
-            for (int b = 0; b < 256; ++b) sum += h[n * 256 + b];
-            if (std::fabs(sum) < 1e-6 * (double)s->nc) { free(h); return CAV_E_SINGULAR_NORM; }
-            c->invW[n] = 1.0 / sum;
-        }
-        free(h);
-    }
     c->k1_valid = 0;
     s->N = N;
-    const int nb = bucket(N);
-    if (nb != s->nb) { s->nb = nb; }
-    s->graph_dirty = true;
+    s->nb = bucket(N);
+    destroy_graph(s);                    // the old graph's kernels were instantiated for the old mode bucket / u pointer
     rc = plan_tma(s);
-    if (rc) return rc;
+    if (rc) return fail(rc);
     return push_ctrl(s);
 }
 

@@ -209,7 +209,24 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
                         const double* Gamma, const double* Phi, int per_replica) {
     if (!b || N < 0 || N > CAV_MAX_MODES) return CAV_E_ARG;
     if (N > 0 && (!u || !omega || !kappa || !g)) return CAV_E_ARG;
+    // overlap normalisation W_n (G4) first, from the caller's host array: N_cells, or sum_r u_n (fixed-order host sum).
+    // CAV_E_SINGULAR_NORM is returned before anything in the handle has changed.
+    std::vector<double> invW(N > 0 ? N : 1, 1.0 / (double)b->nc);
+    if (N > 0 && b->prm.overlap_norm == CAV_NORM_SUM_U) {
+        for (int n = 0; n < N; ++n) {
+            double sum = 0.0;
+            for (int r = 0; r < b->nc; ++r)
+                sum += b->esize == 4 ? (double)((const float*)u)[(size_t)n * b->nc + r] : ((const double*)u)[(size_t)n * b->nc + r];
+            if (std::fabs(sum) < 1e-6 * (double)b->nc) return CAV_E_SINGULAR_NORM;
+            invW[n] = 1.0 / sum;
+        }
+    }
     CKB(cudaStreamSynchronize(b->stream));
+    // a CUDA failure below leaves the batch with no modes (consistent), not with a half-uploaded table
+    struct Guard {
+        cav_batch* b; bool ok;
+        ~Guard() { if (!ok) { b->N = 0; cudaFree(b->d_u); b->d_u = nullptr; b->h_modep.clear(); b->modep_per_rep = 0; cudaGetLastError(); } }
+    } guard{b, false};
     cudaFree(b->d_u);
     b->d_u = nullptr;
     cudaFree(b->d_drive);
@@ -220,17 +237,6 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
         const size_t ub = (size_t)N * b->nc * b->esize;
         CKB(cudaMalloc(&b->d_u, ub));
         CKB(cudaMemcpyAsync(b->d_u, u, ub, cudaMemcpyHostToDevice, b->stream));
-        // overlap normalisation W_n (G4): N_cells, or sum_r u_n (fixed-order host sum)
-        std::vector<double> invW(N, 1.0 / (double)b->nc);
-        if (b->prm.overlap_norm == CAV_NORM_SUM_U) {
-            for (int n = 0; n < N; ++n) {
-                double sum = 0.0;
-                for (int r = 0; r < b->nc; ++r)
-                    sum += b->esize == 4 ? (double)((const float*)u)[(size_t)n * b->nc + r] : ((const double*)u)[(size_t)n * b->nc + r];
-                if (std::fabs(sum) < 1e-6 * (double)b->nc) return CAV_E_SINGULAR_NORM;
-                invW[n] = 1.0 / sum;
-            }
-        }
         const int reps = per_replica ? b->n_rep : 1;
         std::vector<double> mp((size_t)reps * 7 * N);
         for (int r = 0; r < reps; ++r)
@@ -250,6 +256,7 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
     cudaFree(b->d_trace);
     b->d_trace = nullptr; b->trace_cap = 0; b->sample_dt = 0.0;      // the row length changed
     CKB(cudaStreamSynchronize(b->stream));
+    guard.ok = true;
     return CAV_OK;
 }
 

@@ -74,7 +74,7 @@ struct StageArgs {
     void* MS[2];         // materialised stage states (MS[0] doubles as the partial-error field)
     void* K[7];          // slope fields
     const void* u;       // [N][nc]
-    double* partial;     // [kMaxSums][pstride] block partial sums
+    double* partial;     // [2][kMaxSums][pstride] block partial sums, double-buffered by stage parity (stage_partials())
     double* partial_max; // [pstride] block max of |e|^2
     unsigned long long cond_handle;   // cudaGraphConditionalHandle (0: none)
     int pstride;

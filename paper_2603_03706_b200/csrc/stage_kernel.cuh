@@ -211,9 +211,16 @@ struct FinishArgs {
     unsigned long long* probe;
 #endif
 };
-__device__ __forceinline__ FinishArgs finish_args(const StageArgs& S) {
+// Block partial sums are double-buffered by stage parity: stage s writes buffer s & 1 and whoever finishes stage s
+// (the last block of kernel s, or every block of kernel s+1 in its prologue) reads that buffer.  A block of kernel
+// s+1 that starts late (SMs shared with other work) therefore never sees the stage-(s+1) sums another block of
+// the same kernel has already written.
+__device__ __forceinline__ double* stage_partials(const StageArgs& S, const int stage) {
+    return S.partial + (size_t)(stage & 1) * (size_t)kMaxSums * (size_t)S.pstride;
+}
+__device__ __forceinline__ FinishArgs finish_args(const StageArgs& S, const int stage) {
     FinishArgs F;
-    F.ctrl = S.ctrl; F.partial = S.partial; F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
+    F.ctrl = S.ctrl; F.partial = stage_partials(S, stage); F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
     F.inv_nc = S.inv_nc; F.pstride = S.pstride;
 #ifdef CAVMAG_PROBE
     F.probe = S.probe;
@@ -660,7 +667,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
 #pragma unroll
             for (int w = 0; w < nwarp; ++w) acc += swarp[w][i];
             const int comp = (i < 2 * NB) ? i : (2 * N + (i - 2 * NB));
-            A.partial[(size_t)comp * A.pstride + blockIdx.x] = acc;
+            stage_partials(A, STAGE)[(size_t)comp * A.pstride + blockIdx.x] = acc;
         }
     }
     if (STAGE == 7 && tid == 0) {
@@ -680,7 +687,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
         if (s_last) __threadfence();
     }
     __syncthreads();
-    if (s_last) stage_finish<STAGE>(finish_args(A), NSUB, N, trace);
+    if (s_last) stage_finish<STAGE>(finish_args(A, STAGE), NSUB, N, trace);
 }
 
 // Kernel lookup, one translation unit per (T, NSUB): returns the device function for

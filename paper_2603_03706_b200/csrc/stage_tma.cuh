@@ -59,6 +59,7 @@ struct TmaArgs {
     unsigned hbox_tx;              // bytes TMA writes for one halo box (expect_tx)
     unsigned aux_slot_bytes;       // bytes of one aux slot = n_aux*C * 2048
     unsigned ms_slot_bytes;        // n_halo_fields * hbox_bytes
+    int pre_k;                     // 1: k_2..k_{s-2} may be prefetched before the dependency wait (see plan_tma)
 };
 
 // ---- PTX wrappers ----------------------------------------------------------------------
@@ -154,7 +155,7 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
         const int idx = tidc + k * kTmaConsumers;
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
-    reduce_block_partials(A.partial, A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
+    reduce_block_partials(stage_partials(A, PREV), A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
 #pragma unroll
     for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
         const int idx = tidc + k * kTmaConsumers;
@@ -234,8 +235,14 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     // instructions are no-ops without a programmatic dependency.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // In stages 3..7 the producer reads its control words (written by the previous STEP's stage 7 / k_begin, not by
-    // kernel STAGE-1) and issues the first tiles of the mode profiles and of the aux streams y0, k1..k_{s-2} before the
-    // wait: DRAM is under-used while the previous kernel's slowest blocks finish, and this fill is ~10 % of a stage.
+    // kernel STAGE-1) and issues the first tiles of the mode profiles and of the aux streams y0, k1 [, k_2..k_{s-2}]
+    // before the wait: DRAM is under-used while the previous kernel's slowest blocks finish, and this fill is ~10 %
+    // of a stage.  u, y0 and k1 were written before this loop iteration started (the first kernel of the body has
+    // a full dependency), so they are always safe.  Programmatic edges are NOT transitive: kernel s may be
+    // launched while kernel s-2 (which writes k_{s-2}) is still running, unless a block of kernel s can only
+    // become resident on an SM that a block of kernel s-1 has left (which has passed its own wait).  The host
+    // sets TA.pre_k only when that holds: one CTA per SM (every stage's shared memory exceeds half an SM) and a
+    // grid of exactly n_sm blocks.  Otherwise k_2..k_{s-2} follow after the wait with k_{s-1}.
     constexpr bool kPre = STAGE >= 3;
 
     constexpr bool kDeferred = STAGE >= 3;      // this kernel first finishes stage STAGE-1 (see deferred_finish)
@@ -302,6 +309,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             int hm = 0, ha = 0, hu = 0;                 // ring heads
             unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
             int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
+            const int npre = (NAUX > 1) ? (TA.pre_k ? NAUX - 1 : (NAUX - 1 < 2 ? NAUX - 1 : 2)) : 0;   // aux fields fetched before the wait
             if constexpr (kPre) {
                 int zz = z0, txx = tx0, tyy = ty0;
                 for (int p = 0; p < nplanes; ++p) {
@@ -323,11 +331,11 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     if constexpr (NAUX > 1) {
                         if (do_a) {
                             const unsigned bar = full_aux + 8 * pre_a;
-                            mbar_expect_tx(bar, aux_tx);            // the whole slot; its last field follows after the wait
+                            mbar_expect_tx(bar, aux_tx);            // the whole slot; the other fields follow after the wait
                             unsigned dst = aux_ring + (unsigned)pre_a * aux_tx;
 #pragma unroll
                             for (int f = 0; f < NAUX - 1; ++f) {
-                                tma_load_4d(dst, amap[f], x0, y0, zz, 0, bar);
+                                if (f < npre) tma_load_4d(dst, amap[f], x0, y0, zz, 0, bar);
                                 dst += C * APLANE;
                             }
                             ++pre_a;
@@ -367,9 +375,11 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 if constexpr (NAUX > 0) {
                     const unsigned bar = full_aux + 8 * ha;
                     unsigned dst = aux_ring + (unsigned)ha * aux_tx;
-                    if (pre_a > 0) {                          // armed before the dependency wait: only k_{s-1} is missing
+                    if (pre_a > 0) {                          // armed before the dependency wait: k_{s-1} (and what npre left out) is missing
                         --pre_a;
-                        tma_load_4d(dst + (unsigned)((NAUX - 1) * C * APLANE), amap[NAUX - 1], x0, y0, z, 0, bar);
+#pragma unroll
+                        for (int f = 0; f < NAUX; ++f)
+                            if (f >= npre) tma_load_4d(dst + (unsigned)(f * C * APLANE), amap[f], x0, y0, z, 0, bar);
                     } else {
                         mbar_wait(empty_aux + 8 * ha, pa);
                         mbar_expect_tx(bar, aux_tx);
@@ -741,7 +751,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 #pragma unroll
                 for (int w = 0; w < kTmaTY; ++w) acc += swarp[w][i];
                 const int comp = (i < 2 * NB) ? i : (2 * N + (i - 2 * NB));
-                A.partial[(size_t)comp * A.pstride + blockIdx.x] = acc;
+                stage_partials(A, STAGE)[(size_t)comp * A.pstride + blockIdx.x] = acc;
             }
         }
         if (STAGE == 7 && tid == 0) {
@@ -768,7 +778,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             if (s_last) __threadfence();
         }
         __syncthreads();
-        if (s_last) stage_finish<STAGE>(finish_args(A), NSUB, N, trace);
+        if (s_last) stage_finish<STAGE>(finish_args(A, STAGE), NSUB, N, trace);
 #ifdef CAVMAG_PROBE
         __syncthreads();
         if (tid == 0) { CAVMAG_MARK(5); A.probe[((size_t)STAGE * gridDim.x + blockIdx.x) * 32 + 7] = (unsigned long long)s_last; }

@@ -62,6 +62,31 @@ def test_create_validates_arguments_before_touching_the_device(lib_path):
     assert e.value.status == api.CAV_E_ARG
 
 
+def test_binding_refuses_wrong_dtype_or_size(lib_path):
+    """The C ABI takes untyped pointers: the binding checks element type and count of every cell-field buffer
+    against the handle's precision and shape before the library touches it."""
+    import numpy as np
+    from paper_2603_03706_b200 import api
+    h = 0xDEAD                                   # no device needed: the check runs before the library call
+    api._HANDLES[h] = (np.float32, 2, 4 * 3 * 2, 1)
+    try:
+        ok = np.zeros((2, 3, 2, 3, 4), dtype=np.float32)
+        assert api._ptr(ok, *api._field_spec(h))[0] == ok.ctypes.data
+        with pytest.raises(ValueError, match="dtype"):
+            api.cav_set_m(h, ok.astype(np.float64))
+        with pytest.raises(ValueError, match="elements"):
+            api.cav_get_m(h, np.zeros((1, 3, 2, 3, 4), dtype=np.float32))
+        with pytest.raises(ValueError, match="elements"):
+            api.cav_set_modes(h, np.zeros((3, 2, 3, 4), dtype=np.float32), [1.0, 2.0], [0, 0], [0, 0])
+        with pytest.raises(ValueError, match="contiguous"):
+            api.cav_set_m(h, np.zeros((2, 3, 2, 3, 8), dtype=np.float32)[..., ::2])
+        import torch
+        with pytest.raises(ValueError, match="dtype"):
+            api.cav_get_dmdt(h, torch.zeros((2, 3, 2, 3, 4), dtype=torch.float64))
+    finally:
+        api._HANDLES.pop(h, None)
+
+
 def test_no_cpu_fallback_without_device(lib_path):
     """Without a CUDA device the product path fails loudly (CAV_E_UNSUPPORTED); it never
     routes through the oracle."""

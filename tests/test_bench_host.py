@@ -88,3 +88,15 @@ def test_reference_arm_prints_one_contract_line():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
     assert d["config"]["workload"] == "cfg2" and d["gpu_launches"] == 0
+
+
+def test_both_arms_describe_the_workload_with_the_same_config():
+    """`config` names the workload only, identically in the CUDA arm and the --impl reference arm; what differs between
+    the arms (kernel path, launch mode, the oracle's bounded sample) is reported under `impl_config`."""
+    w, prec = bench.make_workload("cfg2")
+    cfg = bench.config_of(w, prec, "cfg2", 1)
+    assert cfg["workload"] == "cfg2" and cfg["parallelism"] == "replicas x1 (no collective)"
+    for key in ("kernel_path", "launch_mode", "stage_overlap", "serpentine", "reference_sample"):
+        assert key not in cfg
+    r = bench.roofline_of("cfg3", *bench.make_workload("cfg3")[:1], "f32", 0.2344 * 20, 20)
+    assert r["bound"] == "hbm" and abs(r["algorithmic_bytes_per_launch"] - 106 * 2097152) < 1 and 0.5 < r["frac"] < 1.2

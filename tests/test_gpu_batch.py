@@ -207,3 +207,28 @@ def test_nonreciprocal_sweep(api):
         wr = copy.deepcopy(w); wr.B0 = tuple(B0[r])
         ref = oracle_of(wr, backward=back).run(wr.m0, wr.a0, fixed_dt=0.1e-12, max_steps=80)
         assert_parity(m[r], a[r], ref, "f64")
+
+
+@pytest.mark.parametrize("driven", [False, True])
+def test_forced_rejections_match_oracle_per_replica(api, driven):
+    """The controller's reject branch in the batch kernel: fp64, adaptive, dt_init = 2 ps on the 5 nm grid (ten times
+    the stability limit) so the first steps are rejected, plus a 0.15 ps pulse in mid-run; three field values in one
+    launch.  Accepted and rejected counts equal the oracle's for every replica, final state within 1e-10."""
+    from test_gpu_parity import _reject_case
+    w, dr = _reject_case(8, driven)
+    ghz = np.array([9.9, 10.0, 10.1])
+    B0 = np.array([[0.0, 0.0, W.b0_for_ghz(f)] for f in ghz])
+    t_end = 8e-12
+    with api.Batch(w, 3, precision="f64", B0=B0) as b:
+        if dr:
+            api.cav_batch_set_drive(b.h, dr["amp"], dr["t0"], dr["sigma"], dr["omega_d"])
+        b.run(t_end, tol=1e-8, dt_init=2e-12)
+        m, a, st = b.get_m(), b.get_a(), b.stats()
+    for r, f in enumerate(ghz):
+        wr = with_field(w, f)
+        ref = oracle_of(wr, drive=dr).run(wr.m0, wr.a0, t_end=t_end, tol=1e-8, dt_init=2e-12)
+        assert ref.rejected >= (8 if driven else 5)
+        assert (st[r]["accepted"], st[r]["rejected"]) == (ref.accepted, ref.rejected), r
+        assert st[r]["rhs_evals"] == ref.rhs_evals and st[r]["t"] == t_end
+        assert abs(st[r]["dt_next"] / ref.dt - 1) < 1e-9
+        assert_parity(m[r], a[r], ref, "f64")
