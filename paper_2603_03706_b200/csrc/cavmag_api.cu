@@ -32,7 +32,8 @@ struct cav_sim {
     double* partial = nullptr;
     double* partial_max = nullptr;
     int pstride = 0;
-    Ctrl* d_ctrl = nullptr;
+    Ctrl* d_ctrl = nullptr;      // canonical instance
+    Ctrl* d_ctrl0 = nullptr;     // step-boundary copy (cavmag_types.cuh)
     Ctrl* h_ctrl = nullptr;      // pinned mirror
     double* d_trace = nullptr;
     int trace_cap = 0;
@@ -104,11 +105,12 @@ __global__ void k_setrun(Ctrl* c, double t_end, double tol, double fixed_dt, dou
 
 // First node of the run graph: decides whether there is anything to do, fixes h for the first
 // step and the mode amplitudes / RF weights of the first kernel, arms the WHILE condition.
-__global__ void k_begin(Ctrl* c, unsigned long long handle) {
+__global__ void k_begin(Ctrl* c, Ctrl* c0, unsigned long long handle) {
     const int tid = threadIdx.x;
     if (tid == 0) {
         c->done = (!(c->t < c->t_end) || c->status != 0) ? 1 : 0;
         c->arrive = 0u;
+        c->pend7 = 0;
         prepare_h(c);
     }
     __syncthreads();
@@ -121,6 +123,11 @@ __global__ void k_begin(Ctrl* c, unsigned long long handle) {
         }
     }
     if (tid == 0 && handle != 0ull) cudaGraphSetConditional((cudaGraphConditionalHandle)handle, c->done ? 0u : 1u);
+    // the step-boundary copy the TMA stage-2 kernel starts from (cavmag_types.cuh)
+    __syncthreads();
+    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(c);
+    unsigned long long* dst = reinterpret_cast<unsigned long long*>(c0);
+    for (int i = tid; i < kCtrlWords; i += blockDim.x) dst[i] = src[i];
 }
 
 template <typename T>
@@ -285,7 +292,13 @@ int plan_tma(cav_sim* s) {
         CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(s->smem_optin - fa.sharedSizeBytes)));
     }
     const bool one_cta = smem_sm > 0 && s->tgrid == s->n_sm;
-    for (int stage = 1; stage <= 7; ++stage) s->targs[stage].pre_k = (one_cta && all_big) ? 1 : 0;
+    for (int stage = 1; stage <= 7; ++stage) {
+        s->targs[stage].pre_k = (one_cta && all_big) ? 1 : 0;
+        // Ctrl (buffer indices, done) is rewritten by block 0 of this step's stage-2 kernel: stage 3 reads it after
+        // its wait, later stages may read it earlier under the same one-CTA-per-SM argument
+        s->targs[stage].pre_ctrl = (one_cta && all_big && stage >= 4) ? 1 : 0;
+        s->targs[stage].N = s->N;
+    }
     s->tma_eligible = true;
     return CAV_OK;
 }
@@ -419,6 +432,7 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     StageArgs A;
     memset(&A, 0, sizeof(A));
     A.ctrl = s->d_ctrl;
+    A.ctrl0 = s->d_ctrl0;
     for (int i = 0; i < 2; ++i) { A.Y[i] = s->Y[i]; A.MS[i] = s->MS[i]; }
     for (int i = 0; i < 7; ++i) A.K[i] = s->K[i];
     A.u = s->u;
@@ -511,10 +525,11 @@ int build_graph_impl(cav_sim* s, bool pdl) {
     StageArgs A = make_args(s, h64);
     double* trace = s->d_trace;
     Ctrl* ctrl = s->d_ctrl;
+    Ctrl* ctrl0 = s->d_ctrl0;
 
     cudaGraphNode_t n_begin, n_k1, n_while;
     {
-        void* params[] = {&ctrl, &h64};
+        void* params[] = {&ctrl, &ctrl0, &h64};
         int rc = add_kernel(s, s->graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params, 0);
         if (rc) return rc;
     }
@@ -574,7 +589,7 @@ int run_stream_mode(cav_sim* s) {
     choose_grid(s);
     decide_path(s);
     StageArgs A = make_args(s, 0ull);
-    k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, 0ull);
+    k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
     CK(cudaGetLastError());
     int rc = launch_stage(s, 1, A);
     if (rc) return rc;
@@ -662,6 +677,8 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     CKC(cudaMalloc(&s->partial, sizeof(double) * 2 * (size_t)kMaxSums * s->pstride));      // two buffers: stage parity
     CKC(cudaMalloc(&s->partial_max, sizeof(double) * (size_t)s->pstride));
     CKC(cudaMalloc(&s->d_ctrl, sizeof(Ctrl)));
+    CKC(cudaMalloc(&s->d_ctrl0, sizeof(Ctrl)));
+    CKC(cudaMemset(s->d_ctrl0, 0, sizeof(Ctrl)));
     CKC(cudaMallocHost(&s->h_ctrl, sizeof(Ctrl)));
     CKC(cudaMallocHost(&s->h_flag, sizeof(int)));
     CKC(cudaMalloc(&s->d_maps, 128 * MAP_COUNT));
@@ -697,6 +714,7 @@ int cav_destroy(cav_sim* s) {
     cudaFree(s->partial);
     cudaFree(s->partial_max);
     cudaFree(s->d_ctrl);
+    cudaFree(s->d_ctrl0);
     cudaFree(s->d_trace);
     cudaFree(s->d_maps);
     cudaFree(s->d_blk);
@@ -947,7 +965,7 @@ static int ensure_k1(cav_sim* s) {
         choose_grid(s);
         decide_path(s);
         StageArgs A = make_args(s, 0ull);
-        k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, 0ull);
+        k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
         CK(cudaGetLastError());
         s->host_launches++;
         rc = launch_stage(s, 1, A);

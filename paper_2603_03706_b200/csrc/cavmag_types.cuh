@@ -28,8 +28,11 @@ constexpr int kMaxBlocks = 16384;      // upper bound on stage-kernel grid size 
      125.0 / 192.0 - 393.0 / 640.0, -2187.0 / 6784.0 + 92097.0 / 339200.0,               \
      11.0 / 84.0 - 187.0 / 2100.0, -1.0 / 40.0}
 
-// Controller + mode state, one instance in device memory per simulation.  Written only by
-// single-block code (k_begin, the last-arriving block of a stage kernel); read by every block.
+// Controller + mode state.  Two instances in device memory per simulation: the canonical one (StageArgs::ctrl,
+// the one the host pulls and pushes) and a step-boundary copy (StageArgs::ctrl0).  Written only by single-block code
+// (k_begin, the last-arriving block of a stage kernel, block 0 of a TMA stage kernel's prologue); read by every block.
+// A kernel whose block 0 rewrites fields that the other blocks of the SAME kernel still have to read (the step
+// controller in the prologue of the TMA stage-2 kernel) reads one instance and writes the other.
 struct Ctrl {
     // ---- run control ----
     double t, t_end, dt, h, tol, fixed_dt, target;
@@ -64,12 +67,15 @@ struct Ctrl {
     long long trace_stride, trace_acc0;
     // ---- last-block-done counter ----
     unsigned int arrive;
-    unsigned int pad;
+    int pend7;      // TMA path: stage 7 of the step in flight is still to be finished (mode ODE, error norm, controller) by
+                    // the prologue of the next stage-2 kernel
 };
 
 // Arguments of every stage kernel (by value; fixed for the lifetime of a CUDA graph).
 struct StageArgs {
-    Ctrl* ctrl;
+    Ctrl* ctrl;          // canonical instance
+    Ctrl* ctrl0;         // step-boundary copy: written by block 0 of the TMA stage-7 kernel (and k_begin / stage 1), read by
+                         // every block of the TMA stage-2 kernel, whose block 0 writes the new state to `ctrl`
     void* Y[2];          // state ping-pong
     void* MS[2];         // materialised stage states (MS[0] doubles as the partial-error field)
     void* K[7];          // slope fields

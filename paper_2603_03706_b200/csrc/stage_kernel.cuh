@@ -177,6 +177,75 @@ __device__ __forceinline__ void reduce_block_partials(const double* partial, con
     }
 }
 
+// max over the blocks' error maxima (one warp; the max is order-independent)
+__device__ __forceinline__ double reduce_block_max(const double* partial_max, const int nblk, const int lane) {
+    double mx = 0.0;
+    for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
+        double v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v[j] = (b0 + 32 * j < nblk) ? __ldcg(partial_max + b0 + 32 * j) : 0.0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) mx = fmax(mx, v[j]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    return mx;
+}
+
+__device__ __forceinline__ double fifth_root(double r);
+
+// The step controller (a7), one thread, on a Ctrl in shared memory: error norm = max(cells, modes), accept / reject,
+// dt proposal fac = clamp(0.8 (tol/err)^(1/5), 0.5, 2), time, FSAL buffer rotation, statistics, trace sampling.
+// smax = max_r |e(r)|^2, serr[n] = |e_a,n|, sred[2N + i] = sum_r m_s,i(r) of the candidate.  `trace` is the device
+// trace buffer (nullptr: none); rows are stored only when write_rows (every caller counts them).  Returns accept.
+__device__ __forceinline__ int controller_step(Ctrl* c, const double smax, const double* serr, const double* sred, const int N,
+                                               const int nsub, const double inv_nc, double* trace, const bool write_rows) {
+    double err = sqrt(smax);
+    for (int n = 0; n < N; ++n) err = fmax(err, serr[n]);
+    const bool finite = err < CUDART_INF;
+    const double h = c->h;
+    bool accept;
+    if (c->adaptive) accept = finite && err <= c->tol;
+    else { accept = true; if (!finite) { accept = false; c->status = -5; } }
+    double fac;
+    if (!finite) fac = 0.5;
+    else if (err == 0.0) fac = 2.0;
+    else { fac = 0.8 * fifth_root(fmin(fmax(c->tol / err, 1e-2), 1e3)); fac = fmin(fmax(fac, 0.5), 2.0); }
+    c->rhs_evals++;
+    c->steps_run++;
+    c->last_err = err;
+    if (accept) {
+        c->t = c->clamped ? c->target : c->t + h;
+        c->ycur ^= 1;
+        c->k1slot = 6 - c->k1slot;
+        c->accepted++;
+        c->dt_min = fmin(c->dt_min, h);
+        c->dt_max = fmax(c->dt_max, h);
+        if (c->adaptive) { const double prop = h * fac; c->dt = c->clamped ? fmax(prop, c->dt) : prop; }
+        for (int i = 0; i < 3 * nsub; ++i) c->mavg[i] = sred[2 * N + i] * inv_nc;
+        const bool take = trace != nullptr && c->sample_dt > 0.0 && c->trace_n < c->trace_cap &&
+                          (c->adaptive ? (c->clamped && c->sample_hit)
+                                       : ((c->accepted - c->trace_acc0) % c->trace_stride == 0));
+        if (take) {
+            if (write_rows) {
+                double* row = trace + (size_t)c->trace_n * (1 + 4 * N + 3 * nsub);
+                row[0] = c->t;
+                for (int n = 0; n < N; ++n) {
+                    row[1 + 2 * n] = c->anew[n][0]; row[2 + 2 * n] = c->anew[n][1];
+                    row[1 + 2 * N + 2 * n] = c->S[n][0]; row[2 + 2 * N + 2 * n] = c->S[n][1];
+                }
+                for (int i = 0; i < 3 * nsub; ++i) row[1 + 4 * N + i] = c->mavg[i];
+            }
+            c->trace_n++;
+        }
+    } else if (c->status == 0) {
+        c->rejected++;
+        c->dt = h * fac;
+    }
+    if (c->adaptive && !(c->dt > 1e-20)) c->status = -6;
+    return accept ? 1 : 0;
+}
+
 // ---------------------------------------------------------------------------------------
 // Tail of every stage kernel, executed by the last block to arrive: deterministic second
 // reduction pass, mode ODEs + stage algebra, and (stage 7) the accept/reject controller.
@@ -202,6 +271,7 @@ __device__ __forceinline__ double fifth_root(double r) {
 // and cost one more dependent memory round trip before the first load can issue).
 struct FinishArgs {
     Ctrl* ctrl;
+    Ctrl* ctrl0;             // step-boundary copy (nullptr: none), kept equal to ctrl by every single-block finish
     const double* partial;
     const double* partial_max;
     unsigned long long cond_handle;
@@ -220,7 +290,7 @@ __device__ __forceinline__ double* stage_partials(const StageArgs& S, const int 
 }
 __device__ __forceinline__ FinishArgs finish_args(const StageArgs& S, const int stage) {
     FinishArgs F;
-    F.ctrl = S.ctrl; F.partial = stage_partials(S, stage); F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
+    F.ctrl = S.ctrl; F.ctrl0 = S.ctrl0; F.partial = stage_partials(S, stage); F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
     F.inv_nc = S.inv_nc; F.pstride = S.pstride;
 #ifdef CAVMAG_PROBE
     F.probe = S.probe;
@@ -252,16 +322,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
     }
     reduce_block_partials(A.partial, A.pstride, nsum, nblk, warp, nwarp, lane, sred);
     if (stage == 7 && warp == nwarp - 1) {
-        double mx = 0.0;
-        for (int b0 = lane; b0 < nblk; b0 += 32 * 8) {
-            double v[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) v[j] = (b0 + 32 * j < nblk) ? __ldcg(A.partial_max + b0 + 32 * j) : 0.0;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) mx = fmax(mx, v[j]);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        const double mx = reduce_block_max(A.partial_max, nblk, lane);
         if (lane == 0) smax = mx;
     }
 #pragma unroll
@@ -279,50 +340,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
     } else {
         __syncthreads();
         if (stage == 7) {
-            if (tid == 0) {
-                double err = sqrt(smax);
-                for (int n = 0; n < N; ++n) err = fmax(err, serr[n]);
-                const bool finite = err < CUDART_INF;
-                const double h = c->h;
-                bool accept;
-                if (c->adaptive) accept = finite && err <= c->tol;
-                else { accept = true; if (!finite) { accept = false; c->status = -5; } }
-                double fac;
-                if (!finite) fac = 0.5;
-                else if (err == 0.0) fac = 2.0;
-                else { fac = 0.8 * fifth_root(fmin(fmax(c->tol / err, 1e-2), 1e3)); fac = fmin(fmax(fac, 0.5), 2.0); }
-                c->rhs_evals++;
-                c->steps_run++;
-                c->last_err = err;
-                if (accept) {
-                    c->t = c->clamped ? c->target : c->t + h;
-                    c->ycur ^= 1;
-                    c->k1slot = 6 - c->k1slot;
-                    c->accepted++;
-                    c->dt_min = fmin(c->dt_min, h);
-                    c->dt_max = fmax(c->dt_max, h);
-                    if (c->adaptive) { const double prop = h * fac; c->dt = c->clamped ? fmax(prop, c->dt) : prop; }
-                    for (int i = 0; i < 3 * nsub; ++i) c->mavg[i] = sred[2 * N + i] * A.inv_nc;
-                    const bool take = trace != nullptr && c->sample_dt > 0.0 && c->trace_n < c->trace_cap &&
-                                      (c->adaptive ? (c->clamped && c->sample_hit)
-                                                   : ((c->accepted - c->trace_acc0) % c->trace_stride == 0));
-                    if (take) {
-                        double* row = trace + (size_t)c->trace_n * (1 + 4 * N + 3 * nsub);
-                        row[0] = c->t;
-                        for (int n = 0; n < N; ++n) {
-                            row[1 + 2 * n] = c->anew[n][0]; row[2 + 2 * n] = c->anew[n][1];
-                            row[1 + 2 * N + 2 * n] = c->S[n][0]; row[2 + 2 * N + 2 * n] = c->S[n][1];
-                        }
-                        for (int i = 0; i < 3 * nsub; ++i) row[1 + 4 * N + i] = c->mavg[i];
-                        c->trace_n++;
-                    }
-                } else if (c->status == 0) {
-                    c->rejected++;
-                    c->dt = h * fac;
-                }
-                if (c->adaptive && !(c->dt > 1e-20)) c->status = -6;
-                s_accept = accept ? 1 : 0;
-            }
+            if (tid == 0) s_accept = controller_step(c, smax, serr, sred, N, nsub, A.inv_nc, trace, true);
             __syncthreads();
             if (tid < N && s_accept) {     // y := y_new (modes), FSAL: ka_1 := ka_7
                 c->a[tid][0] = c->anew[tid][0]; c->a[tid][1] = c->anew[tid][1];
@@ -341,12 +359,16 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
         }
         __syncthreads();
         if (tid < N) mode_stage_state<1>(c, tid);           // a_2 = a_0 + h a21 ka_1
-        if (tid == 0) { c->arrive = 0u; set_cond = (A.cond_handle != 0ull && stage == 7); }
+        if (tid == 0) { c->arrive = 0u; c->pend7 = 0; set_cond = (A.cond_handle != 0ull && stage == 7); }
     }
     // write the working copy back
     __syncthreads();
     CAVMAG_MARKF(10);
     for (int idx = tid; idx < kCtrlWords; idx += nthr) gcw[idx] = sc_words[idx];
+    if (A.ctrl0 != nullptr && (stage == 1 || stage == 7)) {      // the TMA stage-2 kernel starts from the boundary copy
+        unsigned long long* const g0 = reinterpret_cast<unsigned long long*>(A.ctrl0);
+        for (int idx = tid; idx < kCtrlWords; idx += nthr) g0[idx] = sc_words[idx];
+    }
     CAVMAG_MARKF(11);
     if (set_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, c->done ? 0u : 1u);
     CAVMAG_MARKF(12);

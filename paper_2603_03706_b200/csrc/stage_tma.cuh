@@ -60,6 +60,8 @@ struct TmaArgs {
     unsigned aux_slot_bytes;       // bytes of one aux slot = n_aux*C * 2048
     unsigned ms_slot_bytes;        // n_halo_fields * hbox_bytes
     int pre_k;                     // 1: k_2..k_{s-2} may be prefetched before the dependency wait (see plan_tma)
+    int pre_ctrl;                  // 1: the producer may read Ctrl (written by the stage-2 kernel of this step) before the wait
+    int N;                         // number of modes (layout of the stage-7 partial sums: 2N overlaps, then 3 n_sub <m>)
 };
 
 // ---- PTX wrappers ----------------------------------------------------------------------
@@ -155,7 +157,8 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
         const int idx = tidc + k * kTmaConsumers;
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
-    reduce_block_partials(stage_partials(A, PREV), A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
+    if constexpr (NB > 0)
+        reduce_block_partials(stage_partials(A, PREV), A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
 #pragma unroll
     for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
         const int idx = tidc + k * kTmaConsumers;
@@ -169,20 +172,110 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
     if (tidc == 0) probe_mark(A, PREV + 1, 10);         // all consumers' shares are in shared memory
 #endif
     Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
-    if (c->done) return false;                      // launched after the run ended (host-enqueued mode): nothing to do
-    if (tidc < c->N) {
-        const int n = tidc;
-        mode_ode_stage<PREV>(c, n, sred, nullptr);
-        if (blockIdx.x == 0) {
-            constexpr int nxt = (PREV + 1) & 1;
-            gctrl->S[n][0] = c->S[n][0]; gctrl->S[n][1] = c->S[n][1];
-            gctrl->ka[PREV - 1][n][0] = c->ka[PREV - 1][n][0]; gctrl->ka[PREV - 1][n][1] = c->ka[PREV - 1][n][1];
-            gctrl->as[nxt][n][0] = c->as[nxt][n][0]; gctrl->as[nxt][n][1] = c->as[nxt][n][1];
-            gctrl->c[n] = c->c[n];
-            if constexpr (PREV == 6) { gctrl->anew[n][0] = c->anew[n][0]; gctrl->anew[n][1] = c->anew[n][1]; }
+    const bool live = c->done == 0;                 // done: launched after the run ended (the rest of the last loop iteration, or
+                                                    // host-enqueued mode): nothing to finish
+    if (live) {
+        if (tidc < c->N) {
+            const int n = tidc;
+            mode_ode_stage<PREV>(c, n, sred, nullptr);
+            if (blockIdx.x == 0) {
+                constexpr int nxt = (PREV + 1) & 1;
+                gctrl->S[n][0] = c->S[n][0]; gctrl->S[n][1] = c->S[n][1];
+                gctrl->ka[PREV - 1][n][0] = c->ka[PREV - 1][n][0]; gctrl->ka[PREV - 1][n][1] = c->ka[PREV - 1][n][1];
+                gctrl->as[nxt][n][0] = c->as[nxt][n][0]; gctrl->as[nxt][n][1] = c->as[nxt][n][1];
+                gctrl->c[n] = c->c[n];
+                if constexpr (PREV == 6) { gctrl->anew[n][0] = c->anew[n][0]; gctrl->anew[n][1] = c->anew[n][1]; }
+            }
+        }
+        if (tidc == 0) {
+            c->rhs_evals++;                             // evaluation PREV is complete
+            if (blockIdx.x == 0) gctrl->rhs_evals = c->rhs_evals;
         }
     }
-    return true;
+    if constexpr (PREV == 6) {
+        // The stage-7 kernel hands the step over to the next stage-2 kernel through the boundary copy: block 0 stores
+        // its whole working copy there (also when the run is over, so that both instances end up equal).  No block of
+        // THIS kernel reads ctrl0, and the stage-2 kernel starts after this one has completed.
+        if (blockIdx.x == 0) {
+            asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+            unsigned long long* const g0 = reinterpret_cast<unsigned long long*>(A.ctrl0);
+            for (int idx = tidc; idx < kCtrlWords; idx += kTmaConsumers) g0[idx] = sc_words[idx];
+        }
+    }
+    return live;
+}
+
+// Deferred finish of stage 7 AND the step controller, run by the consumer warps of every block of the stage-2 kernel of
+// the next loop iteration (all blocks compute the same bits from the same inputs).  It replaces the "last block to
+// arrive" tail of the stage-7 kernel - a ticket, the second reduction pass, the controller and the graph condition
+// on ONE block with 147 SMs idle, ~10 us of every step on cfg3 - by a prologue that every block runs at once.
+//   reads : the boundary copy ctrl0 (written by block 0 of the stage-7 kernel, by k_begin or by stage 1), the stage-7
+//           block partials (2N overlap sums of m_new, 3 n_sub sums for <m>) and the blocks' error maxima
+//   does  : ka_7 and the mode error (Eq. 12 at the candidate), err = max(cells, modes), accept / reject, dt, t, buffer
+//           rotation, trace row, done, h of the step that starts now, a_2 and its RF weights
+//   writes: block 0 stores the whole new state to the canonical instance `ctrl` (never read by a block of this kernel),
+//           the trace row, and the WHILE condition of the run graph.  The condition lags by one iteration: the loop
+//           body that finds `done` is empty from here on (every later kernel of it returns at once).
+// The producer warp learns buffer indices and `done` from the shared copy through named barrier 2 (bar.arrive here,
+// bar.sync there).  Returns false when the run is over.
+template <int NB, int NSUB>
+__device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaArgs& TA, const int tidc,
+                                                 unsigned long long* sc_words, double* sred, double* serr, double* trace) {
+    const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(A.ctrl0);
+    unsigned long long cw[kCtrlWordsPerConsumer];
+#pragma unroll
+    for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
+        const int idx = tidc + k * kTmaConsumers;
+        cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
+    }
+    const int N = TA.N, warp = tidc >> 5, lane = tidc & 31;
+    const int nsum = 2 * N + 3 * NSUB;
+    // warps 0..6 sum the partials, warp 7 takes the error maxima (stale values when no stage 7 is pending: not used)
+    if (warp < kTmaTY - 1) reduce_block_partials(stage_partials(A, 7), A.pstride, nsum, (int)gridDim.x, warp, kTmaTY - 1, lane, sred);
+    else {
+        const double mx = reduce_block_max(A.partial_max, (int)gridDim.x, lane);
+        if (lane == 0) serr[kMaxModes] = mx;
+    }
+#pragma unroll
+    for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
+        const int idx = tidc + k * kTmaConsumers;
+        if (idx < kCtrlWords) sc_words[idx] = cw[k];
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+    Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
+    const bool write = blockIdx.x == 0;
+    if (c->done == 0 && c->pend7 != 0) {            // uniform over the block (and over the grid)
+        if (tidc < N) mode_ode_stage<7>(c, tidc, sred, serr);
+        asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+        if (tidc == 0) {
+            const int accept = controller_step(c, serr[kMaxModes], serr, sred, N, NSUB, A.inv_nc, trace, write);
+            serr[kMaxModes + 1] = (double)accept;
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+        if (tidc < N && serr[kMaxModes + 1] != 0.0) {     // y := y_new (modes), FSAL: ka_1 := ka_7
+            c->a[tidc][0] = c->anew[tidc][0]; c->a[tidc][1] = c->anew[tidc][1];
+            c->ka[0][tidc][0] = c->ka[6][tidc][0]; c->ka[0][tidc][1] = c->ka[6][tidc][1];
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+        if (tidc == 0) {                                  // start of the next step
+            const bool done = !(c->t < c->t_end) || (c->max_steps > 0 && c->steps_run >= c->max_steps) || c->status != 0;
+            c->done = done ? 1 : 0;
+            prepare_h(c);
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+        if (tidc < N) mode_stage_state<1>(c, tidc);       // a_2 = a_0 + h a21 ka_1
+    }
+    if (tidc == 0) c->pend7 = c->done ? 0 : 1;            // a step starts now: its stage 7 will be pending
+    asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+    asm volatile("bar.arrive 2, %0;" ::"n"(kTmaThreads) : "memory");      // the producer warp may read the shared copy
+    const bool live = c->done == 0;
+    if (write) {
+        unsigned long long* const g1 = reinterpret_cast<unsigned long long*>(A.ctrl);
+        for (int idx = tidc; idx < kCtrlWords; idx += kTmaConsumers) g1[idx] = sc_words[idx];
+        if (tidc == 0 && A.cond_handle != 0ull)
+            cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, live ? 1u : 0u);
+    }
+    return live;
 }
 
 template <typename T, int STAGE, int NSUB, int NB>
@@ -234,20 +327,24 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     // producer lane after it has prefetched what the previous kernel does NOT write (kPre below).  Both
     // instructions are no-ops without a programmatic dependency.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    // In stages 3..7 the producer reads its control words (written by the previous STEP's stage 7 / k_begin, not by
-    // kernel STAGE-1) and issues the first tiles of the mode profiles and of the aux streams y0, k1 [, k_2..k_{s-2}]
-    // before the wait: DRAM is under-used while the previous kernel's slowest blocks finish, and this fill is ~10 %
-    // of a stage.  u, y0 and k1 were written before this loop iteration started (the first kernel of the body has
-    // a full dependency), so they are always safe.  Programmatic edges are NOT transitive: kernel s may be
-    // launched while kernel s-2 (which writes k_{s-2}) is still running, unless a block of kernel s can only
-    // become resident on an SM that a block of kernel s-1 has left (which has passed its own wait).  The host
-    // sets TA.pre_k only when that holds: one CTA per SM (every stage's shared memory exceeds half an SM) and a
-    // grid of exactly n_sm blocks.  Otherwise k_2..k_{s-2} follow after the wait with k_{s-1}.
-    constexpr bool kPre = STAGE >= 3;
+    // What the producer lane may issue BEFORE the dependency wait (DRAM is under-used while the previous kernel's
+    // slowest blocks finish, and this fill is ~10 % of a stage):
+    //   * the mode profiles u: never written, always safe, in every stage >= 2;
+    //   * the aux streams y0, k1 (written before this loop iteration started) - but WHICH buffers they are (ycur,
+    //     k1slot) and whether the run is over is decided by the controller in the prologue of this step's stage-2
+    //     kernel, so the producer must first read Ctrl; and k_2..k_{s-2}, written by kernel s-2.
+    // Programmatic edges are NOT transitive: kernel s may be launched while kernel s-2 is still running, unless a block
+    // of kernel s can only become resident on an SM that a block of kernel s-1 has left (which has passed its own
+    // wait, so kernel s-2 has completed).  The host sets TA.pre_ctrl (stages >= 4: Ctrl as written by this step's
+    // stage-2 kernel) and TA.pre_k only when that holds: one CTA per SM (every stage's shared memory exceeds half an
+    // SM) and a grid of exactly n_sm blocks.  Otherwise only u is fetched early and everything else follows the wait.
+    constexpr bool kPre = STAGE >= 2;
 
-    constexpr bool kDeferred = STAGE >= 3;      // this kernel first finishes stage STAGE-1 (see deferred_finish)
-    __shared__ __align__(16) unsigned long long s_ctrl[kDeferred && NB > 0 ? kCtrlWords : 1];
-    __shared__ double s_red[kDeferred && NB > 0 ? 2 * NB : 1];
+    constexpr bool kDeferred = STAGE >= 2;      // this kernel first finishes the previous stage (deferred_finish / deferred_finish7)
+    constexpr int NRED = STAGE == 2 ? 2 * NB + 3 * NSUB : (NB > 0 ? 2 * NB : 1);
+    __shared__ __align__(16) unsigned long long s_ctrl[kDeferred ? kCtrlWords : 1];
+    __shared__ double s_red[kDeferred ? NRED : 1];
+    __shared__ double s_err[STAGE == 2 ? kMaxModes + 2 : 1];      // stage 2: mode errors, max |e|^2, accept flag
 
     // this CTA's run of plane-tiles; tile coordinates are advanced incrementally (no divisions in the loops)
     const long long q0 = (TA.Q * (long long)blockIdx.x) / gridDim.x;
@@ -275,21 +372,30 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 
     if (warp == kTmaTY) {
         // =============================== TMA producer ===============================
-        if constexpr (!kPre) asm volatile("griddepcontrol.wait;" ::: "memory");
-        {
-            const int done = STAGE == 1 ? ctrl->k1_valid : ctrl->done;
-            N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
-            if (done) return;
+        int done = 0;
+        bool have_ctrl = false;
+        if constexpr (STAGE == 1) {
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+            done = ctrl->k1_valid; N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
+            have_ctrl = true;
+        } else if constexpr (STAGE >= 3) {
+            if (TA.pre_ctrl) {
+                done = ctrl->done; N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
+                have_ctrl = true;
+            }
         }
-        if (kPre && !(lane == 0 && nplanes > 0)) asm volatile("griddepcontrol.wait;" ::: "memory");
-        if (lane == 0 && nplanes > 0) {
-            const unsigned char* maps = TA.maps;
-            auto mp = [&](int i) { return (const void*)(maps + 128 * i); };
-            const void* hmap0 = STAGE == 1 ? mp(MAP_H_Y0 + ycur) : STAGE == 2 ? mp(MAP_H_Y0 + ycur)
-                               : STAGE == 7 ? mp(MAP_H_Y0 + (1 - ycur))
-                               : (STAGE == 3 || STAGE == 5) ? mp(MAP_H_MS0) : mp(MAP_H_MS1);
-            const void* hmap1 = mp(k1slot == 0 ? MAP_H_K0 : MAP_H_K6);     // STAGE 2 only
-            const void* amap[5];
+        if (have_ctrl && done) return;
+        const bool issuer = lane == 0 && nplanes > 0;
+        const unsigned char* maps = TA.maps;
+        auto mp = [&](int i) { return (const void*)(maps + 128 * i); };
+        const void* hmap0 = nullptr;
+        const void* hmap1 = nullptr;                    // STAGE 2 only
+        const void* amap[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+        auto setup_maps = [&]() {                       // needs ycur, k1slot
+            hmap0 = STAGE == 1 ? mp(MAP_H_Y0 + ycur) : STAGE == 2 ? mp(MAP_H_Y0 + ycur)
+                    : STAGE == 7 ? mp(MAP_H_Y0 + (1 - ycur))
+                    : (STAGE == 3 || STAGE == 5) ? mp(MAP_H_MS0) : mp(MAP_H_MS1);
+            hmap1 = mp(k1slot == 0 ? MAP_H_K0 : MAP_H_K6);
             if constexpr (STAGE >= 3 && STAGE <= 6) {
                 amap[0] = mp(MAP_P_Y0 + ycur);
                 amap[1] = mp(k1slot == 0 ? MAP_P_K0 : MAP_P_K6);
@@ -301,20 +407,19 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             } else if constexpr (STAGE == 7) {
                 amap[0] = mp(MAP_P_MS0);      // e6
             }
-            const void* umap = mp(MAP_P_U);
-            constexpr unsigned aux_tx = (unsigned)(NAUX * C) * (unsigned)APLANE;
-            constexpr unsigned u_tx = (unsigned)UCB * (unsigned)APLANE;   // the full box is always counted (OOB modes zero-filled)
-
-            int z = z0, tx = tx0, ty = ty0;
-            int hm = 0, ha = 0, hu = 0;                 // ring heads
-            unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
-            int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
-            const int npre = (NAUX > 1) ? (TA.pre_k ? NAUX - 1 : (NAUX - 1 < 2 ? NAUX - 1 : 2)) : 0;   // aux fields fetched before the wait
-            if constexpr (kPre) {
+        };
+        if (have_ctrl) setup_maps();
+        const void* umap = mp(MAP_P_U);
+        constexpr unsigned aux_tx = (unsigned)(NAUX * C) * (unsigned)APLANE;
+        constexpr unsigned u_tx = (unsigned)UCB * (unsigned)APLANE;   // the full box is always counted (OOB modes zero-filled)
+        int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
+        const int npre = (NAUX > 1) ? (TA.pre_k ? NAUX - 1 : (NAUX - 1 < 2 ? NAUX - 1 : 2)) : 0;   // aux fields fetched before the wait
+        if constexpr (kPre) {
+            if (issuer) {
                 int zz = z0, txx = tx0, tyy = ty0;
                 for (int p = 0; p < nplanes; ++p) {
                     const bool do_u = NB > 0 && pre_u + NCH <= Du;
-                    const bool do_a = NAUX > 1 && pre_a < Da;
+                    const bool do_a = NAUX > 1 && have_ctrl && pre_a < Da;
                     if (!do_u && !do_a) break;
                     const int x0 = txx * TX, y0 = tyy * kTmaTY;
                     if constexpr (NB > 0) {
@@ -343,9 +448,30 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                     }
                     advance(zz, txx, tyy);
                 }
-                asm volatile("griddepcontrol.wait;" ::: "memory");
-                CAVMAG_MARK(13);
             }
+            __syncwarp();
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+            CAVMAG_MARK(13);
+            if constexpr (STAGE == 2) {
+                // the consumers have finished the previous step (deferred_finish7): verdict and buffer indices in s_ctrl
+                asm volatile("bar.sync 2, %0;" ::"n"(kTmaThreads) : "memory");
+                const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
+                done = sc->done; N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot;
+                setup_maps();
+            } else if (!have_ctrl) {
+                done = ctrl->done; N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
+                setup_maps();
+            }
+            if (done) {                             // the run is over: let the early profile loads land, then leave
+                if (issuer)
+                    for (int i = 0; i < pre_u; ++i) mbar_wait(full_u + 8 * i, 0u);
+                return;
+            }
+        }
+        if (issuer) {
+            int z = z0, tx = tx0, ty = ty0;
+            int hm = 0, ha = 0, hu = 0;                 // ring heads
+            unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
             auto issue_ms = [&](int x0, int y0, int zz) {
                 mbar_wait(empty_ms + 8 * hm, pm);
                 const unsigned bar = full_ms + 8 * hm;
@@ -400,22 +526,24 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         asm volatile("griddepcontrol.wait;" ::: "memory");
         if (tid == 0) CAVMAG_MARK(15);
         double hd;
-        if constexpr (kDeferred && NB > 0) {
+        if constexpr (STAGE == 2) {
+            // finish stage 7 of the previous step, run the controller, start this step (all blocks, same bits)
+            if (!deferred_finish7<NB, NSUB>(A, TA, tid, s_ctrl, s_red, s_err, trace)) return;
+            const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
+            N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot; hd = sc->h;
+            if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
+        } else if constexpr (kDeferred) {
             if (!deferred_finish<STAGE - 1, NB>(A, ctrl, tid, s_ctrl, s_red)) return;
             const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
             N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot; hd = sc->h;
-            if (tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
-            if (blockIdx.x == 0 && tid == 0) ctrl->rhs_evals = sc->rhs_evals + 1;
+            if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
         } else {
-            const int done = STAGE == 1 ? ctrl->k1_valid : ctrl->done;
+            const int done = ctrl->k1_valid;            // stage 1: k1 of a fresh state
             N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot; hd = ctrl->h;
             double cv = 0.0;
-            long long evals = 0;
             if (NB > 0 && tid < NB) cv = ctrl->c[tid];
-            if (kDeferred && blockIdx.x == 0 && tid == 0) evals = ctrl->rhs_evals;
             if (done) return;
             if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)cv : (T)0;
-            if (kDeferred && blockIdx.x == 0 && tid == 0) ctrl->rhs_evals = evals + 1;     // no modes: nothing else to finish
         }
         asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
         if (tid == 0) CAVMAG_MARK(1);
@@ -762,9 +890,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         }
     }
 
-    // ---- stages 1 and 7: last-block-done -> second reduction pass, mode ODE, controller.  Stages 2..6 end
-    //      here: their finish runs in the prologue of the next stage kernel (deferred_finish). ----
-    if constexpr (STAGE == 1 || STAGE == 7) {
+    // ---- stage 1 (k1 of a fresh state, once per run at most): last-block-done -> second reduction pass, mode ODE,
+    //      start of the first step.  Stages 2..7 end here: their finish runs in the prologue of the next stage
+    //      kernel (deferred_finish; stage 7 and the step controller: deferred_finish7 in the next stage-2 kernel). ----
+    if constexpr (STAGE == 1) {
         // One fence per block: the barrier orders every thread's stores before thread 0's gpu-scope fence
         // (release); the last block's thread 0 fences again after the ticket (acquire) before the barrier that
         // lets its threads read the other blocks' partials.

@@ -362,8 +362,10 @@ def test_forced_rejections_match_oracle(api, path, n, driven):
     assert (st["accepted"], st["rejected"]) == (ref.accepted, ref.rejected)
     assert st["rhs_evals"] == ref.rhs_evals == 1 + 6 * (ref.accepted + ref.rejected)
     assert st["t"] == t_end
-    assert abs(st["dt_min"] / ref.dt_min - 1) < 1e-9 and abs(st["dt_max"] / ref.dt_max - 1) < 1e-9
-    assert abs(st["dt_next"] / ref.dt - 1) < 1e-9
+    # dt = h * 0.8 (tol/err)^(1/5), and err = |h sum_j d_j k_j| is a difference of slopes that cancel to ~1e-7 of their
+    # size: rounding-order differences between the two implementations move err by ~1e-7 relative, dt by a fifth of that
+    assert abs(st["dt_min"] / ref.dt_min - 1) < 1e-6 and abs(st["dt_max"] / ref.dt_max - 1) < 1e-6
+    assert abs(st["dt_next"] / ref.dt - 1) < 1e-6
     assert_parity(m, a, ref, "f64")
 
 
