@@ -27,7 +27,7 @@ class _Problem(C.Structure):
                 ("renormalize", C.c_int), ("norm_sum_u", C.c_int), ("N", C.c_int),
                 ("u", _dp), ("omega", _dp), ("kappa", _dp), ("g", _dp), ("Gamma", _dp), ("Phi", _dp),
                 ("eta_amp", _dp), ("eta_t0", _dp), ("eta_sigma", _dp), ("eta_wd", _dp),
-                ("g_b", _dp), ("Gamma_b", _dp), ("Phi_b", _dp)]
+                ("g_b", _dp), ("Gamma_b", _dp), ("Phi_b", _dp), ("pol", _dp), ("quad", _dp)]
 
 
 class _Stats(C.Structure):
@@ -48,6 +48,11 @@ def lib():
         _lib.orc_run.argtypes = [C.POINTER(_Problem), _dp, _dp, _dp, C.c_double, C.c_double, C.c_double, _dp,
                                  C.c_longlong, C.c_double, _dp, C.c_int, C.POINTER(C.c_int), C.POINTER(_Stats)]
         _lib.orc_run.restype = C.c_int
+        _lib.orc_run_split.argtypes = [C.POINTER(_Problem), _dp, _dp, _dp, C.c_double, C.c_longlong, C.c_int,
+                                       C.c_longlong, _dp, C.c_int, C.POINTER(C.c_int)]
+        _lib.orc_run_split.restype = C.c_int
+        _lib.orc_dft.argtypes = [_dp, _dp, C.c_int, _dp, C.c_int, _dp]
+        _lib.orc_dft.restype = None
         _lib.orc_tableau.argtypes = [_dp, _dp, _dp, _dp]
         _lib.orc_set_threads.argtypes = [C.c_int]
         _lib.orc_get_threads.restype = C.c_int
@@ -82,7 +87,7 @@ class Oracle:
     or from keyword arguments with the same names."""
 
     def __init__(self, w=None, renormalize: bool = True, norm_sum_u: bool = False, drive: Optional[dict] = None,
-                 backward: Optional[dict] = None, **kw):
+                 backward: Optional[dict] = None, pol=None, quad=None, **kw):
         """drive = dict(amp [N] complex, t0 [N], sigma [N], omega_d [N] or None): the Gaussian-pulse drive
         eta_n(t) = amp_n exp(-(t-t0_n)^2/(2 sigma_n^2)) exp(-i omega_d,n (t-t0_n)) of Eq. 1 / Eq. 12."""
         get = (lambda k: kw[k] if k in kw else getattr(w, k))
@@ -119,6 +124,11 @@ class Oracle:
             self.Gamma_b = None if Gb is None else _c64(np.broadcast_to(np.asarray(Gb, dtype=np.float64), (self.N,)))
             self.Phi_b = None if Pb is None else _c64(np.broadcast_to(np.asarray(Pb, dtype=np.float64), (self.N,)))
             P.g_b, P.Gamma_b, P.Phi_b = _p(self.g_b), _p(self.Gamma_b), _p(self.Phi_b)
+        if pol is not None and self.N:
+            # per-mode polarisation p_n [N][3] (unit vectors) and optional quadrature axes q_n (default z^ x p_n)
+            self.pol = _c64(np.asarray(pol, dtype=np.float64).reshape(self.N, 3))
+            self.quad = None if quad is None else _c64(np.asarray(quad, dtype=np.float64).reshape(self.N, 3))
+            P.pol, P.quad = _p(self.pol), _p(self.quad)
         self.P = P
         self.nc = self.nx * self.ny * self.nz
         self.gamma = P.gamma
@@ -153,6 +163,33 @@ class Oracle:
                          accepted=st.accepted, rejected=st.rejected, rhs_evals=st.rhs_evals,
                          dt_min=st.dt_min, dt_max=st.dt_max, status=st.status,
                          trace=None if trace is None else trace[:ntr.value].copy())
+
+
+    # -- the paper's tier-2 operator-split loop (comparison integrator) ------------------
+    def run_split(self, m, a, dt: float, n_steps: int, n_llg: int = 1, t0: float = 0.0, sample_every: int = 0,
+                  trace_cap: int = 0) -> RunResult:
+        m = _c64(m).reshape(self.n_sub, 3, self.nz, self.ny, self.nx).copy()
+        a2 = np.zeros(max(2 * self.N, 1))
+        a2[:2 * self.N] = np.asarray(a, dtype=np.complex128).reshape(self.N).view(np.float64)
+        t = C.c_double(t0)
+        rowlen = 1 + 4 * self.N + 3 * self.n_sub
+        trace = np.zeros((max(trace_cap, 1), rowlen)) if (sample_every > 0 and trace_cap > 0) else None
+        ntr = C.c_int(0)
+        status = lib().orc_run_split(C.byref(self.P), _p(m), _p(a2), C.byref(t), float(dt), int(n_steps), int(n_llg),
+                                     int(sample_every), _p(trace), int(trace_cap), C.byref(ntr))
+        return RunResult(m=m, a=a2[:2 * self.N].view(np.complex128).copy(), t=t.value, dt=dt, accepted=int(n_steps),
+                         rejected=0, rhs_evals=6 * int(n_steps) * int(n_llg), dt_min=dt, dt_max=dt, status=status,
+                         trace=None if trace is None else trace[:ntr.value].copy())
+
+
+def dft(t, x, w) -> np.ndarray:
+    """Plain Fourier sum X(w_k) = sum_j x_j exp(+i w_k t_j) of a sampled complex trace (orc_dft)."""
+    t = _c64(t)
+    xx = _c64(np.asarray(x, dtype=np.complex128).reshape(-1).view(np.float64))
+    w = _c64(np.atleast_1d(w))
+    out = np.zeros(2 * w.size)
+    lib().orc_dft(_p(t), _p(xx), int(t.size), _p(w), int(w.size), _p(out))
+    return out.view(np.complex128).copy()
 
 
 def tableau():

@@ -21,6 +21,9 @@
 //    (4) c_n  = (2/gamma) Re[G_b,n a_n];  B_rf(r) = x^ sum_n c_n u_n(r)      (G_b = G unless a separate backward
 //        coupling is given: non-reciprocal g_f != g_b with h0 = 2 g_b/gamma)
 //                                                           PAPER.md:65 Eq.5, :121 Eq.13, :159
+//        Per-mode polarisation (the paper fixes x^): with a unit vector p_n and a
+//        quadrature axis q_n (default z^ x p_n) the mode couples to  m_c.p_n - i m_c.q_n  in (2) and its field
+//        points along p_n in (4).  p = x^, q = y^ is the paper's case (reading G32).
 //    (5) B_s  = B0 + (2A/Ms) sum_{d,+-} [m_s(r +- e_d) - m_s(r)]/D_d^2   (open boundary)
 //             + (2Ku/Ms)(m_s . k^) k^ + B_rf - B_E m_other
 //    (6) dm_s/dt = -gamma/(1+alpha^2) [ m x B + alpha m x (m x B) ]
@@ -32,6 +35,17 @@
 //  PARITY UNPINNED: the step-size controller constants (0.8, 1/5, [0.5,2]), the error-norm
 //  composition and the default initial step — the paper names "RK45 adaptive" only
 //  (PAPER.md:150); adaptive runs are compared on observables.
+//
+//  Second integrator, orc_run_split: the paper's TIER-2 operator-split loop (PAPER.md:169-193 Listing 1, :199),
+//  kept as a comparison scheme: per step dt, (i) read the overlaps S_n of the current m,
+//  (ii) advance a_n over dt by classic RK4 with S_n held constant, (iii) set the RF field from the NEW a_n and hold it
+//  constant, (iv) advance the LLG equation over dt.  Reading G33: step (iv) = n_llg Dormand-Prince 5(4) steps of dt/n_llg
+//  with the same per-cell renormalisation as the unified step (mumax+ runs its own adaptive solver there, unspecified).
+//  Pins: first-order convergence of the Rabi period to pi/g and the printed errors (Fig. 11).
+//
+//  orc_dft: the plain discrete Fourier sum X(w) = sum_j x_j exp(+i w t_j) of a sampled complex trace at arbitrary
+//  frequencies w (signals ~ exp(-i w t)) - the definition behind the paper's zero-padded FFT spectra
+//  |FFT(m^-)|^2 + |FFT(a)|^2.  Pinned against numpy.fft on the FFT grid.
 //
 //  Build:  g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC  (see oracle/build.py)
 // =====================================================================================
@@ -73,6 +87,9 @@ struct orc_problem {
     const double* g_b;       // [N] rad/s
     const double* Gamma_b;   // [N] rad/s (NULL: 0)
     const double* Phi_b;     // [N] rad   (NULL: 0)
+    // per-mode polarisation (reading G32): pol == NULL: every mode along x^ with quadrature y^
+    const double* pol;       // [N][3] unit vectors p_n: direction of the mode's RF field
+    const double* quad;      // [N][3] quadrature axes q_n (NULL: q_n = z^ x p_n): the mode couples to m.p_n - i m.q_n
 };
 
 struct orc_stats {
@@ -102,27 +119,44 @@ namespace {
 
 inline long long ncell(const orc_problem* P) { return (long long)P->nx * P->ny * P->nz; }
 
+// polarisation p_n and quadrature axis q_n of mode n (reading G32): x^, y^ unless given; q defaults to z^ x p
+void mode_axes(const orc_problem* P, int n, double* pv, double* qv) {
+    if (!P->pol) { pv[0] = 1.0; pv[1] = 0.0; pv[2] = 0.0; qv[0] = 0.0; qv[1] = 1.0; qv[2] = 0.0; return; }
+    for (int i = 0; i < 3; ++i) pv[i] = P->pol[3 * n + i];
+    if (P->quad) { for (int i = 0; i < 3; ++i) qv[i] = P->quad[3 * n + i]; }
+    else { qv[0] = -pv[1]; qv[1] = pv[0]; qv[2] = 0.0; }      // z^ x p
+}
+
 // ---- step (2): S_n = (1/W_n) sum_r u_n(r) (m_c,x(r) - i m_c,y(r)) ---------------------
 // Summed plane by plane in fixed z order so the result does not depend on the thread count.
 void overlaps(const orc_problem* P, const double* m, double* S /*[N][2]*/) {
     const long long nc = ncell(P), plane = (long long)P->nx * P->ny;
     for (int n = 0; n < P->N; ++n) {
         const double* un = P->u + (long long)n * nc;
+        double pv[3], qv[3];
+        mode_axes(P, n, pv, qv);
         std::vector<double> pre(P->nz), pim(P->nz), pw(P->nz);
 #pragma omp parallel for schedule(static)
         for (int z = 0; z < P->nz; ++z) {
             double sre = 0.0, sim = 0.0, sw = 0.0;
             for (long long i = (long long)z * plane; i < (long long)(z + 1) * plane; ++i) {
-                double mcx, mcy;
+                double mcx, mcy, mcz;
                 if (P->n_sub == 1) {
                     mcx = m[0 * nc + i];
                     mcy = m[1 * nc + i];
+                    mcz = m[2 * nc + i];
                 } else {  // step (1): net magnetisation couples
                     mcx = 0.5 * (m[0 * nc + i] + m[3 * nc + 0 * nc + i]);
                     mcy = 0.5 * (m[1 * nc + i] + m[3 * nc + 1 * nc + i]);
+                    mcz = 0.5 * (m[2 * nc + i] + m[3 * nc + 2 * nc + i]);
                 }
-                sre += un[i] * mcx;       // Re[u (mx - i my)] = u mx
-                sim += -(un[i] * mcy);    // Im[u (mx - i my)] = -u my
+                if (!P->pol) {
+                    sre += un[i] * mcx;       // Re[u (mx - i my)] = u mx
+                    sim += -(un[i] * mcy);    // Im[u (mx - i my)] = -u my
+                } else {                      // u (m.p - i m.q)
+                    sre += un[i] * (mcx * pv[0] + mcy * pv[1] + mcz * pv[2]);
+                    sim += -(un[i] * (mcx * qv[0] + mcy * qv[1] + mcz * qv[2]));
+                }
                 sw += un[i];
             }
             pre[z] = sre; pim[z] = sim; pw[z] = sw;
@@ -135,46 +169,54 @@ void overlaps(const orc_problem* P, const double* m, double* S /*[N][2]*/) {
     }
 }
 
-// ---- the coupled right-hand side f(t, m, a) ---------------------------------------------
-void rhs(const orc_problem* P, double t, const double* m, const double* a, double* dm, double* da, double* S_out) {
-    const int nx = P->nx, ny = P->ny, nz = P->nz, N = P->N;
-    const long long nc = ncell(P);
-    std::vector<double> S(2 * (size_t)(N > 0 ? N : 1));
-    overlaps(P, m, S.data());
-    if (S_out) std::memcpy(S_out, S.data(), sizeof(double) * 2 * N);
-
-    // steps (3) and (4)
-    std::vector<double> c((size_t)(N > 0 ? N : 1));
-    for (int n = 0; n < N; ++n) {
+// ---- steps (3), (4): mode slopes da_n/dt from given overlaps S, and the RF weights c_n = (2/gamma) Re[G_b,n a_n] ----
+void mode_rhs(const orc_problem* P, double t, const double* a, const double* S, double* da, double* c) {
+    for (int n = 0; n < P->N; ++n) {
         const double Gre = P->g[n] + P->Gamma[n] * std::cos(P->Phi[n]);
         const double Gim = P->Gamma[n] * std::sin(P->Phi[n]);
         const double are = a[2 * n], aim = a[2 * n + 1];
         const double Sre = S[2 * n], Sim = S[2 * n + 1];
         // -(i w + kappa) a  =  (-kappa are + w aim) + i (-kappa aim - w are)
         // i G S             =  (-(Gre Sim + Gim Sre)) + i (Gre Sre - Gim Sim)
-        da[2 * n + 0] = (-P->kappa[n] * are + P->omega[n] * aim) - (Gre * Sim + Gim * Sre);
-        da[2 * n + 1] = (-P->kappa[n] * aim - P->omega[n] * are) + (Gre * Sre - Gim * Sim);
-        double Gbre = Gre, Gbim = Gim;                        // backward coupling: reciprocal unless given
-        if (P->g_b) {
-            const double Gm = P->Gamma_b ? P->Gamma_b[n] : 0.0, Ph = P->Phi_b ? P->Phi_b[n] : 0.0;
-            Gbre = P->g_b[n] + Gm * std::cos(Ph);
-            Gbim = Gm * std::sin(Ph);
+        if (da) {
+            da[2 * n + 0] = (-P->kappa[n] * are + P->omega[n] * aim) - (Gre * Sim + Gim * Sre);
+            da[2 * n + 1] = (-P->kappa[n] * aim - P->omega[n] * are) + (Gre * Sre - Gim * Sim);
+            if (P->eta_amp) {   // + eta_n(t): Gaussian envelope times carrier e^{-i w_d (t - t0)}
+                const double x = t - P->eta_t0[n];
+                const double env = std::exp(-(x * x) / (2.0 * P->eta_sigma[n] * P->eta_sigma[n]));
+                const double ph = P->eta_wd ? P->eta_wd[n] * x : 0.0;
+                const double Are = P->eta_amp[2 * n], Aim = P->eta_amp[2 * n + 1];
+                da[2 * n + 0] += env * (Are * std::cos(ph) + Aim * std::sin(ph));
+                da[2 * n + 1] += env * (Aim * std::cos(ph) - Are * std::sin(ph));
+            }
         }
-        c[n] = (2.0 / P->gamma) * (Gbre * are - Gbim * aim);   // (2/gamma) Re[G_b a]
-        if (P->eta_amp) {   // + eta_n(t): Gaussian envelope times carrier e^{-i w_d (t - t0)}
-            const double x = t - P->eta_t0[n];
-            const double env = std::exp(-(x * x) / (2.0 * P->eta_sigma[n] * P->eta_sigma[n]));
-            const double ph = P->eta_wd ? P->eta_wd[n] * x : 0.0;
-            const double Are = P->eta_amp[2 * n], Aim = P->eta_amp[2 * n + 1];
-            da[2 * n + 0] += env * (Are * std::cos(ph) + Aim * std::sin(ph));
-            da[2 * n + 1] += env * (Aim * std::cos(ph) - Are * std::sin(ph));
+        if (c) {
+            double Gbre = Gre, Gbim = Gim;                        // backward coupling: reciprocal unless given
+            if (P->g_b) {
+                const double Gm = P->Gamma_b ? P->Gamma_b[n] : 0.0, Ph = P->Phi_b ? P->Phi_b[n] : 0.0;
+                Gbre = P->g_b[n] + Gm * std::cos(Ph);
+                Gbim = Gm * std::sin(Ph);
+            }
+            c[n] = (2.0 / P->gamma) * (Gbre * are - Gbim * aim);   // (2/gamma) Re[G_b a]
         }
     }
+}
 
+// ---- steps (5), (6): dm/dt of every cell for given RF weights c_n ----
+void llg_rhs(const orc_problem* P, const double* m, const double* c, double* dm) {
+    const int nx = P->nx, ny = P->ny, nz = P->nz, N = P->N;
+    const long long nc = ncell(P);
     const double pref_ex = 2.0 * P->Aex / P->Ms;
     const double pref_an = 2.0 * P->Ku / P->Ms;
     const double wx = 1.0 / (P->dx * P->dx), wy = 1.0 / (P->dy * P->dy), wz = 1.0 / (P->dz * P->dz);
     const double llg = -P->gamma / (1.0 + P->alpha * P->alpha);
+    std::vector<double> cp(3 * (size_t)(N > 0 ? N : 1));      // c_n p_n (general polarisation only)
+    if (P->pol)
+        for (int n = 0; n < N; ++n) {
+            double pv[3], qv[3];
+            mode_axes(P, n, pv, qv);
+            for (int i = 0; i < 3; ++i) cp[3 * n + i] = c[n] * pv[i];
+        }
 
     for (int s = 0; s < P->n_sub; ++s) {
         const double* ms = m + (long long)s * 3 * nc;
@@ -198,9 +240,18 @@ void rhs(const orc_problem* P, double t, const double* m, const double* a, doubl
                     Bx += pref_ex * lx; By += pref_ex * ly; Bz += pref_ex * lz;
                     const double mk = mx * P->axis[0] + my * P->axis[1] + mz * P->axis[2];
                     Bx += pref_an * mk * P->axis[0]; By += pref_an * mk * P->axis[1]; Bz += pref_an * mk * P->axis[2];
-                    double brf = 0.0;
-                    for (int n = 0; n < N; ++n) brf += c[n] * P->u[(long long)n * nc + i];
-                    Bx += brf;                       // RF field along x^
+                    if (!P->pol) {
+                        double brf = 0.0;
+                        for (int n = 0; n < N; ++n) brf += c[n] * P->u[(long long)n * nc + i];
+                        Bx += brf;                       // RF field along x^
+                    } else {                             // RF field sum_n c_n u_n(r) p_n (reading G32)
+                        double bx = 0.0, by = 0.0, bz = 0.0;
+                        for (int n = 0; n < N; ++n) {
+                            const double un = P->u[(long long)n * nc + i];
+                            bx += cp[3 * n] * un; by += cp[3 * n + 1] * un; bz += cp[3 * n + 2] * un;
+                        }
+                        Bx += bx; By += by; Bz += bz;
+                    }
                     if (mo) { Bx -= P->B_exch_inter * mo[i]; By -= P->B_exch_inter * mo[nc + i]; Bz -= P->B_exch_inter * mo[2 * nc + i]; }
                     // step (6): LLG in explicit Landau-Lifshitz form
                     const double tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;   // m x B
@@ -210,6 +261,17 @@ void rhs(const orc_problem* P, double t, const double* m, const double* a, doubl
                     ds[2 * nc + i] = llg * (tz + P->alpha * dz_);
                 }
     }
+}
+
+// ---- the coupled right-hand side f(t, m, a): every term at the same state (no operator splitting) ----
+void rhs(const orc_problem* P, double t, const double* m, const double* a, double* dm, double* da, double* S_out) {
+    const int N = P->N;
+    std::vector<double> S(2 * (size_t)(N > 0 ? N : 1));
+    overlaps(P, m, S.data());
+    if (S_out) std::memcpy(S_out, S.data(), sizeof(double) * 2 * N);
+    std::vector<double> c((size_t)(N > 0 ? N : 1));
+    mode_rhs(P, t, a, S.data(), da, c.data());
+    llg_rhs(P, m, c.data(), dm);
 }
 
 // Dormand-Prince 5(4) (Dormand & Prince 1980), textbook constants — the paper gives none (G11).
@@ -400,6 +462,112 @@ int orc_run(const orc_problem* P, double* m, double* a, double* t_io, double t_e
     s.dt_next = dt; s.t = t;
     if (st) *st = s;
     return s.status;
+}
+
+// ---- the paper's tier-2 operator-split loop as a comparison integrator (PAPER.md:169-193 Listing 1, :199) ----
+// n_steps steps of size dt from *t_io.  Per step:
+//   (i)   S_n = overlaps of the current m                               ("Read magnetization from GPU")
+//   (ii)  a_n <- classic RK4 over dt of da/dt = -(i w + kappa) a + i G S + eta(t) with S held constant
+//                                                                        ("Step cavity ODE (CPU, RK4)")
+//   (iii) c_n = (2/gamma) Re[G_b a_n] from the NEW amplitudes, held constant   ("H_rf = h0 * a.real", then bias field)
+//   (iv)  m <- n_llg Dormand-Prince 5(4) steps of dt/n_llg of the LLG equation in that constant RF field, each followed
+//         by the per-cell renormalisation of the unified step                  ("world.timesolver.run(dt)"; reading G33)
+// Trace rows as orc_run, one per step (sample_every steps), S = overlaps of the state the row belongs to.
+int orc_run_split(const orc_problem* P, double* m, double* a, double* t_io, double dt, long long n_steps, int n_llg,
+                  long long sample_every, double* trace, int trace_cap, int* n_trace) {
+    const long long nc = ncell(P), nm = (long long)P->n_sub * 3 * nc;
+    const int N = P->N, na = 2 * N;
+    if (n_llg < 1) n_llg = 1;
+    std::vector<double> S((size_t)(na > 0 ? na : 1)), c((size_t)(N > 0 ? N : 1));
+    std::vector<double> k1a(na > 0 ? na : 1), k2a(na > 0 ? na : 1), k3a(na > 0 ? na : 1), k4a(na > 0 ? na : 1), tmp(na > 0 ? na : 1);
+    std::vector<double> k[6], ys(nm);
+    for (auto& v : k) v.assign(nm, 0.0);
+    const int rowlen = 1 + 4 * N + 3 * P->n_sub;
+    int ntr = 0;
+    double t = *t_io;
+    for (long long step = 0; step < n_steps; ++step) {
+        overlaps(P, m, S.data());                                                     // (i)
+        // (ii) classic RK4, S frozen
+        mode_rhs(P, t, a, S.data(), k1a.data(), nullptr);
+        for (int i = 0; i < na; ++i) tmp[i] = a[i] + 0.5 * dt * k1a[i];
+        mode_rhs(P, t + 0.5 * dt, tmp.data(), S.data(), k2a.data(), nullptr);
+        for (int i = 0; i < na; ++i) tmp[i] = a[i] + 0.5 * dt * k2a[i];
+        mode_rhs(P, t + 0.5 * dt, tmp.data(), S.data(), k3a.data(), nullptr);
+        for (int i = 0; i < na; ++i) tmp[i] = a[i] + dt * k3a[i];
+        mode_rhs(P, t + dt, tmp.data(), S.data(), k4a.data(), nullptr);
+        for (int i = 0; i < na; ++i) a[i] = a[i] + (dt / 6.0) * (k1a[i] + 2.0 * k2a[i] + 2.0 * k3a[i] + k4a[i]);
+        mode_rhs(P, t + dt, a, S.data(), nullptr, c.data());                          // (iii)
+        // (iv) LLG over dt in the constant field
+        const double h = dt / (double)n_llg;
+        for (int sub = 0; sub < n_llg; ++sub) {
+            const double A[6][5] = {{0, 0, 0, 0, 0}, {A21, 0, 0, 0, 0}, {A31, A32, 0, 0, 0}, {A41, A42, A43, 0, 0},
+                                    {A51, A52, A53, A54, 0}, {A61, A62, A63, A64, A65}};
+            llg_rhs(P, m, c.data(), k[0].data());
+            for (int st = 1; st < 6; ++st) {
+#pragma omp parallel for schedule(static)
+                for (long long i = 0; i < nm; ++i) {
+                    double acc = 0.0;
+                    for (int j = 0; j < st; ++j) acc += A[st][j] * k[j][i];
+                    ys[i] = m[i] + h * acc;
+                }
+                llg_rhs(P, ys.data(), c.data(), k[st].data());
+            }
+            const double b[6] = {B1, 0.0, B3, B4, B5, B6};
+#pragma omp parallel for schedule(static)
+            for (long long i = 0; i < nm; ++i) {
+                double acc = 0.0;
+                for (int j = 0; j < 6; ++j) acc += b[j] * k[j][i];
+                m[i] = m[i] + h * acc;
+            }
+            if (P->renormalize) {
+                for (int s = 0; s < P->n_sub; ++s) {
+                    double* y = m + (long long)s * 3 * nc;
+#pragma omp parallel for schedule(static)
+                    for (long long i = 0; i < nc; ++i) {
+                        const double n2 = y[i] * y[i] + y[nc + i] * y[nc + i] + y[2 * nc + i] * y[2 * nc + i];
+                        const double inv = 1.0 / std::sqrt(n2);
+                        y[i] *= inv; y[nc + i] *= inv; y[2 * nc + i] *= inv;
+                    }
+                }
+            }
+        }
+        t = *t_io + (double)(step + 1) * dt;
+        if (trace && trace_cap > 0 && sample_every > 0 && (step + 1) % sample_every == 0 && ntr < trace_cap) {
+            overlaps(P, m, S.data());
+            double* row = trace + (long long)ntr * rowlen;
+            row[0] = t;
+            for (int i = 0; i < na; ++i) row[1 + i] = a[i];
+            for (int i = 0; i < na; ++i) row[1 + na + i] = S[i];
+            for (int sub = 0; sub < P->n_sub; ++sub)
+                for (int cidx = 0; cidx < 3; ++cidx) {
+                    const double* f = m + ((long long)sub * 3 + cidx) * nc;
+                    double acc = 0.0;
+                    for (long long i = 0; i < nc; ++i) acc += f[i];
+                    row[1 + 2 * na + 3 * sub + cidx] = acc / (double)nc;
+                }
+            ntr++;
+        }
+    }
+    *t_io = t;
+    if (n_trace) *n_trace = ntr;
+    for (long long i = 0; i < nm; ++i) if (!std::isfinite(m[i])) return 1;
+    return 0;
+}
+
+// ---- the plain discrete Fourier sum of a sampled complex trace ----
+// X[k] = sum_j x[j] exp(+i w[k] t[j]) for n samples (x as [n][2] = Re, Im) and nw angular frequencies w: a component
+// x ~ exp(-i w0 t) (the paper's sign convention) peaks at w = w0.  out is [nw][2].
+void orc_dft(const double* t, const double* x, int n, const double* w, int nw, double* out) {
+    for (int k = 0; k < nw; ++k) {
+        double re = 0.0, im = 0.0;
+        for (int j = 0; j < n; ++j) {
+            const double ph = w[k] * t[j];
+            const double cs = std::cos(ph), sn = std::sin(ph);
+            re += x[2 * j] * cs - x[2 * j + 1] * sn;
+            im += x[2 * j] * sn + x[2 * j + 1] * cs;
+        }
+        out[2 * k] = re; out[2 * k + 1] = im;
+    }
 }
 
 // The tableau, exposed so the tests can check its identities (row sums, sum b = 1, sum d = 0).

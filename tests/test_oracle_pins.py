@@ -660,3 +660,182 @@ def test_nonreciprocal_coupling_geometric_mean():
     r4 = Oracle(w, backward=dict(g=w.g, Gamma=w.Gamma, Phi=w.Phi)).run(w.m0, w.a0, fixed_dt=0.5e-12, max_steps=200)
     r5 = Oracle(w).run(w.m0, w.a0, fixed_dt=0.5e-12, max_steps=200)
     assert np.array_equal(r4.m, r5.m) and np.array_equal(r4.a, r5.a)
+
+
+# ----------------------------------------------------------------------------------------
+# per-mode polarisation (the paper fixes x^; reading G32)
+# ----------------------------------------------------------------------------------------
+def _rot_z(v, phi):
+    c, s = math.cos(phi), math.sin(phi)
+    out = np.array(v, dtype=np.float64, copy=True)
+    out[..., 0, :, :, :] = c * v[..., 0, :, :, :] - s * v[..., 1, :, :, :]
+    out[..., 1, :, :, :] = s * v[..., 0, :, :, :] + c * v[..., 1, :, :, :]
+    return out
+
+
+def test_polarisation_y_reproduces_the_rabi_period():
+    """A mode polarised along y^ (quadrature axis z^ x y^ = -x^) couples to m.y^ + i m.x^ and drives B_y: the problem is
+    the paper's rotated by 90 degrees about the static field, so T_R = pi/g must come out again -
+    nothing in this run touches the x^-polarised code path the other pins cover."""
+    w = W.macrospin(5.0, [5.0], 50.0, 0.0, alpha=0.0, a0=[0.01], n=2)
+    r = Oracle(w, pol=[[0.0, 1.0, 0.0]]).run(w.m0, w.a0, t_end=26e-9, tol=1e-9, sample_dt=25e-12, trace_cap=1040)
+    T = rabi_period(r.trace[:, 0], r.trace[:, 1] ** 2 + r.trace[:, 2] ** 2)
+    assert abs(T / 10e-9 - 1) < 2e-3
+    # with the wrong quadrature sign (q = +x^: the counter-rotating component) there is no exchange (PAPER.md:355)
+    r2 = Oracle(w, pol=[[0.0, 1.0, 0.0]], quad=[[1.0, 0.0, 0.0]]).run(w.m0, w.a0, t_end=26e-9, tol=1e-9,
+                                                                       sample_dt=25e-12, trace_cap=1040)
+    pa = r2.trace[:, 1] ** 2 + r2.trace[:, 2] ** 2
+    assert pa.min() > 0.8 * pa.max()                      # only the fast counter-rotating ripple, no population exchange
+
+
+def test_polarisation_is_covariant_under_rotation_about_the_field():
+    """B0 along z^, anisotropy axis z^: rotating the initial magnetisation AND every mode's polarisation by phi about z^
+    rotates the whole trajectory (the equations are covariant; a_n is a scalar).  Three profiled modes with different
+    axes, exchange on, mixed coupling."""
+    w = W.cfg3(nx=6, ny=5, nz=4)
+    N = 3
+    w.u, w.omega, w.kappa, w.g, w.Gamma, w.Phi = w.u[:N], w.omega[:N], w.kappa[:N], w.g[:N] * 30, w.g[:N] * 10, np.array([0.3, 0.0, 1.0])
+    w.ku_axis = (0.0, 0.0, 1.0)
+    w.m0 = W.tilted_state(5, 1, 6, 5, 4, 0.3)[None]
+    w.a0 = np.array([1e-2, 2e-2j, -1e-2 + 1e-2j])
+    ang = np.array([0.0, 0.7, 2.1])
+    pol = np.stack([np.cos(ang), np.sin(ang), np.zeros(3)], axis=1)
+    phi = 0.9
+    pol_r = np.stack([np.cos(ang + phi), np.sin(ang + phi), np.zeros(3)], axis=1)
+    r1 = Oracle(w, pol=pol).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=200)
+    r2 = Oracle(w, pol=pol_r).run(_rot_z(w.m0, phi), w.a0, fixed_dt=0.1e-12, max_steps=200)
+    assert np.abs(r2.m - _rot_z(r1.m, phi)).max() < 1e-12
+    assert np.abs(r2.a - r1.a).max() < 1e-12 * np.abs(r1.a).max()
+    # the polarisation matters: all modes along x^ give another trajectory
+    r0 = Oracle(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=200)
+    assert np.abs(r0.a - r1.a).max() > 1e-4 * np.abs(r1.a).max()
+    # p = x^ given explicitly is the default, bit for bit
+    rx = Oracle(w, pol=np.tile([1.0, 0.0, 0.0], (N, 1))).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=50)
+    rd = Oracle(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=50)
+    assert np.abs(rx.m - rd.m).max() < 1e-15 and np.abs(rx.a - rd.a).max() < 1e-15 * np.abs(rd.a).max()
+
+
+def test_longitudinal_polarisation_closed_form():
+    """p = z^ (along the static field, q = z^ x p = 0): the mode sees the constant S = <u m_z> = 1 and its field points
+    along z^, so m = z^ never moves and a(t) = a_p + (a_0 - a_p) exp(-(i w + kappa) t), a_p = i G/(i w + kappa)
+    (Eq. 12 with a constant source).  Pins the m.p projection and the q default."""
+    w = W.macrospin(5.0, [5.0], 50.0, 20.0, alpha=1e-3, a0=[0.01], n=2)
+    T = 0.4e-9
+    r = Oracle(w, pol=[[0.0, 0.0, 1.0]]).run(w.m0, w.a0, t_end=T, tol=1e-12)
+    lam = 1j * w.omega[0] + w.kappa[0]
+    a_p = 1j * w.g[0] / lam
+    exact = a_p + (w.a0[0] - a_p) * np.exp(-lam * T)
+    assert abs(r.a[0] - exact) < 1e-9 * abs(exact)
+    assert np.abs(r.m[0, 2] - 1.0).max() < 1e-15 and np.abs(r.m[0, :2]).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------
+# the paper's tier-2 operator-split loop as a comparison integrator (PAPER.md:169-193, :199; reading G33)
+# ----------------------------------------------------------------------------------------
+def _rk4_R(z):
+    return 1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24
+
+
+def test_split_cavity_half_is_classic_rk4():
+    """g = 0: the cavity half alone.  Classic RK4 on a' = lambda a multiplies by R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24,
+    z = lambda dt, every step (PAPER.md:199 'fourth-order Runge-Kutta'): a_n = a_0 R(z)^n exactly."""
+    w = W.macrospin(5.0, [5.0, 5.3], 0.0, [1.0, 30.0], alpha=1e-3, a0=[0.01, 0.02j], tilt=0.1, n=2)
+    dt, n = 1e-12, 500
+    r = Oracle(w).run_split(w.m0, w.a0, dt, n)
+    z = -(1j * w.omega + w.kappa) * dt
+    assert np.abs(r.a - w.a0 * _rk4_R(z) ** n).max() < 1e-13
+    assert abs(r.t - n * dt) < 1e-24
+
+
+def test_split_llg_half_is_the_unified_step_without_modes():
+    """g = 0: the LLG half alone is n_llg Dormand-Prince steps of dt/n_llg with per-cell renormalisation, i.e. exactly
+    what the (independently pinned) unified integrator does on the same plain-LLG problem at fixed step dt/n_llg."""
+    w = W.cfg1("b", n=4)
+    w.g = np.zeros(1)
+    h = 0.1e-12
+    r = Oracle(w).run_split(w.m0, w.a0, 2 * h, 50, n_llg=2)
+    ref = Oracle(w).run(w.m0, w.a0, fixed_dt=h, max_steps=100)
+    assert np.abs(r.m - ref.m).max() < 1e-15
+
+
+def _split_one_step_map(wc, kap, g, wm, dt, field_from_new_a=True):
+    """Hand-derived linear one-step map of Listing 1 for the macrospin at small angle, alpha = 0,
+    on the vector (a, a*, mu, mu*), mu = m_x - i m_y:
+      cavity half (RK4, mu frozen):  a' = R(z) a + i g dt phi(z) mu,  z = -(i wc + kappa) dt,
+                                     phi(z) = 1 + z/2 + z^2/6 + z^3/24   (RK4 on a' = lambda a + const)
+      LLG half (field b = (2/gamma) g Re a' frozen):  mu' = -i wm mu + i g (a' + a'*)  integrated
+                                     exactly over dt:  mu(dt) = E mu + g (a' + a'*) (1 - E)/wm,  E = exp(-i wm dt)."""
+    z = -(1j * wc + kap) * dt
+    R, phi = _rk4_R(z), 1 + z / 2 + z ** 2 / 6 + z ** 3 / 24
+    E = np.exp(-1j * wm * dt)
+    c = g * (1 - E) / wm
+    M = np.zeros((4, 4), dtype=np.complex128)
+    M[0] = [R, 0, 1j * g * dt * phi, 0]
+    M[1] = np.conj([0, R, 0, 1j * g * dt * phi])
+    src = M[0] + M[1] if field_from_new_a else np.array([1, 1, 0, 0], dtype=np.complex128)
+    M[2] = c * src + np.array([0, 0, E, 0])
+    M[3] = np.conj(c) * (M[0] + M[1] if field_from_new_a else src) + np.array([0, 0, 0, np.conj(E)])
+    return M
+
+
+@pytest.mark.parametrize("dt_ps", [2.0, 4.0])
+def test_split_rabi_period_follows_the_exact_one_step_map(dt_ps):
+    """g/2pi = 50 MHz at 5 GHz, a(0) = 0.01 (Fig. 11): the Rabi period of the operator-split
+    loop is 2 pi / (W+ - W-) with exp(-i W dt) the eigenvalues of the hand-derived one-step map above - NOT pi/g: the
+    splitting error is what this integrator is kept for.  The map with the field taken from the OLD amplitudes (the
+    other possible reading of Listing 1) gives a period that differs by several times the tolerance."""
+    dt = dt_ps * 1e-12
+    w = W.macrospin(5.0, [5.0], 50.0, 0.0, alpha=0.0, a0=[0.01], n=2)
+    T = 32e-9
+    n = int(round(T / dt))
+    se = max(1, int(round(24e-12 / dt)))
+    r = Oracle(w).run_split(w.m0, w.a0, dt, n, sample_every=se, trace_cap=n // se)
+    T_sim = rabi_period(r.trace[:, 0], r.trace[:, 1] ** 2 + r.trace[:, 2] ** 2)
+
+    def period(new):
+        lam = np.linalg.eigvals(_split_one_step_map(w.omega[0], 0.0, w.g[0], GAMMA * w.B0[2], dt, new))
+        W_ = np.sort((1j * np.log(lam) / dt).real)
+        Wp = W_[W_ > 0]                       # the two polariton branches near +wc
+        return TWO_PI / (Wp[1] - Wp[0])
+    T_new, T_old = period(True), period(False)
+    assert abs(T_sim / T_new - 1) < 3e-5
+    assert abs(T_old / T_new - 1) > 3e-4                  # the pin tells the two readings apart
+    assert abs(T_new / 10e-9 - 1) > 1e-4                  # and the splitting error is visible at this step size
+    # the paper's bound: "the error remains below 3 % for all tested step sizes" up to 4 ps (PAPER.md:424)
+    assert abs(T_sim / 10e-9 - 1) < 0.03
+
+
+def test_split_converges_to_the_unified_integrator():
+    """dt -> 0: the operator-split state approaches the unified RK45 one, and "the operator splitting is first order in
+    dt": halving dt halves the distance.  (The Rabi PERIOD converges faster - reading m before and
+    setting the field after the cavity step cancels its first-order term, see the one-step map above.)"""
+    w = W.macrospin(5.0, [5.0], 50.0, 1.0, alpha=1e-3, a0=[0.01], tilt=0.02, n=2)
+    T = 2e-9
+    ref = Oracle(w).run(w.m0, w.a0, t_end=T, tol=1e-12)
+    errs = []
+    for dt in (2e-12, 1e-12, 0.5e-12):
+        r = Oracle(w).run_split(w.m0, w.a0, dt, int(round(T / dt)))
+        errs.append(abs(r.a[0] - ref.a[0]))
+    assert 1.8 < errs[0] / errs[1] < 2.2 and 1.8 < errs[1] / errs[2] < 2.2 and errs[2] < 1e-4
+
+
+# ----------------------------------------------------------------------------------------
+# the plain Fourier sum behind the paper's spectra (PAPER.md:227-229, :261)
+# ----------------------------------------------------------------------------------------
+def test_dft_equals_numpy_fft_on_the_fft_grid_and_peaks_at_the_signal_frequency():
+    from oracle import dft
+    rng = np.random.default_rng(3)
+    n, d = 256, 20e-12
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    t = d * np.arange(n)
+    k = np.arange(n)
+    X = dft(t, x, TWO_PI * k / (n * d))                   # sum_j x_j exp(+2 pi i j k / n) = n * ifft(x)
+    assert np.abs(X - n * np.fft.ifft(x)).max() < 1e-10 * n
+    # a time origin t0 only multiplies by exp(i w t0)
+    X2 = dft(t + 3e-9, x, TWO_PI * k / (n * d))
+    assert np.abs(X2 - X * np.exp(1j * TWO_PI * k / (n * d) * 3e-9)).max() < 1e-9 * n
+    # x ~ exp(-i w0 t) (PAPER.md:39) peaks at +w0, off the FFT grid (the paper zero-pads 4x for that, PAPER.md:229)
+    w0 = TWO_PI * 5.013e9
+    ws = TWO_PI * np.linspace(4.9e9, 5.1e9, 401)
+    P = np.abs(dft(t, np.exp(-1j * w0 * t), ws)) ** 2
+    assert abs(ws[P.argmax()] - w0) <= TWO_PI * 0.5e6 + 1e-3
