@@ -205,6 +205,42 @@ int cav_get_kernel_path(cav_sim* sim, int* path);
 int cav_set_stage_overlap(cav_sim* sim, int on);
 int cav_get_stage_overlap(cav_sim* sim, int* active);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * Variants.
+ * --------------------------------------------------------------------------------------------------------- */
+
+/* Per-mode polarisation.  The paper applies every mode's RF field along x^ and couples it to
+ * m^- = m_x - i m_y (Eqs. 1-2).  With a polarisation p_n and a quadrature axis q_n per mode
+ *     S_n = (1/W_n) sum_r u_n(r) (m_c.p_n - i m_c.q_n),      B_rf(r) = sum_n c_n u_n(r) p_n
+ * (reading G32; p = x^, q = y^ is the paper's case).  pol: [N][3] host, normalised on entry; quad: [N][3] host,
+ * used as given, or NULL for q_n = z^ x p_n (static field along z^).  pol == NULL restores x^.  Call after cav_set_modes
+ * (a new mode set restores x^).  Implemented in the small-grid kernel: CAV_E_UNSUPPORTED for grids of more than
+ * 512 x (number of SMs) cells; the run then uses CAV_PATH_BLOCK / CAV_PATH_COOP whatever cav_set_kernel_path says, and
+ * cav_get_dmdt / cav_get_dadt (which evaluate one stage with the stage kernels) return CAV_E_UNSUPPORTED; the overlaps
+ * S_n are in the trace rows. */
+int cav_set_polarisation(cav_sim* sim, const double* pol, const double* quad);
+
+/* Integrator.  CAV_INTEGRATOR_UNIFIED (default): LLG and mode ODEs in ONE Dormand-Prince step (tier 1).
+ * CAV_INTEGRATOR_SPLIT: the paper's tier-2 co-simulation loop (PAPER.md:169-193 Listing 1, :199), kept as a comparison
+ * scheme: per step dt, (i) read the overlaps S_n of the current m, (ii) advance a_n over dt by classic RK4 with S_n held
+ * constant, (iii) set the RF field from the new a_n and hold it constant, (iv) advance the LLG equation over dt by n_llg
+ * Dormand-Prince steps of dt/n_llg (reading G33).  Fixed step only: cav_run* must be called with
+ * fixed_dt = dt (CAV_E_ARG otherwise); max_steps counts co-simulation steps; the statistics count LLG sub-steps
+ * (accepted = steps x n_llg, 6 n_llg + 1 evaluations per step); choose a trace sample_dt that is a multiple of dt.
+ * Small-grid kernel only, as cav_set_polarisation (CAV_E_UNSUPPORTED beyond). */
+enum { CAV_INTEGRATOR_UNIFIED = 0, CAV_INTEGRATOR_SPLIT = 1 };
+int cav_set_integrator(cav_sim* sim, int integrator, int n_llg);
+
+/* On-device spectroscopy: the Fourier sums behind the paper's spectra |FFT(m^-)|^2 + |FFT(a)|^2,
+ * accumulated inside the step controller at every trace sample (cav_set_trace decides when) instead of copying the
+ * trace to the host:   X[k][sig] += x_sig(t_j) exp(+i w_k t_j),   w_k = omega_lo + k (omega_hi - omega_lo)/(n_bins - 1),
+ * for the 2N signals x = a_1..a_N, S_1..S_N (a component ~ exp(-i w0 t), peaks at w_k = w0; a frequency
+ * grid finer than 1/T is the paper's zero padding).  Any path, any grid.  n_bins = 0 switches it off; the call zeroes
+ * the sums; a new mode set drops them.  cav_get_spectrum copies [n_bins][2N][2] doubles to the host and reports the
+ * number of samples accumulated. */
+int cav_set_spectrum(cav_sim* sim, int n_bins, double omega_lo, double omega_hi);
+int cav_get_spectrum(cav_sim* sim, double* out /* [n_bins][2N][2] host */, long long* n_samples);
+
 /* Number of kernels this library has launched for this handle (stage kernels + setup). */
 int cav_get_launch_count(cav_sim* sim, long long* n);
 
@@ -244,6 +280,13 @@ int cav_batch_set_backaction(cav_batch* b, const double* g_b, const double* Gamm
 
 /* Drive as cav_set_drive, common to all replicas ([N] arrays).  Call after cav_batch_set_modes. */
 int cav_batch_set_drive(cav_batch* b, const double* amp_re_im, const double* t0, const double* sigma, const double* omega_d);
+
+/* Polarisation, integrator and spectrum as cav_set_polarisation / cav_set_integrator / cav_set_spectrum, common to all
+ * replicas; the spectrum is kept per replica: [n_rep][n_bins][2N][2], n_samples [n_rep].  Call after cav_batch_set_modes. */
+int cav_batch_set_polarisation(cav_batch* b, const double* pol, const double* quad);
+int cav_batch_set_integrator(cav_batch* b, int integrator, int n_llg);
+int cav_batch_set_spectrum(cav_batch* b, int n_bins, double omega_lo, double omega_hi);
+int cav_batch_get_spectrum(cav_batch* b, double* out, long long* n_samples);
 
 /* Trace rows as cav_set_trace, per replica; resets the traces. */
 int cav_batch_set_trace(cav_batch* b, double sample_dt, int capacity);

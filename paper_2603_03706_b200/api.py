@@ -24,6 +24,7 @@ CAV_F32, CAV_F64 = 0, 1
 CAV_NORM_NCELLS, CAV_NORM_SUM_U = 0, 1
 CAV_LAUNCH_GRAPH, CAV_LAUNCH_STREAM = 0, 1
 CAV_PATH_AUTO, CAV_PATH_GENERIC, CAV_PATH_TMA, CAV_PATH_BLOCK, CAV_PATH_COOP = 0, 1, 2, 3, 4
+CAV_INTEGRATOR_UNIFIED, CAV_INTEGRATOR_SPLIT = 0, 1
 CAV_MAX_MODES = 32
 
 
@@ -66,6 +67,14 @@ _SIGS = {
     "cav_set_drive": ([_vp, _dp, _dp, _dp, _dp], _i),
     "cav_set_backaction": ([_vp, _dp, _dp, _dp], _i),
     "cav_batch_set_backaction": ([_vp, _dp, _dp, _dp], _i),
+    "cav_set_polarisation": ([_vp, _dp, _dp], _i),
+    "cav_set_integrator": ([_vp, _i, _i], _i),
+    "cav_set_spectrum": ([_vp, _i, _d, _d], _i),
+    "cav_get_spectrum": ([_vp, _dp, C.POINTER(_ll)], _i),
+    "cav_batch_set_polarisation": ([_vp, _dp, _dp], _i),
+    "cav_batch_set_integrator": ([_vp, _i, _i], _i),
+    "cav_batch_set_spectrum": ([_vp, _i, _d, _d], _i),
+    "cav_batch_get_spectrum": ([_vp, _dp, C.POINTER(_ll)], _i),
     "cav_set_m": ([_vp, _vp, _i], _i),
     "cav_get_m": ([_vp, _vp, _i], _i),
     "cav_set_a": ([_vp, _dp], _i),
@@ -477,6 +486,59 @@ def cav_set_backaction(sim, g_b, Gamma_b=None, Phi_b=None) -> None:
 def cav_batch_set_backaction(b, g_b, Gamma_b=None, Phi_b=None) -> None:
     args, keep = _back_args(g_b, Gamma_b, Phi_b)
     _check(_lib.cav_batch_set_backaction(b, *args), "cav_batch_set_backaction")
+
+
+def _pol_args(pol, quad):
+    if pol is None:
+        return (None, None), ()
+    p = np.ascontiguousarray(np.asarray(pol, dtype=np.float64).reshape(-1, 3))
+    q = None if quad is None else np.ascontiguousarray(np.asarray(quad, dtype=np.float64).reshape(-1, 3))
+    if q is not None and q.shape != p.shape:
+        raise ValueError("quad must have the shape of pol")
+    return (p.ctypes.data_as(_dp), None if q is None else q.ctypes.data_as(_dp)), (p, q)
+
+
+def cav_set_polarisation(sim, pol, quad=None) -> None:
+    """pol [N][3] (None: x^ again), quad [N][3] or None (z^ x p)."""
+    args, keep = _pol_args(pol, quad)
+    _check(_lib.cav_set_polarisation(sim, *args), "cav_set_polarisation", sim)
+
+
+def cav_batch_set_polarisation(b, pol, quad=None) -> None:
+    args, keep = _pol_args(pol, quad)
+    _check(_lib.cav_batch_set_polarisation(b, *args), "cav_batch_set_polarisation")
+
+
+def cav_set_integrator(sim, integrator: int, n_llg: int = 1) -> None:
+    _check(_lib.cav_set_integrator(sim, int(integrator), int(n_llg)), "cav_set_integrator", sim)
+
+
+def cav_batch_set_integrator(b, integrator: int, n_llg: int = 1) -> None:
+    _check(_lib.cav_batch_set_integrator(b, int(integrator), int(n_llg)), "cav_batch_set_integrator")
+
+
+def cav_set_spectrum(sim, n_bins: int, omega_lo: float = 0.0, omega_hi: float = 0.0) -> None:
+    _check(_lib.cav_set_spectrum(sim, int(n_bins), float(omega_lo), float(omega_hi)), "cav_set_spectrum", sim)
+
+
+def cav_get_spectrum(sim, n_bins: int, N: int):
+    """Returns (X [n_bins][2N] complex, n_samples)."""
+    out = np.zeros((n_bins, 2 * N, 2))
+    n = _ll()
+    _check(_lib.cav_get_spectrum(sim, out.ctypes.data_as(_dp), C.byref(n)), "cav_get_spectrum", sim)
+    return out[..., 0] + 1j * out[..., 1], n.value
+
+
+def cav_batch_set_spectrum(b, n_bins: int, omega_lo: float = 0.0, omega_hi: float = 0.0) -> None:
+    _check(_lib.cav_batch_set_spectrum(b, int(n_bins), float(omega_lo), float(omega_hi)), "cav_batch_set_spectrum")
+
+
+def cav_batch_get_spectrum(b, n_rep: int, n_bins: int, N: int):
+    """Returns (X [n_rep][n_bins][2N] complex, n_samples [n_rep])."""
+    out = np.zeros((n_rep, n_bins, 2 * N, 2))
+    ns = (_ll * n_rep)()
+    _check(_lib.cav_batch_get_spectrum(b, out.ctypes.data_as(_dp), ns), "cav_batch_get_spectrum")
+    return out[..., 0] + 1j * out[..., 1], np.array(list(ns))
 
 
 def cav_set_drive(sim, amp, t0=None, sigma=None, omega_d=None) -> None:

@@ -56,6 +56,14 @@ struct BatchArgs {
     double* cmax[2];              // [nblk] block maxima of |e|^2, double-buffered by step parity
     unsigned long long* bar;      // grid-barrier counter (zeroed before the launch)
     int nblk;
+    // SURVEY.md 8(f3) / 8(f2b) variants
+    const double* pol;            // [N][6]: polarisation p_n (3) and quadrature axis q_n (3) per mode, or NULL (x^, y^: PAPER.md:52)
+    int split_nllg;               // 0: unified RK45 step; n >= 1: the paper's tier-2 operator-split loop, one
+                                  // cavity RK4 step per n LLG sub-steps; fixed_dt is then the LLG sub-step and max_steps counts sub-steps
+    double* spec;                 // [n_rep][spec_K][2N][2] Fourier sums X(w_k) += x(t_j) exp(+i w_k t_j) of a_n, S_n at the trace samples, or NULL
+    long long* spec_n;            // [n_rep] samples accumulated
+    int spec_K;
+    double spec_w0, spec_dw;      // w_k = spec_w0 + k spec_dw
 };
 
 // Shared mode / controller state of one replica.
@@ -63,6 +71,7 @@ struct BatchShared {
     double omega[kMaxModes], kappa[kMaxModes], Gre[kMaxModes], Gim[kMaxModes], invW[kMaxModes], Gbre[kMaxModes], Gbim[kMaxModes];
     double a[kMaxModes][2], as[kMaxModes][2], anew[kMaxModes][2], ka[7][kMaxModes][2], S[kMaxModes][2];
     double c[kMaxModes], serr[kMaxModes];
+    double pol[kMaxModes][6];
     double eta_re[kMaxModes], eta_im[kMaxModes], eta_t0[kMaxModes], eta_i2s2[kMaxModes], eta_wd[kMaxModes];
     double part[32][2 * kMaxModes + 6];     // per-warp partial sums: overlaps (2N) then <m_s> (3 n_sub)
     double wmax[32];
@@ -70,7 +79,7 @@ struct BatchShared {
     double red2[2 * kMaxModes + 6];         // COOP: sums over all blocks
     double t, dt, h, target, err;
     long long steps;
-    int clamped, sample_hit, accept, done, status, trace_n;
+    int clamped, sample_hit, accept, done, status, trace_n, took;
     long long accepted, rejected, rhs_evals, trace_stride, trace_acc0;
     double dt_min, dt_max;
 };
@@ -79,6 +88,7 @@ struct BatchShared {
 int launch_batch_kernel(BatchArgs& A, bool f32, int n_sub, bool two_per_sm, size_t smem_optin, cudaStream_t stream,
                         cudaError_t* cuda_err);
 int launch_coop_kernel(BatchArgs& A, bool f32, int n_sub, cudaStream_t stream, cudaError_t* cuda_err);
+int pack_polarisation(int N, const double* pol, const double* quad, double* out /*[N][6]*/);
 
 template <int ROW>
 __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, const double two_over_gamma) {
@@ -90,6 +100,37 @@ __device__ __forceinline__ void batch_stage_state(BatchShared& sh, const int n, 
     sh.c[n] = two_over_gamma * (sh.Gbre[n] * are - sh.Gbim[n] * aim);
 }
 
+
+// The cavity half of the operator-split loop: classic RK4 over H of da/dt = -(i w + kappa) a + i G S + eta(t)
+// with the overlap S_n of the current magnetisation held constant; leaves the new amplitude in anew and the RF weight
+// c_n = (2/gamma) Re[G_b a_new] that the LLG half keeps constant ("H_rf = h0 * a.real", Listing 1).
+__device__ __forceinline__ void split_cavity_step(BatchShared& sh, const int n, const double t, const double H,
+                                                  const bool drive, const double two_over_gamma) {
+    const double Sre = sh.S[n][0], Sim = sh.S[n][1], Gre = sh.Gre[n], Gim = sh.Gim[n];
+    const double om = sh.omega[n], ka = sh.kappa[n];
+    auto f = [&](const double are, const double aim, const double tt, double& kre, double& kim) {
+        kre = (-ka * are + om * aim) - (Gre * Sim + Gim * Sre);
+        kim = (-ka * aim - om * are) + (Gre * Sre - Gim * Sim);
+        if (drive) {
+            const double x = tt - sh.eta_t0[n];
+            const double env = exp(-(x * x) * sh.eta_i2s2[n]);
+            double sn, cs;
+            sincos(sh.eta_wd[n] * x, &sn, &cs);
+            kre += env * (sh.eta_re[n] * cs + sh.eta_im[n] * sn);
+            kim += env * (sh.eta_im[n] * cs - sh.eta_re[n] * sn);
+        }
+    };
+    const double ar = sh.a[n][0], ai = sh.a[n][1];
+    double k1r, k1i, k2r, k2i, k3r, k3i, k4r, k4i;
+    f(ar, ai, t, k1r, k1i);
+    f(ar + 0.5 * H * k1r, ai + 0.5 * H * k1i, t + 0.5 * H, k2r, k2i);
+    f(ar + 0.5 * H * k2r, ai + 0.5 * H * k2i, t + 0.5 * H, k3r, k3i);
+    f(ar + H * k3r, ai + H * k3i, t + H, k4r, k4i);
+    const double nr = ar + (H / 6.0) * (k1r + 2.0 * k2r + 2.0 * k3r + k4r);
+    const double ni = ai + (H / 6.0) * (k1i + 2.0 * k2i + 2.0 * k3i + k4i);
+    sh.anew[n][0] = nr; sh.anew[n][1] = ni;
+    sh.c[n] = two_over_gamma * (sh.Gbre[n] * nr - sh.Gbim[n] * ni);
+}
 
 // MAXT: block-size bucket (128 / 256 / 512 / 1024 threads) - the register budget per thread follows from it.  MINB = 2 (the
 // 512-thread ferromagnet bucket, chosen by the host when there are more replicas than SMs) asks for two blocks per SM: 64
@@ -163,12 +204,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
             sh.eta_re[tid] = A.drive[tid]; sh.eta_im[tid] = A.drive[N + tid]; sh.eta_t0[tid] = A.drive[2 * N + tid];
             sh.eta_i2s2[tid] = A.drive[3 * N + tid]; sh.eta_wd[tid] = A.drive[4 * N + tid];
         }
+        if (A.pol) {
+#pragma unroll
+            for (int i = 0; i < 6; ++i) sh.pol[tid][i] = A.pol[6 * tid + i];
+        }
     }
     if (tid == 0) {
         const BatchCtl& cl = A.ctl[rep];
         sh.t = cl.t; sh.dt_min = cl.dt_min; sh.dt_max = cl.dt_max; sh.err = cl.last_err;
         sh.accepted = cl.accepted; sh.rejected = cl.rejected; sh.rhs_evals = cl.rhs_evals; sh.trace_acc0 = cl.trace_acc0;
-        sh.status = cl.status; sh.trace_n = cl.trace_n; sh.steps = 0;
+        sh.status = cl.status; sh.trace_n = cl.trace_n; sh.steps = 0; sh.took = 0;
         const bool adaptive = A.tol > 0.0;
         if (adaptive) sh.dt = A.dt_init > 0.0 ? A.dt_init : (cl.dt > 0.0 ? cl.dt : 1e-14);
         else {
@@ -179,6 +224,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
     }
     __syncthreads();
     const T* __restrict__ up = (!COOP && A.u_in_smem) ? sm_u : ug;
+    const bool polar = A.pol != nullptr;
+    const bool split = A.split_nllg > 0;
 
     // ---- one evaluation of the coupled right-hand side at stage s (1..7): slope k of the own cell, and in
     //      thread n the mode slope ka_s and the amplitudes / RF weights of the next stage state ----
@@ -193,14 +240,23 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                 for (int c = 0; c < 3; ++c) fld[(size_t)(q * 3 + c) * nc + cell] = ms[q][c];
         }
         __syncthreads();                                             // [A] c_n of this stage (and, !COOP, the stage state) published
-        T mcx, mcy;
-        if constexpr (NSUB == 1) { mcx = ms[0][0]; mcy = ms[0][1]; }
-        else { mcx = (T)0.5 * (ms[0][0] + ms[1][0]); mcy = (T)0.5 * (ms[0][1] + ms[1][1]); }
-        T brf = (T)0;
+        T mcx, mcy, mcz;
+        if constexpr (NSUB == 1) { mcx = ms[0][0]; mcy = ms[0][1]; mcz = ms[0][2]; }
+        else { mcx = (T)0.5 * (ms[0][0] + ms[1][0]); mcy = (T)0.5 * (ms[0][1] + ms[1][1]); mcz = (T)0.5 * (ms[0][2] + ms[1][2]); }
+        T brf = (T)0, brfy = (T)0, brfz = (T)0;
         for (int n = 0; n < N; ++n) {
             const T un = up[(size_t)n * nc + cell];
-            brf += (T)sh.c[n] * un;
-            double px = active ? (double)(un * mcx) : 0.0, py = active ? (double)(un * mcy) : 0.0;
+            T ux, uy;                                                // u (m_c.p - i m_c.q): real part, minus imaginary part
+            if (!polar) {                                            // p = x^, q = y^
+                brf += (T)sh.c[n] * un;
+                ux = un * mcx; uy = un * mcy;
+            } else {                                                 // reading G32: field along p_n, coupling to m.p_n - i m.q_n
+                const double cn = sh.c[n];
+                brf += (T)(cn * sh.pol[n][0]) * un; brfy += (T)(cn * sh.pol[n][1]) * un; brfz += (T)(cn * sh.pol[n][2]) * un;
+                ux = un * (mcx * (T)sh.pol[n][0] + mcy * (T)sh.pol[n][1] + mcz * (T)sh.pol[n][2]);
+                uy = un * (mcx * (T)sh.pol[n][3] + mcy * (T)sh.pol[n][4] + mcz * (T)sh.pol[n][5]);
+            }
+            double px = active ? (double)ux : 0.0, py = active ? (double)uy : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 px += __shfl_xor_sync(0xffffffffu, px, o);
@@ -248,8 +304,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
             const T mx = ms[q][0], my = ms[q][1], mz = ms[q][2];
             const T mk = mx * axx + my * axy + mz * axz;
             T Bx = B0x + lap[0] + anp * mk * axx + brf;
-            T By = B0y + lap[1] + anp * mk * axy;
-            T Bz = B0z + lap[2] + anp * mk * axz;
+            T By = B0y + lap[1] + anp * mk * axy + brfy;
+            T Bz = B0z + lap[2] + anp * mk * axz + brfz;
             if constexpr (NSUB == 2) { Bx -= BE * ms[1 - q][0]; By -= BE * ms[1 - q][1]; Bz -= BE * ms[1 - q][2]; }
             const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
             const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
@@ -270,6 +326,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
             }
             const double Sre = sx * sh.invW[n], Sim = -sy * sh.invW[n];
             sh.S[n][0] = Sre; sh.S[n][1] = Sim;
+            if (split) {                                             // operator-split loop: the amplitudes advance once per cavity step
+                if constexpr (s == 7) sh.serr[n] = 0.0;
+            } else {
             const double are = sh.as[n][0], aim = sh.as[n][1];
             const double Gre = sh.Gre[n], Gim = sh.Gim[n];
             double kre = (-sh.kappa[n] * are + sh.omega[n] * aim) - (Gre * Sim + Gim * Sre);
@@ -293,6 +352,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                 for (int j = 0; j < 7; ++j) { ere += kD[j] * sh.ka[j][n][0]; eim += kD[j] * sh.ka[j][n][1]; }
                 const double e = fabs(sh.h) * sqrt(ere * ere + eim * eim);
                 sh.serr[n] = (e < CUDART_INF) ? e : CUDART_INF;
+            }
             }
         } else if (s == 7 && tid >= 32 && tid < 32 + 3 * NSUB) {     // a second warp sums <m_s>
             const int i = tid - 32;
@@ -331,7 +391,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         }
         __syncthreads();
         if (sh.done) break;
-        if (tid < N) batch_stage_state<1>(sh, tid, A.two_over_gamma);      // a_2 = a_0 + h a21 ka_1
+        if (split) {
+            // Listing 1: the overlaps S_n of the current m are in sh.S (7th evaluation of the last step,
+            // or the evaluation before the loop); every split_nllg sub-steps: cavity RK4 over the whole cavity step, then
+            // the slope k1 in the NEW constant RF field (no FSAL across a field jump)
+            if (sh.steps % A.split_nllg == 0) {
+                if (tid < N) split_cavity_step(sh, tid, sh.t, sh.h * (double)A.split_nllg, A.drive != nullptr, A.two_over_gamma);
+                eval(std::integral_constant<int, 1>{}, y, k1);
+            }
+        } else if (tid < N) batch_stage_state<1>(sh, tid, A.two_over_gamma);      // a_2 = a_0 + h a21 ka_1
         const T h = (T)sh.h;
 
 #define CAVMAG_BATCH_STAGE(S, EXPR)                                                        \
@@ -408,6 +476,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
 
         // ---- controller (stage_finish<7> in stage_kernel.cuh, same constants) ----
         if (tid == 0) {
+            sh.took = 0;
             double mx = 0.0;
             for (int w = 0; w < (COOP ? 1 : nwarp); ++w) mx = fmax(mx, sh.wmax[w]);
             double err = sqrt(mx);
@@ -442,14 +511,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                     for (int i = 0; i < 3 * NSUB; ++i) row[1 + 4 * N + i] = sh.red[i];
                 }
                 if (take) sh.trace_n++;
+                sh.took = take ? 1 : 0;
             } else if (sh.status == 0) {
                 sh.rejected++;
                 sh.dt = hh * fac;
+                sh.took = 0;
             }
             if (adaptive && !(sh.dt > 1e-20)) sh.status = -6;
             sh.accept = accept ? 1 : 0;
         }
         __syncthreads();                                                 // [D]
+        if (A.spec != nullptr && sh.took && sh.accept && writer) {       // Fourier sums of this sample (a_new, S of the new state)
+            dft_accumulate(A.spec + (size_t)rep * A.spec_K * 4 * N, A.spec_K, A.spec_w0, A.spec_dw, N, sh.t, sh.anew, sh.S,
+                           tid, (int)blockDim.x);
+            if (tid == 0) A.spec_n[rep]++;
+        }
         if (sh.accept) {                                                 // y := y_new, FSAL: k1 := k7
 #pragma unroll
             for (int q = 0; q < NSUB; ++q)

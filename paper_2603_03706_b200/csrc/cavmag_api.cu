@@ -43,8 +43,10 @@ struct cav_sim {
     int launch_mode = CAV_LAUNCH_GRAPH;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t exec = nullptr;
+    // two run graphs: [0] one step per iteration of the device-side WHILE loop, [1] kLoopUnroll steps per iteration (long
+    // runs on the TMA path: the step boundary inside the body is a programmatic edge like the stage boundaries)
+    cudaGraph_t graph[2] = {nullptr, nullptr};
+    cudaGraphExec_t exec[2] = {nullptr, nullptr};
     bool graph_dirty = true;
     long long host_launches = 0;
     int* h_flag = nullptr;       // pinned
@@ -69,6 +71,10 @@ struct cav_sim {
     bool use_block = false;            // CAV_PATH_BLOCK: the whole run in one thread block (k_batch with one replica)
     unsigned char* d_blk = nullptr;    // bridge buffers of the block path: BatchCtl, a, mode parameters, drive, B0
     bool want_pdl = true;              // cav_set_stage_overlap
+    // ---- SURVEY.md 8(f3) / 8(f2) variants ----
+    double* d_pol = nullptr;           // [N][6] polarisation + quadrature axes, or NULL: x^, y^
+    int split_nllg = 0;                // 0: unified RK45; n >= 1: operator-split comparison integrator, n LLG sub-steps per cavity step
+    double* d_spec = nullptr;          // [spec_K][2N][2] Fourier sums, or NULL
     bool graph_pdl = false;            // loop-body edges of the current graph are programmatic dependencies
 };
 
@@ -311,8 +317,10 @@ constexpr int kCoopThreads = 512;
 void decide_path(cav_sim* s) {
     const bool block_ok = s->nc <= kBatchMaxCells;
     const bool coop_ok = !block_ok && s->nc <= (long long)s->n_sm * kCoopThreads;
-    s->use_block = (s->kernel_path == CAV_PATH_BLOCK && block_ok) || (s->kernel_path == CAV_PATH_AUTO && block_ok);
-    s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO);
+    // a non-default polarisation and the operator-split comparison integrator exist in the small-grid kernel only
+    const bool small_only = s->d_pol != nullptr || s->split_nllg > 0;
+    s->use_block = block_ok && (s->kernel_path == CAV_PATH_BLOCK || s->kernel_path == CAV_PATH_AUTO || small_only);
+    s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO || small_only);
     if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
     else s->use_tma = s->tma_eligible && s->targs[1].Q >= (long long)s->n_sm;
@@ -392,6 +400,17 @@ int run_block_path(cav_sim* s, double t_end, double tol, double fixed_dt, double
     A.sample_dt = hc->sample_dt; A.trace_t0 = hc->trace_t0; A.trace_cap = hc->trace_cap;
     A.row_len = 1 + 4 * s->N + 3 * p.n_sub; A.trace = s->d_trace;
     A.drive = hc->drive_on ? reinterpret_cast<const double*>(s->d_blk + kBlkDrive) : nullptr;
+    A.pol = s->d_pol;
+    if (s->split_nllg > 0) {
+        if (!(fixed_dt > 0.0)) return CAV_E_ARG;         // the co-simulation loop is a fixed-step scheme
+        A.split_nllg = s->split_nllg;
+        A.fixed_dt = fixed_dt / (double)s->split_nllg;   // the kernel counts LLG sub-steps
+        A.max_steps = max_steps > 0 ? max_steps * s->split_nllg : 0;
+    }
+    if (s->d_spec && hc->spec_K > 0) {
+        A.spec = s->d_spec; A.spec_K = hc->spec_K; A.spec_w0 = hc->spec_w0; A.spec_dw = hc->spec_dw;
+        A.spec_n = &s->d_ctrl->spec_n;                   // counted straight into Ctrl (the bridge kernels do not touch it)
+    }
     cudaError_t ce = cudaSuccess;
     int rc;
     if (s->use_coop) {
@@ -438,6 +457,7 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     A.u = s->u;
     A.partial = s->partial;
     A.partial_max = s->partial_max;
+    A.spec = s->d_spec;
     A.cond_handle = handle;
     A.pstride = s->pstride;
     A.nx = s->grid.nx; A.ny = s->grid.ny; A.nz = s->grid.nz;
@@ -479,9 +499,15 @@ int push_ctrl(cav_sim* s) {
     return CAV_OK;
 }
 
+constexpr int kLoopUnroll = 4;            // steps per WHILE iteration of the long-run graph
+constexpr long long kUnrollMinSteps = 64; // runs bounded to fewer steps use the one-step body (up to 6 kLoopUnroll - 1 empty
+                                          // kernels follow the step that ends a run)
+
 void destroy_graph(cav_sim* s) {
-    if (s->exec) { cudaGraphExecDestroy(s->exec); s->exec = nullptr; }
-    if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+    for (int i = 0; i < 2; ++i) {
+        if (s->exec[i]) { cudaGraphExecDestroy(s->exec[i]); s->exec[i] = nullptr; }
+        if (s->graph[i]) { cudaGraphDestroy(s->graph[i]); s->graph[i] = nullptr; }
+    }
     s->graph_dirty = true;
 }
 
@@ -510,17 +536,20 @@ int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraph
     return CAV_OK;
 }
 
-// begin -> K1 -> WHILE { K2 -> K3 -> K4 -> K5 -> K6 -> K7 }
-// On the TMA path the edges K2 -> ... -> K7 inside the loop body are programmatic dependencies: the next
-// stage kernel's blocks become resident (barrier init, tensor-map prefetch) as the SMs drain and only then
-// wait for the previous kernel to complete.
-int build_graph_impl(cav_sim* s, bool pdl) {
-    destroy_graph(s);
+// begin -> K1 -> WHILE { K2 -> K3 -> K4 -> K5 -> K6 -> K7 [-> K2 -> ... -> K7] x (unroll - 1) }
+// On the TMA path the edges between consecutive stage kernels inside the loop body are programmatic dependencies: the
+// next stage kernel's blocks become resident (barrier init, tensor-map prefetch, early profile loads) as the SMs drain
+// and only then wait for the previous kernel to complete.  The step controller runs in the prologue of every stage-2
+// kernel, so a body may hold several steps: the WHILE condition is then evaluated once per `unroll` steps (one loop
+// iteration costs ~6 us of idle GPU between K7 and the next K2), and the kernels after the step that ends the run
+// return at once.
+int build_graph_impl(cav_sim* s, int which, bool pdl, int unroll) {
     choose_grid(s);
     decide_path(s);
-    CK(cudaGraphCreate(&s->graph, 0));
+    CK(cudaGraphCreate(&s->graph[which], 0));
+    cudaGraph_t graph = s->graph[which];
     cudaGraphConditionalHandle handle;
-    CK(cudaGraphConditionalHandleCreate(&handle, s->graph, 0, cudaGraphCondAssignDefault));
+    CK(cudaGraphConditionalHandleCreate(&handle, graph, 0, cudaGraphCondAssignDefault));
     unsigned long long h64 = (unsigned long long)handle;
     StageArgs A = make_args(s, h64);
     double* trace = s->d_trace;
@@ -530,14 +559,14 @@ int build_graph_impl(cav_sim* s, bool pdl) {
     cudaGraphNode_t n_begin, n_k1, n_while;
     {
         void* params[] = {&ctrl, &ctrl0, &h64};
-        int rc = add_kernel(s, s->graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params, 0);
+        int rc = add_kernel(s, graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params, 0);
         if (rc) return rc;
     }
     {
         void* params[] = {&A, &trace};
         void* tparams[] = {&A, &s->targs[1], &trace};
-        int rc = s->use_tma ? add_kernel(s, s->graph, &n_k1, &n_begin, stage_tma_fn(s, 1), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[1])
-                            : add_kernel(s, s->graph, &n_k1, &n_begin, stage_fn(s, 1), dim3(s->nblocks), dim3(kBlock), params, 0);
+        int rc = s->use_tma ? add_kernel(s, graph, &n_k1, &n_begin, stage_tma_fn(s, 1), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[1])
+                            : add_kernel(s, graph, &n_k1, &n_begin, stage_fn(s, 1), dim3(s->nblocks), dim3(kBlock), params, 0);
         if (rc) return rc;
     }
     cudaGraphNodeParams cp = {};
@@ -545,32 +574,43 @@ int build_graph_impl(cav_sim* s, bool pdl) {
     cp.conditional.handle = handle;
     cp.conditional.type = cudaGraphCondTypeWhile;
     cp.conditional.size = 1;
-    CK(cudaGraphAddNode(&n_while, s->graph, &n_k1, 1, &cp));
+    CK(cudaGraphAddNode(&n_while, graph, &n_k1, 1, &cp));
     cudaGraph_t body = cp.conditional.phGraph_out[0];
     cudaGraphNode_t prev;
-    for (int stage = 2; stage <= 7; ++stage) {
-        void* params[] = {&A, &trace};
-        void* tparams[] = {&A, &s->targs[stage], &trace};
-        cudaGraphNode_t node;
-        const cudaGraphNode_t* dep = stage == 2 ? nullptr : &prev;
-        int rc = s->use_tma ? add_kernel(s, body, &node, dep, stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], pdl)
-                            : add_kernel(s, body, &node, dep, stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0);
-        if (rc) return rc;
-        prev = node;
-    }
-    CK(cudaGraphInstantiate(&s->exec, s->graph, 0));
-    s->graph_dirty = false;
+    for (int u = 0; u < unroll; ++u)
+        for (int stage = 2; stage <= 7; ++stage) {
+            void* params[] = {&A, &trace};
+            void* tparams[] = {&A, &s->targs[stage], &trace};
+            cudaGraphNode_t node;
+            const cudaGraphNode_t* dep = (u == 0 && stage == 2) ? nullptr : &prev;
+            int rc = s->use_tma ? add_kernel(s, body, &node, dep, stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], pdl)
+                                : add_kernel(s, body, &node, dep, stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0);
+            if (rc) return rc;
+            prev = node;
+        }
+    CK(cudaGraphInstantiate(&s->exec[which], graph, 0));
     return CAV_OK;
 }
 
 int build_graph(cav_sim* s) {
+    destroy_graph(s);
     decide_path(s);
+    // the generic kernels finish a step in the last block of K7 and set the condition there: one step per iteration
+    const int unroll1 = s->use_tma ? kLoopUnroll : 1;
     if (s->use_tma && s->want_pdl) {
-        if (build_graph_impl(s, true) == CAV_OK) { s->graph_pdl = true; return CAV_OK; }
+        if (build_graph_impl(s, 0, true, 1) == CAV_OK && build_graph_impl(s, 1, true, unroll1) == CAV_OK) {
+            s->graph_pdl = true;
+            s->graph_dirty = false;
+            return CAV_OK;
+        }
         cudaGetLastError();          // programmatic edges refused here: fall back to full dependencies
+        destroy_graph(s);
     }
     s->graph_pdl = false;
-    return build_graph_impl(s, false);
+    int rc = build_graph_impl(s, 0, false, 1);
+    if (rc == CAV_OK) rc = build_graph_impl(s, 1, false, unroll1);
+    if (rc == CAV_OK) s->graph_dirty = false;
+    return rc;
 }
 
 int launch_stage(cav_sim* s, int stage, StageArgs& A) {
@@ -719,6 +759,8 @@ int cav_destroy(cav_sim* s) {
     cudaFree(s->d_maps);
     cudaFree(s->d_blk);
     cudaFree(s->d_coop);
+    cudaFree(s->d_pol);
+    cudaFree(s->d_spec);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     if (s->h_flag) cudaFreeHost(s->h_flag);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -775,7 +817,7 @@ int cav_set_stage_overlap(cav_sim* s, int on) {
 
 int cav_get_stage_overlap(cav_sim* s, int* active) {
     if (!s || !active) return CAV_E_ARG;
-    *active = (s->exec && !s->graph_dirty && s->graph_pdl) ? 1 : 0;
+    *active = (s->exec[0] && !s->graph_dirty && s->graph_pdl) ? 1 : 0;
     return CAV_OK;
 }
 
@@ -856,7 +898,10 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         c->invW[n] = invW[n];
         c->a[n][0] = c->a[n][1] = 0.0;
     }
-    c->drive_on = 0;                     // a new mode set clears the drive
+    c->drive_on = 0;                     // a new mode set clears the drive,
+    cudaFree(s->d_pol); s->d_pol = nullptr;          // the polarisation (back to x^)
+    cudaFree(s->d_spec); s->d_spec = nullptr;        // and the spectrum (its layout depends on N)
+    c->spec_K = 0; c->spec_n = 0;
     c->k1_valid = 0;
     s->N = N;
     s->nb = bucket(N);
@@ -882,6 +927,74 @@ int cav_set_backaction(cav_sim* s, const double* g_b, const double* Gamma_b, con
     }
     c->k1_valid = 0;                     // dm/dt of the current state changes
     return push_ctrl(s);
+}
+
+int cav_set_polarisation(cav_sim* s, const double* pol, const double* quad) {
+    if (!s) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    cudaFree(s->d_pol);
+    s->d_pol = nullptr;
+    s->graph_dirty = true;
+    s->h_ctrl->k1_valid = 0;             // dm/dt and da/dt of the current state change
+    if (pol && s->N > 0) {
+        double h[6 * CAV_MAX_MODES];
+        rc = pack_polarisation(s->N, pol, quad, h);
+        if (rc) return rc;
+        CK(cudaMalloc(&s->d_pol, sizeof(double) * 6 * s->N));
+        CK(cudaMemcpyAsync(s->d_pol, h, sizeof(double) * 6 * s->N, cudaMemcpyHostToDevice, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+        decide_path(s);
+        if (!s->use_block && !s->use_coop) {             // the grid is beyond the small-grid kernel
+            cudaFree(s->d_pol);
+            s->d_pol = nullptr;
+            push_ctrl(s);
+            return CAV_E_UNSUPPORTED;
+        }
+    }
+    return push_ctrl(s);
+}
+
+int cav_set_integrator(cav_sim* s, int integrator, int n_llg) {
+    if (!s || (integrator != CAV_INTEGRATOR_UNIFIED && integrator != CAV_INTEGRATOR_SPLIT)) return CAV_E_ARG;
+    if (integrator == CAV_INTEGRATOR_SPLIT && n_llg < 1) return CAV_E_ARG;
+    const int old = s->split_nllg;
+    s->split_nllg = integrator == CAV_INTEGRATOR_SPLIT ? n_llg : 0;
+    if (s->split_nllg > 0) {
+        decide_path(s);
+        if (!s->use_block && !s->use_coop) { s->split_nllg = old; return CAV_E_UNSUPPORTED; }
+    }
+    s->graph_dirty = true;
+    return CAV_OK;
+}
+
+int cav_set_spectrum(cav_sim* s, int n_bins, double omega_lo, double omega_hi) {
+    if (!s || n_bins < 0 || (n_bins > 1 && !(omega_hi > omega_lo))) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    cudaFree(s->d_spec);
+    s->d_spec = nullptr;
+    s->graph_dirty = true;               // the pointer is a kernel argument
+    Ctrl* c = s->h_ctrl;
+    c->spec_K = 0; c->spec_n = 0;
+    if (n_bins > 0 && s->N > 0) {
+        const size_t bytes = sizeof(double) * (size_t)n_bins * 4 * s->N;
+        CK(cudaMalloc(&s->d_spec, bytes));
+        CK(cudaMemsetAsync(s->d_spec, 0, bytes, s->stream));
+        c->spec_K = n_bins; c->spec_w0 = omega_lo; c->spec_dw = n_bins > 1 ? (omega_hi - omega_lo) / (double)(n_bins - 1) : 0.0;
+    }
+    return push_ctrl(s);
+}
+
+int cav_get_spectrum(cav_sim* s, double* out, long long* n_samples) {
+    if (!s || !out) return CAV_E_ARG;
+    if (!s->d_spec) return CAV_E_STATE;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, s->d_spec, sizeof(double) * (size_t)s->h_ctrl->spec_K * 4 * s->N, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    if (n_samples) *n_samples = s->h_ctrl->spec_n;
+    return s->h_ctrl->status;
 }
 
 int cav_set_drive(cav_sim* s, const double* amp, const double* t0, const double* sigma, const double* omega_d) {
@@ -959,6 +1072,7 @@ int cav_get_a(cav_sim* s, double* out) {
 
 static int ensure_k1(cav_sim* s) {
     if (!s->m_set) return CAV_E_STATE;
+    if (s->d_pol != nullptr) return CAV_E_UNSUPPORTED;     // the stage kernels evaluate x^-polarised modes only (cavmag.h)
     int rc = sync_pull(s);
     if (rc) return rc;
     if (!s->h_ctrl->k1_valid) {
@@ -1010,16 +1124,18 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     if (std::isinf(t_end) && max_steps == 0) return CAV_E_ARG;
     decide_path(s);
     if (s->use_block || s->use_coop) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
+    if (s->d_pol != nullptr || s->split_nllg > 0) return CAV_E_UNSUPPORTED;     // grid beyond the small-grid kernel (cavmag.h)
     s->last_run_block = false;
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     CK(cudaGetLastError());
     s->host_launches++;
     if (s->launch_mode == CAV_LAUNCH_GRAPH) {
-        if (s->graph_dirty || !s->exec) {
+        if (s->graph_dirty || !s->exec[0] || !s->exec[1]) {
             int rc = build_graph(s);
             if (rc) return rc;
         }
-        CK(cudaGraphLaunch(s->exec, s->stream));
+        const int which = (max_steps == 0 || max_steps >= kUnrollMinSteps) ? 1 : 0;
+        CK(cudaGraphLaunch(s->exec[which], s->stream));
         s->host_launches++;   // k_begin
         return CAV_OK;
     }
@@ -1121,5 +1237,19 @@ int cav_get_launch_count(cav_sim* s, long long* n) {
     *n = s->host_launches + s->h_ctrl->rhs_evals;
     return CAV_OK;
 }
+
+#ifdef CAVMAG_PROBE
+// profiling builds only (-DCAVMAG_PROBE; not declared in cavmag.h): the per-block timestamps of the last launches
+int cav_debug_probe(cav_sim* s, unsigned long long* out /*[8][256][32]*/, int while_running) {
+    if (!s || !out) return CAV_E_ARG;
+    if (!while_running) CK(cudaStreamSynchronize(s->stream));
+    cudaStream_t side;                      // a snapshot while the run graph is still looping (marks of the empty last iteration would overwrite a finished run's)
+    CK(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
+    CK(cudaMemcpyAsync(out, s->d_probe, 8 * 256 * 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, side));
+    CK(cudaStreamSynchronize(side));
+    cudaStreamDestroy(side);
+    return CAV_OK;
+}
+#endif
 
 }  // extern "C"

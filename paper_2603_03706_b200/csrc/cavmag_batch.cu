@@ -22,6 +22,12 @@ struct cav_batch {
     double* d_modep = nullptr;
     std::vector<double> h_modep;   // host mirror of d_modep
     double* d_drive = nullptr;     // [5][N] or NULL: no drive
+    double* d_pol = nullptr;       // [N][6] polarisation + quadrature axes or NULL: x^, y^
+    int split_nllg = 0;            // 0: unified RK45; n >= 1: operator-split loop with n LLG sub-steps per cavity step
+    double* d_spec = nullptr;      // [n_rep][spec_K][2N][2] Fourier sums or NULL
+    long long* d_spec_n = nullptr; // [n_rep]
+    int spec_K = 0;
+    double spec_w0 = 0.0, spec_dw = 0.0;
     int modep_per_rep = 0;
     void* d_m = nullptr;
     double* d_a = nullptr;
@@ -82,6 +88,20 @@ int pull_ctl(cav_batch* b, std::vector<BatchCtl>& h) {
 }  // namespace
 
 namespace cavmag {
+
+// [N][6] = (p_n, q_n): p_n normalised; q_n as given, or z^ x p_n (reading G32).  CAV_E_ARG for a zero vector.
+int pack_polarisation(int N, const double* pol, const double* quad, double* out) {
+    for (int n = 0; n < N; ++n) {
+        const double* p = pol + 3 * n;
+        const double len = std::sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2]);
+        if (!(len > 0.0)) return CAV_E_ARG;
+        double* o = out + 6 * n;
+        for (int i = 0; i < 3; ++i) o[i] = p[i] / len;
+        if (quad) { for (int i = 0; i < 3; ++i) o[3 + i] = quad[3 * n + i]; }
+        else { o[3] = -o[1]; o[4] = o[0]; o[5] = 0.0; }
+    }
+    return CAV_OK;
+}
 
 // Launches k_batch for A.n_rep replicas (also used by cav_run for a single tiny grid: CAV_PATH_BLOCK).
 int launch_batch_kernel(BatchArgs& A, bool f32, int n_sub, bool two_per_sm, size_t smem_optin, cudaStream_t stream,
@@ -182,6 +202,7 @@ int cav_batch_destroy(cav_batch* b) {
     if (!b) return CAV_E_ARG;
     if (b->stream) cudaStreamSynchronize(b->stream);
     cudaFree(b->d_B0); cudaFree(b->d_u); cudaFree(b->d_modep); cudaFree(b->d_drive); cudaFree(b->d_m); cudaFree(b->d_a);
+    cudaFree(b->d_pol); cudaFree(b->d_spec); cudaFree(b->d_spec_n);
     cudaFree(b->d_ctl); cudaFree(b->d_trace);
     if (b->own_stream && b->stream) cudaStreamDestroy(b->stream);
     cudaGetLastError();
@@ -230,7 +251,11 @@ int cav_batch_set_modes(cav_batch* b, int N, const void* u, const double* omega,
     cudaFree(b->d_u);
     b->d_u = nullptr;
     cudaFree(b->d_drive);
-    b->d_drive = nullptr;                  // a new mode set clears the drive
+    b->d_drive = nullptr;                  // a new mode set clears the drive,
+    cudaFree(b->d_pol);
+    b->d_pol = nullptr;                    // the polarisation (back to x^)
+    cudaFree(b->d_spec); cudaFree(b->d_spec_n);
+    b->d_spec = nullptr; b->d_spec_n = nullptr; b->spec_K = 0;      // and the spectrum (its layout depends on N)
     b->N = N;
     b->modep_per_rep = per_replica ? 1 : 0;
     if (N > 0) {
@@ -387,11 +412,68 @@ int cav_batch_run(cav_batch* b, double t_end, double tol, double fixed_dt, doubl
     A.sample_dt = b->sample_dt; A.trace_t0 = b->trace_t0; A.trace_cap = b->trace_cap; A.row_len = row_len_of(b);
     A.trace = b->d_trace;
     A.drive = b->d_drive;
+    A.pol = b->d_pol;
+    A.spec = b->d_spec; A.spec_n = b->d_spec_n; A.spec_K = b->spec_K; A.spec_w0 = b->spec_w0; A.spec_dw = b->spec_dw;
+    if (b->split_nllg > 0) {
+        // the comparison integrator is the paper's fixed-step co-simulation loop: fixed_dt is the co-simulation step;
+        // the kernel counts LLG sub-steps
+        if (!(fixed_dt > 0.0)) return CAV_E_ARG;
+        A.split_nllg = b->split_nllg;
+        A.fixed_dt = fixed_dt / (double)b->split_nllg;
+        A.max_steps = max_steps > 0 ? max_steps * b->split_nllg : 0;
+    }
 
     cudaError_t ce = cudaSuccess;
     int rc = cavmag::launch_batch_kernel(A, p.precision == CAV_F32, p.n_sub, b->n_rep > b->n_sm, b->smem_optin, b->stream, &ce);
     if (rc == CAV_E_CUDA || rc == CAV_E_NOMEM) snprintf(b->cuda_err, sizeof(b->cuda_err), "k_batch launch: %s", cudaGetErrorString(ce));
     return rc;
+}
+
+int cav_batch_set_polarisation(cav_batch* b, const double* pol, const double* quad) {
+    if (!b) return CAV_E_ARG;
+    CKB(cudaStreamSynchronize(b->stream));
+    cudaFree(b->d_pol);
+    b->d_pol = nullptr;
+    if (!pol || b->N == 0) return CAV_OK;
+    std::vector<double> h(6 * (size_t)b->N);
+    int rc = cavmag::pack_polarisation(b->N, pol, quad, h.data());
+    if (rc) return rc;
+    CKB(cudaMalloc(&b->d_pol, sizeof(double) * h.size()));
+    CKB(cudaMemcpyAsync(b->d_pol, h.data(), sizeof(double) * h.size(), cudaMemcpyHostToDevice, b->stream));
+    CKB(cudaStreamSynchronize(b->stream));
+    return CAV_OK;
+}
+
+int cav_batch_set_integrator(cav_batch* b, int integrator, int n_llg) {
+    if (!b || (integrator != CAV_INTEGRATOR_UNIFIED && integrator != CAV_INTEGRATOR_SPLIT)) return CAV_E_ARG;
+    if (integrator == CAV_INTEGRATOR_SPLIT && n_llg < 1) return CAV_E_ARG;
+    b->split_nllg = integrator == CAV_INTEGRATOR_SPLIT ? n_llg : 0;
+    return CAV_OK;
+}
+
+int cav_batch_set_spectrum(cav_batch* b, int n_bins, double omega_lo, double omega_hi) {
+    if (!b || n_bins < 0 || (n_bins > 1 && !(omega_hi > omega_lo))) return CAV_E_ARG;
+    CKB(cudaStreamSynchronize(b->stream));
+    cudaFree(b->d_spec); cudaFree(b->d_spec_n);
+    b->d_spec = nullptr; b->d_spec_n = nullptr; b->spec_K = 0;
+    if (n_bins == 0 || b->N == 0) return CAV_OK;
+    const size_t bytes = sizeof(double) * (size_t)b->n_rep * n_bins * 4 * b->N;
+    CKB(cudaMalloc(&b->d_spec, bytes));
+    CKB(cudaMalloc(&b->d_spec_n, sizeof(long long) * b->n_rep));
+    CKB(cudaMemsetAsync(b->d_spec, 0, bytes, b->stream));
+    CKB(cudaMemsetAsync(b->d_spec_n, 0, sizeof(long long) * b->n_rep, b->stream));
+    CKB(cudaStreamSynchronize(b->stream));
+    b->spec_K = n_bins; b->spec_w0 = omega_lo; b->spec_dw = n_bins > 1 ? (omega_hi - omega_lo) / (double)(n_bins - 1) : 0.0;
+    return CAV_OK;
+}
+
+int cav_batch_get_spectrum(cav_batch* b, double* out, long long* n_samples) {
+    if (!b || !out) return CAV_E_ARG;
+    if (!b->d_spec) return CAV_E_STATE;
+    CKB(cudaMemcpyAsync(out, b->d_spec, sizeof(double) * (size_t)b->n_rep * b->spec_K * 4 * b->N, cudaMemcpyDeviceToHost, b->stream));
+    if (n_samples) CKB(cudaMemcpyAsync(n_samples, b->d_spec_n, sizeof(long long) * b->n_rep, cudaMemcpyDeviceToHost, b->stream));
+    CKB(cudaStreamSynchronize(b->stream));
+    return CAV_OK;
 }
 
 int cav_batch_get_m(cav_batch* b, void* m_out) {

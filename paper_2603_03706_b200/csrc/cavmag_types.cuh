@@ -65,6 +65,10 @@ struct Ctrl {
     double sample_dt, trace_t0;
     int trace_cap, trace_n;
     long long trace_stride, trace_acc0;
+    // ---- on-device spectroscopy: Fourier sums at the trace samples ----
+    int spec_K, took;              // bins (0: off); took: the controller just stored a trace sample (transient)
+    double spec_w0, spec_dw;       // w_k = spec_w0 + k spec_dw
+    long long spec_n;              // samples accumulated
     // ---- last-block-done counter ----
     unsigned int arrive;
     int pend7;      // TMA path: stage 7 of the step in flight is still to be finished (mode ODE, error norm, controller) by
@@ -82,6 +86,7 @@ struct StageArgs {
     const void* u;       // [N][nc]
     double* partial;     // [2][kMaxSums][pstride] block partial sums, double-buffered by stage parity (stage_partials())
     double* partial_max; // [pstride] block max of |e|^2
+    double* spec;        // [spec_K][2N][2] Fourier sums X_k += x(t_j) exp(+i w_k t_j), x = a_1..a_N, S_1..S_N, or nullptr
     unsigned long long cond_handle;   // cudaGraphConditionalHandle (0: none)
     int pstride;
     int nx, ny, nz;

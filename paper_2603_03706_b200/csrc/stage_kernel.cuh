@@ -177,6 +177,24 @@ __device__ __forceinline__ void reduce_block_partials(const double* partial, con
     }
 }
 
+// On-device spectroscopy: at a trace sample (time t, amplitudes a_n, overlaps S_n)
+// every bin k adds x exp(+i w_k t) for the 2N signals x = a_1..a_N, S_1..S_N.  Thread k owns bin k, k + nthr, ...: no
+// two threads touch the same accumulator, and successive samples are ordered by the kernel's own barriers.
+__device__ __forceinline__ void dft_accumulate(double* spec, const int K, const double w0, const double dw, const int N,
+                                               const double t, const double (*a)[2], const double (*S)[2],
+                                               const int tid, const int nthr) {
+    for (int k = tid; k < K; k += nthr) {
+        double sn, cs;
+        sincos((w0 + (double)k * dw) * t, &sn, &cs);
+        double* X = spec + (size_t)k * 4 * N;
+        for (int sig = 0; sig < 2 * N; ++sig) {
+            const double xr = sig < N ? a[sig][0] : S[sig - N][0], xi = sig < N ? a[sig][1] : S[sig - N][1];
+            X[2 * sig] += xr * cs - xi * sn;
+            X[2 * sig + 1] += xr * sn + xi * cs;
+        }
+    }
+}
+
 // max over the blocks' error maxima (one warp; the max is order-independent)
 __device__ __forceinline__ double reduce_block_max(const double* partial_max, const int nblk, const int lane) {
     double mx = 0.0;
@@ -214,6 +232,7 @@ __device__ __forceinline__ int controller_step(Ctrl* c, const double smax, const
     c->rhs_evals++;
     c->steps_run++;
     c->last_err = err;
+    c->took = 0;
     if (accept) {
         c->t = c->clamped ? c->target : c->t + h;
         c->ycur ^= 1;
@@ -237,6 +256,8 @@ __device__ __forceinline__ int controller_step(Ctrl* c, const double smax, const
                 for (int i = 0; i < 3 * nsub; ++i) row[1 + 4 * N + i] = c->mavg[i];
             }
             c->trace_n++;
+            c->took = 1;
+            if (c->spec_K > 0) c->spec_n++;
         }
     } else if (c->status == 0) {
         c->rejected++;
@@ -272,6 +293,7 @@ __device__ __forceinline__ double fifth_root(double r) {
 struct FinishArgs {
     Ctrl* ctrl;
     Ctrl* ctrl0;             // step-boundary copy (nullptr: none), kept equal to ctrl by every single-block finish
+    double* spec;            // Fourier sums [spec_K][2N][2] or nullptr
     const double* partial;
     const double* partial_max;
     unsigned long long cond_handle;
@@ -290,7 +312,7 @@ __device__ __forceinline__ double* stage_partials(const StageArgs& S, const int 
 }
 __device__ __forceinline__ FinishArgs finish_args(const StageArgs& S, const int stage) {
     FinishArgs F;
-    F.ctrl = S.ctrl; F.ctrl0 = S.ctrl0; F.partial = stage_partials(S, stage); F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
+    F.ctrl = S.ctrl; F.ctrl0 = S.ctrl0; F.spec = S.spec; F.partial = stage_partials(S, stage); F.partial_max = S.partial_max; F.cond_handle = S.cond_handle;
     F.inv_nc = S.inv_nc; F.pstride = S.pstride;
 #ifdef CAVMAG_PROBE
     F.probe = S.probe;
@@ -342,6 +364,8 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
         if (stage == 7) {
             if (tid == 0) s_accept = controller_step(c, smax, serr, sred, N, nsub, A.inv_nc, trace, true);
             __syncthreads();
+            if (A.spec != nullptr && c->spec_K > 0 && c->took)       // Fourier sums of this trace sample
+                dft_accumulate(A.spec, c->spec_K, c->spec_w0, c->spec_dw, N, c->t, c->anew, c->S, tid, nthr);
             if (tid < N && s_accept) {     // y := y_new (modes), FSAL: ka_1 := ka_7
                 c->a[tid][0] = c->anew[tid][0]; c->a[tid][1] = c->anew[tid][1];
                 c->ka[0][tid][0] = c->ka[6][tid][0]; c->ka[0][tid][1] = c->ka[6][tid][1];

@@ -252,6 +252,8 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
             serr[kMaxModes + 1] = (double)accept;
         }
         asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+        if (write && A.spec != nullptr && c->spec_K > 0 && c->took)       // Fourier sums of this trace sample
+            dft_accumulate(A.spec, c->spec_K, c->spec_w0, c->spec_dw, N, c->t, c->anew, c->S, tidc, kTmaConsumers);
         if (tidc < N && serr[kMaxModes + 1] != 0.0) {     // y := y_new (modes), FSAL: ka_1 := ka_7
             c->a[tidc][0] = c->anew[tidc][0]; c->a[tidc][1] = c->anew[tidc][1];
             c->ka[0][tidc][0] = c->ka[6][tidc][0]; c->ka[0][tidc][1] = c->ka[6][tidc][1];
@@ -268,6 +270,9 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     if (tidc == 0) c->pend7 = c->done ? 0 : 1;            // a step starts now: its stage 7 will be pending
     asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
     asm volatile("bar.arrive 2, %0;" ::"n"(kTmaThreads) : "memory");      // the producer warp may read the shared copy
+#ifdef CAVMAG_PROBE
+    if (tidc == 0) probe_mark(A, 2, 10);                // verdict and the new step's control data are in shared memory
+#endif
     const bool live = c->done == 0;
     if (write) {
         unsigned long long* const g1 = reinterpret_cast<unsigned long long*>(A.ctrl);

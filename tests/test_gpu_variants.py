@@ -1,0 +1,262 @@
+"""GPU parity of the SURVEY.md 8(f2)/8(f3) variants against the fp64 CPU oracle (-m gpu), through the C ABI:
+per-mode polarisation (cav_set_polarisation), the paper's tier-2 operator-split loop as a comparison integrator
+(cav_set_integrator) and the on-device Fourier sums of the trace (cav_set_spectrum).  Tolerances as in
+test_gpu_parity.py (north_star; G23)."""
+import copy
+import math
+import os
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+for p in (ROOT, os.path.dirname(os.path.abspath(__file__))):
+    if p not in sys.path:
+        sys.path.insert(0, p)
+
+import cavmag_workloads as W  # noqa: E402
+from test_gpu_parity import api, assert_parity, open_sim, oracle_of, small_problem  # noqa: E402,F401
+
+pytestmark = pytest.mark.gpu
+TWO_PI = 2.0 * math.pi
+
+
+def _axes(N, seed=3):
+    """Seeded polarisations p_n (unit vectors, any direction) and quadrature axes q_n (unit, orthogonal to p_n)."""
+    r = W.uniform01(seed, 7, 6 * N).reshape(N, 6) - 0.5
+    p = r[:, :3] / np.linalg.norm(r[:, :3], axis=1, keepdims=True)
+    q = r[:, 3:] - (r[:, 3:] * p).sum(axis=1, keepdims=True) * p
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    return p, q
+
+
+# ----------------------------------------------------------------------------------------
+# per-mode polarisation
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,N,n_sub,dt,path", [
+    ((16, 8, 4), 3, 1, 0.1e-12, "block"),
+    ((8, 8, 4), 1, 2, 0.02e-12, "block"),
+    ((40, 9, 7), 3, 1, 0.1e-12, "coop"),
+    ((20, 12, 6), 2, 2, 0.02e-12, "coop"),
+])
+@pytest.mark.parametrize("with_quad", [False, True])
+def test_polarisation_fixed_steps(api, prec, shape, N, n_sub, dt, path, with_quad):
+    w = small_problem(*shape, N, n_sub)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    p, q = _axes(N)
+    quad = q if with_quad else None
+    if not with_quad:                      # default quadrature z^ x p needs p in the plane for a sensible coupling; any p works
+        p[:, 2] *= 0.3
+        p /= np.linalg.norm(p, axis=1, keepdims=True)
+    ref = oracle_of(w, pol=p, quad=quad).run(w.m0, w.a0, fixed_dt=dt, max_steps=120)
+    with open_sim(api, w, prec, path) as sim:
+        api.cav_set_polarisation(sim.h, p, quad)
+        api.cav_set_trace(sim.h, 120 * dt, 1)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=120)
+        m, a = sim.get_m(), sim.get_a()
+        row = api.cav_get_trace(sim.h)[0]
+        with pytest.raises(api.CavError) as e:          # one-stage evaluation exists for x^-polarised modes only
+            api.cav_get_dadt(sim.h, N)
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+    S = row[1 + 2 * N:1 + 4 * N:2] + 1j * row[2 + 2 * N:2 + 4 * N:2]
+    assert_parity(m, a, ref, prec)
+    plain = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=120)
+    assert np.abs(plain.a - ref.a).max() > 1e-4 * np.abs(ref.a).max()          # the polarisation is not a detail here (parity bar: 1e-10)
+    mc = ref.m.mean(axis=0)
+    S_direct = np.array([(w.u[n] * (np.tensordot(p[n], mc, 1) - 1j * np.tensordot(
+        (quad[n] if with_quad else np.array([-p[n, 1], p[n, 0], 0.0])), mc, 1))).mean() for n in range(N)])
+    assert np.abs(S - S_direct).max() < (1e-13 if prec == "f64" else 2e-6)
+
+
+def test_polarisation_default_and_limits(api):
+    w = small_problem(16, 8, 4, 2, 1)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=40)
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_set_polarisation(sim.h, _axes(2)[0])
+        api.cav_set_polarisation(sim.h, None)                                   # back to x^
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=40)
+        assert_parity(sim.get_m(), sim.get_a(), ref, "f64")
+        with pytest.raises(api.CavError) as e:
+            api.cav_set_polarisation(sim.h, np.zeros((2, 3)))
+        assert e.value.status == api.CAV_E_ARG
+    big = small_problem(512, 160, 2, 1, 1)                                      # 163 840 cells > 512 x SMs
+    with api.Sim(big, precision="f32") as sim:
+        with pytest.raises(api.CavError) as e:
+            api.cav_set_polarisation(sim.h, [[0.0, 1.0, 0.0]])
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+        with pytest.raises(api.CavError) as e:
+            api.cav_set_integrator(sim.h, api.CAV_INTEGRATOR_SPLIT, 1)
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+
+
+def test_polarisation_batch(api):
+    w = small_problem(8, 8, 2, 2, 1)
+    p, q = _axes(2, seed=9)
+    B0 = np.array([[0.01, -0.02, W.b0_for_ghz(f)] for f in (9.5, 10.5)])
+    with api.Batch(w, 2, precision="f64", B0=B0) as b:
+        api.cav_batch_set_polarisation(b.h, p, q)
+        b.run(math.inf, fixed_dt=0.1e-12, max_steps=80)
+        m, a = b.get_m(), b.get_a()
+    for r in range(2):
+        wr = copy.deepcopy(w); wr.B0 = tuple(B0[r])
+        ref = oracle_of(wr, pol=p, quad=q).run(wr.m0, wr.a0, fixed_dt=0.1e-12, max_steps=80)
+        assert_parity(m[r], a[r], ref, "f64")
+
+
+# ----------------------------------------------------------------------------------------
+# the operator-split comparison integrator (PAPER.md:169-193 Listing 1, :199)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,N,n_sub,dt,n_llg,path", [
+    ((8, 8, 1), 1, 1, 0.2e-12, 1, "block"),        # the paper's grid
+    ((16, 8, 4), 3, 1, 0.3e-12, 3, "block"),       # exchange on: sub-steps keep the LLG half stable
+    ((8, 4, 4), 1, 2, 0.04e-12, 2, "block"),
+    ((40, 9, 7), 3, 1, 0.2e-12, 2, "coop"),
+])
+def test_split_fixed_steps(api, prec, shape, N, n_sub, dt, n_llg, path):
+    w = small_problem(*shape, N, n_sub)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    amp = (2e10 * (1 + np.arange(N)) * np.exp(0.7j * np.arange(N))).astype(np.complex128)
+    dr = dict(amp=amp, t0=np.full(N, 20 * dt), sigma=np.full(N, 8 * dt), omega_d=np.asarray(w.omega) * 0.97)
+    n = 60
+    ref = oracle_of(w, drive=dr).run_split(w.m0, w.a0, dt, n, n_llg=n_llg, sample_every=5, trace_cap=n // 5)
+    with open_sim(api, w, prec, path) as sim:
+        api.cav_set_drive(sim.h, dr["amp"], dr["t0"], dr["sigma"], dr["omega_d"])
+        api.cav_set_integrator(sim.h, api.CAV_INTEGRATOR_SPLIT, n_llg)
+        api.cav_set_trace(sim.h, 5 * dt, n // 5)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=n)
+        m, a = sim.get_m(), sim.get_a()
+        st = api.cav_get_stats(sim.h)
+        tr = api.cav_get_trace(sim.h)
+        with pytest.raises(api.CavError) as e:                                  # a fixed-step scheme
+            api.cav_run(sim.h, 1e-9, tol=1e-6)
+        assert e.value.status == api.CAV_E_ARG
+    assert st["accepted"] == n * n_llg and st["rejected"] == 0 and abs(st["t"] - n * dt) < 1e-22
+    assert_parity(m, a, ref, prec)
+    assert tr.shape == ref.trace.shape
+    tol = 1e-9 if prec == "f64" else 2e-4
+    assert np.abs(tr[:, 0] - ref.trace[:, 0]).max() < 1e-22
+    assert np.abs(tr[:, 1:] - ref.trace[:, 1:]).max() <= tol * max(np.abs(ref.trace[:, 1:]).max(), 1.0)
+    # it IS another integrator: the unified step from the same state differs by the splitting error
+    uni = oracle_of(w, drive=dr).run(w.m0, w.a0, fixed_dt=dt / n_llg, max_steps=n * n_llg)
+    assert np.abs(uni.a - ref.a).max() > 1e-7 * np.abs(ref.a).max()             # (parity bar: 1e-10)
+
+
+def test_split_batch_rabi_sweep(api):
+    """The paper's Fig. 11 protocol in one launch: g/2pi = 50 MHz at 5 GHz, a(0) = 0.01, co-simulation steps of 2 ps,
+    three field values; every replica against the operator-split oracle (whose Rabi period is pinned by the
+    hand-derived one-step map)."""
+    w = W.macrospin(5.0, [5.0], 50.0, 0.0, alpha=0.0, a0=[0.01], n=4)
+    ghz = np.array([4.98, 5.0, 5.02])
+    B0 = np.array([[0.0, 0.0, W.b0_for_ghz(f)] for f in ghz])
+    dt, n = 2e-12, 2000
+    with api.Batch(w, 3, precision="f64", B0=B0) as b:
+        api.cav_batch_set_integrator(b.h, api.CAV_INTEGRATOR_SPLIT, 1)
+        b.run(math.inf, fixed_dt=dt, max_steps=n)
+        m, a, st = b.get_m(), b.get_a(), b.stats()
+    for r in range(3):
+        wr = copy.deepcopy(w); wr.B0 = tuple(B0[r])
+        ref = oracle_of(wr).run_split(wr.m0, wr.a0, dt, n)
+        assert st[r]["accepted"] == n and abs(st[r]["t"] - n * dt) < 1e-21
+        assert_parity(m[r], a[r], ref, "f64")
+
+
+# ----------------------------------------------------------------------------------------
+# on-device Fourier sums of the trace
+# ----------------------------------------------------------------------------------------
+def _spectrum_case():
+    w = small_problem(40, 9, 7, 3, 1)
+    w.a0 = np.array([1e-2, 2e-2j, -1e-2 + 1e-2j])
+    return w
+
+
+@pytest.mark.parametrize("path", ["generic", "tma", "coop"])
+@pytest.mark.parametrize("adaptive", [False, True])
+def test_spectrum_equals_dft_of_the_trace(api, path, adaptive):
+    from oracle import dft
+    w = _spectrum_case()
+    N, K = 3, 97
+    lo, hi = TWO_PI * 8.5e9, TWO_PI * 11.5e9
+    sdt, cap = 1.0e-12, 64
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_trace(sim.h, sdt, cap)
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+        if adaptive:
+            api.cav_run(sim.h, cap * sdt, tol=1e-7)
+        else:
+            api.cav_run_steps(sim.h, math.inf, fixed_dt=0.1e-12, max_steps=cap * 10)
+        tr = api.cav_get_trace(sim.h)
+        X, ns = api.cav_get_spectrum(sim.h, K, N)
+        # a second run keeps accumulating; cav_set_spectrum zeroes
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+        X0, n0 = api.cav_get_spectrum(sim.h, K, N)
+    assert tr.shape[0] == cap and ns == cap and n0 == 0 and np.abs(X0).max() == 0.0
+    wk = np.linspace(lo, hi, K)
+    for n in range(N):
+        ref_a = dft(tr[:, 0], tr[:, 1 + 2 * n] + 1j * tr[:, 2 + 2 * n], wk)
+        ref_S = dft(tr[:, 0], tr[:, 1 + 2 * N + 2 * n] + 1j * tr[:, 2 + 2 * N + 2 * n], wk)
+        assert np.abs(X[:, n] - ref_a).max() <= 1e-12 * np.abs(ref_a).max() * cap
+        assert np.abs(X[:, N + n] - ref_S).max() <= 1e-12 * np.abs(ref_S).max() * cap
+    if not adaptive:        # and against the oracle's own trajectory
+        ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=cap * 10, sample_dt=sdt, trace_cap=cap)
+        for n in range(N):
+            ref_a = dft(ref.trace[:, 0], ref.trace[:, 1 + 2 * n] + 1j * ref.trace[:, 2 + 2 * n], wk)
+            assert np.abs(X[:, n] - ref_a).max() <= 1e-9 * np.abs(ref_a).max()
+
+
+def test_spectrum_batch_and_block(api):
+    from oracle import dft
+    w = small_problem(8, 8, 2, 2, 1)
+    w.a0 = np.array([1e-2, 2e-2j])
+    N, K = 2, 33
+    lo, hi = TWO_PI * 8e9, TWO_PI * 12e9
+    wk = np.linspace(lo, hi, K)
+    B0 = np.array([[0.01, -0.02, W.b0_for_ghz(f)] for f in (9.0, 10.0, 11.0)])
+    with api.Batch(w, 3, precision="f64", B0=B0) as b:
+        api.cav_batch_set_trace(b.h, 1e-12, 40)
+        api.cav_batch_set_spectrum(b.h, K, lo, hi)
+        b.run(40e-12, tol=1e-8)
+        trs = api.cav_batch_get_trace(b.h, 3, 40)
+        X, ns = api.cav_batch_get_spectrum(b.h, 3, K, N)
+    assert list(ns) == [40, 40, 40]
+    for r in range(3):
+        tr = trs[r]
+        for n in range(N):
+            ref_a = dft(tr[:, 0], tr[:, 1 + 2 * n] + 1j * tr[:, 2 + 2 * n], wk)
+            assert np.abs(X[r, :, n] - ref_a).max() <= 1e-12 * np.abs(ref_a).max() * 40
+    assert np.abs(X[0] - X[2]).max() > 1e-3 * np.abs(X[0]).max()
+    with open_sim(api, w, "f64", "block") as sim:
+        api.cav_set_trace(sim.h, 1e-12, 40)
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+        api.cav_run(sim.h, 40e-12, tol=1e-8)
+        tr = api.cav_get_trace(sim.h)
+        Xs, n_s = api.cav_get_spectrum(sim.h, K, N)
+    assert n_s == 40
+    ref_a = dft(tr[:, 0], tr[:, 1] + 1j * tr[:, 2], wk)
+    assert np.abs(Xs[:, 0] - ref_a).max() <= 1e-12 * np.abs(ref_a).max() * 40
+
+
+def test_spectrum_shows_both_polariton_branches(api):
+    """The paper's spectroscopy read-out: |X_a(w)|^2 + |X_S(w)|^2 of a coupled run peaks at the two
+    polariton frequencies of Eq. 6, straight from the device bins (no trace copied)."""
+    g = 50.0
+    w = W.macrospin(5.0, [5.0], g, 1.0, alpha=1e-4, a0=[0.01], n=4)
+    K = 401
+    lo, hi = TWO_PI * 4.9e9, TWO_PI * 5.1e9
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_set_trace(sim.h, 20e-12, 3000)
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+        api.cav_run(sim.h, 60e-9, tol=1e-8)
+        X, ns = api.cav_get_spectrum(sim.h, K, 1)
+    assert ns == 3000
+    P = np.abs(X[:, 0]) ** 2 + np.abs(X[:, 1]) ** 2
+    f = np.linspace(4.9e9, 5.1e9, K)
+    lo_peak = f[:K // 2][P[:K // 2].argmax()]
+    hi_peak = f[K // 2:][P[K // 2:].argmax()]
+    assert abs(lo_peak - (5e9 - g * 1e6)) < 3e6 and abs(hi_peak - (5e9 + g * 1e6)) < 3e6
