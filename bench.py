@@ -53,6 +53,8 @@ def make_workload(name: str, rank: int = 0):
     seed_shift = 17 * rank
     if name == "cfg3":
         return W.cfg3(seed=3000 + seed_shift, dtype=np.float32), "f32"
+    if name == "cfg3_nx250":      # cfg3 with rows that are not a multiple of 16 bytes (padded inside the library, TMA path)
+        return W.cfg3(nx=250, seed=3000 + seed_shift, dtype=np.float32), "f32"
     if name == "cfg5":
         return W.cfg5(seed=5000 + seed_shift, dtype=np.float32), "f32"
     if name == "cfg4":

@@ -179,8 +179,11 @@ int cav_set_block_cells(cav_sim* sim, int cells_per_block);
 int cav_set_sweep_order(cav_sim* sim, int serpentine);
 
 /* Which implementation of the fused stage kernel runs (same arithmetic, PAPER.md:150-159 / DESIGN.md "Kernels"):
- *   CAV_PATH_TMA      persistent TMA/mbarrier-pipelined kernel; needs nx*sizeof(T) % 16 == 0 and a mode count whose
- *                     streams fit the shared-memory rings, else cav_set_kernel_path returns CAV_E_UNSUPPORTED;
+ *   CAV_PATH_TMA      persistent TMA/mbarrier-pipelined kernel; needs 16-byte row strides and a mode count whose streams fit
+ *                     the shared-memory rings, else cav_set_kernel_path returns CAV_E_UNSUPPORTED.  Grids of more than
+ *                     512 x (number of SMs) cells whose nx*sizeof(T) is not a multiple of 16 are stored with padded rows
+ *                     inside the library (the ABI arrays stay dense) and run on this path only: GENERIC / BLOCK / COOP
+ *                     then return CAV_E_UNSUPPORTED; smaller grids with such an nx are not eligible;
  *   CAV_PATH_GENERIC  register/LDG kernel for any shape;
  *   CAV_PATH_BLOCK    grids of at most 1024 cells: the whole run in ONE thread block (the batched small-grid kernel with a
  *                     single replica: stage state in shared memory, slopes in registers, no launch per stage); the

@@ -23,7 +23,10 @@ struct cav_sim {
     int vecw = 1;            // cells per thread (4 float / 2 double / 1)
     int vec = 0;             // 1: vectorised kernels
     size_t esize = 4;
-    size_t field_bytes = 0;  // n_sub*3*nc*esize
+    size_t field_bytes = 0;  // n_sub*3*ncp*esize (device buffers; rows padded when `padded`)
+    int pitch = 0;           // elements per row in device memory (>= nx)
+    long long ncp = 0;       // pitch*ny*nz
+    bool padded = false;     // pitch > nx: only the TMA kernels run on this handle (cavmag_types.cuh)
     void* Y[2] = {nullptr, nullptr};
     void* MS[2] = {nullptr, nullptr};
     void* K[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -210,7 +213,8 @@ bool encode_map(const cav_sim* s, CUtensorMap* out, void* base, int C, int bx, i
     if (!enc || !base || C < 1) return false;
     const cuuint64_t es = s->esize;
     cuuint64_t dims[4] = {(cuuint64_t)s->grid.nx, (cuuint64_t)s->grid.ny, (cuuint64_t)s->grid.nz, (cuuint64_t)C};
-    cuuint64_t strides[3] = {dims[0] * es, dims[0] * dims[1] * es, (cuuint64_t)s->nc * es};
+    const cuuint64_t row = (cuuint64_t)s->pitch * es;           // rows padded to a multiple of 16 bytes when nx is not
+    cuuint64_t strides[3] = {row, row * dims[1], (cuuint64_t)s->ncp * es};
     cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, (cuuint32_t)(boxC > 0 ? boxC : C)};
     cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     const CUtensorMapDataType dt = s->prm.precision == CAV_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
@@ -225,7 +229,7 @@ int tma_stage_naux(int stage) { return stage <= 2 ? 0 : stage == 7 ? 1 : stage =
 int plan_tma(cav_sim* s) {
     s->tma_eligible = false;
     const int es = (int)s->esize;
-    if (((long long)s->grid.nx * es) % 16 != 0) return CAV_OK;         // TMA global strides must be multiples of 16 B
+    if (((long long)s->pitch * es) % 16 != 0) return CAV_OK;           // TMA global strides must be multiples of 16 B
     if (!get_encoder() || !s->d_maps) return CAV_OK;
     const int TX = kTmaRowBytes / es, HX = kTmaHaloBytes / es, C = 3 * s->prm.n_sub;
     CUtensorMap h[MAP_COUNT];
@@ -312,6 +316,22 @@ int plan_tma(cav_sim* s) {
 StageArgs make_args(const cav_sim* s, unsigned long long handle);
 int sync_pull(cav_sim* s);
 
+// Dense ABI array [ncomp][nz][ny][nx]  <->  device buffer with rows of s->pitch elements (a plain copy when not padded).
+int copy_in(cav_sim* s, void* dst, const void* src, int ncomp, bool src_is_device) {
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    if (!s->padded) { CK(cudaMemcpyAsync(dst, src, (size_t)ncomp * s->nc * s->esize, kind, s->stream)); return CAV_OK; }
+    const size_t w = (size_t)s->grid.nx * s->esize;
+    CK(cudaMemcpy2DAsync(dst, (size_t)s->pitch * s->esize, src, w, w, (size_t)ncomp * s->grid.ny * s->grid.nz, kind, s->stream));
+    return CAV_OK;
+}
+int copy_out(cav_sim* s, void* dst, const void* src, int ncomp, bool dst_is_device) {
+    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (!s->padded) { CK(cudaMemcpyAsync(dst, src, (size_t)ncomp * s->nc * s->esize, kind, s->stream)); return CAV_OK; }
+    const size_t w = (size_t)s->grid.nx * s->esize;
+    CK(cudaMemcpy2DAsync(dst, w, src, (size_t)s->pitch * s->esize, w, (size_t)ncomp * s->grid.ny * s->grid.nz, kind, s->stream));
+    return CAV_OK;
+}
+
 constexpr int kCoopThreads = 512;
 
 void decide_path(cav_sim* s) {
@@ -321,7 +341,8 @@ void decide_path(cav_sim* s) {
     const bool small_only = s->d_pol != nullptr || s->split_nllg > 0;
     s->use_block = block_ok && (s->kernel_path == CAV_PATH_BLOCK || s->kernel_path == CAV_PATH_AUTO || small_only);
     s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO || small_only);
-    if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
+    if (s->padded) { s->use_block = s->use_coop = false; s->use_tma = s->tma_eligible; }       // padded rows: TMA kernels only
+    else if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
     else s->use_tma = s->tma_eligible && s->targs[1].Q >= (long long)s->n_sm;
 }
@@ -464,6 +485,8 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     A.iters = s->iters;
     A.serpentine = s->serpentine;
     A.nc = s->nc;
+    A.pitch = s->pitch;
+    A.ncp = s->ncp;
     A.inv_nc = 1.0 / (double)s->nc;
     A.nvec = s->nvec;
     const cav_params& p = s->prm;
@@ -500,8 +523,8 @@ int push_ctrl(cav_sim* s) {
 }
 
 constexpr int kLoopUnroll = 4;            // steps per WHILE iteration of the long-run graph
-constexpr long long kUnrollMinSteps = 64; // runs bounded to fewer steps use the one-step body (up to 6 kLoopUnroll - 1 empty
-                                          // kernels follow the step that ends a run)
+constexpr long long kUnrollMinSteps = 8;  // runs bounded to fewer steps use the one-step body (when max_steps is not a multiple of
+                                          // kLoopUnroll, or the run ends at t_end, up to 6 kLoopUnroll - 1 empty kernels follow the last step)
 
 void destroy_graph(cav_sim* s) {
     for (int i = 0; i < 2; ++i) {
@@ -588,7 +611,16 @@ int build_graph_impl(cav_sim* s, int which, bool pdl, int unroll) {
             if (rc) return rc;
             prev = node;
         }
+    if (s->use_tma) {
+        // after the loop: one more stage-2 kernel, which finishes stage 7 of the last step (controller, trace, statistics)
+        // and returns; when the loop has already seen `done` it returns at once
+        void* tparams[] = {&A, &s->targs[2], &trace};
+        cudaGraphNode_t n_fin;
+        int rc = add_kernel(s, graph, &n_fin, &n_while, stage_tma_fn(s, 2), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[2]);
+        if (rc) return rc;
+    }
     CK(cudaGraphInstantiate(&s->exec[which], graph, 0));
+    CK(cudaGraphUpload(s->exec[which], s->stream));      // not inside the first (possibly timed) launch
     return CAV_OK;
 }
 
@@ -695,7 +727,19 @@ int cav_create(const cav_grid* grid, const cav_params* prm, cav_sim** out) {
     s->vec = (grid->nx % vw == 0) ? 1 : 0;
     s->vecw = s->vec ? vw : 1;
     s->nvec = s->nc / s->vecw;
-    s->field_bytes = (size_t)prm->n_sub * 3 * s->nc * s->esize;
+    // Row pitch.  The TMA path needs 16-byte row strides; a large grid whose nx * sizeof(T) is not a multiple of 16 is
+    // stored with padded rows (the ABI stays dense: strided copies in and out) instead of falling back to the generic
+    // kernels at half the throughput.  Grids in the range of the single-block / cooperative kernel stay dense.
+    s->pitch = grid->nx;
+    {
+        const int per16 = 16 / (int)s->esize, per128 = 128 / (int)s->esize;
+        const bool small = s->nc <= (long long)dp.multiProcessorCount * 512;
+        // padded rows start on 128-byte lines (a 16-byte pitch measured 16 % slower on cfg3 with nx = 250: every 256-byte
+        // tile row then straddles one more 32-byte sector and the stores split sectors)
+        if (grid->nx % per16 != 0 && !small) { s->pitch = (grid->nx + per128 - 1) / per128 * per128; s->padded = true; }
+    }
+    s->ncp = (long long)s->pitch * grid->ny * grid->nz;
+    s->field_bytes = (size_t)prm->n_sub * 3 * s->ncp * s->esize;
     const long long biters = (s->nvec + kBlock - 1) / kBlock;
     long long pmax = biters < kMaxBlocks ? biters : kMaxBlocks;       // generic kernel: one partial per block
     if (pmax < dp.multiProcessorCount) pmax = dp.multiProcessorCount;  // TMA kernel: one partial per SM
@@ -794,6 +838,7 @@ int cav_set_block_cells(cav_sim* s, int cells) {
 int cav_set_kernel_path(cav_sim* s, int path) {
     if (!s || (path != CAV_PATH_AUTO && path != CAV_PATH_GENERIC && path != CAV_PATH_TMA && path != CAV_PATH_BLOCK && path != CAV_PATH_COOP)) return CAV_E_ARG;
     if (path == CAV_PATH_TMA && !s->tma_eligible) return CAV_E_UNSUPPORTED;
+    if (s->padded && path != CAV_PATH_TMA && path != CAV_PATH_AUTO) return CAV_E_UNSUPPORTED;      // rows padded for the TMA path
     if (path == CAV_PATH_BLOCK && s->nc > kBatchMaxCells) return CAV_E_UNSUPPORTED;
     if (path == CAV_PATH_COOP && (s->nc <= kBatchMaxCells || s->nc > (long long)s->n_sm * kCoopThreads)) return CAV_E_UNSUPPORTED;
     s->kernel_path = path;
@@ -850,7 +895,7 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         return code;
     };
     auto cuda_fail = [&](cudaError_t e) { return fail(e == cudaErrorMemoryAllocation ? CAV_E_NOMEM : CAV_E_CUDA, e); };
-    const size_t bytes = (size_t)N * s->nc * s->esize;
+    const size_t bytes = (size_t)N * s->ncp * s->esize;
     cudaError_t e;
     if (bytes > s->u_bytes) {
         cudaFree(s->u);
@@ -859,16 +904,18 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         if ((e = cudaMalloc(&s->u, bytes)) != cudaSuccess) return cuda_fail(e);
         s->u_bytes = bytes;
     }
-    if (N > 0 && (e = cudaMemcpyAsync(s->u, u, bytes, u_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream)) != cudaSuccess)
-        return cuda_fail(e);
+    if (N > 0) {
+        if (s->padded && (e = cudaMemsetAsync(s->u, 0, bytes, s->stream)) != cudaSuccess) return cuda_fail(e);     // pad cells: u = 0
+        if (copy_in(s, s->u, u, N, u_is_device != 0) != CAV_OK) return fail(CAV_E_CUDA);
+    }
     // overlap normalisation W_n into a temporary first: CAV_E_SINGULAR_NORM must not leave half-set mode tables behind
     double invW[kMaxModes];
     for (int n = 0; n < N; ++n) invW[n] = 1.0 / (double)s->nc;
     if (N > 0 && s->prm.overlap_norm == CAV_NORM_SUM_U) {
         double* d_out = nullptr;
         if ((e = cudaMalloc(&d_out, sizeof(double) * 256 * N)) != cudaSuccess) return cuda_fail(e);
-        if (s->prm.precision == CAV_F32) k_sum_u<float><<<dim3(256, N), 256, 0, s->stream>>>((const float*)s->u, s->nc, d_out);
-        else k_sum_u<double><<<dim3(256, N), 256, 0, s->stream>>>((const double*)s->u, s->nc, d_out);
+        if (s->prm.precision == CAV_F32) k_sum_u<float><<<dim3(256, N), 256, 0, s->stream>>>((const float*)s->u, s->ncp, d_out);
+        else k_sum_u<double><<<dim3(256, N), 256, 0, s->stream>>>((const double*)s->u, s->ncp, d_out);
         s->host_launches++;
         double* h = new (std::nothrow) double[256 * (size_t)N];
         if (!h) { cudaFree(d_out); return fail(CAV_E_NOMEM); }
@@ -1025,15 +1072,16 @@ int cav_set_m(cav_sim* s, const void* m, int is_device) {
     int rc = sync_pull(s);
     if (rc) return rc;
     const void* src = m;
-    if (!is_device) {
-        CK(cudaMemcpyAsync(s->MS[1], m, s->field_bytes, cudaMemcpyHostToDevice, s->stream));
+    if (!is_device || s->padded) {       // staged through MS[1] (host source, or rows to be padded)
+        rc = copy_in(s, s->MS[1], m, 3 * s->prm.n_sub, is_device != 0);
+        if (rc) return rc;
         src = s->MS[1];
     }
     void* dst = s->Y[s->h_ctrl->ycur];
-    const long long n = s->nc * s->prm.n_sub;
+    const long long n = s->ncp * s->prm.n_sub;        // pad cells included: they are never read back as cells
     const int blocks = (int)((n + 255) / 256);
-    if (s->prm.precision == CAV_F32) k_normalize<float><<<blocks, 256, 0, s->stream>>>((const float*)src, (float*)dst, s->nc, s->prm.n_sub);
-    else k_normalize<double><<<blocks, 256, 0, s->stream>>>((const double*)src, (double*)dst, s->nc, s->prm.n_sub);
+    if (s->prm.precision == CAV_F32) k_normalize<float><<<blocks, 256, 0, s->stream>>>((const float*)src, (float*)dst, s->ncp, s->prm.n_sub);
+    else k_normalize<double><<<blocks, 256, 0, s->stream>>>((const double*)src, (double*)dst, s->ncp, s->prm.n_sub);
     CK(cudaGetLastError());
     s->host_launches++;
     s->h_ctrl->k1_valid = 0;
@@ -1047,8 +1095,8 @@ int cav_get_m(cav_sim* s, void* out, int is_device) {
     if (!s->m_set) return CAV_E_STATE;
     int rc = sync_pull(s);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(out, s->Y[s->h_ctrl->ycur], s->field_bytes,
-                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    rc = copy_out(s, out, s->Y[s->h_ctrl->ycur], 3 * s->prm.n_sub, is_device != 0);
+    if (rc) return rc;
     CK(cudaStreamSynchronize(s->stream));
     return s->h_ctrl->status;
 }
@@ -1078,6 +1126,7 @@ static int ensure_k1(cav_sim* s) {
     if (!s->h_ctrl->k1_valid) {
         choose_grid(s);
         decide_path(s);
+        if (s->padded && !s->use_tma) return CAV_E_UNSUPPORTED;
         StageArgs A = make_args(s, 0ull);
         k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
         CK(cudaGetLastError());
@@ -1093,8 +1142,8 @@ int cav_get_dmdt(cav_sim* s, void* out, int is_device) {
     if (!s || !out) return CAV_E_ARG;
     int rc = ensure_k1(s);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(out, s->K[s->h_ctrl->k1slot], s->field_bytes,
-                       is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    rc = copy_out(s, out, s->K[s->h_ctrl->k1slot], 3 * s->prm.n_sub, is_device != 0);
+    if (rc) return rc;
     CK(cudaStreamSynchronize(s->stream));
     return s->h_ctrl->status;
 }
@@ -1125,6 +1174,7 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     decide_path(s);
     if (s->use_block || s->use_coop) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     if (s->d_pol != nullptr || s->split_nllg > 0) return CAV_E_UNSUPPORTED;     // grid beyond the small-grid kernel (cavmag.h)
+    if (s->padded && !s->use_tma) return CAV_E_UNSUPPORTED;                     // padded rows are only understood by the TMA kernels
     s->last_run_block = false;
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     CK(cudaGetLastError());
@@ -1136,7 +1186,7 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
         }
         const int which = (max_steps == 0 || max_steps >= kUnrollMinSteps) ? 1 : 0;
         CK(cudaGraphLaunch(s->exec[which], s->stream));
-        s->host_launches++;   // k_begin
+        s->host_launches += s->use_tma ? 2 : 1;   // k_begin (+ the stage-2 kernel after the loop that finishes the last step)
         return CAV_OK;
     }
     s->host_launches++;

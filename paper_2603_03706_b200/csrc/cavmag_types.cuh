@@ -93,6 +93,11 @@ struct StageArgs {
     int iters;           // block-iterations per block (kBlock*VEC cells each)
     int serpentine;      // 1: odd stages sweep the grid backwards (L2 reuse across kernels)
     long long nc;        // cells
+    // Memory layout of every cell field and of u: rows of `pitch` elements (pitch >= nx; pitch == nx unless the grid is
+    // large, nx * sizeof(T) is not a multiple of 16 bytes and the TMA path needs 16-byte row strides), `ncp` = pitch * ny * nz
+    // elements per component.  Only the TMA kernels understand pitch > nx; the C ABI always takes and returns dense arrays.
+    int pitch;
+    long long ncp;
     double inv_nc;       // 1/nc
     long long nvec;      // nc / VEC
     double B0[3];

@@ -277,8 +277,13 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     if (write) {
         unsigned long long* const g1 = reinterpret_cast<unsigned long long*>(A.ctrl);
         for (int idx = tidc; idx < kCtrlWords; idx += kTmaConsumers) g1[idx] = sc_words[idx];
-        if (tidc == 0 && A.cond_handle != 0ull)
-            cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, live ? 1u : 0u);
+        if (tidc == 0 && A.cond_handle != 0ull) {
+            // A run bounded by max_steps knows its last step when that step STARTS (rejected steps count): the loop can
+            // stop after this body, and the stage-2 kernel that follows the WHILE node finishes the step.  A run bounded
+            // by t_end only learns it from the controller: the condition then lags one iteration (empty kernels).
+            const bool last = c->max_steps > 0 && c->steps_run + 1 >= c->max_steps;
+            cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, (live && !last) ? 1u : 0u);
+        }
     }
     return live;
 }
@@ -306,7 +311,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nx = A.nx, ny = A.ny, nz = A.nz;
-    const long long nc = A.nc;
+    const long long nc = A.ncp;                 // component stride in memory (rows padded to 16 bytes: cavmag_types.cuh)
     const int Dm = TA.Dm, Da = TA.Da, Du = TA.Du;
 
     const unsigned ms_ring = (smem_u32(smem_raw) + 127u) & ~127u;
@@ -578,7 +583,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         for (int i = 0; i < NSUB * 3; ++i) sm[i] = (T)0;
         T emax2 = (T)0;
 
-        const long long plane = (long long)nx * ny;
+        const long long plane = (long long)A.pitch * ny;     // plane stride in memory
         const unsigned crow = (unsigned)((warp + 1) * kTmaHaloRowBytes + kTmaHaloBytes + lane * 8);   // centre, within a comp plane
         const unsigned arow = (unsigned)(warp * kTmaRowBytes + lane * 8);
 
@@ -600,7 +605,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         // per-tile quantities (refreshed when the tile changes)
         bool active = false;
         long long cell = 0;                          // global cell index of this lane's first cell in plane z
-        T wxl = (T)0, wxr = (T)0, wym = (T)0, wyp = (T)0;
+        T wxl = (T)0, wxr = (T)0, wxi = (T)0, wym = (T)0, wyp = (T)0;
         bool new_tile = true;
 
         // stage state from a halo box (STAGE 2: formed on the fly from y0 and k1)
@@ -630,9 +635,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 // open boundary (G9): an out-of-grid neighbour gets weight 0; its TMA-zero-filled value is finite
                 wxl = gx > 0 ? wx : (T)0;
                 wxr = gx + VEC < nx ? wx : (T)0;
+                wxi = gx + 1 < nx ? wx : (T)0;          // neighbour inside the lane's pair (a padded row may end on an odd nx)
                 wym = gy > 0 ? wy : (T)0;
                 wyp = gy < ny - 1 ? wy : (T)0;
-                cell = (long long)z * plane + (long long)gy * nx + gx;
+                cell = (long long)z * plane + (long long)gy * A.pitch + gx;
                 new_tile = false;
             }
             const bool seg_start = (pl == 0 || z == zfirst);
@@ -715,7 +721,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                         const T left = (v == 0) ? xl : mc[s][c].v[v > 0 ? v - 1 : 0];
                         const T right = (v == VEC - 1) ? xr : mc[s][c].v[v < VEC - 1 ? v + 1 : VEC - 1];
                         T l = (left - m0) * ((v == 0) ? wxl : wx);
-                        l += (right - m0) * ((v == VEC - 1) ? wxr : wx);
+                        l += (right - m0) * ((v == VEC - 1) ? wxr : wxi);
                         l += (nym.v[v] - m0) * wym;
                         l += (nyp.v[v] - m0) * wyp;
                         l += (nzm.v[v] - m0) * wzm;

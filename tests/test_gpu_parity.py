@@ -743,6 +743,43 @@ def test_nonreciprocal_rabi_period_geometric_mean(api):
 
 
 # ----------------------------------------------------------------------------------------
+# large grids whose rows are not a multiple of 16 bytes: padded rows inside the library, TMA path (no generic-kernel cliff)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,nx", [("f32", 250), ("f32", 251), ("f64", 251), ("f32", 61)])
+@pytest.mark.parametrize("n_sub,N", [(1, 3), (2, 1)])
+def test_unaligned_rows_run_on_the_tma_path(api, prec, nx, n_sub, N):
+    """nx * sizeof(T) % 16 != 0 on a grid beyond the cooperative kernel's range: the library pads the rows of its own
+    buffers (the ABI arrays stay dense) and runs the TMA kernels.  Odd nx ends a row in the middle of a lane's pair of
+    cells.  Right-hand side and 12 fixed steps element by element against the oracle."""
+    ny, nz = (40, 8) if nx > 100 else (160, 8)
+    w = small_problem(nx, ny, nz, N, n_sub)
+    assert w.nx * w.ny * w.nz > 512 * 148
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+    o = oracle_of(w)
+    dm_ref, da_ref, S_ref = o.rhs(w.m0, w.a0)
+    ref = o.run(w.m0, w.a0, fixed_dt=dt, max_steps=12)
+    with api.Sim(w, precision=prec) as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        with pytest.raises(api.CavError) as e:
+            api.cav_set_kernel_path(sim.h, api.CAV_PATH_GENERIC)
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+        dm = np.empty(sim.shape_m, dtype=sim.np_dtype)
+        api.cav_get_dmdt(sim.h, dm)
+        S = api.cav_get_overlaps(sim.h, N)
+        assert np.abs(sim.get_m().astype(np.float64) - w.m0).max() < (1e-15 if prec == "f64" else 2.5e-7)      # dense in, dense out (normalised on entry)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=12)
+        m, a = sim.get_m(), sim.get_a()
+    scale = np.abs(dm_ref).max()
+    assert np.abs(dm - dm_ref).max() <= (2e-13 if prec == "f64" else 2e-5) * scale
+    assert np.abs(S - S_ref).max() <= (1e-14 if prec == "f64" else 2e-6)
+    assert_parity(m, a, ref, prec)
+
+
+# ----------------------------------------------------------------------------------------
 # TMA path with several plane-tiles per block (marching in z, tile-column changes inside a run, serpentine sweep)
 # ----------------------------------------------------------------------------------------
 @pytest.mark.parametrize("prec", ["f64", "f32"])
