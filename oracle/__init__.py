@@ -27,7 +27,7 @@ class _Problem(C.Structure):
                 ("renormalize", C.c_int), ("norm_sum_u", C.c_int), ("N", C.c_int),
                 ("u", _dp), ("omega", _dp), ("kappa", _dp), ("g", _dp), ("Gamma", _dp), ("Phi", _dp),
                 ("eta_amp", _dp), ("eta_t0", _dp), ("eta_sigma", _dp), ("eta_wd", _dp),
-                ("g_b", _dp), ("Gamma_b", _dp), ("Phi_b", _dp), ("pol", _dp), ("quad", _dp)]
+                ("g_b", _dp), ("Gamma_b", _dp), ("Phi_b", _dp), ("pol", _dp), ("quad", _dp), ("demag_N", _dp)]
 
 
 class _Stats(C.Structure):
@@ -53,6 +53,8 @@ def lib():
         _lib.orc_run_split.restype = C.c_int
         _lib.orc_dft.argtypes = [_dp, _dp, C.c_int, _dp, C.c_int, _dp]
         _lib.orc_dft.restype = None
+        _lib.orc_demag_tensor.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _dp]
+        _lib.orc_demag_tensor.restype = None
         _lib.orc_tableau.argtypes = [_dp, _dp, _dp, _dp]
         _lib.orc_set_threads.argtypes = [C.c_int]
         _lib.orc_get_threads.restype = C.c_int
@@ -87,7 +89,7 @@ class Oracle:
     or from keyword arguments with the same names."""
 
     def __init__(self, w=None, renormalize: bool = True, norm_sum_u: bool = False, drive: Optional[dict] = None,
-                 backward: Optional[dict] = None, pol=None, quad=None, **kw):
+                 backward: Optional[dict] = None, pol=None, quad=None, demag: bool = False, **kw):
         """drive = dict(amp [N] complex, t0 [N], sigma [N], omega_d [N] or None): the Gaussian-pulse drive
         eta_n(t) = amp_n exp(-(t-t0_n)^2/(2 sigma_n^2)) exp(-i omega_d,n (t-t0_n)) of Eq. 1 / Eq. 12."""
         get = (lambda k: kw[k] if k in kw else getattr(w, k))
@@ -129,6 +131,10 @@ class Oracle:
             self.pol = _c64(np.asarray(pol, dtype=np.float64).reshape(self.N, 3))
             self.quad = None if quad is None else _c64(np.asarray(quad, dtype=np.float64).reshape(self.N, 3))
             P.pol, P.quad = _p(self.pol), _p(self.quad)
+        if demag:
+            # dipolar field (reading G34; off in the paper): tensor table for every cell offset
+            self.demag_N = demag_tensor(self.nx, self.ny, self.nz, P.dx, P.dy, P.dz)
+            P.demag_N = _p(self.demag_N)
         self.P = P
         self.nc = self.nx * self.ny * self.nz
         self.gamma = P.gamma
@@ -180,6 +186,13 @@ class Oracle:
         return RunResult(m=m, a=a2[:2 * self.N].view(np.complex128).copy(), t=t.value, dt=dt, accepted=int(n_steps),
                          rejected=0, rhs_evals=6 * int(n_steps) * int(n_llg), dt_min=dt, dt_max=dt, status=status,
                          trace=None if trace is None else trace[:ntr.value].copy())
+
+
+def demag_tensor(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float) -> np.ndarray:
+    """[2nz-1][2ny-1][2nx-1][6] demagnetising tensor (xx, yy, zz, xy, xz, yz) between two cells at every offset."""
+    out = np.zeros((2 * nz - 1, 2 * ny - 1, 2 * nx - 1, 6))
+    lib().orc_demag_tensor(int(nx), int(ny), int(nz), float(dx), float(dy), float(dz), _p(out))
+    return out
 
 
 def dft(t, x, w) -> np.ndarray:

@@ -47,6 +47,14 @@
 //  frequencies w (signals ~ exp(-i w t)) - the definition behind the paper's zero-padded FFT spectra
 //  |FFT(m^-)|^2 + |FFT(a)|^2.  Pinned against numpy.fft on the FFT grid.
 //
+//  Dipolar (demagnetising) field: the paper switches it off ("Dipolar interactions are
+//  disabled", :97 Walker modes "not considered"); real samples need it, so it is an OPTIONAL term here (reading G34):
+//      B_d(r_i) = -mu0 Ms sum_j N(r_i - r_j) . m_tot(r_j),   m_tot = sum over sublattices,  open boundary (finite sample)
+//  with N the demagnetising tensor between two uniformly magnetised cells averaged over the target cell (Newell,
+//  Williams & Dunlop 1993, restated in orc_demag_tensor).  The oracle is the plain definition: a direct O(N_cells^2) sum.
+//  Pins: self term of a cube = 1/3, trace 1 at the origin and 0 elsewhere, point-dipole far field, brute-force
+//  sub-cell dipole sums, demagnetising factors of a uniformly magnetised cube / slab.
+//
 //  Build:  g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC  (see oracle/build.py)
 // =====================================================================================
 #include <cmath>
@@ -90,6 +98,8 @@ struct orc_problem {
     // per-mode polarisation (reading G32): pol == NULL: every mode along x^ with quadrature y^
     const double* pol;       // [N][3] unit vectors p_n: direction of the mode's RF field
     const double* quad;      // [N][3] quadrature axes q_n (NULL: q_n = z^ x p_n): the mode couples to m.p_n - i m.q_n
+    // dipolar field (reading G34): NULL = off (the paper's setting)
+    const double* demag_N;   // [(2nz-1)][(2ny-1)][(2nx-1)][6] tensor N(dx_i, dy_j, dz_k) for offsets -(n-1)..(n-1): xx,yy,zz,xy,xz,yz
 };
 
 struct orc_stats {
@@ -202,6 +212,31 @@ void mode_rhs(const orc_problem* P, double t, const double* a, const double* S, 
     }
 }
 
+// ---- dipolar field (reading G34): B_d(r_i) = -mu0 Ms sum_j N(r_i - r_j) . m_tot(r_j), direct sum over all pairs ----
+void demag_field(const orc_problem* P, const double* m, double* bd /*[3][nc]*/) {
+    const int nx = P->nx, ny = P->ny, nz = P->nz;
+    const long long nc = ncell(P);
+    const int tx = 2 * nx - 1, ty = 2 * ny - 1;
+    const double pref = -4e-7 * M_PI * P->Ms;
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < nc; ++i) {
+        const int xi = (int)(i % nx), yi = (int)((i / nx) % ny), zi = (int)(i / ((long long)nx * ny));
+        double hx = 0.0, hy = 0.0, hz = 0.0;
+        for (int zj = 0; zj < nz; ++zj)
+            for (int yj = 0; yj < ny; ++yj)
+                for (int xj = 0; xj < nx; ++xj) {
+                    const long long j = ((long long)zj * ny + yj) * nx + xj;
+                    double mx = m[j], my = m[nc + j], mz = m[2 * nc + j];
+                    if (P->n_sub == 2) { mx += m[3 * nc + j]; my += m[4 * nc + j]; mz += m[5 * nc + j]; }
+                    const double* T = P->demag_N + 6 * (((long long)(zi - zj + nz - 1) * ty + (yi - yj + ny - 1)) * tx + (xi - xj + nx - 1));
+                    hx += T[0] * mx + T[3] * my + T[4] * mz;
+                    hy += T[3] * mx + T[1] * my + T[5] * mz;
+                    hz += T[4] * mx + T[5] * my + T[2] * mz;
+                }
+        bd[i] = pref * hx; bd[nc + i] = pref * hy; bd[2 * nc + i] = pref * hz;
+    }
+}
+
 // ---- steps (5), (6): dm/dt of every cell for given RF weights c_n ----
 void llg_rhs(const orc_problem* P, const double* m, const double* c, double* dm) {
     const int nx = P->nx, ny = P->ny, nz = P->nz, N = P->N;
@@ -210,6 +245,8 @@ void llg_rhs(const orc_problem* P, const double* m, const double* c, double* dm)
     const double pref_an = 2.0 * P->Ku / P->Ms;
     const double wx = 1.0 / (P->dx * P->dx), wy = 1.0 / (P->dy * P->dy), wz = 1.0 / (P->dz * P->dz);
     const double llg = -P->gamma / (1.0 + P->alpha * P->alpha);
+    std::vector<double> bdem;                                   // dipolar field of the total magnetisation, [3][nc]
+    if (P->demag_N) { bdem.assign(3 * (size_t)nc, 0.0); demag_field(P, m, bdem.data()); }
     std::vector<double> cp(3 * (size_t)(N > 0 ? N : 1));      // c_n p_n (general polarisation only)
     if (P->pol)
         for (int n = 0; n < N; ++n) {
@@ -253,6 +290,7 @@ void llg_rhs(const orc_problem* P, const double* m, const double* c, double* dm)
                         Bx += bx; By += by; Bz += bz;
                     }
                     if (mo) { Bx -= P->B_exch_inter * mo[i]; By -= P->B_exch_inter * mo[nc + i]; Bz -= P->B_exch_inter * mo[2 * nc + i]; }
+                    if (P->demag_N) { Bx += bdem[i]; By += bdem[nc + i]; Bz += bdem[2 * nc + i]; }
                     // step (6): LLG in explicit Landau-Lifshitz form
                     const double tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;   // m x B
                     const double dx_ = my * tz - mz * ty, dy_ = mz * tx - mx * tz, dz_ = mx * ty - my * tx; // m x (m x B)
@@ -568,6 +606,61 @@ void orc_dft(const double* t, const double* x, int n, const double* w, int nw, d
         }
         out[2 * k] = re; out[2 * k + 1] = im;
     }
+}
+
+// ---- demagnetising tensor between two equal rectangular cells (Newell, Williams & Dunlop, J. Geophys. Res. 98, 9551
+//      (1993)), restated: with V = dx dy dz and the second-difference weights w = (1, -2, 1),
+//        N_xx(X,Y,Z) = -1/(4 pi V) sum_{i,j,k in {-1,0,1}} w_i w_j w_k f(X + i dx, Y + j dy, Z + k dz)
+//        N_xy(X,Y,Z) = -1/(4 pi V) sum_{i,j,k}              w_i w_j w_k g(X + i dx, Y + j dy, Z + k dz)
+//      the other components by permuting the axes.  f is even in x, y, z; g is odd in x and y, even in z. ----
+static double newell_f(double x, double y, double z) {
+    x = std::fabs(x); y = std::fabs(y); z = std::fabs(z);
+    const double x2 = x * x, y2 = y * y, z2 = z * z, R = std::sqrt(x2 + y2 + z2);
+    double r = (1.0 / 6.0) * (2.0 * x2 - y2 - z2) * R;
+    if (y > 0.0 && x2 + z2 > 0.0) r += 0.5 * y * (z2 - x2) * std::asinh(y / std::sqrt(x2 + z2));
+    if (z > 0.0 && x2 + y2 > 0.0) r += 0.5 * z * (y2 - x2) * std::asinh(z / std::sqrt(x2 + y2));
+    if (x > 0.0 && y > 0.0 && z > 0.0) r -= x * y * z * std::atan(y * z / (x * R));
+    return r;
+}
+static double newell_g(double x, double y, double z) {
+    z = std::fabs(z);
+    const double x2 = x * x, y2 = y * y, z2 = z * z, R = std::sqrt(x2 + y2 + z2);
+    double r = -x * y * R / 3.0;
+    if (x2 + y2 > 0.0) r += x * y * z * std::asinh(z / std::sqrt(x2 + y2));
+    if (y2 + z2 > 0.0) r += (y / 6.0) * (3.0 * z2 - y2) * std::asinh(x / std::sqrt(y2 + z2));
+    if (x2 + z2 > 0.0) r += (x / 6.0) * (3.0 * z2 - x2) * std::asinh(y / std::sqrt(x2 + z2));
+    if (z > 0.0) r -= (z * z2 / 6.0) * std::atan(x * y / (z * R));
+    if (y != 0.0) r -= (z * y2 / 2.0) * std::atan(x * z / (y * R));
+    if (x != 0.0) r -= (z * x2 / 2.0) * std::atan(y * z / (x * R));
+    return r;
+}
+static double newell_sum(double (*fn)(double, double, double), double X, double Y, double Z, double dx, double dy, double dz) {
+    const double w[3] = {1.0, -2.0, 1.0};
+    double acc = 0.0;
+    for (int i = -1; i <= 1; ++i)
+        for (int j = -1; j <= 1; ++j)
+            for (int k = -1; k <= 1; ++k) acc += w[i + 1] * w[j + 1] * w[k + 1] * fn(X + i * dx, Y + j * dy, Z + k * dz);
+    return -acc / (4.0 * M_PI * dx * dy * dz);
+}
+
+// out[(2nz-1)][(2ny-1)][(2nx-1)][6] = (N_xx, N_yy, N_zz, N_xy, N_xz, N_yz) at the offsets (i dx, j dy, k dz), |i| < nx etc.
+void orc_demag_tensor(int nx, int ny, int nz, double dx, double dy, double dz, double* out) {
+    const int tx = 2 * nx - 1, ty = 2 * ny - 1, tz = 2 * nz - 1;
+    // work in units of dx so that the formulas see numbers of order one
+    const double sy = dy / dx, sz = dz / dx;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < tz; ++k)
+        for (int j = 0; j < ty; ++j)
+            for (int i = 0; i < tx; ++i) {
+                const double X = (double)(i - (nx - 1)), Y = (double)(j - (ny - 1)) * sy, Z = (double)(k - (nz - 1)) * sz;
+                double* o = out + 6 * (((long long)k * ty + j) * tx + i);
+                o[0] = newell_sum(newell_f, X, Y, Z, 1.0, sy, sz);
+                o[1] = newell_sum(newell_f, Y, X, Z, sy, 1.0, sz);
+                o[2] = newell_sum(newell_f, Z, Y, X, sz, sy, 1.0);
+                o[3] = newell_sum(newell_g, X, Y, Z, 1.0, sy, sz);
+                o[4] = newell_sum(newell_g, X, Z, Y, 1.0, sz, sy);
+                o[5] = newell_sum(newell_g, Y, Z, X, sy, sz, 1.0);
+            }
 }
 
 // The tableau, exposed so the tests can check its identities (row sums, sum b = 1, sum d = 0).

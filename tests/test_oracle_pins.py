@@ -839,3 +839,106 @@ def test_dft_equals_numpy_fft_on_the_fft_grid_and_peaks_at_the_signal_frequency(
     ws = TWO_PI * np.linspace(4.9e9, 5.1e9, 401)
     P = np.abs(dft(t, np.exp(-1j * w0 * t), ws)) ** 2
     assert abs(ws[P.argmax()] - w0) <= TWO_PI * 0.5e6 + 1e-3
+
+
+# ----------------------------------------------------------------------------------------
+# dipolar (demagnetising) field, SURVEY.md 8(f4) - off in the paper; reading G34
+# ----------------------------------------------------------------------------------------
+MU0 = 4e-7 * math.pi
+
+
+def test_demag_tensor_identities():
+    """Newell tensor: a cube's self term is 1/3 per axis, off-diagonals vanish there; the trace is 1 at the origin and 0
+    for every other offset (div B = 0 outside the source cell); N_ij(-r) = N_ij(r); N_xy is odd in x and in y."""
+    from oracle import demag_tensor
+    T = demag_tensor(4, 3, 5, 2e-9, 2e-9, 2e-9)
+    c = T[4, 2, 3]
+    assert np.abs(c[:3] - 1.0 / 3.0).max() < 1e-12 and np.abs(c[3:]).max() < 1e-12
+    tr = T[..., :3].sum(axis=-1)
+    tr[4, 2, 3] -= 1.0
+    assert np.abs(tr).max() < 1e-11
+    assert np.abs(T - T[::-1, ::-1, ::-1]).max() < 1e-12
+    assert np.abs(T[:, :, :, 3] + T[:, :, ::-1, 3]).max() < 1e-12 and np.abs(T[:, :, :, 3] + T[:, ::-1, :, 3]).max() < 1e-12
+    # anisotropic cell: the thin direction carries almost all of the self demagnetisation
+    Tp = demag_tensor(1, 1, 1, 100e-9, 100e-9, 1e-9)[0, 0, 0]
+    assert abs(Tp[:3].sum() - 1.0) < 1e-10 and Tp[2] > 0.95 and abs(Tp[0] - Tp[1]) < 1e-10
+
+
+def test_demag_tensor_far_field_and_brute_force():
+    """Far away the cell pair is a pair of point dipoles, N_ij -> V/(4 pi) (delta_ij/r^3 - 3 r_i r_j/r^5), with a
+    relative correction ~ (cell/r)^2; nearby, the tensor equals the average over sub-cell dipole pairs (brute force)."""
+    from oracle import demag_tensor
+    d = np.array([1.0, 1.5, 0.7])
+    T = demag_tensor(12, 12, 12, *d)
+    idx = {0: (0, 0), 1: (1, 1), 2: (2, 2), 3: (0, 1), 4: (0, 2), 5: (1, 2)}
+
+    def dip(r):
+        R = np.linalg.norm(r)
+        return (np.eye(3) / R ** 3 - 3 * np.outer(r, r) / R ** 5) / (4 * math.pi)
+    for off in ((11, 4, -7), (-9, 10, 11)):
+        r = np.array(off) * d
+        D = dip(r) * d.prod()
+        got = T[11 + off[2], 11 + off[1], 11 + off[0]]
+        for k, (i, j) in idx.items():
+            assert abs(got[k] - D[i, j]) < 0.02 * np.abs(D).max()
+    n = 6
+    sub = (np.arange(n) + 0.5) / n - 0.5
+    g = np.stack(np.meshgrid(sub, sub, sub, indexing="ij"), -1).reshape(-1, 3) * d
+    for off in ((2, 1, 0), (1, 1, 1), (0, 0, 2)):
+        r0 = np.array(off) * d
+        acc = np.zeros((3, 3))
+        for a in g:
+            rr = r0 + a - g                                    # target sub-point minus source sub-points
+            R = np.linalg.norm(rr, axis=1)
+            acc += (np.eye(3)[None] / R[:, None, None] ** 3 - 3 * rr[:, :, None] * rr[:, None, :] / R[:, None, None] ** 5).sum(0)
+        D = acc / (4 * math.pi) * d.prod() / n ** 6
+        got = T[11 + off[2], 11 + off[1], 11 + off[0]]
+        for k, (i, j) in idx.items():
+            assert abs(got[k] - D[i, j]) < 0.02 * np.abs(D).max(), (off, k)
+
+
+def test_demag_field_of_uniform_bodies():
+    """Uniformly magnetised cube of n^3 cells: the volume-averaged demagnetising factor is exactly 1/3 per axis (sum over
+    all cell pairs of N_aa / n^3).  A 41 x 41 x 1 slab: the field at the centre cell, read through the torque on a slightly
+    tilted uniform state, has N_zz - N_xx close to 1 (thin-film limit) - the oracle's direct sum, not the table alone."""
+    from oracle import demag_tensor
+    T = demag_tensor(5, 5, 5, 5e-9, 5e-9, 5e-9)
+    cnt = np.array([[[(5 - abs(i)) * (5 - abs(j)) * (5 - abs(k)) for i in range(-4, 5)] for j in range(-4, 5)] for k in range(-4, 5)])
+    for axis in range(3):
+        assert abs((T[..., axis] * cnt).sum() / 125.0 - 1.0 / 3.0) < 1e-12
+    ws = W.macrospin(5.0, [5.0], 0.0, 0.0, alpha=0.0, n=2)
+    ws.nx = ws.ny = 41; ws.nz = 1
+    ws.u = np.ones((1, 1, 41, 41)); ws.B0 = (0.0, 0.0, 0.0)
+    o = Oracle(ws, demag=True)
+    eps = 1e-6
+    m0 = np.zeros((1, 3, 1, 41, 41)); m0[0, 2] = 1.0; m0[0, 0] = eps           # m = z^ + eps x^
+    dm, _, _ = o.rhs(m0 / math.sqrt(1 + eps * eps), np.zeros(1, dtype=np.complex128))
+    # B_d = -mu0 Ms (N_zz z^ + eps N_xx x^) at the centre;  (m x B)_y = m_z B_x - m_x B_z = eps mu0 Ms (N_zz - N_xx)
+    # dm_y/dt = -gamma (m x B)_y
+    diff = dm[0, 1, 0, 20, 20] / (-GAMMA * eps * MU0 * ws.Ms)
+    assert 0.90 < diff < 1.0
+    # the same number from the table: sum over the slab of N_zz - N_xx seen from the centre cell
+    Ts = demag_tensor(41, 41, 1, ws.dx, ws.dy, ws.dz)[0, 20:61, 20:61]
+    assert abs(diff - (Ts[..., 2] - Ts[..., 0]).sum()) < 1e-6
+
+
+def test_demag_shifts_the_kittel_line_of_a_platelet():
+    """One flat cell (100 x 100 x 2 nm) magnetised along its normal in B0 z^: the macrospin precesses at
+    w = gamma (B0 - mu0 Ms (N_zz - N_xx)) (Kittel's formula for a body with demagnetising factors N; small angle,
+    alpha = 0).  Pins the sign and size of the dipolar term inside the LLG right-hand side."""
+    from oracle import demag_tensor
+    w = W.macrospin(10.0, [5.0], 0.0, 0.0, alpha=0.0, tilt=1e-3, n=1)
+    w.dx = w.dy = 100e-9; w.dz = 2e-9
+    N = demag_tensor(1, 1, 1, w.dx, w.dy, w.dz)[0, 0, 0]
+    om = GAMMA * (w.B0[2] - MU0 * w.Ms * (N[2] - N[0]))
+    T = 2e-9
+    r = Oracle(w, demag=True).run(w.m0, w.a0, t_end=T, tol=1e-11)
+    phase = math.atan2(r.m[0, 1, 0, 0, 0], r.m[0, 0, 0, 0, 0])
+    expect = (om * T + math.pi) % TWO_PI - math.pi
+    assert abs(((phase - expect) + math.pi) % TWO_PI - math.pi) < 2e-4
+    assert abs(om / (GAMMA * w.B0[2]) - 1) > 0.3                   # the shift is large here (mu0 Ms = 0.176 T)
+    # and off by default: the paper's setting (PAPER.md:217)
+    r0 = Oracle(w).run(w.m0, w.a0, t_end=T, tol=1e-11)
+    ph0 = math.atan2(r0.m[0, 1, 0, 0, 0], r0.m[0, 0, 0, 0, 0])
+    e0 = (GAMMA * w.B0[2] * T + math.pi) % TWO_PI - math.pi
+    assert abs(((ph0 - e0) + math.pi) % TWO_PI - math.pi) < 2e-4
