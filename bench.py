@@ -55,6 +55,8 @@ def make_workload(name: str, rank: int = 0):
         return W.cfg3(seed=3000 + seed_shift, dtype=np.float32), "f32"
     if name == "cfg3_nx250":      # cfg3 with rows that are not a multiple of 16 bytes (padded inside the library, TMA path)
         return W.cfg3(nx=250, seed=3000 + seed_shift, dtype=np.float32), "f32"
+    if name == "cfg3_demag":      # cfg3 with the optional dipolar field on (FFT convolution before every stage; generic kernels)
+        return W.cfg3(seed=3000 + seed_shift, dtype=np.float32), "f32"
     if name == "cfg5":
         return W.cfg5(seed=5000 + seed_shift, dtype=np.float32), "f32"
     if name == "cfg4":
@@ -377,6 +379,9 @@ def run_cuda(args):
     sim = api.Sim(w, precision=prec, stream=stream.cuda_stream, path=path)
     h = sim.h
     path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma", api.CAV_PATH_BLOCK: "block", api.CAV_PATH_COOP: "coop"}[api.cav_get_kernel_path(h)]
+    if name.endswith("_demag"):
+        api.cav_set_demag(h, 1)
+        path_used = "generic + FFT convolution (host-enqueued)"
     if args.no_stage_overlap:
         api.cav_set_stage_overlap(h, 0)
     if args.no_serpentine:

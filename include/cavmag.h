@@ -234,6 +234,16 @@ int cav_set_polarisation(cav_sim* sim, const double* pol, const double* quad);
 enum { CAV_INTEGRATOR_UNIFIED = 0, CAV_INTEGRATOR_SPLIT = 1 };
 int cav_set_integrator(cav_sim* sim, int integrator, int n_llg);
 
+/* Dipolar (demagnetising) field.  The paper switches it off ("Dipolar interactions are
+ * disabled"), so it is off by default; on = 1 adds
+ *     B_d(r_i) = -mu0 Ms sum_j N(r_i - r_j) . m_tot(r_j)       (open boundary; N: Newell's cell-averaged tensor; m_tot: sum
+ * over the sublattices) to the effective field of every evaluation, as a zero-padded FFT convolution (cuFFT, loaded on
+ * demand: CAV_E_UNSUPPORTED if it cannot be) enqueued before each stage kernel.  A different roofline from the fused
+ * stencil (six 3-D FFTs of 8x the grid per evaluation): runs use the generic stage kernels with host-enqueued launches
+ * whatever cav_set_kernel_path / cav_set_launch_mode say.  Not available with cav_set_polarisation / the split integrator,
+ * nor for grids stored with padded rows (CAV_E_UNSUPPORTED).  DESIGN.md reading G34. */
+int cav_set_demag(cav_sim* sim, int on);
+
 /* On-device spectroscopy: the Fourier sums behind the paper's spectra |FFT(m^-)|^2 + |FFT(a)|^2,
  * accumulated inside the step controller at every trace sample (cav_set_trace decides when) instead of copying the
  * trace to the host:   X[k][sig] += x_sig(t_j) exp(+i w_k t_j),   w_k = omega_lo + k (omega_hi - omega_lo)/(n_bins - 1),

@@ -69,6 +69,7 @@ _SIGS = {
     "cav_batch_set_backaction": ([_vp, _dp, _dp, _dp], _i),
     "cav_set_polarisation": ([_vp, _dp, _dp], _i),
     "cav_set_integrator": ([_vp, _i, _i], _i),
+    "cav_set_demag": ([_vp, _i], _i),
     "cav_set_spectrum": ([_vp, _i, _d, _d], _i),
     "cav_get_spectrum": ([_vp, _dp, C.POINTER(_ll)], _i),
     "cav_batch_set_polarisation": ([_vp, _dp, _dp], _i),
@@ -515,6 +516,10 @@ def cav_set_integrator(sim, integrator: int, n_llg: int = 1) -> None:
 
 def cav_batch_set_integrator(b, integrator: int, n_llg: int = 1) -> None:
     _check(_lib.cav_batch_set_integrator(b, int(integrator), int(n_llg)), "cav_batch_set_integrator")
+
+
+def cav_set_demag(sim, on: int) -> None:
+    _check(_lib.cav_set_demag(sim, int(on)), "cav_set_demag", sim)
 
 
 def cav_set_spectrum(sim, n_bins: int, omega_lo: float = 0.0, omega_hi: float = 0.0) -> None:

@@ -13,10 +13,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcavmag.so")
-SOURCES = ["cavmag_api.cu", "cavmag_batch.cu", "stage_inst_f32_fm.cu", "stage_inst_f32_afm.cu", "stage_inst_f64_fm.cu",
+SOURCES = ["cavmag_api.cu", "cavmag_batch.cu", "demag.cu", "stage_inst_f32_fm.cu", "stage_inst_f32_afm.cu", "stage_inst_f64_fm.cu",
            "stage_inst_f64_afm.cu", "stage_tma_inst_f32_fm.cu", "stage_tma_inst_f32_afm.cu",
            "stage_tma_inst_f64_fm.cu", "stage_tma_inst_f64_afm.cu"]
-HEADERS = ["cavmag_types.cuh", "stage_kernel.cuh", "stage_tma.cuh", "batch_kernel.cuh", os.path.join("..", "..", "include", "cavmag.h")]
+HEADERS = ["cavmag_types.cuh", "stage_kernel.cuh", "stage_tma.cuh", "batch_kernel.cuh", "demag.cuh", os.path.join("..", "..", "include", "cavmag.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 
@@ -57,7 +57,7 @@ def build(force: bool = False, verbose: bool = False, defines=(), lib: str = LIB
 
     with ThreadPoolExecutor(max_workers=len(srcs)) as ex:
         objs = list(ex.map(compile_one, srcs))
-    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs + ["-ldl"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed:\n" + r.stdout + r.stderr)

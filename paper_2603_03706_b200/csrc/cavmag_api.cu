@@ -13,6 +13,7 @@
 #include "../../include/cavmag.h"
 #include "stage_tma.cuh"
 #include "batch_kernel.cuh"
+#include "demag.cuh"
 
 using namespace cavmag;
 
@@ -78,6 +79,8 @@ struct cav_sim {
     double* d_pol = nullptr;           // [N][6] polarisation + quadrature axes, or NULL: x^, y^
     int split_nllg = 0;                // 0: unified RK45; n >= 1: operator-split comparison integrator, n LLG sub-steps per cavity step
     double* d_spec = nullptr;          // [spec_K][2N][2] Fourier sums, or NULL
+    DemagPlan* demag = nullptr;        // dipolar field by FFT convolution, or NULL: off (the paper's setting)
+    void* d_bdem = nullptr;            // [3][nc] dipolar field of the stage about to be evaluated
     bool graph_pdl = false;            // loop-body edges of the current graph are programmatic dependencies
 };
 
@@ -341,6 +344,7 @@ void decide_path(cav_sim* s) {
     const bool small_only = s->d_pol != nullptr || s->split_nllg > 0;
     s->use_block = block_ok && (s->kernel_path == CAV_PATH_BLOCK || s->kernel_path == CAV_PATH_AUTO || small_only);
     s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO || small_only);
+    if (s->demag) { s->use_block = s->use_coop = s->use_tma = false; return; }                 // dipolar field: generic stage kernels
     if (s->padded) { s->use_block = s->use_coop = false; s->use_tma = s->tma_eligible; }       // padded rows: TMA kernels only
     else if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
@@ -479,6 +483,7 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     A.partial = s->partial;
     A.partial_max = s->partial_max;
     A.spec = s->d_spec;
+    A.bdem = s->demag ? s->d_bdem : nullptr;
     A.cond_handle = handle;
     A.pstride = s->pstride;
     A.nx = s->grid.nx; A.ny = s->grid.ny; A.nz = s->grid.nz;
@@ -647,6 +652,11 @@ int build_graph(cav_sim* s) {
 
 int launch_stage(cav_sim* s, int stage, StageArgs& A) {
     double* trace = s->d_trace;
+    if (s->demag) {          // dipolar field of the state this stage is evaluated at, then the stage kernel that adds it
+        int rc = demag_apply(s->demag, A, stage, s->d_bdem, s->stream);
+        if (rc) { snprintf(s->cuda_err, sizeof(s->cuda_err), "demag_apply failed at stage %d", stage); return rc; }
+        s->host_launches += 5;
+    }
     if (s->use_tma) {
         void* tparams[] = {&A, &s->targs[stage], &trace};
         CK(cudaLaunchKernel(stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], s->stream));
@@ -805,6 +815,8 @@ int cav_destroy(cav_sim* s) {
     cudaFree(s->d_coop);
     cudaFree(s->d_pol);
     cudaFree(s->d_spec);
+    demag_destroy(s->demag);
+    cudaFree(s->d_bdem);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     if (s->h_flag) cudaFreeHost(s->h_flag);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -1015,6 +1027,27 @@ int cav_set_integrator(cav_sim* s, int integrator, int n_llg) {
     return CAV_OK;
 }
 
+int cav_set_demag(cav_sim* s, int on) {
+    if (!s) return CAV_E_ARG;
+    int rc = sync_pull(s);
+    if (rc) return rc;
+    if (!on) {
+        demag_destroy(s->demag);
+        s->demag = nullptr;
+    } else if (!s->demag) {
+        if (s->padded) return CAV_E_UNSUPPORTED;             // rows padded for the TMA path; the dipolar field runs on the generic kernels
+        if (s->d_pol != nullptr || s->split_nllg > 0) return CAV_E_UNSUPPORTED;      // those live in the small-grid kernel
+        if (!s->d_bdem) CK(cudaMalloc(&s->d_bdem, (size_t)3 * s->nc * s->esize));
+        rc = demag_create(&s->demag, s->grid.nx, s->grid.ny, s->grid.nz, s->grid.dx, s->grid.dy, s->grid.dz, s->prm.Ms,
+                          s->prm.n_sub, s->prm.precision == CAV_F32, s->stream, s->cuda_err, (int)sizeof(s->cuda_err));
+        if (rc) return rc;
+    }
+    s->graph_dirty = true;
+    s->h_ctrl->k1_valid = 0;             // dm/dt of the current state changes
+    s->last_run_block = false;
+    return push_ctrl(s);
+}
+
 int cav_set_spectrum(cav_sim* s, int n_bins, double omega_lo, double omega_hi) {
     if (!s || n_bins < 0 || (n_bins > 1 && !(omega_hi > omega_lo))) return CAV_E_ARG;
     int rc = sync_pull(s);
@@ -1179,7 +1212,7 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     CK(cudaGetLastError());
     s->host_launches++;
-    if (s->launch_mode == CAV_LAUNCH_GRAPH) {
+    if (s->launch_mode == CAV_LAUNCH_GRAPH && !s->demag) {
         if (s->graph_dirty || !s->exec[0] || !s->exec[1]) {
             int rc = build_graph(s);
             if (rc) return rc;

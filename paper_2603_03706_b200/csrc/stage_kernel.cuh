@@ -506,6 +506,15 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
             }
         }
 
+        // ---- optional dipolar field (off in the paper): computed before this launch by
+        //      an FFT convolution of this stage's state (demag.cuh), the same for both sublattices ----
+        P bdv[3];
+        const bool has_bd = A.bdem != nullptr;
+        if (has_bd) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) bdv[c] = ldp<T, VEC>((const T*)A.bdem + (long long)c * nc + cell);
+        }
+
 #pragma unroll
         for (int s = 0; s < NSUB; ++s) {
             // ---- 6-neighbour exchange: sum over in-grid neighbours of (m_nb - m)/D^2 ----
@@ -571,6 +580,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
                 if constexpr (NSUB == 2) {
                     Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
                 }
+                if (has_bd) { Bx += bdv[0].v[v]; By += bdv[1].v[v]; Bz += bdv[2].v[v]; }
                 const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
                 const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
                 ks[0].v[v] = llg * (tx + alpha * dx);

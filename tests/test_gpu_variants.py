@@ -260,3 +260,91 @@ def test_spectrum_shows_both_polariton_branches(api):
     lo_peak = f[:K // 2][P[:K // 2].argmax()]
     hi_peak = f[K // 2:][P[K // 2:].argmax()]
     assert abs(lo_peak - (5e9 - g * 1e6)) < 3e6 and abs(hi_peak - (5e9 + g * 1e6)) < 3e6
+
+
+# ----------------------------------------------------------------------------------------
+# dipolar (demagnetising) field by FFT convolution (cav_set_demag; off in the paper)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,N,n_sub,dt", [
+    ((12, 6, 5), 2, 1, 0.1e-12),       # rows shorter than a warp, anisotropic cells (small_problem: 4 x 5 x 6 nm)
+    ((16, 16, 1), 1, 1, 0.1e-12),      # a film: no padding in z
+    ((13, 5, 3), 0, 1, 0.1e-12),       # odd sizes, plain LLG
+    ((8, 6, 4), 1, 2, 0.02e-12),       # two sublattices: the field of m_1 + m_2
+    ((1, 1, 1), 1, 1, 0.1e-12),        # one cell: the self term only
+])
+def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
+    """The FFT convolution against the oracle's direct O(N^2) sum with the Newell tensor: right-hand side cell by cell,
+    then 100 fixed steps."""
+    w = small_problem(*shape, N, n_sub)
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    o = oracle_of(w, demag=True)
+    dm_ref, da_ref, _ = o.rhs(w.m0, w.a0)
+    ref = o.run(w.m0, w.a0, fixed_dt=dt, max_steps=100)
+    with api.Sim(w, precision=prec) as sim:
+        api.cav_set_demag(sim.h, 1)
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_GENERIC
+        dm = np.empty(sim.shape_m, dtype=sim.np_dtype)
+        api.cav_get_dmdt(sim.h, dm)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=100)
+        m, a = sim.get_m(), sim.get_a()
+        st = api.cav_get_stats(sim.h)
+        # switching it off again restores the paper's field
+        api.cav_set_demag(sim.h, 0)
+        dm_off = np.empty(sim.shape_m, dtype=sim.np_dtype)
+        api.cav_get_dmdt(sim.h, dm_off)
+    assert st["accepted"] == 100 and st["rhs_evals"] == 601
+    scale = np.abs(dm_ref).max()
+    assert np.abs(dm - dm_ref).max() <= (5e-13 if prec == "f64" else 3e-5) * scale
+    assert_parity(m, a, ref, prec)
+    plain = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=100)
+    assert np.abs(plain.m - ref.m).max() > 1e-4                       # mu0 Ms = 0.18 T: not a detail
+    dm_plain, _, _ = oracle_of(w).rhs(ref.m, ref.a)
+    assert np.abs(dm_off - dm_plain).max() <= (1e-9 if prec == "f64" else 1e-3) * np.abs(dm_plain).max()
+
+
+def test_demag_adaptive_platelet_kittel_shift(api):
+    """A 24 x 24 x 1 film of flat cells magnetised along its normal: with the dipolar field on, the uniform mode precesses
+    well below gamma B0 (thin-film Kittel shift ~ mu0 Ms); GPU and oracle traces agree on the frequency to 1e-4."""
+    from observables import fit_exponentials, dominant
+    w = W.macrospin(10.0, [5.0], 0.0, 0.0, alpha=0.0, tilt=0.01, n=2)
+    w.nx = w.ny = 24; w.nz = 1
+    w.dx = w.dy = 5e-9; w.dz = 2e-9
+    w.u = np.ones((1, 1, 24, 24))
+    w.m0 = np.broadcast_to(w.m0[:, :, :1, :1, :1], (1, 3, 1, 24, 24)).copy()
+    t_end, sdt = 0.4e-9, 2e-12
+    cap = int(round(t_end / sdt))
+    ref = oracle_of(w, demag=True).run(w.m0, w.a0, t_end=t_end, tol=1e-8, sample_dt=sdt, trace_cap=cap)
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_set_demag(sim.h, 1)
+        api.cav_set_trace(sim.h, sdt, cap)
+        api.cav_run(sim.h, t_end, tol=1e-8)
+        tr = api.cav_get_trace(sim.h)
+    f = []
+    for t in (tr, ref.trace):
+        mu = t[:, 1 + 4] - 1j * t[:, 2 + 4]                           # <m_x> - i <m_y>
+        om, amp = fit_exponentials(mu, sdt, 2)
+        f.append(dominant(om, amp, 1)[0][0].real)
+    assert abs(f[0] / f[1] - 1) < 1e-4
+    assert f[0] < 0.75 * GAMMA_B0(w)
+
+
+def GAMMA_B0(w):
+    return 1.76e11 * w.B0[2]
+
+
+def test_demag_limits(api):
+    w = small_problem(16, 8, 4, 2, 1)
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_set_polarisation(sim.h, [[0, 1, 0], [1, 0, 0]])
+        with pytest.raises(api.CavError) as e:
+            api.cav_set_demag(sim.h, 1)
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+    with api.Sim(w, precision="f64") as sim:
+        api.cav_set_demag(sim.h, 1)
+        with pytest.raises(api.CavError) as e:
+            api.cav_set_polarisation(sim.h, [[0, 1, 0], [1, 0, 0]])
+        assert e.value.status == api.CAV_E_UNSUPPORTED
