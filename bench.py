@@ -671,6 +671,88 @@ def run_concurrent_sweep(args):
 # ----------------------------------------------------------------------------------------
 # --full-run: the configuration exactly as BASELINE.json states it, from t = 0 to its t_end
 # ----------------------------------------------------------------------------------------
+def run_joint_sweep(args):
+    """BASELINE.json configs[1] at its 41 field values through cav_sweep_run: ONE device-side loop over all 41
+    simulations - their plane-tiles form one work list for the persistent TMA grid, every simulation keeps its own step
+    size and accept/reject decisions."""
+    import torch
+    import cavmag_workloads as W
+    from paper_2603_03706_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    ghz = W.cfg2_sweep_ghz()
+    ws = [W.cfg2(f_kittel_ghz=float(f), seed=2000 + i) for i, f in enumerate(ghz)]
+    stream = torch.cuda.Stream()
+    sims = [api.Sim(w, precision="f32", stream=stream.cuda_stream) for w in ws]
+    sw = api.cav_sweep_create(sims)
+    tol, nc, N = ws[0].tol, ws[0].n_cells, ws[0].n_modes
+
+    def run_all(k):
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        api.cav_sweep_run(sw, math.inf, tol=tol, max_steps=k)
+        ev1.record(stream)
+        stream.synchronize()
+        return ev0.elapsed_time(ev1)
+
+    run_all(args.spinup)
+    run_all(max(args.warmup, 3))
+    st0 = [api.cav_get_stats(s.h) for s in sims]
+    sampler = ClockSampler(torch.cuda.current_device())
+    torch.cuda.synchronize()
+    sampler.start()
+    ms = run_all(args.steps)
+    clocks = sampler.stop()
+    st1 = [api.cav_get_stats(s.h) for s in sims]
+    rep_ms = [run_all(args.steps) for _ in range(args.repeats)]
+    evals = sum(b["rhs_evals"] - a["rhs_evals"] for a, b in zip(st0, st1))
+    sim_t = sum(b["t"] - a["t"] for a, b in zip(st0, st1))
+    assert evals == 6 * args.steps * len(sims), evals
+    # e2e: host buffers of all simulations every step
+    k_e2e = min(args.e2e_steps, 20)
+    hosts = [torch.empty(s.shape_m, dtype=torch.float32).pin_memory() for s in sims]
+    for s, hbuf in zip(sims, hosts):
+        api.cav_get_m(s.h, hbuf)
+    a_hosts = [api.cav_get_a(s.h, N) for s in sims]
+    se0 = [api.cav_get_stats(s.h) for s in sims]
+    t0 = time.perf_counter()
+    for _ in range(k_e2e):
+        for i, s in enumerate(sims):
+            api.cav_set_m(s.h, hosts[i]); api.cav_set_a(s.h, a_hosts[i])
+        api.cav_sweep_run(sw, math.inf, tol=tol, max_steps=1)
+        for i, s in enumerate(sims):
+            api.cav_get_m(s.h, hosts[i]); a_hosts[i] = api.cav_get_a(s.h, N)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    se1 = [api.cav_get_stats(s.h) for s in sims]
+    e2e_evals = sum(b["rhs_evals"] - a["rhs_evals"] for a, b in zip(se0, se1))
+    api.cav_sweep_destroy(sw)
+    for s in sims:
+        s.close()
+    value = nc * evals / (ms * 1e-3)
+    bytes_per_cs = algorithmic_bytes_per_cell_step(N, 1, 4) / 6.0
+    achieved = value * bytes_per_cs / 1e9
+    peak, peak_src = hbm_peak()
+    io = int(np.prod(sims[0].shape_m)) * 4 * len(sims) + 16 * N * len(sims)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "cfg2_sweep_joint", "grid": [ws[0].nx, ws[0].ny, ws[0].nz], "cells": nc, "simulations": len(sims),
+                       "modes": N, "mode": "adaptive RK45; 41 simulations in one device-side loop (cav_sweep_run)", "tol": tol,
+                       "l2": "41 x 8.7 MB of cell fields = 355 MB in total exceeds the 126 MB L2"},
+            "sim_ns_per_s": sim_t * 1e9 / (ms * 1e-3), "clocks": clocks,
+            "e2e": {"value": nc * e2e_evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": io, "d2h_bytes_per_step": io,
+                    "steps": k_e2e, "ms_per_step": 1e3 * e2e_s / k_e2e},
+            "gpu_launches": 6 * args.steps + 4 + len(sims),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "kernel": "cavmag::k_stage_tma_sweep (joint launch over 41 simulations)"}}
+    if rep_ms:
+        med = statistics.median(rep_ms)
+        line["repeats"] = {"n": len(rep_ms), "ms_per_step_median": med / args.steps, "roofline_frac_median": achieved / peak * ms / med}
+    print(json.dumps(line), flush=True)
+
+
 def run_full(args):
     """Time to solution of one BASELINE.json config (adaptive tol, its own duration): ONE cav_run call = one launch of the
     device-side step loop; wall time by CUDA events; |m| = 1, finiteness and the step statistics are checked."""
@@ -738,6 +820,8 @@ def main():
         run_batch(args)
     elif args.workload == "cfg2_sweep":
         run_concurrent_sweep(args)
+    elif args.workload == "cfg2_sweep_joint":
+        run_joint_sweep(args)
     else:
         run_cuda(args)
 

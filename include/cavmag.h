@@ -315,6 +315,24 @@ int cav_batch_get_a(cav_batch* b, double* a_out /* [n_rep][N][2] */);
 int cav_batch_get_stats(cav_batch* b, cav_stats* out /* [n_rep] */);
 int cav_batch_get_trace(cav_batch* b, double* out /* [n_rep][capacity][row_len] */, int* n_samples /* [n_rep] */);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * Sweeps of mid-size grids: several simulations in one launch (the paper's 41-point field sweep, PAPER.md:229, :335,
+ * on grids that are too large for cav_batch and too small to fill the GPU alone, e.g. 64 x 64 x 16 cells).
+ * A sweep is a joint LAUNCHER over ordinary cav_sim handles: create and configure every simulation as usual (same grid,
+ * precision, material and cell constants and number of modes; ferromagnet; at most 8 modes; B0, mode parameters, profiles
+ * and state may differ; all on the same stream), then cav_sweep_run advances all of them in ONE device-side loop: the
+ * plane-tiles of all simulations form one work list for the persistent TMA grid, and every simulation keeps its own step
+ * size, accept/reject decisions, trace and statistics.  Afterwards every cav_get_* / cav_set_* call works on the single
+ * handles as before; results are the same as running each simulation alone up to the summation order of the overlap sums.
+ * Do not run a member simulation while a sweep run is in flight; create the sweep after cav_set_modes (it is re-planned
+ * automatically when traces / spectra are re-allocated).  CAV_E_UNSUPPORTED when the TMA path is not eligible.
+ * --------------------------------------------------------------------------------------------------------- */
+typedef struct cav_sweep cav_sweep; /* opaque */
+int cav_sweep_create(cav_sim* const* sims, int n, cav_sweep** out);
+int cav_sweep_destroy(cav_sweep* sweep);
+/* Arguments as cav_run_steps, applied to every simulation.  Asynchronous on the simulations' stream. */
+int cav_sweep_run(cav_sweep* sweep, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps);
+
 const char* cav_strerror(int status);
 const char* cav_last_cuda_error(cav_sim* sim);
 const char* cav_version(void);

@@ -102,6 +102,9 @@ _SIGS = {
     "cav_strerror": ([_i], C.c_char_p),
     "cav_last_cuda_error": ([_vp], C.c_char_p),
     "cav_version": ([], C.c_char_p),
+    "cav_sweep_create": ([C.POINTER(_vp), _i, C.POINTER(_vp)], _i),
+    "cav_sweep_destroy": ([_vp], _i),
+    "cav_sweep_run": ([_vp, _d, _d, _d, _d, _ll], _i),
     "cav_batch_create": ([C.POINTER(cav_grid), C.POINTER(cav_params), _i, C.POINTER(_vp)], _i),
     "cav_batch_destroy": ([_vp], _i),
     "cav_batch_set_stream": ([_vp, _vp], _i),
@@ -413,6 +416,26 @@ class Sim:
 
     def get_a(self) -> np.ndarray:
         return cav_get_a(self.h, self.N)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Sweeps of mid-size grids: a joint launcher over ordinary handles
+# ---------------------------------------------------------------------------------------------------------
+def cav_sweep_create(sims) -> int:
+    """sims: sequence of cav_sim handles (ints) or Sim objects."""
+    hs = [getattr(x, "h", x) for x in sims]
+    arr = (_vp * len(hs))(*hs)
+    out = _vp()
+    _check(_lib.cav_sweep_create(arr, len(hs), C.byref(out)), "cav_sweep_create")
+    return out.value
+
+
+def cav_sweep_destroy(sweep) -> None:
+    _check(_lib.cav_sweep_destroy(sweep), "cav_sweep_destroy")
+
+
+def cav_sweep_run(sweep, t_end: float, tol: float = 0.0, fixed_dt: float = 0.0, dt_init: float = 0.0, max_steps: int = 0) -> None:
+    _check(_lib.cav_sweep_run(sweep, float(t_end), float(tol), float(fixed_dt), float(dt_init), int(max_steps)), "cav_sweep_run")
 
 
 # ---------------------------------------------------------------------------------------------------------

@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include <cuda.h>      // CUtensorMap types only; the encoder is fetched with cudaGetDriverEntryPoint
 
@@ -98,7 +99,11 @@ namespace {
 
 // ---- small kernels around the stage kernels -------------------------------------------------
 
+__device__ void setrun_body(Ctrl* c, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps);
 __global__ void k_setrun(Ctrl* c, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
+    setrun_body(c, t_end, tol, fixed_dt, dt_init, max_steps);
+}
+__device__ void setrun_body(Ctrl* c, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
     c->t_end = t_end;
     c->tol = tol;
     c->adaptive = tol > 0.0 ? 1 : 0;
@@ -117,7 +122,21 @@ __global__ void k_setrun(Ctrl* c, double t_end, double tol, double fixed_dt, dou
 
 // First node of the run graph: decides whether there is anything to do, fixes h for the first
 // step and the mode amplitudes / RF weights of the first kernel, arms the WHILE condition.
-__global__ void k_begin(Ctrl* c, Ctrl* c0, unsigned long long handle) {
+__device__ void begin_body(Ctrl* c, Ctrl* c0, unsigned long long handle);
+
+__global__ void k_begin(Ctrl* c, Ctrl* c0, unsigned long long handle) { begin_body(c, c0, handle); }
+
+// joint launch: one block per simulation, then the WHILE condition = "any simulation has something to do"
+__global__ void k_sweep_setrun(const RepPtrs* reps, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps);
+__global__ void k_sweep_begin(const RepPtrs* reps) { begin_body(reps[blockIdx.x].ctrl, reps[blockIdx.x].ctrl0, 0ull); }
+__global__ void k_sweep_cond(const RepPtrs* reps, int R, unsigned int* live, unsigned long long handle) {
+    unsigned int any = 0u;
+    for (int r = 0; r < R; ++r) any |= reps[r].ctrl->done ? 0u : 1u;
+    *live = 0u;
+    cudaGraphSetConditional((cudaGraphConditionalHandle)handle, any);
+}
+
+__device__ void begin_body(Ctrl* c, Ctrl* c0, unsigned long long handle) {
     const int tid = threadIdx.x;
     if (tid == 0) {
         c->done = (!(c->t < c->t_end) || c->status != 0) ? 1 : 0;
@@ -172,6 +191,10 @@ __global__ void k_sum_u(const T* __restrict__ u, long long nc, double* __restric
         __syncthreads();
     }
     if (threadIdx.x == 0) out[n * gridDim.x + blockIdx.x] = sh[0];
+}
+
+__global__ void k_sweep_setrun(const RepPtrs* reps, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
+    setrun_body(reps[blockIdx.x].ctrl, t_end, tol, fixed_dt, dt_init, max_steps);
 }
 
 const void* stage_tma_fn(const cav_sim* s, int stage) {
@@ -1318,6 +1341,207 @@ int cav_get_launch_count(cav_sim* s, long long* n) {
     int rc = sync_pull(s);
     if (rc) return rc;
     *n = s->host_launches + s->h_ctrl->rhs_evals;
+    return CAV_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Joint launch of several simulations of the same shape (cavmag.h "Sweeps of mid-size grids")
+ * --------------------------------------------------------------------------------------------------------- */
+struct cav_sweep {
+    std::vector<cav_sim*> sims;
+    cudaStream_t stream = nullptr;
+    RepPtrs* d_reps = nullptr;
+    unsigned int* d_live = nullptr;
+    std::vector<RepPtrs> h_reps;
+    cudaGraph_t graph[2] = {nullptr, nullptr};
+    cudaGraphExec_t exec[2] = {nullptr, nullptr};
+    TmaArgs targs[8];
+    size_t tsmem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int tgrid = 0;
+    char cuda_err[256] = {0};
+};
+
+namespace {
+
+void sweep_fill_reps(cav_sweep* w) {
+    w->h_reps.resize(w->sims.size());
+    for (size_t r = 0; r < w->sims.size(); ++r) {
+        cav_sim* q = w->sims[r];
+        RepPtrs& p = w->h_reps[r];
+        memset(&p, 0, sizeof(p));
+        p.ctrl = q->d_ctrl; p.ctrl0 = q->d_ctrl0;
+        for (int i = 0; i < 2; ++i) { p.Y[i] = q->Y[i]; p.MS[i] = q->MS[i]; }
+        for (int i = 0; i < 7; ++i) p.K[i] = q->K[i];
+        p.u = q->u; p.partial = q->partial; p.partial_max = q->partial_max; p.spec = q->d_spec; p.trace = q->d_trace;
+        p.maps = q->d_maps;
+        for (int i = 0; i < 3; ++i) p.B0[i] = q->prm.B0[i];
+    }
+}
+
+void sweep_destroy_graphs(cav_sweep* w) {
+    for (int i = 0; i < 2; ++i) {
+        if (w->exec[i]) { cudaGraphExecDestroy(w->exec[i]); w->exec[i] = nullptr; }
+        if (w->graph[i]) { cudaGraphDestroy(w->graph[i]); w->graph[i] = nullptr; }
+    }
+}
+
+const void* stage_tma_sweep_fn(const cav_sim* q, int stage) {
+    return q->prm.precision == CAV_F32 ? stage_tma_sweep_kernel_f32(stage, q->nb) : stage_tma_sweep_kernel_f64(stage, q->nb);
+}
+
+// k_sweep_begin -> K1 of every simulation (ordinary launches; they return at once when FSAL's k1 is valid) -> k_sweep_cond
+//   -> WHILE { joint K2 .. K7 [x unroll] } -> joint K2 (finishes the last step)
+int sweep_build_graph(cav_sweep* w, int which, int unroll) {
+    cav_sim* s = w->sims[0];                 // CK() reports into the first simulation's error text
+    const int R = (int)w->sims.size();
+    CK(cudaGraphCreate(&w->graph[which], 0));
+    cudaGraph_t graph = w->graph[which];
+    cudaGraphConditionalHandle handle;
+    CK(cudaGraphConditionalHandleCreate(&handle, graph, 0, cudaGraphCondAssignDefault));
+    unsigned long long h64 = (unsigned long long)handle;
+    const RepPtrs* reps = w->d_reps;
+    unsigned int* live = w->d_live;
+    cudaGraphNode_t prev, node;
+    {
+        void* params[] = {(void*)&reps};
+        int rc = add_kernel(s, graph, &prev, nullptr, (const void*)k_sweep_begin, dim3(R), dim3(64), params, 0);
+        if (rc) return rc;
+    }
+    std::vector<StageArgs> A1(R);
+    for (int r = 0; r < R; ++r) {
+        cav_sim* q = w->sims[r];
+        A1[r] = make_args(q, 0ull);
+        double* trace = q->d_trace;
+        void* tparams[] = {&A1[r], &q->targs[1], &trace};
+        int rc = add_kernel(s, graph, &node, &prev, stage_tma_fn(q, 1), dim3(q->tgrid), dim3(kTmaThreads), tparams, q->tsmem[1]);
+        if (rc) return rc;
+        prev = node;
+    }
+    {
+        int Rv = R;
+        void* params[] = {(void*)&reps, &Rv, &live, &h64};
+        int rc = add_kernel(s, graph, &node, &prev, (const void*)k_sweep_cond, dim3(1), dim3(1), params, 0);
+        if (rc) return rc;
+        prev = node;
+    }
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = handle;
+    cp.conditional.type = cudaGraphCondTypeWhile;
+    cp.conditional.size = 1;
+    cudaGraphNode_t n_while;
+    CK(cudaGraphAddNode(&n_while, graph, &prev, 1, &cp));
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    StageArgs A = make_args(s, 0ull);
+    SweepArgs SW;
+    SW.reps = w->d_reps; SW.R = R; SW.live = w->d_live; SW.cond_handle = h64;
+    const bool pdl = s->want_pdl;
+    for (int u = 0; u < unroll; ++u)
+        for (int stage = 2; stage <= 7; ++stage) {
+            void* tparams[] = {&A, &w->targs[stage], &SW};
+            const cudaGraphNode_t* dep = (u == 0 && stage == 2) ? nullptr : &prev;
+            int rc = add_kernel(s, body, &node, dep, stage_tma_sweep_fn(s, stage), dim3(w->tgrid), dim3(kTmaThreads), tparams, w->tsmem[stage], pdl);
+            if (rc) return rc;
+            prev = node;
+        }
+    {
+        void* tparams[] = {&A, &w->targs[2], &SW};
+        int rc = add_kernel(s, graph, &node, &n_while, stage_tma_sweep_fn(s, 2), dim3(w->tgrid), dim3(kTmaThreads), tparams, w->tsmem[2]);
+        if (rc) return rc;
+    }
+    CK(cudaGraphInstantiate(&w->exec[which], graph, 0));
+    CK(cudaGraphUpload(w->exec[which], w->stream));
+    return CAV_OK;
+}
+
+}  // namespace
+
+int cav_sweep_create(cav_sim* const* sims, int n, cav_sweep** out) {
+    if (!sims || !out || n < 1) return CAV_E_ARG;
+    *out = nullptr;
+    cav_sim* s = sims[0];
+    if (!s) return CAV_E_ARG;
+    for (int r = 0; r < n; ++r) {
+        cav_sim* q = sims[r];
+        if (!q || !q->m_set) return q ? CAV_E_STATE : CAV_E_ARG;
+        if (q->grid.nx != s->grid.nx || q->grid.ny != s->grid.ny || q->grid.nz != s->grid.nz || q->prm.precision != s->prm.precision ||
+            q->N != s->N || q->stream != s->stream || q->prm.renormalize != s->prm.renormalize)
+            return CAV_E_ARG;
+        // the joint kernels take the material and cell constants from simulation 0: only B0, the modes and the state may differ
+        if (q->grid.dx != s->grid.dx || q->grid.dy != s->grid.dy || q->grid.dz != s->grid.dz || q->prm.Ms != s->prm.Ms ||
+            q->prm.Aex != s->prm.Aex || q->prm.Ku != s->prm.Ku || q->prm.alpha != s->prm.alpha || q->prm.gamma != s->prm.gamma ||
+            memcmp(q->prm.ku_axis, s->prm.ku_axis, sizeof(s->prm.ku_axis)) != 0)
+            return CAV_E_ARG;
+        if (q->prm.n_sub != 1 || !q->tma_eligible || q->demag || q->d_pol || q->split_nllg > 0 || q->nb > 8) return CAV_E_UNSUPPORTED;
+        for (int r2 = 0; r2 < r; ++r2) if (sims[r2] == q) return CAV_E_ARG;
+    }
+    if (s->targs[1].Q * (long long)n < (long long)s->n_sm) return CAV_E_UNSUPPORTED;      // not enough plane-tiles for a persistent grid
+    cav_sweep* w = new (std::nothrow) cav_sweep();
+    if (!w) return CAV_E_NOMEM;
+    w->sims.assign(sims, sims + n);
+    w->stream = s->stream;
+    w->tgrid = s->n_sm;
+    for (int stage = 1; stage <= 7; ++stage) {
+        w->targs[stage] = s->targs[stage];
+        w->targs[stage].pre_k = 0;           // a joint launch fetches nothing before the dependency wait
+        w->targs[stage].pre_ctrl = 0;
+        w->tsmem[stage] = s->tsmem[stage];
+        if (stage >= 2) {
+            const void* fn = stage_tma_sweep_fn(s, stage);
+            if (!fn) { delete w; return CAV_E_UNSUPPORTED; }
+            cudaFuncAttributes fa;
+            if (cudaFuncGetAttributes(&fa, fn) != cudaSuccess ||
+                cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(s->smem_optin - fa.sharedSizeBytes)) != cudaSuccess ||
+                w->tsmem[stage] + fa.sharedSizeBytes > s->smem_optin) {
+                cudaGetLastError();
+                delete w;
+                return CAV_E_UNSUPPORTED;
+            }
+        }
+    }
+    if (cudaMalloc(&w->d_reps, sizeof(RepPtrs) * n) != cudaSuccess || cudaMalloc(&w->d_live, sizeof(unsigned int)) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(w->d_reps); cudaFree(w->d_live); delete w;
+        return CAV_E_NOMEM;
+    }
+    *out = w;
+    return CAV_OK;
+}
+
+int cav_sweep_destroy(cav_sweep* w) {
+    if (!w) return CAV_E_ARG;
+    if (w->stream) cudaStreamSynchronize(w->stream);
+    sweep_destroy_graphs(w);
+    cudaFree(w->d_reps); cudaFree(w->d_live);
+    cudaGetLastError();
+    delete w;
+    return CAV_OK;
+}
+
+int cav_sweep_run(cav_sweep* w, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps) {
+    if (!w) return CAV_E_ARG;
+    const bool adaptive = tol > 0.0;
+    if (adaptive == (fixed_dt > 0.0)) return CAV_E_ARG;
+    if (std::isnan(t_end) || max_steps < 0 || (std::isinf(t_end) && max_steps == 0)) return CAV_E_ARG;
+    cav_sim* s = w->sims[0];
+    // per-simulation pointers may have changed since the last run (trace, spectrum, mode profiles): refresh, and rebuild
+    // the graphs when anything the graph nodes hold by value did
+    std::vector<RepPtrs> old = w->h_reps;
+    sweep_fill_reps(w);
+    const bool changed = old.size() != w->h_reps.size() || memcmp(old.data(), w->h_reps.data(), sizeof(RepPtrs) * old.size()) != 0;
+    CK(cudaMemcpyAsync(w->d_reps, w->h_reps.data(), sizeof(RepPtrs) * w->h_reps.size(), cudaMemcpyHostToDevice, w->stream));
+    CK(cudaStreamSynchronize(w->stream));
+    if (changed || !w->exec[0] || !w->exec[1]) {
+        sweep_destroy_graphs(w);
+        int rc = sweep_build_graph(w, 0, 1);
+        if (rc == CAV_OK) rc = sweep_build_graph(w, 1, kLoopUnroll);
+        if (rc) { sweep_destroy_graphs(w); return rc; }
+    }
+    const int R = (int)w->sims.size();
+    k_sweep_setrun<<<R, 1, 0, w->stream>>>(w->d_reps, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
+    CK(cudaGetLastError());
+    const int which = (max_steps == 0 || max_steps >= kUnrollMinSteps) ? 1 : 0;
+    CK(cudaGraphLaunch(w->exec[which], w->stream));
+    for (cav_sim* q : w->sims) { q->last_run_block = false; q->host_launches += 2; }
     return CAV_OK;
 }
 

@@ -147,7 +147,8 @@ constexpr int kCtrlWordsPerConsumer = (kCtrlWords + kTmaConsumers - 1) / kTmaCon
 
 template <int PREV, int NB>
 __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __restrict__ gctrl, const int tidc,
-                                                unsigned long long* sc_words, double* sred) {
+                                                unsigned long long* sc_words, double* sred, const int nblk, const bool owner) {
+    // nblk blocks wrote partial sums for this simulation (slots 0..nblk-1); `owner` is the one that writes results back
     // one batch of independent loads: the whole Ctrl (a few words per thread) and all 2*NB x gridDim block partials
     // (rows of modes >= N hold stale values that nothing reads)
     const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(gctrl);
@@ -158,7 +159,7 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
         cw[k] = idx < kCtrlWords ? __ldcg(gcw + idx) : 0ull;
     }
     if constexpr (NB > 0)
-        reduce_block_partials(stage_partials(A, PREV), A.pstride, 2 * NB, (int)gridDim.x, tidc >> 5, kTmaTY, tidc & 31, sred);
+        reduce_block_partials(stage_partials(A, PREV), A.pstride, 2 * NB, nblk, tidc >> 5, kTmaTY, tidc & 31, sred);
 #pragma unroll
     for (int k = 0; k < kCtrlWordsPerConsumer; ++k) {
         const int idx = tidc + k * kTmaConsumers;
@@ -178,7 +179,7 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
         if (tidc < c->N) {
             const int n = tidc;
             mode_ode_stage<PREV>(c, n, sred, nullptr);
-            if (blockIdx.x == 0) {
+            if (owner) {
                 constexpr int nxt = (PREV + 1) & 1;
                 gctrl->S[n][0] = c->S[n][0]; gctrl->S[n][1] = c->S[n][1];
                 gctrl->ka[PREV - 1][n][0] = c->ka[PREV - 1][n][0]; gctrl->ka[PREV - 1][n][1] = c->ka[PREV - 1][n][1];
@@ -189,14 +190,14 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
         }
         if (tidc == 0) {
             c->rhs_evals++;                             // evaluation PREV is complete
-            if (blockIdx.x == 0) gctrl->rhs_evals = c->rhs_evals;
+            if (owner) gctrl->rhs_evals = c->rhs_evals;
         }
     }
     if constexpr (PREV == 6) {
         // The stage-7 kernel hands the step over to the next stage-2 kernel through the boundary copy: block 0 stores
         // its whole working copy there (also when the run is over, so that both instances end up equal).  No block of
         // THIS kernel reads ctrl0, and the stage-2 kernel starts after this one has completed.
-        if (blockIdx.x == 0) {
+        if (owner) {
             asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
             unsigned long long* const g0 = reinterpret_cast<unsigned long long*>(A.ctrl0);
             for (int idx = tidc; idx < kCtrlWords; idx += kTmaConsumers) g0[idx] = sc_words[idx];
@@ -220,7 +221,10 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
 // bar.sync there).  Returns false when the run is over.
 template <int NB, int NSUB>
 __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaArgs& TA, const int tidc,
-                                                 unsigned long long* sc_words, double* sred, double* serr, double* trace) {
+                                                 unsigned long long* sc_words, double* sred, double* serr, double* trace,
+                                                 const int nblk, const bool owner, unsigned int* live_count) {
+    // live_count != nullptr (joint launch of several simulations): the owner reports "this simulation goes on" there
+    // instead of setting the WHILE condition itself
     const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(A.ctrl0);
     unsigned long long cw[kCtrlWordsPerConsumer];
 #pragma unroll
@@ -231,9 +235,9 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     const int N = TA.N, warp = tidc >> 5, lane = tidc & 31;
     const int nsum = 2 * N + 3 * NSUB;
     // warps 0..6 sum the partials, warp 7 takes the error maxima (stale values when no stage 7 is pending: not used)
-    if (warp < kTmaTY - 1) reduce_block_partials(stage_partials(A, 7), A.pstride, nsum, (int)gridDim.x, warp, kTmaTY - 1, lane, sred);
+    if (warp < kTmaTY - 1) reduce_block_partials(stage_partials(A, 7), A.pstride, nsum, nblk, warp, kTmaTY - 1, lane, sred);
     else {
-        const double mx = reduce_block_max(A.partial_max, (int)gridDim.x, lane);
+        const double mx = reduce_block_max(A.partial_max, nblk, lane);
         if (lane == 0) serr[kMaxModes] = mx;
     }
 #pragma unroll
@@ -243,7 +247,7 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     }
     asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
     Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
-    const bool write = blockIdx.x == 0;
+    const bool write = owner;
     if (c->done == 0 && c->pend7 != 0) {            // uniform over the block (and over the grid)
         if (tidc < N) mode_ode_stage<7>(c, tidc, sred, serr);
         asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
@@ -277,19 +281,41 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     if (write) {
         unsigned long long* const g1 = reinterpret_cast<unsigned long long*>(A.ctrl);
         for (int idx = tidc; idx < kCtrlWords; idx += kTmaConsumers) g1[idx] = sc_words[idx];
-        if (tidc == 0 && A.cond_handle != 0ull) {
+        if (tidc == 0) {
             // A run bounded by max_steps knows its last step when that step STARTS (rejected steps count): the loop can
             // stop after this body, and the stage-2 kernel that follows the WHILE node finishes the step.  A run bounded
             // by t_end only learns it from the controller: the condition then lags one iteration (empty kernels).
             const bool last = c->max_steps > 0 && c->steps_run + 1 >= c->max_steps;
-            cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, (live && !last) ? 1u : 0u);
+            if (live_count != nullptr) { if (live && !last) atomicAdd(live_count, 1u); }
+            else if (A.cond_handle != 0ull)
+                cudaGraphSetConditional((cudaGraphConditionalHandle)A.cond_handle, (live && !last) ? 1u : 0u);
         }
     }
     return live;
 }
 
-template <typename T, int STAGE, int NSUB, int NB>
-__global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A, const TmaArgs TA, double* __restrict__ trace) {
+// Joint launch of R independent simulations of the same shape (a field sweep of a mid-size grid): the
+// plane-tiles of all of them form ONE list that the persistent grid cuts into equal runs, so a block may work on (at
+// most a few) different simulations one after the other - a "sub-run" each, with that simulation's buffers, Ctrl, tensor
+// maps and partial-sum slots.  Every simulation keeps its own step size and accept/reject decisions.
+struct RepPtrs {
+    Ctrl* ctrl; Ctrl* ctrl0;
+    void* Y[2]; void* MS[2]; void* K[7];
+    const void* u;
+    double* partial; double* partial_max; double* spec; double* trace;
+    const unsigned char* maps;
+    double B0[3];
+};
+struct SweepArgs {
+    const RepPtrs* reps;            // [R] in device memory
+    int R;
+    unsigned int* live;             // simulations that go on after this step (stage 2 adds, stage 3 turns it into the WHILE condition)
+    unsigned long long cond_handle;
+};
+
+template <typename T, int STAGE, int NSUB, int NB, bool SWEEP>
+__device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs& TA, double* __restrict__ trace0, const SweepArgs& SW) {
+    static_assert(!(SWEEP && STAGE == 1), "stage 1 of a joint launch runs as one ordinary launch per simulation");
     constexpr int VEC = 8 / (int)sizeof(T);              // cells per lane: 2 floats / 1 double
     constexpr int TX = kTmaRowBytes / (int)sizeof(T);    // cells per tile row
     constexpr int HX = kTmaHaloBytes / (int)sizeof(T);   // x halo in cells (16 bytes: 4 floats / 2 doubles)
@@ -303,7 +329,6 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     using P = Pack<T, VEC>;
     const T* const tag = nullptr;
 
-    Ctrl* ctrl = A.ctrl;
     if (threadIdx.x == 0) CAVMAG_MARK(0);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[6 * kTmaMaxDepth];
@@ -357,17 +382,59 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
     __shared__ double s_err[STAGE == 2 ? kMaxModes + 2 : 1];      // stage 2: mode errors, max |e|^2, accept flag
 
     // this CTA's run of plane-tiles; tile coordinates are advanced incrementally (no divisions in the loops)
-    const long long q0 = (TA.Q * (long long)blockIdx.x) / gridDim.x;
-    const long long q1 = (TA.Q * (long long)(blockIdx.x + 1)) / gridDim.x;
-    const int nplanes = (int)(q1 - q0);
+    const long long Qtot = SWEEP ? TA.Q * (long long)SW.R : TA.Q;
+    const long long cq0 = (Qtot * (long long)blockIdx.x) / gridDim.x;
+    const long long cq1 = (Qtot * (long long)(blockIdx.x + 1)) / gridDim.x;
     // Sweep direction: odd stages walk their run backwards (cav_set_sweep_order), so a block starts stage s+1 on the
     // plane-tiles it finished stage s with - their stage state, slopes, y0 and profiles are still in the 126 MB L2.
     const int dir = (A.serpentine && (STAGE & 1)) ? -1 : 1;
     const int zfirst = dir > 0 ? 0 : nz - 1, zlast = dir > 0 ? nz - 1 : 0;
-    const long long qs = dir > 0 ? q0 : q1 - 1;
-    const long long t0 = qs / nz;
-    const int z0 = (int)(qs - t0 * nz);
-    const int tx0 = (int)(t0 % TA.ntx), ty0 = (int)(t0 / TA.ntx);
+    // sub-runs: one per simulation this block's run touches (exactly one without SWEEP)
+    const int r_lo = SWEEP ? (int)(cq0 / TA.Q) : 0;
+    const int r_hi = SWEEP ? (cq1 > cq0 ? (int)((cq1 - 1) / TA.Q) : r_lo - 1) : 0;
+    const int nsr = SWEEP ? r_hi - r_lo + 1 : 1;
+    StageArgs Arep;                                  // SWEEP: the arguments of the current simulation
+    double* trace = trace0;
+    const unsigned char* rep_maps = TA.maps;
+    long long ql0 = cq0, ql1 = cq1;                  // the sub-run, in plane-tiles of its own simulation
+    int slot = (int)blockIdx.x, nblk_r = (int)gridDim.x;       // this block's partial-sum slot / blocks working on the simulation
+    int nplanes = 0, z0 = 0, tx0 = 0, ty0 = 0;                 // the sub-run: length and first plane-tile in sweep order
+    auto set_geometry = [&]() {                                // (64-bit divisions: once per block, not once per role)
+        nplanes = (int)(ql1 - ql0);
+        const long long qs = dir > 0 ? ql0 : ql1 - 1;
+        const long long t0 = qs / nz;
+        z0 = (int)(qs - t0 * nz);
+        tx0 = (int)(t0 % TA.ntx); ty0 = (int)(t0 / TA.ntx);
+    };
+    if constexpr (!SWEEP) set_geometry();
+    auto enter_subrun = [&](const int sr) {
+        if constexpr (SWEEP) {
+            const int r = dir > 0 ? r_lo + sr : r_hi - sr;
+            const long long base = (long long)r * TA.Q, G = gridDim.x;
+            ql0 = (cq0 > base ? cq0 : base) - base;
+            ql1 = (cq1 < base + TA.Q ? cq1 : base + TA.Q) - base;
+            long long bf = (base * G) / Qtot;                        // first block whose run reaches into simulation r
+            while ((Qtot * (bf + 1)) / G <= base) ++bf;
+            long long bl = ((base + TA.Q) * G - 1) / Qtot;           // last block whose run starts before its end
+            if (bl > G - 1) bl = G - 1;
+            while ((Qtot * bl) / G >= base + TA.Q) --bl;
+            slot = (int)((long long)blockIdx.x - bf);
+            nblk_r = (int)(bl - bf + 1);
+            const RepPtrs& rp = SW.reps[r];
+            Arep = A;
+            Arep.ctrl = rp.ctrl; Arep.ctrl0 = rp.ctrl0;
+            Arep.Y[0] = rp.Y[0]; Arep.Y[1] = rp.Y[1]; Arep.MS[0] = rp.MS[0]; Arep.MS[1] = rp.MS[1];
+#pragma unroll
+            for (int i = 0; i < 7; ++i) Arep.K[i] = rp.K[i];
+            Arep.u = rp.u; Arep.partial = rp.partial; Arep.partial_max = rp.partial_max; Arep.spec = rp.spec;
+            Arep.B0[0] = rp.B0[0]; Arep.B0[1] = rp.B0[1]; Arep.B0[2] = rp.B0[2];
+            Arep.cond_handle = 0ull;
+            trace = rp.trace;
+            rep_maps = rp.maps;
+            set_geometry();
+        }
+    };
+    const StageArgs& Aouter = A;
     // next plane-tile of the run in sweep order; returns true when the tile column changes
     auto advance = [&](int& z, int& tx, int& ty) -> bool {
         z += dir;
@@ -382,6 +449,12 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 
     if (warp == kTmaTY) {
         // =============================== TMA producer ===============================
+        int hm = 0, ha = 0, hu = 0;                 // ring heads, carried over the sub-runs
+        unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
+        for (int sr = 0; sr < nsr; ++sr) {
+            enter_subrun(sr);
+            const StageArgs& A = SWEEP ? Arep : Aouter;
+            Ctrl* const ctrl = A.ctrl;
         int done = 0;
         bool have_ctrl = false;
         if constexpr (STAGE == 1) {
@@ -394,9 +467,9 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 have_ctrl = true;
             }
         }
-        if (have_ctrl && done) return;
+        if (have_ctrl && done) return;             // (never in a joint launch: pre_ctrl is off there)
         const bool issuer = lane == 0 && nplanes > 0;
-        const unsigned char* maps = TA.maps;
+        const unsigned char* maps = rep_maps;
         auto mp = [&](int i) { return (const void*)(maps + 128 * i); };
         const void* hmap0 = nullptr;
         const void* hmap1 = nullptr;                    // STAGE 2 only
@@ -425,7 +498,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
         const int npre = (NAUX > 1) ? (TA.pre_k ? NAUX - 1 : (NAUX - 1 < 2 ? NAUX - 1 : 2)) : 0;   // aux fields fetched before the wait
         if constexpr (kPre) {
-            if (issuer) {
+            if (!SWEEP && issuer) {                 // (a joint launch fetches nothing before the wait)
                 int zz = z0, txx = tx0, tyy = ty0;
                 for (int p = 0; p < nplanes; ++p) {
                     const bool do_u = NB > 0 && pre_u + NCH <= Du;
@@ -460,7 +533,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
                 }
             }
             __syncwarp();
-            asm volatile("griddepcontrol.wait;" ::: "memory");
+            if (!SWEEP || sr == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
             CAVMAG_MARK(13);
             if constexpr (STAGE == 2) {
                 // the consumers have finished the previous step (deferred_finish7): verdict and buffer indices in s_ctrl
@@ -475,13 +548,11 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             if (done) {                             // the run is over: let the early profile loads land, then leave
                 if (issuer)
                     for (int i = 0; i < pre_u; ++i) mbar_wait(full_u + 8 * i, 0u);
-                return;
+                if constexpr (SWEEP) continue; else return;
             }
         }
         if (issuer) {
             int z = z0, tx = tx0, ty = ty0;
-            int hm = 0, ha = 0, hu = 0;                 // ring heads
-            unsigned pm = 1, pa = 1, pu = 1;            // parity to wait on for "empty" (first pass: passes immediately)
             auto issue_ms = [&](int x0, int y0, int zz) {
                 mbar_wait(empty_ms + 8 * hm, pm);
                 const unsigned bar = full_ms + 8 * hm;
@@ -531,19 +602,39 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
             }
             CAVMAG_MARK(6);
         }
+        }   // sub-runs
     } else {
         // ================================ consumers =================================
-        asm volatile("griddepcontrol.wait;" ::: "memory");
+        int hm = 0, ha = 0, hu = 0, tm = 0;          // ring heads (next slot to acquire) and the ms tail (next to release), carried over the sub-runs
+        unsigned pm = 0, pa = 0, pu = 0;             // parity to wait on for "full"
+        for (int sr = 0; sr < nsr; ++sr) {
+            enter_subrun(sr);
+            const StageArgs& A = SWEEP ? Arep : Aouter;
+            Ctrl* const ctrl = A.ctrl;
+        if (!SWEEP || sr == 0) {
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+            if constexpr (SWEEP && STAGE == 3) {
+                // the stage-2 kernel has completed: its owners have counted the simulations that go on
+                if (blockIdx.x == 0 && tid == 0) {
+                    const unsigned int v = atomicExch(SW.live, 0u);
+                    if (SW.cond_handle != 0ull) cudaGraphSetConditional((cudaGraphConditionalHandle)SW.cond_handle, v > 0u ? 1u : 0u);
+                }
+            }
+        }
         if (tid == 0) CAVMAG_MARK(15);
         double hd;
         if constexpr (STAGE == 2) {
             // finish stage 7 of the previous step, run the controller, start this step (all blocks, same bits)
-            if (!deferred_finish7<NB, NSUB>(A, TA, tid, s_ctrl, s_red, s_err, trace)) return;
+            if (!deferred_finish7<NB, NSUB>(A, TA, tid, s_ctrl, s_red, s_err, trace, nblk_r, slot == 0, SWEEP ? SW.live : nullptr)) {
+                if constexpr (SWEEP) continue; else return;
+            }
             const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
             N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot; hd = sc->h;
             if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
         } else if constexpr (kDeferred) {
-            if (!deferred_finish<STAGE - 1, NB>(A, ctrl, tid, s_ctrl, s_red)) return;
+            if (!deferred_finish<STAGE - 1, NB>(A, ctrl, tid, s_ctrl, s_red, nblk_r, slot == 0)) {
+                if constexpr (SWEEP) continue; else return;
+            }
             const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
             N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot; hd = sc->h;
             if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
@@ -588,8 +679,6 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         const unsigned arow = (unsigned)(warp * kTmaRowBytes + lane * 8);
 
         int z = z0, tx = tx0, ty = ty0;
-        int hm = 0, ha = 0, hu = 0, tm = 0;          // ring heads (next slot to acquire) and the ms tail (next to release)
-        unsigned pm = 0, pa = 0, pu = 0;             // parity to wait on for "full"
         unsigned sm_zm = 0, sm_zc = 0, sm_zp = 0;    // shared addresses of the live stage-state planes
         auto acquire_ms = [&]() -> unsigned {
             mbar_wait(full_ms + 8 * hm, pm);
@@ -890,15 +979,16 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 #pragma unroll
                 for (int w = 0; w < kTmaTY; ++w) acc += swarp[w][i];
                 const int comp = (i < 2 * NB) ? i : (2 * N + (i - 2 * NB));
-                stage_partials(A, STAGE)[(size_t)comp * A.pstride + blockIdx.x] = acc;
+                stage_partials(A, STAGE)[(size_t)comp * A.pstride + slot] = acc;
             }
         }
         if (STAGE == 7 && tid == 0) {
             double mx = 0.0;
 #pragma unroll
             for (int w = 0; w < kTmaTY; ++w) mx = fmax(mx, swmax[w]);
-            A.partial_max[blockIdx.x] = mx;
+            A.partial_max[slot] = mx;
         }
+        }   // sub-runs
     }
 
     // ---- stage 1 (k1 of a fresh state, once per run at most): last-block-done -> second reduction pass, mode ODE,
@@ -909,6 +999,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
         // (release); the last block's thread 0 fences again after the ticket (acquire) before the barrier that
         // lets its threads read the other blocks' partials.
         __shared__ int s_last;
+        Ctrl* const ctrl = A.ctrl;
         __syncthreads();
         if (tid == 0) {
             __threadfence();
@@ -930,6 +1021,43 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const StageArgs A,
 #endif
     }
 }
+
+template <typename T, int STAGE, int NSUB, int NB>
+__global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const __grid_constant__ StageArgs A, const __grid_constant__ TmaArgs TA,
+                                                              double* __restrict__ trace) {
+    stage_tma_body<T, STAGE, NSUB, NB, false>(A, TA, trace, SweepArgs{nullptr, 1, nullptr, 0ull});
+}
+
+// Joint launch over SW.R simulations of the same shape (ferromagnet): A carries the shared grid / material constants
+// (and simulation 0's pointers, unused), SW.reps the per-simulation pointers.
+template <typename T, int STAGE, int NB>
+__global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma_sweep(const __grid_constant__ StageArgs A, const __grid_constant__ TmaArgs TA,
+                                                                    const __grid_constant__ SweepArgs SW) {
+    stage_tma_body<T, STAGE, 1, NB, true>(A, TA, nullptr, SW);
+}
+
+const void* stage_tma_sweep_kernel_f32(int stage, int nb);
+const void* stage_tma_sweep_kernel_f64(int stage, int nb);
+
+#define CAVMAG_TMA_SWEEP_CASES(T, NB)                                              \
+    switch (stage) {                                                               \
+        case 2: return (const void*)k_stage_tma_sweep<T, 2, NB>;                   \
+        case 3: return (const void*)k_stage_tma_sweep<T, 3, NB>;                   \
+        case 4: return (const void*)k_stage_tma_sweep<T, 4, NB>;                   \
+        case 5: return (const void*)k_stage_tma_sweep<T, 5, NB>;                   \
+        case 6: return (const void*)k_stage_tma_sweep<T, 6, NB>;                   \
+        case 7: return (const void*)k_stage_tma_sweep<T, 7, NB>;                   \
+        default: return nullptr;                                                   \
+    }
+// the sweeps of the paper have 1-3 modes: mode buckets 0, 1, 2 and 8
+#define CAVMAG_DEFINE_TMA_SWEEP_LOOKUP(NAME, T)                                    \
+    const void* NAME(int stage, int nb) {                                          \
+        if (nb == 0) { CAVMAG_TMA_SWEEP_CASES(T, 0) }                              \
+        if (nb == 1) { CAVMAG_TMA_SWEEP_CASES(T, 1) }                              \
+        if (nb == 2) { CAVMAG_TMA_SWEEP_CASES(T, 2) }                              \
+        if (nb == 8) { CAVMAG_TMA_SWEEP_CASES(T, 8) }                              \
+        return nullptr;                                                            \
+    }
 
 const void* stage_tma_kernel_f32_fm(int stage, int nb);
 const void* stage_tma_kernel_f32_afm(int stage, int nb);
