@@ -302,16 +302,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                 lap[c] = l;
             }
             const T mx = ms[q][0], my = ms[q][1], mz = ms[q][2];
-            const T mk = mx * axx + my * axy + mz * axz;
-            T Bx = B0x + lap[0] + anp * mk * axx + brf;
-            T By = B0y + lap[1] + anp * mk * axy + brfy;
-            T Bz = B0z + lap[2] + anp * mk * axz + brfz;
+            T Bx, By, Bz;
+            material_field(mx, my, mz, lap[0], lap[1], lap[2], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
+            Bx += brf;
+            if (polar) { By += brfy; Bz += brfz; }
             if constexpr (NSUB == 2) { Bx -= BE * ms[1 - q][0]; By -= BE * ms[1 - q][1]; Bz -= BE * ms[1 - q][2]; }
-            const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
-            const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
-            k[q][0] = llg * (tx + alpha * dx);
-            k[q][1] = llg * (ty + alpha * dy);
-            k[q][2] = llg * (tz + alpha * dz);
+            llg_slope(mx, my, mz, Bx, By, Bz, alpha, llg, k[q][0], k[q][1], k[q][2]);
         }
         if constexpr (COOP)                                          // fixed-order sum over the blocks' slots (every block: same bits)
             reduce_block_partials(A.cpart[ev & 1], A.nblk, 2 * N + nsum_extra, A.nblk, warp, nwarp, lane, sh.red2);
@@ -402,20 +398,27 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         } else if (tid < N) batch_stage_state<1>(sh, tid, A.two_over_gamma);      // a_2 = a_0 + h a21 ka_1
         const T h = (T)sh.h;
 
-#define CAVMAG_BATCH_STAGE(S, EXPR)                                                        \
-        _Pragma("unroll") for (int q = 0; q < NSUB; ++q)                                   \
-        _Pragma("unroll") for (int c = 0; c < 3; ++c) ms[q][c] = y[q][c] + h * (EXPR);
-        CAVMAG_BATCH_STAGE(2, (T)kA[1][0] * k1[q][c])
+        // stage states m_s = m_0 + h sum_j a_sj k_j (dp_state<ROW>, stage_kernel.cuh) and their evaluations
+        auto stage_state = [&](auto row_tag, auto&&... kj) {
+            constexpr int ROW = decltype(row_tag)::value;
+#pragma unroll
+            for (int q = 0; q < NSUB; ++q)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const T kv[ROW] = {kj[q][c]...};
+                    ms[q][c] = dp_state<ROW>(y[q][c], kv, h);
+                }
+        };
+        stage_state(std::integral_constant<int, 1>{}, k1);
         eval(std::integral_constant<int, 2>{}, ms, k2);
-        CAVMAG_BATCH_STAGE(3, ((T)kA[2][0] * k1[q][c] + (T)kA[2][1] * k2[q][c]))
+        stage_state(std::integral_constant<int, 2>{}, k1, k2);
         eval(std::integral_constant<int, 3>{}, ms, k3);
-        CAVMAG_BATCH_STAGE(4, (((T)kA[3][0] * k1[q][c] + (T)kA[3][1] * k2[q][c]) + (T)kA[3][2] * k3[q][c]))
+        stage_state(std::integral_constant<int, 3>{}, k1, k2, k3);
         eval(std::integral_constant<int, 4>{}, ms, k4);
-        CAVMAG_BATCH_STAGE(5, ((((T)kA[4][0] * k1[q][c] + (T)kA[4][1] * k2[q][c]) + (T)kA[4][2] * k3[q][c]) + (T)kA[4][3] * k4[q][c]))
+        stage_state(std::integral_constant<int, 4>{}, k1, k2, k3, k4);
         eval(std::integral_constant<int, 5>{}, ms, k5);
-        CAVMAG_BATCH_STAGE(6, (((((T)kA[5][0] * k1[q][c] + (T)kA[5][1] * k2[q][c]) + (T)kA[5][2] * k3[q][c]) + (T)kA[5][3] * k4[q][c]) + (T)kA[5][4] * k5[q][c]))
+        stage_state(std::integral_constant<int, 5>{}, k1, k2, k3, k4, k5);
         eval(std::integral_constant<int, 6>{}, ms, k6);
-#undef CAVMAG_BATCH_STAGE
 
         // ---- 5th-order candidate, renormalised per cell (G13), 7th evaluation, error (G12) ----
         T e2max = (T)0;
@@ -424,18 +427,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
             T er[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                T acc = (T)kA[6][0] * k1[q][c];
-                acc += (T)kA[6][2] * k3[q][c];
-                acc += (T)kA[6][3] * k4[q][c];
-                acc += (T)kA[6][4] * k5[q][c];
-                acc += (T)kA[6][5] * k6[q][c];
-                yn[q][c] = y[q][c] + h * acc;
-                T e = (T)kD[0] * k1[q][c];
-                e += (T)kD[2] * k3[q][c];
-                e += (T)kD[3] * k4[q][c];
-                e += (T)kD[4] * k5[q][c];
-                e += (T)kD[5] * k6[q][c];
-                er[c] = h * e;
+                const T kv[6] = {k1[q][c], (T)0, k3[q][c], k4[q][c], k5[q][c], k6[q][c]};      // b_2 = d_2 = 0
+                yn[q][c] = dp_state<6>(y[q][c], kv, h);
+                er[c] = dp_error6(kv, h);
             }
             if (A.renormalize) {
                 const T inv = rsqrt_t<T>(yn[q][0] * yn[q][0] + yn[q][1] * yn[q][1] + yn[q][2] * yn[q][2]);
@@ -446,10 +440,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         eval(std::integral_constant<int, 7>{}, yn, k7);
 #pragma unroll
         for (int q = 0; q < NSUB; ++q) {
-            const T hd7 = h * (T)kD[6];
-            const T ex = k6[q][0] + hd7 * k7[q][0], ey = k6[q][1] + hd7 * k7[q][1], ez = k6[q][2] + hd7 * k7[q][2];
-            T e2 = ex * ex + ey * ey + ez * ez;
-            e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;               // NaN -> +inf so that max propagates it
+            const T e2 = dp_error7_sq(k6[q][0], k6[q][1], k6[q][2], k7[q][0], k7[q][1], k7[q][2], h);
             if (active) e2max = fmax(e2max, e2);
         }
 #pragma unroll

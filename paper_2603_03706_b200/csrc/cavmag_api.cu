@@ -205,6 +205,10 @@ const void* stage_tma_fn(const cav_sim* s, int stage) {
 
 const void* stage_fn(const cav_sim* s, int stage) {
     const bool f32 = s->prm.precision == CAV_F32;
+    if (s->demag) {          // the instantiation that adds the dipolar field
+        if (s->prm.n_sub == 1) return f32 ? stage_kernel_demag_f32_fm(s->vec, stage, s->nb) : stage_kernel_demag_f64_fm(s->vec, stage, s->nb);
+        return f32 ? stage_kernel_demag_f32_afm(s->vec, stage, s->nb) : stage_kernel_demag_f64_afm(s->vec, stage, s->nb);
+    }
     if (s->prm.n_sub == 1) return f32 ? stage_kernel_f32_fm(s->vec, stage, s->nb) : stage_kernel_f64_fm(s->vec, stage, s->nb);
     return f32 ? stage_kernel_f32_afm(s->vec, stage, s->nb) : stage_kernel_f64_afm(s->vec, stage, s->nb);
 }

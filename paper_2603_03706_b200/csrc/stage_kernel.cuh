@@ -79,6 +79,60 @@ template <>
 __device__ __forceinline__ double rsqrt_t<double>(double x) { return 1.0 / sqrt(x); }
 
 // ---------------------------------------------------------------------------------------
+// The per-cell arithmetic of one evaluation, shared by the three kernels (k_stage, k_stage_tma, k_batch): what differs
+// between them is only where the neighbours and the slopes come from.
+// ---------------------------------------------------------------------------------------
+// Material part of the effective field of one cell: B0 + exchange (lap = sum over in-grid neighbours of
+// (m_nb - m) (2A/Ms)/D^2, formed by the caller) + uniaxial anisotropy (2Ku/Ms)(m.k^)k^.  The RF field, the
+// inter-sublattice exchange and the dipolar field are added by the caller in that order.
+template <typename T>
+__device__ __forceinline__ void material_field(const T mx, const T my, const T mz, const T lapx, const T lapy, const T lapz,
+                                               const T B0x, const T B0y, const T B0z, const T anp, const T axx, const T axy,
+                                               const T axz, T& Bx, T& By, T& Bz) {
+    const T mk = mx * axx + my * axy + mz * axz;
+    Bx = B0x + lapx + anp * mk * axx;
+    By = B0y + lapy + anp * mk * axy;
+    Bz = B0z + lapz + anp * mk * axz;
+}
+// LLG slope in the explicit Landau-Lifshitz form: k = llg [m x B + alpha m x (m x B)], llg = -gamma/(1+alpha^2)
+template <typename T>
+__device__ __forceinline__ void llg_slope(const T mx, const T my, const T mz, const T Bx, const T By, const T Bz, const T alpha,
+                                          const T llg, T& kx, T& ky, T& kz) {
+    const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
+    const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
+    kx = llg * (tx + alpha * dx);
+    ky = llg * (ty + alpha * dy);
+    kz = llg * (tz + alpha * dz);
+}
+// Stage state of tableau row ROW (0-based: the state stage ROW+1 is evaluated at; ROW = 6: the 5th-order solution b):
+// m_0 + h sum_{j < ROW} a_{ROW,j} k_j with k[0..ROW-1] = k_1..k_ROW, zero coefficients (b_2) skipped.
+template <int ROW, typename T>
+__device__ __forceinline__ T dp_state(const T m0, const T (&k)[ROW], const T h) {
+    T acc = (T)kA[ROW][0] * k[0];
+#pragma unroll
+    for (int j = 1; j < ROW; ++j)
+        if (kA[ROW][j] != 0.0) acc += (T)kA[ROW][j] * k[j];
+    return m0 + h * acc;
+}
+// Partial error after stage 6, h sum_{j <= 6} d_j k_j (d_2 = 0), and the full error with the 7th slope.
+template <typename T>
+__device__ __forceinline__ T dp_error6(const T (&k)[6], const T h) {
+    T e = (T)kD[0] * k[0];
+    e += (T)kD[2] * k[2];
+    e += (T)kD[3] * k[3];
+    e += (T)kD[4] * k[4];
+    e += (T)kD[5] * k[5];
+    return h * e;
+}
+template <typename T>
+__device__ __forceinline__ T dp_error7_sq(const T e6x, const T e6y, const T e6z, const T k7x, const T k7y, const T k7z, const T h) {
+    const T hd7 = h * (T)kD[6];
+    const T ex = e6x + hd7 * k7x, ey = e6y + hd7 * k7y, ez = e6z + hd7 * k7z;
+    const T e2 = ex * ex + ey * ey + ez * ez;
+    return (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;      // NaN -> +inf so that max propagates it
+}
+
+// ---------------------------------------------------------------------------------------
 // Step preparation (single thread): choose h for the step that starts now.
 // Mirrors the controller spec in DESIGN.md: clamp onto t_end / the next trace sample.
 // ---------------------------------------------------------------------------------------
@@ -401,7 +455,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
 // ---------------------------------------------------------------------------------------
 // the stage kernel
 // ---------------------------------------------------------------------------------------
-template <typename T, int VEC, int STAGE, int NSUB, int NB>
+template <typename T, int VEC, int STAGE, int NSUB, int NB, bool DEMAG = false>
 __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __restrict__ trace) {
     using P = Pack<T, VEC>;
     Ctrl* ctrl = A.ctrl;
@@ -508,9 +562,9 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
 
         // ---- optional dipolar field (off in the paper): computed before this launch by
         //      an FFT convolution of this stage's state (demag.cuh), the same for both sublattices ----
-        P bdv[3];
-        const bool has_bd = A.bdem != nullptr;
-        if (has_bd) {
+        P bdv[3];                                   // (its own instantiation: a runtime branch costs the others registers)
+        constexpr bool has_bd = DEMAG;
+        if constexpr (has_bd) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) bdv[c] = ldp<T, VEC>((const T*)A.bdem + (long long)c * nc + cell);
         }
@@ -573,19 +627,14 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
                 const T mx = mc[s][0].v[v], my = mc[s][1].v[v], mz = mc[s][2].v[v];
-                const T mk = mx * axx + my * axy + mz * axz;
-                T Bx = B0x + lap[0][v] + anp * mk * axx + brf[v];
-                T By = B0y + lap[1][v] + anp * mk * axy;
-                T Bz = B0z + lap[2][v] + anp * mk * axz;
+                T Bx, By, Bz;
+                material_field(mx, my, mz, lap[0][v], lap[1][v], lap[2][v], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
+                Bx += brf[v];
                 if constexpr (NSUB == 2) {
                     Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
                 }
-                if (has_bd) { Bx += bdv[0].v[v]; By += bdv[1].v[v]; Bz += bdv[2].v[v]; }
-                const T tx = my * Bz - mz * By, ty = mz * Bx - mx * Bz, tz = mx * By - my * Bx;
-                const T dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;
-                ks[0].v[v] = llg * (tx + alpha * dx);
-                ks[1].v[v] = llg * (ty + alpha * dy);
-                ks[2].v[v] = llg * (tz + alpha * dz);
+                if constexpr (has_bd) { Bx += bdv[0].v[v]; By += bdv[1].v[v]; Bz += bdv[2].v[v]; }
+                llg_slope(mx, my, mz, Bx, By, Bz, alpha, llg, ks[0].v[v], ks[1].v[v], ks[2].v[v]);
             }
 
             // ---- store k_s, then the fused tail: next stage state / candidate / error ----
@@ -598,28 +647,24 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const long long off = (long long)(s * 3 + c) * nc + cell;
-                    P acc, m0v;
+                    P m0v, q[STAGE];                   // k_1 .. k_STAGE of this component
                     if constexpr (STAGE == 2) {
                         m0v = y0c[s][c];
-#pragma unroll
-                        for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[2][0] * k1c[s][c].v[v];
+                        q[0] = k1c[s][c];
                     } else {
                         m0v = ldp<T, VEC>(y0 + off);
-                        const P q1 = ldp<T, VEC>(k1 + off);
+                        q[0] = ldp<T, VEC>(k1 + off);
 #pragma unroll
-                        for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[STAGE][0] * q1.v[v];
-#pragma unroll
-                        for (int j = 1; j < STAGE - 1; ++j) {
-                            const P qj = ldp<T, VEC>((const T*)A.K[j] + off);
-#pragma unroll
-                            for (int v = 0; v < VEC; ++v) acc.v[v] += (T)kA[STAGE][j] * qj.v[v];
-                        }
+                        for (int j = 1; j < STAGE - 1; ++j) q[j] = ldp<T, VEC>((const T*)A.K[j] + off);
                     }
+                    q[STAGE - 1] = ks[c];
                     P out;
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
-                        acc.v[v] += (T)kA[STAGE][STAGE - 1] * ks[c].v[v];
-                        out.v[v] = m0v.v[v] + h * acc.v[v];
+                        T kv[STAGE];
+#pragma unroll
+                        for (int j = 0; j < STAGE; ++j) kv[j] = q[j].v[v];
+                        out.v[v] = dp_state<STAGE>(m0v.v[v], kv, h);
                     }
                     if (active) stp<T, VEC>(mnext + off, out);
                 }
@@ -636,18 +681,9 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
                     const P q5 = ldp<T, VEC>((const T*)A.K[4] + off);
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
-                        T acc = (T)kA[6][0] * q1.v[v];
-                        acc += (T)kA[6][2] * q3.v[v];
-                        acc += (T)kA[6][3] * q4.v[v];
-                        acc += (T)kA[6][4] * q5.v[v];
-                        acc += (T)kA[6][5] * ks[c].v[v];
-                        y5[c].v[v] = m0v.v[v] + h * acc;
-                        T e = (T)kD[0] * q1.v[v];
-                        e += (T)kD[2] * q3.v[v];
-                        e += (T)kD[3] * q4.v[v];
-                        e += (T)kD[4] * q5.v[v];
-                        e += (T)kD[5] * ks[c].v[v];
-                        er[c].v[v] = h * e;
+                        const T kv[6] = {q1.v[v], (T)0, q3.v[v], q4.v[v], q5.v[v], ks[c].v[v]};      // b_2 = d_2 = 0: k_2 is not read
+                        y5[c].v[v] = dp_state<6>(m0v.v[v], kv, h);
+                        er[c].v[v] = dp_error6(kv, h);
                     }
                 }
                 if (A.renormalize) {
@@ -669,12 +705,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
                 for (int c = 0; c < 3; ++c) er[c] = ldp<T, VEC>(e6 + (long long)(s * 3 + c) * nc + cell);
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
-                    const T hd7 = h * (T)kD[6];
-                    const T ex = er[0].v[v] + hd7 * ks[0].v[v];
-                    const T ey = er[1].v[v] + hd7 * ks[1].v[v];
-                    const T ez = er[2].v[v] + hd7 * ks[2].v[v];
-                    T e2 = ex * ex + ey * ey + ez * ez;
-                    e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;     // NaN -> +inf so that max propagates it
+                    const T e2 = dp_error7_sq(er[0].v[v], er[1].v[v], er[2].v[v], ks[0].v[v], ks[1].v[v], ks[2].v[v], h);
                     if (active) {
                         emax2 = fmax(emax2, e2);
                         sm[s * 3 + 0] += mc[s][0].v[v]; sm[s * 3 + 1] += mc[s][1].v[v]; sm[s * 3 + 2] += mc[s][2].v[v];
@@ -752,18 +783,26 @@ const void* stage_kernel_f32_fm(int vec, int stage, int nb);
 const void* stage_kernel_f32_afm(int vec, int stage, int nb);
 const void* stage_kernel_f64_fm(int vec, int stage, int nb);
 const void* stage_kernel_f64_afm(int vec, int stage, int nb);
+// the same with the dipolar field added (k_stage<..., DEMAG = true>; demag.cuh)
+const void* stage_kernel_demag_f32_fm(int vec, int stage, int nb);
+const void* stage_kernel_demag_f32_afm(int vec, int stage, int nb);
+const void* stage_kernel_demag_f64_fm(int vec, int stage, int nb);
+const void* stage_kernel_demag_f64_afm(int vec, int stage, int nb);
 
 #define CAVMAG_STAGE_CASES(T, VEC, NSUB, NB)                                       \
     switch (stage) {                                                               \
-        case 1: return (const void*)k_stage<T, VEC, 1, NSUB, NB>;                  \
-        case 2: return (const void*)k_stage<T, VEC, 2, NSUB, NB>;                  \
-        case 3: return (const void*)k_stage<T, VEC, 3, NSUB, NB>;                  \
-        case 4: return (const void*)k_stage<T, VEC, 4, NSUB, NB>;                  \
-        case 5: return (const void*)k_stage<T, VEC, 5, NSUB, NB>;                  \
-        case 6: return (const void*)k_stage<T, VEC, 6, NSUB, NB>;                  \
-        case 7: return (const void*)k_stage<T, VEC, 7, NSUB, NB>;                  \
+        case 1: return (const void*)k_stage<T, VEC, 1, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 2: return (const void*)k_stage<T, VEC, 2, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 3: return (const void*)k_stage<T, VEC, 3, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 4: return (const void*)k_stage<T, VEC, 4, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 5: return (const void*)k_stage<T, VEC, 5, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 6: return (const void*)k_stage<T, VEC, 6, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 7: return (const void*)k_stage<T, VEC, 7, NSUB, NB, CAVMAG_DEMAG_INST>; \
         default: return nullptr;                                                   \
     }
+#ifndef CAVMAG_DEMAG_INST
+#define CAVMAG_DEMAG_INST false      // a translation unit that instantiates the dipolar-field variants defines it to true
+#endif
 
 #define CAVMAG_DEFINE_LOOKUP(NAME, T, VECW, NSUB)                                  \
     const void* NAME(int vec, int stage, int nb) {                                 \

@@ -824,18 +824,13 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
                     const T mx = mc[s][0].v[v], my = mc[s][1].v[v], mz = mc[s][2].v[v];
-                    const T mk = mx * axx + my * axy + mz * axz;
-                    T Bx = B0x + lap[0][v] + anp * mk * axx + brf[v];
-                    T By = B0y + lap[1][v] + anp * mk * axy;
-                    T Bz = B0z + lap[2][v] + anp * mk * axz;
+                    T Bx, By, Bz;
+                    material_field(mx, my, mz, lap[0][v], lap[1][v], lap[2][v], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
+                    Bx += brf[v];
                     if constexpr (NSUB == 2) {
                         Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
                     }
-                    const T tx_ = my * Bz - mz * By, ty_ = mz * Bx - mx * Bz, tz_ = mx * By - my * Bx;
-                    const T dx = my * tz_ - mz * ty_, dy = mz * tx_ - mx * tz_, dz = mx * ty_ - my * tx_;
-                    ks[0].v[v] = llg * (tx_ + alpha * dx);
-                    ks[1].v[v] = llg * (ty_ + alpha * dy);
-                    ks[2].v[v] = llg * (tz_ + alpha * dz);
+                    llg_slope(mx, my, mz, Bx, By, Bz, alpha, llg, ks[0].v[v], ks[1].v[v], ks[2].v[v]);
                 }
 
 #pragma unroll
@@ -846,29 +841,23 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
                         const int comp = s * 3 + c;
-                        P acc, m0v;
+                        P m0v, q[STAGE];               // k_1 .. k_STAGE of this component
                         if constexpr (STAGE == 2) {
                             m0v = lds_pack(sm_zc + (unsigned)(comp * HPLANE) + crow, tag);
-                            const P q1 = lds_pack(sm_zc + TA.hbox_bytes + (unsigned)(comp * HPLANE) + crow, tag);
-#pragma unroll
-                            for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[2][0] * q1.v[v];
+                            q[0] = lds_pack(sm_zc + TA.hbox_bytes + (unsigned)(comp * HPLANE) + crow, tag);
                         } else {
                             m0v = lds_pack(axf + (unsigned)(comp * APLANE), tag);
-                            const P q1 = lds_pack(axf + (unsigned)((C + comp) * APLANE), tag);
 #pragma unroll
-                            for (int v = 0; v < VEC; ++v) acc.v[v] = (T)kA[STAGE][0] * q1.v[v];
-#pragma unroll
-                            for (int j = 1; j < STAGE - 1; ++j) {
-                                const P qj = lds_pack(axf + (unsigned)(((1 + j) * C + comp) * APLANE), tag);
-#pragma unroll
-                                for (int v = 0; v < VEC; ++v) acc.v[v] += (T)kA[STAGE][j] * qj.v[v];
-                            }
+                            for (int j = 0; j < STAGE - 1; ++j) q[j] = lds_pack(axf + (unsigned)(((1 + j) * C + comp) * APLANE), tag);
                         }
+                        q[STAGE - 1] = ks[c];
                         P out;
 #pragma unroll
                         for (int v = 0; v < VEC; ++v) {
-                            acc.v[v] += (T)kA[STAGE][STAGE - 1] * ks[c].v[v];
-                            out.v[v] = m0v.v[v] + h * acc.v[v];
+                            T kv[STAGE];
+#pragma unroll
+                            for (int j = 0; j < STAGE; ++j) kv[j] = q[j].v[v];
+                            out.v[v] = dp_state<STAGE>(m0v.v[v], kv, h);
                         }
                         if (active) stp<T, VEC>(mnext + (long long)comp * nc + cell, out);
                     }
@@ -885,18 +874,9 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
                         const P q5 = lds_pack(axf + (unsigned)((4 * C + comp) * APLANE), tag);
 #pragma unroll
                         for (int v = 0; v < VEC; ++v) {
-                            T acc = (T)kA[6][0] * q1.v[v];
-                            acc += (T)kA[6][2] * q3.v[v];
-                            acc += (T)kA[6][3] * q4.v[v];
-                            acc += (T)kA[6][4] * q5.v[v];
-                            acc += (T)kA[6][5] * ks[c].v[v];
-                            y5[c].v[v] = m0v.v[v] + h * acc;
-                            T e = (T)kD[0] * q1.v[v];
-                            e += (T)kD[2] * q3.v[v];
-                            e += (T)kD[3] * q4.v[v];
-                            e += (T)kD[4] * q5.v[v];
-                            e += (T)kD[5] * ks[c].v[v];
-                            er[c].v[v] = h * e;
+                            const T kv[6] = {q1.v[v], (T)0, q3.v[v], q4.v[v], q5.v[v], ks[c].v[v]};      // b_2 = d_2 = 0: k_2 is not read
+                            y5[c].v[v] = dp_state<6>(m0v.v[v], kv, h);
+                            er[c].v[v] = dp_error6(kv, h);
                         }
                     }
                     if (renorm) {
@@ -918,12 +898,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
                     for (int c = 0; c < 3; ++c) er[c] = lds_pack(axf + (unsigned)((s * 3 + c) * APLANE), tag);
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
-                        const T hd7 = h * (T)kD[6];
-                        const T ex = er[0].v[v] + hd7 * ks[0].v[v];
-                        const T ey = er[1].v[v] + hd7 * ks[1].v[v];
-                        const T ez = er[2].v[v] + hd7 * ks[2].v[v];
-                        T e2 = ex * ex + ey * ey + ez * ez;
-                        e2 = (e2 < (T)CUDART_INF) ? e2 : (T)CUDART_INF;     // NaN -> +inf so that max propagates it
+                        const T e2 = dp_error7_sq(er[0].v[v], er[1].v[v], er[2].v[v], ks[0].v[v], ks[1].v[v], ks[2].v[v], h);
                         // out-of-grid lanes hold TMA zero fill: e2 = 0 and m = 0, so they need no mask
                         emax2 = fmax(emax2, e2);
                         sm[s * 3 + 0] += mc[s][0].v[v]; sm[s * 3 + 1] += mc[s][1].v[v]; sm[s * 3 + 2] += mc[s][2].v[v];
