@@ -222,7 +222,7 @@ __device__ __forceinline__ bool deferred_finish(const StageArgs& A, Ctrl* __rest
 template <int NB, int NSUB>
 __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaArgs& TA, const int tidc,
                                                  unsigned long long* sc_words, double* sred, double* serr, double* trace,
-                                                 const int nblk, const bool owner, unsigned int* live_count) {
+                                                 const int nblk, const bool owner, unsigned int* live_count, int& spec_miss) {
     // live_count != nullptr (joint launch of several simulations): the owner reports "this simulation goes on" there
     // instead of setting the WHILE condition itself
     const unsigned long long* gcw = reinterpret_cast<const unsigned long long*>(A.ctrl0);
@@ -247,6 +247,10 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     }
     asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
     Ctrl* const c = reinterpret_cast<Ctrl*>(sc_words);
+    // what the producer warp assumes while this runs (it reads the same words from ctrl0): the pending step is accepted,
+    // i.e. the buffer indices flip; every thread keeps the prediction to compare it with the verdict
+    const int done_in = c->done;
+    const int ycur_pred = c->pend7 ? (c->ycur ^ 1) : c->ycur, k1_pred = c->pend7 ? 6 - c->k1slot : c->k1slot;
     const bool write = owner;
     if (c->done == 0 && c->pend7 != 0) {            // uniform over the block (and over the grid)
         if (tidc < N) mode_ode_stage<7>(c, tidc, sred, serr);
@@ -273,6 +277,7 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
     }
     if (tidc == 0) c->pend7 = c->done ? 0 : 1;            // a step starts now: its stage 7 will be pending
     asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
+    spec_miss = (done_in == 0 && (c->done != 0 || c->ycur != ycur_pred || c->k1slot != k1_pred)) ? 1 : 0;
     asm volatile("bar.arrive 2, %0;" ::"n"(kTmaThreads) : "memory");      // the producer warp may read the shared copy
 #ifdef CAVMAG_PROBE
     if (tidc == 0) probe_mark(A, 2, 10);                // verdict and the new step's control data are in shared memory
@@ -496,6 +501,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
         constexpr unsigned aux_tx = (unsigned)(NAUX * C) * (unsigned)APLANE;
         constexpr unsigned u_tx = (unsigned)UCB * (unsigned)APLANE;   // the full box is always counted (OOB modes zero-filled)
         int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
+        int spec_slots = 0;                         // stage 2: ms slots filled speculatively before the controller's verdict
         const int npre = (NAUX > 1) ? (TA.pre_k ? NAUX - 1 : (NAUX - 1 < 2 ? NAUX - 1 : 2)) : 0;   // aux fields fetched before the wait
         if constexpr (kPre) {
             if (!SWEEP && issuer) {                 // (a joint launch fetches nothing before the wait)
@@ -536,10 +542,50 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
             if (!SWEEP || sr == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
             CAVMAG_MARK(13);
             if constexpr (STAGE == 2) {
-                // the consumers have finished the previous step (deferred_finish7): verdict and buffer indices in s_ctrl
+                // The consumers are finishing the previous step (deferred_finish7: ~5 us for loads, mode algebra and the
+                // controller).  The buffer indices of THIS step depend on its verdict, but a step is almost always
+                // accepted: issue the first stage-state tiles now for "accept" (indices flipped) and check afterwards.
+                bool spec = false;
+                if constexpr (!SWEEP) {
+                    const Ctrl* const c0 = A.ctrl0;             // complete: written by the stage-7 kernel / k_begin / stage 1
+                    const int d0 = c0->done, p7 = c0->pend7, y0c = c0->ycur, k0c = c0->k1slot;
+                    if (!d0) { ycur = p7 ? (y0c ^ 1) : y0c; k1slot = p7 ? 6 - k0c : k0c; spec = true; }
+                    if (spec && issuer) {
+                        setup_maps();
+                        int zz = z0, txx = tx0, tyy = ty0;
+                        for (int p = 0; p < nplanes; ++p) {         // the slots the main loop will ask for, in its order
+                            const int need = (p == 0 || zz == zfirst) ? 3 : 1;
+                            if (spec_slots + need > Dm) break;
+                            const int x0 = txx * TX, y0 = tyy * kTmaTY;
+                            for (int i = 0; i < need; ++i) {
+                                const int zq = need == 3 ? zz - dir + i * dir : zz + dir;
+                                const unsigned bar = full_ms + 8 * spec_slots;
+                                mbar_expect_tx(bar, NH * TA.hbox_tx);
+                                const unsigned dst = ms_ring + (unsigned)spec_slots * TA.ms_slot_bytes;
+                                tma_load_4d(dst, hmap0, x0 - HX, y0 - 1, zq, 0, bar);
+                                if constexpr (NH == 2) tma_load_4d(dst + TA.hbox_bytes, hmap1, x0 - HX, y0 - 1, zq, 0, bar);
+                                ++spec_slots;
+                            }
+                            advance(zz, txx, tyy);
+                        }
+                    }
+                    __syncwarp();
+                }
+                // verdict and buffer indices in s_ctrl
                 asm volatile("bar.sync 2, %0;" ::"n"(kTmaThreads) : "memory");
                 const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
+                const int ys = ycur, ks = k1slot;
                 done = sc->done; N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot;
+                if (spec && (done || ycur != ys || k1slot != ks)) {
+                    // rejected step (or the run is over): the tiles fetched are the wrong buffers.  Let them land, burn the
+                    // phase of the untouched slots as well, and start over - the consumers know (spec_miss) that every
+                    // "full" barrier of the ms ring is one phase ahead.
+                    if (issuer) {
+                        for (int i = 0; i < spec_slots; ++i) mbar_wait(full_ms + 8 * i, 0u);
+                        for (int i = spec_slots; i < Dm; ++i) mbar_expect_tx(full_ms + 8 * i, 0u);
+                    }
+                    spec_slots = 0;
+                }
                 setup_maps();
             } else if (!have_ctrl) {
                 done = ctrl->done; N = ctrl->N; ycur = ctrl->ycur; k1slot = ctrl->k1slot;
@@ -554,6 +600,11 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
         if (issuer) {
             int z = z0, tx = tx0, ty = ty0;
             auto issue_ms = [&](int x0, int y0, int zz) {
+                if (spec_slots > 0) {                   // filled before the verdict, same order
+                    --spec_slots;
+                    if (++hm == Dm) { hm = 0; pm ^= 1u; }
+                    return;
+                }
                 mbar_wait(empty_ms + 8 * hm, pm);
                 const unsigned bar = full_ms + 8 * hm;
                 mbar_expect_tx(bar, NH * TA.hbox_tx);
@@ -625,9 +676,11 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
         double hd;
         if constexpr (STAGE == 2) {
             // finish stage 7 of the previous step, run the controller, start this step (all blocks, same bits)
-            if (!deferred_finish7<NB, NSUB>(A, TA, tid, s_ctrl, s_red, s_err, trace, nblk_r, slot == 0, SWEEP ? SW.live : nullptr)) {
+            int spec_miss = 0;
+            if (!deferred_finish7<NB, NSUB>(A, TA, tid, s_ctrl, s_red, s_err, trace, nblk_r, slot == 0, SWEEP ? SW.live : nullptr, spec_miss)) {
                 if constexpr (SWEEP) continue; else return;
             }
+            if constexpr (!SWEEP) { if (spec_miss) pm = 1u; }      // the producer re-issued its speculative tiles: ms "full" barriers are one phase ahead
             const Ctrl* const sc = reinterpret_cast<const Ctrl*>(s_ctrl);
             N = sc->N; ycur = sc->ycur; k1slot = sc->k1slot; hd = sc->h;
             if (NB > 0 && tid < NB) s_cn[tid] = (tid < N) ? (T)sc->c[tid] : (T)0;
