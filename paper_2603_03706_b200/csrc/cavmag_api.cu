@@ -34,6 +34,7 @@ struct cav_sim {
     void* K[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     void* u = nullptr;
     size_t u_bytes = 0;
+    unsigned long long u_hash = 0;   // FNV-1a of the profile bytes given to cav_set_modes from the host (0: unknown / device source)
     double* partial = nullptr;
     double* partial_max = nullptr;
     int pstride = 0;
@@ -44,6 +45,7 @@ struct cav_sim {
     int trace_cap = 0;
     int N = 0, nb = 0;
     bool m_set = false;
+    bool h_fresh = false;        // h_ctrl equals the device's Ctrl (nothing that writes Ctrl has been enqueued since the last pull / push)
     int iters = 1, nblocks = 1, user_block_cells = 0, serpentine = 1;
     int launch_mode = CAV_LAUNCH_GRAPH;
     cudaStream_t stream = nullptr;
@@ -425,11 +427,7 @@ int run_block_path(cav_sim* s, double t_end, double tol, double fixed_dt, double
     if (!s->d_blk) CK(cudaMalloc(&s->d_blk, kBlkBytes));
     const size_t coop_part = sizeof(double) * (size_t)kMaxSums * s->n_sm, coop_max = sizeof(double) * (size_t)s->n_sm;
     if (s->use_coop && !s->d_coop) CK(cudaMalloc(&s->d_coop, 2 * coop_part + 2 * coop_max + 64));
-    if (!s->last_run_block) {                            // a stage-kernel run may have flipped ycur on the device
-        int rc0 = sync_pull(s);
-        if (rc0) return rc0;
-        s->last_run_block = true;
-    }
+    // (cav_run_steps has pulled Ctrl if a stage-kernel run may have flipped ycur on the device since the last pull)
     const cav_params& p = s->prm;
     const Ctrl* hc = s->h_ctrl;                          // host-set fields only (N, trace and drive settings)
     k_block_in<<<1, 32, 0, s->stream>>>(s->d_ctrl, s->d_blk, p.B0[0], p.B0[1], p.B0[2]);
@@ -542,9 +540,11 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
 }
 
 int sync_pull(cav_sim* s) {
+    if (s->h_fresh) return CAV_OK;       // setters and getters in a row (upload m, upload a, ... ) need one pull, not one each
     CK(cudaStreamSynchronize(s->stream));
     CK(cudaMemcpyAsync(s->h_ctrl, s->d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
+    s->h_fresh = true;
     return CAV_OK;
 }
 
@@ -943,6 +943,18 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         if ((e = cudaMalloc(&s->u, bytes)) != cudaSuccess) return cuda_fail(e);
         s->u_bytes = bytes;
     }
+    s->u_hash = 0;
+    if (N > 0 && !u_is_device) {          // lets a sweep recognise members with identical profiles
+        unsigned long long hsh = 1469598103934665603ull;
+        const unsigned char* pb = (const unsigned char*)u;
+        const size_t nb8 = (size_t)N * s->nc * s->esize;
+        for (size_t i = 0; i < nb8; i += 8) {
+            unsigned long long w8 = 0;
+            memcpy(&w8, pb + i, nb8 - i >= 8 ? 8 : nb8 - i);
+            hsh = (hsh ^ w8) * 1099511628211ull;
+        }
+        s->u_hash = hsh ? hsh : 1ull;
+    }
     if (N > 0) {
         if (s->padded && (e = cudaMemsetAsync(s->u, 0, bytes, s->stream)) != cudaSuccess) return cuda_fail(e);     // pad cells: u = 0
         if (copy_in(s, s->u, u, N, u_is_device != 0) != CAV_OK) return fail(CAV_E_CUDA);
@@ -1188,6 +1200,7 @@ static int ensure_k1(cav_sim* s) {
         decide_path(s);
         if (s->padded && !s->use_tma) return CAV_E_UNSUPPORTED;
         StageArgs A = make_args(s, 0ull);
+        s->h_fresh = false;
         k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
         CK(cudaGetLastError());
         s->host_launches++;
@@ -1232,6 +1245,8 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     if (std::isnan(t_end) || max_steps < 0) return CAV_E_ARG;
     if (std::isinf(t_end) && max_steps == 0) return CAV_E_ARG;
     decide_path(s);
+    if (!s->last_run_block && (s->use_block || s->use_coop)) { int rc0 = sync_pull(s); if (rc0) return rc0; s->last_run_block = true; }
+    s->h_fresh = false;                                        // the run rewrites Ctrl on the device
     if (s->use_block || s->use_coop) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     if (s->d_pol != nullptr || s->split_nllg > 0) return CAV_E_UNSUPPORTED;     // grid beyond the small-grid kernel (cavmag.h)
     if (s->padded && !s->use_tma) return CAV_E_UNSUPPORTED;                     // padded rows are only understood by the TMA kernels
@@ -1369,6 +1384,8 @@ namespace {
 
 void sweep_fill_reps(cav_sweep* w) {
     w->h_reps.resize(w->sims.size());
+    bool same_u = w->sims[0]->u_hash != 0;
+    for (cav_sim* q : w->sims) same_u = same_u && q->u_hash == w->sims[0]->u_hash && q->N == w->sims[0]->N;
     for (size_t r = 0; r < w->sims.size(); ++r) {
         cav_sim* q = w->sims[r];
         RepPtrs& p = w->h_reps[r];
@@ -1378,6 +1395,7 @@ void sweep_fill_reps(cav_sweep* w) {
         for (int i = 0; i < 7; ++i) p.K[i] = q->K[i];
         p.u = q->u; p.partial = q->partial; p.partial_max = q->partial_max; p.spec = q->d_spec; p.trace = q->d_trace;
         p.maps = q->d_maps;
+        p.umap = (same_u ? w->sims[0]->d_maps : q->d_maps) + 128 * MAP_P_U;
         for (int i = 0; i < 3; ++i) p.B0[i] = q->prm.B0[i];
     }
 }
@@ -1545,7 +1563,7 @@ int cav_sweep_run(cav_sweep* w, double t_end, double tol, double fixed_dt, doubl
     CK(cudaGetLastError());
     const int which = (max_steps == 0 || max_steps >= kUnrollMinSteps) ? 1 : 0;
     CK(cudaGraphLaunch(w->exec[which], w->stream));
-    for (cav_sim* q : w->sims) { q->last_run_block = false; q->host_launches += 2; }
+    for (cav_sim* q : w->sims) { q->last_run_block = false; q->h_fresh = false; q->host_launches += 2; }
     return CAV_OK;
 }
 

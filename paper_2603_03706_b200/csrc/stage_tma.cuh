@@ -309,6 +309,8 @@ struct RepPtrs {
     const void* u;
     double* partial; double* partial_max; double* spec; double* trace;
     const unsigned char* maps;
+    const unsigned char* umap;      // tensor map of the mode profiles: the member's own, or member 0's when all members share
+                                    // the same profiles (one copy then serves every member out of L2)
     double B0[3];
 };
 struct SweepArgs {
@@ -401,6 +403,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
     StageArgs Arep;                                  // SWEEP: the arguments of the current simulation
     double* trace = trace0;
     const unsigned char* rep_maps = TA.maps;
+    const unsigned char* rep_umap = TA.maps + 128 * MAP_P_U;
     long long ql0 = cq0, ql1 = cq1;                  // the sub-run, in plane-tiles of its own simulation
     int slot = (int)blockIdx.x, nblk_r = (int)gridDim.x;       // this block's partial-sum slot / blocks working on the simulation
     int nplanes = 0, z0 = 0, tx0 = 0, ty0 = 0;                 // the sub-run: length and first plane-tile in sweep order
@@ -436,6 +439,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
             Arep.cond_handle = 0ull;
             trace = rp.trace;
             rep_maps = rp.maps;
+            rep_umap = rp.umap;
             set_geometry();
         }
     };
@@ -497,7 +501,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
             }
         };
         if (have_ctrl) setup_maps();
-        const void* umap = mp(MAP_P_U);
+        const void* umap = (const void*)rep_umap;
         constexpr unsigned aux_tx = (unsigned)(NAUX * C) * (unsigned)APLANE;
         constexpr unsigned u_tx = (unsigned)UCB * (unsigned)APLANE;   // the full box is always counted (OOB modes zero-filled)
         int pre_a = 0, pre_u = 0;                   // aux slots armed / u slots filled before the dependency wait
