@@ -145,3 +145,36 @@ def test_sweep_argument_checks(api, stream):
     finally:
         for s in sims + [so, lone]:
             s.close()
+
+
+def test_members_stay_ordinary_handles(api, stream):
+    """After a joint run a member can go on alone (cav_run on the single handle), a member that has already reached t_end
+    is skipped by the next joint run, and the on-device Fourier sums accumulate per member."""
+    from oracle import dft
+    ws = _members(5)
+    sims = [api.Sim(w, precision="f64", stream=stream) for w in ws]
+    K, lo, hi = 17, 2 * math.pi * 9e9, 2 * math.pi * 11e9
+    for sim in sims:
+        api.cav_set_trace(sim.h, 1e-12, 8)
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+    sw = api.cav_sweep_create(sims)
+    try:
+        api.cav_sweep_run(sw, math.inf, fixed_dt=0.1e-12, max_steps=40)
+        # member 1 alone for 20 more steps, then everybody to t = 8 ps: member 1 has less to do
+        api.cav_run_steps(sims[1].h, math.inf, fixed_dt=0.1e-12, max_steps=20)
+        api.cav_sweep_run(sw, 8e-12, fixed_dt=0.1e-12)
+        api.cav_sweep_run(sw, 8e-12, fixed_dt=0.1e-12)                 # everybody is at t_end: nothing happens
+        for w, sim in zip(ws, sims):
+            ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=80, sample_dt=1e-12, trace_cap=8)
+            st = api.cav_get_stats(sim.h)
+            assert st["accepted"] == 80 and abs(st["t"] - 8e-12) < 1e-24
+            assert_parity(sim.get_m(), sim.get_a(), ref, "f64")
+            tr = api.cav_get_trace(sim.h)
+            assert tr.shape[0] == 8 and np.abs(tr - ref.trace).max() < 1e-9
+            X, ns = api.cav_get_spectrum(sim.h, K, 2)
+            ref_a = dft(tr[:, 0], tr[:, 1] + 1j * tr[:, 2], np.linspace(lo, hi, K))
+            assert ns == 8 and np.abs(X[:, 0] - ref_a).max() <= 1e-11 * np.abs(ref_a).max()
+    finally:
+        api.cav_sweep_destroy(sw)
+        for sim in sims:
+            sim.close()
