@@ -217,10 +217,9 @@ int cav_get_stage_overlap(cav_sim* sim, int* active);
  *     S_n = (1/W_n) sum_r u_n(r) (m_c.p_n - i m_c.q_n),      B_rf(r) = sum_n c_n u_n(r) p_n
  * (reading G32; p = x^, q = y^ is the paper's case).  pol: [N][3] host, normalised on entry; quad: [N][3] host,
  * used as given, or NULL for q_n = z^ x p_n (static field along z^).  pol == NULL restores x^.  Call after cav_set_modes
- * (a new mode set restores x^).  Implemented in the small-grid kernel: CAV_E_UNSUPPORTED for grids of more than
- * 512 x (number of SMs) cells; the run then uses CAV_PATH_BLOCK / CAV_PATH_COOP whatever cav_set_kernel_path says, and
- * cav_get_dmdt / cav_get_dadt (which evaluate one stage with the stage kernels) return CAV_E_UNSUPPORTED; the overlaps
- * S_n are in the trace rows. */
+ * (a new mode set restores x^).  Implemented in the small-grid kernel (CAV_PATH_BLOCK / CAV_PATH_COOP) and in the generic
+ * stage kernels, which the run then uses whatever cav_set_kernel_path says (the TMA kernels keep the paper's x^);
+ * CAV_E_UNSUPPORTED together with cav_set_demag or on a grid stored with padded rows. */
 int cav_set_polarisation(cav_sim* sim, const double* pol, const double* quad);
 
 /* Integrator.  CAV_INTEGRATOR_UNIFIED (default): LLG and mode ODEs in ONE Dormand-Prince step (tier 1).
@@ -230,7 +229,8 @@ int cav_set_polarisation(cav_sim* sim, const double* pol, const double* quad);
  * Dormand-Prince steps of dt/n_llg (reading G33).  Fixed step only: cav_run* must be called with
  * fixed_dt = dt (CAV_E_ARG otherwise); max_steps counts co-simulation steps; the statistics count LLG sub-steps
  * (accepted = steps x n_llg, 6 n_llg + 1 evaluations per step); choose a trace sample_dt that is a multiple of dt.
- * Small-grid kernel only, as cav_set_polarisation (CAV_E_UNSUPPORTED beyond). */
+ * Small-grid kernel only: CAV_E_UNSUPPORTED for grids of more than 512 x (number of SMs) cells; the run uses
+ * CAV_PATH_BLOCK / CAV_PATH_COOP whatever cav_set_kernel_path says. */
 enum { CAV_INTEGRATOR_UNIFIED = 0, CAV_INTEGRATOR_SPLIT = 1 };
 int cav_set_integrator(cav_sim* sim, int integrator, int n_llg);
 

@@ -207,6 +207,10 @@ const void* stage_tma_fn(const cav_sim* s, int stage) {
 
 const void* stage_fn(const cav_sim* s, int stage) {
     const bool f32 = s->prm.precision == CAV_F32;
+    if (s->d_pol) {          // the instantiation with per-mode polarisation
+        if (s->prm.n_sub == 1) return f32 ? stage_kernel_pol_f32_fm(s->vec, stage, s->nb) : stage_kernel_pol_f64_fm(s->vec, stage, s->nb);
+        return f32 ? stage_kernel_pol_f32_afm(s->vec, stage, s->nb) : stage_kernel_pol_f64_afm(s->vec, stage, s->nb);
+    }
     if (s->demag) {          // the instantiation that adds the dipolar field
         if (s->prm.n_sub == 1) return f32 ? stage_kernel_demag_f32_fm(s->vec, stage, s->nb) : stage_kernel_demag_f64_fm(s->vec, stage, s->nb);
         return f32 ? stage_kernel_demag_f32_afm(s->vec, stage, s->nb) : stage_kernel_demag_f64_afm(s->vec, stage, s->nb);
@@ -369,11 +373,13 @@ constexpr int kCoopThreads = 512;
 void decide_path(cav_sim* s) {
     const bool block_ok = s->nc <= kBatchMaxCells;
     const bool coop_ok = !block_ok && s->nc <= (long long)s->n_sm * kCoopThreads;
-    // a non-default polarisation and the operator-split comparison integrator exist in the small-grid kernel only
-    const bool small_only = s->d_pol != nullptr || s->split_nllg > 0;
+    // the operator-split comparison integrator exists in the small-grid kernel only; a non-default polarisation in the
+    // small-grid kernel and in the generic stage kernels (their own instantiation), not in the TMA kernels
+    const bool small_only = s->split_nllg > 0;
     s->use_block = block_ok && (s->kernel_path == CAV_PATH_BLOCK || s->kernel_path == CAV_PATH_AUTO || small_only);
     s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO || small_only);
     if (s->demag) { s->use_block = s->use_coop = s->use_tma = false; return; }                 // dipolar field: generic stage kernels
+    if (s->d_pol) { s->use_tma = false; return; }                                              // polarisation: small-grid or generic kernels
     if (s->padded) { s->use_block = s->use_coop = false; s->use_tma = s->tma_eligible; }       // padded rows: TMA kernels only
     else if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
@@ -509,6 +515,7 @@ StageArgs make_args(const cav_sim* s, unsigned long long handle) {
     A.partial_max = s->partial_max;
     A.spec = s->d_spec;
     A.bdem = s->demag ? s->d_bdem : nullptr;
+    A.pol = s->d_pol;
     A.cond_handle = handle;
     A.pstride = s->pstride;
     A.nx = s->grid.nx; A.ny = s->grid.ny; A.nz = s->grid.nz;
@@ -1042,8 +1049,7 @@ int cav_set_polarisation(cav_sim* s, const double* pol, const double* quad) {
         CK(cudaMalloc(&s->d_pol, sizeof(double) * 6 * s->N));
         CK(cudaMemcpyAsync(s->d_pol, h, sizeof(double) * 6 * s->N, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
-        decide_path(s);
-        if (!s->use_block && !s->use_coop) {             // the grid is beyond the small-grid kernel
+        if (s->padded || s->demag) {                     // rows padded for the TMA kernels / the dipolar-field kernels: x^ only
             cudaFree(s->d_pol);
             s->d_pol = nullptr;
             push_ctrl(s);
@@ -1192,7 +1198,6 @@ int cav_get_a(cav_sim* s, double* out) {
 
 static int ensure_k1(cav_sim* s) {
     if (!s->m_set) return CAV_E_STATE;
-    if (s->d_pol != nullptr) return CAV_E_UNSUPPORTED;     // the stage kernels evaluate x^-polarised modes only (cavmag.h)
     int rc = sync_pull(s);
     if (rc) return rc;
     if (!s->h_ctrl->k1_valid) {
@@ -1248,7 +1253,7 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     if (!s->last_run_block && (s->use_block || s->use_coop)) { int rc0 = sync_pull(s); if (rc0) return rc0; s->last_run_block = true; }
     s->h_fresh = false;                                        // the run rewrites Ctrl on the device
     if (s->use_block || s->use_coop) return run_block_path(s, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
-    if (s->d_pol != nullptr || s->split_nllg > 0) return CAV_E_UNSUPPORTED;     // grid beyond the small-grid kernel (cavmag.h)
+    if (s->split_nllg > 0) return CAV_E_UNSUPPORTED;                            // grid beyond the small-grid kernel (cavmag.h)
     if (s->padded && !s->use_tma) return CAV_E_UNSUPPORTED;                     // padded rows are only understood by the TMA kernels
     s->last_run_block = false;
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);

@@ -87,6 +87,7 @@ struct StageArgs {
     double* partial;     // [2][kMaxSums][pstride] block partial sums, double-buffered by stage parity (stage_partials())
     double* partial_max; // [pstride] block max of |e|^2
     const void* bdem;    // [3][nc] dipolar field of the state this stage is evaluated at (generic kernels only), or nullptr
+    const double* pol;   // [N][6] polarisation p_n and quadrature axis q_n per mode (generic polarisation kernels only), or nullptr
     double* spec;        // [spec_K][2N][2] Fourier sums X_k += x(t_j) exp(+i w_k t_j), x = a_1..a_N, S_1..S_N, or nullptr
     unsigned long long cond_handle;   // cudaGraphConditionalHandle (0: none)
     int pstride;

@@ -1,6 +1,6 @@
-// Explicit instantiations of the fused stage kernel WITH the dipolar field (k_stage<..., DEMAG = true>): T = double, n_sub = 1 (one TU per pair so
+// Explicit instantiations of the fused stage kernel WITH the dipolar field (k_stage<..., VARIANT = 1>): T = double, n_sub = 1 (one TU per pair so
 // the 56 kernels of each pair compile in parallel with the others).
-#define CAVMAG_DEMAG_INST true
+#define CAVMAG_VARIANT_INST 1
 #include "stage_kernel.cuh"
 
 namespace cavmag {

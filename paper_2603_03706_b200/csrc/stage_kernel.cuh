@@ -455,8 +455,11 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
 // ---------------------------------------------------------------------------------------
 // the stage kernel
 // ---------------------------------------------------------------------------------------
-template <typename T, int VEC, int STAGE, int NSUB, int NB, bool DEMAG = false>
+// VARIANT: 0 = the paper's field; 1 = + dipolar field (A.bdem, demag.cuh); 2 = per-mode polarisation (A.pol, reading G32).
+// Separate instantiations: as runtime branches the extra loads cost the plain kernels registers (6 % on CFG3).
+template <typename T, int VEC, int STAGE, int NSUB, int NB, int VARIANT = 0>
 __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __restrict__ trace) {
+    constexpr bool POL = VARIANT == 2;
     using P = Pack<T, VEC>;
     Ctrl* ctrl = A.ctrl;
     if (STAGE == 1) { if (ctrl->k1_valid) return; }
@@ -534,26 +537,42 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
             }
 
         // ---- mode profiles: RF field weight and overlap partials of THIS stage state ----
-        T brf[VEC];
+        T brf[VEC], brfy[POL ? VEC : 1], brfz[POL ? VEC : 1];
 #pragma unroll
-        for (int v = 0; v < VEC; ++v) brf[v] = (T)0;
+        for (int v = 0; v < VEC; ++v) { brf[v] = (T)0; if constexpr (POL) { brfy[v] = (T)0; brfz[v] = (T)0; } }
         if constexpr (NB > 0) {
-            T mcx[VEC], mcy[VEC];
+            T mcx[VEC], mcy[VEC], mcz[POL ? VEC : 1];
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
-                if constexpr (NSUB == 1) { mcx[v] = mc[0][0].v[v]; mcy[v] = mc[0][1].v[v]; }
-                else { mcx[v] = (T)0.5 * (mc[0][0].v[v] + mc[1][0].v[v]); mcy[v] = (T)0.5 * (mc[0][1].v[v] + mc[1][1].v[v]); }
+                if constexpr (NSUB == 1) { mcx[v] = mc[0][0].v[v]; mcy[v] = mc[0][1].v[v]; if constexpr (POL) mcz[v] = mc[0][2].v[v]; }
+                else {
+                    mcx[v] = (T)0.5 * (mc[0][0].v[v] + mc[1][0].v[v]); mcy[v] = (T)0.5 * (mc[0][1].v[v] + mc[1][1].v[v]);
+                    if constexpr (POL) mcz[v] = (T)0.5 * (mc[0][2].v[v] + mc[1][2].v[v]);
+                }
             }
 #pragma unroll
             for (int n = 0; n < NB; ++n) {
                 if (n < N) {
                     P un = ldp<T, VEC>(uu + (long long)n * nc + cell);
                     T sx = (T)0, sy = (T)0;
+                    if constexpr (!POL) {                  // p = x^, q = y^
 #pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        brf[v] += cn[n] * un.v[v];
-                        sx += un.v[v] * mcx[v];
-                        sy += un.v[v] * mcy[v];
+                        for (int v = 0; v < VEC; ++v) {
+                            brf[v] += cn[n] * un.v[v];
+                            sx += un.v[v] * mcx[v];
+                            sy += un.v[v] * mcy[v];
+                        }
+                    } else {                               // field along p_n, coupling to m.p_n - i m.q_n (reading G32)
+                        const double* pq = A.pol + 6 * n;
+                        const double cd = ctrl->c[n];
+                        const T cp0 = (T)(cd * pq[0]), cp1 = (T)(cd * pq[1]), cp2 = (T)(cd * pq[2]);
+                        const T p0 = (T)pq[0], p1 = (T)pq[1], p2 = (T)pq[2], q0 = (T)pq[3], q1 = (T)pq[4], q2 = (T)pq[5];
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) {
+                            brf[v] += cp0 * un.v[v]; brfy[v] += cp1 * un.v[v]; brfz[v] += cp2 * un.v[v];
+                            sx += un.v[v] * (mcx[v] * p0 + mcy[v] * p1 + mcz[v] * p2);
+                            sy += un.v[v] * (mcx[v] * q0 + mcy[v] * q1 + mcz[v] * q2);
+                        }
                     }
                     if (active) { ox[n] += sx; oy[n] += sy; }
                 }
@@ -563,7 +582,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
         // ---- optional dipolar field (off in the paper): computed before this launch by
         //      an FFT convolution of this stage's state (demag.cuh), the same for both sublattices ----
         P bdv[3];                                   // (its own instantiation: a runtime branch costs the others registers)
-        constexpr bool has_bd = DEMAG;
+        constexpr bool has_bd = VARIANT == 1;
         if constexpr (has_bd) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) bdv[c] = ldp<T, VEC>((const T*)A.bdem + (long long)c * nc + cell);
@@ -630,6 +649,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(const StageArgs A, double* __r
                 T Bx, By, Bz;
                 material_field(mx, my, mz, lap[0][v], lap[1][v], lap[2][v], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
                 Bx += brf[v];
+                if constexpr (POL) { By += brfy[v]; Bz += brfz[v]; }
                 if constexpr (NSUB == 2) {
                     Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
                 }
@@ -788,20 +808,25 @@ const void* stage_kernel_demag_f32_fm(int vec, int stage, int nb);
 const void* stage_kernel_demag_f32_afm(int vec, int stage, int nb);
 const void* stage_kernel_demag_f64_fm(int vec, int stage, int nb);
 const void* stage_kernel_demag_f64_afm(int vec, int stage, int nb);
+// and with per-mode polarisation (k_stage<..., VARIANT = 2>)
+const void* stage_kernel_pol_f32_fm(int vec, int stage, int nb);
+const void* stage_kernel_pol_f32_afm(int vec, int stage, int nb);
+const void* stage_kernel_pol_f64_fm(int vec, int stage, int nb);
+const void* stage_kernel_pol_f64_afm(int vec, int stage, int nb);
 
 #define CAVMAG_STAGE_CASES(T, VEC, NSUB, NB)                                       \
     switch (stage) {                                                               \
-        case 1: return (const void*)k_stage<T, VEC, 1, NSUB, NB, CAVMAG_DEMAG_INST>; \
-        case 2: return (const void*)k_stage<T, VEC, 2, NSUB, NB, CAVMAG_DEMAG_INST>; \
-        case 3: return (const void*)k_stage<T, VEC, 3, NSUB, NB, CAVMAG_DEMAG_INST>; \
-        case 4: return (const void*)k_stage<T, VEC, 4, NSUB, NB, CAVMAG_DEMAG_INST>; \
-        case 5: return (const void*)k_stage<T, VEC, 5, NSUB, NB, CAVMAG_DEMAG_INST>; \
-        case 6: return (const void*)k_stage<T, VEC, 6, NSUB, NB, CAVMAG_DEMAG_INST>; \
-        case 7: return (const void*)k_stage<T, VEC, 7, NSUB, NB, CAVMAG_DEMAG_INST>; \
+        case 1: return (const void*)k_stage<T, VEC, 1, NSUB, NB, CAVMAG_VARIANT_INST>; \
+        case 2: return (const void*)k_stage<T, VEC, 2, NSUB, NB, CAVMAG_VARIANT_INST>; \
+        case 3: return (const void*)k_stage<T, VEC, 3, NSUB, NB, CAVMAG_VARIANT_INST>; \
+        case 4: return (const void*)k_stage<T, VEC, 4, NSUB, NB, CAVMAG_VARIANT_INST>; \
+        case 5: return (const void*)k_stage<T, VEC, 5, NSUB, NB, CAVMAG_VARIANT_INST>; \
+        case 6: return (const void*)k_stage<T, VEC, 6, NSUB, NB, CAVMAG_VARIANT_INST>; \
+        case 7: return (const void*)k_stage<T, VEC, 7, NSUB, NB, CAVMAG_VARIANT_INST>; \
         default: return nullptr;                                                   \
     }
-#ifndef CAVMAG_DEMAG_INST
-#define CAVMAG_DEMAG_INST false      // a translation unit that instantiates the dipolar-field variants defines it to true
+#ifndef CAVMAG_VARIANT_INST
+#define CAVMAG_VARIANT_INST 0        // translation units that instantiate the dipolar-field / polarisation variants define it to 1 / 2
 #endif
 
 #define CAVMAG_DEFINE_LOOKUP(NAME, T, VECW, NSUB)                                  \

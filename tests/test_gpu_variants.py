@@ -40,6 +40,9 @@ def _axes(N, seed=3):
     ((8, 8, 4), 1, 2, 0.02e-12, "block"),
     ((40, 9, 7), 3, 1, 0.1e-12, "coop"),
     ((20, 12, 6), 2, 2, 0.02e-12, "coop"),
+    ((40, 9, 7), 3, 1, 0.1e-12, "generic"),
+    ((13, 5, 3), 2, 2, 0.02e-12, "generic"),       # scalar kernels, two sublattices
+    ((36, 10, 5), 9, 1, 0.1e-12, "generic"),       # 32-mode bucket
 ])
 @pytest.mark.parametrize("with_quad", [False, True])
 def test_polarisation_fixed_steps(api, prec, shape, N, n_sub, dt, path, with_quad):
@@ -59,9 +62,9 @@ def test_polarisation_fixed_steps(api, prec, shape, N, n_sub, dt, path, with_qua
         api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=120)
         m, a = sim.get_m(), sim.get_a()
         row = api.cav_get_trace(sim.h)[0]
-        with pytest.raises(api.CavError) as e:          # one-stage evaluation exists for x^-polarised modes only
-            api.cav_get_dadt(sim.h, N)
-        assert e.value.status == api.CAV_E_UNSUPPORTED
+        dadt = api.cav_get_dadt(sim.h, N)               # one-stage evaluation: the generic polarisation kernels
+    _, da_ref, _ = oracle_of(w, pol=p, quad=quad).rhs(ref.m, ref.a)
+    assert np.abs(dadt - da_ref).max() <= (1e-9 if prec == "f64" else 1e-3) * np.abs(da_ref).max()
     S = row[1 + 2 * N:1 + 4 * N:2] + 1j * row[2 + 2 * N:2 + 4 * N:2]
     assert_parity(m, a, ref, prec)
     plain = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=120)
@@ -85,9 +88,14 @@ def test_polarisation_default_and_limits(api):
         assert e.value.status == api.CAV_E_ARG
     big = small_problem(512, 160, 2, 1, 1)                                      # 163 840 cells > 512 x SMs
     with api.Sim(big, precision="f32") as sim:
-        with pytest.raises(api.CavError) as e:
-            api.cav_set_polarisation(sim.h, [[0.0, 1.0, 0.0]])
-        assert e.value.status == api.CAV_E_UNSUPPORTED
+        # beyond the small-grid kernel a polarised run takes the generic stage kernels (the TMA kernels keep x^)
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_set_polarisation(sim.h, [[0.0, 1.0, 0.0]])
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_GENERIC
+        big.m0 = big.m0.astype(np.float32).astype(np.float64); big.u = big.u.astype(np.float32).astype(np.float64)
+        refb = oracle_of(big, pol=[[0.0, 1.0, 0.0]]).run(big.m0, big.a0, fixed_dt=0.05e-12, max_steps=10)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=10)
+        assert_parity(sim.get_m(), sim.get_a(), refb, "f32")
         with pytest.raises(api.CavError) as e:
             api.cav_set_integrator(sim.h, api.CAV_INTEGRATOR_SPLIT, 1)
         assert e.value.status == api.CAV_E_UNSUPPORTED
