@@ -395,7 +395,8 @@ def run_cuda(args):
     if args.launch_mode == "stream":                  # profiling aid: host-enqueued stage kernels, same kernels
         api.cav_set_launch_mode(h, api.CAV_LAUNCH_STREAM)
     api.cav_run_steps(h, math.inf, tol=tol, max_steps=args.spinup)
-    # warm-up: W steps through the very same graph launch that is timed below
+    # warm-up: W steps (both run graphs - one step and four steps per WHILE iteration - are instantiated and uploaded by the
+    # first run; the spin-up above has already gone through the long-run graph that the timed launch uses)
     api.cav_run_steps(h, math.inf, tol=tol, max_steps=max(args.warmup, 1))
     api.cav_sync(h)
     st0 = api.cav_get_stats(h)

@@ -319,7 +319,7 @@ int cav_batch_get_trace(cav_batch* b, double* out /* [n_rep][capacity][row_len] 
  * Sweeps of mid-size grids: several simulations in one launch (the paper's 41-point field sweep, PAPER.md:229, :335,
  * on grids that are too large for cav_batch and too small to fill the GPU alone, e.g. 64 x 64 x 16 cells).
  * A sweep is a joint LAUNCHER over ordinary cav_sim handles: create and configure every simulation as usual (same grid,
- * precision, material and cell constants and number of modes; ferromagnet; at most 8 modes; B0, mode parameters, profiles
+ * precision, material and cell constants and number of modes; at most 8 modes (2 for the antiferromagnet); B0, mode parameters, profiles
  * and state may differ; all on the same stream), then cav_sweep_run advances all of them in ONE device-side loop: the
  * plane-tiles of all simulations form one work list for the persistent TMA grid, and every simulation keeps its own step
  * size, accept/reject decisions, trace and statistics.  Afterwards every cav_get_* / cav_set_* call works on the single

@@ -1413,7 +1413,8 @@ void sweep_destroy_graphs(cav_sweep* w) {
 }
 
 const void* stage_tma_sweep_fn(const cav_sim* q, int stage) {
-    return q->prm.precision == CAV_F32 ? stage_tma_sweep_kernel_f32(stage, q->nb) : stage_tma_sweep_kernel_f64(stage, q->nb);
+    return q->prm.precision == CAV_F32 ? stage_tma_sweep_kernel_f32(q->prm.n_sub, stage, q->nb)
+                                       : stage_tma_sweep_kernel_f64(q->prm.n_sub, stage, q->nb);
 }
 
 // k_sweep_begin -> K1 of every simulation (ordinary launches; they return at once when FSAL's k1 is valid) -> k_sweep_cond
@@ -1492,14 +1493,15 @@ int cav_sweep_create(cav_sim* const* sims, int n, cav_sweep** out) {
         cav_sim* q = sims[r];
         if (!q || !q->m_set) return q ? CAV_E_STATE : CAV_E_ARG;
         if (q->grid.nx != s->grid.nx || q->grid.ny != s->grid.ny || q->grid.nz != s->grid.nz || q->prm.precision != s->prm.precision ||
-            q->N != s->N || q->stream != s->stream || q->prm.renormalize != s->prm.renormalize)
+            q->N != s->N || q->stream != s->stream || q->prm.renormalize != s->prm.renormalize || q->prm.n_sub != s->prm.n_sub ||
+            q->prm.B_exch_inter != s->prm.B_exch_inter)
             return CAV_E_ARG;
         // the joint kernels take the material and cell constants from simulation 0: only B0, the modes and the state may differ
         if (q->grid.dx != s->grid.dx || q->grid.dy != s->grid.dy || q->grid.dz != s->grid.dz || q->prm.Ms != s->prm.Ms ||
             q->prm.Aex != s->prm.Aex || q->prm.Ku != s->prm.Ku || q->prm.alpha != s->prm.alpha || q->prm.gamma != s->prm.gamma ||
             memcmp(q->prm.ku_axis, s->prm.ku_axis, sizeof(s->prm.ku_axis)) != 0)
             return CAV_E_ARG;
-        if (q->prm.n_sub != 1 || !q->tma_eligible || q->demag || q->d_pol || q->split_nllg > 0 || q->nb > 8) return CAV_E_UNSUPPORTED;
+        if (!q->tma_eligible || q->demag || q->d_pol || q->split_nllg > 0 || q->nb > (q->prm.n_sub == 1 ? 8 : 2)) return CAV_E_UNSUPPORTED;
         for (int r2 = 0; r2 < r; ++r2) if (sims[r2] == q) return CAV_E_ARG;
     }
     if (s->targs[1].Q * (long long)n < (long long)s->n_sm) return CAV_E_UNSUPPORTED;      // not enough plane-tiles for a persistent grid

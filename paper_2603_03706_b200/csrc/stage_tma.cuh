@@ -1060,34 +1060,41 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const __grid_const
     stage_tma_body<T, STAGE, NSUB, NB, false>(A, TA, trace, SweepArgs{nullptr, 1, nullptr, 0ull});
 }
 
-// Joint launch over SW.R simulations of the same shape (ferromagnet): A carries the shared grid / material constants
-// (and simulation 0's pointers, unused), SW.reps the per-simulation pointers.
-template <typename T, int STAGE, int NB>
+// Joint launch over SW.R simulations of the same shape: A carries the shared grid / material constants (and simulation
+// 0's pointers, unused), SW.reps the per-simulation pointers.
+template <typename T, int STAGE, int NSUB, int NB>
 __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma_sweep(const __grid_constant__ StageArgs A, const __grid_constant__ TmaArgs TA,
                                                                     const __grid_constant__ SweepArgs SW) {
-    stage_tma_body<T, STAGE, 1, NB, true>(A, TA, nullptr, SW);
+    stage_tma_body<T, STAGE, NSUB, NB, true>(A, TA, nullptr, SW);
 }
 
-const void* stage_tma_sweep_kernel_f32(int stage, int nb);
-const void* stage_tma_sweep_kernel_f64(int stage, int nb);
+const void* stage_tma_sweep_kernel_f32(int n_sub, int stage, int nb);
+const void* stage_tma_sweep_kernel_f64(int n_sub, int stage, int nb);
 
-#define CAVMAG_TMA_SWEEP_CASES(T, NB)                                              \
+#define CAVMAG_TMA_SWEEP_CASES(T, NSUB, NB)                                        \
     switch (stage) {                                                               \
-        case 2: return (const void*)k_stage_tma_sweep<T, 2, NB>;                   \
-        case 3: return (const void*)k_stage_tma_sweep<T, 3, NB>;                   \
-        case 4: return (const void*)k_stage_tma_sweep<T, 4, NB>;                   \
-        case 5: return (const void*)k_stage_tma_sweep<T, 5, NB>;                   \
-        case 6: return (const void*)k_stage_tma_sweep<T, 6, NB>;                   \
-        case 7: return (const void*)k_stage_tma_sweep<T, 7, NB>;                   \
+        case 2: return (const void*)k_stage_tma_sweep<T, 2, NSUB, NB>;             \
+        case 3: return (const void*)k_stage_tma_sweep<T, 3, NSUB, NB>;             \
+        case 4: return (const void*)k_stage_tma_sweep<T, 4, NSUB, NB>;             \
+        case 5: return (const void*)k_stage_tma_sweep<T, 5, NSUB, NB>;             \
+        case 6: return (const void*)k_stage_tma_sweep<T, 6, NSUB, NB>;             \
+        case 7: return (const void*)k_stage_tma_sweep<T, 7, NSUB, NB>;             \
         default: return nullptr;                                                   \
     }
-// the sweeps of the paper have 1-3 modes: mode buckets 0, 1, 2 and 8
+// the sweeps of the paper have 1-3 modes: mode buckets 0, 1, 2 and 8 for the ferromagnet,
+// 0, 1 and 2 for the two-sublattice antiferromagnet
 #define CAVMAG_DEFINE_TMA_SWEEP_LOOKUP(NAME, T)                                    \
-    const void* NAME(int stage, int nb) {                                          \
-        if (nb == 0) { CAVMAG_TMA_SWEEP_CASES(T, 0) }                              \
-        if (nb == 1) { CAVMAG_TMA_SWEEP_CASES(T, 1) }                              \
-        if (nb == 2) { CAVMAG_TMA_SWEEP_CASES(T, 2) }                              \
-        if (nb == 8) { CAVMAG_TMA_SWEEP_CASES(T, 8) }                              \
+    const void* NAME(int n_sub, int stage, int nb) {                               \
+        if (n_sub == 1) {                                                          \
+            if (nb == 0) { CAVMAG_TMA_SWEEP_CASES(T, 1, 0) }                       \
+            if (nb == 1) { CAVMAG_TMA_SWEEP_CASES(T, 1, 1) }                       \
+            if (nb == 2) { CAVMAG_TMA_SWEEP_CASES(T, 1, 2) }                       \
+            if (nb == 8) { CAVMAG_TMA_SWEEP_CASES(T, 1, 8) }                       \
+        } else {                                                                   \
+            if (nb == 0) { CAVMAG_TMA_SWEEP_CASES(T, 2, 0) }                       \
+            if (nb == 1) { CAVMAG_TMA_SWEEP_CASES(T, 2, 1) }                       \
+            if (nb == 2) { CAVMAG_TMA_SWEEP_CASES(T, 2, 2) }                       \
+        }                                                                          \
         return nullptr;                                                            \
     }
 

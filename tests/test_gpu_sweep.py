@@ -178,3 +178,33 @@ def test_members_stay_ordinary_handles(api, stream):
         api.cav_sweep_destroy(sw)
         for sim in sims:
             sim.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_sweep_of_antiferromagnets(api, prec, stream):
+    """The paper's AFM protocol is a field sweep too: six two-sublattice members of cfg4's recipe on
+    64 x 32 x 8 cells with dissipative coupling and different fields, each against its own oracle run."""
+    ws = []
+    for r in range(6):
+        w = W.cfg4(nx=64, ny=32, nz=8, seed=4000 + r, dissipative=True)
+        w.B0 = (0.0, 0.0, 0.05 * r)
+        w.a0 = np.array([2e-3 + 1e-3j])
+        if prec == "f32":
+            w.m0 = w.m0.astype(np.float32).astype(np.float64)
+            w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+        ws.append(w)
+    sims = [api.Sim(w, precision=prec, stream=stream) for w in ws]
+    sw = api.cav_sweep_create(sims)
+    try:
+        api.cav_sweep_run(sw, math.inf, fixed_dt=0.02e-12, max_steps=60)
+        for w, sim in zip(ws, sims):
+            ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.02e-12, max_steps=60)
+            if prec == "f64":
+                assert_parity(sim.get_m(), sim.get_a(), ref, prec)
+            else:
+                assert np.abs(sim.get_m() - ref.m).max() <= 1e-4
+                assert np.abs(sim.get_a() - ref.a).max() <= 1e-4 * np.abs(ref.a).max()
+    finally:
+        api.cav_sweep_destroy(sw)
+        for sim in sims:
+            sim.close()
