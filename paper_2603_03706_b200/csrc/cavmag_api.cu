@@ -605,6 +605,39 @@ int add_kernel(cav_sim* s, cudaGraph_t g, cudaGraphNode_t* node, const cudaGraph
 // kernel, so a body may hold several steps: the WHILE condition is then evaluated once per `unroll` steps (one loop
 // iteration costs ~6 us of idle GPU between K7 and the next K2), and the kernels after the step that ends the run
 // return at once.
+int launch_stage(cav_sim* s, int stage, StageArgs& A, cudaStream_t stream);
+
+// With the dipolar field a stage is a chain of launches, cuFFT's among them, which only cuFFT can enqueue: those are
+// recorded by stream capture INTO the run graph (stage 1 behind k_begin, stages 2..7 into the body of the WHILE node) from
+// a private stream, so the run is the same single graph launch as without the field.
+int capture_stages(cav_sim* s, cudaGraph_t into, const cudaGraphNode_t* dep, int first, int last, StageArgs& A,
+                   cudaGraphNode_t* tail, size_t* n_tail) {
+    cudaStream_t cs = nullptr;
+    CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    cudaError_t e = cudaStreamBeginCaptureToGraph(cs, into, dep, nullptr, dep ? 1 : 0, cudaStreamCaptureModeThreadLocal);
+    int rc = CAV_OK;
+    if (e == cudaSuccess) {
+        for (int stage = first; stage <= last && rc == CAV_OK; ++stage) rc = launch_stage(s, stage, A, cs);
+        if (rc == CAV_OK && tail) {
+            cudaStreamCaptureStatus st;
+            const cudaGraphNode_t* deps = nullptr;
+            size_t nd = 0;
+            e = cudaStreamGetCaptureInfo(cs, &st, nullptr, nullptr, &deps, &nd);
+            if (e == cudaSuccess && nd >= 1 && nd <= 4) { for (size_t i = 0; i < nd; ++i) tail[i] = deps[i]; *n_tail = nd; }
+            else rc = CAV_E_CUDA;
+        }
+        cudaGraph_t g = nullptr;
+        const cudaError_t e2 = cudaStreamEndCapture(cs, &g);
+        if (e == cudaSuccess) e = e2;
+    }
+    cudaStreamDestroy(cs);
+    if (rc == CAV_OK && e != cudaSuccess) {
+        snprintf(s->cuda_err, sizeof(s->cuda_err), "capture of the dipolar-field stages: %s", cudaGetErrorString(e));
+        rc = CAV_E_CUDA;
+    }
+    return rc;
+}
+
 int build_graph_impl(cav_sim* s, int which, bool pdl, int unroll) {
     choose_grid(s);
     decide_path(s);
@@ -624,21 +657,31 @@ int build_graph_impl(cav_sim* s, int which, bool pdl, int unroll) {
         int rc = add_kernel(s, graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params, 0);
         if (rc) return rc;
     }
-    {
+    cudaGraphNode_t tail[4];
+    size_t n_tail = 1;
+    if (s->demag) {
+        int rc = capture_stages(s, graph, &n_begin, 1, 1, A, tail, &n_tail);
+        if (rc) return rc;
+    } else {
         void* params[] = {&A, &trace};
         void* tparams[] = {&A, &s->targs[1], &trace};
         int rc = s->use_tma ? add_kernel(s, graph, &n_k1, &n_begin, stage_tma_fn(s, 1), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[1])
                             : add_kernel(s, graph, &n_k1, &n_begin, stage_fn(s, 1), dim3(s->nblocks), dim3(kBlock), params, 0);
         if (rc) return rc;
+        tail[0] = n_k1;
     }
     cudaGraphNodeParams cp = {};
     cp.type = cudaGraphNodeTypeConditional;
     cp.conditional.handle = handle;
     cp.conditional.type = cudaGraphCondTypeWhile;
     cp.conditional.size = 1;
-    CK(cudaGraphAddNode(&n_while, graph, &n_k1, 1, &cp));
+    CK(cudaGraphAddNode(&n_while, graph, tail, n_tail, &cp));
     cudaGraph_t body = cp.conditional.phGraph_out[0];
     cudaGraphNode_t prev;
+    if (s->demag) {
+        int rc = capture_stages(s, body, nullptr, 2, 7, A, nullptr, nullptr);
+        if (rc) return rc;
+    } else
     for (int u = 0; u < unroll; ++u)
         for (int stage = 2; stage <= 7; ++stage) {
             void* params[] = {&A, &trace};
@@ -684,19 +727,19 @@ int build_graph(cav_sim* s) {
     return rc;
 }
 
-int launch_stage(cav_sim* s, int stage, StageArgs& A) {
+int launch_stage(cav_sim* s, int stage, StageArgs& A, cudaStream_t stream) {
     double* trace = s->d_trace;
     if (s->demag) {          // dipolar field of the state this stage is evaluated at, then the stage kernel that adds it
-        int rc = demag_apply(s->demag, A, stage, s->d_bdem, s->stream);
+        int rc = demag_apply(s->demag, A, stage, s->d_bdem, stream);
         if (rc) { snprintf(s->cuda_err, sizeof(s->cuda_err), "demag_apply failed at stage %d", stage); return rc; }
-        s->host_launches += 5;
+        if (stream == s->stream) s->host_launches += 5;
     }
     if (s->use_tma) {
         void* tparams[] = {&A, &s->targs[stage], &trace};
-        CK(cudaLaunchKernel(stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], s->stream));
+        CK(cudaLaunchKernel(stage_tma_fn(s, stage), dim3(s->tgrid), dim3(kTmaThreads), tparams, s->tsmem[stage], stream));
     } else {
         void* params[] = {&A, &trace};
-        CK(cudaLaunchKernel(stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0, s->stream));
+        CK(cudaLaunchKernel(stage_fn(s, stage), dim3(s->nblocks), dim3(kBlock), params, 0, stream));
     }
     return CAV_OK;
 }
@@ -707,13 +750,13 @@ int run_stream_mode(cav_sim* s) {
     StageArgs A = make_args(s, 0ull);
     k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
     CK(cudaGetLastError());
-    int rc = launch_stage(s, 1, A);
+    int rc = launch_stage(s, 1, A, s->stream);
     if (rc) return rc;
     const int chunk = 16;
     for (;;) {
         for (int i = 0; i < chunk; ++i)
             for (int stage = 2; stage <= 7; ++stage) {
-                rc = launch_stage(s, stage, A);
+                rc = launch_stage(s, stage, A, s->stream);
                 if (rc) return rc;
             }
         CK(cudaMemcpyAsync(s->h_flag, &s->d_ctrl->done, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
@@ -1209,7 +1252,7 @@ static int ensure_k1(cav_sim* s) {
         k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
         CK(cudaGetLastError());
         s->host_launches++;
-        rc = launch_stage(s, 1, A);
+        rc = launch_stage(s, 1, A, s->stream);
         if (rc) return rc;
         rc = sync_pull(s);
     }
@@ -1259,9 +1302,15 @@ int cav_run_steps(cav_sim* s, double t_end, double tol, double fixed_dt, double 
     k_setrun<<<1, 1, 0, s->stream>>>(s->d_ctrl, t_end, adaptive ? tol : 0.0, adaptive ? 0.0 : fixed_dt, dt_init, max_steps);
     CK(cudaGetLastError());
     s->host_launches++;
-    if (s->launch_mode == CAV_LAUNCH_GRAPH && !s->demag) {
+    if (s->launch_mode == CAV_LAUNCH_GRAPH) {
         if (s->graph_dirty || !s->exec[0] || !s->exec[1]) {
             int rc = build_graph(s);
+            if (rc && s->demag) {                    // cuFFT's launches could not be captured here: enqueue from the host
+                cudaGetLastError();
+                destroy_graph(s);
+                s->host_launches++;
+                return run_stream_mode(s);
+            }
             if (rc) return rc;
         }
         const int which = (max_steps == 0 || max_steps >= kUnrollMinSteps) ? 1 : 0;

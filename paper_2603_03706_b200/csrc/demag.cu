@@ -1,10 +1,21 @@
-// Dipolar field by FFT convolution (see demag.cuh).  cuFFT does the transforms (a library primitive); the tensor, the
-// gather of the stage state, the tensor product and the scatter are kernels of this file.
+// Dipolar field by FFT convolution (see demag.cuh).
+//
+// Layout of one evaluation (nz <= 64, the usual case: films and slabs):
+//   gather   stage state, summed over the sublattices -> [3][nz][Py][Px] real, zero-padded in x and y only
+//   cuFFT    batched 2-D R2C over (y, x), 3 nz planes: the planes that would only hold zeros are never transformed
+//   k_demag_zconv   per (ky, kx) column and in shared memory: zero-pad to Pz, FFT along z, product with the tensor's
+//            transform, inverse FFT along z, keep z < nz - the full [Pz][Py][Px/2+1] spectrum never exists in memory.
+//            The tensor's transform is real and even/odd in every index: one octant of it is stored, as reals.
+//   cuFFT    batched 2-D C2R, then the scatter of the nx x ny corner into the dense field.
+// This moves about a third of the bytes of a padded 3-D transform pair with a separate product kernel (kept below as the
+// fallback for nz > 64, where the columns of a block do not fit shared memory).  cuFFT does the x/y transforms (a library
+// primitive); the tensor, the gather, the z convolution and the scatter are kernels of this file.
 #include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <dlfcn.h>
 #include <new>
+#include <type_traits>
 
 #include <cufft.h>     // types and enums only: the entry points are resolved with dlsym
 
@@ -114,22 +125,306 @@ __global__ void k_store_khat(const cufftDoubleComplex* src, C* dst, long long n,
     dst[i].y = (decltype(dst[i].y))(src[i].y * scale);
 }
 
+// real part of one tensor component's transform on the octant kz <= Pz/2, ky <= Py/2, kx <= Px/2, scaled.  (The tensor
+// is real and, per index, even or odd with a zero at the origin and at the unused offset n: its transform is real, and
+// +-1 times itself under k -> P - k.  The imaginary parts left by rounding are dropped.)
+template <typename T>
+__global__ void k_store_khat_real(const cufftDoubleComplex* src, T* dst, int NZH, int NYH, int NXH, int Py, double scale) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)NZH * NYH * NXH) return;
+    const int kx = (int)(i % NXH), ky = (int)((i / NXH) % NYH), kz = (int)(i / ((long long)NXH * NYH));
+    dst[i] = (T)(src[((long long)kz * Py + ky) * NXH + kx].x * scale);
+}
+
+// columns (ky, kx) per block of the z convolution: a warp per worker row in fp32 (positions and twiddles are warp-uniform)
+template <typename T> struct ZTile { static constexpr int value = sizeof(T) == 4 ? 32 : 16; };
+
+// ---- radix-2 levels of the z transform on values held in registers (W = exp(-2 pi i / Pz), tw[j] = W^j) ----
+template <typename C> __device__ __forceinline__ C c_add(const C& a, const C& b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
+template <typename C> __device__ __forceinline__ C c_sub(const C& a, const C& b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
+template <typename C> __device__ __forceinline__ C c_mul(const C& a, const C& b) { C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
+template <typename C> __device__ __forceinline__ C c_mulc(const C& a, const C& b) { C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r; }   // a conj(b)
+// decimation in frequency, spans h and h/2, on positions p0, p0 + h/2, p0 + h, p0 + 3h/2 (v[0..3]); t1a, t1b: span-h
+// twiddles of the two pairs, t2: span-h/2 twiddle
+template <typename C> __device__ __forceinline__ void dif4(C* v, const C& t1a, const C& t1b, const C& t2) {
+    const C a0 = c_add(v[0], v[2]), a2 = c_mul(c_sub(v[0], v[2]), t1a);
+    const C a1 = c_add(v[1], v[3]), a3 = c_mul(c_sub(v[1], v[3]), t1b);
+    v[0] = c_add(a0, a1); v[1] = c_mul(c_sub(a0, a1), t2);
+    v[2] = c_add(a2, a3); v[3] = c_mul(c_sub(a2, a3), t2);
+}
+// decimation in time with conjugate twiddles, spans h and 2h, on positions p0, p0 + h, p0 + 2h, p0 + 3h
+template <typename C> __device__ __forceinline__ void dit4(C* v, const C& t1, const C& t2a, const C& t2b) {
+    const C b1 = c_mulc(v[1], t1), b3 = c_mulc(v[3], t1);
+    const C a0 = c_add(v[0], b1), a1 = c_sub(v[0], b1);
+    const C a2 = c_mulc(c_add(v[2], b3), t2a), a3 = c_mulc(c_sub(v[2], b3), t2b);
+    v[0] = c_add(a0, a2); v[2] = c_sub(a0, a2);
+    v[1] = c_add(a1, a3); v[3] = c_sub(a1, a3);
+}
+
+// the middle pass (forward spans 2 and 1, product by the caller in between, inverse spans 1 and 2) has only the
+// twiddles 1 and W^(Pz/4) = -i: no complex multiplications
+template <typename C> __device__ __forceinline__ C c_mul_mi(const C& a) { C r; r.x = a.y; r.y = -a.x; return r; }    // a (-i)
+template <typename C> __device__ __forceinline__ C c_mul_pi(const C& a) { C r; r.x = -a.y; r.y = a.x; return r; }    // a (+i) = a conj(-i)
+template <typename C> __device__ __forceinline__ void dif4_mid(C* v) {
+    const C a0 = c_add(v[0], v[2]), a2 = c_sub(v[0], v[2]);
+    const C a1 = c_add(v[1], v[3]), a3 = c_mul_mi(c_sub(v[1], v[3]));
+    v[0] = c_add(a0, a1); v[1] = c_sub(a0, a1);
+    v[2] = c_add(a2, a3); v[3] = c_sub(a2, a3);
+}
+template <typename C> __device__ __forceinline__ void dit4_mid(C* v) {
+    const C a0 = c_add(v[0], v[1]), a1 = c_sub(v[0], v[1]);
+    const C a2 = c_add(v[2], v[3]), a3 = c_mul_pi(c_sub(v[2], v[3]));
+    v[0] = c_add(a0, a2); v[2] = c_sub(a0, a2);
+    v[1] = c_add(a1, a3); v[3] = c_sub(a1, a3);
+}
+// first forward pass of a padded column: v[2] = v[3] = 0 (positions >= Pz/2 >= nz)
+template <typename C> __device__ __forceinline__ void dif4_padded(C* v, const C& t1a, const C& t1b, const C& t2) {
+    const C a2 = c_mul(v[0], t1a), a3 = c_mul(v[1], t1b);
+    const C a0 = v[0], a1 = v[1];
+    v[0] = c_add(a0, a1); v[1] = c_mul(c_sub(a0, a1), t2);
+    v[2] = c_add(a2, a3); v[3] = c_mul(c_sub(a2, a3), t2);
+}
+// last inverse pass of a padded column: only the positions below Pz/2 (v[0], v[1]) are wanted
+template <typename C> __device__ __forceinline__ void dit4_padded(C* v, const C& t1, const C& t2a, const C& t2b) {
+    const C b1 = c_mulc(v[1], t1), b3 = c_mulc(v[3], t1);
+    const C a2 = c_mulc(c_add(v[2], b3), t2a), a3 = c_mulc(c_sub(v[2], b3), t2b);
+    const C x0 = v[0];
+    v[0] = c_add(c_add(x0, b1), a2);
+    v[1] = c_add(c_sub(x0, b1), a3);
+}
+
+// One block: TK consecutive columns (ky, kx) of the half-spectrum, the three field components, the whole z column.
+//   F [3][nz][Py][NXH] complex (in place), K [6][Pz/2+1][Py/2+1][NXH] real, Pz = 2^q >= 2 nz - 1 (q = 0: no z transform)
+// Forward: decimation in frequency (natural order in, bit-reversed out); the product is pointwise, so it is taken at the
+// bit-reversed positions; inverse: decimation in time (bit-reversed in, natural out), unnormalised (1/(Px Py Pz) is
+// folded into K).  A pass does two radix-2 levels on four values per component held in registers (one level on two
+// values where q is odd).  The first pass reads global memory (zero beyond nz), the last one writes it (below nz only),
+// and the last forward pass, the product and the first inverse pass work on the same positions and are one pass:
+// ceil(q/2) * 2 - 1 passes with a shared-memory exchange between them.
+__host__ __device__ constexpr int zconv_rows(int q) { return (1 << q) / 4 < 1 ? 1 : ((1 << q) / 4 > 32 ? 32 : (1 << q) / 4); }   // blockDim.y
+__host__ __device__ constexpr int zconv_min_blocks(int q, int tk, int tsize) {           // registers: 64 (fp32) / 128 (fp64) per thread
+    const int b = 1024 / (zconv_rows(q) * tk) / (tsize == 4 ? 1 : 2);
+    return b < 1 ? 1 : (tsize == 8 && b > 4 ? 4 : b);
+}
+
+template <typename T, typename C, int q>
+__global__ void __launch_bounds__(zconv_rows(q) * ZTile<T>::value, zconv_min_blocks(q, ZTile<T>::value, (int)sizeof(T)))
+k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NXH) {
+    constexpr int Pz = 1 << q;
+    constexpr int NJ = zconv_rows(q);
+    constexpr int kZTile = ZTile<T>::value;
+    extern __shared__ __align__(16) unsigned char zsm[];
+    C* const sm = reinterpret_cast<C*>(zsm);                    // [3][Pz][kZTile]
+    C* const tw = sm + 3 * Pz * kZTile;                         // exp(-2 pi i j / Pz), j < Pz/2
+    T* const ks = reinterpret_cast<T*>(tw + (Pz / 2 > 0 ? Pz / 2 : 1));       // the tensor's transform for this block: [6][Pz/2+1][kZTile]
+    const int k = threadIdx.x, j = threadIdx.y;
+    const long long zs = (long long)Py * NXH;                   // z stride = columns per plane
+    const long long col = (long long)blockIdx.x * kZTile + k;
+    const bool live = col < zs;
+    const int ky = live ? (int)(col / NXH) : 0, kx = live ? (int)(col % NXH) : 0;
+    C* const Fc = F + col;                                      // this thread's column: Fc[(c nz + z) zs]
+    for (int t = j * kZTile + k; t < Pz / 2; t += NJ * kZTile) {
+        double sn, cs;
+        sincospi(-2.0 * (double)t / (double)Pz, &sn, &cs);
+        tw[t].x = (T)cs; tw[t].y = (T)sn;
+    }
+    const int kys = ky <= Py / 2 ? ky : Py - ky;
+    const T sy = ky <= Py / 2 ? (T)1 : (T)-1;
+    constexpr int NZH = Pz / 2 + 1;
+    const int NYH = Py / 2 + 1;
+    const long long cst = (long long)NZH * NYH * NXH;
+    // the block's slice of the tensor's transform goes to shared memory asynchronously: it is needed two passes later
+    if (live) {
+        const T* const Kc = K + (long long)kys * NXH + kx;
+        for (int t = j; t < 6 * NZH; t += NJ) {
+            const int comp = t / NZH, kzs = t % NZH;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(ks + t * kZTile + k);
+            const T* src = Kc + comp * cst + (long long)kzs * NYH * NXH;
+            if constexpr (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+            else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+        }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    // G = Khat F at position pos of the (bit-reversed) spectrum, for the three components in f[0..2]
+    auto product = [&](int pos, C& fx, C& fy, C& fz) {
+        const int kz = q > 0 ? (int)(__brev((unsigned)pos) >> ((32 - q) & 31)) : 0;
+        const int kzs = kz <= Pz / 2 ? kz : Pz - kz;
+        const T sz = kz <= Pz / 2 ? (T)1 : (T)-1;
+        const T* const kk = ks + kzs * kZTile + k;
+        constexpr int cs6 = NZH * kZTile;
+        const T kxx = kk[0], kyy = kk[cs6], kzz = kk[2 * cs6];
+        const T kxy = sy * kk[3 * cs6], kxz = sz * kk[4 * cs6], kyz = sy * sz * kk[5 * cs6];
+        C gx, gy, gz;
+        gx.x = kxx * fx.x + kxy * fy.x + kxz * fz.x; gx.y = kxx * fx.y + kxy * fy.y + kxz * fz.y;
+        gy.x = kxy * fx.x + kyy * fy.x + kyz * fz.x; gy.y = kxy * fx.y + kyy * fy.y + kyz * fz.y;
+        gz.x = kxz * fx.x + kyz * fy.x + kzz * fz.x; gz.y = kxz * fx.y + kyz * fy.y + kzz * fz.y;
+        fx = gx; fy = gy; fz = gz;
+    };
+    C zero; zero.x = (T)0; zero.y = (T)0;
+    if constexpr (q == 0) {                                     // a film: one plane, no z transform
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        if (live && j == 0) {
+            C fx = Fc[0], fy = Fc[zs], fz = Fc[2 * zs];          // (nz = 1)
+            product(0, fx, fy, fz);
+            Fc[0] = fx; Fc[zs] = fy; Fc[2 * zs] = fz;
+        }
+    } else {
+    if constexpr (q <= 2) asm volatile("cp.async.wait_group 0;" ::: "memory");       // one pass: the product is in it
+    __syncthreads();                                            // twiddles
+    constexpr int ngrp = (q + 1) / 2;                           // passes per direction
+    constexpr bool odd = (q & 1) != 0;
+    const long long cz = (long long)nz * zs;                    // component stride
+    // ---------------- forward pass g (the last one goes on into the product and the first inverse pass)
+    auto forward = [&](auto G) {
+        constexpr int g = decltype(G)::value;
+        constexpr bool single = odd && g == ngrp - 1;           // the lone span-1 level
+        constexpr int h = (Pz / 2) >> (2 * g);                  // upper span of this pass
+        constexpr bool first = g == 0, mid = g == ngrp - 1;
+        constexpr bool last_too = mid && ngrp == 1;             // q <= 2: everything in registers
+        if constexpr (!single) {
+            constexpr int hh = h / 2, s1 = Pz / (2 * h);
+#pragma unroll
+            for (int w0 = 0; w0 < Pz / 4; w0 += NJ) {
+                const int w = w0 + j;
+                const int r = w % hh, p0 = (w / hh) * 2 * h + r;
+                const int pos[4] = {p0, p0 + hh, p0 + h, p0 + h + hh};
+                const C t1a = tw[r * s1], t1b = tw[(r + hh) * s1], t2 = tw[r * 2 * s1];
+                C v[3][4];
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if constexpr (first) v[c][e] = (e < 2 && live && pos[e] < nz) ? Fc[c * cz + pos[e] * zs] : zero;
+                        else v[c][e] = sm[(c * Pz + pos[e]) * kZTile + k];
+                    }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    if constexpr (first) dif4_padded(v[c], t1a, t1b, t2);
+                    else if constexpr (mid) dif4_mid(v[c]);
+                    else dif4(v[c], t1a, t1b, t2);
+                }
+                if constexpr (mid) {                            // positions 4w .. 4w+3: product, then inverse spans 1 and 2
+                    if (live) {
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) product(pos[e], v[0][e], v[1][e], v[2][e]);
+                    }
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) dit4_mid(v[c]);
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if constexpr (last_too) { if (live && pos[e] < nz) Fc[c * cz + pos[e] * zs] = v[c][e]; }
+                        else sm[(c * Pz + pos[e]) * kZTile + k] = v[c][e];
+                    }
+            }
+        } else {                                                // span 1 alone (q odd): pairs 2w, 2w+1; then product and inverse span 1
+#pragma unroll
+            for (int w0 = 0; w0 < Pz / 2; w0 += NJ) {
+                const int w = w0 + j;
+                const int pos[2] = {2 * w, 2 * w + 1};
+                C v[3][2];
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        if constexpr (first) v[c][e] = (live && pos[e] < nz) ? Fc[c * cz + pos[e] * zs] : zero;
+                        else v[c][e] = sm[(c * Pz + pos[e]) * kZTile + k];
+                    }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { const C a = v[c][0], b = v[c][1]; v[c][0] = c_add(a, b); v[c][1] = c_sub(a, b); }
+                if (live) {
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) product(pos[e], v[0][e], v[1][e], v[2][e]);
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { const C a = v[c][0], b = v[c][1]; v[c][0] = c_add(a, b); v[c][1] = c_sub(a, b); }
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        if constexpr (last_too) { if (live && pos[e] < nz) Fc[c * cz + pos[e] * zs] = v[c][e]; }
+                        else sm[(c * Pz + pos[e]) * kZTile + k] = v[c][e];
+                    }
+            }
+        }
+        if constexpr (g == ngrp - 2) asm volatile("cp.async.wait_group 0;" ::: "memory");  // the next pass multiplies
+        if constexpr (!last_too) __syncthreads();
+    };
+    // ---------------- inverse pass g >= 1: spans (h, 2h), h = 4, 16, ... (q even) or 2, 8, ... (q odd)
+    auto inverse = [&](auto G) {
+        constexpr int g = decltype(G)::value;
+        constexpr int h = odd ? (2 << (2 * (g - 1))) : (1 << (2 * g));
+        constexpr int s1 = Pz / (2 * h), s2 = Pz / (4 * h);
+        constexpr bool last = g == ngrp - 1;
+#pragma unroll
+        for (int w0 = 0; w0 < Pz / 4; w0 += NJ) {
+            const int w = w0 + j;
+            const int r = w % h, p0 = (w / h) * 4 * h + r;
+            const int pos[4] = {p0, p0 + h, p0 + 2 * h, p0 + 3 * h};
+            const C t1 = tw[r * s1], t2a = tw[r * s2], t2b = tw[(r + h) * s2];
+            C v[3][4];
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[c][e] = sm[(c * Pz + pos[e]) * kZTile + k];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                if constexpr (last) dit4_padded(v[c], t1, t2a, t2b);
+                else dit4(v[c], t1, t2a, t2b);
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    if constexpr (last) { if (e < 2 && live && pos[e] < nz) Fc[c * cz + pos[e] * zs] = v[c][e]; }
+                    else sm[(c * Pz + pos[e]) * kZTile + k] = v[c][e];
+                }
+        }
+        if constexpr (!last) __syncthreads();
+    };
+    using std::integral_constant;
+    forward(integral_constant<int, 0>{});
+    if constexpr (ngrp > 1) forward(integral_constant<int, 1>{});
+    if constexpr (ngrp > 2) forward(integral_constant<int, 2>{});
+    if constexpr (ngrp > 3) forward(integral_constant<int, 3>{});
+    if constexpr (ngrp > 1) inverse(integral_constant<int, 1>{});
+    if constexpr (ngrp > 2) inverse(integral_constant<int, 2>{});
+    if constexpr (ngrp > 3) inverse(integral_constant<int, 3>{});
+    }
+}
+
+template <typename T, typename C>
+const void* zconv_fn(int q) {
+    switch (q) {
+        case 0: return (const void*)k_demag_zconv<T, C, 0>;
+        case 1: return (const void*)k_demag_zconv<T, C, 1>;
+        case 2: return (const void*)k_demag_zconv<T, C, 2>;
+        case 3: return (const void*)k_demag_zconv<T, C, 3>;
+        case 4: return (const void*)k_demag_zconv<T, C, 4>;
+        case 5: return (const void*)k_demag_zconv<T, C, 5>;
+        case 6: return (const void*)k_demag_zconv<T, C, 6>;
+        default: return (const void*)k_demag_zconv<T, C, 7>;
+    }
+}
+
 // The state stage `stage` is evaluated at, summed over the sublattices, into the zero-padded array [3][Pz][Py][Px]
 // (the pad region is zeroed once and never written).  Buffer indices and h as the stage kernel reads them.
 template <typename T>
 __global__ void k_demag_gather(const StageArgs A, int stage, int n_sub, T* pad, int Px, int Py, int Pz) {
     const Ctrl* c = A.ctrl;
     if (stage == 1 ? c->k1_valid : c->done) return;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, z = blockIdx.z;     // grid: (ceil(nx / block), ny, nz)
+    if (x >= A.nx) return;
     const long long nc = A.nc;
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nc) return;
+    const long long i = ((long long)z * A.ny + y) * A.nx + x;
     const int ycur = c->ycur, k1slot = c->k1slot;
     const T* y0 = (const T*)(ycur ? A.Y[1] : A.Y[0]);
     const T* ynew = (const T*)(ycur ? A.Y[0] : A.Y[1]);
     const T* k1 = (const T*)(k1slot ? A.K[6] : A.K[0]);
     const T* ms = stage == 1 ? y0 : stage == 7 ? ynew : (stage == 3 || stage == 5) ? (const T*)A.MS[0] : (const T*)A.MS[1];
     const T ha21 = (T)c->h * (T)kA[1][0];
-    const int x = (int)(i % A.nx), y = (int)((i / A.nx) % A.ny), z = (int)(i / ((long long)A.nx * A.ny));
     const long long o = ((long long)z * Py + y) * Px + x, pvol = (long long)Px * Py * Pz;
     for (int comp = 0; comp < 3; ++comp) {
         T v = (T)0;
@@ -157,9 +452,9 @@ __global__ void k_demag_product(C* F, const C* K, long long nf) {
 
 template <typename T>
 __global__ void k_demag_scatter(const T* conv, T* bdem, int nx, int ny, long long nc, int Px, int Py, int Pz) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nc) return;
-    const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((long long)nx * ny));
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, z = blockIdx.z;     // grid: (ceil(nx / block), ny, nz)
+    if (x >= nx) return;
+    const long long i = ((long long)z * ny + y) * nx + x;
     const long long o = ((long long)z * Py + y) * Px + x, pvol = (long long)Px * Py * Pz;
     for (int comp = 0; comp < 3; ++comp) bdem[comp * nc + i] = conv[comp * pvol + o];
 }
@@ -168,15 +463,22 @@ __global__ void k_demag_scatter(const T* conv, T* bdem, int nx, int ny, long lon
 
 struct DemagPlan {
     int nx = 0, ny = 0, nz = 0, Px = 0, Py = 0, Pz = 0, n_sub = 1;
+    int q = 0;                           // zfused: Pz = 2^q
     bool f32 = true;
-    long long pvol = 0, nf = 0;          // padded real points, complex points per component
-    void* pad = nullptr;                 // [3][pvol] real: gathered state (pad region stays zero)
-    void* freq = nullptr;                // [3][nf] complex
-    void* conv = nullptr;                // [3][pvol] real: unnormalised convolution (scale folded into khat)
-    void* khat = nullptr;                // [6][nf] complex
+    bool zfused = true;                  // z transform + product + inverse z transform in one kernel (nz <= kZFusedMax)
+    int zplanes = 0;                     // planes of the work arrays: nz (zfused) or Pz
+    long long pvol = 0, nf = 0;          // real points, complex points per component of the work arrays
+    void* pad = nullptr;                 // [3][zplanes][Py][Px] real: gathered state (pad region stays zero)
+    void* freq = nullptr;                // [3][zplanes][Py][Px/2+1] complex
+    void* conv = nullptr;                // [3][zplanes][Py][Px] real: unnormalised convolution (scale folded into khat)
+    void* khat = nullptr;                // zfused: [6][Pz/2+1][Py/2+1][Px/2+1] real; else [6][nf] complex
+    size_t zsmem = 0;
+    const void* zfn = nullptr;           // k_demag_zconv<T, C, q>
     cufftHandle fwd = 0, inv = 0;
     bool have_fwd = false, have_inv = false;
 };
+
+constexpr int kZFusedMax = 64;           // largest nz whose z columns (Pz <= 128, three components) and tensor slice fit shared memory
 
 void demag_destroy(DemagPlan* p) {
     if (!p) return;
@@ -197,36 +499,58 @@ int demag_create(DemagPlan** out, int nx, int ny, int nz, double dx, double dy, 
     if (!p) return CAV_E_NOMEM;
     auto fail = [&](int code, const char* what) { snprintf(err, err_len, "demag: %s", what); demag_destroy(p); cudaGetLastError(); return code; };
     p->nx = nx; p->ny = ny; p->nz = nz; p->n_sub = n_sub; p->f32 = f32;
-    p->Px = nx > 1 ? 2 * nx : 1; p->Py = ny > 1 ? 2 * ny : 1; p->Pz = nz > 1 ? 2 * nz : 1;
-    p->pvol = (long long)p->Px * p->Py * p->Pz;
-    p->nf = (long long)p->Pz * p->Py * (p->Px / 2 + 1);
+    p->zfused = nz <= kZFusedMax;
+    p->Px = nx > 1 ? 2 * nx : 1; p->Py = ny > 1 ? 2 * ny : 1;
+    if (p->zfused) { p->Pz = 1; p->q = 0; while (p->Pz < 2 * nz - 1) { p->Pz *= 2; p->q++; } }
+    else p->Pz = 2 * nz;
+    p->zplanes = p->zfused ? nz : p->Pz;
+    const int NXH = p->Px / 2 + 1, NYH = p->Py / 2 + 1, NZH = p->Pz / 2 + 1;
+    p->pvol = (long long)p->Px * p->Py * p->zplanes;
+    p->nf = (long long)p->zplanes * p->Py * NXH;
     const size_t rs = f32 ? 4 : 8, cs = 2 * rs;
+    const size_t kbytes = p->zfused ? (size_t)6 * NZH * NYH * NXH * rs : (size_t)6 * p->nf * cs;
     if (cudaMalloc(&p->pad, 3 * p->pvol * rs) != cudaSuccess || cudaMalloc(&p->conv, 3 * p->pvol * rs) != cudaSuccess ||
-        cudaMalloc(&p->freq, 3 * p->nf * cs) != cudaSuccess || cudaMalloc(&p->khat, 6 * p->nf * cs) != cudaSuccess)
+        cudaMalloc(&p->freq, 3 * p->nf * cs) != cudaSuccess || cudaMalloc(&p->khat, kbytes) != cudaSuccess)
         return fail(CAV_E_NOMEM, "device allocation");
     if (cudaMemsetAsync(p->pad, 0, 3 * p->pvol * rs, stream) != cudaSuccess) return fail(CAV_E_CUDA, "memset");
-    int n[3] = {p->Pz, p->Py, p->Px};
-    if (f.PlanMany(&p->fwd, 3, n, nullptr, 1, 0, nullptr, 1, 0, f32 ? CUFFT_R2C : CUFFT_D2Z, 3) != CUFFT_SUCCESS) return fail(CAV_E_CUDA, "cufftPlanMany (forward)");
+    int n3[3] = {p->Pz, p->Py, p->Px};
+    int n2[2] = {p->Py, p->Px};
+    const int rank = p->zfused ? 2 : 3, batch = p->zfused ? 3 * nz : 3;
+    int* const nn = p->zfused ? n2 : n3;
+    if (f.PlanMany(&p->fwd, rank, nn, nullptr, 1, 0, nullptr, 1, 0, f32 ? CUFFT_R2C : CUFFT_D2Z, batch) != CUFFT_SUCCESS) return fail(CAV_E_CUDA, "cufftPlanMany (forward)");
     p->have_fwd = true;
-    if (f.PlanMany(&p->inv, 3, n, nullptr, 1, 0, nullptr, 1, 0, f32 ? CUFFT_C2R : CUFFT_Z2D, 3) != CUFFT_SUCCESS) return fail(CAV_E_CUDA, "cufftPlanMany (inverse)");
+    if (f.PlanMany(&p->inv, rank, nn, nullptr, 1, 0, nullptr, 1, 0, f32 ? CUFFT_C2R : CUFFT_Z2D, batch) != CUFFT_SUCCESS) return fail(CAV_E_CUDA, "cufftPlanMany (inverse)");
     p->have_inv = true;
-    // tensor table: fp64 on the device, one component at a time through a temporary D2Z plan
+    if (p->zfused) {
+        const size_t tk = f32 ? ZTile<float>::value : ZTile<double>::value;
+        p->zsmem = ((size_t)3 * p->Pz * tk + (size_t)(p->Pz / 2 > 0 ? p->Pz / 2 : 1)) * cs + (size_t)6 * NZH * tk * rs;
+        p->zfn = f32 ? zconv_fn<float, cufftComplex>(p->q) : zconv_fn<double, cufftDoubleComplex>(p->q);
+        const cudaError_t e = cudaFuncSetAttribute(p->zfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->zsmem);
+        if (e != cudaSuccess) return fail(CAV_E_CUDA, "shared memory for the z convolution");
+    }
+    // tensor table: fp64 on the device, one component at a time through a temporary 3-D D2Z plan on [Pz][Py][Px]
+    const long long tvol = (long long)p->Px * p->Py * p->Pz, tnf = (long long)p->Pz * p->Py * NXH;
     double* tn = nullptr;
     cufftDoubleComplex* tk = nullptr;
     cufftHandle tp = 0;
-    if (cudaMalloc(&tn, p->pvol * sizeof(double)) != cudaSuccess || cudaMalloc(&tk, p->nf * sizeof(cufftDoubleComplex)) != cudaSuccess) {
+    if (cudaMalloc(&tn, tvol * sizeof(double)) != cudaSuccess || cudaMalloc(&tk, tnf * sizeof(cufftDoubleComplex)) != cudaSuccess) {
         cudaFree(tn); cudaFree(tk);
         return fail(CAV_E_NOMEM, "tensor scratch");
     }
-    if (f.PlanMany(&tp, 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 1) != CUFFT_SUCCESS) { cudaFree(tn); cudaFree(tk); return fail(CAV_E_CUDA, "cufftPlanMany (tensor)"); }
+    if (f.PlanMany(&tp, 3, n3, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 1) != CUFFT_SUCCESS) { cudaFree(tn); cudaFree(tk); return fail(CAV_E_CUDA, "cufftPlanMany (tensor)"); }
     f.SetStream(tp, stream);
-    const double scale = -4e-7 * CUDART_PI * Ms / (double)p->pvol;
+    const double scale = -4e-7 * CUDART_PI * Ms / (double)tvol;
     const int tb = 256;
     bool ok = true;
     for (int comp = 0; comp < 6 && ok; ++comp) {
-        k_demag_tensor<<<(unsigned)((p->pvol + tb - 1) / tb), tb, 0, stream>>>(tn, comp, nx, ny, nz, p->Px, p->Py, p->Pz, dy / dx, dz / dx);
+        k_demag_tensor<<<(unsigned)((tvol + tb - 1) / tb), tb, 0, stream>>>(tn, comp, nx, ny, nz, p->Px, p->Py, p->Pz, dy / dx, dz / dx);
         ok = ok && f.ExecD2Z(tp, tn, tk) == CUFFT_SUCCESS;
-        if (f32) k_store_khat<cufftComplex><<<(unsigned)((p->nf + tb - 1) / tb), tb, 0, stream>>>(tk, (cufftComplex*)p->khat + comp * p->nf, p->nf, scale);
+        if (p->zfused) {
+            const long long oct = (long long)NZH * NYH * NXH;
+            const unsigned g = (unsigned)((oct + tb - 1) / tb);
+            if (f32) k_store_khat_real<float><<<g, tb, 0, stream>>>(tk, (float*)p->khat + comp * oct, NZH, NYH, NXH, p->Py, scale);
+            else k_store_khat_real<double><<<g, tb, 0, stream>>>(tk, (double*)p->khat + comp * oct, NZH, NYH, NXH, p->Py, scale);
+        } else if (f32) k_store_khat<cufftComplex><<<(unsigned)((p->nf + tb - 1) / tb), tb, 0, stream>>>(tk, (cufftComplex*)p->khat + comp * p->nf, p->nf, scale);
         else k_store_khat<cufftDoubleComplex><<<(unsigned)((p->nf + tb - 1) / tb), tb, 0, stream>>>(tk, (cufftDoubleComplex*)p->khat + comp * p->nf, p->nf, scale);
     }
     ok = ok && cudaStreamSynchronize(stream) == cudaSuccess && cudaGetLastError() == cudaSuccess;
@@ -240,21 +564,31 @@ int demag_create(DemagPlan** out, int nx, int ny, int nz, double dx, double dy, 
 int demag_apply(DemagPlan* p, const StageArgs& A, int stage, void* bdem, cudaStream_t stream) {
     FftApi& f = fft_api();
     const int tb = 256;
-    const unsigned gc = (unsigned)((A.nc + tb - 1) / tb), gf = (unsigned)((p->nf + tb - 1) / tb);
+    const unsigned gf = (unsigned)((p->nf + tb - 1) / tb);
+    const int gtb = A.nx >= 256 ? 256 : (A.nx >= 128 ? 128 : (A.nx >= 64 ? 64 : 32));
+    const dim3 gc((unsigned)((A.nx + gtb - 1) / gtb), (unsigned)A.ny, (unsigned)p->nz);
+    const int NXH = p->Px / 2 + 1;
+    const int tk = p->f32 ? ZTile<float>::value : ZTile<double>::value;
+    const dim3 zgrid((unsigned)(((long long)p->Py * NXH + tk - 1) / tk));
+    const dim3 zblock((unsigned)tk, (unsigned)zconv_rows(p->q));
+    int nzv = p->nz, pyv = p->Py, nxhv = NXH;
+    void* zargs[] = {&p->freq, &p->khat, &nzv, &pyv, &nxhv};
     f.SetStream(p->fwd, stream);
     f.SetStream(p->inv, stream);
     if (p->f32) {
-        k_demag_gather<float><<<gc, tb, 0, stream>>>(A, stage, p->n_sub, (float*)p->pad, p->Px, p->Py, p->Pz);
+        k_demag_gather<float><<<gc, gtb, 0, stream>>>(A, stage, p->n_sub, (float*)p->pad, p->Px, p->Py, p->zplanes);
         if (f.ExecR2C(p->fwd, (cufftReal*)p->pad, (cufftComplex*)p->freq) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        k_demag_product<cufftComplex><<<gf, tb, 0, stream>>>((cufftComplex*)p->freq, (const cufftComplex*)p->khat, p->nf);
+        if (p->zfused) { if (cudaLaunchKernel(p->zfn, zgrid, zblock, zargs, p->zsmem, stream) != cudaSuccess) return CAV_E_CUDA; }
+        else k_demag_product<cufftComplex><<<gf, tb, 0, stream>>>((cufftComplex*)p->freq, (const cufftComplex*)p->khat, p->nf);
         if (f.ExecC2R(p->inv, (cufftComplex*)p->freq, (cufftReal*)p->conv) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        k_demag_scatter<float><<<gc, tb, 0, stream>>>((const float*)p->conv, (float*)bdem, A.nx, A.ny, A.nc, p->Px, p->Py, p->Pz);
+        k_demag_scatter<float><<<gc, gtb, 0, stream>>>((const float*)p->conv, (float*)bdem, A.nx, A.ny, A.nc, p->Px, p->Py, p->zplanes);
     } else {
-        k_demag_gather<double><<<gc, tb, 0, stream>>>(A, stage, p->n_sub, (double*)p->pad, p->Px, p->Py, p->Pz);
+        k_demag_gather<double><<<gc, gtb, 0, stream>>>(A, stage, p->n_sub, (double*)p->pad, p->Px, p->Py, p->zplanes);
         if (f.ExecD2Z(p->fwd, (cufftDoubleReal*)p->pad, (cufftDoubleComplex*)p->freq) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        k_demag_product<cufftDoubleComplex><<<gf, tb, 0, stream>>>((cufftDoubleComplex*)p->freq, (const cufftDoubleComplex*)p->khat, p->nf);
+        if (p->zfused) { if (cudaLaunchKernel(p->zfn, zgrid, zblock, zargs, p->zsmem, stream) != cudaSuccess) return CAV_E_CUDA; }
+        else k_demag_product<cufftDoubleComplex><<<gf, tb, 0, stream>>>((cufftDoubleComplex*)p->freq, (const cufftDoubleComplex*)p->khat, p->nf);
         if (f.ExecZ2D(p->inv, (cufftDoubleComplex*)p->freq, (cufftDoubleReal*)p->conv) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        k_demag_scatter<double><<<gc, tb, 0, stream>>>((const double*)p->conv, (double*)bdem, A.nx, A.ny, A.nc, p->Px, p->Py, p->Pz);
+        k_demag_scatter<double><<<gc, gtb, 0, stream>>>((const double*)p->conv, (double*)bdem, A.nx, A.ny, A.nc, p->Px, p->Py, p->zplanes);
     }
     return cudaGetLastError() == cudaSuccess ? CAV_OK : CAV_E_CUDA;
 }

@@ -1,7 +1,8 @@
 // Optional dipolar (demagnetising) field (the paper switches it off; reading G34):
 //     B_d(r_i) = -mu0 Ms sum_j N(r_i - r_j) . m_tot(r_j)      open boundary, N = Newell's cell-averaged tensor
-// evaluated as a zero-padded FFT convolution before every stage kernel.  This is a different roofline from the fused
-// stencil (six 3-D FFTs per evaluation); it runs on the generic stage kernels with host-enqueued launches.
+// evaluated as a zero-padded FFT convolution before every stage kernel (batched 2-D cuFFT transforms of the occupied planes
+// and one kernel for the z transform, the tensor product and the inverse z transform: demag.cu).  A different roofline
+// from the fused stencil; it runs on the generic stage kernels, its launches captured into the run graph (cavmag_api.cu).
 #pragma once
 #include <cuda_runtime.h>
 

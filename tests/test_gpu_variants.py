@@ -280,6 +280,10 @@ def test_spectrum_shows_both_polariton_branches(api):
     ((13, 5, 3), 0, 1, 0.1e-12),       # odd sizes, plain LLG
     ((8, 6, 4), 1, 2, 0.02e-12),       # two sublattices: the field of m_1 + m_2
     ((1, 1, 1), 1, 1, 0.1e-12),        # one cell: the self term only
+    ((6, 4, 2), 1, 1, 0.1e-12),        # z column of 4 after padding: two radix-2 levels in one pass
+    ((5, 3, 9), 1, 1, 0.1e-12),        # z column of 32: an odd number of levels
+    ((4, 3, 40), 1, 1, 0.1e-12),       # z column of 128: more butterflies than worker rows
+    ((3, 2, 130), 0, 1, 0.1e-12),      # beyond the shared-memory z column: padded 3-D transforms
 ])
 def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
     """The FFT convolution against the oracle's direct O(N^2) sum with the Newell tensor: right-hand side cell by cell,
@@ -306,8 +310,14 @@ def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
         api.cav_get_dmdt(sim.h, dm_off)
     assert st["accepted"] == 100 and st["rhs_evals"] == 601
     scale = np.abs(dm_ref).max()
-    assert np.abs(dm - dm_ref).max() <= (5e-13 if prec == "f64" else 3e-5) * scale
-    assert_parity(m, a, ref, prec)
+    # Newell's closed forms lose digits with distance (27-point second differences of terms ~R^3: ~(R/d)^5 eps relative
+    # in an entry ~(d/R)^3); CPU and device evaluate them with different libm roundings: 1e-11 of the field at 130 cells
+    tol64 = 5e-13 if max(shape) <= 40 else 5e-11
+    assert np.abs(dm - dm_ref).max() <= (tol64 if prec == "f64" else 3e-5) * scale
+    if max(shape) <= 40 or prec == "f32":
+        assert_parity(m, a, ref, prec)
+    else:
+        assert np.abs(m - ref.m).max() <= 1e-9           # (the same loss of digits, integrated over 100 steps)
     plain = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=100)
     assert np.abs(plain.m - ref.m).max() > 1e-4                       # mu0 Ms = 0.18 T: not a detail
     dm_plain, _, _ = oracle_of(w).rhs(ref.m, ref.a)
@@ -342,6 +352,28 @@ def test_demag_adaptive_platelet_kittel_shift(api):
 
 def GAMMA_B0(w):
     return 1.76e11 * w.B0[2]
+
+
+def test_demag_run_is_one_graph_launch(api):
+    """With the dipolar field the FFT launches are captured into the run graph: an adaptive run (with forced rejections)
+    is bitwise what host-enqueued launches give, and cav_run returns before the device has finished."""
+    w = small_problem(20, 12, 6, 2, 1)
+    out = {}
+    for mode in ("graph", "stream"):
+        with api.Sim(w, precision="f64") as sim:
+            api.cav_set_launch_mode(sim.h, api.CAV_LAUNCH_GRAPH if mode == "graph" else api.CAV_LAUNCH_STREAM)
+            api.cav_set_demag(sim.h, 1)
+            n0 = api.cav_get_launch_count(sim.h)
+            api.cav_run(sim.h, 30e-12, tol=1e-9, dt_init=2e-12)
+            st = api.cav_get_stats(sim.h)
+            out[mode] = (sim.get_m(), sim.get_a(), st, api.cav_get_launch_count(sim.h) - n0 - st["rhs_evals"])
+    (mg, ag, sg, hg), (ms, as_, ss, hs) = out["graph"], out["stream"]
+    assert sg["rejected"] > 0 and sg["accepted"] == ss["accepted"] and sg["rejected"] == ss["rejected"]
+    assert np.array_equal(mg, ms) and np.array_equal(ag, as_)
+    assert hg <= 4 < hs                                   # host-side launches: the graph (+ k_setrun) against 5 per stage
+    ref = oracle_of(w, demag=True).run(w.m0, w.a0, t_end=30e-12, tol=1e-9, dt_init=2e-12)
+    assert (ref.accepted, ref.rejected) == (sg["accepted"], sg["rejected"])
+    assert_parity(mg, ag, ref, "f64")
 
 
 def test_demag_limits(api):
