@@ -335,6 +335,29 @@ int cav_sweep_destroy(cav_sweep* sweep);
 /* Arguments as cav_run_steps, applied to every simulation.  Asynchronous on the simulations' stream. */
 int cav_sweep_run(cav_sweep* sweep, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * An entry point that allocates nothing, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): the overlaps of a given state with given mode profiles,
+ *     S_n = (1/N_cells) sum_r u_n(r) (m_c,x(r) - i m_c,y(r)),   m_c = the mean over the sublattices
+ * (Eq. 18 with the paper's polarisation x^; CAV_NORM_NCELLS), the same two-pass fixed-order reduction
+ * as the stage kernels' (block partials in fp64, then one sum in block order: results are bitwise reproducible).
+ *   m_dev  [n_sub][3][nz][ny][nx], u_dev [N][nz][ny][nx]: DEVICE buffers in `precision` (CAV_F32 | CAV_F64), read only
+ *   S_out_dev [N][2] doubles (Re, Im): DEVICE buffer, written; the caller owns all three
+ *   cuda_stream: a cudaStream_t (NULL = the default stream); the call is asynchronous on it
+ * No handle, no cudaMalloc / cudaFree / allocating library routine: the block partials live in ONE file-scope __device__
+ * array of CAV_NOALLOC_SCRATCH_BYTES (1 MiB + 256 B) that every GPU loading the library holds until exit.  Hence the
+ * limits: nx*ny*nz <= CAV_NOALLOC_MAX_CELLS (2^24, the largest configuration of BASELINE.json) and N <= CAV_MAX_MODES;
+ * beyond them CAV_E_UNSUPPORTED, with the reason in cav_noalloc_last_error().  Every call on a device shares that array
+ * (the call clears the words that must start at zero itself): calls that overlap on the GPU - two streams, or two
+ * threads - RACE; serialise them (one stream, or events).  Other errors: CAV_E_ARG, CAV_E_CUDA.
+ * --------------------------------------------------------------------------------------------------------- */
+#define CAV_NOALLOC_MAX_CELLS (1LL << 24)
+#define CAV_NOALLOC_SCRATCH_BYTES (256 + 8 * (CAV_NOALLOC_MAX_CELLS / 8192) * 2 * CAV_MAX_MODES)
+int cav_overlaps_noalloc(const void* m_dev, const void* u_dev, int precision, int nx, int ny, int nz, int n_sub, int N,
+                         double* S_out_dev, void* cuda_stream);
+/* Text of the calling thread's last cav_overlaps_noalloc failure ("" after a success). */
+const char* cav_noalloc_last_error(void);
+
 const char* cav_strerror(int status);
 const char* cav_last_cuda_error(cav_sim* sim);
 const char* cav_version(void);

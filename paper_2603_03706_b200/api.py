@@ -120,6 +120,8 @@ _SIGS = {
     "cav_batch_get_a": ([_vp, _dp], _i),
     "cav_batch_get_stats": ([_vp, C.POINTER(cav_stats)], _i),
     "cav_batch_get_trace": ([_vp, _dp, C.POINTER(_i)], _i),
+    "cav_overlaps_noalloc": ([_vp, _vp, _i, _i, _i, _i, _i, _i, _vp, _vp], _i),
+    "cav_noalloc_last_error": ([], C.c_char_p),
 }
 for _name, (_args, _res) in _SIGS.items():
     _f = getattr(_lib, _name)
@@ -140,6 +142,29 @@ def _check(st: int, where: str, sim=None):
     if st != CAV_OK:
         detail = _lib.cav_last_cuda_error(sim).decode() if (sim and st == CAV_E_CUDA) else ""
         raise CavError(st, where, detail)
+
+
+def cav_noalloc_last_error() -> str:
+    return _lib.cav_noalloc_last_error().decode()
+
+
+def cav_overlaps_noalloc(m, u, S_out, grid, n_sub: int = 1, cuda_stream: int = 0) -> None:
+    """S_n of the device tensors m [n_sub][3][nz][ny][nx] and u [N][nz][ny][nx] into the device tensor S_out [N][2]
+    (float64); grid = (nx, ny, nz).  Allocates nothing (cavmag.h); asynchronous on cuda_stream."""
+    nx, ny, nz = (int(v) for v in grid)
+    N = int(u.shape[0]) if u.dim() == 4 else int(u.numel() // max(nx * ny * nz, 1))
+    prec = {"torch.float32": CAV_F32, "torch.float64": CAV_F64}.get(str(m.dtype))
+    if prec is None or u.dtype != m.dtype:
+        raise ValueError("m and u must both be float32 or both float64")
+    dt = np.float32 if prec == CAV_F32 else np.float64
+    pm, dm, _ = _ptr(m, dt, 3 * int(n_sub) * nx * ny * nz, "m")
+    pu, du, _ = _ptr(u, dt, N * nx * ny * nz, "u")
+    ps, ds, _ = _ptr(S_out, np.float64, 2 * N, "S_out")
+    if not (dm and du and ds):
+        raise ValueError("cav_overlaps_noalloc takes device tensors")
+    st = _lib.cav_overlaps_noalloc(pm, pu, prec, nx, ny, nz, int(n_sub), N, ps, cuda_stream)
+    if st != CAV_OK:
+        raise CavError(st, "cav_overlaps_noalloc", cav_noalloc_last_error())
 
 
 # handle -> (numpy dtype of the cell fields, n_sub, cells, replicas): what a cell-field buffer handed to the

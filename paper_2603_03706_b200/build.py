@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcavmag.so")
-SOURCES = ["cavmag_api.cu", "cavmag_batch.cu", "demag.cu", "stage_inst_f32_fm.cu", "stage_inst_f32_afm.cu", "stage_inst_f64_fm.cu",
+SOURCES = ["cavmag_api.cu", "cavmag_batch.cu", "cavmag_noalloc.cu", "demag.cu", "stage_inst_f32_fm.cu", "stage_inst_f32_afm.cu", "stage_inst_f64_fm.cu",
            "stage_inst_f64_afm.cu", "stage_inst_demag_f32_fm.cu", "stage_inst_demag_f32_afm.cu", "stage_inst_demag_f64_fm.cu",
            "stage_inst_demag_f64_afm.cu", "stage_inst_pol_f32_fm.cu", "stage_inst_pol_f32_afm.cu", "stage_inst_pol_f64_fm.cu", "stage_inst_pol_f64_afm.cu", "stage_tma_inst_f32_fm.cu", "stage_tma_inst_f32_afm.cu",
            "stage_tma_inst_f64_fm.cu", "stage_tma_inst_f64_afm.cu", "stage_tma_inst_sweep_f32.cu", "stage_tma_inst_sweep_f64.cu"]
