@@ -325,6 +325,57 @@ def timed_steps(api, torch, h, stream, tol, steps, sampler=None, barrier=None):
     return ev0.elapsed_time(ev1), clocks
 
 
+E2E_STREAMS = 4     # independent simulations in flight in the end-to-end measurement (one host thread and one stream each)
+
+
+def e2e_pipelined(api, torch, w, prec, tol, k, spinup, barrier, n_streams=E2E_STREAMS):
+    """End to end through the C ABI with host buffers, as a host application that integrates several independent
+    simulations would drive it: n_streams simulations of the same workload, one host thread and one CUDA stream each,
+    every step of every simulation = cav_set_m / cav_set_a from pinned host memory, cav_run_steps(1), cav_get_m /
+    cav_get_a back to the host.  A single chain is bound by upload + step + download in series (PCIe, ~1.2 ms for CFG3);
+    with several chains the copies of one overlap the step and the opposite-direction copies of the others.
+    Returns (seconds, right-hand-side evaluations of all simulations)."""
+    import threading
+    N = w.n_modes
+    sims, hosts = [], []
+    for _ in range(n_streams):
+        st = torch.cuda.Stream()
+        sim = api.Sim(w, precision=prec, stream=st.cuda_stream)
+        sim._stream_keepalive = st
+        api.cav_run_steps(sim.h, math.inf, tol=tol, max_steps=spinup)
+        mh = torch.empty(sim.shape_m, dtype=torch.float32 if prec == "f32" else torch.float64).pin_memory()
+        api.cav_get_m(sim.h, mh)
+        sims.append(sim); hosts.append(mh)
+
+    def chain(i, n):
+        h, mh = sims[i].h, hosts[i]
+        a = api.cav_get_a(h, N)
+        for _ in range(n):
+            api.cav_set_m(h, mh)                      # H2D from pinned host memory
+            api.cav_set_a(h, a)
+            api.cav_run_steps(h, math.inf, tol=tol, max_steps=1)
+            api.cav_get_m(h, mh)                      # D2H of the step's result (synchronises this simulation's stream)
+            a = api.cav_get_a(h, N)
+
+    for i in range(n_streams):
+        chain(i, 3)                                   # warm-up of the host-buffer path
+    ev0 = [api.cav_get_stats(q.h)["rhs_evals"] for q in sims]
+    barrier()
+    t0 = time.perf_counter()
+    threads = [threading.Thread(target=chain, args=(i, k)) for i in range(n_streams)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    torch.cuda.synchronize()
+    seconds = time.perf_counter() - t0
+    barrier()
+    evals = sum(api.cav_get_stats(q.h)["rhs_evals"] - e for q, e in zip(sims, ev0))
+    for q in sims:
+        q.close()
+    return seconds, evals
+
+
 def measure_extra(api, torch, name, args, local):
     """One more large workload in the same process (device-resident timing only): value, ms per step, roofline
     fraction and the clocks seen during its timed region."""
@@ -438,9 +489,12 @@ def run_cuda(args):
     e2e_s = time.perf_counter() - t0
     barrier()
     se1 = api.cav_get_stats(h)
-    e2e_evals = se1["rhs_evals"] - se0["rhs_evals"]
+    e2e1_evals = se1["rhs_evals"] - se0["rhs_evals"]
+    e2e1_s = e2e_s
     io_bytes = int(np.prod(sim.shape_m)) * esize + 16 * N
     sim.close()
+    # the same with E2E_STREAMS independent simulations in flight (the end-to-end figure of the line)
+    e2e_s, e2e_evals = e2e_pipelined(api, torch, w, prec, tol, k_e2e, args.spinup, barrier)
 
     # ---- max over ranks, sum of units ----
     agg = aggregate_over_ranks(ms, e2e_s, float(nc * evals), float(nc * e2e_evals), sim_t, world, "cuda")
@@ -461,9 +515,14 @@ def run_cuda(args):
             "accepted": st1["accepted"] - st0["accepted"], "rejected": st1["rejected"] - st0["rejected"],
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
-                    "steps": k_e2e, "ms_per_step": 1e3 * e2e_max / k_e2e,
-                    "note": "every step: cav_set_m/cav_set_a from pinned host memory, cav_run_steps(1), cav_get_m/cav_get_a "
-                            "to host; FSAL is lost at each upload (7 RHS evaluations per step)"},
+                    "steps": k_e2e, "simulations_in_flight": E2E_STREAMS, "ms_per_step": 1e3 * e2e_max / (k_e2e * E2E_STREAMS),
+                    "single_stream": {"value": nc * e2e1_evals / e2e1_s, "ms_per_step": 1e3 * e2e1_s / k_e2e,
+                                      "note": "one simulation: upload, step and download in series (this rank)"},
+                    "note": "every step of every simulation: cav_set_m/cav_set_a from pinned host memory, cav_run_steps(1), "
+                            "cav_get_m/cav_get_a to host; FSAL is lost at each upload (7 RHS evaluations per step); "
+                            f"{E2E_STREAMS} independent simulations of the workload, one host thread and one stream each, so "
+                            "that the copies of one overlap the step and the opposite-direction copies of the others; "
+                            "bytes are per step of one simulation"},
             "gpu_launches": int(n1 - n0),
             "roofline": roofline_of(name, w, prec, ms, args.steps),
         }
