@@ -217,9 +217,10 @@ int cav_get_stage_overlap(cav_sim* sim, int* active);
  *     S_n = (1/W_n) sum_r u_n(r) (m_c.p_n - i m_c.q_n),      B_rf(r) = sum_n c_n u_n(r) p_n
  * (reading G32; p = x^, q = y^ is the paper's case).  pol: [N][3] host, normalised on entry; quad: [N][3] host,
  * used as given, or NULL for q_n = z^ x p_n (static field along z^).  pol == NULL restores x^.  Call after cav_set_modes
- * (a new mode set restores x^).  Implemented in the small-grid kernel (CAV_PATH_BLOCK / CAV_PATH_COOP) and in the generic
- * stage kernels, which the run then uses whatever cav_set_kernel_path says (the TMA kernels keep the paper's x^);
- * CAV_E_UNSUPPORTED together with cav_set_demag or on a grid stored with padded rows. */
+ * (a new mode set restores x^).  Implemented in the small-grid kernel (CAV_PATH_BLOCK / CAV_PATH_COOP), in the TMA stage
+ * kernels for up to 8 modes (their own instantiation) and in the generic stage kernels, which a run with more modes uses
+ * whatever cav_set_kernel_path says; CAV_E_UNSUPPORTED together with cav_set_demag, in a joint sweep, or with more than
+ * 8 modes on a grid stored with padded rows. */
 int cav_set_polarisation(cav_sim* sim, const double* pol, const double* quad);
 
 /* Integrator.  CAV_INTEGRATOR_UNIFIED (default): LLG and mode ODEs in ONE Dormand-Prince step (tier 1).

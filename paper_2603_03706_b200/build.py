@@ -16,7 +16,8 @@ LIB = os.path.join(HERE, "libcavmag.so")
 SOURCES = ["cavmag_api.cu", "cavmag_batch.cu", "cavmag_noalloc.cu", "demag.cu", "stage_inst_f32_fm.cu", "stage_inst_f32_afm.cu", "stage_inst_f64_fm.cu",
            "stage_inst_f64_afm.cu", "stage_inst_demag_f32_fm.cu", "stage_inst_demag_f32_afm.cu", "stage_inst_demag_f64_fm.cu",
            "stage_inst_demag_f64_afm.cu", "stage_inst_pol_f32_fm.cu", "stage_inst_pol_f32_afm.cu", "stage_inst_pol_f64_fm.cu", "stage_inst_pol_f64_afm.cu", "stage_tma_inst_f32_fm.cu", "stage_tma_inst_f32_afm.cu",
-           "stage_tma_inst_f64_fm.cu", "stage_tma_inst_f64_afm.cu", "stage_tma_inst_sweep_f32.cu", "stage_tma_inst_sweep_f64.cu"]
+           "stage_tma_inst_f64_fm.cu", "stage_tma_inst_f64_afm.cu", "stage_tma_inst_sweep_f32.cu", "stage_tma_inst_sweep_f64.cu",
+           "stage_tma_inst_pol_f32_fm.cu", "stage_tma_inst_pol_f32_afm.cu", "stage_tma_inst_pol_f64_fm.cu", "stage_tma_inst_pol_f64_afm.cu"]
 HEADERS = ["cavmag_types.cuh", "stage_kernel.cuh", "stage_tma.cuh", "batch_kernel.cuh", "demag.cuh", os.path.join("..", "..", "include", "cavmag.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]

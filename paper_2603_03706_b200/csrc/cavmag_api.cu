@@ -201,6 +201,10 @@ __global__ void k_sweep_setrun(const RepPtrs* reps, double t_end, double tol, do
 
 const void* stage_tma_fn(const cav_sim* s, int stage) {
     const bool f32 = s->prm.precision == CAV_F32;
+    if (s->d_pol) {          // the instantiation with per-mode polarisation (mode buckets up to 8; NULL beyond)
+        if (s->prm.n_sub == 1) return f32 ? stage_tma_pol_kernel_f32_fm(stage, s->nb) : stage_tma_pol_kernel_f64_fm(stage, s->nb);
+        return f32 ? stage_tma_pol_kernel_f32_afm(stage, s->nb) : stage_tma_pol_kernel_f64_afm(stage, s->nb);
+    }
     if (s->prm.n_sub == 1) return f32 ? stage_tma_kernel_f32_fm(stage, s->nb) : stage_tma_kernel_f64_fm(stage, s->nb);
     return f32 ? stage_tma_kernel_f32_afm(stage, s->nb) : stage_tma_kernel_f64_afm(stage, s->nb);
 }
@@ -379,7 +383,8 @@ void decide_path(cav_sim* s) {
     s->use_block = block_ok && (s->kernel_path == CAV_PATH_BLOCK || s->kernel_path == CAV_PATH_AUTO || small_only);
     s->use_coop = coop_ok && (s->kernel_path == CAV_PATH_COOP || s->kernel_path == CAV_PATH_AUTO || small_only);
     if (s->demag) { s->use_block = s->use_coop = s->use_tma = false; return; }                 // dipolar field: generic stage kernels
-    if (s->d_pol) { s->use_tma = false; return; }                                              // polarisation: small-grid or generic kernels
+    const bool pol_tma = s->d_pol && s->tma_eligible && stage_tma_fn(s, 2) != nullptr;         // polarisation: TMA kernels for up to 8 modes
+    if (s->d_pol && !pol_tma) { s->use_tma = false; return; }                                  // else small-grid or generic kernels
     if (s->padded) { s->use_block = s->use_coop = false; s->use_tma = s->tma_eligible; }       // padded rows: TMA kernels only
     else if (s->kernel_path == CAV_PATH_GENERIC || s->use_block || s->use_coop) s->use_tma = false;
     else if (s->kernel_path == CAV_PATH_TMA) s->use_tma = s->tma_eligible;
@@ -1092,13 +1097,18 @@ int cav_set_polarisation(cav_sim* s, const double* pol, const double* quad) {
         CK(cudaMalloc(&s->d_pol, sizeof(double) * 6 * s->N));
         CK(cudaMemcpyAsync(s->d_pol, h, sizeof(double) * 6 * s->N, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
-        if (s->padded || s->demag) {                     // rows padded for the TMA kernels / the dipolar-field kernels: x^ only
+        // the dipolar-field kernels know x^ only; rows padded inside the library need the TMA kernels, which take
+        // a polarisation for up to 8 modes
+        if (s->demag || (s->padded && stage_tma_fn(s, 2) == nullptr)) {
             cudaFree(s->d_pol);
             s->d_pol = nullptr;
+            plan_tma(s);
             push_ctrl(s);
             return CAV_E_UNSUPPORTED;
         }
     }
+    rc = plan_tma(s);                    // the polarised TMA kernels are other functions: their own shared-memory budget
+    if (rc) return rc;
     return push_ctrl(s);
 }
 

@@ -320,9 +320,13 @@ struct SweepArgs {
     unsigned long long cond_handle;
 };
 
-template <typename T, int STAGE, int NSUB, int NB, bool SWEEP>
+// POL: per-mode polarisation (A.pol, reading G32; cav_set_polarisation) - its own instantiation, up to 8 modes: the RF field
+// of mode n points along p_n, and the overlap is taken with m.p_n - i m.q_n.  The consumers accumulate the three raw sums
+// sum u_n m_c per mode and project them on p_n, q_n once, before the block reduction (the projection is linear).
+template <typename T, int STAGE, int NSUB, int NB, bool SWEEP, bool POL = false>
 __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs& TA, double* __restrict__ trace0, const SweepArgs& SW) {
     static_assert(!(SWEEP && STAGE == 1), "stage 1 of a joint launch runs as one ordinary launch per simulation");
+    static_assert(!POL || (!SWEEP && NB >= 1 && NB <= 8), "polarisation: single simulations with 1..8 modes");
     constexpr int VEC = 8 / (int)sizeof(T);              // cells per lane: 2 floats / 1 double
     constexpr int TX = kTmaRowBytes / (int)sizeof(T);    // cells per tile row
     constexpr int HX = kTmaHaloBytes / (int)sizeof(T);   // x halo in cells (16 bytes: 4 floats / 2 doubles)
@@ -340,6 +344,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[6 * kTmaMaxDepth];
     __shared__ T s_cn[NB > 0 ? NB : 1];
+    __shared__ T s_pq[POL ? 6 * NB : 1];         // p_n, q_n (constant during a run: loaded before the dependency wait)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nx = A.nx, ny = A.ny, nz = A.nz;
@@ -666,6 +671,9 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
             enter_subrun(sr);
             const StageArgs& A = SWEEP ? Arep : Aouter;
             Ctrl* const ctrl = A.ctrl;
+        if constexpr (POL) {
+            if (tid < 6 * NB) s_pq[tid] = (tid / 6 < TA.N) ? (T)A.pol[tid] : (T)0;      // (visible after the consumers' barrier below)
+        }
         if (!SWEEP || sr == 0) {
             asm volatile("griddepcontrol.wait;" ::: "memory");
             if constexpr (SWEEP && STAGE == 3) {
@@ -712,6 +720,13 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
 #pragma unroll
             for (int n = 0; n < NB; ++n) cn_reg[n] = s_cn[n];
         }
+        T cp_reg[POL ? 3 * NB : 1];                 // c_n p_n: the RF field of mode n per unit of u_n
+        if constexpr (POL) {
+#pragma unroll
+            for (int n = 0; n < NB; ++n)
+#pragma unroll
+                for (int k = 0; k < 3; ++k) cp_reg[3 * n + k] = s_cn[n] * s_pq[6 * n + k];
+        }
         const T B0x = (T)A.B0[0], B0y = (T)A.B0[1], B0z = (T)A.B0[2];
         const T wx = (T)A.ex_wx, wy = (T)A.ex_wy, wz = (T)A.ex_wz;
         const T anp = (T)A.an_pref, axx = (T)A.axis[0], axy = (T)A.axis[1], axz = (T)A.axis[2];
@@ -723,9 +738,9 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
         T* __restrict__ mnext = STAGE == 6 ? ynew : (STAGE == 2 || STAGE == 4) ? (T*)A.MS[0] : (T*)A.MS[1];
         T* __restrict__ e6g = (T*)A.MS[0];
 
-        T ox[NB > 0 ? NB : 1], oy[NB > 0 ? NB : 1];
+        T ox[NB > 0 ? NB : 1], oy[NB > 0 ? NB : 1], oz[POL ? NB : 1];
 #pragma unroll
-        for (int n = 0; n < NB; ++n) { ox[n] = (T)0; oy[n] = (T)0; }
+        for (int n = 0; n < NB; ++n) { ox[n] = (T)0; oy[n] = (T)0; if constexpr (POL) oz[n] = (T)0; }
         T sm[NSUB * 3];
 #pragma unroll
         for (int i = 0; i < NSUB * 3; ++i) sm[i] = (T)0;
@@ -801,15 +816,18 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
                 for (int c = 0; c < 3; ++c) mc[s][c] = ldm(sm_zc, s * 3 + c, crow);
 
             // ---- mode profiles (ring u): RF field and overlap partials of THIS stage state ----
-            T brf[VEC];
+            T brf[VEC], brfy[POL ? VEC : 1], brfz[POL ? VEC : 1];
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) brf[v] = (T)0;
+            for (int v = 0; v < VEC; ++v) { brf[v] = (T)0; if constexpr (POL) { brfy[v] = (T)0; brfz[v] = (T)0; } }
             if constexpr (NB > 0) {
-                T mcx[VEC], mcy[VEC];
+                T mcx[VEC], mcy[VEC], mcz[POL ? VEC : 1];
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
-                    if constexpr (NSUB == 1) { mcx[v] = mc[0][0].v[v]; mcy[v] = mc[0][1].v[v]; }
-                    else { mcx[v] = (T)0.5 * (mc[0][0].v[v] + mc[1][0].v[v]); mcy[v] = (T)0.5 * (mc[0][1].v[v] + mc[1][1].v[v]); }
+                    if constexpr (NSUB == 1) { mcx[v] = mc[0][0].v[v]; mcy[v] = mc[0][1].v[v]; if constexpr (POL) mcz[v] = mc[0][2].v[v]; }
+                    else {
+                        mcx[v] = (T)0.5 * (mc[0][0].v[v] + mc[1][0].v[v]); mcy[v] = (T)0.5 * (mc[0][1].v[v] + mc[1][1].v[v]);
+                        if constexpr (POL) mcz[v] = (T)0.5 * (mc[0][2].v[v] + mc[1][2].v[v]);
+                    }
                 }
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
@@ -824,12 +842,24 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
 #pragma unroll
                     for (int i = 0; i < UCB; ++i) {
                         const int n = ch * kTmaUChunk + i;          // modes >= N: u zero-filled, c_n = 0
-                        const T cn = (NB <= 8) ? cn_reg[NB <= 8 ? n : 0] : s_cn[n];     // few modes: RF weights live in registers
+                        if constexpr (!POL) {
+                            const T cn = (NB <= 8) ? cn_reg[NB <= 8 ? n : 0] : s_cn[n];     // few modes: RF weights live in registers
 #pragma unroll
-                        for (int v = 0; v < VEC; ++v) {
-                            brf[v] += cn * un[i].v[v];
-                            ox[n] += un[i].v[v] * mcx[v];
-                            oy[n] += un[i].v[v] * mcy[v];
+                            for (int v = 0; v < VEC; ++v) {
+                                brf[v] += cn * un[i].v[v];
+                                ox[n] += un[i].v[v] * mcx[v];
+                                oy[n] += un[i].v[v] * mcy[v];
+                            }
+                        } else {
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) {
+                                brf[v] += cp_reg[POL ? 3 * n : 0] * un[i].v[v];
+                                brfy[v] += cp_reg[POL ? 3 * n + 1 : 0] * un[i].v[v];
+                                brfz[v] += cp_reg[POL ? 3 * n + 2 : 0] * un[i].v[v];
+                                ox[n] += un[i].v[v] * mcx[v];
+                                oy[n] += un[i].v[v] * mcy[v];
+                                oz[POL ? n : 0] += un[i].v[v] * mcz[v];
+                            }
                         }
                     }
                 }
@@ -884,6 +914,7 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
                     T Bx, By, Bz;
                     material_field(mx, my, mz, lap[0][v], lap[1][v], lap[2][v], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
                     Bx += brf[v];
+                    if constexpr (POL) { By += brfy[v]; Bz += brfz[v]; }
                     if constexpr (NSUB == 2) {
                         Bx -= BE * mc[1 - s][0].v[v]; By -= BE * mc[1 - s][1].v[v]; Bz -= BE * mc[1 - s][2].v[v];
                     }
@@ -983,7 +1014,13 @@ __device__ __forceinline__ void stage_tma_body(const StageArgs& A, const TmaArgs
         {
             T vals[NS > 0 ? NS : 1];
 #pragma unroll
-            for (int n = 0; n < NB; ++n) { vals[2 * n] = ox[n]; vals[2 * n + 1] = oy[n]; }
+            for (int n = 0; n < NB; ++n) {
+                if constexpr (!POL) { vals[2 * n] = ox[n]; vals[2 * n + 1] = oy[n]; }
+                else {              // sum u (m.p) and sum u (m.q) from the raw sums
+                    vals[2 * n] = ox[n] * s_pq[6 * n] + oy[n] * s_pq[6 * n + 1] + oz[POL ? n : 0] * s_pq[6 * n + 2];
+                    vals[2 * n + 1] = ox[n] * s_pq[6 * n + 3] + oy[n] * s_pq[6 * n + 4] + oz[POL ? n : 0] * s_pq[6 * n + 5];
+                }
+            }
             if constexpr (STAGE == 7) {
 #pragma unroll
                 for (int i = 0; i < 3 * NSUB; ++i) vals[2 * NB + i] = sm[i];
@@ -1060,6 +1097,12 @@ __global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma(const __grid_const
     stage_tma_body<T, STAGE, NSUB, NB, false>(A, TA, trace, SweepArgs{nullptr, 1, nullptr, 0ull});
 }
 
+template <typename T, int STAGE, int NSUB, int NB>
+__global__ void __launch_bounds__(kTmaThreads, 1) k_stage_tma_pol(const __grid_constant__ StageArgs A, const __grid_constant__ TmaArgs TA,
+                                                                  double* __restrict__ trace) {
+    stage_tma_body<T, STAGE, NSUB, NB, false, true>(A, TA, trace, SweepArgs{nullptr, 1, nullptr, 0ull});
+}
+
 // Joint launch over SW.R simulations of the same shape: A carries the shared grid / material constants (and simulation
 // 0's pointers, unused), SW.reps the per-simulation pointers.
 template <typename T, int STAGE, int NSUB, int NB>
@@ -1113,6 +1156,32 @@ const void* stage_tma_kernel_f64_afm(int stage, int nb);
         case 6: return (const void*)k_stage_tma<T, 6, NSUB, NB>;                   \
         case 7: return (const void*)k_stage_tma<T, 7, NSUB, NB>;                   \
         default: return nullptr;                                                   \
+    }
+
+// per-mode polarisation (k_stage_tma_pol): mode buckets 1, 2, 8
+const void* stage_tma_pol_kernel_f32_fm(int stage, int nb);
+const void* stage_tma_pol_kernel_f32_afm(int stage, int nb);
+const void* stage_tma_pol_kernel_f64_fm(int stage, int nb);
+const void* stage_tma_pol_kernel_f64_afm(int stage, int nb);
+
+#define CAVMAG_TMA_POL_STAGE_CASES(T, NSUB, NB)                                    \
+    switch (stage) {                                                               \
+        case 1: return (const void*)k_stage_tma_pol<T, 1, NSUB, NB>;               \
+        case 2: return (const void*)k_stage_tma_pol<T, 2, NSUB, NB>;               \
+        case 3: return (const void*)k_stage_tma_pol<T, 3, NSUB, NB>;               \
+        case 4: return (const void*)k_stage_tma_pol<T, 4, NSUB, NB>;               \
+        case 5: return (const void*)k_stage_tma_pol<T, 5, NSUB, NB>;               \
+        case 6: return (const void*)k_stage_tma_pol<T, 6, NSUB, NB>;               \
+        case 7: return (const void*)k_stage_tma_pol<T, 7, NSUB, NB>;               \
+        default: return nullptr;                                                   \
+    }
+
+#define CAVMAG_DEFINE_TMA_POL_LOOKUP(NAME, T, NSUB)                                \
+    const void* NAME(int stage, int nb) {                                          \
+        if (nb == 1) { CAVMAG_TMA_POL_STAGE_CASES(T, NSUB, 1) }                    \
+        if (nb == 2) { CAVMAG_TMA_POL_STAGE_CASES(T, NSUB, 2) }                    \
+        if (nb == 8) { CAVMAG_TMA_POL_STAGE_CASES(T, NSUB, 8) }                    \
+        return nullptr;                                                            \
     }
 
 #define CAVMAG_DEFINE_TMA_LOOKUP(NAME, T, NSUB)                                    \

@@ -43,6 +43,11 @@ def _axes(N, seed=3):
     ((40, 9, 7), 3, 1, 0.1e-12, "generic"),
     ((13, 5, 3), 2, 2, 0.02e-12, "generic"),       # scalar kernels, two sublattices
     ((36, 10, 5), 9, 1, 0.1e-12, "generic"),       # 32-mode bucket
+    ((72, 19, 5), 3, 1, 0.1e-12, "tma"),           # the TMA kernels' polarised instantiation: 8-mode bucket, ragged tiles
+    ((68, 17, 6), 1, 2, 0.02e-12, "tma"),          # antiferromagnet, one mode
+    ((64, 12, 6), 2, 2, 0.02e-12, "tma"),          # antiferromagnet, two modes
+    ((132, 9, 11), 8, 1, 0.1e-12, "tma"),          # eight modes, three x tiles
+    ((4, 2, 40), 2, 1, 0.1e-12, "tma"),            # one tile, long z march
 ])
 @pytest.mark.parametrize("with_quad", [False, True])
 def test_polarisation_fixed_steps(api, prec, shape, N, n_sub, dt, path, with_quad):
@@ -62,7 +67,9 @@ def test_polarisation_fixed_steps(api, prec, shape, N, n_sub, dt, path, with_qua
         api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=120)
         m, a = sim.get_m(), sim.get_a()
         row = api.cav_get_trace(sim.h)[0]
-        dadt = api.cav_get_dadt(sim.h, N)               # one-stage evaluation: the generic polarisation kernels
+        dadt = api.cav_get_dadt(sim.h, N)               # one-stage evaluation (stage 1 of the same kernel family)
+        want = {"tma": api.CAV_PATH_TMA, "generic": api.CAV_PATH_GENERIC, "block": api.CAV_PATH_BLOCK, "coop": api.CAV_PATH_COOP}[path]
+        assert api.cav_get_kernel_path(sim.h) == want
     _, da_ref, _ = oracle_of(w, pol=p, quad=quad).rhs(ref.m, ref.a)
     assert np.abs(dadt - da_ref).max() <= (1e-9 if prec == "f64" else 1e-3) * np.abs(da_ref).max()
     S = row[1 + 2 * N:1 + 4 * N:2] + 1j * row[2 + 2 * N:2 + 4 * N:2]
@@ -88,10 +95,10 @@ def test_polarisation_default_and_limits(api):
         assert e.value.status == api.CAV_E_ARG
     big = small_problem(512, 160, 2, 1, 1)                                      # 163 840 cells > 512 x SMs
     with api.Sim(big, precision="f32") as sim:
-        # beyond the small-grid kernel a polarised run takes the generic stage kernels (the TMA kernels keep x^)
+        # beyond the small-grid kernel a polarised run stays on the TMA kernels (up to 8 modes; generic kernels beyond)
         assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
         api.cav_set_polarisation(sim.h, [[0.0, 1.0, 0.0]])
-        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_GENERIC
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
         big.m0 = big.m0.astype(np.float32).astype(np.float64); big.u = big.u.astype(np.float32).astype(np.float64)
         refb = oracle_of(big, pol=[[0.0, 1.0, 0.0]]).run(big.m0, big.a0, fixed_dt=0.05e-12, max_steps=10)
         api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=10)
@@ -99,6 +106,28 @@ def test_polarisation_default_and_limits(api):
         with pytest.raises(api.CavError) as e:
             api.cav_set_integrator(sim.h, api.CAV_INTEGRATOR_SPLIT, 1)
         assert e.value.status == api.CAV_E_UNSUPPORTED
+
+
+def test_polarisation_many_modes_and_padded_rows(api):
+    """More than 8 modes: the generic kernels take over on a grid the TMA kernels would run.  Rows padded inside the
+    library (nx = 250 in fp32) exist on the TMA path only: a polarisation is accepted there for up to 8 modes."""
+    w = small_problem(256, 40, 16, 9, 1)
+    with api.Sim(w, precision="f32") as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_set_polarisation(sim.h, _axes(9)[0])
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_GENERIC
+        api.cav_set_polarisation(sim.h, None)
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+    w = small_problem(250, 24, 30, 2, 1)
+    w.m0 = w.m0.astype(np.float32).astype(np.float64); w.u = w.u.astype(np.float32).astype(np.float64)
+    p, q = _axes(2)
+    ref = oracle_of(w, pol=p, quad=q).run(w.m0, w.a0, fixed_dt=0.05e-12, max_steps=20)
+    with api.Sim(w, precision="f32") as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_set_polarisation(sim.h, p, q)
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=20)
+        assert_parity(sim.get_m(), sim.get_a(), ref, "f32")
 
 
 def test_polarisation_batch(api):
