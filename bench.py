@@ -347,18 +347,25 @@ def e2e_pipelined(api, torch, w, prec, tol, k, spinup, barrier, n_streams=E2E_ST
         api.cav_get_m(sim.h, mh)
         sims.append(sim); hosts.append(mh)
 
+    errors = []
+
     def chain(i, n):
-        h, mh = sims[i].h, hosts[i]
-        a = api.cav_get_a(h, N)
-        for _ in range(n):
-            api.cav_set_m(h, mh)                      # H2D from pinned host memory
-            api.cav_set_a(h, a)
-            api.cav_run_steps(h, math.inf, tol=tol, max_steps=1)
-            api.cav_get_m(h, mh)                      # D2H of the step's result (synchronises this simulation's stream)
+        try:
+            h, mh = sims[i].h, hosts[i]
             a = api.cav_get_a(h, N)
+            for _ in range(n):
+                api.cav_set_m(h, mh)                  # H2D from pinned host memory
+                api.cav_set_a(h, a)
+                api.cav_run_steps(h, math.inf, tol=tol, max_steps=1)
+                api.cav_get_m(h, mh)                  # D2H of the step's result (synchronises this simulation's stream)
+                a = api.cav_get_a(h, N)
+        except Exception as e:                        # a failed chain must fail the measurement, not shorten it silently
+            errors.append(e)
 
     for i in range(n_streams):
         chain(i, 3)                                   # warm-up of the host-buffer path
+    if errors:
+        raise errors[0]
     ev0 = [api.cav_get_stats(q.h)["rhs_evals"] for q in sims]
     barrier()
     t0 = time.perf_counter()
@@ -369,6 +376,8 @@ def e2e_pipelined(api, torch, w, prec, tol, k, spinup, barrier, n_streams=E2E_ST
         t.join()
     torch.cuda.synchronize()
     seconds = time.perf_counter() - t0
+    if errors:
+        raise errors[0]
     barrier()
     evals = sum(api.cav_get_stats(q.h)["rhs_evals"] - e for q, e in zip(sims, ev0))
     for q in sims:

@@ -1611,6 +1611,9 @@ int cav_sweep_run(cav_sweep* w, double t_end, double tol, double fixed_dt, doubl
     if (adaptive == (fixed_dt > 0.0)) return CAV_E_ARG;
     if (std::isnan(t_end) || max_steps < 0 || (std::isinf(t_end) && max_steps == 0)) return CAV_E_ARG;
     cav_sim* s = w->sims[0];
+    // what cav_sweep_create refuses must not have been switched on in a member since (the joint kernels know none of it)
+    for (cav_sim* q : w->sims)
+        if (q->d_pol || q->demag || q->split_nllg > 0) return CAV_E_UNSUPPORTED;
     // per-simulation pointers may have changed since the last run (trace, spectrum, mode profiles): refresh, and rebuild
     // the graphs when anything the graph nodes hold by value did
     std::vector<RepPtrs> old = w->h_reps;

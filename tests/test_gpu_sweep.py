@@ -147,6 +147,35 @@ def test_sweep_argument_checks(api, stream):
             s.close()
 
 
+def test_sweep_refuses_members_with_a_variant_switched_on(api, stream):
+    """Polarisation (and the dipolar field, the split integrator) live outside the joint kernels: refused when the sweep
+    is created, and when it is switched on in a member afterwards."""
+    ws = _members(6)
+    sims = [api.Sim(w, precision="f64", stream=stream) for w in ws]
+    sw = None
+    try:
+        api.cav_set_polarisation(sims[2].h, [[0.0, 1.0, 0.0], [1.0, 0.0, 0.0]])
+        with pytest.raises(api.CavError) as e:
+            api.cav_sweep_create(sims)
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+        api.cav_set_polarisation(sims[2].h, None)
+        sw = api.cav_sweep_create(sims)
+        api.cav_sweep_run(sw, math.inf, fixed_dt=0.05e-12, max_steps=2)
+        api.cav_set_polarisation(sims[4].h, [[0.0, 1.0, 0.0], [1.0, 0.0, 0.0]])
+        with pytest.raises(api.CavError) as e:
+            api.cav_sweep_run(sw, math.inf, fixed_dt=0.05e-12, max_steps=2)
+        assert e.value.status == api.CAV_E_UNSUPPORTED
+        api.cav_set_polarisation(sims[4].h, None)
+        api.cav_sweep_run(sw, math.inf, fixed_dt=0.05e-12, max_steps=2)
+        for sim in sims:
+            assert api.cav_get_stats(sim.h)["accepted"] == 4
+    finally:
+        if sw is not None:
+            api.cav_sweep_destroy(sw)
+        for s in sims:
+            s.close()
+
+
 def test_members_stay_ordinary_handles(api, stream):
     """After a joint run a member can go on alone (cav_run on the single handle), a member that has already reached t_end
     is skipped by the next joint run, and the on-device Fourier sums accumulate per member."""
