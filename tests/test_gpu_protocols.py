@@ -107,3 +107,164 @@ def test_anticrossing_sweep_read_out_on_the_device(api):
         api.cav_sweep_destroy(sw)
         for sim in sims:
             sim.close()
+
+
+# ----------------------------------------------------------------------------------------
+# the paper's other lumped protocols on the device: the trace of an adaptive run, fitted with damped exponentials,
+# against the closed forms (Eq. 14 / Eq. 20 and the exact small-signal spectrum) - not against the oracle
+# ----------------------------------------------------------------------------------------
+def _gpu_trace(api, w, t_end, sdt, path, tol=1e-10):
+    cap = int(round(t_end / sdt))
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_trace(sim.h, sdt, cap)
+        api.cav_run(sim.h, t_end, tol=tol)
+        tr = api.cav_get_trace(sim.h)
+        st = api.cav_get_stats(sim.h)
+    assert tr.shape[0] == cap and st["t"] == t_end
+    return tr
+
+
+def _small_signal_spectrum(omega_c, kappa, G, omega_m, alpha):
+    """Complex frequencies (x ~ exp(-i w t)) of N uniform modes + a macrospin near z^, beyond the rotating-wave
+    approximation (Eqs. 3-5, 12-13, 19 linearised; mu = m_x - i m_y):
+        mu' = -(i+alpha) w_m/(1+alpha^2) mu + (i+alpha)/(1+alpha^2) sum_n (G_n a_n + G_n^* a_n^*),  a_n' = -(i w_n + kappa_n) a_n + i G_n mu"""
+    N = len(omega_c)
+    M = np.zeros((N + 1, N + 1), dtype=np.complex128)
+    K = np.zeros((N + 1, N + 1), dtype=np.complex128)
+    d = 1.0 + alpha * alpha
+    for n in range(N):
+        M[n, n] = -(1j * omega_c[n] + kappa[n])
+        M[n, N] = 1j * G[n]
+        M[N, n] = (1j + alpha) / d * G[n]
+        K[N, n] = (1j + alpha) / d * np.conj(G[n])
+    M[N, N] = -(1j + alpha) * omega_m / d
+    lam = 1j * np.linalg.eigvals(np.block([[M, K], [K.conj(), M.conj()]]))
+    return np.sort_complex(lam[lam.real > 0])
+
+
+@pytest.mark.parametrize("path", ["block", "generic"])
+def test_level_attraction_on_the_device(api, path):
+    """PAPER.md:317-333 (Sim 8, Eq. 19-20): purely dissipative coupling g_d/2pi = 50 MHz at resonance: the two real
+    frequencies coalesce and the linewidths split by 2 g_d."""
+    from observables import fit_exponentials, dominant
+    fc, gd, kM, alpha = 5.0, 50.0, 0.5, 3e-4
+    w = W.macrospin(fc, [fc], 0.0, kM, alpha=alpha, a0=[1e-6], Gamma_mhz=[gd], Phi=[-math.pi / 2], n=2)
+    tr = _gpu_trace(api, w, 12e-9, 10e-12, path)
+    om, amp = fit_exponentials(tr[:, 1] + 1j * tr[:, 2], 10e-12, 4)
+    om2, _ = dominant(om, amp, 2)
+    wc, Gd, kap = TWO_PI * fc * 1e9, TWO_PI * gd * 1e6, TWO_PI * kM * 1e6
+    gt = -1j * Gd                                                # the paper's (i g + g_d): g~ = g - i g_d (DESIGN.md G6)
+    wct, wmt = wc - 1j * kap, wc - 1j * alpha * wc
+    root = np.sqrt(gt ** 2 + ((wct - wmt) / 2) ** 2 + 0j)
+    eq20 = np.array([(wct + wmt) / 2 - root, (wct + wmt) / 2 + root])
+    assert abs(om2[0].real - om2[1].real) / TWO_PI < 0.3e6                      # level attraction: one frequency
+    assert abs(abs(om2[0].imag - om2[1].imag) / TWO_PI / 1e6 - 100.0) < 0.5     # linewidths 2 g_d/2pi apart
+    assert np.abs(np.sort(om2.imag) - np.sort(eq20.imag)).max() / TWO_PI < 0.3e6
+    exact = _small_signal_spectrum([wc], [kap], [gt], wc, alpha)
+    assert np.abs(np.sort_complex(om2) - exact).max() / TWO_PI < 20e3
+
+
+@pytest.mark.parametrize("path", ["block", "generic"])
+def test_two_mode_hybridisation_on_the_device(api, path):
+    """PAPER.md:271-285 (Sim 5, Eq. 14): two cavity modes at 4.95 / 5.05 GHz, one magnon between them, g/2pi = 50 MHz:
+    three polariton branches at the eigenvalues of the 3x3 matrix, and the second mode fills up through the magnon."""
+    from observables import fit_exponentials, dominant
+    f1, f2, gM = 4.95, 5.05, 50.0
+    w = W.macrospin(0.5 * (f1 + f2), [f1, f2], gM, 0.0, alpha=0.0, a0=[1e-3, 0.0], n=2)
+    tr = _gpu_trace(api, w, 60e-9, 20e-12, path)
+    g = TWO_PI * gM * 1e6
+    H = np.array([[TWO_PI * f1 * 1e9, g, 0], [g, GAMMA * w.B0[2], g], [0, g, TWO_PI * f2 * 1e9]])
+    ev = np.sort(np.linalg.eigvalsh(H))
+    for n in (0, 1):
+        om, amp = fit_exponentials(tr[:, 1 + 2 * n] + 1j * tr[:, 2 + 2 * n], 20e-12, 6)
+        om3, _ = dominant(om, amp, 3)
+        assert np.abs(om3.real - ev).max() / TWO_PI < 1e6                       # north_star: within 1 MHz
+    a1, a2 = np.hypot(tr[:, 1], tr[:, 2]), np.hypot(tr[:, 3], tr[:, 4])
+    assert a2.max() > 0.5 * a1.max()                                            # magnon-mediated transfer (PAPER.md:283)
+
+
+def test_five_mode_spectrum_on_the_device(api):
+    """Five uniform lossy modes and one damped magnon (the N+1-oscillator problem of north_star) on the 2x2x2 macrospin
+    grid: the six complex frequencies of the device trace against the exact small-signal spectrum (5 kHz) and the
+    rotating-wave arrowhead matrix of Eq. 14 (1 MHz)."""
+    from observables import fit_exponentials, dominant
+    fcs = [9.7, 9.9, 10.0, 10.15, 10.3]
+    gs = [12.0, 20.0, 8.0, 15.0, 25.0]
+    ks = [1.0, 2.0, 0.5, 1.5, 1.0]
+    alpha = 2e-4
+    w = W.macrospin(10.02, fcs, gs, ks, alpha=alpha, a0=[1e-3, 5e-4, -3e-4, 2e-4j, 1e-3], tilt=5e-4, n=2)
+    tr = _gpu_trace(api, w, 120e-9, 20e-12, "block")
+    wm = GAMMA * w.B0[2]
+    exact = _small_signal_spectrum(w.omega, w.kappa, w.g, wm, alpha)
+    H = np.zeros((6, 6), dtype=np.complex128)                    # Eq. 14 with w -> w - i loss (Eq. 7)
+    for n in range(5):
+        H[n, n] = w.omega[n] - 1j * w.kappa[n]
+        H[n, 5] = H[5, n] = w.g[n]
+    H[5, 5] = wm - 1j * alpha * wm
+    rwa = np.sort_complex(np.linalg.eigvals(H))
+    sig = sum((0.3 + n) * (tr[:, 1 + 2 * n] + 1j * tr[:, 2 + 2 * n]) for n in range(5))
+    om, amp = fit_exponentials(sig, 20e-12, 12)
+    om6, _ = dominant(om, amp, 6)
+    om6 = np.sort_complex(om6)
+    assert np.abs(om6 - exact).max() / TWO_PI < 5e3
+    assert np.abs(om6.real - rwa.real).max() / TWO_PI < 1e6
+
+
+def _run_stats(api, w, t_end, sdt, path, tol):
+    cap = int(round(t_end / sdt))
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_trace(sim.h, sdt, cap)
+        api.cav_run(sim.h, t_end, tol=tol)
+        return api.cav_get_trace(sim.h), api.cav_get_stats(sim.h)
+
+
+@pytest.mark.parametrize("path", ["tma", "generic", "coop"])
+def test_mode_selective_coupling_to_a_spin_wave_on_the_device(api, path):
+    """PAPER.md:287-295 (Sim 6) with an exact expectation: the profile u = cos(pi (i + 1/2)/nx) on a 64 x 8 x 4 grid is the
+    k = 1 standing spin wave of the open-boundary stencil; a cavity tuned to its frequency w_1 couples to it with
+    g_eff = g <u phi_1>/sqrt(<phi_1^2>) = g/sqrt(2) (Eq. 18 with W = N_cells), while the uniform precession stays dark.
+    Adaptive run from a(0) != 0: polariton gap 2 g/sqrt(2) and Rabi period pi/(g/sqrt 2), on the spatially resolved
+    kernels (profile-weighted overlap + profile-shaped feedback + exchange)."""
+    from observables import fit_exponentials, dominant, rabi_period
+    nx, ny, nz, d, gM = 64, 8, 4, 5e-9, 50.0
+    phi = W.cosine_profile(1, 0, 0, nx, ny, nz)
+    B0 = W.b0_for_ghz(9.0)
+    w1 = GAMMA * (B0 + 2 * 3.7e-12 / 140e3 * (2 / d ** 2) * (1 - math.cos(math.pi / nx)))
+    m0 = np.zeros((1, 3, nz, ny, nx)); m0[0, 2] = 1.0
+    md = W._modes([w1 / TWO_PI / 1e9], gM, 0.0)
+    w = W.Workload(name="sw", nx=nx, ny=ny, nz=nz, dx=d, dy=d, dz=d, Ms=140e3, Aex=3.7e-12, Ku=0.0, ku_axis=(0, 0, 1),
+                   alpha=0.0, gamma=GAMMA, B0=(0, 0, B0), n_sub=1, B_exch_inter=0.0, u=phi[None], m0=m0,
+                   a0=np.asarray([1e-3], dtype=np.complex128), t_end=0, tol=0, fixed_dt=0, precision="f64", **md)
+    tr, st = _run_stats(api, w, 30e-9, 20e-12, path, 1e-9)
+    a = tr[:, 1] + 1j * tr[:, 2]
+    om, amp = fit_exponentials(a, 20e-12, 4)
+    om2, _ = dominant(om, amp, 2)
+    gap = abs(om2[1].real - om2[0].real) / TWO_PI / 1e6
+    assert abs(gap - 2 * gM / math.sqrt(2)) < 0.3
+    TR = rabi_period(tr[:, 0], np.abs(a) ** 2)
+    assert abs(TR / (math.pi / (TWO_PI * gM * 1e6 / math.sqrt(2))) - 1) < 5e-3         # north_star: within 0.5 %
+    mminus_uniform = tr[:, 1 + 4] - 1j * tr[:, 2 + 4]                                   # <m_x> - i <m_y>: orthogonal to k = 1
+    assert np.abs(mminus_uniform).max() < 1e-12
+    assert st["rejected"] < 0.05 * st["accepted"]
+
+
+@pytest.mark.parametrize("path", ["block", "generic"])
+def test_cooperativity_splitting_on_the_device(api, path):
+    """PAPER.md:246-258 (Sim 3, moderate coupling): g/2pi = 10 MHz, kappa/2pi = 10 MHz, alpha = 3e-4 at 5 GHz:
+    C = g^2/(kappa gamma_m) = 6.7 > 1 and the two lines are resolved.  The paper quotes 2g/2pi = 20.0 MHz as theory and
+    read 21.3 MHz off its FFT; with both loss rates kept (Eq. 7) the gap is 2 sqrt(g^2 - ((kappa - gamma_m)/2)^2) = 18.1 MHz,
+    which is what the device trace gives."""
+    from observables import fit_exponentials, dominant
+    fc, gM, kM, alpha = 5.0, 10.0, 10.0, 3e-4
+    w = W.macrospin(fc, [fc], gM, kM, alpha=alpha, a0=[1e-3], n=2)
+    tr, _ = _run_stats(api, w, 100e-9, 50e-12, path, 1e-10)
+    om, amp = fit_exponentials(tr[:, 1] + 1j * tr[:, 2], 50e-12, 4)
+    om2, _ = dominant(om, amp, 2)
+    gm = alpha * fc * 1e3                                        # gamma_m/2pi = alpha f_m = 1.5 MHz (PAPER.md:89)
+    assert abs(gM ** 2 / (kM * gm) - 6.7) < 0.05
+    gap = abs(om2[1].real - om2[0].real) / TWO_PI / 1e6
+    assert abs(gap - 2 * math.sqrt(gM ** 2 - ((kM - gm) / 2) ** 2)) < 0.05 and abs(gap / 20.0 - 1) < 0.1
+    exact = _small_signal_spectrum([TWO_PI * fc * 1e9], [TWO_PI * kM * 1e6], [TWO_PI * gM * 1e6], TWO_PI * fc * 1e9, alpha)
+    assert np.abs(np.sort_complex(om2) - exact).max() / TWO_PI < 20e3
+    # resolved: the gap exceeds the common linewidth (kappa + gamma_m)/2 of the two hybrid lines
+    assert np.abs(-om2.imag / TWO_PI / 1e6 - 0.5 * (kM + gm)).max() < 0.05 and gap > 0.5 * (kM + gm)
