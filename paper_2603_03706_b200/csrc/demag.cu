@@ -142,6 +142,10 @@ template <typename T> struct ZTile { static constexpr int value = sizeof(T) == 4
 // ---- radix-2 levels of the z transform on values held in registers (W = exp(-2 pi i / Pz), tw[j] = W^j) ----
 template <typename C> __device__ __forceinline__ C c_add(const C& a, const C& b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
 template <typename C> __device__ __forceinline__ C c_sub(const C& a, const C& b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
+// fp32: a complex number is one 64-bit register pair, and sm_100 adds / multiplies both halves in one instruction
+// (FADD2 / FFMA2): half the issue slots of the butterflies, which is what bounds the z convolution
+template <> __device__ __forceinline__ float2 c_add<float2>(const float2& a, const float2& b) { return __fadd2_rn(a, b); }
+template <> __device__ __forceinline__ float2 c_sub<float2>(const float2& a, const float2& b) { return __ffma2_rn(b, make_float2(-1.0f, -1.0f), a); }
 template <typename C> __device__ __forceinline__ C c_mul(const C& a, const C& b) { C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
 template <typename C> __device__ __forceinline__ C c_mulc(const C& a, const C& b) { C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r; }   // a conj(b)
 // decimation in frequency, spans h and h/2, on positions p0, p0 + h/2, p0 + h, p0 + 3h/2 (v[0..3]); t1a, t1b: span-h
