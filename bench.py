@@ -778,10 +778,13 @@ def run_joint_sweep(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    prec = "f64" if args.workload.endswith("_f64") else "f32"            # configs[1]: "fp32 and fp64"
+    esize = 4 if prec == "f32" else 8
+    tdtype = torch.float32 if prec == "f32" else torch.float64
     ghz = W.cfg2_sweep_ghz()
     ws = [W.cfg2(f_kittel_ghz=float(f), seed=2000 + i) for i, f in enumerate(ghz)]
     stream = torch.cuda.Stream()
-    sims = [api.Sim(w, precision="f32", stream=stream.cuda_stream) for w in ws]
+    sims = [api.Sim(w, precision=prec, stream=stream.cuda_stream) for w in ws]
     sw = api.cav_sweep_create(sims)
     tol, nc, N = ws[0].tol, ws[0].n_cells, ws[0].n_modes
 
@@ -808,7 +811,7 @@ def run_joint_sweep(args):
     assert evals == 6 * args.steps * len(sims), evals
     # e2e: host buffers of all simulations every step
     k_e2e = min(args.e2e_steps, 20)
-    hosts = [torch.empty(s.shape_m, dtype=torch.float32).pin_memory() for s in sims]
+    hosts = [torch.empty(s.shape_m, dtype=tdtype).pin_memory() for s in sims]
     for s, hbuf in zip(sims, hosts):
         api.cav_get_m(s.h, hbuf)
     a_hosts = [api.cav_get_a(s.h, N) for s in sims]
@@ -828,16 +831,17 @@ def run_joint_sweep(args):
     for s in sims:
         s.close()
     value = nc * evals / (ms * 1e-3)
-    bytes_per_cs = algorithmic_bytes_per_cell_step(N, 1, 4) / 6.0
+    bytes_per_cs = algorithmic_bytes_per_cell_step(N, 1, esize) / 6.0
     achieved = value * bytes_per_cs / 1e9
     peak, peak_src = hbm_peak()
-    io = int(np.prod(sims[0].shape_m)) * 4 * len(sims) + 16 * N * len(sims)
+    io = int(np.prod(sims[0].shape_m)) * esize * len(sims) + 16 * N * len(sims)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "cfg2_sweep_joint", "grid": [ws[0].nx, ws[0].ny, ws[0].nz], "cells": nc, "simulations": len(sims),
+            "dtype": prec, "data": "synthetic",
+            "config": {"workload": args.workload, "grid": [ws[0].nx, ws[0].ny, ws[0].nz], "cells": nc, "simulations": len(sims),
                        "modes": N, "mode": "adaptive RK45; 41 simulations in one device-side loop (cav_sweep_run)", "tol": tol,
-                       "l2": "41 x 8.7 MB of cell fields = 355 MB in total exceeds the 126 MB L2"},
+                       "precision": prec,
+                       "l2": f"41 x {8.7 * esize / 4:.1f} MB of cell fields = {355 * esize // 4} MB in total exceeds the 126 MB L2"},
             "sim_ns_per_s": sim_t * 1e9 / (ms * 1e-3), "clocks": clocks,
             "e2e": {"value": nc * e2e_evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": io, "d2h_bytes_per_step": io,
                     "steps": k_e2e, "ms_per_step": 1e3 * e2e_s / k_e2e},
@@ -917,7 +921,7 @@ def main():
         run_batch(args)
     elif args.workload == "cfg2_sweep":
         run_concurrent_sweep(args)
-    elif args.workload == "cfg2_sweep_joint":
+    elif args.workload in ("cfg2_sweep_joint", "cfg2_sweep_joint_f64"):
         run_joint_sweep(args)
     else:
         run_cuda(args)
