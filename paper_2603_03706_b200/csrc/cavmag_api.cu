@@ -983,6 +983,7 @@ int cav_set_modes(cav_sim* s, int N, const void* u, int u_is_device, const doubl
         s->N = 0; s->nb = 0;
         Ctrl* c = s->h_ctrl;
         c->N = 0; c->k1_valid = 0; c->drive_on = 0;
+        cudaFree(s->d_pol); s->d_pol = nullptr;          // no modes: nothing to polarise
         destroy_graph(s);
         plan_tma(s);
         push_ctrl(s);
