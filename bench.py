@@ -472,7 +472,7 @@ def run_cuda(args):
     path_used = {api.CAV_PATH_GENERIC: "generic", api.CAV_PATH_TMA: "tma", api.CAV_PATH_BLOCK: "block", api.CAV_PATH_COOP: "coop"}[api.cav_get_kernel_path(h)]
     if name.endswith("_demag"):
         api.cav_set_demag(h, 1)
-        path_used = "generic + FFT convolution (2-D cuFFT + fused z convolution, captured into the run graph)"
+        path_used = "generic + FFT convolution (x: cuFFT on the occupied rows; y, z and the product: own kernels; captured into the run graph)"
     if args.no_stage_overlap:
         api.cav_set_stage_overlap(h, 0)
     if args.no_serpentine:

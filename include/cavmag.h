@@ -239,9 +239,9 @@ int cav_set_integrator(cav_sim* sim, int integrator, int n_llg);
  * disabled"), so it is off by default; on = 1 adds
  *     B_d(r_i) = -mu0 Ms sum_j N(r_i - r_j) . m_tot(r_j)       (open boundary; N: Newell's cell-averaged tensor; m_tot: sum
  * over the sublattices) to the effective field of every evaluation, as a zero-padded FFT convolution (cuFFT, loaded on
- * demand: CAV_E_UNSUPPORTED if it cannot be) in front of each stage kernel.  A different roofline from the fused
- * stencil (six 3-D FFTs of 8x the grid per evaluation): runs use the generic stage kernels whatever
- * cav_set_kernel_path says.  In CAV_LAUNCH_GRAPH mode cuFFT's launches are recorded by stream capture into the body of
+ * demand: CAV_E_UNSUPPORTED if it cannot be, for the transforms along x; the y and z transforms of the occupied rows and
+ * planes and the tensor product are kernels of this library) in front of each stage kernel.  A different roofline from
+ * the fused stencil: runs use the generic stage kernels whatever cav_set_kernel_path says.  In CAV_LAUNCH_GRAPH mode cuFFT's launches are recorded by stream capture into the body of
  * the run graph's WHILE node, so cav_run stays one asynchronous graph launch with no host round trip (if that capture
  * is refused the run is enqueued from the host, as in CAV_LAUNCH_STREAM).  Not available with cav_set_polarisation / the split integrator,
  * nor for grids stored with padded rows (CAV_E_UNSUPPORTED).  DESIGN.md reading G34. */

@@ -1,15 +1,19 @@
 // Dipolar field by FFT convolution (see demag.cuh).
 //
-// Layout of one evaluation (nz <= 64, the usual case: films and slabs):
-//   gather   stage state, summed over the sublattices -> [3][nz][Py][Px] real, zero-padded in x and y only
-//   cuFFT    batched 2-D R2C over (y, x), 3 nz planes: the planes that would only hold zeros are never transformed
+// Layout of one evaluation (nz <= 64 and ny <= 512, the usual case: films and slabs):
+//   gather   stage state, summed over the sublattices -> [3][nz][ny][Px] real, zero-padded in x only
+//   cuFFT    batched 1-D R2C along x over the 3 nz ny occupied rows: rows and planes that would only hold zeros are
+//            never stored or transformed
+//   k_demag_ycol    per (component, z, kx) column and in shared memory: zero-pad the ny rows to Py = 2^qy, FFT along y,
+//            frequency index left in bit-reversed order
 //   k_demag_zconv   per (ky, kx) column and in shared memory: zero-pad to Pz, FFT along z, product with the tensor's
 //            transform, inverse FFT along z, keep z < nz - the full [Pz][Py][Px/2+1] spectrum never exists in memory.
 //            The tensor's transform is real and even/odd in every index: one octant of it is stored, as reals.
-//   cuFFT    batched 2-D C2R, then the scatter of the nx x ny corner into the dense field.
-// This moves about a third of the bytes of a padded 3-D transform pair with a separate product kernel (kept below as the
-// fallback for nz > 64, where the columns of a block do not fit shared memory).  cuFFT does the x/y transforms (a library
-// primitive); the tensor, the gather, the z convolution and the scatter are kernels of this file.
+//   k_demag_ycol    inverse along y, keep the ny rows
+//   cuFFT    batched 1-D C2R along x, then the scatter of the first nx cells of a row into the dense field.
+// Fallbacks: 2-D cuFFT over all Py rows (ny > 512 or nx = 1), padded 3-D cuFFT with a separate product kernel (nz > 64,
+// where the columns of a block do not fit shared memory).  cuFFT does the x transforms (a library primitive); the tensor,
+// the gather, the y and z transforms, the product and the scatter are kernels of this file.
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -213,7 +217,7 @@ __host__ __device__ constexpr int zconv_min_blocks(int q, int tk, int tsize) {  
 
 template <typename T, typename C, int q>
 __global__ void __launch_bounds__(zconv_rows(q) * ZTile<T>::value, zconv_min_blocks(q, ZTile<T>::value, (int)sizeof(T)))
-k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NXH) {
+k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NXH, int qy_rev) {
     constexpr int Pz = 1 << q;
     constexpr int NJ = zconv_rows(q);
     constexpr int kZTile = ZTile<T>::value;
@@ -225,7 +229,9 @@ k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NX
     const long long zs = (long long)Py * NXH;                   // z stride = columns per plane
     const long long col = (long long)blockIdx.x * kZTile + k;
     const bool live = col < zs;
-    const int ky = live ? (int)(col / NXH) : 0, kx = live ? (int)(col % NXH) : 0;
+    const int ky_row = live ? (int)(col / NXH) : 0, kx = live ? (int)(col % NXH) : 0;
+    // (rows written by k_demag_ycol hold the y frequencies in bit-reversed order: qy_rev = log2 Py there, 0 otherwise)
+    const int ky = qy_rev > 0 ? (int)(__brev((unsigned)ky_row) >> (32 - qy_rev)) : ky_row;
     C* const Fc = F + col;                                      // this thread's column: Fc[(c nz + z) zs]
     for (int t = j * kZTile + k; t < Pz / 2; t += NJ * kZTile) {
         double sn, cs;
@@ -413,6 +419,168 @@ const void* zconv_fn(int q) {
     }
 }
 
+// ---- y transform of the occupied rows only ("yfused" layout, Py = 2^q) ----
+// After the x transform only ny of the Py rows of a plane are non-zero, and only ny rows of the result are wanted:
+//   forward (INV = false): in [planes][ny][NXH]  -> zero-pad to Py, transform along y -> out [planes][Py][NXH], frequency
+//                          index in bit-reversed order (the z convolution works column by column and only needs to know
+//                          which frequency a row holds);
+//   inverse (INV = true):  in [planes][Py][NXH] (bit-reversed) -> transform back -> rows y < ny -> out [planes][ny][NXH].
+// Same passes as the z convolution (two radix-2 levels per pass on four values in registers, a lone span-1 level where q
+// is odd; the first pass reads global memory, the last one writes it), one component per column.
+constexpr int kYTile = 16;           // columns (plane, kx) per block
+__host__ __device__ constexpr int ycol_rows(int q) { return (1 << q) / 4 < 1 ? 1 : ((1 << q) / 4 > 32 ? 32 : (1 << q) / 4); }   // blockDim.y
+
+template <typename T, typename C, int q, bool INV>
+__global__ void __launch_bounds__(ycol_rows(q) * kYTile)
+k_demag_ycol(const C* __restrict__ in, C* __restrict__ out, int n_valid, int NXH, long long ncols) {
+    constexpr int P = 1 << q, NJ = ycol_rows(q), TK = kYTile;
+    constexpr int ngrp = (q + 1) / 2;
+    constexpr bool odd = (q & 1) != 0;
+    extern __shared__ __align__(16) unsigned char ysm[];
+    C* const sm = reinterpret_cast<C*>(ysm);                    // [P][TK]
+    C* const tw = sm + P * TK;                                  // exp(-2 pi i j / P), j < P/2
+    const int k = threadIdx.x, j = threadIdx.y;
+    const long long col = (long long)blockIdx.x * TK + k;
+    const bool live = col < ncols;
+    const long long plane = live ? col / NXH : 0;
+    const int kx = live ? (int)(col % NXH) : 0;
+    const C* const ci = in + plane * (long long)(INV ? P : n_valid) * NXH + kx;      // element stride NXH
+    C* const co = out + plane * (long long)(INV ? n_valid : P) * NXH + kx;
+    for (int t = j * TK + k; t < P / 2; t += NJ * TK) {
+        double sn, cs;
+        sincospi(-2.0 * (double)t / (double)P, &sn, &cs);
+        tw[t].x = (T)cs; tw[t].y = (T)sn;
+    }
+    __syncthreads();
+    C zero; zero.x = (T)0; zero.y = (T)0;
+    if constexpr (!INV) {
+        auto forward = [&](auto G) {
+            constexpr int g = decltype(G)::value;
+            constexpr bool single = odd && g == ngrp - 1;
+            constexpr int h = (P / 2) >> (2 * g);
+            constexpr bool first = g == 0, last = g == ngrp - 1;
+            if constexpr (!single) {
+                constexpr int hh = h / 2, s1 = P / (2 * h);
+#pragma unroll
+                for (int w0 = 0; w0 < P / 4; w0 += NJ) {
+                    const int w = w0 + j;
+                    const int r = w % hh, p0 = (w / hh) * 2 * h + r;
+                    const int pos[4] = {p0, p0 + hh, p0 + h, p0 + h + hh};
+                    const C t1a = tw[r * s1], t1b = tw[(r + hh) * s1], t2 = tw[r * 2 * s1];
+                    C v[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if constexpr (first) v[e] = (e < 2 && live && pos[e] < n_valid) ? ci[(long long)pos[e] * NXH] : zero;   // pos >= P/2 >= n_valid: padding
+                        else v[e] = sm[pos[e] * TK + k];
+                    }
+                    if constexpr (first) dif4_padded(v, t1a, t1b, t2);
+                    else dif4(v, t1a, t1b, t2);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if constexpr (last) { if (live) co[(long long)pos[e] * NXH] = v[e]; }
+                        else sm[pos[e] * TK + k] = v[e];
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int w0 = 0; w0 < P / 2; w0 += NJ) {
+                    const int w = w0 + j;
+                    const int pos[2] = {2 * w, 2 * w + 1};
+                    C v[2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        if constexpr (first) v[e] = (live && pos[e] < n_valid) ? ci[(long long)pos[e] * NXH] : zero;
+                        else v[e] = sm[pos[e] * TK + k];
+                    }
+                    const C a = v[0], b = v[1];
+                    v[0] = c_add(a, b); v[1] = c_sub(a, b);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) { if (live) co[(long long)pos[e] * NXH] = v[e]; }      // the lone level is the last one
+                }
+            }
+            if constexpr (!last) __syncthreads();
+        };
+        using std::integral_constant;
+        forward(integral_constant<int, 0>{});
+        if constexpr (ngrp > 1) forward(integral_constant<int, 1>{});
+        if constexpr (ngrp > 2) forward(integral_constant<int, 2>{});
+        if constexpr (ngrp > 3) forward(integral_constant<int, 3>{});
+        if constexpr (ngrp > 4) forward(integral_constant<int, 4>{});
+    } else {
+        auto inverse = [&](auto G) {
+            constexpr int g = decltype(G)::value;
+            constexpr bool single = odd && g == 0;
+            constexpr bool first = g == 0, last = g == ngrp - 1;
+            if constexpr (single) {
+#pragma unroll
+                for (int w0 = 0; w0 < P / 2; w0 += NJ) {
+                    const int w = w0 + j;
+                    const int pos[2] = {2 * w, 2 * w + 1};
+                    C v[2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) v[e] = live ? ci[(long long)pos[e] * NXH] : zero;      // the lone level is the first one
+                    const C a = v[0], b = v[1];
+                    v[0] = c_add(a, b); v[1] = c_sub(a, b);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        if constexpr (last) { if (live && pos[e] < n_valid) co[(long long)pos[e] * NXH] = v[e]; }
+                        else sm[pos[e] * TK + k] = v[e];
+                    }
+                }
+            } else {
+                constexpr int h = odd ? (2 << (2 * (g > 0 ? g - 1 : 0))) : (1 << (2 * g));
+                constexpr int s1 = P / (2 * h), s2 = P / (4 * h);
+#pragma unroll
+                for (int w0 = 0; w0 < P / 4; w0 += NJ) {
+                    const int w = w0 + j;
+                    const int r = w % h, p0 = (w / h) * 4 * h + r;
+                    const int pos[4] = {p0, p0 + h, p0 + 2 * h, p0 + 3 * h};
+                    const C t1 = tw[r * s1], t2a = tw[r * s2], t2b = tw[(r + h) * s2];
+                    C v[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if constexpr (first) v[e] = live ? ci[(long long)pos[e] * NXH] : zero;
+                        else v[e] = sm[pos[e] * TK + k];
+                    }
+                    if constexpr (last) dit4_padded(v, t1, t2a, t2b);       // only the rows below P/2 are wanted
+                    else dit4(v, t1, t2a, t2b);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if constexpr (last) { if (e < 2 && live && pos[e] < n_valid) co[(long long)pos[e] * NXH] = v[e]; }
+                        else sm[pos[e] * TK + k] = v[e];
+                    }
+                }
+            }
+            if constexpr (!last) __syncthreads();
+        };
+        using std::integral_constant;
+        inverse(integral_constant<int, 0>{});
+        if constexpr (ngrp > 1) inverse(integral_constant<int, 1>{});
+        if constexpr (ngrp > 2) inverse(integral_constant<int, 2>{});
+        if constexpr (ngrp > 3) inverse(integral_constant<int, 3>{});
+        if constexpr (ngrp > 4) inverse(integral_constant<int, 4>{});
+    }
+}
+
+constexpr int kYColMaxQ = 10;        // Py <= 1024: [Py][16] complex columns fit the shared memory of a block in both precisions
+
+template <typename T, typename C, bool INV>
+const void* ycol_fn(int q) {
+    switch (q) {
+        case 1: return (const void*)k_demag_ycol<T, C, 1, INV>;
+        case 2: return (const void*)k_demag_ycol<T, C, 2, INV>;
+        case 3: return (const void*)k_demag_ycol<T, C, 3, INV>;
+        case 4: return (const void*)k_demag_ycol<T, C, 4, INV>;
+        case 5: return (const void*)k_demag_ycol<T, C, 5, INV>;
+        case 6: return (const void*)k_demag_ycol<T, C, 6, INV>;
+        case 7: return (const void*)k_demag_ycol<T, C, 7, INV>;
+        case 8: return (const void*)k_demag_ycol<T, C, 8, INV>;
+        case 9: return (const void*)k_demag_ycol<T, C, 9, INV>;
+        case 10: return (const void*)k_demag_ycol<T, C, 10, INV>;
+        default: return nullptr;
+    }
+}
+
 // The state stage `stage` is evaluated at, summed over the sublattices, into the zero-padded array [3][Pz][Py][Px]
 // (the pad region is zeroed once and never written).  Buffer indices and h as the stage kernel reads them.
 template <typename T>
@@ -478,6 +646,14 @@ struct DemagPlan {
     void* khat = nullptr;                // zfused: [6][Pz/2+1][Py/2+1][Px/2+1] real; else [6][nf] complex
     size_t zsmem = 0;
     const void* zfn = nullptr;           // k_demag_zconv<T, C, q>
+    // yfused (zfused, nx > 1, Py = 2^qy <= 1024): cuFFT transforms the ny occupied rows along x only, k_demag_ycol does y
+    bool yfused = false;
+    int qy = 0;
+    void* xf = nullptr;                  // [3][nz][ny][Px/2+1] complex: x-transformed occupied rows (qy > 0)
+    size_t ysmem = 0;
+    const void* yfwd = nullptr;
+    const void* yinv = nullptr;
+    int prows = 0;                       // rows per plane of pad / conv: ny (yfused) or Py
     cufftHandle fwd = 0, inv = 0;
     bool have_fwd = false, have_inv = false;
 };
@@ -489,7 +665,7 @@ void demag_destroy(DemagPlan* p) {
     FftApi& f = fft_api();
     if (p->have_fwd) f.Destroy(p->fwd);
     if (p->have_inv) f.Destroy(p->inv);
-    cudaFree(p->pad); cudaFree(p->freq); cudaFree(p->conv); cudaFree(p->khat);
+    cudaFree(p->pad); cudaFree(p->freq); cudaFree(p->conv); cudaFree(p->khat); cudaFree(p->xf);
     cudaGetLastError();
     delete p;
 }
@@ -507,20 +683,36 @@ int demag_create(DemagPlan** out, int nx, int ny, int nz, double dx, double dy, 
     p->Px = nx > 1 ? 2 * nx : 1; p->Py = ny > 1 ? 2 * ny : 1;
     if (p->zfused) { p->Pz = 1; p->q = 0; while (p->Pz < 2 * nz - 1) { p->Pz *= 2; p->q++; } }
     else p->Pz = 2 * nz;
+    if (p->zfused && nx > 1) {           // y by k_demag_ycol: Py a power of two >= 2 ny - 1
+        int Py2 = 1, qy = 0;
+        while (Py2 < 2 * ny - 1) { Py2 *= 2; qy++; }
+        if (qy <= kYColMaxQ) { p->yfused = true; p->Py = Py2; p->qy = qy; }
+    }
     p->zplanes = p->zfused ? nz : p->Pz;
+    p->prows = p->yfused ? ny : p->Py;
     const int NXH = p->Px / 2 + 1, NYH = p->Py / 2 + 1, NZH = p->Pz / 2 + 1;
-    p->pvol = (long long)p->Px * p->Py * p->zplanes;
+    p->pvol = (long long)p->Px * p->prows * p->zplanes;
     p->nf = (long long)p->zplanes * p->Py * NXH;
     const size_t rs = f32 ? 4 : 8, cs = 2 * rs;
     const size_t kbytes = p->zfused ? (size_t)6 * NZH * NYH * NXH * rs : (size_t)6 * p->nf * cs;
     if (cudaMalloc(&p->pad, 3 * p->pvol * rs) != cudaSuccess || cudaMalloc(&p->conv, 3 * p->pvol * rs) != cudaSuccess ||
         cudaMalloc(&p->freq, 3 * p->nf * cs) != cudaSuccess || cudaMalloc(&p->khat, kbytes) != cudaSuccess)
         return fail(CAV_E_NOMEM, "device allocation");
+    if (p->yfused && p->qy > 0 && cudaMalloc(&p->xf, (size_t)3 * nz * ny * NXH * cs) != cudaSuccess) return fail(CAV_E_NOMEM, "device allocation");
     if (cudaMemsetAsync(p->pad, 0, 3 * p->pvol * rs, stream) != cudaSuccess) return fail(CAV_E_CUDA, "memset");
     int n3[3] = {p->Pz, p->Py, p->Px};
     int n2[2] = {p->Py, p->Px};
-    const int rank = p->zfused ? 2 : 3, batch = p->zfused ? 3 * nz : 3;
-    int* const nn = p->zfused ? n2 : n3;
+    int n1[1] = {p->Px};
+    const int rank = p->yfused ? 1 : (p->zfused ? 2 : 3), batch = p->yfused ? 3 * nz * ny : (p->zfused ? 3 * nz : 3);
+    int* const nn = p->yfused ? n1 : (p->zfused ? n2 : n3);
+    if (p->yfused && p->qy > 0) {
+        p->ysmem = ((size_t)p->Py * kYTile + (size_t)p->Py / 2) * cs;
+        p->yfwd = f32 ? ycol_fn<float, cufftComplex, false>(p->qy) : ycol_fn<double, cufftDoubleComplex, false>(p->qy);
+        p->yinv = f32 ? ycol_fn<float, cufftComplex, true>(p->qy) : ycol_fn<double, cufftDoubleComplex, true>(p->qy);
+        if (cudaFuncSetAttribute(p->yfwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ysmem) != cudaSuccess ||
+            cudaFuncSetAttribute(p->yinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ysmem) != cudaSuccess)
+            return fail(CAV_E_CUDA, "shared memory for the y transform");
+    }
     if (f.PlanMany(&p->fwd, rank, nn, nullptr, 1, 0, nullptr, 1, 0, f32 ? CUFFT_R2C : CUFFT_D2Z, batch) != CUFFT_SUCCESS) return fail(CAV_E_CUDA, "cufftPlanMany (forward)");
     p->have_fwd = true;
     if (f.PlanMany(&p->inv, rank, nn, nullptr, 1, 0, nullptr, 1, 0, f32 ? CUFFT_C2R : CUFFT_Z2D, batch) != CUFFT_SUCCESS) return fail(CAV_E_CUDA, "cufftPlanMany (inverse)");
@@ -575,25 +767,36 @@ int demag_apply(DemagPlan* p, const StageArgs& A, int stage, void* bdem, cudaStr
     const int tk = p->f32 ? ZTile<float>::value : ZTile<double>::value;
     const dim3 zgrid((unsigned)(((long long)p->Py * NXH + tk - 1) / tk));
     const dim3 zblock((unsigned)tk, (unsigned)zconv_rows(p->q));
-    int nzv = p->nz, pyv = p->Py, nxhv = NXH;
-    void* zargs[] = {&p->freq, &p->khat, &nzv, &pyv, &nxhv};
+    int nzv = p->nz, pyv = p->Py, nxhv = NXH, qyrev = (p->yfused ? p->qy : 0);
+    void* zargs[] = {&p->freq, &p->khat, &nzv, &pyv, &nxhv, &qyrev};
+    // y transform of the occupied rows (yfused): columns (component, z, kx)
+    const bool ycol = p->yfused && p->qy > 0;
+    void* const xspec = ycol ? p->xf : p->freq;              // what the x transforms write / read
+    long long ncols = (long long)3 * p->nz * NXH;
+    int nyv = p->ny;
+    const dim3 ygrid((unsigned)((ncols + kYTile - 1) / kYTile));
+    const dim3 yblock((unsigned)kYTile, (unsigned)ycol_rows(p->qy));
+    void* yfargs[] = {&p->xf, &p->freq, &nyv, &nxhv, &ncols};
+    void* yiargs[] = {&p->freq, &p->xf, &nyv, &nxhv, &ncols};
     f.SetStream(p->fwd, stream);
     f.SetStream(p->inv, stream);
-    if (p->f32) {
-        k_demag_gather<float><<<gc, gtb, 0, stream>>>(A, stage, p->n_sub, (float*)p->pad, p->Px, p->Py, p->zplanes);
-        if (f.ExecR2C(p->fwd, (cufftReal*)p->pad, (cufftComplex*)p->freq) != CUFFT_SUCCESS) return CAV_E_CUDA;
+    auto run = [&](auto tag_real, auto tag_cplx) -> int {
+        using R = decltype(tag_real);
+        using Cx = decltype(tag_cplx);
+        k_demag_gather<R><<<gc, gtb, 0, stream>>>(A, stage, p->n_sub, (R*)p->pad, p->Px, p->prows, p->zplanes);
+        if constexpr (sizeof(R) == 4) { if (f.ExecR2C(p->fwd, (cufftReal*)p->pad, (cufftComplex*)xspec) != CUFFT_SUCCESS) return CAV_E_CUDA; }
+        else { if (f.ExecD2Z(p->fwd, (cufftDoubleReal*)p->pad, (cufftDoubleComplex*)xspec) != CUFFT_SUCCESS) return CAV_E_CUDA; }
+        if (ycol && cudaLaunchKernel(p->yfwd, ygrid, yblock, yfargs, p->ysmem, stream) != cudaSuccess) return CAV_E_CUDA;
         if (p->zfused) { if (cudaLaunchKernel(p->zfn, zgrid, zblock, zargs, p->zsmem, stream) != cudaSuccess) return CAV_E_CUDA; }
-        else k_demag_product<cufftComplex><<<gf, tb, 0, stream>>>((cufftComplex*)p->freq, (const cufftComplex*)p->khat, p->nf);
-        if (f.ExecC2R(p->inv, (cufftComplex*)p->freq, (cufftReal*)p->conv) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        k_demag_scatter<float><<<gc, gtb, 0, stream>>>((const float*)p->conv, (float*)bdem, A.nx, A.ny, A.nc, p->Px, p->Py, p->zplanes);
-    } else {
-        k_demag_gather<double><<<gc, gtb, 0, stream>>>(A, stage, p->n_sub, (double*)p->pad, p->Px, p->Py, p->zplanes);
-        if (f.ExecD2Z(p->fwd, (cufftDoubleReal*)p->pad, (cufftDoubleComplex*)p->freq) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        if (p->zfused) { if (cudaLaunchKernel(p->zfn, zgrid, zblock, zargs, p->zsmem, stream) != cudaSuccess) return CAV_E_CUDA; }
-        else k_demag_product<cufftDoubleComplex><<<gf, tb, 0, stream>>>((cufftDoubleComplex*)p->freq, (const cufftDoubleComplex*)p->khat, p->nf);
-        if (f.ExecZ2D(p->inv, (cufftDoubleComplex*)p->freq, (cufftDoubleReal*)p->conv) != CUFFT_SUCCESS) return CAV_E_CUDA;
-        k_demag_scatter<double><<<gc, gtb, 0, stream>>>((const double*)p->conv, (double*)bdem, A.nx, A.ny, A.nc, p->Px, p->Py, p->zplanes);
-    }
+        else k_demag_product<Cx><<<gf, tb, 0, stream>>>((Cx*)p->freq, (const Cx*)p->khat, p->nf);
+        if (ycol && cudaLaunchKernel(p->yinv, ygrid, yblock, yiargs, p->ysmem, stream) != cudaSuccess) return CAV_E_CUDA;
+        if constexpr (sizeof(R) == 4) { if (f.ExecC2R(p->inv, (cufftComplex*)xspec, (cufftReal*)p->conv) != CUFFT_SUCCESS) return CAV_E_CUDA; }
+        else { if (f.ExecZ2D(p->inv, (cufftDoubleComplex*)xspec, (cufftDoubleReal*)p->conv) != CUFFT_SUCCESS) return CAV_E_CUDA; }
+        k_demag_scatter<R><<<gc, gtb, 0, stream>>>((const R*)p->conv, (R*)bdem, A.nx, A.ny, A.nc, p->Px, p->prows, p->zplanes);
+        return CAV_OK;
+    };
+    const int rc = p->f32 ? run(float{}, cufftComplex{}) : run(double{}, cufftDoubleComplex{});
+    if (rc) return rc;
     return cudaGetLastError() == cudaSuccess ? CAV_OK : CAV_E_CUDA;
 }
 

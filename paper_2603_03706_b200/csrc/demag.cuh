@@ -1,7 +1,7 @@
 // Optional dipolar (demagnetising) field (the paper switches it off; reading G34):
 //     B_d(r_i) = -mu0 Ms sum_j N(r_i - r_j) . m_tot(r_j)      open boundary, N = Newell's cell-averaged tensor
-// evaluated as a zero-padded FFT convolution before every stage kernel (batched 2-D cuFFT transforms of the occupied planes
-// and one kernel for the z transform, the tensor product and the inverse z transform: demag.cu).  A different roofline
+// evaluated as a zero-padded FFT convolution before every stage kernel (cuFFT along x over the occupied rows, own kernels
+// for the y transform and for the z transform + tensor product + inverse z transform: demag.cu).  A different roofline
 // from the fused stencil; it runs on the generic stage kernels, its launches captured into the run graph (cavmag_api.cu).
 #pragma once
 #include <cuda_runtime.h>

@@ -313,6 +313,8 @@ def test_spectrum_shows_both_polariton_branches(api):
     ((5, 3, 9), 1, 1, 0.1e-12),        # z column of 32: an odd number of levels
     ((4, 3, 40), 1, 1, 0.1e-12),       # z column of 128: more butterflies than worker rows
     ((3, 2, 130), 0, 1, 0.1e-12),      # beyond the shared-memory z column: padded 3-D transforms
+    ((1, 6, 3), 1, 1, 0.1e-12),        # one cell in x: the y transform stays with cuFFT (2-D plans), z in the fused kernel
+    ((20, 33, 2), 1, 1, 0.1e-12),      # ny = 33: Py = 128 (next power of two above 2 ny - 1 = 65), an odd number of levels
 ])
 def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
     """The FFT convolution against the oracle's direct O(N^2) sum with the Newell tensor: right-hand side cell by cell,
