@@ -315,6 +315,8 @@ def test_spectrum_shows_both_polariton_branches(api):
     ((3, 2, 130), 0, 1, 0.1e-12),      # beyond the shared-memory z column: padded 3-D transforms
     ((1, 6, 3), 1, 1, 0.1e-12),        # one cell in x: the y transform stays with cuFFT (2-D plans), z in the fused kernel
     ((20, 33, 2), 1, 1, 0.1e-12),      # ny = 33: Py = 128 (next power of two above 2 ny - 1 = 65), an odd number of levels
+    ((600, 2, 1), 0, 1, 0.1e-12),      # nx > 512: the x transforms stay with cuFFT (1-D over the occupied rows), y by the column kernel
+    ((7, 3, 2), 1, 2, 0.02e-12),       # odd ny: the last row pair of a plane has one row; two sublattices
 ])
 def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
     """The FFT convolution against the oracle's direct O(N^2) sum with the Newell tensor: right-hand side cell by cell,
@@ -343,12 +345,12 @@ def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
     scale = np.abs(dm_ref).max()
     # Newell's closed forms lose digits with distance (27-point second differences of terms ~R^3: ~(R/d)^5 eps relative
     # in an entry ~(d/R)^3); CPU and device evaluate them with different libm roundings: 1e-11 of the field at 130 cells
-    tol64 = 5e-13 if max(shape) <= 40 else 5e-11
+    tol64 = 5e-13 if max(shape) <= 40 else (5e-11 if max(shape) <= 200 else 5e-9)       # (600 cells: 8e-10 measured)
     assert np.abs(dm - dm_ref).max() <= (tol64 if prec == "f64" else 3e-5) * scale
     if max(shape) <= 40 or prec == "f32":
         assert_parity(m, a, ref, prec)
     else:
-        assert np.abs(m - ref.m).max() <= 1e-9           # (the same loss of digits, integrated over 100 steps)
+        assert np.abs(m - ref.m).max() <= (1e-9 if max(shape) <= 200 else 1e-8)           # (the same loss of digits, integrated over 100 steps)
     plain = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=100)
     assert np.abs(plain.m - ref.m).max() > 1e-4                       # mu0 Ms = 0.18 T: not a detail
     dm_plain, _, _ = oracle_of(w).rhs(ref.m, ref.a)
