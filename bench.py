@@ -43,7 +43,7 @@ UNIT = "cell-stage/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per stage-kernel launch (mean over the six stages of
 # one step) from the `ncu --set full` capture summarised in profiles/ (file named beside each value).
 NCU_TRAFFIC_BYTES = {      # cold-cache captures (ncu flushes between replays); algorithmic bytes in brackets
-    "cfg3": 209.0e6,       # profiles/r2_cfg3_stage_kernels.md      (222.3 MB)
+    "cfg3": 208.6e6,       # profiles/r2_cfg3_stage_kernels.md      (222.3 MB)
     "cfg4": 136.1e6,       # profiles/r2_cfg4_stage_kernels.md      (159.4 MB)
     "cfg4_f64": 334.3e6,   # profiles/r2_cfg4_f64_stage_kernels.md  (318.8 MB)
     "cfg5": 3676.6e6,      # profiles/r2_cfg5_stage_kernels.md      (3389.0 MB): the halo
