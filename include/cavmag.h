@@ -250,12 +250,14 @@ int cav_set_demag(cav_sim* sim, int on);
 /* On-device spectroscopy: the Fourier sums behind the paper's spectra |FFT(m^-)|^2 + |FFT(a)|^2,
  * accumulated inside the step controller at every trace sample (cav_set_trace decides when) instead of copying the
  * trace to the host:   X[k][sig] += x_sig(t_j) exp(+i w_k t_j),   w_k = omega_lo + k (omega_hi - omega_lo)/(n_bins - 1),
- * for the 2N signals x = a_1..a_N, S_1..S_N (a component ~ exp(-i w0 t), peaks at w_k = w0; a frequency
- * grid finer than 1/T is the paper's zero padding).  Any path, any grid.  n_bins = 0 switches it off; the call zeroes
- * the sums; a new mode set drops them.  cav_get_spectrum copies [n_bins][2N][2] doubles to the host and reports the
- * number of samples accumulated. */
+ * for the 2N + n_sub signals x = a_1..a_N, S_1..S_N, mu_1..mu_nsub with mu_s = <m_s,x> - i <m_s,y> the plain average of
+ * sublattice s (the paper's m^-; (mu_1 - mu_2)/2 is the Neel vector's transverse part, PAPER.md:335 - the sums are linear)
+ * (a component ~ exp(-i w0 t), peaks at w_k = w0; a frequency grid finer than 1/T is the paper's zero
+ * padding).  Any path, any grid, N = 0 included.  n_bins = 0 switches it off; the call zeroes the sums; a new mode set
+ * drops them.  cav_get_spectrum copies [n_bins][2N + n_sub][2] doubles to the host and reports the number of samples
+ * accumulated. */
 int cav_set_spectrum(cav_sim* sim, int n_bins, double omega_lo, double omega_hi);
-int cav_get_spectrum(cav_sim* sim, double* out /* [n_bins][2N][2] host */, long long* n_samples);
+int cav_get_spectrum(cav_sim* sim, double* out /* [n_bins][2N + n_sub][2] host */, long long* n_samples);
 
 /* Number of kernels this library has launched for this handle (stage kernels + setup). */
 int cav_get_launch_count(cav_sim* sim, long long* n);
@@ -298,7 +300,7 @@ int cav_batch_set_backaction(cav_batch* b, const double* g_b, const double* Gamm
 int cav_batch_set_drive(cav_batch* b, const double* amp_re_im, const double* t0, const double* sigma, const double* omega_d);
 
 /* Polarisation, integrator and spectrum as cav_set_polarisation / cav_set_integrator / cav_set_spectrum, common to all
- * replicas; the spectrum is kept per replica: [n_rep][n_bins][2N][2], n_samples [n_rep].  Call after cav_batch_set_modes. */
+ * replicas; the spectrum is kept per replica: [n_rep][n_bins][2N + n_sub][2], n_samples [n_rep].  Call after cav_batch_set_modes. */
 int cav_batch_set_polarisation(cav_batch* b, const double* pol, const double* quad);
 int cav_batch_set_integrator(cav_batch* b, int integrator, int n_llg);
 int cav_batch_set_spectrum(cav_batch* b, int n_bins, double omega_lo, double omega_hi);

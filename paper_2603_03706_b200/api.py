@@ -575,8 +575,8 @@ def cav_set_spectrum(sim, n_bins: int, omega_lo: float = 0.0, omega_hi: float = 
 
 
 def cav_get_spectrum(sim, n_bins: int, N: int):
-    """Returns (X [n_bins][2N] complex, n_samples)."""
-    out = np.zeros((n_bins, 2 * N, 2))
+    """Returns (X [n_bins][2N + n_sub] complex, n_samples): columns a_1..a_N, S_1..S_N, then <m_s,x> - i <m_s,y> per sublattice."""
+    out = np.zeros((n_bins, 2 * N + _HANDLES[sim][1], 2))
     n = _ll()
     _check(_lib.cav_get_spectrum(sim, out.ctypes.data_as(_dp), C.byref(n)), "cav_get_spectrum", sim)
     return out[..., 0] + 1j * out[..., 1], n.value
@@ -587,8 +587,8 @@ def cav_batch_set_spectrum(b, n_bins: int, omega_lo: float = 0.0, omega_hi: floa
 
 
 def cav_batch_get_spectrum(b, n_rep: int, n_bins: int, N: int):
-    """Returns (X [n_rep][n_bins][2N] complex, n_samples [n_rep])."""
-    out = np.zeros((n_rep, n_bins, 2 * N, 2))
+    """Returns (X [n_rep][n_bins][2N + n_sub] complex, n_samples [n_rep])."""
+    out = np.zeros((n_rep, n_bins, 2 * N + _HANDLES[b][1], 2))
     ns = (_ll * n_rep)()
     _check(_lib.cav_batch_get_spectrum(b, out.ctypes.data_as(_dp), ns), "cav_batch_get_spectrum")
     return out[..., 0] + 1j * out[..., 1], np.array(list(ns))

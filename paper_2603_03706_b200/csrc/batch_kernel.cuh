@@ -513,8 +513,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
         }
         __syncthreads();                                                 // [D]
         if (A.spec != nullptr && sh.took && sh.accept && writer) {       // Fourier sums of this sample (a_new, S of the new state)
-            dft_accumulate(A.spec + (size_t)rep * A.spec_K * 4 * N, A.spec_K, A.spec_w0, A.spec_dw, N, sh.t, sh.anew, sh.S,
-                           tid, (int)blockDim.x);
+            dft_accumulate(A.spec + (size_t)rep * A.spec_K * 2 * (2 * N + NSUB), A.spec_K, A.spec_w0, A.spec_dw, N, sh.t, sh.anew, sh.S,
+                           sh.red, NSUB, tid, (int)blockDim.x);
             if (tid == 0) A.spec_n[rep]++;
         }
         if (sh.accept) {                                                 // y := y_new, FSAL: k1 := k7

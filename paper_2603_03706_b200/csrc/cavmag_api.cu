@@ -81,7 +81,7 @@ struct cav_sim {
     // ---- SURVEY.md 8(f3) / 8(f2) variants ----
     double* d_pol = nullptr;           // [N][6] polarisation + quadrature axes, or NULL: x^, y^
     int split_nllg = 0;                // 0: unified RK45; n >= 1: operator-split comparison integrator, n LLG sub-steps per cavity step
-    double* d_spec = nullptr;          // [spec_K][2N][2] Fourier sums, or NULL
+    double* d_spec = nullptr;          // [spec_K][2N + n_sub][2] Fourier sums, or NULL
     DemagPlan* demag = nullptr;        // dipolar field by FFT convolution, or NULL: off (the paper's setting)
     void* d_bdem = nullptr;            // [3][nc] dipolar field of the stage about to be evaluated
     bool graph_pdl = false;            // loop-body edges of the current graph are programmatic dependencies
@@ -1156,8 +1156,8 @@ int cav_set_spectrum(cav_sim* s, int n_bins, double omega_lo, double omega_hi) {
     s->graph_dirty = true;               // the pointer is a kernel argument
     Ctrl* c = s->h_ctrl;
     c->spec_K = 0; c->spec_n = 0;
-    if (n_bins > 0 && s->N > 0) {
-        const size_t bytes = sizeof(double) * (size_t)n_bins * 4 * s->N;
+    if (n_bins > 0) {
+        const size_t bytes = sizeof(double) * (size_t)n_bins * 2 * (2 * s->N + s->prm.n_sub);
         CK(cudaMalloc(&s->d_spec, bytes));
         CK(cudaMemsetAsync(s->d_spec, 0, bytes, s->stream));
         c->spec_K = n_bins; c->spec_w0 = omega_lo; c->spec_dw = n_bins > 1 ? (omega_hi - omega_lo) / (double)(n_bins - 1) : 0.0;
@@ -1170,7 +1170,7 @@ int cav_get_spectrum(cav_sim* s, double* out, long long* n_samples) {
     if (!s->d_spec) return CAV_E_STATE;
     int rc = sync_pull(s);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(out, s->d_spec, sizeof(double) * (size_t)s->h_ctrl->spec_K * 4 * s->N, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaMemcpyAsync(out, s->d_spec, sizeof(double) * (size_t)s->h_ctrl->spec_K * 2 * (2 * s->N + s->prm.n_sub), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     if (n_samples) *n_samples = s->h_ctrl->spec_n;
     return s->h_ctrl->status;

@@ -24,7 +24,7 @@ struct cav_batch {
     double* d_drive = nullptr;     // [5][N] or NULL: no drive
     double* d_pol = nullptr;       // [N][6] polarisation + quadrature axes or NULL: x^, y^
     int split_nllg = 0;            // 0: unified RK45; n >= 1: operator-split loop with n LLG sub-steps per cavity step
-    double* d_spec = nullptr;      // [n_rep][spec_K][2N][2] Fourier sums or NULL
+    double* d_spec = nullptr;      // [n_rep][spec_K][2N + n_sub][2] Fourier sums or NULL
     long long* d_spec_n = nullptr; // [n_rep]
     int spec_K = 0;
     double spec_w0 = 0.0, spec_dw = 0.0;
@@ -456,8 +456,8 @@ int cav_batch_set_spectrum(cav_batch* b, int n_bins, double omega_lo, double ome
     CKB(cudaStreamSynchronize(b->stream));
     cudaFree(b->d_spec); cudaFree(b->d_spec_n);
     b->d_spec = nullptr; b->d_spec_n = nullptr; b->spec_K = 0;
-    if (n_bins == 0 || b->N == 0) return CAV_OK;
-    const size_t bytes = sizeof(double) * (size_t)b->n_rep * n_bins * 4 * b->N;
+    if (n_bins == 0) return CAV_OK;
+    const size_t bytes = sizeof(double) * (size_t)b->n_rep * n_bins * 2 * (2 * b->N + b->prm.n_sub);
     CKB(cudaMalloc(&b->d_spec, bytes));
     CKB(cudaMalloc(&b->d_spec_n, sizeof(long long) * b->n_rep));
     CKB(cudaMemsetAsync(b->d_spec, 0, bytes, b->stream));
@@ -470,7 +470,7 @@ int cav_batch_set_spectrum(cav_batch* b, int n_bins, double omega_lo, double ome
 int cav_batch_get_spectrum(cav_batch* b, double* out, long long* n_samples) {
     if (!b || !out) return CAV_E_ARG;
     if (!b->d_spec) return CAV_E_STATE;
-    CKB(cudaMemcpyAsync(out, b->d_spec, sizeof(double) * (size_t)b->n_rep * b->spec_K * 4 * b->N, cudaMemcpyDeviceToHost, b->stream));
+    CKB(cudaMemcpyAsync(out, b->d_spec, sizeof(double) * (size_t)b->n_rep * b->spec_K * 2 * (2 * b->N + b->prm.n_sub), cudaMemcpyDeviceToHost, b->stream));
     if (n_samples) CKB(cudaMemcpyAsync(n_samples, b->d_spec_n, sizeof(long long) * b->n_rep, cudaMemcpyDeviceToHost, b->stream));
     CKB(cudaStreamSynchronize(b->stream));
     return CAV_OK;

@@ -231,18 +231,24 @@ __device__ __forceinline__ void reduce_block_partials(const double* partial, con
     }
 }
 
-// On-device spectroscopy: at a trace sample (time t, amplitudes a_n, overlaps S_n)
-// every bin k adds x exp(+i w_k t) for the 2N signals x = a_1..a_N, S_1..S_N.  Thread k owns bin k, k + nthr, ...: no
-// two threads touch the same accumulator, and successive samples are ordered by the kernel's own barriers.
+// On-device spectroscopy: at a trace sample (time t, amplitudes a_n, overlaps S_n,
+// sublattice means <m_s>) every bin k adds x exp(+i w_k t) for the 2N + n_sub signals x = a_1..a_N, S_1..S_N and
+// mu_s = <m_s,x> - i <m_s,y> (the paper's m^- of the plain average; (mu_1 - mu_2)/2 is the Neel vector's).
+// Thread k owns bin k, k + nthr, ...: no two threads touch the same accumulator, and successive samples are ordered by
+// the kernel's own barriers.
 __device__ __forceinline__ void dft_accumulate(double* spec, const int K, const double w0, const double dw, const int N,
                                                const double t, const double (*a)[2], const double (*S)[2],
-                                               const int tid, const int nthr) {
+                                               const double* mavg, const int nsub, const int tid, const int nthr) {
+    const int nsig = 2 * N + nsub;
     for (int k = tid; k < K; k += nthr) {
         double sn, cs;
         sincos((w0 + (double)k * dw) * t, &sn, &cs);
-        double* X = spec + (size_t)k * 4 * N;
-        for (int sig = 0; sig < 2 * N; ++sig) {
-            const double xr = sig < N ? a[sig][0] : S[sig - N][0], xi = sig < N ? a[sig][1] : S[sig - N][1];
+        double* X = spec + (size_t)k * 2 * nsig;
+        for (int sig = 0; sig < nsig; ++sig) {
+            double xr, xi;
+            if (sig < N) { xr = a[sig][0]; xi = a[sig][1]; }
+            else if (sig < 2 * N) { xr = S[sig - N][0]; xi = S[sig - N][1]; }
+            else { xr = mavg[3 * (sig - 2 * N)]; xi = -mavg[3 * (sig - 2 * N) + 1]; }
             X[2 * sig] += xr * cs - xi * sn;
             X[2 * sig + 1] += xr * sn + xi * cs;
         }
@@ -419,7 +425,7 @@ static __device__ __noinline__ void stage_finish(const FinishArgs A, const int n
             if (tid == 0) s_accept = controller_step(c, smax, serr, sred, N, nsub, A.inv_nc, trace, true);
             __syncthreads();
             if (A.spec != nullptr && c->spec_K > 0 && c->took)       // Fourier sums of this trace sample
-                dft_accumulate(A.spec, c->spec_K, c->spec_w0, c->spec_dw, N, c->t, c->anew, c->S, tid, nthr);
+                dft_accumulate(A.spec, c->spec_K, c->spec_w0, c->spec_dw, N, c->t, c->anew, c->S, c->mavg, nsub, tid, nthr);
             if (tid < N && s_accept) {     // y := y_new (modes), FSAL: ka_1 := ka_7
                 c->a[tid][0] = c->anew[tid][0]; c->a[tid][1] = c->anew[tid][1];
                 c->ka[0][tid][0] = c->ka[6][tid][0]; c->ka[0][tid][1] = c->ka[6][tid][1];

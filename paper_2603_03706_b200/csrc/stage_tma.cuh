@@ -261,7 +261,7 @@ __device__ __forceinline__ bool deferred_finish7(const StageArgs& A, const TmaAr
         }
         asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory");
         if (write && A.spec != nullptr && c->spec_K > 0 && c->took)       // Fourier sums of this trace sample
-            dft_accumulate(A.spec, c->spec_K, c->spec_w0, c->spec_dw, N, c->t, c->anew, c->S, tidc, kTmaConsumers);
+            dft_accumulate(A.spec, c->spec_K, c->spec_w0, c->spec_dw, N, c->t, c->anew, c->S, c->mavg, NSUB, tidc, kTmaConsumers);
         if (tidc < N && serr[kMaxModes + 1] != 0.0) {     // y := y_new (modes), FSAL: ka_1 := ka_7
             c->a[tidc][0] = c->anew[tidc][0]; c->a[tidc][1] = c->anew[tidc][1];
             c->ka[0][tidc][0] = c->ka[6][tidc][0]; c->ka[0][tidc][1] = c->ka[6][tidc][1];

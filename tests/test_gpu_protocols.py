@@ -268,3 +268,66 @@ def test_cooperativity_splitting_on_the_device(api, path):
     assert np.abs(np.sort_complex(om2) - exact).max() / TWO_PI < 20e3
     # resolved: the gap exceeds the common linewidth (kappa + gamma_m)/2 of the two hybrid lines
     assert np.abs(-om2.imag / TWO_PI / 1e6 - 0.5 * (kM + gm)).max() < 0.05 and gap > 0.5 * (kM + gm)
+
+
+@pytest.mark.parametrize("path", ["tma", "generic", "block"])
+def test_neel_vector_spectroscopy_on_the_device(api, path):
+    """PAPER.md:335-345 (Sim 7): the antiferromagnet's resonance read from the Neel vector l = (m_1 - m_2)/2.  The Fourier
+    sums of the two sublattice averages mu_s = <m_s,x> - i <m_s,y> are accumulated on the device (cav_set_spectrum); they are
+    linear, so the Neel spectrum is (X_mu1 - X_mu2)/2.  It equals the DFT of the same run's trace, and it peaks at the line
+    a damped-exponential fit of the Neel trace finds (the AFMR mode, Eq. 15-16, pulled by the cavity)."""
+    from observables import fit_exponentials, dominant
+    from oracle import dft
+    w = W.cfg4(nx=64, ny=8, nz=4) if path != "block" else W.cfg4(nx=8, ny=4, nz=4)
+    N = w.n_modes
+    t_end, sdt = 0.1e-9, 0.5e-12
+    cap = int(round(t_end / sdt))
+    c = 1 + 4 * N
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_trace(sim.h, sdt, cap)
+        tr0 = None
+        # a first short run fixes the frequency window around the Neel line, the second one accumulates the sums
+        api.cav_run(sim.h, t_end, tol=1e-7)
+        tr0 = api.cav_get_trace(sim.h)
+    neel = 0.5 * ((tr0[:, c] - tr0[:, c + 3]) - 1j * (tr0[:, c + 1] - tr0[:, c + 4]))
+    om, amp = fit_exponentials(neel, sdt, 4)
+    line = dominant(om, amp, 1)[0][0].real                      # signed: the Neel mode of this handedness
+    K = 201
+    lo, hi = line - TWO_PI * 40e9, line + TWO_PI * 40e9
+    wk = np.linspace(lo, hi, K)
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_trace(sim.h, sdt, cap)
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+        api.cav_run(sim.h, t_end, tol=1e-7)
+        tr = api.cav_get_trace(sim.h)
+        X, ns = api.cav_get_spectrum(sim.h, K, N)
+    assert ns == cap and X.shape == (K, 2 * N + 2)
+    Xl = 0.5 * (X[:, 2 * N] - X[:, 2 * N + 1])
+    ref = dft(tr[:, 0], 0.5 * ((tr[:, c] - tr[:, c + 3]) - 1j * (tr[:, c + 1] - tr[:, c + 4])), wk)
+    assert np.abs(Xl - ref).max() <= 1e-12 * np.abs(ref).max() * cap
+    peak = wk[np.abs(Xl).argmax()]
+    assert abs(peak - line) <= 1.5 * (wk[1] - wk[0]) + TWO_PI / t_end * 0.6      # within the resolution 1/T of a 0.1 ns record
+
+
+@pytest.mark.parametrize("path", ["block", "generic"])
+def test_kittel_line_from_the_device_spectrum_without_modes(api, path):
+    """No cavity at all (N = 0): the Fourier sums of mu = <m_x> - i <m_y> alone.  A tilted macrospin precesses at
+    gamma B0 (Eq. 9): the device spectrum peaks there and equals the DFT of the same run's trace."""
+    from oracle import dft
+    f0 = 10.0
+    w = W.macrospin(f0, [], [], [], alpha=0.0, tilt=0.05, n=2)
+    T, sdt = 4e-9, 10e-12
+    cap = int(round(T / sdt))
+    K = 161
+    lo, hi = TWO_PI * 9.6e9, TWO_PI * 10.4e9
+    wk = np.linspace(lo, hi, K)
+    with open_sim(api, w, "f64", path) as sim:
+        api.cav_set_trace(sim.h, sdt, cap)
+        api.cav_set_spectrum(sim.h, K, lo, hi)
+        api.cav_run(sim.h, T, tol=1e-9)
+        tr = api.cav_get_trace(sim.h)
+        X, ns = api.cav_get_spectrum(sim.h, K, 0)
+    assert ns == cap and X.shape == (K, 1) and tr.shape == (cap, 4)
+    ref = dft(tr[:, 0], tr[:, 1] - 1j * tr[:, 2], wk)
+    assert np.abs(X[:, 0] - ref).max() <= 1e-12 * np.abs(ref).max() * cap
+    assert abs(wk[np.abs(X[:, 0]).argmax()] / TWO_PI - f0 * 1e9) <= 5e6 + 1e-3      # one 5 MHz bin

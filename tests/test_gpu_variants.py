@@ -240,6 +240,9 @@ def test_spectrum_equals_dft_of_the_trace(api, path, adaptive):
         ref_S = dft(tr[:, 0], tr[:, 1 + 2 * N + 2 * n] + 1j * tr[:, 2 + 2 * N + 2 * n], wk)
         assert np.abs(X[:, n] - ref_a).max() <= 1e-12 * np.abs(ref_a).max() * cap
         assert np.abs(X[:, N + n] - ref_S).max() <= 1e-12 * np.abs(ref_S).max() * cap
+    assert X.shape == (K, 2 * N + 1)                                  # the last column: mu = <m_x> - i <m_y>
+    ref_m = dft(tr[:, 0], tr[:, 1 + 4 * N] - 1j * tr[:, 2 + 4 * N], wk)
+    assert np.abs(X[:, 2 * N] - ref_m).max() <= 1e-12 * np.abs(ref_m).max() * cap
     if not adaptive:        # and against the oracle's own trajectory
         ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=0.1e-12, max_steps=cap * 10, sample_dt=sdt, trace_cap=cap)
         for n in range(N):
@@ -267,6 +270,8 @@ def test_spectrum_batch_and_block(api):
         for n in range(N):
             ref_a = dft(tr[:, 0], tr[:, 1 + 2 * n] + 1j * tr[:, 2 + 2 * n], wk)
             assert np.abs(X[r, :, n] - ref_a).max() <= 1e-12 * np.abs(ref_a).max() * 40
+        ref_m = dft(tr[:, 0], tr[:, 1 + 4 * N] - 1j * tr[:, 2 + 4 * N], wk)
+        assert np.abs(X[r, :, 2 * N] - ref_m).max() <= 1e-12 * np.abs(ref_m).max() * 40
     assert np.abs(X[0] - X[2]).max() > 1e-3 * np.abs(X[0]).max()
     with open_sim(api, w, "f64", "block") as sim:
         api.cav_set_trace(sim.h, 1e-12, 40)
