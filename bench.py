@@ -353,7 +353,7 @@ def timed_steps(api, torch, h, stream, tol, steps, sampler=None, barrier=None):
     return ev0.elapsed_time(ev1), clocks
 
 
-E2E_STREAMS = 4     # independent simulations in flight in the end-to-end measurement (one host thread and one stream each)
+E2E_STREAMS = 8     # independent simulations in flight in the end-to-end measurement (one host thread and one stream each)
 
 
 def e2e_pipelined(api, torch, w, prec, tol, k, spinup, barrier, n_streams=E2E_STREAMS):
