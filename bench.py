@@ -588,7 +588,7 @@ def run_cuda(args):
 # ----------------------------------------------------------------------------------------
 # batched small-grid sweep: --workload cfg1_sweep
 # ----------------------------------------------------------------------------------------
-FLOP_PER_CELL_STAGE_BATCH = 150.0     # field 75 + LLG 30 + stage algebra ~40 + 4N, N = 1
+FLOP_PER_CELL_STAGE_BATCH = 151.0     # measured: fp64 add + mul + 2 fma of k_batch per cell-stage (profiles/r2_batch_flops.md); the formulas give ~150
 
 
 def run_batch(args):
