@@ -425,17 +425,24 @@ const void* zconv_fn(int q) {
 //                          index in bit-reversed order (the z convolution works column by column and only needs to know
 //                          which frequency a row holds);
 //   inverse (INV = true):  in [planes][Py][NXH] (bit-reversed) -> transform back -> rows y < ny -> out [planes][ny][NXH].
-// Same passes as the z convolution (two radix-2 levels per pass on four values in registers, a lone span-1 level where q
-// is odd; the first pass reads global memory, the last one writes it), one component per column.
+// Up to three radix-2 levels per pass on eight values in registers (Py = 512: three passes, two shared-memory exchanges);
+// the first pass reads global memory, the last one writes it; one component per column.
 constexpr int kYTile = 16;           // columns (plane, kx) per block
-__host__ __device__ constexpr int ycol_rows(int q) { return (1 << q) / 4 < 1 ? 1 : ((1 << q) / 4 > 32 ? 32 : (1 << q) / 4); }   // blockDim.y
+// radix-2 levels per pass, in forward order: threes (eight values in registers), a four is two twos: q = 9 is three passes
+__host__ __device__ constexpr int ypass_count(int q) { int n = 0; while (q > 0) { q -= (q >= 3 && q != 4) ? 3 : (q >= 2 ? 2 : 1); ++n; } return n; }
+__host__ __device__ constexpr int ypass_levels(int q, int i) {
+    int L = 0;
+    for (int k = 0; k <= i; ++k) { L = (q >= 3 && q != 4) ? 3 : (q >= 2 ? 2 : 1); q -= L; }
+    return L;
+}
+__host__ __device__ constexpr int ypass_done(int q, int i) { int d = 0; for (int k = 0; k < i; ++k) d += ypass_levels(q, k); return d; }   // levels before pass i
+__host__ __device__ constexpr int ycol_rows(int q) { return (1 << q) / 8 < 1 ? 1 : ((1 << q) / 8 > 32 ? 32 : (1 << q) / 8); }   // blockDim.y
 
 template <typename T, typename C, int q, bool INV>
 __global__ void __launch_bounds__(ycol_rows(q) * kYTile)
 k_demag_ycol(const C* __restrict__ in, C* __restrict__ out, int n_valid, int NXH, long long ncols) {
     constexpr int P = 1 << q, NJ = ycol_rows(q), TK = kYTile;
-    constexpr int ngrp = (q + 1) / 2;
-    constexpr bool odd = (q & 1) != 0;
+    constexpr int NP = ypass_count(q);
     extern __shared__ __align__(16) unsigned char ysm[];
     C* const sm = reinterpret_cast<C*>(ysm);                    // [P][TK]
     C* const tw = sm + P * TK;                                  // exp(-2 pi i j / P), j < P/2
@@ -453,113 +460,62 @@ k_demag_ycol(const C* __restrict__ in, C* __restrict__ out, int n_valid, int NXH
     }
     __syncthreads();
     C zero; zero.x = (T)0; zero.y = (T)0;
-    if constexpr (!INV) {
-        auto forward = [&](auto G) {
-            constexpr int g = decltype(G)::value;
-            constexpr bool single = odd && g == ngrp - 1;
-            constexpr int h = (P / 2) >> (2 * g);
-            constexpr bool first = g == 0, last = g == ngrp - 1;
-            if constexpr (!single) {
-                constexpr int hh = h / 2, s1 = P / (2 * h);
+    // One pass: L radix-2 levels on n = 2^L values held in registers.
+    //   forward (decimation in frequency): spans h, h/2, ..; the values sit hq = h >> (L-1) apart
+    //   inverse (decimation in time):      spans s0, 2 s0, ..; the values sit s0 apart
+    auto pass = [&](auto I) {
+        constexpr int i = decltype(I)::value;                    // pass index in execution order
+        constexpr int fi = INV ? NP - 1 - i : i;                 // the forward pass it mirrors
+        constexpr int L = ypass_levels(q, fi), n = 1 << L;
+        constexpr int h = (P / 2) >> ypass_done(q, fi);          // top span of the forward pass
+        constexpr int hq = h >> (L - 1);                         // distance of the values = lowest span
+        constexpr bool first = i == 0, last = i == NP - 1;
 #pragma unroll
-                for (int w0 = 0; w0 < P / 4; w0 += NJ) {
-                    const int w = w0 + j;
-                    const int r = w % hh, p0 = (w / hh) * 2 * h + r;
-                    const int pos[4] = {p0, p0 + hh, p0 + h, p0 + h + hh};
-                    const C t1a = tw[r * s1], t1b = tw[(r + hh) * s1], t2 = tw[r * 2 * s1];
-                    C v[4];
+        for (int w0 = 0; w0 < P / n; w0 += NJ) {
+            const int w = w0 + j;
+            if (P / n < NJ && w >= P / n) break;
+            const int r = w % hq, p0 = (w / hq) * (hq * n) + r;
+            C v[n];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        if constexpr (first) v[e] = (e < 2 && live && pos[e] < n_valid) ? ci[(long long)pos[e] * NXH] : zero;   // pos >= P/2 >= n_valid: padding
-                        else v[e] = sm[pos[e] * TK + k];
-                    }
-                    if constexpr (first) dif4_padded(v, t1a, t1b, t2);
-                    else dif4(v, t1a, t1b, t2);
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        if constexpr (last) { if (live) co[(long long)pos[e] * NXH] = v[e]; }
-                        else sm[pos[e] * TK + k] = v[e];
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int w0 = 0; w0 < P / 2; w0 += NJ) {
-                    const int w = w0 + j;
-                    const int pos[2] = {2 * w, 2 * w + 1};
-                    C v[2];
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        if constexpr (first) v[e] = (live && pos[e] < n_valid) ? ci[(long long)pos[e] * NXH] : zero;
-                        else v[e] = sm[pos[e] * TK + k];
-                    }
-                    const C a = v[0], b = v[1];
-                    v[0] = c_add(a, b); v[1] = c_sub(a, b);
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) { if (live) co[(long long)pos[e] * NXH] = v[e]; }      // the lone level is the last one
-                }
+            for (int e = 0; e < n; ++e) {
+                const int pos = p0 + e * hq;
+                if constexpr (first) v[e] = (live && (INV || pos < n_valid)) ? ci[(long long)pos * NXH] : zero;    // forward: zero padding beyond n_valid
+                else v[e] = sm[pos * TK + k];
             }
-            if constexpr (!last) __syncthreads();
-        };
-        using std::integral_constant;
-        forward(integral_constant<int, 0>{});
-        if constexpr (ngrp > 1) forward(integral_constant<int, 1>{});
-        if constexpr (ngrp > 2) forward(integral_constant<int, 2>{});
-        if constexpr (ngrp > 3) forward(integral_constant<int, 3>{});
-        if constexpr (ngrp > 4) forward(integral_constant<int, 4>{});
-    } else {
-        auto inverse = [&](auto G) {
-            constexpr int g = decltype(G)::value;
-            constexpr bool single = odd && g == 0;
-            constexpr bool first = g == 0, last = g == ngrp - 1;
-            if constexpr (single) {
 #pragma unroll
-                for (int w0 = 0; w0 < P / 2; w0 += NJ) {
-                    const int w = w0 + j;
-                    const int pos[2] = {2 * w, 2 * w + 1};
-                    C v[2];
+            for (int l = 0; l < L; ++l) {
+                constexpr int dummy = 0; (void)dummy;
+                const int d = INV ? (1 << l) : (1 << (L - 1 - l));          // local distance of a pair
+                const int span = INV ? (hq << l) : (h >> l);
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) v[e] = live ? ci[(long long)pos[e] * NXH] : zero;      // the lone level is the first one
-                    const C a = v[0], b = v[1];
-                    v[0] = c_add(a, b); v[1] = c_sub(a, b);
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        if constexpr (last) { if (live && pos[e] < n_valid) co[(long long)pos[e] * NXH] = v[e]; }
-                        else sm[pos[e] * TK + k] = v[e];
-                    }
-                }
-            } else {
-                constexpr int h = odd ? (2 << (2 * (g > 0 ? g - 1 : 0))) : (1 << (2 * g));
-                constexpr int s1 = P / (2 * h), s2 = P / (4 * h);
-#pragma unroll
-                for (int w0 = 0; w0 < P / 4; w0 += NJ) {
-                    const int w = w0 + j;
-                    const int r = w % h, p0 = (w / h) * 4 * h + r;
-                    const int pos[4] = {p0, p0 + h, p0 + 2 * h, p0 + 3 * h};
-                    const C t1 = tw[r * s1], t2a = tw[r * s2], t2b = tw[(r + h) * s2];
-                    C v[4];
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        if constexpr (first) v[e] = live ? ci[(long long)pos[e] * NXH] : zero;
-                        else v[e] = sm[pos[e] * TK + k];
-                    }
-                    if constexpr (last) dit4_padded(v, t1, t2a, t2b);       // only the rows below P/2 are wanted
-                    else dit4(v, t1, t2a, t2b);
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        if constexpr (last) { if (e < 2 && live && pos[e] < n_valid) co[(long long)pos[e] * NXH] = v[e]; }
-                        else sm[pos[e] * TK + k] = v[e];
+                for (int e = 0; e < n; ++e) {
+                    if (e & d) continue;
+                    const C t = tw[(r + (e % d) * hq) * (P / (2 * span))];
+                    if constexpr (!INV) {
+                        const C lo = v[e], hi = v[e + d];
+                        v[e] = c_add(lo, hi);
+                        v[e + d] = c_mul(c_sub(lo, hi), t);
+                    } else {
+                        const C x = c_mulc(v[e + d], t), lo = v[e];
+                        v[e] = c_add(lo, x);
+                        v[e + d] = c_sub(lo, x);
                     }
                 }
             }
-            if constexpr (!last) __syncthreads();
-        };
-        using std::integral_constant;
-        inverse(integral_constant<int, 0>{});
-        if constexpr (ngrp > 1) inverse(integral_constant<int, 1>{});
-        if constexpr (ngrp > 2) inverse(integral_constant<int, 2>{});
-        if constexpr (ngrp > 3) inverse(integral_constant<int, 3>{});
-        if constexpr (ngrp > 4) inverse(integral_constant<int, 4>{});
-    }
+#pragma unroll
+            for (int e = 0; e < n; ++e) {
+                const int pos = p0 + e * hq;
+                if constexpr (last) { if (live && (!INV || pos < n_valid)) co[(long long)pos * NXH] = v[e]; }      // inverse: keep the rows below n_valid
+                else sm[pos * TK + k] = v[e];
+            }
+        }
+        if constexpr (!last) __syncthreads();
+    };
+    using std::integral_constant;
+    pass(integral_constant<int, 0>{});
+    if constexpr (NP > 1) pass(integral_constant<int, 1>{});
+    if constexpr (NP > 2) pass(integral_constant<int, 2>{});
+    if constexpr (NP > 3) pass(integral_constant<int, 3>{});
 }
 
 constexpr int kYColMaxQ = 10;        // Py <= 1024: [Py][16] complex columns fit the shared memory of a block in both precisions
