@@ -539,28 +539,45 @@ const void* ycol_fn(int q) {
 
 // The state stage `stage` is evaluated at, summed over the sublattices, into the zero-padded array [3][Pz][Py][Px]
 // (the pad region is zeroed once and never written).  Buffer indices and h as the stage kernel reads them.
-template <typename T>
-__global__ void k_demag_gather(const StageArgs A, int stage, int n_sub, T* pad, int Px, int Py, int Pz) {
+constexpr int kGatherRows = 4;       // rows per thread of the gather / scatter kernels (independent loads in flight)
+
+template <typename T, int NSUB>
+__global__ void k_demag_gather(const StageArgs A, int stage, T* __restrict__ pad, int Px, int Py, int Pz) {
     const Ctrl* c = A.ctrl;
     if (stage == 1 ? c->k1_valid : c->done) return;
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, z = blockIdx.z;     // grid: (ceil(nx / block), ny, nz)
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, yb = blockIdx.y * kGatherRows, z = blockIdx.z;   // grid: (ceil(nx / block), ceil(ny / 4), nz)
     if (x >= A.nx) return;
     const long long nc = A.nc;
-    const long long i = ((long long)z * A.ny + y) * A.nx + x;
     const int ycur = c->ycur, k1slot = c->k1slot;
-    const T* y0 = (const T*)(ycur ? A.Y[1] : A.Y[0]);
-    const T* ynew = (const T*)(ycur ? A.Y[0] : A.Y[1]);
-    const T* k1 = (const T*)(k1slot ? A.K[6] : A.K[0]);
-    const T* ms = stage == 1 ? y0 : stage == 7 ? ynew : (stage == 3 || stage == 5) ? (const T*)A.MS[0] : (const T*)A.MS[1];
+    const T* __restrict__ y0 = (const T*)(ycur ? A.Y[1] : A.Y[0]);
+    const T* __restrict__ ynew = (const T*)(ycur ? A.Y[0] : A.Y[1]);
+    const T* __restrict__ k1 = (const T*)(k1slot ? A.K[6] : A.K[0]);
+    const T* __restrict__ ms = stage == 1 ? y0 : stage == 7 ? ynew : (stage == 3 || stage == 5) ? (const T*)A.MS[0] : (const T*)A.MS[1];
     const T ha21 = (T)c->h * (T)kA[1][0];
-    const long long o = ((long long)z * Py + y) * Px + x, pvol = (long long)Px * Py * Pz;
-    for (int comp = 0; comp < 3; ++comp) {
-        T v = (T)0;
-        for (int s = 0; s < n_sub; ++s) {
-            const long long off = (long long)(s * 3 + comp) * nc + i;
-            v += stage == 2 ? y0[off] + ha21 * k1[off] : ms[off];
+    const long long pvol = (long long)Px * Py * Pz;
+    T v[kGatherRows][3];
+#pragma unroll
+    for (int r = 0; r < kGatherRows; ++r) {
+        const int y = yb + r;
+        const long long i = ((long long)z * A.ny + (y < A.ny ? y : A.ny - 1)) * A.nx + x;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+            T acc = (T)0;
+#pragma unroll
+            for (int s = 0; s < NSUB; ++s) {             // (compile-time count: every load of the thread is independent)
+                const long long off = (long long)(s * 3 + comp) * nc + i;
+                acc += stage == 2 ? y0[off] + ha21 * k1[off] : ms[off];
+            }
+            v[r][comp] = acc;
         }
-        pad[comp * pvol + o] = v;
+    }
+#pragma unroll
+    for (int r = 0; r < kGatherRows; ++r) {
+        const int y = yb + r;
+        if (y >= A.ny) break;
+        const long long o = ((long long)z * Py + y) * Px + x;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) pad[comp * pvol + o] = v[r][comp];
     }
 }
 
@@ -579,12 +596,26 @@ __global__ void k_demag_product(C* F, const C* K, long long nf) {
 }
 
 template <typename T>
-__global__ void k_demag_scatter(const T* conv, T* bdem, int nx, int ny, long long nc, int Px, int Py, int Pz) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y, z = blockIdx.z;     // grid: (ceil(nx / block), ny, nz)
+__global__ void k_demag_scatter(const T* __restrict__ conv, T* __restrict__ bdem, int nx, int ny, long long nc, int Px, int Py, int Pz) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, yb = blockIdx.y * kGatherRows, z = blockIdx.z;   // grid: (ceil(nx / block), ceil(ny / 4), nz)
     if (x >= nx) return;
-    const long long i = ((long long)z * ny + y) * nx + x;
-    const long long o = ((long long)z * Py + y) * Px + x, pvol = (long long)Px * Py * Pz;
-    for (int comp = 0; comp < 3; ++comp) bdem[comp * nc + i] = conv[comp * pvol + o];
+    const long long pvol = (long long)Px * Py * Pz;
+    T v[kGatherRows][3];
+#pragma unroll
+    for (int r = 0; r < kGatherRows; ++r) {
+        const int y = yb + r < ny ? yb + r : ny - 1;
+        const long long o = ((long long)z * Py + y) * Px + x;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) v[r][comp] = conv[comp * pvol + o];
+    }
+#pragma unroll
+    for (int r = 0; r < kGatherRows; ++r) {
+        const int y = yb + r;
+        if (y >= ny) break;
+        const long long i = ((long long)z * ny + y) * nx + x;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) bdem[comp * nc + i] = v[r][comp];
+    }
 }
 
 }  // namespace
@@ -718,7 +749,7 @@ int demag_apply(DemagPlan* p, const StageArgs& A, int stage, void* bdem, cudaStr
     const int tb = 256;
     const unsigned gf = (unsigned)((p->nf + tb - 1) / tb);
     const int gtb = A.nx >= 256 ? 256 : (A.nx >= 128 ? 128 : (A.nx >= 64 ? 64 : 32));
-    const dim3 gc((unsigned)((A.nx + gtb - 1) / gtb), (unsigned)A.ny, (unsigned)p->nz);
+    const dim3 gc((unsigned)((A.nx + gtb - 1) / gtb), (unsigned)((A.ny + kGatherRows - 1) / kGatherRows), (unsigned)p->nz);
     const int NXH = p->Px / 2 + 1;
     const int tk = p->f32 ? ZTile<float>::value : ZTile<double>::value;
     const dim3 zgrid((unsigned)(((long long)p->Py * NXH + tk - 1) / tk));
@@ -739,7 +770,8 @@ int demag_apply(DemagPlan* p, const StageArgs& A, int stage, void* bdem, cudaStr
     auto run = [&](auto tag_real, auto tag_cplx) -> int {
         using R = decltype(tag_real);
         using Cx = decltype(tag_cplx);
-        k_demag_gather<R><<<gc, gtb, 0, stream>>>(A, stage, p->n_sub, (R*)p->pad, p->Px, p->prows, p->zplanes);
+        if (p->n_sub == 1) k_demag_gather<R, 1><<<gc, gtb, 0, stream>>>(A, stage, (R*)p->pad, p->Px, p->prows, p->zplanes);
+        else k_demag_gather<R, 2><<<gc, gtb, 0, stream>>>(A, stage, (R*)p->pad, p->Px, p->prows, p->zplanes);
         if constexpr (sizeof(R) == 4) { if (f.ExecR2C(p->fwd, (cufftReal*)p->pad, (cufftComplex*)xspec) != CUFFT_SUCCESS) return CAV_E_CUDA; }
         else { if (f.ExecD2Z(p->fwd, (cufftDoubleReal*)p->pad, (cufftDoubleComplex*)xspec) != CUFFT_SUCCESS) return CAV_E_CUDA; }
         if (ycol && cudaLaunchKernel(p->yfwd, ygrid, yblock, yfargs, p->ysmem, stream) != cudaSuccess) return CAV_E_CUDA;
