@@ -143,84 +143,74 @@ __global__ void k_store_khat_real(const cufftDoubleComplex* src, T* dst, int NZH
 // columns (ky, kx) per block of the z convolution: a warp per worker row in fp32 (positions and twiddles are warp-uniform)
 template <typename T> struct ZTile { static constexpr int value = sizeof(T) == 4 ? 32 : 16; };
 
-// ---- radix-2 levels of the z transform on values held in registers (W = exp(-2 pi i / Pz), tw[j] = W^j) ----
+// ---- complex arithmetic and the radix-2 levels of a pass, on values held in registers ----
 template <typename C> __device__ __forceinline__ C c_add(const C& a, const C& b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
 template <typename C> __device__ __forceinline__ C c_sub(const C& a, const C& b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
 // fp32: a complex number is one 64-bit register pair, and sm_100 adds / multiplies both halves in one instruction
-// (FADD2 / FFMA2): half the issue slots of the butterflies, which is what bounds the z convolution
+// (FADD2 / FFMA2): half the issue slots of the butterflies' additions
 template <> __device__ __forceinline__ float2 c_add<float2>(const float2& a, const float2& b) { return __fadd2_rn(a, b); }
 template <> __device__ __forceinline__ float2 c_sub<float2>(const float2& a, const float2& b) { return __ffma2_rn(b, make_float2(-1.0f, -1.0f), a); }
 template <typename C> __device__ __forceinline__ C c_mul(const C& a, const C& b) { C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
 template <typename C> __device__ __forceinline__ C c_mulc(const C& a, const C& b) { C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r; }   // a conj(b)
-// decimation in frequency, spans h and h/2, on positions p0, p0 + h/2, p0 + h, p0 + 3h/2 (v[0..3]); t1a, t1b: span-h
-// twiddles of the two pairs, t2: span-h/2 twiddle
-template <typename C> __device__ __forceinline__ void dif4(C* v, const C& t1a, const C& t1b, const C& t2) {
-    const C a0 = c_add(v[0], v[2]), a2 = c_mul(c_sub(v[0], v[2]), t1a);
-    const C a1 = c_add(v[1], v[3]), a3 = c_mul(c_sub(v[1], v[3]), t1b);
-    v[0] = c_add(a0, a1); v[1] = c_mul(c_sub(a0, a1), t2);
-    v[2] = c_add(a2, a3); v[3] = c_mul(c_sub(a2, a3), t2);
-}
-// decimation in time with conjugate twiddles, spans h and 2h, on positions p0, p0 + h, p0 + 2h, p0 + 3h
-template <typename C> __device__ __forceinline__ void dit4(C* v, const C& t1, const C& t2a, const C& t2b) {
-    const C b1 = c_mulc(v[1], t1), b3 = c_mulc(v[3], t1);
-    const C a0 = c_add(v[0], b1), a1 = c_sub(v[0], b1);
-    const C a2 = c_mulc(c_add(v[2], b3), t2a), a3 = c_mulc(c_sub(v[2], b3), t2b);
-    v[0] = c_add(a0, a2); v[2] = c_sub(a0, a2);
-    v[1] = c_add(a1, a3); v[3] = c_sub(a1, a3);
-}
 
-// the middle pass (forward spans 2 and 1, product by the caller in between, inverse spans 1 and 2) has only the
-// twiddles 1 and W^(Pz/4) = -i: no complex multiplications
-template <typename C> __device__ __forceinline__ C c_mul_mi(const C& a) { C r; r.x = a.y; r.y = -a.x; return r; }    // a (-i)
-template <typename C> __device__ __forceinline__ C c_mul_pi(const C& a) { C r; r.x = -a.y; r.y = a.x; return r; }    // a (+i) = a conj(-i)
-template <typename C> __device__ __forceinline__ void dif4_mid(C* v) {
-    const C a0 = c_add(v[0], v[2]), a2 = c_sub(v[0], v[2]);
-    const C a1 = c_add(v[1], v[3]), a3 = c_mul_mi(c_sub(v[1], v[3]));
-    v[0] = c_add(a0, a1); v[1] = c_sub(a0, a1);
-    v[2] = c_add(a2, a3); v[3] = c_sub(a2, a3);
+// A transform of length P = 2^q runs in passes of up to three radix-2 levels on 2^L values held in registers, with a
+// shared-memory exchange between passes.  Forward: decimation in frequency (natural order in, bit-reversed out), spans
+// P/2, P/4, .. 1; inverse: decimation in time with conjugate twiddles (bit-reversed in, natural out), the same passes
+// mirrored.  Levels per pass, in forward order: threes, a four is two twos (q = 9: 3 3 3, q = 6: 3 3, q = 7: 3 2 2).
+__host__ __device__ constexpr int fft_pass_count(int q) { int n = 0; while (q > 0) { q -= (q >= 3 && q != 4) ? 3 : (q >= 2 ? 2 : 1); ++n; } return n; }
+__host__ __device__ constexpr int fft_pass_levels(int q, int i) {
+    int L = 0;
+    for (int k = 0; k <= i; ++k) { L = (q >= 3 && q != 4) ? 3 : (q >= 2 ? 2 : 1); q -= L; }
+    return L;
 }
-template <typename C> __device__ __forceinline__ void dit4_mid(C* v) {
-    const C a0 = c_add(v[0], v[1]), a1 = c_sub(v[0], v[1]);
-    const C a2 = c_add(v[2], v[3]), a3 = c_mul_pi(c_sub(v[2], v[3]));
-    v[0] = c_add(a0, a2); v[2] = c_sub(a0, a2);
-    v[1] = c_add(a1, a3); v[3] = c_sub(a1, a3);
-}
-// first forward pass of a padded column: v[2] = v[3] = 0 (positions >= Pz/2 >= nz)
-template <typename C> __device__ __forceinline__ void dif4_padded(C* v, const C& t1a, const C& t1b, const C& t2) {
-    const C a2 = c_mul(v[0], t1a), a3 = c_mul(v[1], t1b);
-    const C a0 = v[0], a1 = v[1];
-    v[0] = c_add(a0, a1); v[1] = c_mul(c_sub(a0, a1), t2);
-    v[2] = c_add(a2, a3); v[3] = c_mul(c_sub(a2, a3), t2);
-}
-// last inverse pass of a padded column: only the positions below Pz/2 (v[0], v[1]) are wanted
-template <typename C> __device__ __forceinline__ void dit4_padded(C* v, const C& t1, const C& t2a, const C& t2b) {
-    const C b1 = c_mulc(v[1], t1), b3 = c_mulc(v[3], t1);
-    const C a2 = c_mulc(c_add(v[2], b3), t2a), a3 = c_mulc(c_sub(v[2], b3), t2b);
-    const C x0 = v[0];
-    v[0] = c_add(c_add(x0, b1), a2);
-    v[1] = c_add(c_sub(x0, b1), a3);
+__host__ __device__ constexpr int fft_pass_done(int q, int i) { int d = 0; for (int k = 0; k < i; ++k) d += fft_pass_levels(q, k); return d; }   // levels before pass i
+__host__ __device__ constexpr int fft_rows(int q) { return (1 << q) / 8 < 1 ? 1 : ((1 << q) / 8 > 32 ? 32 : (1 << q) / 8); }   // blockDim.y: groups of a pass in flight
+
+// The L levels of one pass on v[c][e], e < 2^L: the values of a group sit HQ positions apart (positions p0 + e HQ,
+// p0 = (w / HQ) (HQ 2^L) + r, r = w % HQ for group w), level l pairs values d apart (forward d = 2^(L-1-l), inverse 2^l)
+// inside a span of HQ d positions; tw[t] = exp(-2 pi i t / P).
+template <typename C, int P, int NC, int L, int HQ, bool INV>
+__device__ __forceinline__ void fft_levels(C (&v)[NC][1 << L], const C* __restrict__ tw, const int r) {
+    constexpr int n = 1 << L;
+#pragma unroll
+    for (int l = 0; l < L; ++l) {
+        const int d = INV ? (1 << l) : (1 << (L - 1 - l));
+#pragma unroll
+        for (int e = 0; e < n; ++e) {
+            if (e & d) continue;
+            const C t = tw[(r + (e % d) * HQ) * (P / (2 * HQ * d))];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                if constexpr (!INV) {
+                    const C lo = v[c][e], hi = v[c][e + d];
+                    v[c][e] = c_add(lo, hi);
+                    v[c][e + d] = c_mul(c_sub(lo, hi), t);
+                } else {
+                    const C x = c_mulc(v[c][e + d], t), lo = v[c][e];
+                    v[c][e] = c_add(lo, x);
+                    v[c][e + d] = c_sub(lo, x);
+                }
+            }
+        }
+    }
 }
 
 // One block: TK consecutive columns (ky, kx) of the half-spectrum, the three field components, the whole z column.
 //   F [3][nz][Py][NXH] complex (in place), K [6][Pz/2+1][Py/2+1][NXH] real, Pz = 2^q >= 2 nz - 1 (q = 0: no z transform)
-// Forward: decimation in frequency (natural order in, bit-reversed out); the product is pointwise, so it is taken at the
-// bit-reversed positions; inverse: decimation in time (bit-reversed in, natural out), unnormalised (1/(Px Py Pz) is
-// folded into K).  A pass does two radix-2 levels on four values per component held in registers (one level on two
-// values where q is odd).  The first pass reads global memory (zero beyond nz), the last one writes it (below nz only),
-// and the last forward pass, the product and the first inverse pass work on the same positions and are one pass:
-// ceil(q/2) * 2 - 1 passes with a shared-memory exchange between them.
-__host__ __device__ constexpr int zconv_rows(int q) { return (1 << q) / 4 < 1 ? 1 : ((1 << q) / 4 > 32 ? 32 : (1 << q) / 4); }   // blockDim.y
-__host__ __device__ constexpr int zconv_min_blocks(int q, int tk, int tsize) {           // registers: 64 (fp32) / 128 (fp64) per thread
-    const int b = 1024 / (zconv_rows(q) * tk) / (tsize == 4 ? 1 : 2);
-    return b < 1 ? 1 : (tsize == 8 && b > 4 ? 4 : b);
-}
+// The first forward pass reads global memory (zero beyond nz); the last forward pass leaves the bit-reversed spectrum of
+// its 2^L positions in registers, where it is multiplied by the tensor's transform (pointwise, so at the bit-reversed
+// positions) and taken through the first inverse pass - the same positions - at once; the last inverse pass writes the
+// planes below nz to global memory.  q = 6: three passes with two shared-memory exchanges.  The inverse is unnormalised
+// (1/(Px Py Pz) is folded into K).
+__host__ __device__ constexpr int zconv_rows(int q) { return fft_rows(q); }   // blockDim.y
 
 template <typename T, typename C, int q>
-__global__ void __launch_bounds__(zconv_rows(q) * ZTile<T>::value, zconv_min_blocks(q, ZTile<T>::value, (int)sizeof(T)))
+__global__ void __launch_bounds__(zconv_rows(q) * ZTile<T>::value)
 k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NXH, int qy_rev) {
     constexpr int Pz = 1 << q;
     constexpr int NJ = zconv_rows(q);
     constexpr int kZTile = ZTile<T>::value;
+    constexpr int NP = fft_pass_count(q);
     extern __shared__ __align__(16) unsigned char zsm[];
     C* const sm = reinterpret_cast<C*>(zsm);                    // [3][Pz][kZTile]
     C* const tw = sm + 3 * Pz * kZTile;                         // exp(-2 pi i j / Pz), j < Pz/2
@@ -243,7 +233,7 @@ k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NX
     constexpr int NZH = Pz / 2 + 1;
     const int NYH = Py / 2 + 1;
     const long long cst = (long long)NZH * NYH * NXH;
-    // the block's slice of the tensor's transform goes to shared memory asynchronously: it is needed two passes later
+    // the block's slice of the tensor's transform goes to shared memory asynchronously: it is needed after the forward passes
     if (live) {
         const T* const Kc = K + (long long)kys * NXH + kx;
         for (int t = j; t < 6 * NZH; t += NJ) {
@@ -255,7 +245,7 @@ k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NX
         }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
-    // G = Khat F at position pos of the (bit-reversed) spectrum, for the three components in f[0..2]
+    // G = Khat F at position pos of the (bit-reversed) spectrum, for the three components
     auto product = [&](int pos, C& fx, C& fy, C& fz) {
         const int kz = q > 0 ? (int)(__brev((unsigned)pos) >> ((32 - q) & 31)) : 0;
         const int kzs = kz <= Pz / 2 ? kz : Pz - kz;
@@ -279,129 +269,58 @@ k_demag_zconv(C* __restrict__ F, const T* __restrict__ K, int nz, int Py, int NX
             Fc[0] = fx; Fc[zs] = fy; Fc[2 * zs] = fz;
         }
     } else {
-    if constexpr (q <= 2) asm volatile("cp.async.wait_group 0;" ::: "memory");       // one pass: the product is in it
+    if constexpr (NP == 1) asm volatile("cp.async.wait_group 0;" ::: "memory");       // one pass: the product is in it
     __syncthreads();                                            // twiddles
-    constexpr int ngrp = (q + 1) / 2;                           // passes per direction
-    constexpr bool odd = (q & 1) != 0;
     const long long cz = (long long)nz * zs;                    // component stride
-    // ---------------- forward pass g (the last one goes on into the product and the first inverse pass)
-    auto forward = [&](auto G) {
-        constexpr int g = decltype(G)::value;
-        constexpr bool single = odd && g == ngrp - 1;           // the lone span-1 level
-        constexpr int h = (Pz / 2) >> (2 * g);                  // upper span of this pass
-        constexpr bool first = g == 0, mid = g == ngrp - 1;
-        constexpr bool last_too = mid && ngrp == 1;             // q <= 2: everything in registers
-        if constexpr (!single) {
-            constexpr int hh = h / 2, s1 = Pz / (2 * h);
+    // Step i of 2 NP - 1: forward passes 0 .. NP-2, the middle step (forward pass NP-1, product, inverse pass 0), inverse
+    // passes 1 .. NP-1 (inverse pass k mirrors forward pass NP-1-k: the same groups and positions)
+    auto step = [&](auto I) {
+        constexpr int i = decltype(I)::value;
+        constexpr bool mid = i == NP - 1, inv = i > NP - 1;
+        constexpr int fi = inv ? 2 * (NP - 1) - i : i;           // the forward pass whose groups this step works on
+        constexpr int L = fft_pass_levels(q, fi), n = 1 << L;
+        constexpr int HQ = ((Pz / 2) >> fft_pass_done(q, fi)) >> (L - 1);
+        constexpr bool first = i == 0, last = i == 2 * NP - 2;
 #pragma unroll
-            for (int w0 = 0; w0 < Pz / 4; w0 += NJ) {
-                const int w = w0 + j;
-                const int r = w % hh, p0 = (w / hh) * 2 * h + r;
-                const int pos[4] = {p0, p0 + hh, p0 + h, p0 + h + hh};
-                const C t1a = tw[r * s1], t1b = tw[(r + hh) * s1], t2 = tw[r * 2 * s1];
-                C v[3][4];
+        for (int w0 = 0; w0 < Pz / n; w0 += NJ) {
+            const int w = w0 + j;
+            if (Pz / n < NJ && w >= Pz / n) break;
+            const int r = w % HQ, p0 = (w / HQ) * (HQ * n) + r;
+            C v[3][n];
 #pragma unroll
-                for (int c = 0; c < 3; ++c)
+            for (int c = 0; c < 3; ++c)
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        if constexpr (first) v[c][e] = (e < 2 && live && pos[e] < nz) ? Fc[c * cz + pos[e] * zs] : zero;
-                        else v[c][e] = sm[(c * Pz + pos[e]) * kZTile + k];
-                    }
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    if constexpr (first) dif4_padded(v[c], t1a, t1b, t2);
-                    else if constexpr (mid) dif4_mid(v[c]);
-                    else dif4(v[c], t1a, t1b, t2);
+                for (int e = 0; e < n; ++e) {
+                    const int pos = p0 + e * HQ;
+                    if constexpr (first) v[c][e] = (live && pos < nz) ? Fc[c * cz + pos * zs] : zero;      // zero padding beyond nz
+                    else v[c][e] = sm[(c * Pz + pos) * kZTile + k];
                 }
-                if constexpr (mid) {                            // positions 4w .. 4w+3: product, then inverse spans 1 and 2
-                    if (live) {
-#pragma unroll
-                        for (int e = 0; e < 4; ++e) product(pos[e], v[0][e], v[1][e], v[2][e]);
-                    }
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) dit4_mid(v[c]);
-                }
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        if constexpr (last_too) { if (live && pos[e] < nz) Fc[c * cz + pos[e] * zs] = v[c][e]; }
-                        else sm[(c * Pz + pos[e]) * kZTile + k] = v[c][e];
-                    }
-            }
-        } else {                                                // span 1 alone (q odd): pairs 2w, 2w+1; then product and inverse span 1
-#pragma unroll
-            for (int w0 = 0; w0 < Pz / 2; w0 += NJ) {
-                const int w = w0 + j;
-                const int pos[2] = {2 * w, 2 * w + 1};
-                C v[3][2];
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        if constexpr (first) v[c][e] = (live && pos[e] < nz) ? Fc[c * cz + pos[e] * zs] : zero;
-                        else v[c][e] = sm[(c * Pz + pos[e]) * kZTile + k];
-                    }
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { const C a = v[c][0], b = v[c][1]; v[c][0] = c_add(a, b); v[c][1] = c_sub(a, b); }
+            if constexpr (!inv) fft_levels<C, Pz, 3, L, HQ, false>(v, tw, r);
+            if constexpr (mid) {
                 if (live) {
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) product(pos[e], v[0][e], v[1][e], v[2][e]);
+                    for (int e = 0; e < n; ++e) product(p0 + e * HQ, v[0][e], v[1][e], v[2][e]);
                 }
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { const C a = v[c][0], b = v[c][1]; v[c][0] = c_add(a, b); v[c][1] = c_sub(a, b); }
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        if constexpr (last_too) { if (live && pos[e] < nz) Fc[c * cz + pos[e] * zs] = v[c][e]; }
-                        else sm[(c * Pz + pos[e]) * kZTile + k] = v[c][e];
-                    }
             }
-        }
-        if constexpr (g == ngrp - 2) asm volatile("cp.async.wait_group 0;" ::: "memory");  // the next pass multiplies
-        if constexpr (!last_too) __syncthreads();
-    };
-    // ---------------- inverse pass g >= 1: spans (h, 2h), h = 4, 16, ... (q even) or 2, 8, ... (q odd)
-    auto inverse = [&](auto G) {
-        constexpr int g = decltype(G)::value;
-        constexpr int h = odd ? (2 << (2 * (g - 1))) : (1 << (2 * g));
-        constexpr int s1 = Pz / (2 * h), s2 = Pz / (4 * h);
-        constexpr bool last = g == ngrp - 1;
-#pragma unroll
-        for (int w0 = 0; w0 < Pz / 4; w0 += NJ) {
-            const int w = w0 + j;
-            const int r = w % h, p0 = (w / h) * 4 * h + r;
-            const int pos[4] = {p0, p0 + h, p0 + 2 * h, p0 + 3 * h};
-            const C t1 = tw[r * s1], t2a = tw[r * s2], t2b = tw[(r + h) * s2];
-            C v[3][4];
+            if constexpr (mid || inv) fft_levels<C, Pz, 3, L, HQ, true>(v, tw, r);
 #pragma unroll
             for (int c = 0; c < 3; ++c)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) v[c][e] = sm[(c * Pz + pos[e]) * kZTile + k];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                if constexpr (last) dit4_padded(v[c], t1, t2a, t2b);
-                else dit4(v[c], t1, t2a, t2b);
-            }
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    if constexpr (last) { if (e < 2 && live && pos[e] < nz) Fc[c * cz + pos[e] * zs] = v[c][e]; }
-                    else sm[(c * Pz + pos[e]) * kZTile + k] = v[c][e];
+                for (int e = 0; e < n; ++e) {
+                    const int pos = p0 + e * HQ;
+                    if constexpr (last) { if (live && pos < nz) Fc[c * cz + pos * zs] = v[c][e]; }         // keep the planes below nz
+                    else sm[(c * Pz + pos) * kZTile + k] = v[c][e];
                 }
         }
+        if constexpr (i == NP - 2) asm volatile("cp.async.wait_group 0;" ::: "memory");    // the next step multiplies
         if constexpr (!last) __syncthreads();
     };
     using std::integral_constant;
-    forward(integral_constant<int, 0>{});
-    if constexpr (ngrp > 1) forward(integral_constant<int, 1>{});
-    if constexpr (ngrp > 2) forward(integral_constant<int, 2>{});
-    if constexpr (ngrp > 3) forward(integral_constant<int, 3>{});
-    if constexpr (ngrp > 1) inverse(integral_constant<int, 1>{});
-    if constexpr (ngrp > 2) inverse(integral_constant<int, 2>{});
-    if constexpr (ngrp > 3) inverse(integral_constant<int, 3>{});
+    step(integral_constant<int, 0>{});
+    if constexpr (2 * NP - 1 > 1) step(integral_constant<int, 1>{});
+    if constexpr (2 * NP - 1 > 2) step(integral_constant<int, 2>{});
+    if constexpr (2 * NP - 1 > 3) step(integral_constant<int, 3>{});
+    if constexpr (2 * NP - 1 > 4) step(integral_constant<int, 4>{});
     }
 }
 
@@ -428,21 +347,13 @@ const void* zconv_fn(int q) {
 // Up to three radix-2 levels per pass on eight values in registers (Py = 512: three passes, two shared-memory exchanges);
 // the first pass reads global memory, the last one writes it; one component per column.
 constexpr int kYTile = 16;           // columns (plane, kx) per block
-// radix-2 levels per pass, in forward order: threes (eight values in registers), a four is two twos: q = 9 is three passes
-__host__ __device__ constexpr int ypass_count(int q) { int n = 0; while (q > 0) { q -= (q >= 3 && q != 4) ? 3 : (q >= 2 ? 2 : 1); ++n; } return n; }
-__host__ __device__ constexpr int ypass_levels(int q, int i) {
-    int L = 0;
-    for (int k = 0; k <= i; ++k) { L = (q >= 3 && q != 4) ? 3 : (q >= 2 ? 2 : 1); q -= L; }
-    return L;
-}
-__host__ __device__ constexpr int ypass_done(int q, int i) { int d = 0; for (int k = 0; k < i; ++k) d += ypass_levels(q, k); return d; }   // levels before pass i
-__host__ __device__ constexpr int ycol_rows(int q) { return (1 << q) / 8 < 1 ? 1 : ((1 << q) / 8 > 32 ? 32 : (1 << q) / 8); }   // blockDim.y
+__host__ __device__ constexpr int ycol_rows(int q) { return fft_rows(q); }   // blockDim.y
 
 template <typename T, typename C, int q, bool INV>
 __global__ void __launch_bounds__(ycol_rows(q) * kYTile)
 k_demag_ycol(const C* __restrict__ in, C* __restrict__ out, int n_valid, int NXH, long long ncols) {
     constexpr int P = 1 << q, NJ = ycol_rows(q), TK = kYTile;
-    constexpr int NP = ypass_count(q);
+    constexpr int NP = fft_pass_count(q);
     extern __shared__ __align__(16) unsigned char ysm[];
     C* const sm = reinterpret_cast<C*>(ysm);                    // [P][TK]
     C* const tw = sm + P * TK;                                  // exp(-2 pi i j / P), j < P/2
@@ -460,53 +371,30 @@ k_demag_ycol(const C* __restrict__ in, C* __restrict__ out, int n_valid, int NXH
     }
     __syncthreads();
     C zero; zero.x = (T)0; zero.y = (T)0;
-    // One pass: L radix-2 levels on n = 2^L values held in registers.
-    //   forward (decimation in frequency): spans h, h/2, ..; the values sit hq = h >> (L-1) apart
-    //   inverse (decimation in time):      spans s0, 2 s0, ..; the values sit s0 apart
     auto pass = [&](auto I) {
         constexpr int i = decltype(I)::value;                    // pass index in execution order
         constexpr int fi = INV ? NP - 1 - i : i;                 // the forward pass it mirrors
-        constexpr int L = ypass_levels(q, fi), n = 1 << L;
-        constexpr int h = (P / 2) >> ypass_done(q, fi);          // top span of the forward pass
-        constexpr int hq = h >> (L - 1);                         // distance of the values = lowest span
+        constexpr int L = fft_pass_levels(q, fi), n = 1 << L;
+        constexpr int HQ = ((P / 2) >> fft_pass_done(q, fi)) >> (L - 1);
         constexpr bool first = i == 0, last = i == NP - 1;
 #pragma unroll
         for (int w0 = 0; w0 < P / n; w0 += NJ) {
             const int w = w0 + j;
             if (P / n < NJ && w >= P / n) break;
-            const int r = w % hq, p0 = (w / hq) * (hq * n) + r;
-            C v[n];
+            const int r = w % HQ, p0 = (w / HQ) * (HQ * n) + r;
+            C v[1][n];
 #pragma unroll
             for (int e = 0; e < n; ++e) {
-                const int pos = p0 + e * hq;
-                if constexpr (first) v[e] = (live && (INV || pos < n_valid)) ? ci[(long long)pos * NXH] : zero;    // forward: zero padding beyond n_valid
-                else v[e] = sm[pos * TK + k];
+                const int pos = p0 + e * HQ;
+                if constexpr (first) v[0][e] = (live && (INV || pos < n_valid)) ? ci[(long long)pos * NXH] : zero;    // forward: zero padding beyond n_valid
+                else v[0][e] = sm[pos * TK + k];
             }
-#pragma unroll
-            for (int l = 0; l < L; ++l) {
-                constexpr int dummy = 0; (void)dummy;
-                const int d = INV ? (1 << l) : (1 << (L - 1 - l));          // local distance of a pair
-                const int span = INV ? (hq << l) : (h >> l);
-#pragma unroll
-                for (int e = 0; e < n; ++e) {
-                    if (e & d) continue;
-                    const C t = tw[(r + (e % d) * hq) * (P / (2 * span))];
-                    if constexpr (!INV) {
-                        const C lo = v[e], hi = v[e + d];
-                        v[e] = c_add(lo, hi);
-                        v[e + d] = c_mul(c_sub(lo, hi), t);
-                    } else {
-                        const C x = c_mulc(v[e + d], t), lo = v[e];
-                        v[e] = c_add(lo, x);
-                        v[e + d] = c_sub(lo, x);
-                    }
-                }
-            }
+            fft_levels<C, P, 1, L, HQ, INV>(v, tw, r);
 #pragma unroll
             for (int e = 0; e < n; ++e) {
-                const int pos = p0 + e * hq;
-                if constexpr (last) { if (live && (!INV || pos < n_valid)) co[(long long)pos * NXH] = v[e]; }      // inverse: keep the rows below n_valid
-                else sm[pos * TK + k] = v[e];
+                const int pos = p0 + e * HQ;
+                if constexpr (last) { if (live && (!INV || pos < n_valid)) co[(long long)pos * NXH] = v[0][e]; }      // inverse: keep the rows below n_valid
+                else sm[pos * TK + k] = v[0][e];
             }
         }
         if constexpr (!last) __syncthreads();
