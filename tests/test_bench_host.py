@@ -75,6 +75,20 @@ def test_algorithmic_bytes_match_design_table():
     assert bench.algorithmic_bytes_per_cell_step(2, 1, 4) == 492        # cfg2 fp32: 82
 
 
+def test_dipolar_chain_byte_count_matches_design():
+    """859 MB for the FFT-convolution chain of one evaluation on CFG3 in fp32 (gather 126, R2C 202, z
+    convolution with the tensor octant 255, C2R 202, scatter 50, the field read by the stage kernel 25), counted from the
+    array sizes - a fixed yardstick that does not follow the implementation."""
+    w, prec = bench.make_workload("cfg3_demag")
+    b = bench.demag_bytes_per_evaluation(w, 4)
+    nc, real2, cplx2 = 256 * 256 * 32, 512 * 512 * 32, 32 * 512 * 257
+    octant = 6 * 33 * 257 * 257
+    assert b == 4 * ((3 * nc + 3 * real2) + (3 * real2 + 6 * cplx2) + (12 * cplx2 + octant) + (6 * cplx2 + 3 * real2) + 6 * nc + 3 * nc)
+    assert abs(b / 1e6 - 859.2) < 0.1
+    r = bench.roofline_of("cfg3_demag", w, prec, 2.19 * 10, 10)
+    assert r["bound"] == "hbm" and abs(r["algorithmic_bytes_per_launch"] / 1e6 - 1081.5) < 0.5 and 0.3 < r["frac"] < 0.6
+
+
 def test_reference_arm_prints_one_contract_line():
     """bench.py --impl reference: the oracle on the host cores, one JSON line with the base contract's keys."""
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "cfg2",
