@@ -138,8 +138,29 @@ __global__ void k_sweep_cond(const RepPtrs* reps, int R, unsigned int* live, uns
     cudaGraphSetConditional((cudaGraphConditionalHandle)handle, any);
 }
 
-__device__ void begin_body(Ctrl* c, Ctrl* c0, unsigned long long handle) {
+// (One block of kBeginThreads threads.  The control block is fetched with one batch of independent loads into shared
+// memory, worked on there, and written to both instances with one batch of stores: three L2 round trips instead of one
+// per dependent field - this kernel heads every run, so its latency is all of a one-step run's overhead.)
+constexpr int kBeginThreads = 128;
+constexpr int kBeginWords = (kCtrlWords + kBeginThreads - 1) / kBeginThreads;
+
+__device__ void begin_body(Ctrl* gc, Ctrl* c0, unsigned long long handle) {
+    __shared__ __align__(16) unsigned long long sw[kCtrlWords];
     const int tid = threadIdx.x;
+    const unsigned long long* const src = reinterpret_cast<const unsigned long long*>(gc);
+    unsigned long long v[kBeginWords];
+#pragma unroll
+    for (int k = 0; k < kBeginWords; ++k) {
+        const int i = tid + k * kBeginThreads;
+        v[k] = i < kCtrlWords ? __ldcg(src + i) : 0ull;
+    }
+#pragma unroll
+    for (int k = 0; k < kBeginWords; ++k) {
+        const int i = tid + k * kBeginThreads;
+        if (i < kCtrlWords) sw[i] = v[k];
+    }
+    __syncthreads();
+    Ctrl* const c = reinterpret_cast<Ctrl*>(sw);
     if (tid == 0) {
         c->done = (!(c->t < c->t_end) || c->status != 0) ? 1 : 0;
         c->arrive = 0u;
@@ -156,11 +177,15 @@ __device__ void begin_body(Ctrl* c, Ctrl* c0, unsigned long long handle) {
         }
     }
     if (tid == 0 && handle != 0ull) cudaGraphSetConditional((cudaGraphConditionalHandle)handle, c->done ? 0u : 1u);
-    // the step-boundary copy the TMA stage-2 kernel starts from (cavmag_types.cuh)
     __syncthreads();
-    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(c);
-    unsigned long long* dst = reinterpret_cast<unsigned long long*>(c0);
-    for (int i = tid; i < kCtrlWords; i += blockDim.x) dst[i] = src[i];
+    // the canonical instance, and the step-boundary copy the TMA stage-2 kernel starts from (cavmag_types.cuh)
+    unsigned long long* const d1 = reinterpret_cast<unsigned long long*>(gc);
+    unsigned long long* const d0 = reinterpret_cast<unsigned long long*>(c0);
+#pragma unroll
+    for (int k = 0; k < kBeginWords; ++k) {
+        const int i = tid + k * kBeginThreads;
+        if (i < kCtrlWords) { const unsigned long long x = sw[i]; d1[i] = x; d0[i] = x; }
+    }
 }
 
 template <typename T>
@@ -659,7 +684,7 @@ int build_graph_impl(cav_sim* s, int which, bool pdl, int unroll) {
     cudaGraphNode_t n_begin, n_k1, n_while;
     {
         void* params[] = {&ctrl, &ctrl0, &h64};
-        int rc = add_kernel(s, graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(64), params, 0);
+        int rc = add_kernel(s, graph, &n_begin, nullptr, (const void*)k_begin, dim3(1), dim3(kBeginThreads), params, 0);
         if (rc) return rc;
     }
     cudaGraphNode_t tail[4];
@@ -753,7 +778,7 @@ int run_stream_mode(cav_sim* s) {
     choose_grid(s);
     decide_path(s);
     StageArgs A = make_args(s, 0ull);
-    k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
+    k_begin<<<1, kBeginThreads, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
     CK(cudaGetLastError());
     int rc = launch_stage(s, 1, A, s->stream);
     if (rc) return rc;
@@ -1260,7 +1285,7 @@ static int ensure_k1(cav_sim* s) {
         if (s->padded && !s->use_tma) return CAV_E_UNSUPPORTED;
         StageArgs A = make_args(s, 0ull);
         s->h_fresh = false;
-        k_begin<<<1, 64, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
+        k_begin<<<1, kBeginThreads, 0, s->stream>>>(s->d_ctrl, s->d_ctrl0, 0ull);
         CK(cudaGetLastError());
         s->host_launches++;
         rc = launch_stage(s, 1, A, s->stream);
@@ -1492,7 +1517,7 @@ int sweep_build_graph(cav_sweep* w, int which, int unroll) {
     cudaGraphNode_t prev, node;
     {
         void* params[] = {(void*)&reps};
-        int rc = add_kernel(s, graph, &prev, nullptr, (const void*)k_sweep_begin, dim3(R), dim3(64), params, 0);
+        int rc = add_kernel(s, graph, &prev, nullptr, (const void*)k_sweep_begin, dim3(R), dim3(kBeginThreads), params, 0);
         if (rc) return rc;
     }
     std::vector<StageArgs> A1(R);
