@@ -132,10 +132,14 @@ __global__ void k_begin(Ctrl* c, Ctrl* c0, unsigned long long handle) { begin_bo
 __global__ void k_sweep_setrun(const RepPtrs* reps, double t_end, double tol, double fixed_dt, double dt_init, long long max_steps);
 __global__ void k_sweep_begin(const RepPtrs* reps) { begin_body(reps[blockIdx.x].ctrl, reps[blockIdx.x].ctrl0, 0ull); }
 __global__ void k_sweep_cond(const RepPtrs* reps, int R, unsigned int* live, unsigned long long handle) {
-    unsigned int any = 0u;
-    for (int r = 0; r < R; ++r) any |= reps[r].ctrl->done ? 0u : 1u;
-    *live = 0u;
-    cudaGraphSetConditional((cudaGraphConditionalHandle)handle, any);
+    // one thread per simulation (strided): the two dependent loads per member run side by side, not one after the other
+    unsigned int mine = 0u;
+    for (int r = threadIdx.x; r < R; r += blockDim.x) mine |= reps[r].ctrl->done ? 0u : 1u;
+    const int any = __syncthreads_or((int)mine);
+    if (threadIdx.x == 0) {
+        *live = 0u;
+        cudaGraphSetConditional((cudaGraphConditionalHandle)handle, any ? 1u : 0u);
+    }
 }
 
 // (One block of kBeginThreads threads.  The control block is fetched with one batch of independent loads into shared
@@ -1533,7 +1537,7 @@ int sweep_build_graph(cav_sweep* w, int which, int unroll) {
     {
         int Rv = R;
         void* params[] = {(void*)&reps, &Rv, &live, &h64};
-        int rc = add_kernel(s, graph, &node, &prev, (const void*)k_sweep_cond, dim3(1), dim3(1), params, 0);
+        int rc = add_kernel(s, graph, &node, &prev, (const void*)k_sweep_cond, dim3(1), dim3(128), params, 0);
         if (rc) return rc;
         prev = node;
     }
