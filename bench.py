@@ -1,6 +1,8 @@
 """bench.py — throughput of the fused LLG + cavity-mode RK45 step (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg5|cfg4|cfg4_f64|cfg2|cfg1|cfg1_sweep|cfg2_sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg5|cfg4|cfg4_f64|cfg2|cfg2_f64|cfg1|cfg1_sweep|
+                     cfg2_sweep|cfg2_sweep_joint|cfg2_sweep_joint_f64|cfg3_nx250|cfg3_demag]
+    python bench.py --workload <wl> --full-run    # the config exactly as BASELINE.json states it: time to solution
     python bench.py --impl reference ...          # the fp64 CPU oracle on the host cores
 
 A "step" is one Dormand-Prince RK45 step of the whole coupled system: six fused stage kernels
@@ -18,6 +20,11 @@ with cav_set_stream), barrier + synchronize on both sides, max over ranks.  The 
 ONE cav_run_steps call = one CUDA-graph launch whose WHILE node loops on the device.
 N > 1: independent replicas (different seeds) per GPU, no data-path collective ("replicas only",
 DESIGN.md) -> weak scaling.
+
+`e2e`: the same metric through the C ABI with HOST buffers - every step of every simulation uploads m and a from
+pinned host memory, takes one step and downloads m and a - with E2E_STREAMS independent simulations in flight (one host
+thread and one stream each, so the copies of one overlap the step and the opposite-direction copies of the others);
+`e2e.single_stream` is one such chain alone.
 """
 from __future__ import annotations
 
