@@ -671,7 +671,7 @@ def run_batch(args):
             "roofline": {"bound": "alu", "achieved": flops, "peak": peak, "unit": "TFLOP/s", "frac": flops / peak,
                          "traffic": None, "kernel": "cavmag::k_batch",
                          "note": "fp64 vector peak derived from unit counts; the kernel is barrier/latency-bound "
-                                 "(14 block barriers per step on a 512-thread block)"},
+                                 "(15 block barriers per step on a 512-thread block)"},
             "single_simulation_cell_stage_per_s": single,
             "speedup_vs_one_simulation_at_a_time": value / single}
     print(json.dumps(line), flush=True)

@@ -239,7 +239,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) fld[(size_t)(q * 3 + c) * nc + cell] = ms[q][c];
         }
-        __syncthreads();                                             // [A] c_n of this stage (and, !COOP, the stage state) published
+        // COOP: [A] publishes c_n of this stage before the mode loop.  One block per simulation: c_n was published by the
+        // previous evaluation's [B] (stages 1-2: written since by the step's first stage state - one more barrier), and [A]
+        // sits behind the mode loop, where it also publishes the block's partial sums: the mode thread's fp64 chain then
+        // runs beside the other warps' stencil instead of after it.
+        if constexpr (COOP || s <= 2) __syncthreads();
         T mcx, mcy, mcz;
         if constexpr (NSUB == 1) { mcx = ms[0][0]; mcy = ms[0][1]; mcz = ms[0][2]; }
         else { mcx = (T)0.5 * (ms[0][0] + ms[1][0]); mcy = (T)0.5 * (ms[0][1] + ms[1][1]); mcz = (T)0.5 * (ms[0][2] + ms[1][2]); }
@@ -273,45 +277,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
                 if (lane == 0) sh.part[warp][2 * N + i] = v;
             }
         }
-        if constexpr (COOP) {
-            __syncthreads();
-            if (tid < 2 * N + nsum_extra) {                          // fixed-order block sum -> this block's slot
-                double v = 0.0;
-                for (int w = 0; w < nwarp; ++w) v += sh.part[w][tid];
-                A.cpart[ev & 1][(size_t)tid * A.nblk + blockIdx.x] = v;
-            }
-            grid_barrier();                                          // stage state, partials and c_n of all blocks published
-        }
-        auto rd = [&](const T* f, int i) -> T {
-            if constexpr (COOP) return __ldcg(f + i);                // written by other SMs: read at L2
-            else return f[i];
-        };
-#pragma unroll
-        for (int q = 0; q < NSUB; ++q) {
-            T lap[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const T* f = fld + (size_t)(q * 3 + c) * nc;
-                const T m0 = ms[q][c];
-                T l = (rd(f, ixm) - m0) * wxm;
-                l += (rd(f, ixp) - m0) * wxp;
-                l += (rd(f, iym) - m0) * wym;
-                l += (rd(f, iyp) - m0) * wyp;
-                l += (rd(f, izm) - m0) * wzm;
-                l += (rd(f, izp) - m0) * wzp;
-                lap[c] = l;
-            }
-            const T mx = ms[q][0], my = ms[q][1], mz = ms[q][2];
-            T Bx, By, Bz;
-            material_field(mx, my, mz, lap[0], lap[1], lap[2], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
-            Bx += brf;
-            if (polar) { By += brfy; Bz += brfz; }
-            if constexpr (NSUB == 2) { Bx -= BE * ms[1 - q][0]; By -= BE * ms[1 - q][1]; Bz -= BE * ms[1 - q][2]; }
-            llg_slope(mx, my, mz, Bx, By, Bz, alpha, llg, k[q][0], k[q][1], k[q][2]);
-        }
-        if constexpr (COOP)                                          // fixed-order sum over the blocks' slots (every block: same bits)
-            reduce_block_partials(A.cpart[ev & 1], A.nblk, 2 * N + nsum_extra, A.nblk, warp, nwarp, lane, sh.red2);
-        __syncthreads();                                             // [B] partial sums published, stage-state buffer free again
+        // thread n: S_n, the mode slope ka_s and the amplitudes / RF weights of the next stage state; a second warp: <m_s>
+        auto mode_block = [&]() {
         if (tid < N) {
             const int n = tid;
             double sx = 0.0, sy = 0.0;
@@ -360,6 +327,51 @@ __global__ void __launch_bounds__(MAXT, MINB) k_batch(const BatchArgs A) {
             }
             sh.red[i] = v * A.inv_nc;
         }
+        };
+        if constexpr (!COOP) {
+            __syncthreads();                                         // [A] stage state and partial sums of the block published
+            mode_block();
+        }
+        if constexpr (COOP) {
+            __syncthreads();
+            if (tid < 2 * N + nsum_extra) {                          // fixed-order block sum -> this block's slot
+                double v = 0.0;
+                for (int w = 0; w < nwarp; ++w) v += sh.part[w][tid];
+                A.cpart[ev & 1][(size_t)tid * A.nblk + blockIdx.x] = v;
+            }
+            grid_barrier();                                          // stage state, partials and c_n of all blocks published
+        }
+        auto rd = [&](const T* f, int i) -> T {
+            if constexpr (COOP) return __ldcg(f + i);                // written by other SMs: read at L2
+            else return f[i];
+        };
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q) {
+            T lap[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const T* f = fld + (size_t)(q * 3 + c) * nc;
+                const T m0 = ms[q][c];
+                T l = (rd(f, ixm) - m0) * wxm;
+                l += (rd(f, ixp) - m0) * wxp;
+                l += (rd(f, iym) - m0) * wym;
+                l += (rd(f, iyp) - m0) * wyp;
+                l += (rd(f, izm) - m0) * wzm;
+                l += (rd(f, izp) - m0) * wzp;
+                lap[c] = l;
+            }
+            const T mx = ms[q][0], my = ms[q][1], mz = ms[q][2];
+            T Bx, By, Bz;
+            material_field(mx, my, mz, lap[0], lap[1], lap[2], B0x, B0y, B0z, anp, axx, axy, axz, Bx, By, Bz);
+            Bx += brf;
+            if (polar) { By += brfy; Bz += brfz; }
+            if constexpr (NSUB == 2) { Bx -= BE * ms[1 - q][0]; By -= BE * ms[1 - q][1]; Bz -= BE * ms[1 - q][2]; }
+            llg_slope(mx, my, mz, Bx, By, Bz, alpha, llg, k[q][0], k[q][1], k[q][2]);
+        }
+        if constexpr (COOP)                                          // fixed-order sum over the blocks' slots (every block: same bits)
+            reduce_block_partials(A.cpart[ev & 1], A.nblk, 2 * N + nsum_extra, A.nblk, warp, nwarp, lane, sh.red2);
+        __syncthreads();                                             // [B] stage-state buffer free again; COOP: partial sums published; else: c_n, a_s of the next stage published
+        if constexpr (COOP) mode_block();
         if (tid == 0) sh.rhs_evals++;
         ++ev;
     };
