@@ -1,6 +1,6 @@
 // Dipolar field by FFT convolution (see demag.cuh).
 //
-// Layout of one evaluation (nz <= 64 and ny <= 512, the usual case: films and slabs):
+// Layout of one evaluation (nz <= 64 and ny <= 512 - 256 in fp64 -, the usual case: films and slabs):
 //   gather   stage state, summed over the sublattices -> [3][nz][ny][Px] real, zero-padded in x only
 //   cuFFT    batched 1-D R2C along x over the 3 nz ny occupied rows: rows and planes that would only hold zeros are
 //            never stored or transformed
@@ -11,7 +11,7 @@
 //            The tensor's transform is real and even/odd in every index: one octant of it is stored, as reals.
 //   k_demag_ycol    inverse along y, keep the ny rows
 //   cuFFT    batched 1-D C2R along x, then the scatter of the first nx cells of a row into the dense field.
-// Fallbacks: 2-D cuFFT over all Py rows (ny > 512 or nx = 1), padded 3-D cuFFT with a separate product kernel (nz > 64,
+// Fallbacks: 2-D cuFFT over all Py rows (ny beyond that, or nx = 1), padded 3-D cuFFT with a separate product kernel (nz > 64,
 // where the columns of a block do not fit shared memory).  cuFFT does the x transforms (a library primitive); the tensor,
 // the gather, the y and z transforms, the product and the scatter are kernels of this file.
 #include <cmath>
@@ -406,7 +406,7 @@ k_demag_ycol(const C* __restrict__ in, C* __restrict__ out, int n_valid, int NXH
     if constexpr (NP > 3) pass(integral_constant<int, 3>{});
 }
 
-constexpr int kYColMaxQ = 10;        // Py <= 1024: [Py][16] complex columns fit the shared memory of a block in both precisions
+constexpr int kYColMaxQ = 10;        // fp32: Py <= 1024 ([Py][16] complex columns = 128 KB of shared memory); fp64: Py <= 512
 
 template <typename T, typename C, bool INV>
 const void* ycol_fn(int q) {
@@ -561,7 +561,7 @@ int demag_create(DemagPlan** out, int nx, int ny, int nz, double dx, double dy, 
     if (p->zfused && nx > 1) {           // y by k_demag_ycol: Py a power of two >= 2 ny - 1
         int Py2 = 1, qy = 0;
         while (Py2 < 2 * ny - 1) { Py2 *= 2; qy++; }
-        if (qy <= kYColMaxQ) { p->yfused = true; p->Py = Py2; p->qy = qy; }
+        if (qy <= (f32 ? kYColMaxQ : kYColMaxQ - 1)) { p->yfused = true; p->Py = Py2; p->qy = qy; }
     }
     p->zplanes = p->zfused ? nz : p->Pz;
     p->prows = p->yfused ? ny : p->Py;

@@ -322,6 +322,8 @@ def test_spectrum_shows_both_polariton_branches(api):
     ((20, 33, 2), 1, 1, 0.1e-12),      # ny = 33: Py = 128 (next power of two above 2 ny - 1 = 65), an odd number of levels
     ((600, 2, 1), 0, 1, 0.1e-12),      # nx > 512: the x transforms stay with cuFFT (1-D over the occupied rows), y by the column kernel
     ((7, 3, 2), 1, 2, 0.02e-12),       # odd ny: the last row pair of a plane has one row; two sublattices
+    ((2, 130, 1), 0, 1, 0.1e-12),      # Py = 512: the three radix-8 passes of the y kernel that CFG3 runs
+    ((2, 260, 2), 0, 1, 0.1e-12),      # Py = 1024: the largest y transform of the column kernel (3 3 2 2)
 ])
 def test_demag_matches_the_direct_sum(api, prec, shape, N, n_sub, dt):
     """The FFT convolution against the oracle's direct O(N^2) sum with the Newell tensor: right-hand side cell by cell,
