@@ -17,7 +17,7 @@ def _free(torch):
 
 
 def _cycle(api, torch, k):
-    w = small_problem(128, 24, 20, 2, 1)                       # TMA path (480 plane-tiles)
+    w = small_problem(128, 32, 24, 2, 1)                       # TMA path (98 304 cells)
     st = torch.cuda.Stream()
     with api.Sim(w, precision="f32", stream=st.cuda_stream) as sim:
         api.cav_set_trace(sim.h, 1e-12, 64)
@@ -61,3 +61,57 @@ def test_handles_give_their_device_memory_back(api):
     free1 = _free(torch)
     # the driver hands memory out in 2 MiB granules and keeps a few cached: a leak of one handle per cycle would be >= 100 MB here
     assert free0 - free1 < 16 * 2 ** 20, (free0, free1)
+
+
+def test_setters_in_any_order_leave_a_consistent_handle(api):
+    """Settings that replace device tables or switch kernel families, applied between runs in orders a user might try: every
+    run afterwards matches a fresh handle configured directly (bitwise: same kernels, same inputs)."""
+    from test_gpu_parity import oracle_of
+    w = small_problem(128, 32, 24, 2, 1)                        # 98 304 cells: beyond the cooperative kernel, TMA path
+    p = [[0.0, 1.0, 0.0], [0.6, 0.0, 0.8]]
+
+    def final(configure, steps=6):
+        with api.Sim(w, precision="f64") as sim:
+            configure(sim)
+            api.cav_set_m(sim.h, np.ascontiguousarray(w.m0))
+            api.cav_set_a(sim.h, w.a0)
+            api.cav_set_time(sim.h, 0.0)
+            api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=steps)
+            return sim.get_m(), sim.get_a(), api.cav_get_kernel_path(sim.h)
+
+    def modes(sim):
+        api.cav_set_modes(sim.h, np.ascontiguousarray(w.u), w.omega, w.kappa, w.g, w.Gamma, w.Phi)
+
+    # polarisation: direct / after a detour through the dipolar field, a spectrum, a run and a new mode set
+    m0, a0, path0 = final(lambda s: api.cav_set_polarisation(s.h, p))
+
+    def detour(sim):
+        api.cav_set_demag(sim.h, 1)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=2)
+        api.cav_set_demag(sim.h, 0)
+        api.cav_set_trace(sim.h, 0.1e-12, 8)
+        api.cav_set_spectrum(sim.h, 9, 5e10, 7e10)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=2)
+        modes(sim)                                    # drops polarisation, spectrum, drive
+        api.cav_set_spectrum(sim.h, 0)
+        api.cav_set_trace(sim.h, 0.0, 0)
+        api.cav_set_polarisation(sim.h, p)
+    m1, a1, path1 = final(detour)
+    assert path0 == path1 == api.CAV_PATH_TMA
+    assert np.array_equal(m0, m1) and np.array_equal(a0, a1)
+    ref = oracle_of(w, pol=p).run(w.m0, w.a0, fixed_dt=0.05e-12, max_steps=6)
+    assert np.abs(m0 - ref.m).max() <= 1e-10 and np.abs(a0 - ref.a).max() <= 1e-10 * np.abs(ref.a).max()
+
+    # the dipolar field: direct / after polarisation was set and taken back, on a forced generic path and back to auto
+    md, ad, pathd = final(lambda s: api.cav_set_demag(s.h, 1), steps=3)
+
+    def detour2(sim):
+        api.cav_set_polarisation(sim.h, p)
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=0.05e-12, max_steps=2)
+        api.cav_set_polarisation(sim.h, None)
+        api.cav_set_kernel_path(sim.h, api.CAV_PATH_GENERIC)
+        api.cav_set_kernel_path(sim.h, api.CAV_PATH_AUTO)
+        api.cav_set_demag(sim.h, 1)
+    me, ae, pathe = final(detour2, steps=3)
+    assert pathd == pathe == api.CAV_PATH_GENERIC
+    assert np.array_equal(md, me) and np.array_equal(ad, ae)
