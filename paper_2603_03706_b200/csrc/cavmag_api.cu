@@ -351,7 +351,7 @@ int plan_tma(cav_sim* s) {
         const bool has_a = t.aux_slot_bytes > 0, has_u = t.u_slot_bytes > 0;
         double best = -1e9;
         int bDa = 0, bDu = 0, bDm = 0;
-        for (int Da = has_a ? 2 : 0; Da <= (has_a ? 4 : 0); ++Da)
+        for (int Da = has_a ? 1 : 0; Da <= (has_a ? 4 : 0); ++Da)       // (one aux slot - no look-ahead - only where two do not fit)
             for (int Du = has_u ? 2 : 0; Du <= (has_u ? kTmaMaxDepth : 0); ++Du)
                 for (int Dm = 4; Dm <= 8; ++Dm) {
                     const size_t bytes = (size_t)Da * t.aux_slot_bytes + (size_t)Du * t.u_slot_bytes + (size_t)Dm * t.ms_slot_bytes + 128;

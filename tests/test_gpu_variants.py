@@ -48,6 +48,7 @@ def _axes(N, seed=3):
     ((64, 12, 6), 2, 2, 0.02e-12, "tma"),          # antiferromagnet, two modes
     ((132, 9, 11), 8, 1, 0.1e-12, "tma"),          # eight modes, three x tiles
     ((4, 2, 40), 2, 1, 0.1e-12, "tma"),            # one tile, long z march
+    ((68, 17, 6), 8, 2, 0.02e-12, "tma"),          # antiferromagnet with eight modes: one aux slot in stage 6
 ])
 @pytest.mark.parametrize("with_quad", [False, True])
 def test_polarisation_fixed_steps(api, prec, shape, N, n_sub, dt, path, with_quad):
