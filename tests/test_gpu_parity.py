@@ -799,3 +799,23 @@ def test_tma_multi_plane_runs(api, prec, n_sub, N, serpentine):
         api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=6)
         m, a = sim.get_m(), sim.get_a()
     assert_parity(m, a, ref, prec)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n_sub,N", [(1, 0), (1, 3), (1, 9), (1, 32), (2, 0), (2, 2), (2, 3), (2, 8), (2, 9), (2, 32)])
+def test_every_mode_bucket_and_sublattice_count_runs_on_the_tma_kernels(api, prec, n_sub, N):
+    """A grid with enough plane-tiles takes the TMA kernels under CAV_PATH_AUTO for every mode bucket (0, 1, 2, 8, 32) and one or
+    two sublattices - also where the planner has to give a ring its minimum depth (two sublattices with more than two
+    modes) - and matches the oracle there."""
+    w = small_problem(64, 32, 80, N, n_sub)
+    dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=12)
+    with api.Sim(w, precision=prec) as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=12)
+        m, a = sim.get_m(), sim.get_a()
+    assert_parity(m, a, ref, prec)
