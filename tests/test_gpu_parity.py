@@ -746,7 +746,7 @@ def test_nonreciprocal_rabi_period_geometric_mean(api):
 # large grids whose rows are not a multiple of 16 bytes: padded rows inside the library, TMA path (no generic-kernel cliff)
 # ----------------------------------------------------------------------------------------
 @pytest.mark.parametrize("prec,nx", [("f32", 250), ("f32", 251), ("f64", 251), ("f32", 61)])
-@pytest.mark.parametrize("n_sub,N", [(1, 3), (2, 1)])
+@pytest.mark.parametrize("n_sub,N", [(1, 3), (2, 1), (2, 4)])
 def test_unaligned_rows_run_on_the_tma_path(api, prec, nx, n_sub, N):
     """nx * sizeof(T) % 16 != 0 on a grid beyond the cooperative kernel's range: the library pads the rows of its own
     buffers (the ABI arrays stay dense) and runs the TMA kernels.  Odd nx ends a row in the middle of a lane's pair of
