@@ -819,3 +819,27 @@ def test_every_mode_bucket_and_sublattice_count_runs_on_the_tma_kernels(api, pre
         api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=12)
         m, a = sim.get_m(), sim.get_a()
     assert_parity(m, a, ref, prec)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("shape,n_sub,N", [
+    ((512, 256, 1), 1, 2),      # a film: one plane, both z neighbours outside the grid
+    ((512, 256, 1), 2, 1),      # the same with two sublattices
+    ((256, 256, 2), 1, 3),      # two planes
+    ((64, 2048, 1), 1, 2),      # one tile column per row of tiles, 256 tile rows
+    ((8, 8, 2048), 1, 2),       # a needle along z: one tile, the longest z march
+    ((2048, 8, 8), 2, 2),       # a needle along x: 32 tile columns, two sublattices
+])
+def test_extreme_aspect_ratios_on_the_tma_path(api, prec, shape, n_sub, N):
+    w = small_problem(*shape, N, n_sub)
+    dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+    if prec == "f32":
+        w.m0 = w.m0.astype(np.float32).astype(np.float64)
+        w.m0 /= np.linalg.norm(w.m0, axis=1, keepdims=True)
+        w.u = w.u.astype(np.float32).astype(np.float64)
+    ref = oracle_of(w).run(w.m0, w.a0, fixed_dt=dt, max_steps=8)
+    with api.Sim(w, precision=prec) as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=8)
+        m, a = sim.get_m(), sim.get_a()
+    assert_parity(m, a, ref, prec)
