@@ -843,3 +843,18 @@ def test_extreme_aspect_ratios_on_the_tma_path(api, prec, shape, n_sub, N):
         api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=8)
         m, a = sim.get_m(), sim.get_a()
     assert_parity(m, a, ref, prec)
+
+
+def test_forced_rejections_with_two_sublattices_and_eight_modes(api):
+    """The TMA configuration with a single aux slot (two sublattices, eight modes: DESIGN.md 5.3) through accepted and
+    rejected steps: the step sequence of the oracle, state within 1e-10."""
+    w = small_problem(64, 32, 80, 8, 2)
+    ref = oracle_of(w).run(w.m0, w.a0, t_end=1.5e-12, tol=1e-9, dt_init=0.2e-12)
+    assert ref.rejected > 0
+    with api.Sim(w, precision="f64") as sim:
+        assert api.cav_get_kernel_path(sim.h) == api.CAV_PATH_TMA
+        api.cav_run(sim.h, 1.5e-12, tol=1e-9, dt_init=0.2e-12)
+        st = api.cav_get_stats(sim.h)
+        m, a = sim.get_m(), sim.get_a()
+    assert (st["accepted"], st["rejected"]) == (ref.accepted, ref.rejected)
+    assert_parity(m, a, ref, "f64")
