@@ -71,3 +71,37 @@ def test_dipolar_field_on_random_small_grids(api):
             assert err <= (5e-13 if prec == "f64" else 3e-5), (prec, nx, ny, nz, n_sub, N, err)
         done += 1
     assert done >= 45
+
+
+def test_small_grid_kernels_and_generic_kernels_agree_on_random_adaptive_runs(api):
+    """Grids in the range of the single-block and the cooperative kernel (CAV_PATH_AUTO) against the generic stage kernels:
+    short adaptive runs with a too large first step - in fp64 the same accepted / rejected counts and the same state."""
+    rng = np.random.default_rng(4242)
+    paths = set()
+    for _ in range(100):
+        prec = "f64" if rng.random() < 0.5 else "f32"
+        if rng.random() < 0.5:
+            nx, ny, nz = int(rng.integers(8, 70)), int(rng.integers(4, 40)), int(rng.integers(1, 30))
+        else:
+            nx, ny, nz = int(rng.integers(1, 17)), int(rng.integers(1, 9)), int(rng.integers(1, 9))
+        if nx * ny * nz > 75000:
+            continue
+        n_sub = int(rng.integers(1, 3))
+        N = int(rng.choice([0, 1, 2, 3, 8, 32]))
+        w = small_problem(nx, ny, nz, N, n_sub, seed=int(rng.integers(1, 1000)))
+        dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+        out = {}
+        for name, path in (("auto", None), ("generic", api.CAV_PATH_GENERIC)):
+            with api.Sim(w, precision=prec, path=path) as sim:
+                api.cav_run(sim.h, 8 * dt, tol=1e-7 if prec == "f64" else 1e-5, dt_init=3 * dt)
+                out[name] = (sim.get_m().astype(np.float64), sim.get_a(), api.cav_get_stats(sim.h))
+                if name == "auto":
+                    paths.add(api.cav_get_kernel_path(sim.h))
+        dm = np.abs(out["auto"][0] - out["generic"][0]).max()
+        assert dm <= (1e-11 if prec == "f64" else 5e-6), (prec, nx, ny, nz, n_sub, N, dm)
+        if prec == "f64":
+            sa, sg = out["auto"][2], out["generic"][2]
+            assert (sa["accepted"], sa["rejected"]) == (sg["accepted"], sg["rejected"]), (nx, ny, nz, n_sub, N)
+            if N:
+                assert np.abs(out["auto"][1] - out["generic"][1]).max() <= 1e-11 * max(np.abs(out["generic"][1]).max(), 1e-3)
+    assert {api.CAV_PATH_BLOCK, api.CAV_PATH_COOP} <= paths
