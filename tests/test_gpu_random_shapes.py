@@ -105,3 +105,52 @@ def test_small_grid_kernels_and_generic_kernels_agree_on_random_adaptive_runs(ap
             if N:
                 assert np.abs(out["auto"][1] - out["generic"][1]).max() <= 1e-11 * max(np.abs(out["generic"][1]).max(), 1e-3)
     assert {api.CAV_PATH_BLOCK, api.CAV_PATH_COOP} <= paths
+
+
+def test_joint_sweeps_of_random_shapes_equal_solo_runs(api):
+    """Random member counts, shapes, mode counts, sublattices and precisions: members of a joint sweep (adaptive, first step
+    too large) take the step sequence of the same simulation run alone on the TMA kernels and end in the same state."""
+    import torch
+    import cavmag_workloads as W
+    rng = np.random.default_rng(99)
+    st = torch.cuda.Stream()
+    done = 0
+    for _ in range(25):
+        prec = "f64" if rng.random() < 0.5 else "f32"
+        es = 8 if prec == "f64" else 4
+        n_sub = int(rng.integers(1, 3))
+        N = int(rng.choice([1, 2])) if n_sub == 2 else int(rng.choice([1, 2, 3, 8]))
+        nx = int(rng.integers(2, 12)) * 16 // es * (2 if es == 4 else 4) // 2
+        ny, nz = int(rng.integers(4, 40)), int(rng.integers(2, 16))
+        R = int(rng.integers(3, 40))
+        dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+        tol = 1e-7 if prec == "f64" else 1e-5
+        ws = []
+        for r in range(R):
+            w = small_problem(nx, ny, nz, N, n_sub, seed=7 + (r % 3))
+            w.B0 = (0.01, -0.02, W.b0_for_ghz(9.0 + 0.05 * r))
+            ws.append(w)
+        sims = [api.Sim(w, precision=prec, stream=st.cuda_stream) for w in ws]
+        sw = None
+        try:
+            try:
+                sw = api.cav_sweep_create(sims)
+            except api.CavError as e:                  # fewer plane-tiles in total than SMs
+                assert e.status == api.CAV_E_UNSUPPORTED
+                continue
+            api.cav_sweep_run(sw, 10 * dt, tol=tol, dt_init=3 * dt)
+            for r in sorted(set(int(x) for x in rng.integers(0, R, 2))):
+                with api.Sim(ws[r], precision=prec, path=api.CAV_PATH_TMA) as solo:
+                    api.cav_run(solo.h, 10 * dt, tol=tol, dt_init=3 * dt)
+                    ms, as_, ss = solo.get_m(), solo.get_a(), api.cav_get_stats(solo.h)
+                m, a, s1 = sims[r].get_m(), sims[r].get_a(), api.cav_get_stats(sims[r].h)
+                assert (s1["accepted"], s1["rejected"]) == (ss["accepted"], ss["rejected"]), (prec, nx, ny, nz, n_sub, N, R, r)
+                assert np.abs(m.astype(np.float64) - ms.astype(np.float64)).max() <= (1e-12 if prec == "f64" else 1e-6)
+                assert np.abs(a - as_).max() <= (1e-12 if prec == "f64" else 1e-6) * max(np.abs(as_).max(), 1e-3)
+            done += 1
+        finally:
+            if sw is not None:
+                api.cav_sweep_destroy(sw)
+            for s in sims:
+                s.close()
+    assert done >= 15
