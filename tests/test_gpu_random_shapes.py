@@ -154,3 +154,57 @@ def test_joint_sweeps_of_random_shapes_equal_solo_runs(api):
             for s in sims:
                 s.close()
     assert done >= 15
+
+
+def test_random_feature_combinations_agree_across_kernel_families(api):
+    """Drive, non-reciprocal coupling, per-mode polarisation, sum-u normalisation, renormalisation off, trace, Fourier sums,
+    fixed or adaptive stepping - switched on at random - on the TMA kernels, the generic kernels and whatever CAV_PATH_AUTO
+    picks (single-block / cooperative kernel here): the same state, trace, spectrum and step counts in fp64."""
+    rng = np.random.default_rng(2024)
+    two_pi = 2 * math.pi
+    families = set()
+    for _ in range(60):
+        n_sub = int(rng.integers(1, 3))
+        N = int(rng.choice([1, 2, 3, 8]))
+        nx = int(rng.integers(2, 10)) * 8
+        ny, nz = int(rng.integers(3, 30)), int(rng.integers(2, 24))
+        w = small_problem(nx, ny, nz, N, n_sub, seed=int(rng.integers(1, 1000)))
+        dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+        f = dict(drive=rng.random() < 0.5, back=rng.random() < 0.5, pol=rng.random() < 0.5, sumu=rng.random() < 0.3,
+                 norenorm=rng.random() < 0.3, spec=rng.random() < 0.5, adaptive=rng.random() < 0.5)
+        amp = (rng.normal(size=N) + 1j * rng.normal(size=N)) * 1e9
+        gb = two_pi * 1e6 * rng.uniform(5, 40, size=N)
+        p = rng.normal(size=(N, 3))
+        p /= np.linalg.norm(p, axis=1, keepdims=True)
+        if f["sumu"]:
+            w.u = w.u + 0.7                              # keeps sum u away from zero
+        out = {}
+        for name, path in (("tma", api.CAV_PATH_TMA), ("generic", api.CAV_PATH_GENERIC), ("auto", None)):
+            with api.Sim(w, precision="f64", path=path, renormalize=not f["norenorm"],
+                         overlap_norm=api.CAV_NORM_SUM_U if f["sumu"] else api.CAV_NORM_NCELLS) as sim:
+                if f["drive"]:
+                    api.cav_set_drive(sim.h, amp, 2 * dt, 3 * dt, two_pi * 10e9)
+                if f["back"]:
+                    api.cav_set_backaction(sim.h, gb)
+                if f["pol"]:
+                    api.cav_set_polarisation(sim.h, p)
+                api.cav_set_trace(sim.h, 2 * dt, 4)
+                if f["spec"]:
+                    api.cav_set_spectrum(sim.h, 5, two_pi * 9e9, two_pi * 11e9)
+                if f["adaptive"]:
+                    api.cav_run(sim.h, 8 * dt, tol=1e-8, dt_init=3 * dt)
+                else:
+                    api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=8)
+                X = api.cav_get_spectrum(sim.h, 5, N)[0] if f["spec"] else np.zeros(1)
+                out[name] = (sim.get_m(), sim.get_a(), api.cav_get_trace(sim.h), X, api.cav_get_stats(sim.h))
+                families.add(api.cav_get_kernel_path(sim.h))
+        ref = out["generic"]
+        for name in ("tma", "auto"):
+            o = out[name]
+            what = (name, nx, ny, nz, n_sub, N, f)
+            assert np.abs(o[0] - ref[0]).max() <= 1e-11, what
+            assert np.abs(o[1] - ref[1]).max() <= 1e-11 * max(np.abs(ref[1]).max(), 1e-6), what
+            assert o[2].shape == ref[2].shape and np.abs(o[2] - ref[2]).max() <= 1e-10 * max(np.abs(ref[2]).max(), 1e-6), what
+            assert np.abs(o[3] - ref[3]).max() <= 1e-10 * max(np.abs(ref[3]).max(), 1e-6), what
+            assert (o[4]["accepted"], o[4]["rejected"]) == (ref[4]["accepted"], ref[4]["rejected"]), what
+    assert {api.CAV_PATH_TMA, api.CAV_PATH_GENERIC, api.CAV_PATH_COOP} <= families
