@@ -208,3 +208,58 @@ def test_random_feature_combinations_agree_across_kernel_families(api):
             assert np.abs(o[3] - ref[3]).max() <= 1e-10 * max(np.abs(ref[3]).max(), 1e-6), what
             assert (o[4]["accepted"], o[4]["rejected"]) == (ref[4]["accepted"], ref[4]["rejected"]), what
     assert {api.CAV_PATH_TMA, api.CAV_PATH_GENERIC, api.CAV_PATH_COOP} <= families
+
+
+def test_random_batches_equal_generic_single_runs(api):
+    """cav_batch_run on random tiny grids (up to 1024 cells), replica counts, mode counts, sublattices, precisions, with a
+    drive and a polarisation switched on at random: a replica equals the same problem run alone on the generic kernels."""
+    import cavmag_workloads as W
+    rng = np.random.default_rng(31)
+    two_pi = 2 * math.pi
+    for _ in range(40):
+        prec = "f64" if rng.random() < 0.6 else "f32"
+        n_sub = int(rng.integers(1, 3))
+        N = int(rng.choice([0, 1, 2, 3, 8]))
+        while True:
+            nx, ny, nz = int(rng.integers(1, 17)), int(rng.integers(1, 12)), int(rng.integers(1, 12))
+            if nx * ny * nz <= 1024:
+                break
+        R = int(rng.integers(1, 12))
+        w = small_problem(nx, ny, nz, N, n_sub, seed=int(rng.integers(1, 1000)))
+        dt = 0.05e-12 if n_sub == 1 else 0.01e-12
+        B0 = np.array([[0.01 * r, -0.02, W.b0_for_ghz(9.0 + 0.3 * r)] for r in range(R)])
+        f = dict(drive=N > 0 and rng.random() < 0.4, pol=N > 0 and rng.random() < 0.4, adaptive=rng.random() < 0.6)
+        amp = (rng.normal(size=max(N, 1)) + 1j * rng.normal(size=max(N, 1)))[:N] * 1e9
+        p = rng.normal(size=(max(N, 1), 3))[:N]
+        if N:
+            p /= np.linalg.norm(p, axis=1, keepdims=True)
+        tol = 1e-8 if prec == "f64" else 1e-5
+        with api.Batch(w, R, precision=prec, B0=B0) as b:
+            if f["drive"]:
+                api.cav_batch_set_drive(b.h, amp, 2 * dt, 3 * dt, two_pi * 10e9)
+            if f["pol"]:
+                api.cav_batch_set_polarisation(b.h, p)
+            if f["adaptive"]:
+                b.run(8 * dt, tol=tol, dt_init=3 * dt)
+            else:
+                b.run(math.inf, fixed_dt=dt, max_steps=8)
+            mb, ab, sb = b.get_m(), b.get_a(), b.stats()
+        for r in sorted(set(int(x) for x in rng.integers(0, R, 2))):
+            w2 = copy.deepcopy(w)
+            w2.B0 = tuple(B0[r])
+            with api.Sim(w2, precision=prec, path=api.CAV_PATH_GENERIC) as sim:
+                if f["drive"]:
+                    api.cav_set_drive(sim.h, amp, 2 * dt, 3 * dt, two_pi * 10e9)
+                if f["pol"]:
+                    api.cav_set_polarisation(sim.h, p)
+                if f["adaptive"]:
+                    api.cav_run(sim.h, 8 * dt, tol=tol, dt_init=3 * dt)
+                else:
+                    api.cav_run_steps(sim.h, math.inf, fixed_dt=dt, max_steps=8)
+                ms, as_, ss = sim.get_m(), sim.get_a(), api.cav_get_stats(sim.h)
+            what = (prec, nx, ny, nz, n_sub, N, R, r, f)
+            assert np.abs(mb[r].astype(np.float64) - ms.astype(np.float64)).max() <= (1e-11 if prec == "f64" else 5e-6), what
+            if prec == "f64":
+                assert (sb[r]["accepted"], sb[r]["rejected"]) == (ss["accepted"], ss["rejected"]), what
+                if N:
+                    assert np.abs(ab[r] - as_).max() <= 1e-11 * max(np.abs(as_).max(), 1e-6), what
